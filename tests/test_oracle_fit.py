@@ -1,0 +1,283 @@
+"""Pins of the oracle's adaptive vertex fit (O7) and cleanup (O8).  PAPER.md L167-247."""
+import numpy as np
+from scipy.optimize import minimize
+
+from synth import events
+
+K = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
+
+
+def _tracks(rng, n, P, sig=(0.01, 0.1), zstate=None, noise=True, slope=0.25):
+    tx = np.clip(rng.normal(0, slope, n), -0.4, 0.4); ty = np.clip(rng.normal(0, slope, n), -0.4, 0.4)
+    s = rng.uniform(*sig, n)
+    z = np.full(n, P[2]) if zstate is None else zstate
+    x = P[0] + (z - P[2]) * tx + (s * rng.normal(0, 1, n) if noise else 0)
+    y = P[1] + (z - P[2]) * ty + (s * rng.normal(0, 1, n) if noise else 0)
+    t = dict(x=x, y=y, z=z, tx=tx, ty=ty, var_x=s ** 2, var_y=s ** 2, var_tx=np.full(n, 1e-6), var_ty=np.full(n, 1e-6))
+    return {k: np.asarray(v, np.float32) for k, v in t.items()}
+
+
+def _wls(t, idx, zseed):
+    """Analytic weighted least squares alpha* = (sum H^T W H)^-1 sum H^T W m, via numpy lstsq on the
+    whitened stacked system (an independent route: no normal equations)."""
+    a = {k: t[k][idx].astype(np.float64) for k in K}
+    dz = zseed - a["z"]
+    sx = np.sqrt(a["var_x"] + dz ** 2 * a["var_tx"]); sy = np.sqrt(a["var_y"] + dz ** 2 * a["var_ty"])
+    n = len(idx)
+    # x_i - z_i tx_i = X - Z tx_i   ->  rows [1, 0, -tx] / sx ; same for y
+    A = np.zeros((2 * n, 3)); b = np.zeros(2 * n)
+    A[:n, 0] = 1 / sx; A[:n, 2] = -a["tx"] / sx; b[:n] = (a["x"] - a["z"] * a["tx"]) / sx
+    A[n:, 1] = 1 / sy; A[n:, 2] = -a["ty"] / sy; b[n:] = (a["y"] - a["z"] * a["ty"]) / sy
+    sol, *_ = np.linalg.lstsq(A, b, rcond=None)
+    cov = np.linalg.inv(A.T @ A)
+    return sol, cov
+
+
+def test_unit_weight_fit_is_the_analytic_weighted_mean(oracle):
+    """'If not for the presence of the weights w_i, the solution would be exact' (L223): with
+    chi2_max = inf one Newton step lands on the analytic WLS point and the second step is zero."""
+    rng = np.random.default_rng(11)
+    p = oracle.default_params(chi2_max=np.inf)
+    for _ in range(20):
+        P = (rng.normal(0, 0.04), rng.normal(0, 0.04), rng.normal(0, 45))
+        n = int(rng.integers(3, 60))
+        t = _tracks(rng, n, P, zstate=P[2] + rng.uniform(-20, 20, n))
+        idx = np.arange(n)
+        seed = (0.0, 0.0, P[2] + rng.uniform(-0.5, 0.5))
+        r = oracle.fit(t, idx, seed, p)
+        sol, cov = _wls(t, idx, seed[2])
+        assert r["rc"] == 0 and r["niter"] == 2
+        assert np.allclose(r["trace"][0, :3], sol, atol=1e-9)
+        assert abs(r["trace"][1, 10]) < 1e-9 and abs(r["trace"][1, 9]) < 1e-12    # dz, dchi2 of step 2
+        assert np.allclose(r["pos"], sol, atol=1e-9)
+        C = r["cov"]
+        Cm = np.array([[C[0], C[1], C[2]], [C[1], C[3], C[4]], [C[2], C[4], C[5]]])
+        assert np.allclose(Cm, cov, rtol=1e-8, atol=1e-14)                           # Eq. 14
+        assert np.all(r["w"] == 1.0) and r["ntrk"] == n
+
+
+def test_noiseless_tracks_recover_the_point(oracle):
+    """Brute force on tiny events: noiseless tracks from one point recover that point."""
+    rng = np.random.default_rng(12)
+    p = oracle.default_params()
+    for n in (2, 3, 5, 40):
+        P = (0.02, -0.03, rng.normal(0, 45))
+        t = _tracks(rng, n, P, sig=(0.05, 0.1), zstate=P[2] + rng.uniform(-10, 10, n), noise=False)
+        # seed 0.03 mm off: residuals ~ 0.03 * slope stay well inside the Tukey cut-off
+        r = oracle.fit(t, np.arange(n), (0.0, 0.0, P[2] + 0.03), p)
+        assert r["rc"] == 0
+        assert np.allclose(r["pos"], P, atol=2e-5)       # fp32 inputs: |x| ~ 4, ulp ~ 5e-7
+        assert np.all(r["w"] > 0.999) and r["chi2"] < 1e-3
+
+
+def test_newton_step_vs_numerical_minimiser(oracle):
+    """Brute force: with the weights frozen at the values of the oracle's LAST iteration, a Nelder-Mead /
+    BFGS minimisation of chi2 = sum w_i chi2_i (Eq. 6-9) over (x, y, z) agrees with pos (Eq. 13)."""
+    rng = np.random.default_rng(13)
+    p = oracle.default_params(conv_dchi2=1e-12, conv_dz=1e-9, max_iter=16)
+    for _ in range(10):
+        P = (rng.normal(0, 0.04), rng.normal(0, 0.04), rng.normal(0, 45))
+        n = int(rng.integers(8, 40))
+        t = _tracks(rng, n, P)
+        # contaminate with outliers so that the Tukey weights matter
+        t["x"][:2] += np.float32(0.4)
+        seed = (0.0, 0.0, P[2] + 0.2)
+        r = oracle.fit(t, np.arange(n), seed, p)
+        assert r["rc"] == 0
+        a = {k: t[k].astype(np.float64) for k in K}
+        dz = seed[2] - a["z"]
+        Wx = 1 / (a["var_x"] + dz ** 2 * a["var_tx"]); Wy = 1 / (a["var_y"] + dz ** 2 * a["var_ty"])
+        w = r["w"]
+
+        def chi2(al):
+            rx = a["x"] + (al[2] - a["z"]) * a["tx"] - al[0]
+            ry = a["y"] + (al[2] - a["z"]) * a["ty"] - al[1]
+            return float(np.sum(w * (rx * rx * Wx + ry * ry * Wy)))
+        res = minimize(chi2, np.array(seed), method="Nelder-Mead", options=dict(xatol=1e-10, fatol=1e-14, maxiter=4000))
+        assert np.allclose(res.x, r["pos"], atol=2e-5)
+        # Tukey (Eq. 18): recompute the weights independently at the pre-step position of the last iteration
+        prev = r["trace"][r["niter"] - 2, :3] if r["niter"] > 1 else np.array(seed)
+        rx = a["x"] + (prev[2] - a["z"]) * a["tx"] - prev[0]; ry = a["y"] + (prev[2] - a["z"]) * a["ty"] - prev[1]
+        c = rx * rx * Wx + ry * ry * Wy
+        wexp = np.where(c < 12, (1 - c / 12) ** 2, 0.0)
+        assert np.allclose(w, wexp, atol=1e-12)
+        assert w[0] == 0.0 or w[0] < 0.3
+        assert r["ntrk"] == int((wexp > 0).sum())
+        assert abs(r["chi2"] - float(np.sum(wexp * c))) < 1e-9
+
+
+def test_fit_invariants(oracle, cfg0, cfg0_oracle):
+    """dchi2 <= 0 (Eq. 17 with positive-definite A), C symmetric positive definite, iterations in 1..10,
+    'typically three to seven' (L225)."""
+    d = cfg0_oracle["debug"]
+    tr = d["trace"]
+    ni = d["seed_niter"]
+    ok = ni > 0
+    assert ok.sum() > 4000
+    for e, k in zip(*np.nonzero(ok)):
+        t = tr[e, k, :ni[e, k]]
+        assert np.all(t[:, 9] <= 1e-12)
+        C = t[-1, 3:9]
+        Cm = np.array([[C[0], C[1], C[2]], [C[1], C[3], C[4]], [C[2], C[4], C[5]]])
+        assert np.all(np.linalg.eigvalsh(Cm) > 0)
+    n = ni[ok]
+    assert n.min() >= 2 and n.max() <= 10
+    frac_3_7 = np.mean((n >= 3) & (n <= 7))
+    assert frac_3_7 > 0.8
+    assert np.mean(n == 10) < 0.1
+
+
+def test_pull_width_on_synthetic_events(oracle, cfg0, cfg0_oracle):
+    """'the PV estimator is unbiased, and uncertainties are well estimated' (L307): z pull of matched
+    vertices has mean ~0 and width ~1 on the synthetic configs[0]."""
+    o = cfg0_oracle
+    tr = cfg0["truth"]
+    pulls = []
+    matched = 0
+    for e in range(1000):
+        tz = tr["pv_z"][tr["pv_event"] == e]
+        nt = tr["pv_ntracks"][tr["pv_event"] == e]
+        for v in range(o["n_vtx"][e]):
+            z, s = o["vtx_pos"][e, v, 2], np.sqrt(o["vtx_cov"][e, v, 5])
+            j = np.argmin(np.abs(tz - z))
+            if abs(tz[j] - z) < 5 * s and nt[j] >= 10 and np.sum(np.abs(tz - tz[j]) < 3.0) == 1:
+                pulls.append((z - tz[j]) / s); matched += 1
+    pulls = np.array(pulls)
+    assert matched > 2000
+    core = pulls[np.abs(pulls) < 4]
+    assert abs(core.mean()) < 0.06
+    assert 0.9 < core.std() < 1.15
+
+
+def test_efficiency_and_fakes_on_synthetic_events(oracle, cfg0, cfg0_oracle):
+    """Eq. 20-21 figures of merit on configs[0] (sanity, not a parity gate): efficiency of reconstructible
+    PVs (>= 4 tracks, L257) above 90 %, fake rate below 3 % (paper: 93 % / 1.7 %, L297-303)."""
+    o = cfg0_oracle
+    tr = cfg0["truth"]
+    n_rec = n_fake = n_mc = n_found = 0
+    for e in range(1000):
+        sel = tr["pv_event"] == e
+        tz, nt = tr["pv_z"][sel], tr["pv_ntracks"][sel]
+        vz = o["vtx_pos"][e, :o["n_vtx"][e], 2]
+        vs = np.sqrt(o["vtx_cov"][e, :o["n_vtx"][e], 5])
+        used = np.zeros(len(vz), bool)
+        for z, n in zip(tz, nt):
+            if n < 4:
+                continue
+            n_mc += 1
+            if len(vz):
+                j = int(np.argmin(np.abs(vz - z)))
+                if abs(vz[j] - z) < 5 * vs[j]:
+                    n_found += 1; used[j] = True
+        n_rec += len(vz)
+        for j in range(len(vz)):
+            if not used[j] and (len(tz) == 0 or np.min(np.abs(tz - vz[j])) > 5 * vs[j]):
+                n_fake += 1
+    assert n_found / n_mc > 0.90
+    assert n_fake / n_rec < 0.03
+
+
+def test_singular_fit_and_bad_covariance(oracle):
+    p = oracle.default_params()
+    rng = np.random.default_rng(14)
+    t = _tracks(rng, 6, (0, 0, 0))
+    # one usable track only -> fewer than 2 tracks with w > 0 -> singular
+    t["x"][1:] += np.float32(50.0)
+    r = oracle.fit(t, np.arange(6), (0.0, 0.0, 0.0), p)
+    assert r["rc"] == -1 and r["niter"] == -1
+    # non-positive variance: that track is ignored (w = 0), the rest still fits (R-7)
+    t = _tracks(rng, 10, (0, 0, 0)); t["var_x"][0] = np.float32(-1.0)
+    r = oracle.fit(t, np.arange(10), (0.0, 0.0, 0.1), p)
+    assert r["rc"] == 0 and r["w"][0] == 0.0 and r["ntrk"] <= 9
+
+
+def _one_event(parts):
+    ev = {k: np.concatenate([q[k] for q in parts]) for k in K}
+    return events.from_lists([ev])
+
+
+def test_cleanup_duplicate_removal_and_cuts(oracle):
+    """O8 on hand-built events: duplicates (L245), min tracks in the PV (Table 2), beamline distance (L247)."""
+    rng = np.random.default_rng(15)
+    p = oracle.default_params()
+    # (a) two well separated PVs survive
+    ev = _one_event([_tracks(rng, 30, (0.0, 0.0, -20.0)), _tracks(rng, 25, (0.0, 0.0, 30.0))])
+    o = oracle.find(ev, p, debug=True)
+    assert o["n_vtx"][0] == 2 and sorted(o["vtx_ntracks"][0, :2]) == sorted(o["debug"]["seed_ntrk"][0, :2])
+    assert set(o["trk_vertex"]) <= {-1, 0, 1}
+    # (b) beamline distance: a displaced pp vertex (0.5 mm in x) is discarded, its tracks released ...
+    ev = _one_event([_tracks(rng, 30, (0.5, 0.0, 10.0))])
+    o = oracle.find(ev, p, debug=True)
+    # (the displaced vertex smears z_poca, so several seeds may appear; none may survive, and the
+    # best-populated one must die by the beamline-distance cut)
+    ns = o["debug"]["n_seeds"][0]
+    best = int(np.argmax(o["debug"]["seed_ntrk"][0, :ns]))
+    assert o["n_vtx"][0] == 0 and ns >= 1 and o["debug"]["seed_fate"][0, best] == -4
+    assert abs(o["debug"]["seed_pos"][0, best, 0] - 0.5) < 0.1
+    assert np.all(o["trk_vertex"] == -1) and np.all(o["trk_weight"] == 0)
+    # ... but not in the gas region (cut applies to the pp region only)
+    ev = _one_event([_tracks(rng, 30, (0.5, 0.0, -400.0), slope=0.15)])
+    o = oracle.find(ev, p, debug=True)
+    assert o["n_vtx"][0] == 1
+    # (c) min tracks in the PV: 3 tracks make a seed (>= 3) but not a pp PV (>= 4); in the gas cell 3 suffice
+    three = _tracks(rng, 3, (0.0, 0.0, 5.0), sig=(0.01, 0.012))
+    o = oracle.find(_one_event([three]), p, debug=True)
+    assert o["debug"]["n_seeds"][0] == 1 and o["n_vtx"][0] == 0 and o["debug"]["seed_fate"][0, 0] == -3
+    three = _tracks(rng, 3, (0.0, 0.0, -420.0), sig=(0.01, 0.012))
+    o = oracle.find(_one_event([three]), p, debug=True)
+    assert o["n_vtx"][0] == 1 and o["vtx_ntracks"][0, 0] == 3
+    # (d) duplicates (L245): with merge_ratio raised to 1e6 every pair of neighbours 3 mm apart counts as
+    # duplicates ((dz)^2 / (s1^2 + s2^2) ~ 9 / 2e-3); the greedy z-ordered sweep keeps the most populated
+    pm = oracle.default_params(merge_ratio=1e6)
+    A = _tracks(rng, 10, (0.0, 0.0, 0.0)); B = _tracks(rng, 30, (0.0, 0.0, 3.0)); Cc = _tracks(rng, 20, (0.0, 0.0, 6.0))
+    ev = _one_event([A, B, Cc])
+    o = oracle.find(ev, pm, debug=True)
+    assert o["debug"]["n_seeds"][0] == 3 and list(o["debug"]["seed_fate"][0, :3]) == [-2, 0, -2]
+    assert o["n_vtx"][0] == 1 and abs(o["vtx_pos"][0, 0, 2] - 3.0) < 0.1
+    tv = o["trk_vertex"]
+    assert np.all(tv[:10] == -1) and np.all(tv[40:] == -1) and np.all(o["trk_weight"][:10] == 0)
+    assert (tv[10:40] == 0).sum() >= 28
+    o = oracle.find(ev, p, debug=True)                 # default ratio 25: 3 mm apart are distinct PVs
+    assert o["n_vtx"][0] == 3
+    # tie: equal track counts (noiseless tracks, all weights ~1) -> the lower z is kept
+    A = _tracks(rng, 10, (0.0, 0.0, 0.0), noise=False); B = _tracks(rng, 10, (0.0, 0.0, 3.0), noise=False)
+    o = oracle.find(_one_event([A, B]), pm, debug=True)
+    assert list(o["debug"]["seed_ntrk"][0, :2]) == [10, 10] and list(o["debug"]["seed_fate"][0, :2]) == [0, -2]
+    # the ratio itself: two PVs 3 mm apart with sigma_z^2 sum known from the output -> threshold just above/below
+    o = oracle.find(_one_event([A, B]), p, debug=True)
+    d = o["debug"]
+    ratio = (d["seed_pos"][0, 1, 2] - d["seed_pos"][0, 0, 2]) ** 2 / (d["seed_cov"][0, 0, 5] + d["seed_cov"][0, 1, 5])
+    assert oracle.find(_one_event([A, B]), oracle.default_params(merge_ratio=ratio * 1.01))["n_vtx"][0] == 1
+    assert oracle.find(_one_event([A, B]), oracle.default_params(merge_ratio=ratio * 0.99))["n_vtx"][0] == 2
+
+
+def test_close_pairs_merge_at_small_separation(oracle):
+    """configs[3]: at dz = 0.1 mm exactly one vertex survives; at 5 mm two are resolved (L127: 'cannot
+    separate vertices that are closer than about 2 mm')."""
+    d = events.generate(events.config(3, 1200))
+    o = oracle.find(d, oracle.default_params())
+    nv = o["n_vtx"]
+    sep_idx = np.arange(1200) % 6
+    assert np.mean(nv[sep_idx == 0] == 1) > 0.98
+    assert np.mean(nv[sep_idx == 5] == 2) > 0.97
+    two = [np.mean(nv[sep_idx == j] == 2) for j in range(6)]
+    assert two[0] < 0.02 and all(two[j] <= two[j + 1] + 0.03 for j in range(5))
+
+
+def test_thread_count_and_track_order_invariance(oracle):
+    d = events.generate(events.config(1, 300))
+    p = oracle.default_params()
+    a = oracle.find(d, p, n_threads=1)
+    b = oracle.find(d, p, n_threads=4)
+    for k in ("vtx_pos", "vtx_cov", "n_vtx", "trk_vertex", "trk_weight", "vtx_niter"):
+        assert np.array_equal(a[k], b[k])
+    # reversing the track order inside each event changes only floating-point summation order
+    off = d["offsets"]
+    perm = np.concatenate([np.arange(off[e + 1] - 1, off[e] - 1, -1) for e in range(300)])
+    d2 = {k: d[k][perm] for k in events.FIELDS}; d2["offsets"] = off; d2["n_events"] = 300
+    c = oracle.find(d2, p)
+    assert np.array_equal(a["n_vtx"], c["n_vtx"])
+    same_iter = a["vtx_niter"] == c["vtx_niter"]
+    assert same_iter.mean() > 0.999
+    assert np.abs(a["vtx_pos"] - c["vtx_pos"])[same_iter].max() < 1e-9
+    assert np.array_equal(a["trk_vertex"][perm], c["trk_vertex"])
