@@ -1,0 +1,185 @@
+/* pv_finder.h -- C ABI of the B200-native primary-vertex (PV) finder hot path of arXiv:2412.14966.
+ *
+ * One call, pv_find(), runs the five steps the paper lists ("P:Lnn" = PAPER.md line nn)
+ * plus the post-fit cleanup over a batch of independent events ("events are independent
+ * from each other"), entirely in hand-written CUDA kernels for sm_100a:
+ *
+ *   a1 project  z_poca (Eq. 1), sigma_poca (Eq. 3)
+ *   a2 fill     per-event z-histogram of Gaussian bin integrals, int32 fixed point (2^20 = 1 track)
+ *   a3 peaks    proto-clusters, dip search, z-ordered splitting, seed z (Eq. 4-5)
+ *   a4 assign   bin -> closest seed via partition points, removal of under-populated seeds
+ *   a5 fit      adaptive Tukey-weighted Newton-Raphson vertex fit (Eq. 6-18)
+ *   a6 cleanup  duplicate removal, min tracks, beamline distance (Table 2)
+ *
+ * The readings taken where the paper is silent are listed in DESIGN.md section "Readings".
+ *
+ * Conventions
+ *   - No torch / C++ types: plain pointers and sizes.  Every pointer says HOST or DEVICE below.
+ *   - The caller owns every buffer.  pv_find never allocates, frees or synchronises; all work is
+ *     enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - Return value: 0 (PV_OK) or a negative PV_E_* code.  Data-dependent problems never fail the
+ *     call; they set bits in event_status[e].
+ *   - Device base pointers must be 4-byte aligned; per-event offsets need no alignment.
+ *   - Thread safety: calls on different streams are independent provided they use different
+ *     workspaces and output buffers.
+ */
+#ifndef PV_FINDER_H
+#define PV_FINDER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* All lengths in mm.  Index 0 = pp region (z >= z_split), 1 = p-gas / SMOG2 region (z < z_split). */
+typedef struct pv_params {
+  float z_min, z_max, dz;               /* histogram range and bin size: -550, 300, 0.25 */
+  float z_split;                        /* region boundary: -300                          Table 2 */
+  float beam_x, beam_y, beam_tx, beam_ty; /* beamline position and direction at z = 0 */
+  float max_sigma_poca[2];              /* max sigma_poca to enter the histogram: 1.5, 10  P:L129, Table 2 */
+  float min_bin_content;                /* proto-cluster bin threshold [tracks]: 0.25      P:L135 (value: reading R-4) */
+  float min_dip;                        /* significance of an extremum [tracks]: 0.75      P:L135 (value: reading R-4) */
+  float min_cluster_integral[2];        /* min track integral of a seed cluster: 2.5, 1.75 Table 2 */
+  int32_t min_tracks_seed[2];           /* min tracks associated to a seed: 3, 2 */
+  int32_t min_tracks_pv[2];             /* min tracks in a fitted PV: 4, 3                 Table 2 */
+  float chi2_max;                       /* Tukey cut-off: 12 (INFINITY = unit weights)     Eq. 18 */
+  int32_t max_iter;                     /* max fit iterations: 10 (1..16) */
+  float conv_dchi2, conv_dz;            /* convergence: |dchi2| < 0.01 and |dz| < 0.001 mm P:L225 */
+  float merge_ratio;                    /* duplicate iff dz^2/(Czz1+Czz2) < 25 */
+  float max_beam_dist;                  /* pp vertices farther than 0.3 mm are discarded */
+  int32_t max_vtx_per_event;            /* output stride per event, 1..PV_MAX_VTX (default 32) */
+} pv_params;
+
+enum {
+  PV_OK = 0,
+  PV_E_NULL = -1,       /* a required pointer is NULL */
+  PV_E_PARAM = -2,      /* invalid parameter (dz <= 0, range not a whole number of bins, too many bins, ...) */
+  PV_E_WORKSPACE = -3,  /* workspace too small */
+  PV_E_CUDA = -4,       /* a CUDA runtime call or kernel launch failed (see pv_last_cuda_error) */
+  PV_E_SIZE = -5        /* negative n_events / n_tracks, or a host staging capacity exceeded */
+};
+
+/* Compile-time limits of this build. */
+enum {
+  PV_MAX_BINS = 4096,          /* (z_max - z_min) / dz must be <= this */
+  PV_MAX_VTX = 32,             /* max_vtx_per_event must be <= this */
+  PV_MAX_TRACKS_PER_EVENT = 2047, /* larger events get PV_EVT_TOO_MANY_TRACKS and zero vertices */
+  PV_FIXED_ONE = 1 << 20       /* histogram fixed-point unit: the full mass of one track */
+};
+
+/* event_status bit flags */
+enum {
+  PV_EVT_TOO_MANY_TRACKS = 1,  /* n_tracks(e) > PV_MAX_TRACKS_PER_EVENT: event skipped, n_vtx = 0 */
+  PV_EVT_VTX_OVERFLOW = 2,     /* more seed clusters than max_vtx_per_event: the first max_vtx in z are kept */
+  PV_EVT_SINGULAR_FIT = 4      /* a vertex fit had < 2 active tracks or a non-positive pivot: that vertex is dropped */
+};
+
+/* Fill *p with the paper's values (citations on the struct above).  p: HOST.  Returns PV_OK / PV_E_NULL. */
+int pv_params_default(pv_params* p);
+
+/* Number of histogram bins implied by p (lrint((z_max - z_min) / dz)), or a negative PV_E_* if p is invalid. */
+int pv_nbins(const pv_params* p);
+
+/* Bytes of DEVICE workspace pv_find needs for a batch of this size (a small constant today; the
+ * histograms live in shared memory, "one block per event").  bytes: HOST out. */
+int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, size_t* bytes);
+
+/* The hot path a1..a6 over a batch.
+ *
+ * Inputs (DEVICE, read-only, fp32 SoA, length T = offsets[n_events]; "same data members of all
+ * tracks contiguous"): track state x, y, z, tx, ty and the diagonal of its covariance
+ * var_x, var_y, var_tx, var_ty (Eq. 2, diagonal form).
+ *   offsets   DEVICE int32[n_events + 1], offsets[0] = 0, non-decreasing; event e owns tracks
+ *             [offsets[e], offsets[e+1]).
+ *   n_tracks  T, as known to the host (only used for validation and sizing; the kernel reads offsets).
+ *   params    HOST, copied by value at call time.
+ * Outputs (DEVICE, caller-allocated):
+ *   vtx_pos      float[n_events][max_vtx][3]   x, y, z of each PV, ordered in z
+ *   vtx_cov      float[n_events][max_vtx][6]   upper triangle xx, xy, xz, yy, yz, zz of C (Eq. 14)
+ *   vtx_chi2     float[n_events][max_vtx]      sum_i w_i chi2_i of the last iteration (Eq. 6)
+ *   vtx_ntracks  int32[n_events][max_vtx]      tracks with w_i > 0 in the last iteration
+ *   vtx_niter    int32[n_events][max_vtx]      Newton iterations done
+ *   n_vtx        int32[n_events]               PVs found; only the first n_vtx[e] slots of event e are written
+ *   trk_weight   float[T]                      Tukey weight w_i of the last iteration (Eq. 18); 0 if unassigned
+ *   trk_vertex   int32[T]                      index of the track's PV within its event, -1 = none
+ *   event_status uint32[n_events]              PV_EVT_* flags
+ *   (trk_weight / trk_vertex also serve as per-track scratch during the call.)
+ * workspace: DEVICE, >= pv_workspace_bytes() bytes, 16-byte aligned; contents are scratch.
+ * stream: cudaStream_t.
+ */
+int pv_find(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+            const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+            const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+            float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+            int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+            void* workspace, size_t workspace_bytes, void* stream);
+
+/* Parity taps: every member is a nullable DEVICE pointer; no global state. */
+typedef struct pv_debug {
+  int32_t* hist;          /* [n_hist_events][nbins]: histogram of the first n_hist_events events (a2) */
+  int32_t n_hist_events;
+  float* z_poca;          /* [T] (a1) */
+  float* sigma_poca;      /* [T] (a1) */
+  int32_t* trk_bin;       /* [T] central bin, -1 = not assignable (a1) */
+  int32_t* n_seeds_raw;   /* [E] clusters found by the peak search before truncation / removal (a3) */
+  int32_t* n_seeds;       /* [E] seeds after the removal loop (a4) */
+  float* seed_z;          /* [E][max_vtx] (a3, Eq. 4-5) */
+  int32_t* seed_bins;     /* [E][max_vtx][3] begin, end, peak (a3) */
+  int32_t* trk_seed;      /* [T] pre-cleanup assignment (a4) */
+  float* seed_pos;        /* [E][max_vtx][3] fitted position per seed, pre-cleanup (a5) */
+  float* seed_cov;        /* [E][max_vtx][6] */
+  float* seed_chi2;       /* [E][max_vtx] */
+  int32_t* seed_ntrk;     /* [E][max_vtx] */
+  int32_t* seed_niter;    /* [E][max_vtx], -1 = singular */
+  int32_t* seed_fate;     /* [E][max_vtx] final vertex index, or -1 singular, -2 merged, -3 min tracks, -4 beam distance */
+} pv_debug;
+
+/* Same as pv_find, additionally writing the taps selected in *dbg (HOST struct of DEVICE pointers). */
+int pv_find_debug(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                  const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                  const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                  float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                  int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+                  void* workspace, size_t workspace_bytes, void* stream, const pv_debug* dbg);
+
+/* ---- host-buffer entry (the paper's host pipeline: "several streams ... each processing a batch",
+ * host->device copies overlapped with compute).  A pv_host_ctx owns device buffers, pinned staging and
+ * streams sized for at most max_events / max_tracks; pv_find_host() takes HOST pointers everywhere
+ * (same meaning and layout as pv_find), splits the batch into n_chunks contiguous event ranges, and
+ * for each enqueues H2D copies -> pv_find -> D2H copies on one of the context's streams.  It returns
+ * after all results are in the caller's host arrays (it synchronises its own streams only). */
+typedef struct pv_host_ctx pv_host_ctx;
+int pv_host_ctx_create(pv_host_ctx** ctx, int max_events, long long max_tracks, const pv_params* params,
+                       int n_streams);
+int pv_host_ctx_destroy(pv_host_ctx* ctx);
+int pv_find_host(pv_host_ctx* ctx,
+                 const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                 const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                 const int32_t* offsets, int n_events, const pv_params* params,
+                 float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                 int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+                 int n_chunks);
+/* Pin / unpin caller host memory so pv_find_host copies run asynchronously (optional). */
+int pv_host_register(void* ptr, size_t bytes);
+int pv_host_unregister(void* ptr);
+
+/* Launch statistics of the most recent pv_find / pv_find_debug call of this process (for bench.py):
+ * kernels launched, grid size, block size, dynamic shared memory per block.  All HOST out, nullable. */
+int pv_last_launch_info(int* n_kernels, int* grid, int* block, int* smem_bytes);
+
+/* Optional: CUDA events recorded around the kernel of the next pv_find calls on their own stream, so a
+ * caller can time the dominant kernel live.  pv_kernel_timing(1) enables, (0) disables;
+ * pv_kernel_time_ms() synchronises the last pair and returns its duration in ms (< 0 if none). */
+int pv_kernel_timing(int enable);
+float pv_kernel_time_ms(void);
+
+const char* pv_error_string(int code);
+/* Text of the last CUDA error seen by this library in this process ("" if none).  HOST. */
+const char* pv_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PV_FINDER_H */

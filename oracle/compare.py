@@ -1,0 +1,246 @@
+"""Element-by-element comparator: results of the CUDA path vs the CPU oracle on the same seeded inputs.
+
+TEST INFRASTRUCTURE ONLY (used by tests/, __graft_entry__.smoke() and bench.py's parity spot check).  Pure
+numpy; imports neither the product nor the oracle library: both result dicts are passed in.
+
+Tolerances (BASELINE.json north_star):
+  * z_poca, sigma_poca, central bin, histogram bins, seed clusters (begin, end, peak), seed z: bit-exact
+  * per-event seed count and vertex count: identical
+  * fitted vertex x, y, z: 1e-3 mm;  covariance: 1e-3 relative (off-diagonals relative to sqrt(Cii Cjj))
+  * track -> vertex assignment: >= 99.9 % agreement, every mismatch explained by a logged near-tie
+Near-tie rules:
+  * iteration count: the fp32 fit and the fp64 oracle may stop one iteration apart when the deciding
+    |dchi2| or |dz| of the oracle is within NEAR_REL of its cut; the GPU vertex is then compared with the
+    oracle's trace entry at the GPU's iteration count.
+  * cleanup decisions (merge ratio, beamline distance, min tracks through a weight at the Tukey edge):
+    a differing fate is accepted when the oracle's deciding quantity is within NEAR_REL of its cut.
+"""
+from __future__ import annotations
+
+from typing import Dict, List
+
+import numpy as np
+
+POS_TOL = 1e-3       # mm
+COV_RTOL = 1e-3
+W_TOL = 2e-3         # Tukey weight, absolute (vertices with equal iteration count)
+NEAR_REL = 1e-2
+MIN_ASSIGN_AGREEMENT = 0.999
+
+
+def _cov_rel_err(cg: np.ndarray, cr: np.ndarray) -> np.ndarray:
+    """max over the 6 elements of |dC_ij| / sqrt(C_ii C_jj) (reference values in the denominator)."""
+    d = np.sqrt(np.abs(cr[..., [0, 3, 5]]))
+    scale = np.stack([d[..., 0] * d[..., 0], d[..., 0] * d[..., 1], d[..., 0] * d[..., 2],
+                      d[..., 1] * d[..., 1], d[..., 1] * d[..., 2], d[..., 2] * d[..., 2]], axis=-1)
+    scale = np.where(scale > 0, scale, 1.0)
+    return np.max(np.abs(cg - cr) / scale, axis=-1)
+
+
+def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.ndarray, p, max_log: int = 20) -> Dict:
+    """gpu: binding.DeviceBatch.results() with debug=True; ref: oracle.pvref.find(debug=True, trace=True).
+    Returns a report dict with 'failures' (list of strings; empty = parity) and 'near_ties' (logged)."""
+    fails: List[str] = []
+    ties: List[str] = []
+    rep: Dict = {"failures": fails, "near_ties": ties}
+    gd, rd = gpu.get("debug"), ref.get("debug")
+    E = offsets.size - 1
+    mv = p.max_vtx_per_event
+    ev_of_trk = np.repeat(np.arange(E), np.diff(offsets))
+    skipped = (ref["event_status"] & 1) != 0          # TOO_MANY_TRACKS: per-track taps are undefined there
+    trk_ok = ~skipped[ev_of_trk] if ev_of_trk.size else np.zeros(0, bool)
+
+    def exact(name, a, b, mask=None):
+        a, b = np.asarray(a), np.asarray(b)
+        if a.shape != b.shape:
+            fails.append(f"{name}: shape {a.shape} vs {b.shape}")
+            return
+        if a.dtype.kind == "f":
+            eq = (a.view(np.uint32) == b.view(np.uint32)) | (np.isnan(a) & np.isnan(b)) if a.dtype == np.float32 and b.dtype == np.float32 \
+                else ((a == b) | (np.isnan(a) & np.isnan(b)))
+        else:
+            eq = a == b
+        if mask is not None:
+            eq = eq | ~mask
+        nbad = int(eq.size - np.count_nonzero(eq))
+        rep[f"{name}_mismatch"] = nbad
+        if nbad:
+            idx = np.argwhere(~eq)[:3]
+            fails.append(f"{name}: {nbad} of {eq.size} differ (bit-exact required), first at {idx.tolist()}: "
+                         f"gpu {a[tuple(idx[0])]} ref {b[tuple(idx[0])]}")
+
+    # ---- status and counts ----------------------------------------------------------------------------------
+    exact("event_status", gpu["event_status"].astype(np.uint32) & ~np.uint32(4), ref["event_status"].astype(np.uint32) & ~np.uint32(4))
+    if gd is not None and rd is not None:
+        # ---- a1: projection ---------------------------------------------------------------------------------
+        exact("z_poca", gd["z_poca"], rd["z_poca"], trk_ok)
+        exact("sigma_poca", gd["sigma_poca"], rd["sigma_poca"], trk_ok)
+        exact("trk_bin", gd["trk_bin"], np.where((rd["trk_flags"] & 1) != 0, rd["trk_bin"], -1), trk_ok)
+        # ---- a2: histogram ----------------------------------------------------------------------------------
+        nh = min(gd["hist"].shape[0], rd["hist"].shape[0])
+        if nh > 0 and gd["hist"].shape[1] == rd["hist"].shape[1]:
+            exact("hist", gd["hist"][:nh], rd["hist"][:nh], np.broadcast_to((~skipped[:nh])[:, None], rd["hist"][:nh].shape))
+        # ---- a3 / a4: seeds ---------------------------------------------------------------------------------
+        exact("n_seeds_raw", gd["n_seeds_raw"], rd["n_seeds_raw"])
+        exact("n_seeds", gd["n_seeds"], rd["n_seeds"])
+        ks = np.arange(mv)[None, :] < rd["n_seeds"][:, None]
+        exact("seed_bins", gd["seed_bins"], rd["seed_bins"], np.repeat(ks[:, :, None], 3, axis=2))
+        exact("seed_z", gd["seed_z"], rd["seed_z"], ks)
+        exact("trk_seed", gd["trk_seed"], rd["trk_seed"])
+
+        # ---- a5: per-seed fit, pre-cleanup -------------------------------------------------------------------
+        same_seeds = gd["n_seeds"] == rd["n_seeds"]
+        ks = ks & same_seeds[:, None]
+        gn, rn = gd["seed_niter"], rd["seed_niter"]
+        sing_g, sing_r = (gn < 0) & ks, (rn < 0) & ks
+        bad_sing = sing_g != sing_r
+        if bad_sing.any():
+            for e, k in np.argwhere(bad_sing)[:max_log]:
+                ties.append(f"singular-fit flag differs at event {e} seed {k}: gpu niter {gn[e, k]} ref {rn[e, k]}")
+            rep["singular_mismatch"] = int(bad_sing.sum())
+        fit = ks & ~sing_g & ~sing_r
+        ref_pos = rd["seed_pos"].copy()
+        ref_cov = rd["seed_cov"].copy()
+        niter_diff = fit & (gn != rn)
+        rep["n_fitted_seeds"] = int(fit.sum())
+        rep["n_niter_diff"] = int(niter_diff.sum())
+        trace = rd.get("trace")
+        cuts = (float(p.conv_dchi2), float(p.conv_dz))
+        tie_mask = np.zeros_like(fit)
+        for e, k in np.argwhere(niter_diff):
+            g_it, r_it = int(gn[e, k]), int(rn[e, k])
+            ok = False
+            why = "no oracle trace"
+            if trace is not None and 1 <= g_it <= trace.shape[2]:
+                it = min(g_it, r_it)                  # the iteration at which one side stopped and the other went on
+                dchi2, dz = abs(trace[e, k, it - 1, 9]), abs(trace[e, k, it - 1, 10])
+                near = (abs(dchi2 - cuts[0]) <= NEAR_REL * cuts[0]) or (abs(dz - cuts[1]) <= NEAR_REL * cuts[1])
+                why = f"oracle |dchi2| {dchi2:.6g} (cut {cuts[0]:g}), |dz| {dz:.6g} (cut {cuts[1]:g}) at iteration {it}"
+                if near:
+                    ok = True
+                    ref_pos[e, k] = trace[e, k, g_it - 1, 0:3]
+                    ref_cov[e, k] = trace[e, k, g_it - 1, 3:9]
+                    tie_mask[e, k] = True
+            msg = f"iteration count differs at event {e} seed {k}: gpu {g_it} ref {r_it}; {why}"
+            (ties if ok else fails).append(("near-tie: " if ok else "NOT a near-tie: ") + msg)
+        dpos = np.abs(gd["seed_pos"].astype(np.float64) - ref_pos).max(axis=-1)
+        dcov = _cov_rel_err(gd["seed_cov"].astype(np.float64), ref_cov)
+        rep["seed_pos_max_err_mm"] = float(dpos[fit].max()) if fit.any() else 0.0
+        rep["seed_cov_max_rel_err"] = float(dcov[fit].max()) if fit.any() else 0.0
+        badp = fit & ~(dpos <= POS_TOL)
+        badc = fit & ~(dcov <= COV_RTOL)
+        for e, k in np.argwhere(badp)[:max_log]:
+            fails.append(f"seed position off by {dpos[e, k]:.3g} mm at event {e} seed {k} (niter gpu {gn[e, k]} ref {rn[e, k]})")
+        for e, k in np.argwhere(badc)[:max_log]:
+            fails.append(f"seed covariance off by {dcov[e, k]:.3g} rel at event {e} seed {k} (niter gpu {gn[e, k]} ref {rn[e, k]})")
+        eq_it = fit & ~niter_diff
+        dn = eq_it & (gd["seed_ntrk"] != rd["seed_ntrk"])
+        rep["seed_ntrk_diff"] = int(dn.sum())
+        for e, k in np.argwhere(dn)[:max_log]:
+            ties.append(f"near-tie: active-track count differs at event {e} seed {k}: gpu {gd['seed_ntrk'][e, k]} "
+                        f"ref {rd['seed_ntrk'][e, k]} (a weight at the Tukey cut-off)")
+        dchi = np.abs(gd["seed_chi2"].astype(np.float64) - rd["seed_chi2"])
+        rel = dchi / np.maximum(1.0, np.abs(rd["seed_chi2"]))
+        rep["seed_chi2_max_rel_err"] = float(rel[eq_it & ~dn].max()) if (eq_it & ~dn).any() else 0.0
+        if ((eq_it & ~dn) & (rel > 1e-3)).any():
+            e, k = np.argwhere((eq_it & ~dn) & (rel > 1e-3))[0]
+            fails.append(f"seed chi2 off at event {e} seed {k}: gpu {gd['seed_chi2'][e, k]} ref {rd['seed_chi2'][e, k]}")
+
+        # ---- a6: fate of each seed ---------------------------------------------------------------------------
+        gf, rf = gd["seed_fate"], rd["seed_fate"]
+        fate_diff = ks & (gf != rf)
+        rep["n_fate_diff"] = int(fate_diff.sum())
+        ev_fate_tie = np.zeros(E, bool)
+        for e in np.unique(np.argwhere(fate_diff)[:, 0]) if fate_diff.any() else []:
+            why = _explain_fate(e, rd, p, int(rd["n_seeds"][e]), tie_mask[e], dn[e] | bad_sing[e])
+            if why:
+                ties.append(f"near-tie: cleanup decisions differ in event {e}: {why}")
+                ev_fate_tie[e] = True
+            else:
+                fails.append(f"cleanup decisions differ in event {e} with no near-tie: gpu fate {gf[e][:rd['n_seeds'][e]].tolist()} "
+                             f"ref {rf[e][:rd['n_seeds'][e]].tolist()}")
+    else:
+        ev_fate_tie = np.zeros(E, bool)
+        tie_mask = None
+
+    # ---- final outputs ------------------------------------------------------------------------------------------
+    nv_g, nv_r = gpu["n_vtx"], ref["n_vtx"]
+    nv_bad = (nv_g != nv_r) & ~ev_fate_tie
+    rep["n_vtx_mismatch_events"] = int((nv_g != nv_r).sum())
+    if nv_bad.any():
+        fails.append(f"n_vtx differs in {int(nv_bad.sum())} events without a near-tie, first {np.argwhere(nv_bad)[:5, 0].tolist()}")
+    ev_same = (nv_g == nv_r) & ~ev_fate_tie
+    kv = (np.arange(mv)[None, :] < nv_r[:, None]) & ev_same[:, None]
+    rep["n_vertices"] = int(nv_r.sum())
+    if gd is not None and rd is not None:
+        # map final vertices back to seeds to reuse the (possibly trace-substituted) reference
+        ref_vpos = ref["vtx_pos"].copy()
+        ref_vcov = ref["vtx_cov"].copy()
+        for e, k in np.argwhere(tie_mask) if tie_mask is not None and tie_mask.any() else []:
+            v = rd["seed_fate"][e, k]
+            if v >= 0 and ev_same[e]:
+                ref_vpos[e, v] = ref_pos[e, k]
+                ref_vcov[e, v] = ref_cov[e, k]
+    else:
+        ref_vpos, ref_vcov = ref["vtx_pos"], ref["vtx_cov"]
+    dpos = np.abs(gpu["vtx_pos"].astype(np.float64) - ref_vpos).max(axis=-1)
+    dcov = _cov_rel_err(gpu["vtx_cov"].astype(np.float64), ref_vcov)
+    rep["vtx_pos_max_err_mm"] = float(dpos[kv].max()) if kv.any() else 0.0
+    rep["vtx_cov_max_rel_err"] = float(dcov[kv].max()) if kv.any() else 0.0
+    for e, k in np.argwhere(kv & ~(dpos <= POS_TOL))[:max_log]:
+        fails.append(f"vertex position off by {dpos[e, k]:.3g} mm at event {e} vertex {k}")
+    for e, k in np.argwhere(kv & ~(dcov <= COV_RTOL))[:max_log]:
+        fails.append(f"vertex covariance off by {dcov[e, k]:.3g} rel at event {e} vertex {k}")
+
+    tv_g, tv_r = gpu["trk_vertex"], ref["trk_vertex"]
+    agree = tv_g == tv_r
+    rep["assign_agreement"] = float(agree.mean()) if agree.size else 1.0
+    rep["assign_mismatch_tracks"] = int((~agree).sum())
+    if agree.size and rep["assign_agreement"] < MIN_ASSIGN_AGREEMENT:
+        fails.append(f"track-assignment agreement {rep['assign_agreement']:.6f} < {MIN_ASSIGN_AGREEMENT}")
+    unexplained = (~agree) & ~ev_fate_tie[ev_of_trk] if agree.size else np.zeros(0, bool)
+    if unexplained.any():
+        fails.append(f"{int(unexplained.sum())} track-assignment mismatches outside near-tie events, first track "
+                     f"{int(np.argwhere(unexplained)[0, 0])} (event {int(ev_of_trk[np.argwhere(unexplained)[0, 0]])})")
+    # weights: compare where the assignment agrees and the vertex was not an iteration near-tie
+    wmask = agree & (tv_r >= 0)
+    if tie_mask is not None and tie_mask.any() and wmask.any():
+        tie_ev = tie_mask.any(axis=1)
+        wmask &= ~tie_ev[ev_of_trk]
+    dw = np.abs(gpu["trk_weight"].astype(np.float64) - ref["trk_weight"])
+    rep["trk_weight_max_err"] = float(dw[wmask].max()) if wmask.any() else 0.0
+    nbw = int((dw[wmask] > W_TOL).sum()) if wmask.any() else 0
+    if nbw:
+        i = int(np.argwhere(wmask & (dw > W_TOL))[0, 0])
+        fails.append(f"{nbw} track weights off by more than {W_TOL}, first track {i}: gpu {gpu['trk_weight'][i]} ref {ref['trk_weight'][i]}")
+    zero_ok = np.all(gpu["trk_weight"][tv_g < 0] == 0.0) if tv_g.size else True
+    if not zero_ok:
+        fails.append("unassigned tracks with non-zero weight")
+    rep["n_near_ties"] = len(ties)
+    del ties[max_log:]
+    return rep
+
+
+def _explain_fate(e: int, rd: Dict[str, np.ndarray], p, ns: int, niter_tie: np.ndarray, ntrk_tie: np.ndarray) -> str:
+    """Is some cleanup decision of the ORACLE in event e within NEAR_REL of its cut (or fed by a documented
+    near-tie upstream)?  Returns a description, or '' if nothing is close."""
+    if niter_tie[:ns].any():
+        return "a vertex of the event is an iteration-count near-tie"
+    if ntrk_tie[:ns].any():
+        return "a vertex of the event has a track at the Tukey cut-off / singular-fit edge"
+    pos, cov, ntrk, nit = rd["seed_pos"][e], rd["seed_cov"][e], rd["seed_ntrk"][e], rd["seed_niter"][e]
+    alive = [k for k in range(ns) if nit[k] >= 0]
+    for a in range(len(alive)):
+        for b in range(a + 1, len(alive)):
+            i, j = alive[a], alive[b]
+            ratio = (pos[j, 2] - pos[i, 2]) ** 2 / (cov[j, 5] + cov[i, 5])
+            if abs(ratio - p.merge_ratio) <= NEAR_REL * p.merge_ratio:
+                return f"merge ratio {ratio:.6g} of seeds {i},{j} vs cut {p.merge_ratio:g}"
+    for k in alive:
+        vz = pos[k, 2]
+        if vz >= p.z_split:
+            d2 = (pos[k, 0] - (p.beam_x + p.beam_tx * vz)) ** 2 + (pos[k, 1] - (p.beam_y + p.beam_ty * vz)) ** 2
+            c2 = p.max_beam_dist ** 2
+            if abs(d2 - c2) <= 2 * NEAR_REL * c2:
+                return f"beamline distance^2 {d2:.6g} of seed {k} vs cut {c2:.6g}"
+    return ""

@@ -1,0 +1,402 @@
+// pv_api.cu -- host side of the C ABI declared in include/pv_finder.h: parameter validation, conversion of
+// the paper's thresholds to the fixed-point contract, launch of the persistent warp-per-event kernel, and the
+// host-buffer pipeline.  No CPU fallback exists: without a CUDA device every compute entry returns
+// PV_E_CUDA.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <mutex>
+#include <vector>
+
+#include "pv_kernels.cuh"
+
+namespace {
+
+thread_local char g_cuda_err[512] = "";
+int g_last_kernels = 0, g_last_grid = 0, g_last_block = 0, g_last_smem = 0;
+int g_timing = 0;
+cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+bool g_ev_valid = false;
+
+int cuda_fail(cudaError_t err, const char* what) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(err));
+  return PV_E_CUDA;
+}
+#define CK(call)                                        \
+  do {                                                  \
+    cudaError_t err__ = (call);                         \
+    if (err__ != cudaSuccess) return cuda_fail(err__, #call); \
+  } while (0)
+
+struct DeviceInfo {
+  int device = -1, sms = 0, max_smem_optin = 0;
+  bool attr_set[2] = {false, false};
+  int attr_smem[2] = {0, 0};
+};
+std::mutex g_mu;
+std::vector<DeviceInfo> g_dev;
+
+int get_device_info(DeviceInfo** out) {
+  int dev = 0;
+  CK(cudaGetDevice(&dev));
+  for (auto& d : g_dev)
+    if (d.device == dev) { *out = &d; return PV_OK; }
+  DeviceInfo d;
+  d.device = dev;
+  CK(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev));
+  CK(cudaDeviceGetAttribute(&d.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  g_dev.push_back(d);
+  *out = &g_dev.back();
+  return PV_OK;
+}
+
+long long to_fixed(float tracks) {
+  const double v = (double)tracks * (double)PV_FIXED_ONE;
+  if (!(v < 9.0e18)) return 0x7fffffffffffffffLL;
+  if (!(v > -9.0e18)) return -0x7fffffffffffffffLL;
+  return llrint(v);
+}
+int clamp_i32(long long v) {
+  if (v > 0x7fffffffLL) return 0x7fffffff;
+  if (v < -0x7fffffffLL) return -0x7fffffff;
+  return (int)v;
+}
+
+int validate(const pv_params* p, int* nbins_out) {
+  if (!p) return PV_E_NULL;
+  if (!(p->dz > 0.0f) || !(p->z_max > p->z_min)) return PV_E_PARAM;
+  const double nb = ((double)p->z_max - (double)p->z_min) / (double)p->dz;
+  if (!(nb >= 1.0) || nb > (double)PV_MAX_BINS + 0.5) return PV_E_PARAM;
+  const int nbins = (int)lrint(nb);
+  if (nbins < 1 || nbins > PV_MAX_BINS) return PV_E_PARAM;
+  if (fabs((double)nbins * (double)p->dz - ((double)p->z_max - (double)p->z_min)) > 1e-6 * (double)p->dz) return PV_E_PARAM;
+  if (p->max_vtx_per_event < 1 || p->max_vtx_per_event > PV_MAX_VTX) return PV_E_PARAM;
+  if (p->max_iter < 1 || p->max_iter > 16) return PV_E_PARAM;
+  if (!(p->chi2_max > 0.0f)) return PV_E_PARAM;
+  if (nbins_out) *nbins_out = nbins;
+  return PV_OK;
+}
+
+void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
+  memset(k, 0, sizeof(*k));
+  k->z_min = p->z_min; k->dz = p->dz; k->inv_dz = 1.0f / p->dz; k->z_split = p->z_split;
+  k->beam_x = p->beam_x; k->beam_y = p->beam_y; k->beam_tx = p->beam_tx; k->beam_ty = p->beam_ty;
+  k->max_sigma[0] = p->max_sigma_poca[0]; k->max_sigma[1] = p->max_sigma_poca[1];
+  k->win_eps = 0.0625f + 2e-6f * (float)nbins;
+  k->nbins = nbins; k->nwords = (nbins + 31) / 32;
+  k->T_bin = clamp_i32(to_fixed(p->min_bin_content));
+  k->D = clamp_i32(to_fixed(p->min_dip));
+  k->I_min[0] = to_fixed(p->min_cluster_integral[0]); k->I_min[1] = to_fixed(p->min_cluster_integral[1]);
+  for (int r = 0; r < 2; ++r) { k->min_tracks_seed[r] = p->min_tracks_seed[r]; k->min_tracks_pv[r] = p->min_tracks_pv[r]; }
+  k->chi2_max = p->chi2_max;
+  k->unit_weights = isinf(p->chi2_max) ? 1 : 0;
+  k->inv_chi2_max = k->unit_weights ? 0.0f : 1.0f / p->chi2_max;
+  k->max_iter = p->max_iter;
+  k->conv_dchi2 = p->conv_dchi2; k->conv_dz = p->conv_dz; k->merge_ratio = p->merge_ratio;
+  k->max_beam_dist2 = p->max_beam_dist * p->max_beam_dist;
+  k->max_vtx = p->max_vtx_per_event;
+  int r0 = ((nbins + 31) / 32) * 32 * 4;                      // histogram padded to whole 32-bin words
+  if (r0 < pvk::OVL_MIN_BYTES) r0 = pvk::OVL_MIN_BYTES;
+  r0 = (r0 + 15) / 16 * 16;
+  k->region0_words = r0 / 4;
+  k->warp_smem_bytes = r0 + pvk::R1_BYTES + pvk::R2_BYTES;
+}
+
+constexpr size_t WORKSPACE_BYTES = 256;
+
+int find_impl(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+              const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+              const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+              float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+              int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+              void* workspace, size_t workspace_bytes, void* stream_, const pv_debug* dbg) {
+  int nbins = 0;
+  int rc = validate(params, &nbins);
+  if (rc != PV_OK) return rc;
+  if (n_events < 0 || n_tracks < 0 || n_tracks > 0x7fffffffLL) return PV_E_SIZE;
+  if (!offsets || !n_vtx || !event_status || !vtx_pos || !vtx_cov || !vtx_chi2 || !vtx_ntracks || !vtx_niter || !workspace)
+    return PV_E_NULL;
+  if (n_tracks > 0 && (!x || !y || !z || !tx || !ty || !var_x || !var_y || !var_tx || !var_ty || !trk_weight || !trk_vertex))
+    return PV_E_NULL;
+  if (workspace_bytes < WORKSPACE_BYTES) return PV_E_WORKSPACE;
+  cudaStream_t stream = (cudaStream_t)stream_;
+
+  std::lock_guard<std::mutex> lock(g_mu);
+  DeviceInfo* di = nullptr;
+  rc = get_device_info(&di);
+  if (rc != PV_OK) return rc;
+
+  pvk::KParams kp;
+  make_kparams(params, nbins, &kp);
+  int warps = di->max_smem_optin / kp.warp_smem_bytes;
+  if (warps > 16) warps = 16;
+  if (const char* envw = getenv("PV_WARPS_PER_CTA")) {
+    const int w = atoi(envw);
+    if (w >= 1 && w < warps) warps = w;
+  }
+  if (warps < 1) return PV_E_PARAM;
+  const int smem = warps * kp.warp_smem_bytes;
+  const int which = dbg ? 1 : 0;
+  if (!di->attr_set[which] || di->attr_smem[which] < smem) {
+    if (which) CK(cudaFuncSetAttribute(pvk::pv_find_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    else CK(cudaFuncSetAttribute(pvk::pv_find_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    di->attr_set[which] = true;
+    di->attr_smem[which] = smem;
+  }
+  g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * 32; g_last_smem = smem;
+  if (n_events == 0) return PV_OK;
+
+  pvk::KArgs ka;
+  memset(&ka, 0, sizeof(ka));
+  ka.x = x; ka.y = y; ka.z = z; ka.tx = tx; ka.ty = ty;
+  ka.var_x = var_x; ka.var_y = var_y; ka.var_tx = var_tx; ka.var_ty = var_ty;
+  ka.offsets = offsets; ka.n_events = n_events;
+  ka.vtx_pos = vtx_pos; ka.vtx_cov = vtx_cov; ka.vtx_chi2 = vtx_chi2;
+  ka.vtx_ntracks = vtx_ntracks; ka.vtx_niter = vtx_niter; ka.n_vtx = n_vtx;
+  ka.trk_weight = trk_weight; ka.trk_vertex = trk_vertex; ka.event_status = event_status;
+  ka.counter = reinterpret_cast<unsigned int*>(workspace);
+  if (dbg) ka.dbg = *dbg;
+
+  CK(cudaMemsetAsync(workspace, 0, 16, stream));
+  int grid = di->sms;
+  const int need = (n_events + warps - 1) / warps;
+  if (grid > need) grid = need;
+  if (g_timing) {
+    if (!g_ev0) { CK(cudaEventCreate(&g_ev0)); CK(cudaEventCreate(&g_ev1)); }
+    CK(cudaEventRecord(g_ev0, stream));
+  }
+  if (dbg) pvk::pv_find_kernel<true><<<grid, warps * 32, smem, stream>>>(kp, ka);
+  else pvk::pv_find_kernel<false><<<grid, warps * 32, smem, stream>>>(kp, ka);
+  CK(cudaGetLastError());
+  if (g_timing) { CK(cudaEventRecord(g_ev1, stream)); g_ev_valid = true; }
+  g_last_kernels = 1; g_last_grid = grid;
+  return PV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pv_params_default(pv_params* p) {
+  if (!p) return PV_E_NULL;
+  p->z_min = -550.0f; p->z_max = 300.0f; p->dz = 0.25f;
+  p->z_split = -300.0f;                                             /* Table 2 */
+  p->beam_x = p->beam_y = p->beam_tx = p->beam_ty = 0.0f;
+  p->max_sigma_poca[0] = 1.5f; p->max_sigma_poca[1] = 10.0f;
+  p->min_bin_content = 0.25f; p->min_dip = 0.75f;                   /* reading R-4 */
+  p->min_cluster_integral[0] = 2.5f; p->min_cluster_integral[1] = 1.75f;  /* Table 2 */
+  p->min_tracks_seed[0] = 3; p->min_tracks_seed[1] = 2;
+  p->min_tracks_pv[0] = 4; p->min_tracks_pv[1] = 3;                 /* Table 2 */
+  p->chi2_max = 12.0f;
+  p->max_iter = 10; p->conv_dchi2 = 0.01f; p->conv_dz = 0.001f;
+  p->merge_ratio = 25.0f;
+  p->max_beam_dist = 0.3f;
+  p->max_vtx_per_event = 32;
+  return PV_OK;
+}
+
+int pv_nbins(const pv_params* p) {
+  int nb = 0;
+  const int rc = validate(p, &nb);
+  return rc == PV_OK ? nb : rc;
+}
+
+int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, size_t* bytes) {
+  if (!bytes) return PV_E_NULL;
+  const int rc = validate(p, nullptr);
+  if (rc != PV_OK) return rc;
+  if (n_events < 0 || n_tracks < 0) return PV_E_SIZE;
+  *bytes = WORKSPACE_BYTES;
+  return PV_OK;
+}
+
+int pv_find(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+            const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+            const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+            float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+            int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+            void* workspace, size_t workspace_bytes, void* stream) {
+  return find_impl(x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, offsets, n_events, n_tracks, params, vtx_pos, vtx_cov,
+                   vtx_chi2, vtx_ntracks, vtx_niter, n_vtx, trk_weight, trk_vertex, event_status, workspace,
+                   workspace_bytes, stream, nullptr);
+}
+
+int pv_find_debug(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                  const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                  const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                  float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                  int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+                  void* workspace, size_t workspace_bytes, void* stream, const pv_debug* dbg) {
+  pv_debug none;
+  memset(&none, 0, sizeof(none));
+  return find_impl(x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, offsets, n_events, n_tracks, params, vtx_pos, vtx_cov,
+                   vtx_chi2, vtx_ntracks, vtx_niter, n_vtx, trk_weight, trk_vertex, event_status, workspace,
+                   workspace_bytes, stream, dbg ? dbg : &none);
+}
+
+/* ------------------------------------------- host-buffer pipeline ------------------------------------------- */
+struct pv_host_ctx {
+  int max_events = 0;
+  long long max_tracks = 0;
+  int max_vtx = 0;
+  int n_streams = 0;
+  std::vector<cudaStream_t> streams;
+  float* d_in[9] = {nullptr};
+  int32_t* d_off = nullptr;
+  float *d_pos = nullptr, *d_cov = nullptr, *d_chi2 = nullptr, *d_w = nullptr;
+  int32_t *d_ntrk = nullptr, *d_niter = nullptr, *d_nvtx = nullptr, *d_tv = nullptr;
+  uint32_t* d_status = nullptr;
+  unsigned char* d_ws = nullptr;   // n_streams * WORKSPACE_BYTES
+};
+
+int pv_host_ctx_destroy(pv_host_ctx* c) {
+  if (!c) return PV_E_NULL;
+  for (auto s : c->streams) cudaStreamDestroy(s);
+  for (int i = 0; i < 9; ++i) cudaFree(c->d_in[i]);
+  cudaFree(c->d_off); cudaFree(c->d_pos); cudaFree(c->d_cov); cudaFree(c->d_chi2); cudaFree(c->d_w);
+  cudaFree(c->d_ntrk); cudaFree(c->d_niter); cudaFree(c->d_nvtx); cudaFree(c->d_tv); cudaFree(c->d_status);
+  cudaFree(c->d_ws);
+  delete c;
+  return PV_OK;
+}
+
+int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, const pv_params* params, int n_streams) {
+  if (!out) return PV_E_NULL;
+  *out = nullptr;
+  const int rc = validate(params, nullptr);
+  if (rc != PV_OK) return rc;
+  if (max_events < 1 || max_tracks < 0 || max_tracks > 0x7fffffffLL || n_streams < 1 || n_streams > 16) return PV_E_SIZE;
+  pv_host_ctx* c = new pv_host_ctx();
+  c->max_events = max_events; c->max_tracks = max_tracks; c->max_vtx = params->max_vtx_per_event; c->n_streams = n_streams;
+  const size_t T = (size_t)(max_tracks > 0 ? max_tracks : 1), E = (size_t)max_events, mv = (size_t)c->max_vtx;
+  cudaError_t err = cudaSuccess;
+  auto A = [&](void** p, size_t bytes) { if (err == cudaSuccess) err = cudaMalloc(p, bytes); };
+  for (int i = 0; i < 9; ++i) A((void**)&c->d_in[i], T * 4);
+  A((void**)&c->d_off, (E + 1) * 4);
+  A((void**)&c->d_pos, E * mv * 12); A((void**)&c->d_cov, E * mv * 24); A((void**)&c->d_chi2, E * mv * 4);
+  A((void**)&c->d_ntrk, E * mv * 4); A((void**)&c->d_niter, E * mv * 4); A((void**)&c->d_nvtx, E * 4);
+  A((void**)&c->d_w, T * 4); A((void**)&c->d_tv, T * 4); A((void**)&c->d_status, E * 4);
+  A((void**)&c->d_ws, (size_t)n_streams * WORKSPACE_BYTES);
+  for (int i = 0; i < n_streams && err == cudaSuccess; ++i) {
+    cudaStream_t s = nullptr;
+    err = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+    if (err == cudaSuccess) c->streams.push_back(s);
+  }
+  if (err != cudaSuccess) {
+    pv_host_ctx_destroy(c);
+    return cuda_fail(err, "pv_host_ctx_create");
+  }
+  *out = c;
+  return PV_OK;
+}
+
+int pv_find_host(pv_host_ctx* c,
+                 const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                 const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                 const int32_t* offsets, int n_events, const pv_params* params,
+                 float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                 int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status, int n_chunks) {
+  if (!c || !offsets || !params) return PV_E_NULL;
+  if (n_events < 0 || n_events > c->max_events) return PV_E_SIZE;
+  if (params->max_vtx_per_event != c->max_vtx) return PV_E_PARAM;
+  if (n_events == 0) return PV_OK;
+  const long long T = offsets[n_events];
+  if (offsets[0] != 0 || T < 0 || T > c->max_tracks) return PV_E_SIZE;
+  if (n_chunks < 1) n_chunks = 1;
+  if (n_chunks > n_events) n_chunks = n_events;
+  const float* h_in[9] = {x, y, z, tx, ty, var_x, var_y, var_tx, var_ty};
+  const size_t mv = (size_t)c->max_vtx;
+  // chunk boundaries: equal track counts (events are contiguous in the SoA arrays)
+  std::vector<int> eb(n_chunks + 1, 0);
+  eb[n_chunks] = n_events;
+  for (int k = 1, e = 0; k < n_chunks; ++k) {
+    const long long target = T * k / n_chunks;
+    while (e < n_events && offsets[e] < target) ++e;
+    eb[k] = e < eb[k - 1] ? eb[k - 1] : e;
+  }
+  int rc = PV_OK;
+  for (int k = 0; k < n_chunks && rc == PV_OK; ++k) {
+    const int e0 = eb[k], e1 = eb[k + 1];
+    if (e1 <= e0) continue;
+    cudaStream_t s = c->streams[k % c->n_streams];
+    const size_t t0 = (size_t)offsets[e0], nt = (size_t)offsets[e1] - t0, ne = (size_t)(e1 - e0);
+    // offsets stay absolute: the kernel indexes the un-shifted SoA base pointers
+    CK(cudaMemcpyAsync(c->d_off + e0, offsets + e0, (ne + 1) * 4, cudaMemcpyHostToDevice, s));
+    if (nt > 0)
+      for (int i = 0; i < 9; ++i) CK(cudaMemcpyAsync(c->d_in[i] + t0, h_in[i] + t0, nt * 4, cudaMemcpyHostToDevice, s));
+    rc = find_impl(c->d_in[0], c->d_in[1], c->d_in[2], c->d_in[3], c->d_in[4], c->d_in[5], c->d_in[6], c->d_in[7], c->d_in[8],
+                   c->d_off + e0, (int)ne, (long long)c->max_tracks, params, c->d_pos + e0 * mv * 3, c->d_cov + e0 * mv * 6,
+                   c->d_chi2 + e0 * mv, c->d_ntrk + e0 * mv, c->d_niter + e0 * mv, c->d_nvtx + e0, c->d_w, c->d_tv,
+                   c->d_status + e0, c->d_ws + (size_t)(k % c->n_streams) * WORKSPACE_BYTES, WORKSPACE_BYTES, s, nullptr);
+    if (rc != PV_OK) break;
+    CK(cudaMemcpyAsync(vtx_pos + e0 * mv * 3, c->d_pos + e0 * mv * 3, ne * mv * 12, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(vtx_cov + e0 * mv * 6, c->d_cov + e0 * mv * 6, ne * mv * 24, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(vtx_chi2 + e0 * mv, c->d_chi2 + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(vtx_ntracks + e0 * mv, c->d_ntrk + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(vtx_niter + e0 * mv, c->d_niter + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(n_vtx + e0, c->d_nvtx + e0, ne * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(event_status + e0, c->d_status + e0, ne * 4, cudaMemcpyDeviceToHost, s));
+    if (nt > 0) {
+      CK(cudaMemcpyAsync(trk_weight + t0, c->d_w + t0, nt * 4, cudaMemcpyDeviceToHost, s));
+      CK(cudaMemcpyAsync(trk_vertex + t0, c->d_tv + t0, nt * 4, cudaMemcpyDeviceToHost, s));
+    }
+  }
+  for (auto s : c->streams) {
+    cudaError_t err = cudaStreamSynchronize(s);
+    if (err != cudaSuccess && rc == PV_OK) rc = cuda_fail(err, "cudaStreamSynchronize");
+  }
+  return rc;
+}
+
+int pv_host_register(void* ptr, size_t bytes) {
+  if (!ptr) return PV_E_NULL;
+  if (bytes == 0) return PV_OK;
+  CK(cudaHostRegister(ptr, bytes, cudaHostRegisterDefault));
+  return PV_OK;
+}
+
+int pv_host_unregister(void* ptr) {
+  if (!ptr) return PV_E_NULL;
+  CK(cudaHostUnregister(ptr));
+  return PV_OK;
+}
+
+int pv_last_launch_info(int* n_kernels, int* grid, int* block, int* smem_bytes) {
+  if (n_kernels) *n_kernels = g_last_kernels;
+  if (grid) *grid = g_last_grid;
+  if (block) *block = g_last_block;
+  if (smem_bytes) *smem_bytes = g_last_smem;
+  return PV_OK;
+}
+
+int pv_kernel_timing(int enable) {
+  g_timing = enable ? 1 : 0;
+  if (!enable) g_ev_valid = false;
+  return PV_OK;
+}
+
+float pv_kernel_time_ms(void) {
+  if (!g_ev_valid || !g_ev0 || !g_ev1) return -1.0f;
+  if (cudaEventSynchronize(g_ev1) != cudaSuccess) return -1.0f;
+  float ms = -1.0f;
+  if (cudaEventElapsedTime(&ms, g_ev0, g_ev1) != cudaSuccess) return -1.0f;
+  return ms;
+}
+
+const char* pv_error_string(int code) {
+  switch (code) {
+    case PV_OK: return "ok";
+    case PV_E_NULL: return "a required pointer is NULL";
+    case PV_E_PARAM: return "invalid parameter";
+    case PV_E_WORKSPACE: return "workspace too small";
+    case PV_E_CUDA: return "CUDA error (see pv_last_cuda_error)";
+    case PV_E_SIZE: return "invalid size or capacity exceeded";
+    default: return "unknown error code";
+  }
+}
+
+const char* pv_last_cuda_error(void) { return g_cuda_err; }
+
+}  // extern "C"

@@ -1,0 +1,184 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+All tests here need a B200 (`-m gpu`)."""
+import numpy as np
+import pytest
+
+from synth import events
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pv():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2412_14966_b200 import build as pvbuild
+    pvbuild.build()
+    import paper_2412_14966_b200 as pv
+    return pv
+
+
+def _both(pv, oracle, data, n_hist=None, **over):
+    from oracle import compare
+    p = pv.default_params(**over)
+    po = oracle.default_params(**over)
+    E = data["offsets"].size - 1
+    nh = E if n_hist is None else min(n_hist, E)
+    got = pv.find(data, p, debug=True, n_hist_events=nh)
+    ref = oracle.find(data, po, debug=True, n_hist_events=nh, trace=True, n_threads=8)
+    rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
+    return got, ref, rep
+
+
+def _assert_parity(rep, allow_ties_frac=0.01):
+    assert not rep["failures"], "\n".join(rep["failures"][:10])
+    for t in rep["near_ties"][:10]:
+        print("LOGGED", t)
+    nfit = max(rep.get("n_fitted_seeds", 1), 1)
+    assert rep["n_near_ties"] <= max(2, allow_ties_frac * nfit), (rep["n_near_ties"], nfit)
+
+
+def test_config0_every_tap(pv, oracle, cfg0):
+    """configs[0]: 1000 events; bit-exact projection, histograms (all 1000), seeds, assignment; fit within
+    1e-3 mm / 1e-3 rel; identical vertex counts."""
+    got, ref, rep = _both(pv, oracle, cfg0)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep)
+    assert rep["hist_mismatch"] == 0 and rep["seed_z_mismatch"] == 0 and rep["trk_seed_mismatch"] == 0
+    assert rep["n_vertices"] > 4000
+    assert rep["assign_agreement"] >= 0.999
+
+
+@pytest.mark.parametrize("idx,n", [(1, 3000), (2, 1500), (3, 3000)])
+def test_config_slices(pv, oracle, idx, n):
+    """The first n events of configs[1..3] (SMOG2 region, high pile-up, close pairs)."""
+    data = events.generate(events.config(idx, n))
+    got, ref, rep = _both(pv, oracle, data, n_hist=300)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep)
+    if idx == 1:
+        assert (ref["vtx_pos"][..., 2][np.arange(32)[None, :] < ref["n_vtx"][:, None]] < -300).sum() > 100   # p-gas PVs present
+
+
+def test_empty_and_degenerate_events(pv, oracle):
+    """Empty batch, events without tracks, single-track events, tracks parallel to the beamline, NaN / zero
+    variances, tracks outside the histogram range."""
+    got = pv.find(dict(events.from_lists([])))
+    assert got["n_vtx"].size == 0
+    rng = np.random.default_rng(5)
+    base = events.generate(events.config(0, 6))
+    evs = []
+    off = base["offsets"]
+    for e in range(6):
+        evs.append({k: base[k][off[e]:off[e + 1]].copy() for k in events.FIELDS})
+    empty = {k: np.zeros(0, np.float32) for k in events.FIELDS}
+    one = {k: v[:1] for k, v in evs[0].items()}
+    par = {k: v.copy() for k, v in evs[1].items()}
+    par["tx"][:5] = 0.0; par["ty"][:5] = 0.0                     # parallel to the beamline: invalid
+    par["var_x"][5:8] = 0.0                                      # sigma_poca = 0: not histogrammed
+    par["var_x"][8:10] = np.nan
+    par["var_y"][10:12] = -1.0                                   # unusable in the fit
+    far = {k: v.copy() for k, v in evs[2].items()}
+    far["z"][:10] += 5000.0                                      # out of the histogram range
+    far["x"][10:14] = 50.0                                       # far from the beamline
+    lst = [empty, evs[0], empty, one, par, far, evs[3], empty]
+    data = events.from_lists(lst)
+    got, ref, rep = _both(pv, oracle, data)
+    _assert_parity(rep)
+    assert list(got["n_vtx"][[0, 2, 3, 7]]) == [0, 0, 0, 0]
+
+
+def test_too_many_tracks_and_vertex_overflow(pv, oracle):
+    """An event above PV_MAX_TRACKS_PER_EVENT is skipped with its flag; max_vtx_per_event smaller than the
+    number of seeds keeps the first ones in z and flags the event."""
+    big = events.generate(events.config(2, 40))
+    n = int(big["offsets"][-1])
+    assert n > 2047
+    huge = {k: big[k][:2200] for k in events.FIELDS}
+    exact = {k: big[k][:2047] for k in events.FIELDS}
+    small = events.generate(events.config(0, 3))
+    so = small["offsets"]
+    lst = [huge, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, exact, {k: small[k][so[1]:so[2]] for k in events.FIELDS}]
+    data = events.from_lists(lst)
+    got, ref, rep = _both(pv, oracle, data, max_vtx_per_event=32)
+    _assert_parity(rep, allow_ties_frac=0.05)
+    assert got["event_status"][0] & 1 and got["n_vtx"][0] == 0
+    assert np.all(got["trk_vertex"][:2200] == -1) and np.all(got["trk_weight"][:2200] == 0)
+    assert got["n_vtx"][2] > 10                                   # 2047 tracks of 40 merged pile-up events
+    got, ref, rep = _both(pv, oracle, events.generate(events.config(2, 300)), max_vtx_per_event=4)
+    _assert_parity(rep, allow_ties_frac=0.05)
+    assert (got["event_status"] & 2).sum() > 100 and np.array_equal(got["event_status"] & 2, ref["event_status"] & 2)
+
+
+def test_other_parameters(pv, oracle):
+    """Displaced and tilted beamline, unit weights (chi2_max = inf), another binning, tighter
+    convergence: the parameters travel through the ABI and both sides agree."""
+    data = events.generate(events.config(1, 800))
+    d2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in data.items()}
+    d2["x"] = (d2["x"] + 0.8 + 1e-3 * d2["z"]).astype(np.float32)
+    d2["y"] = (d2["y"] - 0.4 - 5e-4 * d2["z"]).astype(np.float32)
+    _, _, rep = _both(pv, oracle, d2, n_hist=100, beam_x=0.8, beam_y=-0.4, beam_tx=1e-3, beam_ty=-5e-4)
+    _assert_parity(rep)
+    assert rep["n_vertices"] > 3000
+    _, _, rep = _both(pv, oracle, data, n_hist=100, chi2_max=np.inf)
+    _assert_parity(rep)
+    _, _, rep = _both(pv, oracle, data, n_hist=100, dz=0.5, min_dip=0.5, min_bin_content=0.4)
+    _assert_parity(rep)
+    _, _, rep = _both(pv, oracle, data, n_hist=100, conv_dz=1e-4, conv_dchi2=1e-3, max_iter=16, merge_ratio=9.0)
+    _assert_parity(rep, allow_ties_frac=0.03)
+
+
+def test_runs_are_reproducible(pv, cfg0):
+    """Integer histograms and a fixed summation order: two runs give bit-identical outputs."""
+    a = pv.find(cfg0)
+    b = pv.find(cfg0)
+    for k in a:
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+
+
+def test_full_size_throughput_config(pv, oracle):
+    """configs[1] at its full size (100 000 events), non-debug kernel, the launch configuration bench.py times;
+    the oracle (8 threads) is compared on every final output."""
+    from oracle import compare
+    data = events.generate(events.config(1))
+    p = pv.default_params()
+    got = pv.find(data, p)
+    info = pv.last_launch_info()
+    assert info["n_kernels"] == 1 and info["grid"] >= 100
+    ref = oracle.find(data, oracle.default_params(), debug=True, trace=True, n_threads=8)
+    ref_nodebug = {k: v for k, v in ref.items() if k != "debug"}
+    rep = compare.compare(got, ref_nodebug, data["offsets"], p)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    # without the taps the comparator cannot explain iteration near-ties: bound them instead
+    hard = [f for f in rep["failures"] if "position off" not in f and "covariance off" not in f and "weights off" not in f
+            and "n_vtx differs" not in f and "mismatches outside" not in f]
+    assert not hard, hard[:5]
+    assert rep["n_vtx_mismatch_events"] <= 20
+    assert rep["assign_agreement"] >= 0.999
+    nv = np.arange(32)[None, :] < np.minimum(got["n_vtx"], ref["n_vtx"])[:, None]
+    same = (got["n_vtx"] == ref["n_vtx"])[:, None] & nv
+    d = np.abs(got["vtx_pos"].astype(np.float64) - ref["vtx_pos"]).max(axis=-1)[same]
+    assert (d > 1e-3).mean() < 2e-3, (d > 1e-3).mean()            # iteration near-ties only, < 0.2 %
+    assert np.quantile(d, 0.99) < 1e-4
+
+
+def test_host_pipeline_matches_device_path(pv, cfg0):
+    """pv_find_host (HOST buffers, chunked over streams) returns exactly what pv_find returns."""
+    p = pv.default_params()
+    a = pv.find(cfg0, p)
+    E, T = cfg0["offsets"].size - 1, int(cfg0["offsets"][-1])
+    hp = pv.HostPipeline(E, T, p, n_streams=3)
+    data = hp.pin_inputs(cfg0)
+    out = hp.alloc_outputs(E, T)
+    for chunks in (1, 5):
+        for v in out.values():
+            v[...] = 0
+        hp.find(data, out, n_chunks=chunks)
+        for k in a:
+            nv = a["n_vtx"]
+            if k.startswith("vtx_"):
+                m = np.arange(p.max_vtx_per_event)[None, :] < nv[:, None]
+                assert np.array_equal(out[k][m], a[k][m]), (k, chunks)
+            else:
+                assert np.array_equal(out[k].view(a[k].dtype), a[k]), (k, chunks)
+    hp.close()
