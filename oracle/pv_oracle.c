@@ -303,6 +303,65 @@ static void chol3_solve(const double L[3][3], const double b[3], double x[3]) {
   }
 }
 
+/* One Newton-Raphson iteration (Eq. 6-17) at the vertex position a[]: fills the Tukey weights w[] (Eq. 18),
+ * the step (Eq. 13), C (Eq. 14), dchi2 (Eq. 17), chi2 (Eq. 6) and the number of tracks with w > 0.
+ * Returns -1 when fewer than 2 tracks are active or the Hessian is not positive definite. */
+static int fit_iteration(int m, const int32_t *idx,
+                         const float *x, const float *y, const float *z, const float *tx, const float *ty,
+                         const double *Wx, const double *Wy, const double a[3], double chi2_max,
+                         double *w, double step[3], double C[3][3], double *dchi2_o, double *chi2_o, int *nact_o) {
+  double A[3][3] = {{0}}, g[3] = {0, 0, 0};
+  double chi2 = 0.0;
+  int nact = 0;
+  for (int j = 0; j < m; ++j) {
+    int i = idx[j];
+    double wi = 0.0;
+    if (Wx[j] > 0.0) {
+      /* residual Eq. 9 */
+      double rx = (double)x[i] + (a[2] - (double)z[i]) * (double)tx[i] - a[0];
+      double ry = (double)y[i] + (a[2] - (double)z[i]) * (double)ty[i] - a[1];
+      double chi2_i = rx * rx * Wx[j] + ry * ry * Wy[j];            /* Eq. 7 */
+      if (isinf(chi2_max)) wi = 1.0;
+      else if (chi2_i < chi2_max) { double u = 1.0 - chi2_i / chi2_max; wi = u * u; }  /* Eq. 18 */
+      /* H_i = [[-1,0,tx],[0,-1,ty]] (Eq. 12); accumulate w H^T W H (Eq. 11 / 2) and w H^T W r (Eq. 10 / 2) */
+      double Hm[2][3] = {{-1.0, 0.0, (double)tx[i]}, {0.0, -1.0, (double)ty[i]}};
+      double Wd[2] = {Wx[j], Wy[j]}, r[2] = {rx, ry};
+      for (int c = 0; c < 2; ++c)
+        for (int k = 0; k < 3; ++k) {
+          g[k] += wi * Hm[c][k] * Wd[c] * r[c];
+          for (int l = 0; l < 3; ++l) A[k][l] += wi * Hm[c][k] * Wd[c] * Hm[c][l];
+        }
+      chi2 += wi * chi2_i;                                          /* Eq. 6 */
+    }
+    w[j] = wi;
+    if (wi > 0.0) ++nact;
+  }
+  *chi2_o = chi2; *nact_o = nact;
+  if (nact < 2) return -1;
+  double L[3][3];
+  if (chol3(A, L) != 0) return -1;
+  /* Newton-Raphson step Eq. 13: alpha1 = alpha0 - (d2chi2)^-1 dchi2 = alpha0 - A^-1 g */
+  double mg[3] = {-g[0], -g[1], -g[2]};
+  chol3_solve(L, mg, step);
+  /* covariance Eq. 14: C = A^-1, column by column */
+  for (int k = 0; k < 3; ++k) {
+    double ek[3] = {0, 0, 0}, col[3];
+    ek[k] = 1.0;
+    chol3_solve(L, ek, col);
+    for (int l = 0; l < 3; ++l) C[l][k] = col[l];
+  }
+  /* Eq. 17: dchi2 = 1/2 (alpha1 - alpha0) . dchi2/dalpha = step . g */
+  *dchi2_o = step[0] * g[0] + step[1] * g[1] + step[2] * g[2];
+  return 0;
+}
+
+static void trace_row(double *trace, int it, const double a[3], double C[3][3], double dchi2, double dz) {
+  double *t = trace + (size_t)(it - 1) * PVO_TRACE_STRIDE;
+  t[0] = a[0]; t[1] = a[1]; t[2] = a[2];
+  t[3] = C[0][0]; t[4] = C[0][1]; t[5] = C[0][2]; t[6] = C[1][1]; t[7] = C[1][2]; t[8] = C[2][2];
+  t[9] = dchi2; t[10] = dz;
+}
+
 int pvo_fit(int m, const int32_t *idx,
             const float *x, const float *y, const float *z, const float *tx, const float *ty,
             const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
@@ -327,56 +386,26 @@ int pvo_fit(int m, const int32_t *idx,
   int rc = -1, niter = 0, nact = 0;
   double C[3][3] = {{0}}, chi2 = 0.0;
   for (int it = 1; it <= p->max_iter; ++it) {
-    double A[3][3] = {{0}}, g[3] = {0, 0, 0};
-    chi2 = 0.0; nact = 0;
-    for (int j = 0; j < m; ++j) {
-      int i = idx[j];
-      double wi = 0.0;
-      if (Wx[j] > 0.0) {
-        /* residual Eq. 9 */
-        double rx = (double)x[i] + (a[2] - (double)z[i]) * (double)tx[i] - a[0];
-        double ry = (double)y[i] + (a[2] - (double)z[i]) * (double)ty[i] - a[1];
-        double chi2_i = rx * rx * Wx[j] + ry * ry * Wy[j];            /* Eq. 7 */
-        if (isinf(chi2_max)) wi = 1.0;
-        else if (chi2_i < chi2_max) { double u = 1.0 - chi2_i / chi2_max; wi = u * u; }  /* Eq. 18 */
-        /* H_i = [[-1,0,tx],[0,-1,ty]] (Eq. 12); accumulate w H^T W H (Eq. 11 / 2) and w H^T W r (Eq. 10 / 2) */
-        double Hm[2][3] = {{-1.0, 0.0, (double)tx[i]}, {0.0, -1.0, (double)ty[i]}};
-        double Wd[2] = {Wx[j], Wy[j]}, r[2] = {rx, ry};
-        for (int c = 0; c < 2; ++c)
-          for (int k = 0; k < 3; ++k) {
-            g[k] += wi * Hm[c][k] * Wd[c] * r[c];
-            for (int l = 0; l < 3; ++l) A[k][l] += wi * Hm[c][k] * Wd[c] * Hm[c][l];
-          }
-        chi2 += wi * chi2_i;                                          /* Eq. 6 */
-      }
-      w[j] = wi;
-      if (wi > 0.0) ++nact;
-    }
-    if (nact < 2) { rc = -1; break; }
-    double L[3][3];
-    if (chol3(A, L) != 0) { rc = -1; break; }
-    /* Newton-Raphson step Eq. 13: alpha1 = alpha0 - (d2chi2)^-1 dchi2 = alpha0 - A^-1 g */
-    double step[3], mg[3] = {-g[0], -g[1], -g[2]};
-    chol3_solve(L, mg, step);
-    /* covariance Eq. 14: C = A^-1, column by column */
-    for (int k = 0; k < 3; ++k) {
-      double ek[3] = {0, 0, 0}, col[3];
-      ek[k] = 1.0;
-      chol3_solve(L, ek, col);
-      for (int l = 0; l < 3; ++l) C[l][k] = col[l];
-    }
-    /* Eq. 17: dchi2 = 1/2 (alpha1 - alpha0) . dchi2/dalpha = step . g */
-    double dchi2 = step[0] * g[0] + step[1] * g[1] + step[2] * g[2];
+    double step[3], dchi2;
+    if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, a, chi2_max, w, step, C, &dchi2, &chi2, &nact) != 0) { rc = -1; break; }
     for (int k = 0; k < 3; ++k) a[k] += step[k];
     niter = it; rc = 0;
-    if (trace && it <= PVO_TRACE_ITERS) {
-      double *t = trace + (size_t)(it - 1) * PVO_TRACE_STRIDE;
-      t[0] = a[0]; t[1] = a[1]; t[2] = a[2];
-      t[3] = C[0][0]; t[4] = C[0][1]; t[5] = C[0][2]; t[6] = C[1][1]; t[7] = C[1][2]; t[8] = C[2][2];
-      t[9] = dchi2; t[10] = step[2];
-    }
+    if (trace && it <= PVO_TRACE_ITERS) trace_row(trace, it, a, C, dchi2, step[2]);
     /* convergence (x86 flavour) */
     if (fabs(dchi2) < (double)p->conv_dchi2 && fabs(step[2]) < (double)p->conv_dz) break;
+  }
+  /* Trace only (N1): keep iterating past the stopping point on COPIES, so that a
+   * comparator can look up what one more iteration would have given.  Nothing below changes an output. */
+  if (trace && rc == 0 && niter < p->max_iter) {
+    double at[3] = {a[0], a[1], a[2]}, Ct[3][3], chi2t, dchi2t, stept[3];
+    int nactt;
+    double *wt = (double *)malloc(sizeof(double) * (size_t)(m + 1));
+    for (int it = niter + 1; it <= p->max_iter && it <= PVO_TRACE_ITERS; ++it) {
+      if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, at, chi2_max, wt, stept, Ct, &dchi2t, &chi2t, &nactt) != 0) break;
+      for (int k = 0; k < 3; ++k) at[k] += stept[k];
+      trace_row(trace, it, at, Ct, dchi2t, stept[2]);
+    }
+    free(wt);
   }
   free(Wx);
   if (rc != 0) { *out_niter = -1; *out_ntrk = 0; return -1; }

@@ -267,10 +267,9 @@ __device__ __forceinline__ void covariance(const Sums& S, float* C) {
 }
 
 // W = V^-1 "evaluated and inverted only once, using the vertex position of the seed", Eq. 2 diagonal.
-__device__ __forceinline__ void track_weight_matrix(float zseed, float z, float vx, float vy, float vtx, float vty,
+__device__ __forceinline__ void track_weight_matrix(float zl, float vx, float vy, float vtx, float vty,
                                                     float& Wx, float& Wy) {
-  const float dz = zseed - z;
-  const float dz2 = dz * dz;
+  const float dz2 = zl * zl;                               // zl = z_trk - z_seed
   const float Vx = fmaf(dz2, vtx, vx), Vy = fmaf(dz2, vty, vy);
   const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);
   Wx = ok ? 1.0f / Vx : -1.0f;
@@ -520,9 +519,11 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
     const bool big = m > FIT_G * FIT_KF;
     if (big) m = 0;
     const float zsv = vact ? zs[v] : 0.0f;
-    float ax = __fmaf_rn(P.beam_tx, zsv, P.beam_x);       // "xy position ... using the known beamline"
-    float ay = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-    float az = zsv;
+    const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
+    const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+    // The fit runs in the seed's local frame (x - sx, y - sy, z - zseed): every quantity is O(mm), so fp32
+    // keeps ~1e-7 mm instead of ulp(550 mm) = 6e-5 mm, and the iterates follow the fp64 oracle.
+    float ax = 0.0f, ay = 0.0f, az = 0.0f;
     float fx[FIT_KF], fy[FIT_KF], fz[FIT_KF], ftx[FIT_KF], fty[FIT_KF], fWx[FIT_KF], fWy[FIT_KF], fw[FIT_KF];
 #pragma unroll
     for (int s = 0; s < FIT_KF; ++s) {
@@ -531,9 +532,9 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
       fx[s] = fy[s] = fz[s] = ftx[s] = fty[s] = 0.0f;
       if (t < m) {
         const int g = t0 + (int)sidx[o + t];
-        fx[s] = __ldg(A.x + g); fy[s] = __ldg(A.y + g); fz[s] = __ldg(A.z + g);
+        fx[s] = __ldg(A.x + g) - sx; fy[s] = __ldg(A.y + g) - sy; fz[s] = __ldg(A.z + g) - zsv;
         ftx[s] = __ldg(A.tx + g); fty[s] = __ldg(A.ty + g);
-        track_weight_matrix(zsv, fz[s], __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g),
+        track_weight_matrix(fz[s], __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g),
                             __ldg(A.var_ty + g), fWx[s], fWy[s]);
       }
     }
@@ -571,7 +572,7 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
         if (j == 0) {
           float C[6];
           covariance(L, C);
-          V[0 * MAXV + v] = ax; V[1 * MAXV + v] = ay; V[2 * MAXV + v] = az;
+          V[0 * MAXV + v] = sx + ax; V[1 * MAXV + v] = sy + ay; V[2 * MAXV + v] = zsv + az;
 #pragma unroll
           for (int c = 0; c < 6; ++c) V[(3 + c) * MAXV + v] = C[c];
           V[9 * MAXV + v] = L.chi2;
@@ -593,7 +594,8 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
     if (m <= FIT_G * FIT_KF) continue;
     const int o = off[v];
     const float zsv = zs[v];
-    float ax = __fmaf_rn(P.beam_tx, zsv, P.beam_x), ay = __fmaf_rn(P.beam_ty, zsv, P.beam_y), az = zsv;
+    const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+    float ax = 0.0f, ay = 0.0f, az = 0.0f;                 // local frame, as in the fast path
     float px = ax, py = ay, pz = az;                       // vertex position the last weights were taken at
     bool sing = false;
     int niter = 0;
@@ -604,11 +606,10 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
       sums_zero(S);
       for (int t = lane; t < m; t += 32) {
         const int g = t0 + (int)sidx[o + t];
-        const float tz = __ldg(A.z + g);
+        const float zl = __ldg(A.z + g) - zsv;
         float Wx, Wy;
-        track_weight_matrix(zsv, tz, __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g), __ldg(A.var_ty + g),
-                            Wx, Wy);
-        track_accum(__ldg(A.x + g), __ldg(A.y + g), tz, __ldg(A.tx + g), __ldg(A.ty + g), Wx, Wy, ax, ay, az, P, S);
+        track_weight_matrix(zl, __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g), __ldg(A.var_ty + g), Wx, Wy);
+        track_accum(__ldg(A.x + g) - sx, __ldg(A.y + g) - sy, zl, __ldg(A.tx + g), __ldg(A.ty + g), Wx, Wy, ax, ay, az, P, S);
       }
       sums_reduce<32>(S);
       float dx, dy, dzs, dchi2;
@@ -625,7 +626,7 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
       if (lane == 0) {
         float C[6];
         covariance(L, C);
-        V[0 * MAXV + v] = ax; V[1 * MAXV + v] = ay; V[2 * MAXV + v] = az;
+        V[0 * MAXV + v] = sx + ax; V[1 * MAXV + v] = sy + ay; V[2 * MAXV + v] = zsv + az;
         for (int c = 0; c < 6; ++c) V[(3 + c) * MAXV + v] = C[c];
         V[9 * MAXV + v] = L.chi2;
         reinterpret_cast<int*>(V)[10 * MAXV + v] = (int)L.nact;
@@ -633,14 +634,13 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
       }
       for (int t = lane; t < m; t += 32) {                 // weights of the last iteration, recomputed
         const int g = t0 + (int)sidx[o + t];
-        const float tz = __ldg(A.z + g);
+        const float zl = __ldg(A.z + g) - zsv;
         float Wx, Wy;
-        track_weight_matrix(zsv, tz, __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g), __ldg(A.var_ty + g),
-                            Wx, Wy);
+        track_weight_matrix(zl, __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g), __ldg(A.var_ty + g), Wx, Wy);
         Sums dummy;
         sums_zero(dummy);
-        A.trk_weight[g] = track_accum(__ldg(A.x + g), __ldg(A.y + g), tz, __ldg(A.tx + g), __ldg(A.ty + g), Wx, Wy,
-                                      px, py, pz, P, dummy);
+        A.trk_weight[g] = track_accum(__ldg(A.x + g) - sx, __ldg(A.y + g) - sy, zl, __ldg(A.tx + g), __ldg(A.ty + g),
+                                      Wx, Wy, px, py, pz, P, dummy);
       }
     }
   }
