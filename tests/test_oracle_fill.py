@@ -140,3 +140,26 @@ def test_l1_vs_l0_bound_on_events(oracle, cfg0_oracle):
             m += (edges[1:] > a - 10 * b) & (edges[:-1] < a + 10 * b)
         assert np.all(np.abs(H1 - H0) <= m * per_track + 1e-12)
         assert np.abs(H1 - H0).max() < 0.06
+
+
+def test_frozen_cdf_coefficients_are_the_documented_fit(oracle):
+    """The seven fp32 literals of the CDF contract (R-6) are the least-squares fit oracle/fit_cdf_poly.py
+    describes: recompute them from scipy's Phi and compare with the literals in pv_oracle.c bit by bit."""
+    import os
+    import re
+    from oracle import fit_cdf_poly
+    src = open(os.path.join(os.path.dirname(fit_cdf_poly.__file__), "pv_oracle.c")).read()
+    body = re.search(r"PVO_G\[7\]\s*=\s*\{(.*?)\}", src, flags=re.S).group(1)
+    frozen = np.array([float.fromhex(t.strip().rstrip("f")) for t in body.split(",")], dtype=np.float32)
+    assert frozen.size == 7
+    assert np.array_equal(frozen.view(np.uint32), fit_cdf_poly.fit().view(np.uint32))
+    # and the polynomial stays within 1e-5 of its target over the whole support, in fp32 arithmetic
+    s = np.linspace(-1, 1, 20001).astype(np.float32)
+    t = s * s
+    g = np.full_like(s, frozen[6])
+    for j in range(5, -1, -1):
+        g = (g * t + frozen[j]).astype(np.float32)
+    F = (s * g + np.float32(0.5)).astype(np.float64)
+    tail = ndtr(-3.0)
+    assert np.abs(F - (ndtr(3.0 * s.astype(np.float64)) - tail) / (1 - 2 * tail)).max() < 1e-5
+
