@@ -221,7 +221,7 @@ int pvo_peaks(const int32_t *H, const pvo_params *p, int cap, int32_t *begin, in
 }
 
 /* ===================================== O5 : seed position ============================================ */
-/* Eq. 4-5; neighbours are raw histogram bins, 0 beyond the ends (R-5). */
+/* Eq. 4-5; neighbours are raw histogram bins, 0 beyond the ends (R-10). */
 float pvo_seed_z(const int32_t *H, int i, const pvo_params *p) {
   int nbins = pvo_nbins(p);
   int64_t Nm = i > 0 ? H[i - 1] : 0;
@@ -244,7 +244,7 @@ int pvo_assign(int n, const int32_t *bin, const int32_t *flags, int n_seeds,
     for (int i = 0; i < n; ++i) trk_seed[i] = -1;
     if (n_seeds == 0) break;
     /* partition point = "the bin in between of the upper bound of one cluster and the lower bound of
-     * the next cluster"; bins < part[k] belong to seed k, the others to k+1 ... (R-6) */
+     * the next cluster"; bins < part[k] belong to seed k, the others to k+1 ... (R-11) */
     for (int k = 0; k + 1 < n_seeds; ++k) part[k] = (end[k] + begin[k + 1]) / 2;
     for (int k = 0; k < n_seeds; ++k) cnt[k] = 0;
     for (int i = 0; i < n; ++i) {

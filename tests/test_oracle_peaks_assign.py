@@ -81,7 +81,7 @@ def test_peak_invariants_on_events(oracle, cfg0_oracle):
 
 
 def test_assign_partition_points_and_unassignable(oracle):
-    """Partition point = floor((end_k + begin_{k+1}) / 2) (L163, R-6); bins < p -> k, >= p -> k+1."""
+    """Partition point = floor((end_k + begin_{k+1}) / 2) (L163, R-11); bins < p -> k, >= p -> k+1."""
     p = oracle.default_params(min_tracks_seed=(1, 1))
     begin, end, peak = [2100, 2120, 2131], [2110, 2131, 2140], [2105, 2125, 2135]
     zs = [0.0, 1.0, 2.0]
