@@ -82,8 +82,9 @@ int pv_params_default(pv_params* p);
 /* Number of histogram bins implied by p (lrint((z_max - z_min) / dz)), or a negative PV_E_* if p is invalid. */
 int pv_nbins(const pv_params* p);
 
-/* Bytes of DEVICE workspace pv_find needs for a batch of this size (a small constant today; the
- * histograms live in shared memory, "one block per event").  bytes: HOST out. */
+/* Bytes of DEVICE workspace pv_find needs for a batch of this size: 256 B of counters, one 16-byte seed
+ * record per (event, vertex slot) and 2 B per track (track lists sorted by seed) handed from the seed kernel
+ * to the fit kernel.  The histograms live in shared memory ("one block per event").  bytes: HOST out. */
 int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, size_t* bytes);
 
 /* The hot path a1..a6 over a batch.
@@ -101,12 +102,13 @@ int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, siz
  *   vtx_chi2     float[n_events][max_vtx]      sum_i w_i chi2_i of the last iteration (Eq. 6)
  *   vtx_ntracks  int32[n_events][max_vtx]      tracks with w_i > 0 in the last iteration
  *   vtx_niter    int32[n_events][max_vtx]      Newton iterations done
- *   n_vtx        int32[n_events]               PVs found; only the first n_vtx[e] slots of event e are written
+ *   n_vtx        int32[n_events]               PVs found; the first n_vtx[e] slots of event e hold them, the
+ *                                              other slots of the event are scratch (pre-cleanup seeds)
  *   trk_weight   float[T]                      Tukey weight w_i of the last iteration (Eq. 18); 0 if unassigned
  *   trk_vertex   int32[T]                      index of the track's PV within its event, -1 = none
  *   event_status uint32[n_events]              PV_EVT_* flags
  *   (trk_weight / trk_vertex also serve as per-track scratch during the call.)
- * workspace: DEVICE, >= pv_workspace_bytes() bytes, 16-byte aligned; contents are scratch.
+ * workspace: DEVICE, >= pv_workspace_bytes(n_events, n_tracks, params) bytes, 16-byte aligned; scratch.
  * stream: cudaStream_t.
  */
 int pv_find(const float* x, const float* y, const float* z, const float* tx, const float* ty,
@@ -166,14 +168,18 @@ int pv_host_register(void* ptr, size_t bytes);
 int pv_host_unregister(void* ptr);
 
 /* Launch statistics of the most recent pv_find / pv_find_debug call of this process (for bench.py):
- * kernels launched, grid size, block size, dynamic shared memory per block.  All HOST out, nullable. */
+ * kernels launched (3: seed, fit, cleanup), and grid size, block size, dynamic shared memory per block of
+ * the seed kernel.  All HOST out, nullable. */
 int pv_last_launch_info(int* n_kernels, int* grid, int* block, int* smem_bytes);
 
-/* Optional: CUDA events recorded around the kernel of the next pv_find calls on their own stream, so a
- * caller can time the dominant kernel live.  pv_kernel_timing(1) enables, (0) disables;
- * pv_kernel_time_ms() synchronises the last pair and returns its duration in ms (< 0 if none). */
+/* Optional: CUDA events recorded around each kernel of the next pv_find calls on their own stream, so a
+ * caller can time the kernels live.  pv_kernel_timing(1) enables, (0) disables; pv_kernel_time_ms()
+ * synchronises the last call's events and returns the duration of its three kernels in ms (< 0 if none);
+ * pv_kernel_times_ms() writes up to n per-kernel durations (seed a1-a4, fit a5, cleanup a6) to ms (HOST)
+ * and returns the number of kernels (3), or a negative PV_E_*. */
 int pv_kernel_timing(int enable);
 float pv_kernel_time_ms(void);
+int pv_kernel_times_ms(float* ms, int n);
 
 const char* pv_error_string(int code);
 /* Text of the last CUDA error seen by this library in this process ("" if none).  HOST. */

@@ -27,7 +27,7 @@ FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 EXPORTS = (
     "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug",
     "pv_host_ctx_create", "pv_host_ctx_destroy", "pv_find_host", "pv_host_register", "pv_host_unregister",
-    "pv_last_launch_info", "pv_kernel_timing", "pv_kernel_time_ms", "pv_error_string", "pv_last_cuda_error",
+    "pv_last_launch_info", "pv_kernel_timing", "pv_kernel_time_ms", "pv_kernel_times_ms", "pv_error_string", "pv_last_cuda_error",
 )
 
 
@@ -84,6 +84,7 @@ def lib():
         L.pv_last_launch_info.argtypes = [C.POINTER(i32)] * 4
         L.pv_kernel_timing.argtypes = [i32]
         L.pv_kernel_time_ms.restype = C.c_float
+        L.pv_kernel_times_ms.argtypes = [C.POINTER(C.c_float), i32]
         L.pv_error_string.argtypes = [i32]
         L.pv_error_string.restype = C.c_char_p
         L.pv_last_cuda_error.restype = C.c_char_p

@@ -1,5 +1,5 @@
 // pv_api.cu -- host side of the C ABI declared in include/pv_finder.h: parameter validation, conversion of
-// the paper's thresholds to the fixed-point contract, launch of the persistent warp-per-event kernel, and the
+// the paper's thresholds to the fixed-point contract, launch of the three kernels (seed, fit, cleanup), and the
 // host-buffer pipeline.  No CPU fallback exists: without a CUDA device every compute entry returns
 // PV_E_CUDA.
 #include <math.h>
@@ -17,7 +17,8 @@ namespace {
 thread_local char g_cuda_err[512] = "";
 int g_last_kernels = 0, g_last_grid = 0, g_last_block = 0, g_last_smem = 0;
 int g_timing = 0;
-cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+constexpr int N_KERNELS = 3;
+cudaEvent_t g_ev[N_KERNELS + 1] = {nullptr, nullptr, nullptr, nullptr};
 bool g_ev_valid = false;
 
 int cuda_fail(cudaError_t err, const char* what) {
@@ -34,6 +35,7 @@ struct DeviceInfo {
   int device = -1, sms = 0, max_smem_optin = 0;
   bool attr_set[2] = {false, false};
   int attr_smem[2] = {0, 0};
+  int fit_blocks_per_sm = 0;
 };
 std::mutex g_mu;
 std::vector<DeviceInfo> g_dev;
@@ -75,6 +77,7 @@ int validate(const pv_params* p, int* nbins_out) {
   if (p->max_vtx_per_event < 1 || p->max_vtx_per_event > PV_MAX_VTX) return PV_E_PARAM;
   if (p->max_iter < 1 || p->max_iter > 16) return PV_E_PARAM;
   if (!(p->chi2_max > 0.0f)) return PV_E_PARAM;
+  if (!(p->min_bin_content >= 0.0f)) return PV_E_PARAM;      // only bins a track wrote can start a proto-cluster
   if (nbins_out) *nbins_out = nbins;
   return PV_OK;
 }
@@ -88,7 +91,8 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->nbins = nbins; k->nwords = (nbins + 31) / 32;
   k->T_bin = clamp_i32(to_fixed(p->min_bin_content));
   k->D = clamp_i32(to_fixed(p->min_dip));
-  k->I_min[0] = to_fixed(p->min_cluster_integral[0]); k->I_min[1] = to_fixed(p->min_cluster_integral[1]);
+  k->I_min[0] = clamp_i32(to_fixed(p->min_cluster_integral[0]));   // an event holds < 2047 * 2^20 < 2^31
+  k->I_min[1] = clamp_i32(to_fixed(p->min_cluster_integral[1]));
   for (int r = 0; r < 2; ++r) { k->min_tracks_seed[r] = p->min_tracks_seed[r]; k->min_tracks_pv[r] = p->min_tracks_pv[r]; }
   k->chi2_max = p->chi2_max;
   k->unit_weights = isinf(p->chi2_max) ? 1 : 0;
@@ -97,14 +101,18 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->conv_dchi2 = p->conv_dchi2; k->conv_dz = p->conv_dz; k->merge_ratio = p->merge_ratio;
   k->max_beam_dist2 = p->max_beam_dist * p->max_beam_dist;
   k->max_vtx = p->max_vtx_per_event;
-  int r0 = ((nbins + 31) / 32) * 32 * 4;                      // histogram padded to whole 32-bin words
-  if (r0 < pvk::OVL_MIN_BYTES) r0 = pvk::OVL_MIN_BYTES;
-  r0 = (r0 + 15) / 16 * 16;
+  const int r0 = ((nbins + 31) / 32) * 32 * 4;                // histogram padded to whole 32-bin words
   k->region0_words = r0 / 4;
-  k->warp_smem_bytes = r0 + pvk::R1_BYTES + pvk::R2_BYTES;
+  k->warp_smem_bytes = r0 + pvk::SM_TAIL_BYTES;
 }
 
-constexpr size_t WORKSPACE_BYTES = 256;
+// Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | sidx, 2 B per track.
+constexpr size_t WS_COUNTERS = 256;
+size_t ws_rec_bytes(int n_events, int max_vtx) { return (size_t)n_events * (size_t)max_vtx * sizeof(pvk::SeedRec); }
+size_t ws_bytes(int n_events, long long n_tracks, int max_vtx) {
+  return WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + (((size_t)n_tracks * 2 + 15) / 16) * 16 + 16;
+}
+
 
 int find_impl(const float* x, const float* y, const float* z, const float* tx, const float* ty,
               const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
@@ -121,7 +129,8 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     return PV_E_NULL;
   if (n_tracks > 0 && (!x || !y || !z || !tx || !ty || !var_x || !var_y || !var_tx || !var_ty || !trk_weight || !trk_vertex))
     return PV_E_NULL;
-  if (workspace_bytes < WORKSPACE_BYTES) return PV_E_WORKSPACE;
+  if (workspace_bytes < ws_bytes(n_events, n_tracks, params->max_vtx_per_event)) return PV_E_WORKSPACE;
+  if (((uintptr_t)workspace & 15) != 0) return PV_E_PARAM;
   cudaStream_t stream = (cudaStream_t)stream_;
 
   std::lock_guard<std::mutex> lock(g_mu);
@@ -141,13 +150,17 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   const int smem = warps * kp.warp_smem_bytes;
   const int which = dbg ? 1 : 0;
   if (!di->attr_set[which] || di->attr_smem[which] < smem) {
-    if (which) CK(cudaFuncSetAttribute(pvk::pv_find_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    else CK(cudaFuncSetAttribute(pvk::pv_find_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    if (which) CK(cudaFuncSetAttribute(pvk::seed_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    else CK(cudaFuncSetAttribute(pvk::seed_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     di->attr_set[which] = true;
     di->attr_smem[which] = smem;
   }
+  if (di->fit_blocks_per_sm == 0) {
+    int nb = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel, 256, 0));
+    di->fit_blocks_per_sm = nb > 0 ? nb : 1;
+  }
   g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * 32; g_last_smem = smem;
-  if (n_events == 0) return PV_OK;
 
   pvk::KArgs ka;
   memset(&ka, 0, sizeof(ka));
@@ -157,22 +170,45 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.vtx_pos = vtx_pos; ka.vtx_cov = vtx_cov; ka.vtx_chi2 = vtx_chi2;
   ka.vtx_ntracks = vtx_ntracks; ka.vtx_niter = vtx_niter; ka.n_vtx = n_vtx;
   ka.trk_weight = trk_weight; ka.trk_vertex = trk_vertex; ka.event_status = event_status;
-  ka.counter = reinterpret_cast<unsigned int*>(workspace);
+  unsigned char* ws = reinterpret_cast<unsigned char*>(workspace);
+  ka.evt_counter = reinterpret_cast<unsigned int*>(ws);
+  ka.seed_counter = reinterpret_cast<unsigned int*>(ws + 16);
+  ka.rec = reinterpret_cast<pvk::SeedRec*>(ws + WS_COUNTERS);
+  ka.sidx = reinterpret_cast<uint16_t*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
   if (dbg) ka.dbg = *dbg;
 
-  CK(cudaMemsetAsync(workspace, 0, 16, stream));
+  const bool timing = g_timing != 0;
+  if (timing && !g_ev[0])
+    for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
+  CK(cudaMemsetAsync(workspace, 0, 32, stream));
+  // a1..a4: persistent, one CTA per SM, one warp per event
   int grid = di->sms;
   const int need = (n_events + warps - 1) / warps;
   if (grid > need) grid = need;
-  if (g_timing) {
-    if (!g_ev0) { CK(cudaEventCreate(&g_ev0)); CK(cudaEventCreate(&g_ev1)); }
-    CK(cudaEventRecord(g_ev0, stream));
-  }
-  if (dbg) pvk::pv_find_kernel<true><<<grid, warps * 32, smem, stream>>>(kp, ka);
-  else pvk::pv_find_kernel<false><<<grid, warps * 32, smem, stream>>>(kp, ka);
+  if (timing) CK(cudaEventRecord(g_ev[0], stream));
+  if (dbg) pvk::seed_kernel<true><<<grid, warps * 32, smem, stream>>>(kp, ka);
+  else pvk::seed_kernel<false><<<grid, warps * 32, smem, stream>>>(kp, ka);
   CK(cudaGetLastError());
-  if (g_timing) { CK(cudaEventRecord(g_ev1, stream)); g_ev_valid = true; }
-  g_last_kernels = 1; g_last_grid = grid;
+  if (timing) CK(cudaEventRecord(g_ev[1], stream));
+  // a5: 8 lanes per seed, grid-stride over the seed records
+  {
+    long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm;
+    const long long most = ((long long)n_events * params->max_vtx_per_event + 31) / 32;   // 32 seeds per 256-thread CTA
+    if (fit_grid > most) fit_grid = most;
+    if (fit_grid < 1) fit_grid = 1;
+    pvk::fit_kernel<<<(int)fit_grid, 256, 0, stream>>>(kp, ka);
+    CK(cudaGetLastError());
+  }
+  if (timing) CK(cudaEventRecord(g_ev[2], stream));
+  // a6: one warp per event
+  {
+    const int cgrid = (n_events + 7) / 8;
+    if (dbg) pvk::cleanup_kernel<true><<<cgrid, 256, 0, stream>>>(kp, ka);
+    else pvk::cleanup_kernel<false><<<cgrid, 256, 0, stream>>>(kp, ka);
+    CK(cudaGetLastError());
+  }
+  if (timing) { CK(cudaEventRecord(g_ev[3], stream)); g_ev_valid = true; }
+  g_last_kernels = N_KERNELS; g_last_grid = grid;
   return PV_OK;
 }
 
@@ -209,7 +245,8 @@ int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, siz
   const int rc = validate(p, nullptr);
   if (rc != PV_OK) return rc;
   if (n_events < 0 || n_tracks < 0) return PV_E_SIZE;
-  *bytes = WORKSPACE_BYTES;
+  if (n_tracks > 0x7fffffffLL) return PV_E_SIZE;
+  *bytes = ws_bytes(n_events, n_tracks, p->max_vtx_per_event);
   return PV_OK;
 }
 
@@ -249,7 +286,8 @@ struct pv_host_ctx {
   float *d_pos = nullptr, *d_cov = nullptr, *d_chi2 = nullptr, *d_w = nullptr;
   int32_t *d_ntrk = nullptr, *d_niter = nullptr, *d_nvtx = nullptr, *d_tv = nullptr;
   uint32_t* d_status = nullptr;
-  unsigned char* d_ws = nullptr;   // n_streams * WORKSPACE_BYTES
+  unsigned char* d_ws = nullptr;   // n_streams workspaces of ws_stride bytes each
+  size_t ws_stride = 0;
 };
 
 int pv_host_ctx_destroy(pv_host_ctx* c) {
@@ -279,7 +317,8 @@ int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, 
   A((void**)&c->d_pos, E * mv * 12); A((void**)&c->d_cov, E * mv * 24); A((void**)&c->d_chi2, E * mv * 4);
   A((void**)&c->d_ntrk, E * mv * 4); A((void**)&c->d_niter, E * mv * 4); A((void**)&c->d_nvtx, E * 4);
   A((void**)&c->d_w, T * 4); A((void**)&c->d_tv, T * 4); A((void**)&c->d_status, E * 4);
-  A((void**)&c->d_ws, (size_t)n_streams * WORKSPACE_BYTES);
+  c->ws_stride = (ws_bytes(max_events, max_tracks, c->max_vtx) + 255) / 256 * 256;
+  A((void**)&c->d_ws, (size_t)n_streams * c->ws_stride);
   for (int i = 0; i < n_streams && err == cudaSuccess; ++i) {
     cudaStream_t s = nullptr;
     err = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
@@ -330,7 +369,7 @@ int pv_find_host(pv_host_ctx* c,
     rc = find_impl(c->d_in[0], c->d_in[1], c->d_in[2], c->d_in[3], c->d_in[4], c->d_in[5], c->d_in[6], c->d_in[7], c->d_in[8],
                    c->d_off + e0, (int)ne, (long long)c->max_tracks, params, c->d_pos + e0 * mv * 3, c->d_cov + e0 * mv * 6,
                    c->d_chi2 + e0 * mv, c->d_ntrk + e0 * mv, c->d_niter + e0 * mv, c->d_nvtx + e0, c->d_w, c->d_tv,
-                   c->d_status + e0, c->d_ws + (size_t)(k % c->n_streams) * WORKSPACE_BYTES, WORKSPACE_BYTES, s, nullptr);
+                   c->d_status + e0, c->d_ws + (size_t)(k % c->n_streams) * c->ws_stride, c->ws_stride, s, nullptr);
     if (rc != PV_OK) break;
     CK(cudaMemcpyAsync(vtx_pos + e0 * mv * 3, c->d_pos + e0 * mv * 3, ne * mv * 12, cudaMemcpyDeviceToHost, s));
     CK(cudaMemcpyAsync(vtx_cov + e0 * mv * 6, c->d_cov + e0 * mv * 6, ne * mv * 24, cudaMemcpyDeviceToHost, s));
@@ -379,11 +418,19 @@ int pv_kernel_timing(int enable) {
 }
 
 float pv_kernel_time_ms(void) {
-  if (!g_ev_valid || !g_ev0 || !g_ev1) return -1.0f;
-  if (cudaEventSynchronize(g_ev1) != cudaSuccess) return -1.0f;
+  if (!g_ev_valid || !g_ev[0]) return -1.0f;
+  if (cudaEventSynchronize(g_ev[N_KERNELS]) != cudaSuccess) return -1.0f;
   float ms = -1.0f;
-  if (cudaEventElapsedTime(&ms, g_ev0, g_ev1) != cudaSuccess) return -1.0f;
+  if (cudaEventElapsedTime(&ms, g_ev[0], g_ev[N_KERNELS]) != cudaSuccess) return -1.0f;
   return ms;
+}
+
+int pv_kernel_times_ms(float* ms, int n) {
+  if (!ms) return PV_E_NULL;
+  if (!g_ev_valid || !g_ev[0]) return PV_E_SIZE;
+  CK(cudaEventSynchronize(g_ev[N_KERNELS]));
+  for (int i = 0; i < n && i < N_KERNELS; ++i) CK(cudaEventElapsedTime(&ms[i], g_ev[i], g_ev[i + 1]));
+  return N_KERNELS;
 }
 
 const char* pv_error_string(int code) {

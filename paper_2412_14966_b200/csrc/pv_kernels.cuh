@@ -1,23 +1,23 @@
 // pv_kernels.cuh -- sm_100a kernels of the PV-finder hot path (arXiv:2412.14966, "P:Lnn" = PAPER.md line nn).
 //
-// Execution model: ONE WARP PER EVENT.  A persistent grid of one CTA per
-// SM holds as many warps as per-event shared-memory histograms fit ("one block per event",
-// re-cut for 117-track events: a warp owns an event end to end, so every step is synchronised with
-// __syncwarp / shuffles / ballots only and nothing goes through HBM between the steps).  Warps pull
-// event indices from a global counter.  Steps a1..a6 of include/pv_finder.h run back to back:
+// Three kernels per pv_find call:
 //
-//   a1+a2  thread per track: POCA projection (fp32 contract, bit-exact with the CPU oracle) and
-//          fixed-point Gaussian bin integrals added to the warp's int32 shared-memory histogram
-//   a3     ballot bitmap of bins above threshold -> proto-cluster starts -> one lane per proto-cluster
-//          runs the z-ordered hysteresis sweep; warp scan orders the emitted seed clusters in z
-//   a4     partition points, per-track seed by comparison, ballot counting, removal loop,
-//          match_any counting sort of the tracks by seed
-//   a5     8 lanes per vertex (4 vertices per warp pass), tracks register-resident, xor-shuffle
-//          reduction of the normal equations, closed-form 3x3 solve of the arrow-shaped Hessian
-//   a6     z-ordered duplicate sweep, cuts, compaction, final per-track outputs
+//   seed_kernel     a1..a4  one WARP per event, persistent grid, per-warp int32 shared-memory histogram.
+//                           POCA projection (fp32 contract, bit-exact with the CPU oracle), tracks sorted by
+//                           window length so the fixed-point Gaussian fill runs with full lanes, threshold
+//                           bitmap of the touched histogram words only, one lane per proto-cluster for the
+//                           z-ordered hysteresis sweep, seed positions, association with the removal loop,
+//                           deterministic counting sort of the tracks by seed -> seed records in HBM.
+//   fit_kernel      a5      8 lanes per vertex seed, flat over all seeds of the batch (no histogram, so it
+//                           runs at full occupancy): tracks register-resident, xor-shuffle reduction of the
+//                           normal equations, closed-form solve of the arrow-shaped 3x3 Hessian.
+//   cleanup_kernel  a6      one warp per event: z-ordered duplicate sweep, cuts, compaction, final per-track
+//                           vertex index and weight.
 //
+// The v1 single fused kernel (profiles/r1_v1_fused_kernel.md) was 87 KB of SASS and lost 42 % of its issue
+// slots to instruction-cache misses with 14 warps per SM in different phases; each kernel here is small.
 // This file shares nothing with oracle/ (the frozen CDF coefficients below are the numbers of
-// DESIGN.md "CDF contract", restated).
+// DESIGN.md section 3, restated).
 #pragma once
 
 #include <cuda_runtime.h>
@@ -30,18 +30,22 @@ namespace pvk {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
+constexpr int CHUNK = 128;          // tracks per fill chunk: 4 register slots per lane
+constexpr int SLOTS = CHUNK / 32;
 constexpr int FIT_G = 8;            // lanes per vertex in the fit
 constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
 constexpr int FIT_KF = 6;           // register-resident tracks per lane (fast path: <= FIT_G*FIT_KF tracks)
+constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
+constexpr int PROTO_CAP = 512;      // proto-cluster starts of one round of 32 touched words (<= 16 per word)
 
-// Per-warp shared-memory layout (bytes).  Region 0 holds the histogram during a1-a3 and is re-used
-// (the histogram is dead once the seed positions are known) for the seed-sorted track index list and
-// the per-vertex fit results during a4-a6.
-constexpr int OVL_SIDX_BYTES = 4096;                 // uint16 sidx[2048]
-constexpr int OVL_VTX_FIELDS = 13;                   // pos3 cov6 chi2 ntrk niter = 12, +1 spare
-constexpr int OVL_MIN_BYTES = OVL_SIDX_BYTES + OVL_VTX_FIELDS * MAXV * 4;
-constexpr int R1_BYTES = 1296;                       // peaks: bm[128] sbw[128] cum[130 u16]; assign: cnt cur part off
-constexpr int R2_BYTES = 4 * MAXV * 4;               // seeds: begin end peak z
+// Per-warp shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
+constexpr int SM_BM = 0;                               // unsigned bm[128]     bins above threshold, bit per bin
+constexpr int SM_TOUCHED = SM_BM + MAX_WORDS * 4;      // unsigned touched[4]  histogram words written by the fill
+constexpr int SM_TWL = SM_TOUCHED + 16;                // uint8 twl[128]       list of touched words, ascending
+constexpr int SM_CNT = SM_TWL + MAX_WORDS;             // int cnt[32], cur[32], off[33+3]
+constexpr int SM_SEED = SM_CNT + (32 + 32 + 36) * 4;   // int sb[32], se[32], sp[32]; float zs[32]; int part[32]
+constexpr int SM_STAGE = SM_SEED + 5 * MAXV * 4;       // float4 stage[128] (fill)  /  uint16 protostart[512] (peaks)
+constexpr int SM_TAIL_BYTES = SM_STAGE + CHUNK * 16;
 
 struct KParams {
   float z_min, dz, inv_dz, z_split;
@@ -50,15 +54,23 @@ struct KParams {
   float win_eps;                 // safety margin of the fill window, in bins
   int nbins, nwords;             // nwords = ceil(nbins / 32)
   int T_bin, D;                  // thresholds in fixed point, clamped to int32
-  long long I_min[2];
+  int I_min[2];                  // min cluster integral, fixed point clamped to int32 (an event holds < 2^31)
   int min_tracks_seed[2], min_tracks_pv[2];
   float chi2_max, inv_chi2_max;
   int unit_weights;              // chi2_max == inf
   int max_iter;
   float conv_dchi2, conv_dz, merge_ratio, max_beam_dist2;
   int max_vtx;
-  int region0_words;             // int32 words of region 0 (multiple of 4)
+  int region0_words;             // int32 words of the histogram region (multiple of 32)
   int warp_smem_bytes;
+};
+
+// One vertex seed handed from seed_kernel to fit_kernel (16 bytes, read as one int4).
+struct SeedRec {
+  int e;                         // event
+  int k_cnt;                     // seed index within the event | track count << 5
+  int begin;                     // first entry of the seed's track list in sidx[] (absolute)
+  float z;                       // z_seed (Eq. 4)
 };
 
 struct KArgs {
@@ -70,12 +82,12 @@ struct KArgs {
   float* trk_weight;
   int32_t* trk_vertex;
   uint32_t* event_status;
-  unsigned int* counter;
+  unsigned int* evt_counter;     // workspace: next event of the persistent seed kernel
+  unsigned int* seed_counter;    // workspace: seed records written so far
+  SeedRec* rec;                  // workspace: [n_events * max_vtx]
+  uint16_t* sidx;                // workspace: [T] track indices (local to the event) sorted by seed
   pv_debug dbg;
 };
-
-// ---- frozen CDF contract: F(u) = 1/2 + s*G(s^2), s = u/3, odd degree-13 polynomial; the seven
-// fp32 coefficients are literals inside edge_q() ---------------------------------------------------------------
 
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -117,27 +129,36 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 }
 
 // ---- a3: z-ordered hysteresis sweep over one proto-cluster starting at bin b0 (R-4) --------
-// Returns the number of seed clusters the proto-cluster yields.  With WRITE, cluster j is stored at
-// index base + j of (sb, se, sp) when that is < max_vtx.
-template <bool WRITE>
-__device__ int sweep(const int* __restrict__ H, int b0, const KParams& P, int base, int* sb, int* se, int* sp) {
+// Returns the number of seed clusters the proto-cluster yields.  Clusters 0 and 1 are returned in c0 / c1;
+// cluster j is also stored at index wbase + j of (sb, se, sp) when wbase >= 0 and that index is < max_vtx.
+// (Single call site, inside a loop, so that the code exists once.)
+struct Cl { int b, e, p; };
+
+__device__ __forceinline__ int sweep(const int* __restrict__ H, int b0, const KParams& P, int wbase,
+                                     int* sb, int* se, int* sp, Cl& c0, Cl& c1) {
   int start = b0;
   int h = H[b0];
   bool look_max = true;
   int mx = h, mn = 0, mnp = b0;
-  long long sum = h;                         // integral of [start, k]
+  int sum = h;                               // integral of [start, k]
   int amax = h, amaxp = b0;                  // argmax of [start, k], ties -> lowest bin
-  long long snap_sum = 0;                    // the same over [start, mnp)
+  int snap_sum = 0;                          // the same over [start, mnp)
   int snap_amax = 0, snap_amaxp = b0;
   int smax = h, smaxp = b0;                  // argmax of [mnp, k]
   int count = 0;
   bool have = false;                         // last emitted cluster, held back because the tail may join it
   int lb = 0, le = 0, lp = 0, lpv = 0, lj = 0;
+  auto flush = [&]() {
+    if (lj == 0) { c0.b = lb; c0.e = le; c0.p = lp; }
+    if (lj == 1) { c1.b = lb; c1.e = le; c1.p = lp; }
+    if (wbase >= 0 && wbase + lj < P.max_vtx) { sb[wbase + lj] = lb; se[wbase + lj] = le; sp[wbase + lj] = lp; }
+  };
   int k = b0 + 1;
+#pragma unroll 1
   for (; k < P.nbins; ++k) {
     h = H[k];
     if (!(h > P.T_bin)) break;
-    const long long prev_sum = sum;
+    const int prev_sum = sum;
     const int prev_amax = amax, prev_amaxp = amaxp;
     sum += h;
     if (h > amax) { amax = h; amaxp = k; }
@@ -158,7 +179,7 @@ __device__ int sweep(const int* __restrict__ H, int b0, const KParams& P, int ba
       } else if (h - mn > P.D) {             // significant minimum at mnp, with a maximum on either side
         mx = h; look_max = true;
         if (snap_sum >= P.I_min[bin_region(snap_amaxp, P)]) {
-          if (WRITE && have && base + lj < P.max_vtx) { sb[base + lj] = lb; se[base + lj] = le; sp[base + lj] = lp; }
+          if (have) flush();
           lb = start; le = mnp; lp = snap_amaxp; lpv = snap_amax; lj = count; have = true;
           ++count;
           start = mnp;                       // the minimum bin opens the right-hand cluster
@@ -169,15 +190,388 @@ __device__ int sweep(const int* __restrict__ H, int b0, const KParams& P, int ba
   }
   // tail [start, k)
   if (sum >= P.I_min[bin_region(amaxp, P)]) {
-    if (WRITE && have && base + lj < P.max_vtx) { sb[base + lj] = lb; se[base + lj] = le; sp[base + lj] = lp; }
+    if (have) flush();
     lb = start; le = k; lp = amaxp; lj = count; have = true;
     ++count;
   } else if (have) {                         // remainder joins the last cluster of this proto-cluster
     le = k;
     if (amax > lpv) { lp = amaxp; lpv = amax; }
   }
-  if (WRITE && have && base + lj < P.max_vtx) { sb[base + lj] = lb; se[base + lj] = le; sp[base + lj] = lp; }
+  if (have) flush();
   return count;
+}
+
+// ---- a1: POCA projection of one track (Eq. 1, Eq. 3; fp32 contract of DESIGN.md section 3) ---------------------
+struct Proj {
+  float zp, sg, inv;             // z_poca, sigma_poca, 1 / (3 sigma_poca)
+  int bin;                       // central bin, -1 = not assignable
+  bool fill;                     // enters the histogram
+};
+
+__device__ __forceinline__ Proj project(float x, float y, float z, float tx, float ty, float vx, const KParams& P) {
+  Proj r;
+  r.zp = __int_as_float(0x7fc00000); r.sg = r.zp; r.inv = 0.0f; r.bin = -1; r.fill = false;
+  const float dtx = __fsub_rn(tx, P.beam_tx), dty = __fsub_rn(ty, P.beam_ty);
+  const float den = __fmaf_rn(dty, dty, __fmul_rn(dtx, dtx));
+  if (den >= 1e-12f) {                                    // R-3: not parallel to the beamline
+    const float bx = __fmaf_rn(P.beam_tx, z, P.beam_x), by = __fmaf_rn(P.beam_ty, z, P.beam_y);
+    const float num = __fmaf_rn(dty, __fsub_rn(by, y), __fmul_rn(dtx, __fsub_rn(bx, x)));
+    r.zp = __fadd_rn(z, __fdiv_rn(num, den));
+    r.sg = __fsqrt_rn(__fdiv_rn(vx, den));
+    const float fb = floorf(__fmul_rn(__fsub_rn(r.zp, P.z_min), P.inv_dz));
+    if (fb >= 0.0f && fb < (float)P.nbins) {
+      r.bin = (int)fb;
+      const int region = r.zp < P.z_split ? 1 : 0;        // R-5
+      r.inv = __fdiv_rn(1.0f, __fmul_rn(3.0f, r.sg));
+      r.fill = r.sg > 0.0f && r.sg <= P.max_sigma[region] && r.inv < INFINITY;
+    }
+  }
+  return r;
+}
+
+// ---- seed_kernel: a1..a4 for one event, one warp --------------------------------------------------------------
+template <bool DBG>
+__device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int lane) {
+  int* H = reinterpret_cast<int*>(wsm);
+  unsigned char* tail = wsm + (size_t)P.region0_words * 4;
+  unsigned* bm = reinterpret_cast<unsigned*>(tail + SM_BM);
+  unsigned* touched = reinterpret_cast<unsigned*>(tail + SM_TOUCHED);
+  uint8_t* twl = reinterpret_cast<uint8_t*>(tail + SM_TWL);
+  int* cnt = reinterpret_cast<int*>(tail + SM_CNT);
+  int* cur = cnt + 32;
+  int* sb = reinterpret_cast<int*>(tail + SM_SEED);
+  int* se = sb + MAXV;
+  int* sp = se + MAXV;
+  float* zs = reinterpret_cast<float*>(sp + MAXV);
+  int* part = reinterpret_cast<int*>(zs + MAXV);
+  float4* stage = reinterpret_cast<float4*>(tail + SM_STAGE);
+  uint16_t* protostart = reinterpret_cast<uint16_t*>(tail + SM_STAGE);   // overlay: the stage is dead after the fill
+
+  const int t0 = __ldg(A.offsets + e);
+  const int n = __ldg(A.offsets + e + 1) - t0;
+  const size_t ev = (size_t)e * P.max_vtx;
+  unsigned status = 0;
+
+  if (n > MAX_TRK) {
+#pragma unroll 1
+    for (int i = lane; i < n; i += 32) A.trk_vertex[t0 + i] = -1;
+    if (DBG && A.dbg.trk_seed) for (int i = lane; i < n; i += 32) A.dbg.trk_seed[t0 + i] = -1;
+    if (lane == 0) {
+      A.n_vtx[e] = 0;
+      A.event_status[e] = PV_EVT_TOO_MANY_TRACKS;
+      if (DBG && A.dbg.n_seeds) A.dbg.n_seeds[e] = 0;
+      if (DBG && A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = 0;
+    }
+    return;
+  }
+
+  // ================= a1 + a2: projection (Eq. 1, Eq. 3) and histogram fill (P:L125-131) ===================
+  // Chunks of CHUNK tracks, SLOTS per lane.  Within a chunk the histogrammed tracks are counting-sorted by
+  // window length (bins), so the 32 lanes of a fill pass run loops of (nearly) the same length.  The adds are
+  // integer, so the order changes nothing.
+  const bool one_chunk = n <= CHUNK;
+  int binr[SLOTS];                                         // central bins of a single-chunk event stay in registers
+#pragma unroll
+  for (int s = 0; s < SLOTS; ++s) binr[s] = -1;
+#pragma unroll 1
+  for (int c0 = 0; c0 < n; c0 += CHUNK) {
+    float zp[SLOTS], inv[SLOTS], kf[SLOTS];
+    int nb[SLOTS];
+    float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
+#pragma unroll
+    for (int s = 0; s < SLOTS; ++s) {                      // all loads first (24 in flight per lane)
+      const int i = c0 + s * 32 + lane;
+      const int t = t0 + (i < n ? i : n - 1);
+      lx[s] = __ldg(A.x + t); ly[s] = __ldg(A.y + t); lz[s] = __ldg(A.z + t);
+      ltx[s] = __ldg(A.tx + t); lty[s] = __ldg(A.ty + t); lvx[s] = __ldg(A.var_x + t);
+    }
+    cnt[lane] = 0;
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < SLOTS; ++s) {
+      const int i = c0 + s * 32 + lane;
+      nb[s] = 0; zp[s] = 0.0f; inv[s] = 0.0f; kf[s] = 0.0f;
+      if (i < n) {
+        const Proj r = project(lx[s], ly[s], lz[s], ltx[s], lty[s], lvx[s], P);
+        if (one_chunk) binr[s] = r.bin; else A.trk_vertex[t0 + i] = r.bin;   // large events: HBM scratch, read back in a4
+        if (DBG) {
+          if (A.dbg.z_poca) A.dbg.z_poca[t0 + i] = r.zp;
+          if (A.dbg.sigma_poca) A.dbg.sigma_poca[t0 + i] = r.sg;
+          if (A.dbg.trk_bin) A.dbg.trk_bin[t0 + i] = r.bin;
+        }
+        if (r.fill) {
+          // window: a superset of the +-3 sigma support; edges outside it give exactly 0 or 2^20
+          const float w3 = 3.0f * r.sg;
+          const float fa = floorf((r.zp - w3 - P.z_min) * P.inv_dz - P.win_eps);
+          const float fb2 = floorf((r.zp + w3 - P.z_min) * P.inv_dz + P.win_eps) + 1.0f;
+          const int lo = (int)fmaxf(fa, 0.0f);
+          const int hi = (int)fminf(fb2, (float)P.nbins);
+          nb[s] = hi - lo; zp[s] = r.zp; inv[s] = r.inv; kf[s] = (float)lo;
+          if (nb[s] > 0) atomicAdd(&cnt[min(nb[s], 31)], 1);
+        }
+      }
+    }
+    __syncwarp();
+    int total;
+    {
+      const int c = cnt[lane];
+      const int inc = warp_incl_scan(c, lane);
+      total = __shfl_sync(FULL, inc, 31);
+      __syncwarp();
+      cnt[lane] = inc - c;                                 // first staging slot of each window-length class
+    }
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < SLOTS; ++s) {
+      if (nb[s] > 0) {
+        const int pos = atomicAdd(&cnt[min(nb[s], 31)], 1);
+        stage[pos] = make_float4(zp[s], inv[s], kf[s], __int_as_float(nb[s]));
+      }
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int p0 = 0; p0 < total; p0 += 32) {
+      const int idx = p0 + lane;
+      float4 st = make_float4(0.0f, 0.0f, 0.0f, __int_as_float(0));
+      if (idx < total) st = stage[idx];
+      const int nbl = __float_as_int(st.w);
+      const int b0 = (int)st.z;
+      if (nbl > 0) {                                       // histogram words this track writes
+        const int w1 = (b0 + nbl - 1) >> 5;
+#pragma unroll 1
+        for (int w = b0 >> 5; w <= w1; ++w) atomicOr(&touched[w >> 5], 1u << (w & 31));
+      }
+      const int mx = __reduce_max_sync(FULL, nbl);
+      float kfl = st.z;
+      int q0 = edge_q(kfl, st.x, st.y, P);
+#pragma unroll 1
+      for (int j = 0; j < mx; ++j) {
+        kfl += 1.0f;
+        const int q1 = edge_q(kfl, st.x, st.y, P);
+        const int d = q1 - q0;
+        if (j < nbl && d != 0) atomicAdd(&H[b0 + j], d);
+        q0 = q1;
+      }
+    }
+    __syncwarp();
+  }
+
+  if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
+    for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
+
+  // ================= a3: peak search (P:L133-137) and seed position (Eq. 4-5) ==============================
+  // List of the touched histogram words, ascending; only these can hold bins above the threshold.
+  int ntw = 0;
+#pragma unroll
+  for (int q = 0; q < MAX_WORDS / 32; ++q) {
+    const unsigned m = touched[q];
+    if ((m >> lane) & 1u) twl[ntw + __popc(m & lanemask_lt())] = (uint8_t)(q * 32 + lane);
+    ntw += __popc(m);
+  }
+  __syncwarp();
+#pragma unroll 1
+  for (int i = 0; i < ntw; ++i) {
+    const int w = twl[i];
+    const unsigned m = __ballot_sync(FULL, w * 32 + lane < P.nbins && H[w * 32 + lane] > P.T_bin);
+    if (lane == 0) bm[w] = m;
+  }
+  __syncwarp();
+
+  int n_raw = 0;
+#pragma unroll 1
+  for (int r0 = 0; r0 < ntw; r0 += 32) {                   // rounds of 32 touched words (one round in practice)
+    int n_proto;
+    {
+      unsigned sbits = 0;
+      int w = 0;
+      if (r0 + lane < ntw) {
+        w = twl[r0 + lane];
+        const unsigned m = bm[w];
+        const unsigned prev = w > 0 ? (bm[w - 1] >> 31) : 0u;
+        sbits = m & ~((m << 1) | prev);                    // first bin of each run of bins above threshold
+      }
+      const int c = __popc(sbits);
+      const int inc = warp_incl_scan(c, lane);
+      n_proto = __shfl_sync(FULL, inc, 31);
+      int o = inc - c;
+      while (sbits) {
+        protostart[o++] = (uint16_t)(w * 32 + __ffs(sbits) - 1);
+        sbits &= sbits - 1;
+      }
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int p0 = 0; p0 < n_proto; p0 += 32) {             // one lane per proto-cluster
+      const int p = p0 + lane;
+      const bool act = p < n_proto;
+      const int b0 = act ? (int)protostart[p] : 0;
+      Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
+      int c = 0, base = 0;
+#pragma unroll 1
+      for (int rep = 0; rep < 2; ++rep) {                  // rep 1 (rare): proto-clusters with three or more seeds
+        const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
+        if (!__any_sync(FULL, run)) break;
+        if (run) {
+          const int cc = sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+          if (rep == 0) c = cc;
+        }
+        if (rep == 0) {
+          const int inc = warp_incl_scan(c, lane);
+          base = n_raw + inc - c;
+          if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
+          if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
+          n_raw += __shfl_sync(FULL, inc, 31);
+        }
+      }
+    }
+    __syncwarp();
+  }
+  int ns = n_raw;
+  if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
+  __syncwarp();
+  if (lane < ns) {                                         // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
+    const int i = sp[lane];
+    const long long Nm = i > 0 ? H[i - 1] : 0;
+    const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
+    const long long N0 = H[i];
+    const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
+    const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
+    const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
+    zs[lane] = __fmaf_rn(delta, P.dz, zi);
+  }
+  __syncwarp();
+  // the histogram is dead from here on: clear what this event touched for the next one
+#pragma unroll 1
+  for (int i = 0; i < ntw; ++i) H[(int)twl[i] * 32 + lane] = 0;
+#pragma unroll 1
+  for (int i = lane; i < ntw; i += 32) bm[twl[i]] = 0;
+  if (lane < MAX_WORDS / 32) touched[lane] = 0;
+
+  // ================= a4: association (R-11) ====================================================
+  // Central bins: single-chunk events keep them in shared memory (int16, behind the proto-cluster list),
+  // larger events read them back from the trk_vertex scratch.
+  int16_t* binsm = reinterpret_cast<int16_t*>(tail + SM_STAGE + PROTO_CAP * 2);
+  if (one_chunk) {
+#pragma unroll
+    for (int s = 0; s < SLOTS; ++s) binsm[s * 32 + lane] = (int16_t)binr[s];
+  }
+  auto seed_of = [&](int i) -> int {                       // seed index of track i, -1 = none
+    if (i >= n || ns == 0) return -1;
+    const int b = one_chunk ? (int)binsm[i] : A.trk_vertex[t0 + i];
+    if (b < 0) return -1;
+    int s = 0;
+#pragma unroll 1
+    for (int k = 0; k + 1 < ns; ++k) s += (b >= part[k]) ? 1 : 0;   // bins < part[k] belong to seed <= k
+    return s;
+  };
+  for (;;) {
+    if (ns == 0) break;
+    __syncwarp();
+    if (lane + 1 < ns) part[lane] = (se[lane] + sb[lane + 1]) / 2;
+    cnt[lane] = 0;
+    __syncwarp();
+#pragma unroll 1
+    for (int i0 = 0; i0 < n; i0 += 32) {
+      const int s = seed_of(i0 + lane);
+      const unsigned m = __match_any_sync(FULL, s);
+      if (s >= 0 && (m & lanemask_lt()) == 0) cnt[s] += __popc(m);
+      __syncwarp();
+    }
+    // "the seed cluster is removed ... and the procedure is repeated" (P:L163): least populated, ties lowest z
+    int key = 0x7fffffff;
+    if (lane < ns) {
+      const int region = zs[lane] < P.z_split ? 1 : 0;
+      const int c = cnt[lane];
+      if (c < P.min_tracks_seed[region]) key = (c << 6) | lane;
+    }
+    key = __reduce_min_sync(FULL, key);
+    if (key == 0x7fffffff) break;
+    const int worst = key & 63;
+    int nb = 0, ne = 0, np = 0;
+    float nz = 0.0f;
+    const bool mv = lane >= worst && lane + 1 < ns;
+    if (mv) { nb = sb[lane + 1]; ne = se[lane + 1]; np = sp[lane + 1]; nz = zs[lane + 1]; }
+    __syncwarp();
+    if (mv) { sb[lane] = nb; se[lane] = ne; sp[lane] = np; zs[lane] = nz; }
+    --ns;
+  }
+  __syncwarp();
+  // counting sort of the tracks by seed (deterministic: track order is kept inside a seed)
+  int myc = 0, myoff = 0;
+  {
+    myc = lane < ns ? cnt[lane] : 0;
+    const int inc = warp_incl_scan(myc, lane);
+    myoff = inc - myc;
+    cur[lane] = myoff;
+  }
+  __syncwarp();
+#pragma unroll 1
+  for (int i0 = 0; i0 < n; i0 += 32) {
+    const int i = i0 + lane;
+    const int s = seed_of(i);
+    if (i < n) {
+      A.trk_vertex[t0 + i] = s;                            // scratch: seed index, read back by cleanup_kernel
+      if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
+    }
+    const unsigned m = __match_any_sync(FULL, s);
+    const int rank = __popc(m & lanemask_lt());
+    if (s >= 0) A.sidx[t0 + cur[s] + rank] = (uint16_t)i;
+    __syncwarp();
+    if (s >= 0 && rank == 0) cur[s] += __popc(m);
+    __syncwarp();
+  }
+  // seed records for fit_kernel
+  int rbase = 0;
+  if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
+  rbase = __shfl_sync(FULL, rbase, 0);
+  if (lane < ns) {
+    int4 r;
+    r.x = e; r.y = lane | (myc << 5); r.z = t0 + myoff; r.w = __float_as_int(zs[lane]);
+    reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
+  }
+  if (lane == 0) {
+    A.n_vtx[e] = ns;                                       // scratch: seeds of the event, replaced by cleanup_kernel
+    A.event_status[e] = status;
+  }
+  if (DBG) {
+    if (lane == 0) {
+      if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
+      if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
+    }
+    if (lane < ns) {
+      if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
+      if (A.dbg.seed_bins) {
+        A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
+        A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
+        A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
+      }
+    }
+  }
+  __syncwarp();
+}
+
+template <bool DBG>
+__global__ void __launch_bounds__(512, 1) seed_kernel(const __grid_constant__ KParams P,
+                                                      const __grid_constant__ KArgs A) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  unsigned char* wsm = smem_raw + (size_t)warp * P.warp_smem_bytes;
+  {
+    int4* Z = reinterpret_cast<int4*>(wsm);                // histogram, bitmap and touched words start at zero
+    const int nq = (P.region0_words * 4 + SM_TWL) >> 4;
+#pragma unroll 1
+    for (int i = lane; i < nq; i += 32) Z[i] = make_int4(0, 0, 0, 0);
+  }
+  __syncwarp();
+  int e = 0;
+  if (lane == 0) e = (int)atomicAdd(A.evt_counter, 1u);
+  e = __shfl_sync(FULL, e, 0);
+  while (e < A.n_events) {
+    int nxt = 0;
+    if (lane == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);   // issued now, consumed after this event
+    seed_event<DBG>(e, P, A, wsm, lane);
+    e = __shfl_sync(FULL, nxt, 0);
+  }
 }
 
 // ---- a5: one track's contribution to the normal equations (Eq. 6-12, 18) -------------------------------
@@ -209,14 +603,32 @@ __device__ __forceinline__ void sums_reduce(Sums& S) {
   }
 }
 
-// Returns the Tukey weight of the track at the current vertex (ax, ay, az); Wx < 0 marks an unusable track.
-__device__ __forceinline__ float track_accum(float x, float y, float z, float tx, float ty, float Wx, float Wy,
-                                             float ax, float ay, float az, const KParams& P, Sums& S) {
-  if (!(Wx > 0.0f)) return 0.0f;
-  const float dz = az - z;
-  const float rx = fmaf(dz, tx, x) - ax;               // residual, Eq. 9
-  const float ry = fmaf(dz, ty, y) - ay;
-  const float cx = rx * Wx, cy = ry * Wy;
+// A track in the seed's local frame (x - x_seed, y - y_seed, z - z_seed): every quantity is O(mm), so fp32
+// keeps ~1e-7 mm instead of ulp(550 mm) = 6e-5 mm and the iterates follow the fp64 oracle.
+// x0 = x - z tx, so the residual Eq. 9 is rx = x0 + az tx - ax.  Wx = 0 marks an unusable or absent track.
+struct Trk { float x0, y0, tx, ty, Wx, Wy; };
+
+// W = V^-1 "evaluated and inverted only once, using the vertex position of the seed" (P:L190), Eq. 2 diagonal.
+__device__ __forceinline__ Trk load_track(const KArgs& A, int g, float sx, float sy, float zsv) {
+  Trk T;
+  const float zl = __ldg(A.z + g) - zsv;
+  T.tx = __ldg(A.tx + g); T.ty = __ldg(A.ty + g);
+  T.x0 = fmaf(-zl, T.tx, __ldg(A.x + g) - sx);
+  T.y0 = fmaf(-zl, T.ty, __ldg(A.y + g) - sy);
+  const float dz2 = zl * zl;
+  const float Vx = fmaf(dz2, __ldg(A.var_tx + g), __ldg(A.var_x + g));
+  const float Vy = fmaf(dz2, __ldg(A.var_ty + g), __ldg(A.var_y + g));
+  const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
+  T.Wx = ok ? __fdividef(1.0f, Vx) : 0.0f;
+  T.Wy = ok ? __fdividef(1.0f, Vy) : 0.0f;
+  return T;
+}
+
+// Returns the Tukey weight of the track at the current vertex (ax, ay, az).
+__device__ __forceinline__ float track_accum(const Trk& T, float ax, float ay, float az, const KParams& P, Sums& S) {
+  const float rx = fmaf(az, T.tx, T.x0) - ax;          // residual, Eq. 9
+  const float ry = fmaf(az, T.ty, T.y0) - ay;
+  const float cx = rx * T.Wx, cy = ry * T.Wy;
   const float chi = fmaf(rx, cx, ry * cy);             // Eq. 7
   float w;
   if (P.unit_weights) {
@@ -225,13 +637,14 @@ __device__ __forceinline__ float track_accum(float x, float y, float z, float tx
     const float u = fmaxf(fmaf(chi, -P.inv_chi2_max, 1.0f), 0.0f);
     w = chi < P.chi2_max ? u * u : 0.0f;               // Tukey bi-square, Eq. 18
   }
-  const float wWx = w * Wx, wWy = w * Wy;
-  const float p = wWx * tx, q = wWy * ty;
+  w = T.Wx > 0.0f ? w : 0.0f;
+  const float wWx = w * T.Wx, wWy = w * T.Wy;
+  const float p = wWx * T.tx, q = wWy * T.ty;
   S.a += wWx; S.b += wWy; S.c += p; S.d += q;
-  S.e = fmaf(p, tx, fmaf(q, ty, S.e));
+  S.e = fmaf(p, T.tx, fmaf(q, T.ty, S.e));
   const float wcx = w * cx, wcy = w * cy;
   S.gx += wcx; S.gy += wcy;
-  S.gz = fmaf(wcx, tx, fmaf(wcy, ty, S.gz));
+  S.gz = fmaf(wcx, T.tx, fmaf(wcy, T.ty, S.gz));
   S.chi2 = fmaf(w, chi, S.chi2);
   S.nact += (w > 0.0f) ? 1.0f : 0.0f;
   return w;
@@ -239,438 +652,213 @@ __device__ __forceinline__ float track_accum(float x, float y, float z, float tx
 
 // Newton-Raphson step Eq. 13 on the arrow-shaped Hessian A = [[a,0,-c],[0,b,-d],[-c,-d,e]]:
 // returns false when the fit is singular (fewer than 2 active tracks or a non-positive pivot).
-__device__ __forceinline__ bool newton_step(const Sums& S, float& dx, float& dy, float& dzs, float& dchi2) {
+// C = A^-1 (Eq. 14), upper triangle xx xy xz yy yz zz.
+__device__ __forceinline__ bool newton_step(const Sums& S, float& dx, float& dy, float& dzs, float& dchi2, float* C) {
   if (S.nact < 2.0f) return false;
   if (!(S.a > 0.0f) || !(S.b > 0.0f)) return false;
-  const float ia = 1.0f / S.a, ib = 1.0f / S.b;
+  const float ia = __fdividef(1.0f, S.a), ib = __fdividef(1.0f, S.b);
   const float ca = S.c * ia, db = S.d * ib;
   const float sch = S.e - S.c * ca - S.d * db;         // Schur complement = third Cholesky pivot squared
   if (!(sch > 0.0f)) return false;
-  dzs = (ca * S.gx + db * S.gy - S.gz) / sch;
+  const float is = __fdividef(1.0f, sch);
+  dzs = (ca * S.gx + db * S.gy - S.gz) * is;
   dx = (S.gx + S.c * dzs) * ia;
   dy = (S.gy + S.d * dzs) * ib;
   dchi2 = dzs * S.gz - dx * S.gx - dy * S.gy;          // Eq. 17
-  return true;
-}
-
-// C = A^-1 (Eq. 14), upper triangle xx xy xz yy yz zz.
-__device__ __forceinline__ void covariance(const Sums& S, float* C) {
-  const float ia = 1.0f / S.a, ib = 1.0f / S.b;
-  const float ca = S.c * ia, db = S.d * ib;
-  const float is = 1.0f / (S.e - S.c * ca - S.d * db);
   C[0] = fmaf(ca * ca, is, ia);
   C[1] = ca * db * is;
   C[2] = ca * is;
   C[3] = fmaf(db * db, is, ib);
   C[4] = db * is;
   C[5] = is;
+  return true;
 }
 
-// W = V^-1 "evaluated and inverted only once, using the vertex position of the seed" (P:L190), Eq. 2 diagonal.
-__device__ __forceinline__ void track_weight_matrix(float zl, float vx, float vy, float vtx, float vty,
-                                                    float& Wx, float& Wy) {
-  const float dz2 = zl * zl;                               // zl = z_trk - z_seed
-  const float Vx = fmaf(dz2, vtx, vx), Vy = fmaf(dz2, vty, vy);
-  const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);
-  Wx = ok ? 1.0f / Vx : -1.0f;
-  Wy = ok ? 1.0f / Vy : -1.0f;
+__device__ __forceinline__ void store_vertex(const KArgs& A, size_t o, float x, float y, float z, const float* C,
+                                             float chi2, int ntrk, int niter) {
+  A.vtx_pos[o * 3 + 0] = x; A.vtx_pos[o * 3 + 1] = y; A.vtx_pos[o * 3 + 2] = z;
+#pragma unroll
+  for (int c = 0; c < 6; ++c) A.vtx_cov[o * 6 + c] = C[c];
+  A.vtx_chi2[o] = chi2; A.vtx_ntracks[o] = ntrk; A.vtx_niter[o] = niter;
 }
 
-// ---- one event, one warp ---------------------------------------------------------------------------------
-template <bool DBG>
-__device__ void process_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int lane) {
-  int* H = reinterpret_cast<int*>(wsm);
-  uint16_t* sidx = reinterpret_cast<uint16_t*>(wsm);                       // overlay, valid after a3
-  float* V = reinterpret_cast<float*>(wsm + OVL_SIDX_BYTES);              // overlay: V[f * MAXV + k]
-  unsigned char* r1 = wsm + (size_t)P.region0_words * 4;
-  unsigned* bm = reinterpret_cast<unsigned*>(r1);                          // peaks
-  unsigned* sbw = bm + 128;
-  uint16_t* cum = reinterpret_cast<uint16_t*>(sbw + 128);
-  int* cnt = reinterpret_cast<int*>(r1);                                   // assign (after peaks)
-  int* cur = cnt + MAXV;
-  int* part = cur + MAXV;
-  int* off = part + MAXV;                                                  // MAXV + 1 entries
-  int* sb = reinterpret_cast<int*>(r1 + R1_BYTES);
-  int* se = sb + MAXV;
-  int* sp = se + MAXV;
-  float* zs = reinterpret_cast<float*>(sp + MAXV);
-
-  const int t0 = A.offsets[e];
-  const int n = A.offsets[e + 1] - t0;
-  const size_t ev = (size_t)e * P.max_vtx;
-  unsigned status = 0;
-
-  if (n > MAX_TRK) {
-    for (int i = lane; i < n; i += 32) { A.trk_vertex[t0 + i] = -1; A.trk_weight[t0 + i] = 0.0f; }
-    if (DBG && A.dbg.trk_seed) for (int i = lane; i < n; i += 32) A.dbg.trk_seed[t0 + i] = -1;
-    if (lane == 0) {
-      A.n_vtx[e] = 0;
-      A.event_status[e] = PV_EVT_TOO_MANY_TRACKS;
-      if (DBG && A.dbg.n_seeds) A.dbg.n_seeds[e] = 0;
-      if (DBG && A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = 0;
-    }
-    return;
-  }
-
-  // ================= a1 + a2: projection (Eq. 1, Eq. 3) and histogram fill (P:L125-131) ===================
-  for (int i = lane; i < n; i += 32) {
-    const int t = t0 + i;
-    const float x = __ldg(A.x + t), y = __ldg(A.y + t), z = __ldg(A.z + t);
-    const float tx = __ldg(A.tx + t), ty = __ldg(A.ty + t), vx = __ldg(A.var_x + t);
-    const float dtx = __fsub_rn(tx, P.beam_tx), dty = __fsub_rn(ty, P.beam_ty);
-    const float den = __fmaf_rn(dty, dty, __fmul_rn(dtx, dtx));
-    float zp = __int_as_float(0x7fc00000), sg = zp;
-    int bin = -1;
-    bool fill = false;
-    float inv = 0.0f;
-    if (den >= 1e-12f) {                                  // R-3: not parallel to the beamline
-      const float bx = __fmaf_rn(P.beam_tx, z, P.beam_x), by = __fmaf_rn(P.beam_ty, z, P.beam_y);
-      const float num = __fmaf_rn(dty, __fsub_rn(by, y), __fmul_rn(dtx, __fsub_rn(bx, x)));
-      zp = __fadd_rn(z, __fdiv_rn(num, den));
-      sg = __fsqrt_rn(__fdiv_rn(vx, den));
-      const float fb = floorf(__fmul_rn(__fsub_rn(zp, P.z_min), P.inv_dz));
-      if (fb >= 0.0f && fb < (float)P.nbins) {
-        bin = (int)fb;
-        const int region = zp < P.z_split ? 1 : 0;
-        inv = __fdiv_rn(1.0f, __fmul_rn(3.0f, sg));
-        fill = sg > 0.0f && sg <= P.max_sigma[region] && inv < INFINITY;
-      }
-    }
-    A.trk_vertex[t] = bin;                                // scratch: central bin, read back in a4
-    if (DBG) {
-      if (A.dbg.z_poca) A.dbg.z_poca[t] = zp;
-      if (A.dbg.sigma_poca) A.dbg.sigma_poca[t] = sg;
-      if (A.dbg.trk_bin) A.dbg.trk_bin[t] = bin;
-    }
-    if (fill) {
-      // window: a superset of the +-3 sigma support; edges outside it give exactly 0 or 2^20
-      const float w3 = 3.0f * sg;
-      const float fa = floorf((zp - w3 - P.z_min) * P.inv_dz - P.win_eps);
-      const float fb2 = floorf((zp + w3 - P.z_min) * P.inv_dz + P.win_eps) + 1.0f;
-      const int lo = (int)fmaxf(fa, 0.0f);
-      const int hi = (int)fminf(fb2, (float)P.nbins);
-      float kf = (float)lo;
-      int q0 = edge_q(kf, zp, inv, P);
-      for (int b = lo; b < hi; ++b) {
-        kf += 1.0f;
-        const int q1 = edge_q(kf, zp, inv, P);
-        const int d = q1 - q0;
-        if (d != 0) atomicAdd(&H[b], d);
-        q0 = q1;
-      }
-    }
-  }
-  __syncwarp();
-
-  if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
-    for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
-
-  // ================= a3: peak search (P:L133-137) and seed position (Eq. 4-5) ==============================
-  const int nw = P.nwords;
-  for (int w = 0; w < nw; ++w) {
-    const int b = w * 32 + lane;
-    const int v = b < P.nbins ? H[b] : 0;
-    const unsigned m = __ballot_sync(FULL, v > P.T_bin);
-    if (lane == 0) bm[w] = m;
-  }
-  __syncwarp();
-  int n_proto = 0;
-  for (int w0 = 0; w0 < nw; w0 += 32) {
-    const int w = w0 + lane;
-    unsigned sbits = 0;
-    if (w < nw) {
-      const unsigned m = bm[w];
-      const unsigned prev = w > 0 ? (bm[w - 1] >> 31) : 0u;
-      sbits = m & ~((m << 1) | prev);                     // first bin of each run of bins above threshold
-      sbw[w] = sbits;
-    }
-    const int c = __popc(sbits);
-    const int inc = warp_incl_scan(c, lane);
-    if (w < nw) cum[w] = (uint16_t)(n_proto + inc - c);
-    n_proto += __shfl_sync(FULL, inc, 31);
-  }
-  if (lane == 0) cum[nw] = (uint16_t)n_proto;
-  __syncwarp();
-
-  int n_raw = 0;
-  for (int p0 = 0; p0 < n_proto; p0 += 32) {
-    const int p = p0 + lane;
-    int b0 = -1, c = 0;
-    if (p < n_proto) {
-      int lo = 0, hi = nw;                                // largest w with cum[w] <= p
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if ((int)cum[mid] <= p) lo = mid; else hi = mid;
-      }
-      unsigned sbits = sbw[lo];
-      for (int r = p - (int)cum[lo]; r > 0; --r) sbits &= sbits - 1;
-      b0 = lo * 32 + __ffs(sbits) - 1;
-      c = sweep<false>(H, b0, P, 0, sb, se, sp);
-    }
-    const int inc = warp_incl_scan(c, lane);
-    const int base = n_raw + inc - c;
-    if (c > 0 && base < P.max_vtx) sweep<true>(H, b0, P, base, sb, se, sp);
-    n_raw += __shfl_sync(FULL, inc, 31);
-  }
-  int ns = n_raw;
-  if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
-  __syncwarp();
-  if (lane < ns) {                                         // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
-    const int i = sp[lane];
-    const long long Nm = i > 0 ? H[i - 1] : 0;
-    const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
-    const long long N0 = H[i];
-    const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
-    const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
-    const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
-    zs[lane] = __fmaf_rn(delta, P.dz, zi);
-  }
-  __syncwarp();                                            // histogram is dead from here on
-
-  // ================= a4: association =========================================================
-  int mycnt = 0;
-  for (;;) {
-    if (ns == 0) break;
-    if (lane + 1 < ns) part[lane] = (se[lane] + sb[lane + 1]) / 2;   // bins < part[k] belong to seed <= k
-    __syncwarp();
-    mycnt = 0;
-    for (int i0 = 0; i0 < n; i0 += 32) {
-      const int i = i0 + lane;
-      int s = -1;
-      if (i < n) {
-        const int b = A.trk_vertex[t0 + i];
-        if (b >= 0) {
-          s = 0;
-          for (int k = 0; k + 1 < ns; ++k) s += (b >= part[k]) ? 1 : 0;
-        }
-      }
-      for (int k = 0; k < ns; ++k) {
-        const int c = __popc(__ballot_sync(FULL, s == k));
-        if (lane == k) mycnt += c;
-      }
-    }
-    // "the seed cluster is removed ... and the procedure is repeated" (P:L163): least populated, ties lowest z
-    int key = 0x7fffffff;
-    if (lane < ns) {
-      const int region = zs[lane] < P.z_split ? 1 : 0;
-      if (mycnt < P.min_tracks_seed[region]) key = (mycnt << 6) | lane;
-    }
-    key = __reduce_min_sync(FULL, key);
-    if (key == 0x7fffffff) break;
-    const int worst = key & 63;
-    int nb = 0, ne = 0, np = 0;
-    float nz = 0.0f;
-    const bool mv = lane >= worst && lane + 1 < ns;
-    if (mv) { nb = sb[lane + 1]; ne = se[lane + 1]; np = sp[lane + 1]; nz = zs[lane + 1]; }
-    __syncwarp();
-    if (mv) { sb[lane] = nb; se[lane] = ne; sp[lane] = np; zs[lane] = nz; }
-    --ns;
-    __syncwarp();
-  }
-  // counting sort of the tracks by seed (deterministic: track order is kept inside a seed)
-  {
-    const int c = lane < ns ? mycnt : 0;
-    const int inc = warp_incl_scan(c, lane);
-    if (lane < ns) { cnt[lane] = c; off[lane] = inc - c; cur[lane] = inc - c; }
-    if (lane == 31) off[ns < MAXV ? ns : MAXV] = inc;
-  }
-  __syncwarp();
-  for (int i0 = 0; i0 < n; i0 += 32) {
-    const int i = i0 + lane;
-    int s = -1;
-    if (i < n) {
-      const int b = A.trk_vertex[t0 + i];
-      if (b >= 0 && ns > 0) {
-        s = 0;
-        for (int k = 0; k + 1 < ns; ++k) s += (b >= part[k]) ? 1 : 0;
-      }
-      A.trk_vertex[t0 + i] = s;                           // scratch: seed index, read back in a6
-      if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
-    }
-    const unsigned m = __match_any_sync(FULL, s);
-    const int rank = __popc(m & lanemask_lt());
-    if (s >= 0) sidx[cur[s] + rank] = (uint16_t)i;
-    __syncwarp();
-    if (s >= 0 && rank == 0) cur[s] += __popc(m);
-    __syncwarp();
-  }
-  if (DBG) {
-    if (lane == 0) {
-      if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
-      if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
-    }
-    if (lane < ns) {
-      if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
-      if (A.dbg.seed_bins) {
-        A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
-        A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
-        A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
-      }
-    }
-  }
-
-  // ================= a5: adaptive vertex fit =================================================
-  // Fast path: FIT_G lanes per vertex, tracks register-resident.
-  for (int v0 = 0; v0 < ns; v0 += FIT_VPW) {
-    const int v = v0 + lane / FIT_G, j = lane % FIT_G;
-    const bool vact = v < ns;
-    int m = vact ? cnt[v] : 0;
-    const int o = vact ? off[v] : 0;
+// ---- fit_kernel: a5, FIT_G lanes per seed, flat over the seed records of the batch (R-12) -----
+// Results go to slot (event, seed index) of the vertex arrays; cleanup_kernel compacts them in place.
+__global__ void __launch_bounds__(256, 3) fit_kernel(const __grid_constant__ KParams P,
+                                                     const __grid_constant__ KArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int j = lane % FIT_G, gl = lane / FIT_G;
+  const int total = (int)*A.seed_counter;
+  const int nwarps = (gridDim.x * blockDim.x) >> 5;
+  const int wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  for (int base = wg * FIT_VPW; base < total; base += nwarps * FIT_VPW) {
+    const int g = base + gl;
+    const bool vact = g < total;
+    int4 r = make_int4(0, 0, 0, 0);
+    if (vact) r = __ldg(reinterpret_cast<const int4*>(A.rec) + g);
+    const int e = r.x, k = r.y & 31;
+    int m = r.y >> 5;
+    const float zsv = __int_as_float(r.w);
     const bool big = m > FIT_G * FIT_KF;
     if (big) m = 0;
-    const float zsv = vact ? zs[v] : 0.0f;
+    const int t0 = vact ? __ldg(A.offsets + e) : 0;
     const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
     const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-    // The fit runs in the seed's local frame (x - sx, y - sy, z - zseed): every quantity is O(mm), so fp32
-    // keeps ~1e-7 mm instead of ulp(550 mm) = 6e-5 mm, and the iterates follow the fp64 oracle.
-    float ax = 0.0f, ay = 0.0f, az = 0.0f;
-    float fx[FIT_KF], fy[FIT_KF], fz[FIT_KF], ftx[FIT_KF], fty[FIT_KF], fWx[FIT_KF], fWy[FIT_KF], fw[FIT_KF];
+    Trk T[FIT_KF];
+    float fw[FIT_KF];
+    int mmax = m;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mmax = max(mmax, __shfl_xor_sync(FULL, mmax, o));
+    const int nslot = (mmax + FIT_G - 1) / FIT_G;          // warp-uniform number of register slots in use
 #pragma unroll
     for (int s = 0; s < FIT_KF; ++s) {
       const int t = j + FIT_G * s;
-      fWx[s] = -1.0f; fWy[s] = -1.0f; fw[s] = 0.0f;
-      fx[s] = fy[s] = fz[s] = ftx[s] = fty[s] = 0.0f;
-      if (t < m) {
-        const int g = t0 + (int)sidx[o + t];
-        fx[s] = __ldg(A.x + g) - sx; fy[s] = __ldg(A.y + g) - sy; fz[s] = __ldg(A.z + g) - zsv;
-        ftx[s] = __ldg(A.tx + g); fty[s] = __ldg(A.ty + g);
-        track_weight_matrix(fz[s], __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g),
-                            __ldg(A.var_ty + g), fWx[s], fWy[s]);
-      }
+      T[s].x0 = T[s].y0 = T[s].tx = T[s].ty = T[s].Wx = T[s].Wy = 0.0f;
+      fw[s] = 0.0f;
+      if (t < m) T[s] = load_track(A, t0 + (int)A.sidx[r.z + t], sx, sy, zsv);
     }
+    float ax = 0.0f, ay = 0.0f, az = 0.0f;
     bool run = vact && !big;
     bool sing = false;
     int niter = 0;
-    Sums L;                                                // sums of the last iteration done
-    sums_zero(L);
+    float C[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+    float chi2 = 0.0f, nact = 0.0f;
+#pragma unroll 1
     for (int it = 1; it <= P.max_iter; ++it) {
       Sums S;
       sums_zero(S);
       if (run) {
 #pragma unroll
         for (int s = 0; s < FIT_KF; ++s)
-          fw[s] = track_accum(fx[s], fy[s], fz[s], ftx[s], fty[s], fWx[s], fWy[s], ax, ay, az, P, S);
+          if (s < nslot) fw[s] = track_accum(T[s], ax, ay, az, P, S);
       }
       sums_reduce<FIT_G>(S);
       if (run) {
         float dx, dy, dzs, dchi2;
-        if (!newton_step(S, dx, dy, dzs, dchi2)) {
+        if (!newton_step(S, dx, dy, dzs, dchi2, C)) {
           sing = true; run = false;
         } else {
           ax += dx; ay += dy; az += dzs;
-          L = S; niter = it;
+          chi2 = S.chi2; nact = S.nact; niter = it;
           if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) run = false;
         }
       }
       if (!__any_sync(FULL, run)) break;
     }
     if (vact && !big) {
+      const size_t o = (size_t)e * P.max_vtx + k;
       if (sing) {
-        status |= PV_EVT_SINGULAR_FIT;
-        if (j == 0) reinterpret_cast<int*>(V)[11 * MAXV + v] = -1;
+        if (j == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
       } else {
-        if (j == 0) {
-          float C[6];
-          covariance(L, C);
-          V[0 * MAXV + v] = sx + ax; V[1 * MAXV + v] = sy + ay; V[2 * MAXV + v] = zsv + az;
-#pragma unroll
-          for (int c = 0; c < 6; ++c) V[(3 + c) * MAXV + v] = C[c];
-          V[9 * MAXV + v] = L.chi2;
-          reinterpret_cast<int*>(V)[10 * MAXV + v] = (int)L.nact;
-          reinterpret_cast<int*>(V)[11 * MAXV + v] = niter;
-        }
+        if (j == 0) store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)nact, niter);
 #pragma unroll
         for (int s = 0; s < FIT_KF; ++s) {
           const int t = j + FIT_G * s;
-          if (t < m) A.trk_weight[t0 + (int)sidx[o + t]] = fw[s];
+          if (t < m) A.trk_weight[t0 + (int)A.sidx[r.z + t]] = fw[s];
+        }
+      }
+    }
+    // Seeds with more tracks than the register-resident path holds: the whole warp strides over the track
+    // list and re-reads the tracks (L1-resident) every iteration.
+    unsigned bigm = __ballot_sync(FULL, vact && big && j == 0);
+    while (bigm) {
+      const int src = __ffs(bigm) - 1;
+      bigm &= bigm - 1;
+      const int be = __shfl_sync(FULL, e, src), bk = __shfl_sync(FULL, k, src);
+      const int bm_ = __shfl_sync(FULL, r.y, src) >> 5, bo = __shfl_sync(FULL, r.z, src);
+      const int bt0 = __shfl_sync(FULL, t0, src);
+      const float bz = __shfl_sync(FULL, zsv, src);
+      const float bx = __fmaf_rn(P.beam_tx, bz, P.beam_x), by = __fmaf_rn(P.beam_ty, bz, P.beam_y);
+      float qx = 0.0f, qy = 0.0f, qz = 0.0f;               // current position (local frame)
+      float px = 0.0f, py = 0.0f, pz = 0.0f;               // position the last weights were taken at
+      bool bsing = false;
+      int bit = 0;
+      float bchi2 = 0.0f, bnact = 0.0f;
+#pragma unroll 1
+      for (int it = 1; it <= P.max_iter; ++it) {
+        Sums S;
+        sums_zero(S);
+        for (int t = lane; t < bm_; t += 32) {
+          const Trk U = load_track(A, bt0 + (int)A.sidx[bo + t], bx, by, bz);
+          track_accum(U, qx, qy, qz, P, S);
+        }
+        sums_reduce<32>(S);
+        float dx, dy, dzs, dchi2;
+        if (!newton_step(S, dx, dy, dzs, dchi2, C)) { bsing = true; break; }
+        px = qx; py = qy; pz = qz;
+        qx += dx; qy += dy; qz += dzs;
+        bchi2 = S.chi2; bnact = S.nact; bit = it;
+        if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
+      }
+      const size_t o = (size_t)be * P.max_vtx + bk;
+      if (bsing) {
+        if (lane == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
+      } else {
+        if (lane == 0) store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)bnact, bit);
+        for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration, recomputed
+          const int gt = bt0 + (int)A.sidx[bo + t];
+          const Trk U = load_track(A, gt, bx, by, bz);
+          Sums dummy;
+          sums_zero(dummy);
+          A.trk_weight[gt] = track_accum(U, px, py, pz, P, dummy);
         }
       }
     }
   }
-  // Slow path: vertices with more tracks than the register-resident path holds; the whole warp strides
-  // over the track list and re-reads the tracks (L2-resident) every iteration.
-  for (int v = 0; v < ns; ++v) {
-    const int m = cnt[v];
-    if (m <= FIT_G * FIT_KF) continue;
-    const int o = off[v];
-    const float zsv = zs[v];
-    const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-    float ax = 0.0f, ay = 0.0f, az = 0.0f;                 // local frame, as in the fast path
-    float px = ax, py = ay, pz = az;                       // vertex position the last weights were taken at
-    bool sing = false;
-    int niter = 0;
-    Sums L;
-    sums_zero(L);
-    for (int it = 1; it <= P.max_iter; ++it) {
-      Sums S;
-      sums_zero(S);
-      for (int t = lane; t < m; t += 32) {
-        const int g = t0 + (int)sidx[o + t];
-        const float zl = __ldg(A.z + g) - zsv;
-        float Wx, Wy;
-        track_weight_matrix(zl, __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g), __ldg(A.var_ty + g), Wx, Wy);
-        track_accum(__ldg(A.x + g) - sx, __ldg(A.y + g) - sy, zl, __ldg(A.tx + g), __ldg(A.ty + g), Wx, Wy, ax, ay, az, P, S);
-      }
-      sums_reduce<32>(S);
-      float dx, dy, dzs, dchi2;
-      if (!newton_step(S, dx, dy, dzs, dchi2)) { sing = true; break; }
-      px = ax; py = ay; pz = az;
-      ax += dx; ay += dy; az += dzs;
-      L = S; niter = it;
-      if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
-    }
-    if (sing) {
-      status |= PV_EVT_SINGULAR_FIT;
-      if (lane == 0) reinterpret_cast<int*>(V)[11 * MAXV + v] = -1;
-    } else {
-      if (lane == 0) {
-        float C[6];
-        covariance(L, C);
-        V[0 * MAXV + v] = sx + ax; V[1 * MAXV + v] = sy + ay; V[2 * MAXV + v] = zsv + az;
-        for (int c = 0; c < 6; ++c) V[(3 + c) * MAXV + v] = C[c];
-        V[9 * MAXV + v] = L.chi2;
-        reinterpret_cast<int*>(V)[10 * MAXV + v] = (int)L.nact;
-        reinterpret_cast<int*>(V)[11 * MAXV + v] = niter;
-      }
-      for (int t = lane; t < m; t += 32) {                 // weights of the last iteration, recomputed
-        const int g = t0 + (int)sidx[o + t];
-        const float zl = __ldg(A.z + g) - zsv;
-        float Wx, Wy;
-        track_weight_matrix(zl, __ldg(A.var_x + g), __ldg(A.var_y + g), __ldg(A.var_tx + g), __ldg(A.var_ty + g), Wx, Wy);
-        Sums dummy;
-        sums_zero(dummy);
-        A.trk_weight[g] = track_accum(__ldg(A.x + g) - sx, __ldg(A.y + g) - sy, zl, __ldg(A.tx + g), __ldg(A.ty + g),
-                                      Wx, Wy, px, py, pz, P, dummy);
-      }
-    }
-  }
-  status = __reduce_or_sync(FULL, status);
-  __syncwarp();
+}
 
-  // ================= a6: cleanup (Table 2) =====================================================
-  const int* Vi = reinterpret_cast<const int*>(V);
-  unsigned alive = 0;                                      // bit k: seed k still a vertex candidate
-  {
-    const bool ok = lane < ns && Vi[11 * MAXV + lane] >= 0;
-    alive = __ballot_sync(FULL, ok);
+// ---- cleanup_kernel: a6, one warp per event (Table 2, R-9) ------------------------------------
+// Lane k holds seed k of the event (position, covariance, ... as fit_kernel left them in slot k of the vertex
+// arrays), the duplicate sweep runs on shuffles, survivors are compacted in place in z order, and every
+// track gets its final vertex index (weight 0 when it has none).
+template <bool DBG>
+__global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KParams P,
+                                                      const __grid_constant__ KArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (e >= A.n_events) return;
+  const int ns = A.n_vtx[e];                               // seeds of the event (seed_kernel)
+  const int t0 = __ldg(A.offsets + e);
+  const int n = __ldg(A.offsets + e + 1) - t0;
+  const size_t ev = (size_t)e * P.max_vtx;
+  float vp[3] = {0.0f, 0.0f, 0.0f}, vc[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+  float vchi2 = 0.0f;
+  int vntrk = 0, vniter = -1;
+  if (lane < ns) {
+    const size_t o = ev + lane;
+    vniter = A.vtx_niter[o];
+    if (vniter >= 0) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) vp[c] = A.vtx_pos[o * 3 + c];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) vc[c] = A.vtx_cov[o * 6 + c];
+      vchi2 = A.vtx_chi2[o]; vntrk = A.vtx_ntracks[o];
+    }
   }
+  const unsigned alive = __ballot_sync(FULL, lane < ns && vniter >= 0);
+  // duplicate removal: greedy sweep in z order; duplicate iff dz^2 / (Czz_v + Czz_s) < merge_ratio; the one
+  // "with fewer associated tracks" is rejected, ties keep the lower z.
   unsigned merged = 0;
   {
-    // duplicate removal: greedy sweep in z order; duplicate iff dz^2 / (Czz_v + Czz_s) < merge_ratio; the one
-    // "with fewer associated tracks" is rejected, ties keep the lower z (R-9).  Every lane runs the same
-    // short serial loop on broadcast shared-memory reads.
     int s = -1;
-    for (int v = 0; v < ns; ++v) {
-      if (!((alive >> v) & 1u)) continue;
-      if (s < 0) { s = v; continue; }
-      const float dzv = V[2 * MAXV + v] - V[2 * MAXV + s];
-      const float ratio = dzv * dzv / (V[8 * MAXV + v] + V[8 * MAXV + s]);
-      if (ratio < P.merge_ratio) {
-        if (Vi[10 * MAXV + v] > Vi[10 * MAXV + s]) { merged |= 1u << s; s = v; }
-        else merged |= 1u << v;
-      } else {
-        s = v;
+    float zs_ = 0.0f, cs_ = 0.0f;
+    int ns_ = 0;
+    unsigned rest = alive;
+    while (rest) {
+      const int v = __ffs(rest) - 1;
+      rest &= rest - 1;
+      const float zv = __shfl_sync(FULL, vp[2], v), cv = __shfl_sync(FULL, vc[5], v);
+      const int nv = __shfl_sync(FULL, vntrk, v);
+      bool take = true;
+      if (s >= 0) {
+        const float dzv = zv - zs_;
+        const float ratio = dzv * dzv / (cv + cs_);
+        if (ratio < P.merge_ratio) {
+          if (nv > ns_) merged |= 1u << s;
+          else { merged |= 1u << v; take = false; }
+        }
       }
+      if (take) { s = v; zs_ = zv; cs_ = cv; ns_ = nv; }
     }
   }
   int fate = -9;
@@ -679,13 +867,12 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
     if (!((alive >> lane) & 1u)) fate = -1;
     else if ((merged >> lane) & 1u) fate = -2;
     else {
-      const float vx = V[0 * MAXV + lane], vy = V[1 * MAXV + lane], vz = V[2 * MAXV + lane];
-      const int region = vz < P.z_split ? 1 : 0;
-      if (Vi[10 * MAXV + lane] < P.min_tracks_pv[region]) fate = -3;        // Table 2 "Min. tracks in the PV"
+      const int region = vp[2] < P.z_split ? 1 : 0;
+      if (vntrk < P.min_tracks_pv[region]) fate = -3;                       // Table 2 "Min. tracks in the PV"
       else {
         keep = true;
         if (region == 0) {
-          const float dx = vx - fmaf(P.beam_tx, vz, P.beam_x), dy = vy - fmaf(P.beam_ty, vz, P.beam_y);
+          const float dx = vp[0] - fmaf(P.beam_tx, vp[2], P.beam_x), dy = vp[1] - fmaf(P.beam_ty, vp[2], P.beam_y);
           if (fmaf(dx, dx, dy * dy) > P.max_beam_dist2) { keep = false; fate = -4; }
         }
       }
@@ -693,33 +880,27 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
   }
   const unsigned kept = __ballot_sync(FULL, keep);
   const int myidx = __popc(kept & lanemask_lt());
-  if (keep) {
-    fate = myidx;
-    const size_t o = ev + myidx;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) A.vtx_pos[o * 3 + c] = V[c * MAXV + lane];
-#pragma unroll
-    for (int c = 0; c < 6; ++c) A.vtx_cov[o * 6 + c] = V[(3 + c) * MAXV + lane];
-    A.vtx_chi2[o] = V[9 * MAXV + lane];
-    A.vtx_ntracks[o] = Vi[10 * MAXV + lane];
-    A.vtx_niter[o] = Vi[11 * MAXV + lane];
-  }
-  if (lane == 0) {
-    A.n_vtx[e] = __popc(kept);
-    A.event_status[e] = status;
-  }
   if (DBG && lane < ns) {
     const size_t o = ev + lane;
-    const bool fitted = (alive >> lane) & 1u;
-    if (A.dbg.seed_niter) A.dbg.seed_niter[o] = Vi[11 * MAXV + lane];
-    if (A.dbg.seed_fate) A.dbg.seed_fate[o] = fate;
-    if (fitted) {
-      if (A.dbg.seed_pos) for (int c = 0; c < 3; ++c) A.dbg.seed_pos[o * 3 + c] = V[c * MAXV + lane];
-      if (A.dbg.seed_cov) for (int c = 0; c < 6; ++c) A.dbg.seed_cov[o * 6 + c] = V[(3 + c) * MAXV + lane];
-      if (A.dbg.seed_chi2) A.dbg.seed_chi2[o] = V[9 * MAXV + lane];
-      if (A.dbg.seed_ntrk) A.dbg.seed_ntrk[o] = Vi[10 * MAXV + lane];
+    if (A.dbg.seed_niter) A.dbg.seed_niter[o] = vniter;
+    if (A.dbg.seed_fate) A.dbg.seed_fate[o] = keep ? myidx : fate;
+    if (vniter >= 0) {
+      if (A.dbg.seed_pos) for (int c = 0; c < 3; ++c) A.dbg.seed_pos[o * 3 + c] = vp[c];
+      if (A.dbg.seed_cov) for (int c = 0; c < 6; ++c) A.dbg.seed_cov[o * 6 + c] = vc[c];
+      if (A.dbg.seed_chi2) A.dbg.seed_chi2[o] = vchi2;
+      if (A.dbg.seed_ntrk) A.dbg.seed_ntrk[o] = vntrk;
     }
   }
+  __syncwarp();                                            // every lane has read its slot: compact in place
+  if (keep) {
+    const size_t o = ev + myidx;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) A.vtx_pos[o * 3 + c] = vp[c];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) A.vtx_cov[o * 6 + c] = vc[c];
+    A.vtx_chi2[o] = vchi2; A.vtx_ntracks[o] = vntrk; A.vtx_niter[o] = vniter;
+  }
+  if (lane == 0) A.n_vtx[e] = __popc(kept);
   // final per-track outputs; tracks of rejected vertices are released (R-9)
   for (int i = lane; i < n; i += 32) {
     const int s = A.trk_vertex[t0 + i];
@@ -727,35 +908,6 @@ __device__ void process_event(const int e, const KParams& P, const KArgs& A, uns
     if (s >= 0 && ((kept >> s) & 1u)) vtx = __popc(kept & ((1u << s) - 1u));
     A.trk_vertex[t0 + i] = vtx;
     if (vtx < 0) A.trk_weight[t0 + i] = 0.0f;
-  }
-  __syncwarp();
-  // re-zero region 0 for the next event
-  {
-    int4* Z = reinterpret_cast<int4*>(wsm);
-    const int nq = P.region0_words >> 2;
-    for (int i = lane; i < nq; i += 32) Z[i] = make_int4(0, 0, 0, 0);
-  }
-  __syncwarp();
-}
-
-template <bool DBG>
-__global__ void __launch_bounds__(512, 1) pv_find_kernel(const __grid_constant__ KParams P,
-                                                         const __grid_constant__ KArgs A) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  unsigned char* wsm = smem_raw + (size_t)warp * P.warp_smem_bytes;
-  {
-    int4* Z = reinterpret_cast<int4*>(wsm);
-    const int nq = P.region0_words >> 2;
-    for (int i = lane; i < nq; i += 32) Z[i] = make_int4(0, 0, 0, 0);
-  }
-  __syncwarp();
-  for (;;) {
-    int e = 0;
-    if (lane == 0) e = (int)atomicAdd(A.counter, 1u);
-    e = __shfl_sync(FULL, e, 0);
-    if (e >= A.n_events) break;
-    process_event<DBG>(e, P, A, wsm, lane);
   }
 }
 

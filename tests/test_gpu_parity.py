@@ -144,7 +144,7 @@ def test_full_size_throughput_config(pv, oracle):
     p = pv.default_params()
     got = pv.find(data, p)
     info = pv.last_launch_info()
-    assert info["n_kernels"] == 1 and info["grid"] >= 100
+    assert info["n_kernels"] == 3 and info["grid"] >= 100
     ref = oracle.find(data, oracle.default_params(), debug=True, trace=True, n_threads=8)
     ref_nodebug = {k: v for k, v in ref.items() if k != "debug"}
     rep = compare.compare(got, ref_nodebug, data["offsets"], p)
