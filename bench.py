@@ -3,8 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1] [--events E]
 
-A step is one pass of the whole hot path (a1..a6, one pv_find call = one kernel launch) over one batch of
-synthetic events: configs[1] of BASELINE.json (100 000 events, mu = 5 pp + SMOG2, seed 2), resident in HBM.
+A step is one pass of the whole hot path (a1..a6, one pv_find call = three kernel launches: seed, fit, cleanup)
+over one batch of synthetic events: configs[1] of BASELINE.json (100 000 events, mu = 5 pp + SMOG2, seed 2), resident in HBM.
 Rank 0 prints ONE JSON line.  Under torchrun (N > 1) every rank processes its own batch of the same model
 (different generator blocks), no data-path collective: events are independent -> "scaling": "weak".
 
@@ -85,12 +85,26 @@ def gen_batch(cfg_idx: int, n_events, rank: int):
     return events.generate(m), m
 
 
+KERNELS = ("seed_kernel", "fit_kernel", "cleanup_kernel")
+
+
 def algorithmic_bytes(data, n_vtx_total: int) -> int:
     """SURVEY.md 8(d) / DESIGN.md: compulsory HBM traffic of one pass: 9 fp32 inputs + offsets read,
     trk_vertex + trk_weight written, 48 B per vertex (pos 12, cov 24, chi2 4, ntrk 4, niter 4), n_vtx + status."""
     T = int(data["offsets"][-1])
     E = int(data["offsets"].size - 1)
     return T * 36 + (E + 1) * 4 + T * 8 + n_vtx_total * 48 + E * 8
+
+
+def algorithmic_bytes_by_kernel(data, n_vtx_total: int):
+    """The same compulsory bytes attributed to the kernel that first reads / last writes them:
+    seed reads the 6 arrays of Eq. 1 / Eq. 3 and the offsets; fit reads the other 3 (var_y, var_tx, var_ty) and
+    writes trk_weight; cleanup writes the vertices, n_vtx, status and trk_vertex.  Intermediate records (seed
+    records, sorted track lists, per-seed fit slots) and re-reads are NOT algorithmic."""
+    T = int(data["offsets"][-1])
+    E = int(data["offsets"].size - 1)
+    return {"seed_kernel": T * 24 + (E + 1) * 4, "fit_kernel": T * 12 + T * 4,
+            "cleanup_kernel": T * 4 + n_vtx_total * 48 + E * 8}
 
 
 def run_oracle(data, n_threads: int):
@@ -178,7 +192,18 @@ def main_ours(args):
     sampler.sample()
     sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
-    last_kernel_ms = float(L.pv_kernel_time_ms())
+    # per-kernel durations: CUDA events recorded by the library on the launching stream around each of the
+    # three launches, read back after every step of a second pass over the same K steps (not part of `value`)
+    import ctypes
+    kt = np.zeros((args.steps, len(KERNELS)))
+    buf = (ctypes.c_float * len(KERNELS))()
+    for i in range(args.steps):
+        with torch.cuda.stream(stream):
+            batch.find(stream)
+        stream.synchronize()
+        L.pv_kernel_times_ms(buf, len(KERNELS))
+        kt[i] = list(buf)
+    kernel_ms = kt.mean(axis=0)
     L.pv_kernel_timing(0)
     info = pv.last_launch_info()
     if world > 1:
@@ -219,17 +244,21 @@ def main_ours(args):
     value = world * E * args.steps / (ms_total * 1e-3)
     peak, peak_src = hbm_peak()
     alg = algorithmic_bytes(data, n_vtx_total)
-    kernel_ms = ms_step                      # a step is ONE launch of pv_find_kernel (+ a 16-byte memset)
-    achieved = alg / (kernel_ms * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    alg_k = algorithmic_bytes_by_kernel(data, n_vtx_total)
+    assert sum(alg_k.values()) == alg
+    traffic_k = {}
+    tpath = os.path.join(ROOT, "profiles", "dram_traffic.csv")      # copied from the committed ncu --set full capture
     if os.path.exists(tpath):
-        try:
-            tj = json.load(open(tpath))
-            if tj.get("events") == E and tj.get("config") == args.config:
-                traffic = tj.get("dram_bytes_per_launch")
-        except Exception:
-            pass
+        import csv
+        for row in csv.DictReader(open(tpath)):
+            if int(row["config"]) == args.config and int(row["events"]) == E:
+                traffic_k[row["kernel"]] = int(row["dram_bytes_per_launch"])
+    ksum = float(kernel_ms.sum())
+    kernels = [{"name": n, "ms": float(kernel_ms[i]), "share": float(kernel_ms[i] / ksum),
+                "algorithmic_bytes": alg_k[n], "achieved_gbs": alg_k[n] / (kernel_ms[i] * 1e-3) / 1e9,
+                "traffic": traffic_k.get(n)} for i, n in enumerate(KERNELS)]
+    dom = max(kernels, key=lambda k: k["ms"])
+    achieved = dom["achieved_gbs"]
 
     # ---- cpu_baseline: the oracle, as it stands, on this box's host cores --------------------------------------
     cores = os.cpu_count() or 1
@@ -259,9 +288,12 @@ def main_ours(args):
                 "api": "pv_find_host (pinned host buffers, 4 streams)", "matches_device_path": e2e_ok},
         "gpu_launches": args.steps * info["n_kernels"],
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src, "kernel": "pvk::pv_find_kernel<false>",
-                     "algorithmic_bytes_per_launch": alg, "kernel_ms": kernel_ms, "last_kernel_ms_cuda_events": last_kernel_ms,
-                     "note": "latency/issue-bound path: see DESIGN.md 'Roofline'"},
+                     "traffic": dom["traffic"], "peak_source": peak_src, "kernel": "pvk::" + dom["name"],
+                     "algorithmic_bytes_per_launch": dom["algorithmic_bytes"], "kernel_ms": dom["ms"],
+                     "kernels": kernels,
+                     "path": {"algorithmic_bytes_per_step": alg, "ms_per_step": ms_step,
+                              "achieved": alg / (ms_step * 1e-3) / 1e9, "frac": alg / (ms_step * 1e-3) / 1e9 / peak},
+                     "note": "issue/latency-bound path, not HBM-bound: see DESIGN.md section 8"},
         "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
