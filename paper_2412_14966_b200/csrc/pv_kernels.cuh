@@ -32,20 +32,26 @@ constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
 constexpr int CHUNK = 128;          // tracks per fill chunk: 4 register slots per lane
 constexpr int SLOTS = CHUNK / 32;
+constexpr int UNIT = 8;             // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
+constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
+constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int FIT_G = 8;            // lanes per vertex in the fit
 constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
 constexpr int FIT_KF = 6;           // register-resident tracks per lane (fast path: <= FIT_G*FIT_KF tracks)
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
-constexpr int PROTO_CAP = 512;      // proto-cluster starts of one round of 32 touched words (<= 16 per word)
+constexpr int PROTO_CAP = 512;      // proto-cluster starts of one sweep round (<= 16 per touched word)
 
 // Per-warp shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
-constexpr int SM_BM = 0;                               // unsigned bm[128]     bins above threshold, bit per bin
-constexpr int SM_TOUCHED = SM_BM + MAX_WORDS * 4;      // unsigned touched[4]  histogram words written by the fill
-constexpr int SM_TWL = SM_TOUCHED + 16;                // uint8 twl[128]       list of touched words, ascending
-constexpr int SM_CNT = SM_TWL + MAX_WORDS;             // int cnt[32], cur[32], off[33+3]
-constexpr int SM_SEED = SM_CNT + (32 + 32 + 36) * 4;   // int sb[32], se[32], sp[32]; float zs[32]; int part[32]
-constexpr int SM_STAGE = SM_SEED + 5 * MAXV * 4;       // float4 stage[128] (fill)  /  uint16 protostart[512] (peaks)
-constexpr int SM_TAIL_BYTES = SM_STAGE + CHUNK * 16;
+constexpr int SM_TOUCHED = 0;                          // uint8 tb[128]        histogram words written by the fill
+constexpr int SM_TWL = SM_TOUCHED + MAX_WORDS;         // uint8 twl[128]       list of touched words, ascending
+constexpr int SM_CNT = SM_TWL + MAX_WORDS;             // int cnt[32], cur[32]
+constexpr int SM_SEED = SM_CNT + (32 + 32) * 4;        // int sb[32], se[32], sp[32]; float zs[32]; int part[32]
+constexpr int SM_STAGE = SM_SEED + 5 * MAXV * 4;       // float zp[128], inv[128]; int lonb[128]   (fill)
+constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // uint16 list[256]  (fill); with the stage: protostart[] (peaks)
+constexpr int SM_BINS = SM_LIST + LIST_CAP * 2;        // int16 binsm[256]     central bins of the first 256 tracks
+constexpr int SM_TAIL_BYTES = SM_BINS + BINS_SM * 2;
+static_assert(PROTO_CAP * 2 <= CHUNK * 12 + LIST_CAP * 2, "protostart overlays the fill stage and unit list");
+static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0, "alignment of the vector loads");
 
 struct KParams {
   float z_min, dz, inv_dz, z_split;
@@ -95,10 +101,16 @@ __device__ __forceinline__ unsigned lanemask_lt() {
   return m;
 }
 
-// Fixed-point CDF at the bin edge with float index kf (contract: every op rounded once).
-__device__ __forceinline__ int edge_q(float kf, float zp, float inv, const KParams& P) {
+// Fixed-point CDF at the bin edge with float index kf (contract of DESIGN.md section 3: every op rounded
+// once).  Returns the BITS of c + 8.0f: in [8, 9] one ulp is 2^-20, so the round-to-nearest-even addition is
+// rint(c * 2^20) and the difference of two results is the difference of the two fixed-point values Q.
+// The contract's forced Q = 0 for s <= -1 and Q = 2^20 for s >= 1 are reproduced by clamping s to [-1, 1]: the
+// frozen polynomial gives G(1) = 0x1.000098p-1 > 1/2 in this Horner order, so fma(+-1, G(1), 0.5) saturates to
+// exactly 1 / 0.
+__device__ __forceinline__ int edge_r(float kf, float zp, float inv, const KParams& P) {
   const float e = __fmaf_rn(kf, P.dz, P.z_min);
-  const float s = __fmul_rn(__fsub_rn(e, zp), inv);
+  float s = __fmul_rn(__fsub_rn(e, zp), inv);
+  s = fminf(fmaxf(s, -1.0f), 1.0f);
   const float t = __fmul_rn(s, s);
   float g = 0x1.3e0392p-3f;
   g = __fmaf_rn(g, t, -0x1.862240p-1f);
@@ -107,11 +119,8 @@ __device__ __forceinline__ int edge_q(float kf, float zp, float inv, const KPara
   g = __fmaf_rn(g, t, 0x1.32067cp+1f);
   g = __fmaf_rn(g, t, -0x1.cbf272p+0f);
   g = __fmaf_rn(g, t, 0x1.3331cep+0f);
-  float c = __saturatef(__fmaf_rn(s, g, 0.5f));
-  int q = __float2int_rn(__fmul_rn(c, 1048576.0f));
-  q = (s <= -1.0f) ? 0 : q;
-  q = (s >= 1.0f) ? PV_FIXED_ONE : q;
-  return q;
+  const float c = __saturatef(__fmaf_rn(s, g, 0.5f));
+  return __float_as_int(__fadd_rn(c, 8.0f));
 }
 
 __device__ __forceinline__ int bin_region(int b, const KParams& P) {
@@ -234,8 +243,7 @@ template <bool DBG>
 __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int lane) {
   int* H = reinterpret_cast<int*>(wsm);
   unsigned char* tail = wsm + (size_t)P.region0_words * 4;
-  unsigned* bm = reinterpret_cast<unsigned*>(tail + SM_BM);
-  unsigned* touched = reinterpret_cast<unsigned*>(tail + SM_TOUCHED);
+  uint8_t* tb = reinterpret_cast<uint8_t*>(tail + SM_TOUCHED);
   uint8_t* twl = reinterpret_cast<uint8_t*>(tail + SM_TWL);
   int* cnt = reinterpret_cast<int*>(tail + SM_CNT);
   int* cur = cnt + 32;
@@ -244,8 +252,12 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   int* sp = se + MAXV;
   float* zs = reinterpret_cast<float*>(sp + MAXV);
   int* part = reinterpret_cast<int*>(zs + MAXV);
-  float4* stage = reinterpret_cast<float4*>(tail + SM_STAGE);
-  uint16_t* protostart = reinterpret_cast<uint16_t*>(tail + SM_STAGE);   // overlay: the stage is dead after the fill
+  float* st_zp = reinterpret_cast<float*>(tail + SM_STAGE);
+  float* st_inv = st_zp + CHUNK;
+  int* st_lonb = reinterpret_cast<int*>(st_inv + CHUNK);
+  uint16_t* list = reinterpret_cast<uint16_t*>(tail + SM_LIST);
+  uint16_t* protostart = reinterpret_cast<uint16_t*>(tail + SM_STAGE);   // overlay: stage and list are dead after the fill
+  int16_t* binsm = reinterpret_cast<int16_t*>(tail + SM_BINS);
 
   const int t0 = __ldg(A.offsets + e);
   const int n = __ldg(A.offsets + e + 1) - t0;
@@ -266,17 +278,12 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   }
 
   // ================= a1 + a2: projection (Eq. 1, Eq. 3) and histogram fill ===================
-  // Chunks of CHUNK tracks, SLOTS per lane.  Within a chunk the histogrammed tracks are counting-sorted by
-  // window length (bins), so the 32 lanes of a fill pass run loops of (nearly) the same length.  The adds are
-  // integer, so the order changes nothing.
-  const bool one_chunk = n <= CHUNK;
-  int binr[SLOTS];                                         // central bins of a single-chunk event stay in registers
-#pragma unroll
-  for (int s = 0; s < SLOTS; ++s) binr[s] = -1;
+  // Chunks of CHUNK tracks, SLOTS per lane.  The window of a histogrammed track is cut into units of UNIT bins;
+  // the units of the chunk form one flat list, and a fill pass gives every lane one unit: UNIT + 1 independent
+  // CDF edges (instruction-level parallelism instead of one dependent Horner chain per lane) and UNIT
+  // predicated integer adds.  The adds are integers, so the order changes nothing.
 #pragma unroll 1
   for (int c0 = 0; c0 < n; c0 += CHUNK) {
-    float zp[SLOTS], inv[SLOTS], kf[SLOTS];
-    int nb[SLOTS];
     float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
 #pragma unroll
     for (int s = 0; s < SLOTS; ++s) {                      // all loads first (24 in flight per lane)
@@ -285,15 +292,15 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
       lx[s] = __ldg(A.x + t); ly[s] = __ldg(A.y + t); lz[s] = __ldg(A.z + t);
       ltx[s] = __ldg(A.tx + t); lty[s] = __ldg(A.ty + t); lvx[s] = __ldg(A.var_x + t);
     }
-    cnt[lane] = 0;
-    __syncwarp();
+    int nun[SLOTS];                                        // fill units of my tracks
+    int myunits = 0;
 #pragma unroll
     for (int s = 0; s < SLOTS; ++s) {
       const int i = c0 + s * 32 + lane;
-      nb[s] = 0; zp[s] = 0.0f; inv[s] = 0.0f; kf[s] = 0.0f;
+      nun[s] = 0;
       if (i < n) {
         const Proj r = project(lx[s], ly[s], lz[s], ltx[s], lty[s], lvx[s], P);
-        if (one_chunk) binr[s] = r.bin; else A.trk_vertex[t0 + i] = r.bin;   // large events: HBM scratch, read back in a4
+        if (i < BINS_SM) binsm[i] = (int16_t)r.bin; else A.trk_vertex[t0 + i] = r.bin;   // large events: HBM scratch, read back in a4
         if (DBG) {
           if (A.dbg.z_poca) A.dbg.z_poca[t0 + i] = r.zp;
           if (A.dbg.sigma_poca) A.dbg.sigma_poca[t0 + i] = r.sg;
@@ -306,51 +313,55 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
           const float fb2 = floorf((r.zp + w3 - P.z_min) * P.inv_dz + P.win_eps) + 1.0f;
           const int lo = (int)fmaxf(fa, 0.0f);
           const int hi = (int)fminf(fb2, (float)P.nbins);
-          nb[s] = hi - lo; zp[s] = r.zp; inv[s] = r.inv; kf[s] = (float)lo;
-          if (nb[s] > 0) atomicAdd(&cnt[min(nb[s], 31)], 1);
+          const int nb = hi - lo;
+          if (nb > 0) {
+            nun[s] = (nb + UNIT - 1) / UNIT;
+            st_zp[s * 32 + lane] = r.zp; st_inv[s * 32 + lane] = r.inv; st_lonb[s * 32 + lane] = lo | (nb << 12);
+          }
         }
       }
+      myunits += nun[s];
     }
-    __syncwarp();
-    int total;
-    {
-      const int c = cnt[lane];
-      const int inc = warp_incl_scan(c, lane);
-      total = __shfl_sync(FULL, inc, 31);
+    const int incl = warp_incl_scan(myunits, lane);
+    const int total = __shfl_sync(FULL, incl, 31);
+#pragma unroll 1
+    for (int R = 0; R < total; R += LIST_CAP) {            // one round unless the chunk holds very wide tracks
       __syncwarp();
-      cnt[lane] = inc - c;                                 // first staging slot of each window-length class
-    }
-    __syncwarp();
+      {
+        int g = incl - myunits - R;                        // list position of my first unit in this round
 #pragma unroll
-    for (int s = 0; s < SLOTS; ++s) {
-      if (nb[s] > 0) {
-        const int pos = atomicAdd(&cnt[min(nb[s], 31)], 1);
-        stage[pos] = make_float4(zp[s], inv[s], kf[s], __int_as_float(nb[s]));
+        for (int s = 0; s < SLOTS; ++s) {
+          const int tk = s * 32 + lane;
+#pragma unroll 1
+          for (int u = 0; u < nun[s]; ++u, ++g)
+            if ((unsigned)g < (unsigned)LIST_CAP) list[g] = (uint16_t)(tk | (u << 7));
+        }
       }
-    }
-    __syncwarp();
+      __syncwarp();
+      const int nl = min(total - R, LIST_CAP);
 #pragma unroll 1
-    for (int p0 = 0; p0 < total; p0 += 32) {
-      const int idx = p0 + lane;
-      float4 st = make_float4(0.0f, 0.0f, 0.0f, __int_as_float(0));
-      if (idx < total) st = stage[idx];
-      const int nbl = __float_as_int(st.w);
-      const int b0 = (int)st.z;
-      if (nbl > 0) {                                       // histogram words this track writes
-        const int w1 = (b0 + nbl - 1) >> 5;
-#pragma unroll 1
-        for (int w = b0 >> 5; w <= w1; ++w) atomicOr(&touched[w >> 5], 1u << (w & 31));
-      }
-      const int mx = __reduce_max_sync(FULL, nbl);
-      float kfl = st.z;
-      int q0 = edge_q(kfl, st.x, st.y, P);
-#pragma unroll 1
-      for (int j = 0; j < mx; ++j) {
-        kfl += 1.0f;
-        const int q1 = edge_q(kfl, st.x, st.y, P);
-        const int d = q1 - q0;
-        if (j < nbl && d != 0) atomicAdd(&H[b0 + j], d);
-        q0 = q1;
+      for (int p0 = 0; p0 < nl; p0 += 32) {
+        const int idx = p0 + lane;
+        const bool act = idx < nl;
+        const int ent = list[act ? idx : nl - 1];
+        const int tk = ent & 127, u = ent >> 7;
+        const float zp = st_zp[tk], inv = st_inv[tk];
+        const int lonb = st_lonb[tk];
+        const int b0 = (lonb & 0xfff) + u * UNIT;
+        const int rem = act ? (lonb >> 12) - u * UNIT : 0;   // bins of this unit: min(rem, UNIT)
+        if (act) {                                         // histogram words this unit writes
+          tb[b0 >> 5] = 1;
+          tb[(b0 + min(rem, UNIT) - 1) >> 5] = 1;
+        }
+        const float kf = (float)b0;
+        int r[UNIT + 1];
+#pragma unroll
+        for (int j = 0; j <= UNIT; ++j) r[j] = edge_r(kf + (float)j, zp, inv, P);
+#pragma unroll
+        for (int j = 0; j < UNIT; ++j) {
+          const int d = r[j + 1] - r[j];
+          if (j < rem && d != 0) atomicAdd(&H[b0 + j], d);
+        }
       }
     }
     __syncwarp();
@@ -361,70 +372,67 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
 
   // ================= a3: peak search and seed position (Eq. 4-5) ==============================
   // List of the touched histogram words, ascending; only these can hold bins above the threshold.
-  int ntw = 0;
+  int ntw;
+  {
+    const unsigned f4 = reinterpret_cast<const unsigned*>(tb)[lane];   // flags of words 4 lane .. 4 lane + 3
+    const int c = (f4 & 1u) + ((f4 >> 8) & 1u) + ((f4 >> 16) & 1u) + ((f4 >> 24) & 1u);
+    const int inc = warp_incl_scan(c, lane);
+    ntw = __shfl_sync(FULL, inc, 31);
+    int o = inc - c;
 #pragma unroll
-  for (int q = 0; q < MAX_WORDS / 32; ++q) {
-    const unsigned m = touched[q];
-    if ((m >> lane) & 1u) twl[ntw + __popc(m & lanemask_lt())] = (uint8_t)(q * 32 + lane);
-    ntw += __popc(m);
-  }
-  __syncwarp();
-#pragma unroll 1
-  for (int i = 0; i < ntw; ++i) {
-    const int w = twl[i];
-    const unsigned m = __ballot_sync(FULL, w * 32 + lane < P.nbins && H[w * 32 + lane] > P.T_bin);
-    if (lane == 0) bm[w] = m;
+    for (int q = 0; q < 4; ++q)
+      if ((f4 >> (8 * q)) & 1u) twl[o++] = (uint8_t)(4 * lane + q);
+    __syncwarp();
+    reinterpret_cast<unsigned*>(tb)[lane] = 0;             // clean for the next event
   }
   __syncwarp();
 
   int n_raw = 0;
+  {
+    int i = 0;
+    int prev_w = -2;
+    unsigned prev_m = 0;
 #pragma unroll 1
-  for (int r0 = 0; r0 < ntw; r0 += 32) {                   // rounds of 32 touched words (one round in practice)
-    int n_proto;
-    {
-      unsigned sbits = 0;
-      int w = 0;
-      if (r0 + lane < ntw) {
-        w = twl[r0 + lane];
-        const unsigned m = bm[w];
-        const unsigned prev = w > 0 ? (bm[w - 1] >> 31) : 0u;
-        sbits = m & ~((m << 1) | prev);                    // first bin of each run of bins above threshold
+    while (i < ntw) {                                      // rounds of <= PROTO_CAP proto-clusters (one in practice)
+      int n_proto = 0;
+#pragma unroll 1
+      for (; i < ntw && n_proto + 16 <= PROTO_CAP; ++i) {  // a word of 32 bins starts at most 16 runs
+        const int w = twl[i];
+        const int b = w * 32 + lane;
+        const unsigned m = __ballot_sync(FULL, b < P.nbins && H[b] > P.T_bin);
+        const unsigned carry = (prev_w == w - 1) ? (prev_m >> 31) : 0u;
+        const unsigned starts = m & ~((m << 1) | carry);   // first bin of each run of bins above threshold
+        if ((starts >> lane) & 1u) protostart[n_proto + __popc(starts & lanemask_lt())] = (uint16_t)b;
+        n_proto += __popc(starts);
+        prev_w = w; prev_m = m;
       }
-      const int c = __popc(sbits);
-      const int inc = warp_incl_scan(c, lane);
-      n_proto = __shfl_sync(FULL, inc, 31);
-      int o = inc - c;
-      while (sbits) {
-        protostart[o++] = (uint16_t)(w * 32 + __ffs(sbits) - 1);
-        sbits &= sbits - 1;
-      }
-    }
-    __syncwarp();
+      __syncwarp();
 #pragma unroll 1
-    for (int p0 = 0; p0 < n_proto; p0 += 32) {             // one lane per proto-cluster
-      const int p = p0 + lane;
-      const bool act = p < n_proto;
-      const int b0 = act ? (int)protostart[p] : 0;
-      Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
-      int c = 0, base = 0;
+      for (int p0 = 0; p0 < n_proto; p0 += 32) {           // one lane per proto-cluster
+        const int p = p0 + lane;
+        const bool act = p < n_proto;
+        const int b0 = act ? (int)protostart[p] : 0;
+        Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
+        int c = 0, base = 0;
 #pragma unroll 1
-      for (int rep = 0; rep < 2; ++rep) {                  // rep 1 (rare): proto-clusters with three or more seeds
-        const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
-        if (!__any_sync(FULL, run)) break;
-        if (run) {
-          const int cc = sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
-          if (rep == 0) c = cc;
-        }
-        if (rep == 0) {
-          const int inc = warp_incl_scan(c, lane);
-          base = n_raw + inc - c;
-          if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
-          if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
-          n_raw += __shfl_sync(FULL, inc, 31);
+        for (int rep = 0; rep < 2; ++rep) {                // rep 1 (rare): proto-clusters with three or more seeds
+          const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
+          if (!__any_sync(FULL, run)) break;
+          if (run) {
+            const int cc = sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+            if (rep == 0) c = cc;
+          }
+          if (rep == 0) {
+            const int inc = warp_incl_scan(c, lane);
+            base = n_raw + inc - c;
+            if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
+            if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
+            n_raw += __shfl_sync(FULL, inc, 31);
+          }
         }
       }
+      __syncwarp();
     }
-    __syncwarp();
   }
   int ns = n_raw;
   if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
@@ -443,31 +451,26 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   // the histogram is dead from here on: clear what this event touched for the next one
 #pragma unroll 1
   for (int i = 0; i < ntw; ++i) H[(int)twl[i] * 32 + lane] = 0;
-#pragma unroll 1
-  for (int i = lane; i < ntw; i += 32) bm[twl[i]] = 0;
-  if (lane < MAX_WORDS / 32) touched[lane] = 0;
 
   // ================= a4: association (R-11) ====================================================
-  // Central bins: single-chunk events keep them in shared memory (int16, behind the proto-cluster list),
-  // larger events read them back from the trk_vertex scratch.
-  int16_t* binsm = reinterpret_cast<int16_t*>(tail + SM_STAGE + PROTO_CAP * 2);
-  if (one_chunk) {
-#pragma unroll
-    for (int s = 0; s < SLOTS; ++s) binsm[s * 32 + lane] = (int16_t)binr[s];
-  }
+  // Central bins: the first BINS_SM tracks keep them in shared memory, the rest read them back from the
+  // trk_vertex scratch.  part[] is padded with INT_MAX to whole groups of four.
   auto seed_of = [&](int i) -> int {                       // seed index of track i, -1 = none
     if (i >= n || ns == 0) return -1;
-    const int b = one_chunk ? (int)binsm[i] : A.trk_vertex[t0 + i];
+    const int b = i < BINS_SM ? (int)binsm[i] : A.trk_vertex[t0 + i];
     if (b < 0) return -1;
     int s = 0;
 #pragma unroll 1
-    for (int k = 0; k + 1 < ns; ++k) s += (b >= part[k]) ? 1 : 0;   // bins < part[k] belong to seed <= k
+    for (int k = 0; k + 1 < ns; k += 4) {                  // bins < part[k] belong to seed <= k
+      const int4 pk = *reinterpret_cast<const int4*>(part + k);
+      s += (b >= pk.x ? 1 : 0) + (b >= pk.y ? 1 : 0) + (b >= pk.z ? 1 : 0) + (b >= pk.w ? 1 : 0);
+    }
     return s;
   };
   for (;;) {
     if (ns == 0) break;
     __syncwarp();
-    if (lane + 1 < ns) part[lane] = (se[lane] + sb[lane + 1]) / 2;
+    part[lane] = lane + 1 < ns ? (se[lane] + sb[lane + 1]) / 2 : 0x7fffffff;
     cnt[lane] = 0;
     __syncwarp();
 #pragma unroll 1
@@ -557,7 +560,7 @@ __global__ void __launch_bounds__(512, 1) seed_kernel(const __grid_constant__ KP
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   unsigned char* wsm = smem_raw + (size_t)warp * P.warp_smem_bytes;
   {
-    int4* Z = reinterpret_cast<int4*>(wsm);                // histogram, bitmap and touched words start at zero
+    int4* Z = reinterpret_cast<int4*>(wsm);                // histogram and touched-word flags start at zero
     const int nq = (P.region0_words * 4 + SM_TWL) >> 4;
 #pragma unroll 1
     for (int i = lane; i < nq; i += 32) Z[i] = make_int4(0, 0, 0, 0);
