@@ -106,11 +106,12 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->warp_smem_bytes = r0 + pvk::SM_TAIL_BYTES;
 }
 
-// Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | sidx, 2 B per track.
+// Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | fit-ready track records,
+// 32 B per track, sorted by seed.
 constexpr size_t WS_COUNTERS = 256;
 size_t ws_rec_bytes(int n_events, int max_vtx) { return (size_t)n_events * (size_t)max_vtx * sizeof(pvk::SeedRec); }
 size_t ws_bytes(int n_events, long long n_tracks, int max_vtx) {
-  return WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + (((size_t)n_tracks * 2 + 15) / 16) * 16 + 16;
+  return WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + (size_t)n_tracks * 32 + 16;
 }
 
 
@@ -157,7 +158,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   }
   if (di->fit_blocks_per_sm == 0) {
     int nb = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel, 256, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel, pvk::FIT_BLOCK, 0));
     di->fit_blocks_per_sm = nb > 0 ? nb : 1;
   }
   g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * 32; g_last_smem = smem;
@@ -174,7 +175,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.evt_counter = reinterpret_cast<unsigned int*>(ws);
   ka.seed_counter = reinterpret_cast<unsigned int*>(ws + 16);
   ka.rec = reinterpret_cast<pvk::SeedRec*>(ws + WS_COUNTERS);
-  ka.sidx = reinterpret_cast<uint16_t*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
+  ka.ftrk = reinterpret_cast<float4*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
   if (dbg) ka.dbg = *dbg;
 
   const bool timing = g_timing != 0;
@@ -190,13 +191,13 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   else pvk::seed_kernel<false><<<grid, warps * 32, smem, stream>>>(kp, ka);
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
-  // a5: 8 lanes per seed, grid-stride over the seed records
+  // a5: FIT_G lanes per seed, warps stride over windows of 32 seed records
   {
     long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm;
-    const long long most = ((long long)n_events * params->max_vtx_per_event + 31) / 32;   // 32 seeds per 256-thread CTA
+    const long long most = ((long long)n_events * params->max_vtx_per_event + pvk::FIT_BLOCK - 1) / pvk::FIT_BLOCK;
     if (fit_grid > most) fit_grid = most;
     if (fit_grid < 1) fit_grid = 1;
-    pvk::fit_kernel<<<(int)fit_grid, 256, 0, stream>>>(kp, ka);
+    pvk::fit_kernel<<<(int)fit_grid, pvk::FIT_BLOCK, 0, stream>>>(kp, ka);
     CK(cudaGetLastError());
   }
   if (timing) CK(cudaEventRecord(g_ev[2], stream));

@@ -35,9 +35,11 @@ constexpr int SLOTS = CHUNK / 32;
 constexpr int UNIT = 8;             // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
-constexpr int FIT_G = 8;            // lanes per vertex in the fit
+constexpr int FIT_G = 4;            // lanes per vertex in the fit
 constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
-constexpr int FIT_KF = 6;           // register-resident tracks per lane (fast path: <= FIT_G*FIT_KF tracks)
+constexpr int FIT_KF = 8;           // register-resident tracks per lane (fast path: <= FIT_G*FIT_KF tracks)
+constexpr int FIT_BLOCK = 128;      // threads per CTA of fit_kernel (warps are autonomous)
+constexpr int FIT_MIN_BLOCKS = 4;   // CTAs per SM the register budget is held to
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
 constexpr int PROTO_CAP = 512;      // proto-cluster starts of one sweep round (<= 16 per touched word)
 
@@ -75,7 +77,7 @@ struct KParams {
 struct SeedRec {
   int e;                         // event
   int k_cnt;                     // seed index within the event | track count << 5
-  int begin;                     // first entry of the seed's track list in sidx[] (absolute)
+  int begin;                     // first record of the seed's tracks in ftrk[] (absolute)
   float z;                       // z_seed (Eq. 4)
 };
 
@@ -91,7 +93,7 @@ struct KArgs {
   unsigned int* evt_counter;     // workspace: next event of the persistent seed kernel
   unsigned int* seed_counter;    // workspace: seed records written so far
   SeedRec* rec;                  // workspace: [n_events * max_vtx]
-  uint16_t* sidx;                // workspace: [T] track indices (local to the event) sorted by seed
+  float4* ftrk;                  // workspace: [T][2] fit-ready track records sorted by seed
   pv_debug dbg;
 };
 
@@ -238,6 +240,46 @@ __device__ __forceinline__ Proj project(float x, float y, float z, float tx, flo
   return r;
 }
 
+// ---- fit-ready track record (written by seed_kernel in seed order, read by fit_kernel) -------------------
+// A track in the seed's local frame (x - x_seed, y - y_seed, z - z_seed): every quantity is O(mm), so fp32
+// keeps ~1e-7 mm instead of ulp(550 mm) = 6e-5 mm and the iterates follow the fp64 oracle.
+// x0 = x - z tx, so the residual Eq. 9 is rx = x0 + az tx - ax.
+// W = V^-1 "evaluated and inverted only once, using the vertex position of the seed" (P:L190), Eq. 2 diagonal.
+// A slot without a usable track (none, or R-7) is DEAD: with Tukey weights it is {x0 = 1e15, Wx = 1, rest 0},
+// so that chi2_i = 1e30 gives w = 0 exactly and every product stays finite and zero -- no select in the loop;
+// with unit weights (chi2_max = inf) it is all zeros (W = 0) and the active-track count is taken at load time.
+// 32 bytes in HBM: {x0, y0, tx, ty} {Wx, Wy, track index, 0}.
+struct Trk { float x0, y0, tx, ty, Wx, Wy; };
+
+__device__ __forceinline__ Trk dead_track(const KParams& P) {
+  Trk T;
+  T.x0 = P.unit_weights ? 0.0f : 1e15f;
+  T.Wx = P.unit_weights ? 0.0f : 1.0f;
+  T.y0 = T.tx = T.ty = T.Wy = 0.0f;
+  return T;
+}
+__device__ __forceinline__ bool track_is_dead(const Trk& T, const KParams& P) {
+  return P.unit_weights ? !(T.Wx > 0.0f) : (T.x0 == 1e15f);
+}
+
+struct RawTrk { float x, y, z, tx, ty, vx, vy, vtx, vty; };
+
+__device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, float sx, float sy, float zsv) {
+  Trk T;
+  const float zl = R.z - zsv;
+  T.tx = R.tx; T.ty = R.ty;
+  T.x0 = fmaf(-zl, R.tx, R.x - sx);
+  T.y0 = fmaf(-zl, R.ty, R.y - sy);
+  const float dz2 = zl * zl;
+  const float Vx = fmaf(dz2, R.vtx, R.vx);
+  const float Vy = fmaf(dz2, R.vty, R.vy);
+  const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
+  T.Wx = __fdividef(1.0f, Vx);
+  T.Wy = __fdividef(1.0f, Vy);
+  if (!ok) T = dead_track(P);
+  return T;
+}
+
 // ---- seed_kernel: a1..a4 for one event, one warp --------------------------------------------------------------
 template <bool DBG>
 __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int lane) {
@@ -282,15 +324,28 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   // the units of the chunk form one flat list, and a fill pass gives every lane one unit: UNIT + 1 independent
   // CDF edges (instruction-level parallelism instead of one dependent Horner chain per lane) and UNIT
   // predicated integer adds.  The adds are integers, so the order changes nothing.
+  RawTrk held[SLOTS];                                      // the first CHUNK tracks stay in registers until a4 has
+#pragma unroll                                             // sorted them by seed (no second trip to memory)
+  for (int s = 0; s < SLOTS; ++s) held[s] = RawTrk{0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll 1
   for (int c0 = 0; c0 < n; c0 += CHUNK) {
     float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
 #pragma unroll
-    for (int s = 0; s < SLOTS; ++s) {                      // all loads first (24 in flight per lane)
+    for (int s = 0; s < SLOTS; ++s) {                      // all loads first (24 or 36 in flight per lane)
       const int i = c0 + s * 32 + lane;
       const int t = t0 + (i < n ? i : n - 1);
       lx[s] = __ldg(A.x + t); ly[s] = __ldg(A.y + t); lz[s] = __ldg(A.z + t);
       ltx[s] = __ldg(A.tx + t); lty[s] = __ldg(A.ty + t); lvx[s] = __ldg(A.var_x + t);
+      if (c0 == 0) {
+        held[s].vy = __ldg(A.var_y + t); held[s].vtx = __ldg(A.var_tx + t); held[s].vty = __ldg(A.var_ty + t);
+      }
+    }
+    if (c0 == 0) {
+#pragma unroll
+      for (int s = 0; s < SLOTS; ++s) {
+        held[s].x = lx[s]; held[s].y = ly[s]; held[s].z = lz[s];
+        held[s].tx = ltx[s]; held[s].ty = lty[s]; held[s].vx = lvx[s];
+      }
     }
     int nun[SLOTS];                                        // fill units of my tracks
     int myunits = 0;
@@ -499,7 +554,8 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     --ns;
   }
   __syncwarp();
-  // counting sort of the tracks by seed (deterministic: track order is kept inside a seed)
+  // counting sort of the tracks by seed (deterministic: track order is kept inside a seed); every assigned
+  // track is written as a fit-ready record (local frame of its seed, W at the seed position) at its sorted place
   int myc = 0, myoff = 0;
   {
     myc = lane < ns ? cnt[lane] : 0;
@@ -508,9 +564,7 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     cur[lane] = myoff;
   }
   __syncwarp();
-#pragma unroll 1
-  for (int i0 = 0; i0 < n; i0 += 32) {
-    const int i = i0 + lane;
+  auto place = [&](const int i, const RawTrk& R, const bool from_memory) {
     const int s = seed_of(i);
     if (i < n) {
       A.trk_vertex[t0 + i] = s;                            // scratch: seed index, read back by cleanup_kernel
@@ -518,11 +572,30 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     }
     const unsigned m = __match_any_sync(FULL, s);
     const int rank = __popc(m & lanemask_lt());
-    if (s >= 0) A.sidx[t0 + cur[s] + rank] = (uint16_t)i;
+    if (s >= 0) {
+      RawTrk Q = R;
+      if (from_memory) {
+        const int g = t0 + i;
+        Q.x = __ldg(A.x + g); Q.y = __ldg(A.y + g); Q.z = __ldg(A.z + g); Q.tx = __ldg(A.tx + g); Q.ty = __ldg(A.ty + g);
+        Q.vx = __ldg(A.var_x + g); Q.vy = __ldg(A.var_y + g); Q.vtx = __ldg(A.var_tx + g); Q.vty = __ldg(A.var_ty + g);
+      }
+      const float zsv = zs[s];
+      const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
+      const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+      const Trk T = make_track(P, Q, sx, sy, zsv);
+      float4* o = A.ftrk + 2 * (size_t)(t0 + cur[s] + rank);
+      o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
+      o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), 0.0f);
+    }
     __syncwarp();
     if (s >= 0 && rank == 0) cur[s] += __popc(m);
     __syncwarp();
-  }
+  };
+#pragma unroll
+  for (int sl = 0; sl < SLOTS; ++sl)
+    if (sl * 32 < n) place(sl * 32 + lane, held[sl], false);
+#pragma unroll 1
+  for (int i0 = CHUNK; i0 < n; i0 += 32) place(i0 + lane, held[0], true);
   // seed records for fit_kernel
   int rbase = 0;
   if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
@@ -606,48 +679,21 @@ __device__ __forceinline__ void sums_reduce(Sums& S) {
   }
 }
 
-// A track in the seed's local frame (x - x_seed, y - y_seed, z - z_seed): every quantity is O(mm), so fp32
-// keeps ~1e-7 mm instead of ulp(550 mm) = 6e-5 mm and the iterates follow the fp64 oracle.
-// x0 = x - z tx, so the residual Eq. 9 is rx = x0 + az tx - ax.  Wx = 0 marks an unusable or absent track.
-struct Trk { float x0, y0, tx, ty, Wx, Wy; };
-
-// W = V^-1 "evaluated and inverted only once, using the vertex position of the seed" (P:L190), Eq. 2 diagonal.
-__device__ __forceinline__ Trk load_track(const KArgs& A, int g, float sx, float sy, float zsv) {
-  Trk T;
-  const float zl = __ldg(A.z + g) - zsv;
-  T.tx = __ldg(A.tx + g); T.ty = __ldg(A.ty + g);
-  T.x0 = fmaf(-zl, T.tx, __ldg(A.x + g) - sx);
-  T.y0 = fmaf(-zl, T.ty, __ldg(A.y + g) - sy);
-  const float dz2 = zl * zl;
-  const float Vx = fmaf(dz2, __ldg(A.var_tx + g), __ldg(A.var_x + g));
-  const float Vy = fmaf(dz2, __ldg(A.var_ty + g), __ldg(A.var_y + g));
-  const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
-  T.Wx = ok ? __fdividef(1.0f, Vx) : 0.0f;
-  T.Wy = ok ? __fdividef(1.0f, Vy) : 0.0f;
-  return T;
-}
-
-// Returns the Tukey weight of the track at the current vertex (ax, ay, az).
+// Adds the track to the sums and returns its Tukey weight at the current vertex (ax, ay, az).
 __device__ __forceinline__ float track_accum(const Trk& T, float ax, float ay, float az, const KParams& P, Sums& S) {
   const float rx = fmaf(az, T.tx, T.x0) - ax;          // residual, Eq. 9
   const float ry = fmaf(az, T.ty, T.y0) - ay;
-  const float cx = rx * T.Wx, cy = ry * T.Wy;
-  const float chi = fmaf(rx, cx, ry * cy);             // Eq. 7
-  float w;
-  if (P.unit_weights) {
-    w = 1.0f;
-  } else {
-    const float u = fmaxf(fmaf(chi, -P.inv_chi2_max, 1.0f), 0.0f);
-    w = chi < P.chi2_max ? u * u : 0.0f;               // Tukey bi-square, Eq. 18
-  }
-  w = T.Wx > 0.0f ? w : 0.0f;
+  const float chi = fmaf(rx * rx, T.Wx, ry * ry * T.Wy);   // Eq. 7
+  // Tukey bi-square, Eq. 18: (1 - chi/chi_max)^2 below chi_max, else 0; inv_chi2_max = 0 gives unit weights
+  const float u = fmaxf(fmaf(chi, -P.inv_chi2_max, 1.0f), 0.0f);
+  const float w = u * u;
   const float wWx = w * T.Wx, wWy = w * T.Wy;
   const float p = wWx * T.tx, q = wWy * T.ty;
   S.a += wWx; S.b += wWy; S.c += p; S.d += q;
   S.e = fmaf(p, T.tx, fmaf(q, T.ty, S.e));
-  const float wcx = w * cx, wcy = w * cy;
-  S.gx += wcx; S.gy += wcy;
-  S.gz = fmaf(wcx, T.tx, fmaf(wcy, T.ty, S.gz));
+  S.gx = fmaf(wWx, rx, S.gx);
+  S.gy = fmaf(wWy, ry, S.gy);
+  S.gz = fmaf(p, rx, fmaf(q, ry, S.gz));
   S.chi2 = fmaf(w, chi, S.chi2);
   S.nact += (w > 0.0f) ? 1.0f : 0.0f;
   return w;
@@ -685,125 +731,222 @@ __device__ __forceinline__ void store_vertex(const KArgs& A, size_t o, float x, 
   A.vtx_chi2[o] = chi2; A.vtx_ntracks[o] = ntrk; A.vtx_niter[o] = niter;
 }
 
-// ---- fit_kernel: a5, FIT_G lanes per seed, flat over the seed records of the batch (R-12) -----
+// ---- fit_kernel: a5, FIT_G lanes per seed (R-12) ---------------------------------------------------
+// Warps are autonomous (no CTA barrier): a warp takes a window of 32 seed records (one per lane), sorts them by
+// track count with a shuffle bitonic sort (so the FIT_VPW seeds it fits together need the same number of
+// register slots), and fits them in 32 / FIT_VPW passes.  Tracks are read as 32-byte fit-ready records
+// (two 16-byte loads) and stay in registers; the normal equations are reduced with xor-shuffles inside the
+// FIT_G lanes; every lane solves its seed's 3x3 system in closed form.
 // Results go to slot (event, seed index) of the vertex arrays; cleanup_kernel compacts them in place.
-__global__ void __launch_bounds__(256, 3) fit_kernel(const __grid_constant__ KParams P,
-                                                     const __grid_constant__ KArgs A) {
+__device__ __forceinline__ Trk read_track(const KArgs& A, int rec, int& idx) {
+  const float4 a = __ldg(A.ftrk + 2 * (size_t)rec), b = __ldg(A.ftrk + 2 * (size_t)rec + 1);
+  Trk T;
+  T.x0 = a.x; T.y0 = a.y; T.tx = a.z; T.ty = a.w; T.Wx = b.x; T.Wy = b.y;
+  idx = __float_as_int(b.z);
+  return T;
+}
+
+__global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __grid_constant__ KParams P,
+                                                                        const __grid_constant__ KArgs A) {
   const int lane = threadIdx.x & 31;
   const int j = lane % FIT_G, gl = lane / FIT_G;
   const int total = (int)*A.seed_counter;
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
   const int wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  for (int base = wg * FIT_VPW; base < total; base += nwarps * FIT_VPW) {
-    const int g = base + gl;
-    const bool vact = g < total;
-    int4 r = make_int4(0, 0, 0, 0);
-    if (vact) r = __ldg(reinterpret_cast<const int4*>(A.rec) + g);
-    const int e = r.x, k = r.y & 31;
-    int m = r.y >> 5;
-    const float zsv = __int_as_float(r.w);
-    const bool big = m > FIT_G * FIT_KF;
-    if (big) m = 0;
-    const int t0 = vact ? __ldg(A.offsets + e) : 0;
-    const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
-    const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-    Trk T[FIT_KF];
-    float fw[FIT_KF];
-    int mmax = m;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) mmax = max(mmax, __shfl_xor_sync(FULL, mmax, o));
-    const int nslot = (mmax + FIT_G - 1) / FIT_G;          // warp-uniform number of register slots in use
-#pragma unroll
-    for (int s = 0; s < FIT_KF; ++s) {
-      const int t = j + FIT_G * s;
-      T[s].x0 = T[s].y0 = T[s].tx = T[s].ty = T[s].Wx = T[s].Wy = 0.0f;
-      fw[s] = 0.0f;
-      if (t < m) T[s] = load_track(A, t0 + (int)A.sidx[r.z + t], sx, sy, zsv);
+  // Latency hiding without spare registers: the records of the NEXT window are loaded one window ahead and
+  // their track lines prefetched into L2 during this window; the tracks of the next PASS are prefetched into L1
+  // while this pass iterates.
+  auto prefetch_tracks = [&](int begin, int m, int first, int step, bool l1) {
+    const char* base = reinterpret_cast<const char*>(A.ftrk + 2 * (size_t)begin);
+    const int bytes = m * 32;
+    for (int off = first * 128; off < bytes; off += step * 128) {
+      if (l1) asm volatile("prefetch.global.L1 [%0];" ::"l"(base + off));
+      else asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
     }
-    float ax = 0.0f, ay = 0.0f, az = 0.0f;
-    bool run = vact && !big;
-    bool sing = false;
-    int niter = 0;
-    float C[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
-    float chi2 = 0.0f, nact = 0.0f;
+    if (first == 0 && bytes > 0) {                         // the records are 32-byte aligned, not line aligned
+      if (l1) asm volatile("prefetch.global.L1 [%0];" ::"l"(base + bytes - 1));
+      else asm volatile("prefetch.global.L2 [%0];" ::"l"(base + bytes - 1));
+    }
+  };
+  int4 wr_next = make_int4(0, 0, 0, 0);
+  if (wg * 32 + lane < total) wr_next = __ldg(reinterpret_cast<const int4*>(A.rec) + wg * 32 + lane);
 #pragma unroll 1
-    for (int it = 1; it <= P.max_iter; ++it) {
-      Sums S;
-      sums_zero(S);
-      if (run) {
-#pragma unroll
-        for (int s = 0; s < FIT_KF; ++s)
-          if (s < nslot) fw[s] = track_accum(T[s], ax, ay, az, P, S);
-      }
-      sums_reduce<FIT_G>(S);
-      if (run) {
-        float dx, dy, dzs, dchi2;
-        if (!newton_step(S, dx, dy, dzs, dchi2, C)) {
-          sing = true; run = false;
-        } else {
-          ax += dx; ay += dy; az += dzs;
-          chi2 = S.chi2; nact = S.nact; niter = it;
-          if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) run = false;
-        }
-      }
-      if (!__any_sync(FULL, run)) break;
+  for (int wb = wg * 32; wb < total; wb += nwarps * 32) {
+    const int4 wr = wr_next;
+    {
+      const int nb = wb + nwarps * 32 + lane;
+      wr_next = make_int4(0, 0, 0, 0);
+      if (nb < total) wr_next = __ldg(reinterpret_cast<const int4*>(A.rec) + nb);
     }
-    if (vact && !big) {
-      const size_t o = (size_t)e * P.max_vtx + k;
-      if (sing) {
-        if (j == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
-      } else {
-        if (j == 0) store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)nact, niter);
+    // bitonic sort of (track count, lane) keys, ascending; absent records (count 0) come first
+    int key = ((wr.y >> 5) << 5) | lane;
+#pragma unroll
+    for (int kk = 2; kk <= 32; kk <<= 1) {
+#pragma unroll
+      for (int jj = kk >> 1; jj > 0; jj >>= 1) {
+        const int other = __shfl_xor_sync(FULL, key, jj);
+        const bool up = ((lane & kk) == 0) == ((lane & jj) == 0);     // keep the smaller key
+        key = up ? min(key, other) : max(key, other);
+      }
+    }
+    {                                                      // first pass of this window: L1 prefetch (short lead)
+      const int src = __shfl_sync(FULL, key, gl) & 31;
+      const int pz = __shfl_sync(FULL, wr.z, src), pm = __shfl_sync(FULL, wr.y, src) >> 5;
+      prefetch_tracks(pz, min(pm, FIT_G * FIT_KF), j, FIT_G, true);
+    }
+#pragma unroll 1
+    for (int pass = 0; pass < 32 / FIT_VPW; ++pass) {
+      const int src = __shfl_sync(FULL, key, pass * FIT_VPW + gl) & 31;   // lane holding my group's record
+      int4 r;
+      r.x = __shfl_sync(FULL, wr.x, src); r.y = __shfl_sync(FULL, wr.y, src);
+      r.z = __shfl_sync(FULL, wr.z, src); r.w = __shfl_sync(FULL, wr.w, src);
+      if (pass + 1 < 32 / FIT_VPW) {                       // tracks of the next pass -> L1
+        const int nsrc = __shfl_sync(FULL, key, (pass + 1) * FIT_VPW + gl) & 31;
+        const int pz = __shfl_sync(FULL, wr.z, nsrc), pm = __shfl_sync(FULL, wr.y, nsrc) >> 5;
+        prefetch_tracks(pz, min(pm, FIT_G * FIT_KF), j, FIT_G, true);
+      } else {                                             // tracks of the next window -> L2 (one record per lane)
+        prefetch_tracks(wr_next.z, min(wr_next.y >> 5, 2 * FIT_G * FIT_KF), 0, 1, false);
+      }
+      const int e = r.x, k = r.y & 31;
+      int m = r.y >> 5;
+      const bool vact = m > 0;                               // every real seed holds >= 2 tracks
+      if (!__any_sync(FULL, vact)) continue;
+      const float zsv = __int_as_float(r.w);
+      const bool big = m > FIT_G * FIT_KF;
+      if (big) m = 0;
+      const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
+      const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+      Trk T[FIT_KF];
+      float fw[FIT_KF];
+      int mmax = m;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) mmax = max(mmax, __shfl_xor_sync(FULL, mmax, o));
+      const int nslot = (mmax + FIT_G - 1) / FIT_G;          // warp-uniform number of register slots in use
+      float nvalid = 0.0f;                                   // usable tracks (unit-weight mode: the active count)
+      {
+        // every lane loads unconditionally (clamped record index), all loads in flight at once; absent slots are
+        // replaced by dead tracks afterwards (predicated loads would chain through the predicate registers)
+        float4 qa[FIT_KF];
+        float2 qb[FIT_KF];
+        const int last = max(m - 1, 0);
 #pragma unroll
         for (int s = 0; s < FIT_KF; ++s) {
-          const int t = j + FIT_G * s;
-          if (t < m) A.trk_weight[t0 + (int)A.sidx[r.z + t]] = fw[s];
+          const float4* q = A.ftrk + 2 * (size_t)(r.z + min(j + FIT_G * s, last));
+          qa[s] = __ldg(q);
+          qb[s] = __ldg(reinterpret_cast<const float2*>(q + 1));
+        }
+        const Trk dead = dead_track(P);
+#pragma unroll
+        for (int s = 0; s < FIT_KF; ++s) {
+          const bool have = j + FIT_G * s < m;
+          T[s].x0 = have ? qa[s].x : dead.x0; T[s].y0 = have ? qa[s].y : dead.y0;
+          T[s].tx = have ? qa[s].z : dead.tx; T[s].ty = have ? qa[s].w : dead.ty;
+          T[s].Wx = have ? qb[s].x : dead.Wx; T[s].Wy = have ? qb[s].y : dead.Wy;
+          fw[s] = 0.0f;
+          nvalid += track_is_dead(T[s], P) ? 0.0f : 1.0f;
         }
       }
-    }
-    // Seeds with more tracks than the register-resident path holds: the whole warp strides over the track
-    // list and re-reads the tracks (L1-resident) every iteration.
-    unsigned bigm = __ballot_sync(FULL, vact && big && j == 0);
-    while (bigm) {
-      const int src = __ffs(bigm) - 1;
-      bigm &= bigm - 1;
-      const int be = __shfl_sync(FULL, e, src), bk = __shfl_sync(FULL, k, src);
-      const int bm_ = __shfl_sync(FULL, r.y, src) >> 5, bo = __shfl_sync(FULL, r.z, src);
-      const int bt0 = __shfl_sync(FULL, t0, src);
-      const float bz = __shfl_sync(FULL, zsv, src);
-      const float bx = __fmaf_rn(P.beam_tx, bz, P.beam_x), by = __fmaf_rn(P.beam_ty, bz, P.beam_y);
-      float qx = 0.0f, qy = 0.0f, qz = 0.0f;               // current position (local frame)
-      float px = 0.0f, py = 0.0f, pz = 0.0f;               // position the last weights were taken at
-      bool bsing = false;
-      int bit = 0;
-      float bchi2 = 0.0f, bnact = 0.0f;
+      if (P.unit_weights) {
+#pragma unroll
+        for (int o = FIT_G / 2; o > 0; o >>= 1) nvalid += __shfl_xor_sync(FULL, nvalid, o);
+      }
+      float ax = 0.0f, ay = 0.0f, az = 0.0f;
+      bool run = vact && !big;
+      bool sing = false;
+      int niter = 0;
+      float C[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+      float chi2 = 0.0f, nact = 0.0f;
 #pragma unroll 1
       for (int it = 1; it <= P.max_iter; ++it) {
         Sums S;
         sums_zero(S);
-        for (int t = lane; t < bm_; t += 32) {
-          const Trk U = load_track(A, bt0 + (int)A.sidx[bo + t], bx, by, bz);
-          track_accum(U, qx, qy, qz, P, S);
+        if (run) {
+#pragma unroll
+          for (int s = 0; s < FIT_KF; ++s)
+            if (s < nslot) fw[s] = track_accum(T[s], ax, ay, az, P, S);
         }
-        sums_reduce<32>(S);
-        float dx, dy, dzs, dchi2;
-        if (!newton_step(S, dx, dy, dzs, dchi2, C)) { bsing = true; break; }
-        px = qx; py = qy; pz = qz;
-        qx += dx; qy += dy; qz += dzs;
-        bchi2 = S.chi2; bnact = S.nact; bit = it;
-        if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
+        sums_reduce<FIT_G>(S);
+        if (P.unit_weights) S.nact = nvalid;
+        if (run) {
+          float dx, dy, dzs, dchi2;
+          if (!newton_step(S, dx, dy, dzs, dchi2, C)) {
+            sing = true; run = false;
+          } else {
+            ax += dx; ay += dy; az += dzs;
+            chi2 = S.chi2; nact = S.nact; niter = it;
+            if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) run = false;
+          }
+        }
+        if (!__any_sync(FULL, run)) break;
       }
-      const size_t o = (size_t)be * P.max_vtx + bk;
-      if (bsing) {
-        if (lane == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
-      } else {
-        if (lane == 0) store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)bnact, bit);
-        for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration, recomputed
-          const int gt = bt0 + (int)A.sidx[bo + t];
-          const Trk U = load_track(A, gt, bx, by, bz);
-          Sums dummy;
-          sums_zero(dummy);
-          A.trk_weight[gt] = track_accum(U, px, py, pz, P, dummy);
+      if (vact && !big) {
+        const size_t o = (size_t)e * P.max_vtx + k;
+        if (sing) {
+          if (j == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
+        } else {
+          if (j == 0) store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)nact, niter);
+#pragma unroll
+          for (int s = 0; s < FIT_KF; ++s) {
+            const int t = j + FIT_G * s;
+            if (t < m) {
+              const int idx = __float_as_int(__ldg(reinterpret_cast<const float*>(A.ftrk + 2 * (size_t)(r.z + t) + 1) + 2));
+              A.trk_weight[idx] = track_is_dead(T[s], P) ? 0.0f : fw[s];
+            }
+          }
+        }
+      }
+      // Seeds with more tracks than the register-resident path holds: the whole warp strides over the seed's
+      // records (contiguous, L1-resident after the first iteration).
+      unsigned bigm = __ballot_sync(FULL, vact && big && j == 0);
+      while (bigm) {
+        const int bsrc = __ffs(bigm) - 1;
+        bigm &= bigm - 1;
+        const int be = __shfl_sync(FULL, e, bsrc), bk = __shfl_sync(FULL, k, bsrc);
+        const int bm_ = __shfl_sync(FULL, r.y, bsrc) >> 5, bo = __shfl_sync(FULL, r.z, bsrc);
+        const float bz = __shfl_sync(FULL, zsv, bsrc);
+        const float bx = __fmaf_rn(P.beam_tx, bz, P.beam_x), by = __fmaf_rn(P.beam_ty, bz, P.beam_y);
+        float qx = 0.0f, qy = 0.0f, qz = 0.0f;               // current position (local frame)
+        float px = 0.0f, py = 0.0f, pz = 0.0f;               // position the last weights were taken at
+        bool bsing = false;
+        int bit = 0;
+        float bchi2 = 0.0f, bnact = 0.0f;
+#pragma unroll 1
+        for (int it = 1; it <= P.max_iter; ++it) {
+          Sums S;
+          sums_zero(S);
+          float nv = 0.0f;
+          for (int t = lane; t < bm_; t += 32) {
+            int idx;
+            const Trk U = read_track(A, bo + t, idx);
+            nv += track_is_dead(U, P) ? 0.0f : 1.0f;
+            track_accum(U, qx, qy, qz, P, S);
+          }
+          sums_reduce<32>(S);
+          if (P.unit_weights) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) nv += __shfl_xor_sync(FULL, nv, o);
+            S.nact = nv;
+          }
+          float dx, dy, dzs, dchi2;
+          if (!newton_step(S, dx, dy, dzs, dchi2, C)) { bsing = true; break; }
+          px = qx; py = qy; pz = qz;
+          qx += dx; qy += dy; qz += dzs;
+          bchi2 = S.chi2; bnact = S.nact; bit = it;
+          if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
+        }
+        const size_t o = (size_t)be * P.max_vtx + bk;
+        if (bsing) {
+          if (lane == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
+        } else {
+          if (lane == 0) store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)bnact, bit);
+          for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration, recomputed
+            int idx;
+            const Trk U = read_track(A, bo + t, idx);
+            Sums dummy;
+            sums_zero(dummy);
+            const float w = track_accum(U, px, py, pz, P, dummy);
+            A.trk_weight[idx] = track_is_dead(U, P) ? 0.0f : w;
+          }
         }
       }
     }
