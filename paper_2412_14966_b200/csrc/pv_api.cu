@@ -141,9 +141,9 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
 
   pvk::KParams kp;
   make_kparams(params, nbins, &kp);
-  int warps = di->max_smem_optin / kp.warp_smem_bytes;
-  if (warps > 16) warps = 16;
-  if (const char* envw = getenv("PV_WARPS_PER_CTA")) {
+  int warps = di->max_smem_optin / kp.warp_smem_bytes;        // teams (events in flight) per CTA
+  if (warps > pvk::MAX_TEAMS) warps = pvk::MAX_TEAMS;
+  if (const char* envw = getenv("PV_TEAMS_PER_CTA")) {
     const int w = atoi(envw);
     if (w >= 1 && w < warps) warps = w;
   }
@@ -161,7 +161,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel, pvk::FIT_BLOCK, 0));
     di->fit_blocks_per_sm = nb > 0 ? nb : 1;
   }
-  g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * 32; g_last_smem = smem;
+  g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * pvk::TEAM; g_last_smem = smem;
 
   pvk::KArgs ka;
   memset(&ka, 0, sizeof(ka));
@@ -182,13 +182,13 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
   CK(cudaMemsetAsync(workspace, 0, 32, stream));
-  // a1..a4: persistent, one CTA per SM, one warp per event
+  // a1..a4: persistent, one CTA per SM, one team of two warps per event
   int grid = di->sms;
   const int need = (n_events + warps - 1) / warps;
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
-  if (dbg) pvk::seed_kernel<true><<<grid, warps * 32, smem, stream>>>(kp, ka);
-  else pvk::seed_kernel<false><<<grid, warps * 32, smem, stream>>>(kp, ka);
+  if (dbg) pvk::seed_kernel<true><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+  else pvk::seed_kernel<false><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
   // a5: FIT_G lanes per seed, warps stride over windows of 32 seed records

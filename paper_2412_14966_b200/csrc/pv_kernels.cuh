@@ -30,8 +30,11 @@ namespace pvk {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
-constexpr int CHUNK = 128;          // tracks per fill chunk: 4 register slots per lane
-constexpr int SLOTS = CHUNK / 32;
+constexpr int TEAM_WARPS = 2;       // warps per event in seed_kernel
+constexpr int TEAM = 32 * TEAM_WARPS;
+constexpr int MAX_TEAMS = 13;       // events in flight per CTA (named barriers 1..13; 13 histograms fill 227 KB)
+constexpr int CHUNK = 128;          // tracks per fill chunk
+constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
 constexpr int UNIT = 8;             // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
@@ -41,19 +44,22 @@ constexpr int FIT_KF = 8;           // register-resident tracks per lane (fast p
 constexpr int FIT_BLOCK = 128;      // threads per CTA of fit_kernel (warps are autonomous)
 constexpr int FIT_MIN_BLOCKS = 4;   // CTAs per SM the register budget is held to
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
-constexpr int PROTO_CAP = 512;      // proto-cluster starts of one sweep round (<= 16 per touched word)
+constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
 
-// Per-warp shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
+// Per-team shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
 constexpr int SM_TOUCHED = 0;                          // uint8 tb[128]        histogram words written by the fill
 constexpr int SM_TWL = SM_TOUCHED + MAX_WORDS;         // uint8 twl[128]       list of touched words, ascending
-constexpr int SM_CNT = SM_TWL + MAX_WORDS;             // int cnt[32], cur[32]
-constexpr int SM_SEED = SM_CNT + (32 + 32) * 4;        // int sb[32], se[32], sp[32]; float zs[32]; int part[32]
-constexpr int SM_STAGE = SM_SEED + 5 * MAXV * 4;       // float zp[128], inv[128]; int lonb[128]   (fill)
-constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // uint16 list[256]  (fill); with the stage: protostart[] (peaks)
+constexpr int SM_CNT = SM_TWL + MAX_WORDS;             // int cnt[2][32]       tracks per seed, per warp
+constexpr int SM_CUR = SM_CNT + TEAM_WARPS * 32 * 4;   // int cur[2][32]       running record position, per warp
+constexpr int SM_SEED = SM_CUR + TEAM_WARPS * 32 * 4;  // int sb[32], se[32], sp[32]; float zs[32]; int part[32]
+constexpr int SM_MISC = SM_SEED + 5 * MAXV * 4;        // int misc[16]         warp totals, next event
+constexpr int SM_STAGE = SM_MISC + 64;                 // float zp[128], inv[128]; int lonb[128]   (fill)
+constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // uint16 list[256]  (fill)
 constexpr int SM_BINS = SM_LIST + LIST_CAP * 2;        // int16 binsm[256]     central bins of the first 256 tracks
 constexpr int SM_TAIL_BYTES = SM_BINS + BINS_SM * 2;
-static_assert(PROTO_CAP * 2 <= CHUNK * 12 + LIST_CAP * 2, "protostart overlays the fill stage and unit list");
-static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0, "alignment of the vector loads");
+// peak search overlays on the (dead) stage and list: uint16 protostart[2][PROTO_CAP]; int sb1[32], se1[32], sp1[32]
+static_assert(TEAM_WARPS * PROTO_CAP * 2 + 3 * MAXV * 4 <= CHUNK * 12 + LIST_CAP * 2, "peak-search overlays fit");
+static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0 && SM_TAIL_BYTES % 16 == 0, "alignment of the vector accesses");
 
 struct KParams {
   float z_min, dz, inv_dz, z_split;
@@ -280,25 +286,36 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
   return T;
 }
 
-// ---- seed_kernel: a1..a4 for one event, one warp --------------------------------------------------------------
+// ---- seed_kernel: a1..a4 for one event, one TEAM of two warps ---------------------------------------------------
+// The CTA holds up to MAX_TEAMS teams, each with its own histogram in shared memory and its own named barrier.
+__device__ __forceinline__ void team_sync(int bar) {
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(TEAM) : "memory");
+}
+
 template <bool DBG>
-__device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int lane) {
+__device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt, const int bar) {
+  const int lane = tt & 31, tw = tt >> 5;
   int* H = reinterpret_cast<int*>(wsm);
   unsigned char* tail = wsm + (size_t)P.region0_words * 4;
   uint8_t* tb = reinterpret_cast<uint8_t*>(tail + SM_TOUCHED);
   uint8_t* twl = reinterpret_cast<uint8_t*>(tail + SM_TWL);
-  int* cnt = reinterpret_cast<int*>(tail + SM_CNT);
-  int* cur = cnt + 32;
+  int* cnt = reinterpret_cast<int*>(tail + SM_CNT);          // cnt[warp][seed]
+  int* cur = reinterpret_cast<int*>(tail + SM_CUR) + tw * 32;   // my warp's running record positions
   int* sb = reinterpret_cast<int*>(tail + SM_SEED);
   int* se = sb + MAXV;
   int* sp = se + MAXV;
   float* zs = reinterpret_cast<float*>(sp + MAXV);
   int* part = reinterpret_cast<int*>(zs + MAXV);
+  int* misc = reinterpret_cast<int*>(tail + SM_MISC);
   float* st_zp = reinterpret_cast<float*>(tail + SM_STAGE);
   float* st_inv = st_zp + CHUNK;
   int* st_lonb = reinterpret_cast<int*>(st_inv + CHUNK);
   uint16_t* list = reinterpret_cast<uint16_t*>(tail + SM_LIST);
-  uint16_t* protostart = reinterpret_cast<uint16_t*>(tail + SM_STAGE);   // overlay: stage and list are dead after the fill
+  // overlays of the peak search: stage and list are dead after the fill
+  uint16_t* protostart = reinterpret_cast<uint16_t*>(tail + SM_STAGE) + tw * PROTO_CAP;
+  int* sb1 = reinterpret_cast<int*>(tail + SM_STAGE + TEAM_WARPS * PROTO_CAP * 2);
+  int* se1 = sb1 + MAXV;
+  int* sp1 = se1 + MAXV;
   int16_t* binsm = reinterpret_cast<int16_t*>(tail + SM_BINS);
 
   const int t0 = __ldg(A.offsets + e);
@@ -308,9 +325,9 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
 
   if (n > MAX_TRK) {
 #pragma unroll 1
-    for (int i = lane; i < n; i += 32) A.trk_vertex[t0 + i] = -1;
-    if (DBG && A.dbg.trk_seed) for (int i = lane; i < n; i += 32) A.dbg.trk_seed[t0 + i] = -1;
-    if (lane == 0) {
+    for (int i = tt; i < n; i += TEAM) A.trk_vertex[t0 + i] = -1;
+    if (DBG && A.dbg.trk_seed) for (int i = tt; i < n; i += TEAM) A.dbg.trk_seed[t0 + i] = -1;
+    if (tt == 0) {
       A.n_vtx[e] = 0;
       A.event_status[e] = PV_EVT_TOO_MANY_TRACKS;
       if (DBG && A.dbg.n_seeds) A.dbg.n_seeds[e] = 0;
@@ -320,9 +337,9 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   }
 
   // ================= a1 + a2: projection (Eq. 1, Eq. 3) and histogram fill ===================
-  // Chunks of CHUNK tracks, SLOTS per lane.  The window of a histogrammed track is cut into units of UNIT bins;
-  // the units of the chunk form one flat list, and a fill pass gives every lane one unit: UNIT + 1 independent
-  // CDF edges (instruction-level parallelism instead of one dependent Horner chain per lane) and UNIT
+  // Chunks of CHUNK tracks, SLOTS per thread.  The window of a histogrammed track is cut into units of UNIT
+  // bins; the units of the chunk form one flat list, and a fill pass gives every thread one unit: UNIT + 1
+  // independent CDF edges (instruction-level parallelism instead of one dependent Horner chain) and UNIT
   // predicated integer adds.  The adds are integers, so the order changes nothing.
   RawTrk held[SLOTS];                                      // the first CHUNK tracks stay in registers until a4 has
 #pragma unroll                                             // sorted them by seed (no second trip to memory)
@@ -331,8 +348,8 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   for (int c0 = 0; c0 < n; c0 += CHUNK) {
     float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
 #pragma unroll
-    for (int s = 0; s < SLOTS; ++s) {                      // all loads first (24 or 36 in flight per lane)
-      const int i = c0 + s * 32 + lane;
+    for (int s = 0; s < SLOTS; ++s) {                      // all loads first
+      const int i = c0 + s * TEAM + tt;
       const int t = t0 + (i < n ? i : n - 1);
       lx[s] = __ldg(A.x + t); ly[s] = __ldg(A.y + t); lz[s] = __ldg(A.z + t);
       ltx[s] = __ldg(A.tx + t); lty[s] = __ldg(A.ty + t); lvx[s] = __ldg(A.var_x + t);
@@ -351,7 +368,7 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     int myunits = 0;
 #pragma unroll
     for (int s = 0; s < SLOTS; ++s) {
-      const int i = c0 + s * 32 + lane;
+      const int i = c0 + s * TEAM + tt;
       nun[s] = 0;
       if (i < n) {
         const Proj r = project(lx[s], ly[s], lz[s], ltx[s], lty[s], lvx[s], P);
@@ -371,31 +388,34 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
           const int nb = hi - lo;
           if (nb > 0) {
             nun[s] = (nb + UNIT - 1) / UNIT;
-            st_zp[s * 32 + lane] = r.zp; st_inv[s * 32 + lane] = r.inv; st_lonb[s * 32 + lane] = lo | (nb << 12);
+            st_zp[s * TEAM + tt] = r.zp; st_inv[s * TEAM + tt] = r.inv; st_lonb[s * TEAM + tt] = lo | (nb << 12);
           }
         }
       }
       myunits += nun[s];
     }
     const int incl = warp_incl_scan(myunits, lane);
-    const int total = __shfl_sync(FULL, incl, 31);
+    if (lane == 31) misc[tw] = incl;
+    team_sync(bar);
+    const int total = misc[0] + misc[1];
+    const int first = incl - myunits + (tw ? misc[0] : 0);  // list position of my first unit
 #pragma unroll 1
     for (int R = 0; R < total; R += LIST_CAP) {            // one round unless the chunk holds very wide tracks
-      __syncwarp();
+      if (R > 0) team_sync(bar);
       {
-        int g = incl - myunits - R;                        // list position of my first unit in this round
+        int g = first - R;
 #pragma unroll
         for (int s = 0; s < SLOTS; ++s) {
-          const int tk = s * 32 + lane;
+          const int tk = s * TEAM + tt;
 #pragma unroll 1
           for (int u = 0; u < nun[s]; ++u, ++g)
             if ((unsigned)g < (unsigned)LIST_CAP) list[g] = (uint16_t)(tk | (u << 7));
         }
       }
-      __syncwarp();
+      team_sync(bar);
       const int nl = min(total - R, LIST_CAP);
 #pragma unroll 1
-      for (int p0 = 0; p0 < nl; p0 += 32) {
+      for (int p0 = tw * 32; p0 < nl; p0 += TEAM) {
         const int idx = p0 + lane;
         const bool act = idx < nl;
         const int ent = list[act ? idx : nl - 1];
@@ -419,11 +439,11 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
         }
       }
     }
-    __syncwarp();
+    team_sync(bar);
   }
 
   if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
-    for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
+    for (int b = tt; b < P.nbins; b += TEAM) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
 
   // ================= a3: peak search and seed position (Eq. 4-5) ==============================
   // List of the touched histogram words, ascending; only these can hold bins above the threshold.
@@ -433,25 +453,37 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     const int c = (f4 & 1u) + ((f4 >> 8) & 1u) + ((f4 >> 16) & 1u) + ((f4 >> 24) & 1u);
     const int inc = warp_incl_scan(c, lane);
     ntw = __shfl_sync(FULL, inc, 31);
-    int o = inc - c;
+    if (tw == 0) {
+      int o = inc - c;
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
-      if ((f4 >> (8 * q)) & 1u) twl[o++] = (uint8_t)(4 * lane + q);
-    __syncwarp();
-    reinterpret_cast<unsigned*>(tb)[lane] = 0;             // clean for the next event
+      for (int q = 0; q < 4; ++q)
+        if ((f4 >> (8 * q)) & 1u) twl[o++] = (uint8_t)(4 * lane + q);
+    }
   }
-  __syncwarp();
+  team_sync(bar);
+  if (tw == 1) reinterpret_cast<unsigned*>(tb)[lane] = 0;  // clean for the next event (both warps have read it)
 
-  int n_raw = 0;
+  // Each warp takes half of the touched words: proto-cluster starts, then one lane per proto-cluster for the
+  // z-ordered sweep; warp 0 writes its seeds to (sb, se, sp), warp 1 to (sb1, se1, sp1), appended afterwards.
+  int nraw_w = 0;
   {
-    int i = 0;
+    const int half = (ntw + 1) >> 1;
+    int i = tw ? half : 0;
+    const int iend = tw ? ntw : half;
+    int* wb_ = tw ? sb1 : sb;
+    int* we_ = tw ? se1 : se;
+    int* wp_ = tw ? sp1 : sp;
     int prev_w = -2;
     unsigned prev_m = 0;
+    if (i > 0 && i < iend) {                               // does a run continue from the other warp's last word?
+      const int pw = twl[i - 1];
+      if (pw == (int)twl[i] - 1) { prev_w = pw; prev_m = (H[pw * 32 + 31] > P.T_bin) ? 0x80000000u : 0u; }
+    }
 #pragma unroll 1
-    while (i < ntw) {                                      // rounds of <= PROTO_CAP proto-clusters (one in practice)
+    while (i < iend) {                                     // rounds of <= PROTO_CAP proto-clusters (one in practice)
       int n_proto = 0;
 #pragma unroll 1
-      for (; i < ntw && n_proto + 16 <= PROTO_CAP; ++i) {  // a word of 32 bins starts at most 16 runs
+      for (; i < iend && n_proto + 16 <= PROTO_CAP; ++i) { // a word of 32 bins starts at most 16 runs
         const int w = twl[i];
         const int b = w * 32 + lane;
         const unsigned m = __ballot_sync(FULL, b < P.nbins && H[b] > P.T_bin);
@@ -474,25 +506,33 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
           const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
           if (!__any_sync(FULL, run)) break;
           if (run) {
-            const int cc = sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+            const int cc = sweep(H, b0, P, rep ? base : -1, wb_, we_, wp_, c0, c1);
             if (rep == 0) c = cc;
           }
           if (rep == 0) {
             const int inc = warp_incl_scan(c, lane);
-            base = n_raw + inc - c;
-            if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
-            if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
-            n_raw += __shfl_sync(FULL, inc, 31);
+            base = nraw_w + inc - c;
+            if (c > 0 && base < P.max_vtx) { wb_[base] = c0.b; we_[base] = c0.e; wp_[base] = c0.p; }
+            if (c > 1 && base + 1 < P.max_vtx) { wb_[base + 1] = c1.b; we_[base + 1] = c1.e; wp_[base + 1] = c1.p; }
+            nraw_w += __shfl_sync(FULL, inc, 31);
           }
         }
       }
       __syncwarp();
     }
+    if (lane == 0) misc[2 + tw] = nraw_w;
+  }
+  team_sync(bar);
+  const int nraw0 = misc[2];
+  const int n_raw = nraw0 + misc[3];
+  if (tw == 1) {                                           // append warp 1's seeds (they lie above warp 0's in z)
+    const int k = nraw0 + lane;
+    if (lane < min(misc[3], P.max_vtx) && k < P.max_vtx) { sb[k] = sb1[lane]; se[k] = se1[lane]; sp[k] = sp1[lane]; }
   }
   int ns = n_raw;
   if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
-  __syncwarp();
-  if (lane < ns) {                                         // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
+  team_sync(bar);
+  if (tw == 0 && lane < ns) {                              // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
     const int i = sp[lane];
     const long long Nm = i > 0 ? H[i - 1] : 0;
     const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
@@ -502,14 +542,15 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
     zs[lane] = __fmaf_rn(delta, P.dz, zi);
   }
-  __syncwarp();
+  team_sync(bar);
   // the histogram is dead from here on: clear what this event touched for the next one
 #pragma unroll 1
-  for (int i = 0; i < ntw; ++i) H[(int)twl[i] * 32 + lane] = 0;
+  for (int i = tw; i < ntw; i += TEAM_WARPS) H[(int)twl[i] * 32 + lane] = 0;
 
   // ================= a4: association (R-11) ====================================================
   // Central bins: the first BINS_SM tracks keep them in shared memory, the rest read them back from the
-  // trk_vertex scratch.  part[] is padded with INT_MAX to whole groups of four.
+  // trk_vertex scratch.  part[] is padded with INT_MAX to whole groups of four.  Warp w takes the tracks
+  // [64 k + 32 w, 64 k + 32 w + 32).
   auto seed_of = [&](int i) -> int {                       // seed index of track i, -1 = none
     if (i >= n || ns == 0) return -1;
     const int b = i < BINS_SM ? (int)binsm[i] : A.trk_vertex[t0 + i];
@@ -524,44 +565,48 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   };
   for (;;) {
     if (ns == 0) break;
-    __syncwarp();
-    part[lane] = lane + 1 < ns ? (se[lane] + sb[lane + 1]) / 2 : 0x7fffffff;
-    cnt[lane] = 0;
-    __syncwarp();
+    if (tw == 0) part[lane] = lane + 1 < ns ? (se[lane] + sb[lane + 1]) / 2 : 0x7fffffff;
+    cnt[tw * 32 + lane] = 0;
+    team_sync(bar);
 #pragma unroll 1
-    for (int i0 = 0; i0 < n; i0 += 32) {
+    for (int i0 = tw * 32; i0 < n; i0 += TEAM) {
       const int s = seed_of(i0 + lane);
       const unsigned m = __match_any_sync(FULL, s);
-      if (s >= 0 && (m & lanemask_lt()) == 0) cnt[s] += __popc(m);
+      if (s >= 0 && (m & lanemask_lt()) == 0) cnt[tw * 32 + s] += __popc(m);
       __syncwarp();
     }
+    team_sync(bar);
     // "the seed cluster is removed ... and the procedure is repeated": least populated, ties lowest z
     int key = 0x7fffffff;
     if (lane < ns) {
       const int region = zs[lane] < P.z_split ? 1 : 0;
-      const int c = cnt[lane];
+      const int c = cnt[lane] + cnt[32 + lane];
       if (c < P.min_tracks_seed[region]) key = (c << 6) | lane;
     }
-    key = __reduce_min_sync(FULL, key);
+    key = __reduce_min_sync(FULL, key);                    // both warps take the same decision
     if (key == 0x7fffffff) break;
-    const int worst = key & 63;
-    int nb = 0, ne = 0, np = 0;
-    float nz = 0.0f;
-    const bool mv = lane >= worst && lane + 1 < ns;
-    if (mv) { nb = sb[lane + 1]; ne = se[lane + 1]; np = sp[lane + 1]; nz = zs[lane + 1]; }
-    __syncwarp();
-    if (mv) { sb[lane] = nb; se[lane] = ne; sp[lane] = np; zs[lane] = nz; }
+    team_sync(bar);                                        // rare path: everyone has read the seed arrays
+    if (tw == 0) {
+      const int worst = key & 63;
+      int nb = 0, ne = 0, np = 0;
+      float nz = 0.0f;
+      const bool mv = lane >= worst && lane + 1 < ns;
+      if (mv) { nb = sb[lane + 1]; ne = se[lane + 1]; np = sp[lane + 1]; nz = zs[lane + 1]; }
+      __syncwarp();
+      if (mv) { sb[lane] = nb; se[lane] = ne; sp[lane] = np; zs[lane] = nz; }
+    }
     --ns;
+    team_sync(bar);
   }
-  __syncwarp();
-  // counting sort of the tracks by seed (deterministic: track order is kept inside a seed); every assigned
-  // track is written as a fit-ready record (local frame of its seed, W at the seed position) at its sorted place
+  // counting sort of the tracks by seed: a seed's records are warp 0's tracks in track order, then warp 1's
+  // (deterministic); every assigned track is written as a fit-ready record (local frame of its seed, W at the
+  // seed position) at its sorted place
   int myc = 0, myoff = 0;
   {
-    myc = lane < ns ? cnt[lane] : 0;
+    myc = (ns > 0 && lane < ns) ? cnt[lane] + cnt[32 + lane] : 0;
     const int inc = warp_incl_scan(myc, lane);
     myoff = inc - myc;
-    cur[lane] = myoff;
+    cur[lane] = myoff + ((tw && ns > 0) ? cnt[lane] : 0);
   }
   __syncwarp();
   auto place = [&](const int i, const RawTrk& R, const bool from_memory) {
@@ -593,60 +638,65 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   };
 #pragma unroll
   for (int sl = 0; sl < SLOTS; ++sl)
-    if (sl * 32 < n) place(sl * 32 + lane, held[sl], false);
+    if (sl * TEAM + tw * 32 < n) place(sl * TEAM + tt, held[sl], false);
 #pragma unroll 1
-  for (int i0 = CHUNK; i0 < n; i0 += 32) place(i0 + lane, held[0], true);
+  for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) place(i0 + lane, held[0], true);
   // seed records for fit_kernel
-  int rbase = 0;
-  if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
-  rbase = __shfl_sync(FULL, rbase, 0);
-  if (lane < ns) {
-    int4 r;
-    r.x = e; r.y = lane | (myc << 5); r.z = t0 + myoff; r.w = __float_as_int(zs[lane]);
-    reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
-  }
-  if (lane == 0) {
-    A.n_vtx[e] = ns;                                       // scratch: seeds of the event, replaced by cleanup_kernel
-    A.event_status[e] = status;
-  }
-  if (DBG) {
-    if (lane == 0) {
-      if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
-      if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
-    }
+  if (tw == 0) {
+    int rbase = 0;
+    if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
+    rbase = __shfl_sync(FULL, rbase, 0);
     if (lane < ns) {
-      if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
-      if (A.dbg.seed_bins) {
-        A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
-        A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
-        A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
+      int4 r;
+      r.x = e; r.y = lane | (myc << 5); r.z = t0 + myoff; r.w = __float_as_int(zs[lane]);
+      reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
+    }
+    if (lane == 0) {
+      A.n_vtx[e] = ns;                                     // scratch: seeds of the event, replaced by cleanup_kernel
+      A.event_status[e] = status;
+    }
+    if (DBG) {
+      if (lane == 0) {
+        if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
+        if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
+      }
+      if (lane < ns) {
+        if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
+        if (A.dbg.seed_bins) {
+          A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
+          A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
+          A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
+        }
       }
     }
   }
-  __syncwarp();
 }
 
 template <bool DBG>
-__global__ void __launch_bounds__(512, 1) seed_kernel(const __grid_constant__ KParams P,
-                                                      const __grid_constant__ KArgs A) {
+__global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_constant__ KParams P,
+                                                                   const __grid_constant__ KArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  unsigned char* wsm = smem_raw + (size_t)warp * P.warp_smem_bytes;
+  const int team = threadIdx.x / TEAM, tt = threadIdx.x % TEAM;
+  const int bar = 1 + team;                                // named barrier of the team (0 is __syncthreads)
+  unsigned char* wsm = smem_raw + (size_t)team * P.warp_smem_bytes;
+  int* misc = reinterpret_cast<int*>(wsm + (size_t)P.region0_words * 4 + SM_MISC);
   {
     int4* Z = reinterpret_cast<int4*>(wsm);                // histogram and touched-word flags start at zero
     const int nq = (P.region0_words * 4 + SM_TWL) >> 4;
 #pragma unroll 1
-    for (int i = lane; i < nq; i += 32) Z[i] = make_int4(0, 0, 0, 0);
+    for (int i = tt; i < nq; i += TEAM) Z[i] = make_int4(0, 0, 0, 0);
   }
-  __syncwarp();
-  int e = 0;
-  if (lane == 0) e = (int)atomicAdd(A.evt_counter, 1u);
-  e = __shfl_sync(FULL, e, 0);
+  if (tt == 0) misc[8] = (int)atomicAdd(A.evt_counter, 1u);
+  team_sync(bar);
+  int e = misc[8];
   while (e < A.n_events) {
     int nxt = 0;
-    if (lane == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);   // issued now, consumed after this event
-    seed_event<DBG>(e, P, A, wsm, lane);
-    e = __shfl_sync(FULL, nxt, 0);
+    if (tt == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);  // issued now, consumed after this event
+    seed_event<DBG>(e, P, A, wsm, tt, bar);
+    team_sync(bar);                                        // the team is done with this event's shared memory
+    if (tt == 0) misc[8] = nxt;
+    team_sync(bar);
+    e = misc[8];
   }
 }
 
