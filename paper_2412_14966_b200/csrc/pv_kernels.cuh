@@ -1017,6 +1017,9 @@ __global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KP
   const int t0 = __ldg(A.offsets + e);
   const int n = __ldg(A.offsets + e + 1) - t0;
   const size_t ev = (size_t)e * P.max_vtx;
+  int sv[4];                                               // seed index of my first four tracks: loads issued now,
+#pragma unroll                                             // consumed after the vertex sweep
+  for (int q = 0; q < 4; ++q) sv[q] = (lane + 32 * q < n) ? A.trk_vertex[t0 + lane + 32 * q] : -1;
   float vp[3] = {0.0f, 0.0f, 0.0f}, vc[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
   float vchi2 = 0.0f;
   int vntrk = 0, vniter = -1;
@@ -1098,13 +1101,16 @@ __global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KP
   }
   if (lane == 0) A.n_vtx[e] = __popc(kept);
   // final per-track outputs; tracks of rejected vertices are released (R-9)
-  for (int i = lane; i < n; i += 32) {
-    const int s = A.trk_vertex[t0 + i];
+  auto finish = [&](int i, int s) {
     int vtx = -1;
     if (s >= 0 && ((kept >> s) & 1u)) vtx = __popc(kept & ((1u << s) - 1u));
     A.trk_vertex[t0 + i] = vtx;
     if (vtx < 0) A.trk_weight[t0 + i] = 0.0f;
-  }
+  };
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+    if (lane + 32 * q < n) finish(lane + 32 * q, sv[q]);
+  for (int i = 128 + lane; i < n; i += 32) finish(i, A.trk_vertex[t0 + i]);
 }
 
 }  // namespace pvk
