@@ -171,38 +171,33 @@ __device__ __forceinline__ int sweep(const int* __restrict__ H, int b0, const KP
     if (wbase >= 0 && wbase + lj < P.max_vtx) { sb[wbase + lj] = lb; se[wbase + lj] = le; sp[wbase + lj] = lp; }
   };
   int k = b0 + 1;
+  // The state machine is written with selects: one step is ~30 straight-line instructions (the branchy form
+  // cost ~45 with the register moves at its merge points); only the rare split is a branch.
 #pragma unroll 1
   for (; k < P.nbins; ++k) {
     h = H[k];
     if (!(h > P.T_bin)) break;
-    const int prev_sum = sum;
-    const int prev_amax = amax, prev_amaxp = amaxp;
+    const bool c_up = h > mx, c_dn = mx - h > P.D, c_lt = h < mn, c_rise = h - mn > P.D;
+    const bool to_min = look_max && !c_up && c_dn;          // a significant maximum lies behind: look for the minimum
+    const bool new_min = to_min || (!look_max && c_lt);     // this bin is the running minimum
+    const bool to_max = !look_max && !c_lt && c_rise;       // significant minimum at mnp, with a maximum on either side
+    snap_sum = new_min ? sum : snap_sum;                    // integral and argmax of [start, k): before this bin
+    snap_amax = new_min ? amax : snap_amax;
+    snap_amaxp = new_min ? amaxp : snap_amaxp;
     sum += h;
-    if (h > amax) { amax = h; amaxp = k; }
-    if (h > smax) { smax = h; smaxp = k; }
-    if (look_max) {
-      if (h > mx) {
-        mx = h;
-      } else if (mx - h > P.D) {             // a significant maximum lies behind: start looking for the minimum
-        mn = h; mnp = k; look_max = false;
-        snap_sum = prev_sum; snap_amax = prev_amax; snap_amaxp = prev_amaxp;
-        smax = h; smaxp = k;
-      }
-    } else {
-      if (h < mn) {
-        mn = h; mnp = k;
-        snap_sum = prev_sum; snap_amax = prev_amax; snap_amaxp = prev_amaxp;
-        smax = h; smaxp = k;
-      } else if (h - mn > P.D) {             // significant minimum at mnp, with a maximum on either side
-        mx = h; look_max = true;
-        if (snap_sum >= P.I_min[bin_region(snap_amaxp, P)]) {
-          if (have) flush();
-          lb = start; le = mnp; lp = snap_amaxp; lpv = snap_amax; lj = count; have = true;
-          ++count;
-          start = mnp;                       // the minimum bin opens the right-hand cluster
-          sum -= snap_sum; amax = smax; amaxp = smaxp;
-        }
-      }
+    const bool g1 = h > amax;
+    amax = g1 ? h : amax; amaxp = g1 ? k : amaxp;
+    const bool g2 = new_min || h > smax;
+    smax = g2 ? h : smax; smaxp = g2 ? k : smaxp;
+    mn = new_min ? h : mn; mnp = new_min ? k : mnp;
+    mx = ((look_max && c_up) || to_max) ? h : mx;
+    look_max = (look_max && !to_min) || to_max;
+    if (to_max && snap_sum >= P.I_min[bin_region(snap_amaxp, P)]) {
+      if (have) flush();
+      lb = start; le = mnp; lp = snap_amaxp; lpv = snap_amax; lj = count; have = true;
+      ++count;
+      start = mnp;                                         // the minimum bin opens the right-hand cluster
+      sum -= snap_sum; amax = smax; amaxp = smaxp;
     }
   }
   // tail [start, k)
