@@ -5,3 +5,4 @@ this package is its thin Python binding.
 """
 from .binding import (DeviceBatch, HostPipeline, Params, Debug, PvError, default_params, find, lib, nbins,  # noqa: F401
                       workspace_bytes, last_launch_info, EXPORTS, FIELDS)
+from . import shard  # noqa: F401,E402

@@ -88,6 +88,42 @@ def test_empty_and_degenerate_events(pv, oracle):
     assert list(got["n_vtx"][[0, 2, 3, 7]]) == [0, 0, 0, 0]
 
 
+def test_wide_tracks_many_fill_units(pv, oracle):
+    """Events whose tracks have sigma_poca of several mm in the p-gas region (window of up to ~240 bins = 30 fill
+    units each): the flat unit list of a chunk overflows its capacity and is processed in several rounds; a
+    second event mixes such tracks with narrow ones across the two-chunk boundary."""
+    rng = np.random.default_rng(11)
+
+    def gas_event(n, sig_lo, sig_hi, slope):
+        z0 = -450.0
+        tx = rng.normal(0, slope, n).astype(np.float32)
+        ty = rng.normal(0, slope, n).astype(np.float32)
+        sig = rng.uniform(sig_lo, sig_hi, n).astype(np.float32)
+        ev = dict(x=(sig * rng.normal(0, 1, n)).astype(np.float32), y=(sig * rng.normal(0, 1, n)).astype(np.float32),
+                  z=np.full(n, z0, np.float32), tx=tx, ty=ty, var_x=sig * sig, var_y=sig * sig,
+                  var_tx=np.full(n, 1e-6, np.float32), var_ty=np.full(n, 1e-6, np.float32))
+        return ev
+    wide = gas_event(200, 0.3, 0.6, 0.08)          # sigma_poca ~ 4..10 mm: most pass the 10 mm gas cut
+    mixed = gas_event(150, 0.01, 0.5, 0.1)
+    data = events.from_lists([wide, mixed, gas_event(40, 0.02, 0.05, 0.15)])
+    got, ref, rep = _both(pv, oracle, data)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep, allow_ties_frac=0.5)
+    sp = ref["debug"]["sigma_poca"][:200]
+    assert (sp > 5.0).sum() > 30 and rep["hist_mismatch"] == 0      # units per chunk well above the list capacity
+    assert ref["debug"]["hist"][0].sum() > 100 * (1 << 20)
+
+
+@pytest.mark.parametrize("n", [1000, 10000])
+def test_batch_sweep_config4(pv, oracle, n):
+    """configs[4] (seed 5, the configs[1] event model) at the batch sizes the oracle finishes in seconds; the
+    larger sizes of the sweep are bench.py --config 4 --events N runs."""
+    data = events.generate(events.config(4, n))
+    got, ref, rep = _both(pv, oracle, data, n_hist=200)
+    _assert_parity(rep)
+    assert rep["assign_agreement"] >= 0.999
+
+
 def test_too_many_tracks_and_vertex_overflow(pv, oracle):
     """An event above PV_MAX_TRACKS_PER_EVENT is skipped with its flag; max_vtx_per_event smaller than the
     number of seeds keeps the first ones in z and flags the event."""
