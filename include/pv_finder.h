@@ -83,8 +83,9 @@ int pv_params_default(pv_params* p);
 int pv_nbins(const pv_params* p);
 
 /* Bytes of DEVICE workspace pv_find needs for a batch of this size: 256 B of counters, one 16-byte seed
- * record per (event, vertex slot) and 2 B per track (track lists sorted by seed) handed from the seed kernel
- * to the fit kernel.  The histograms live in shared memory ("one block per event").  bytes: HOST out. */
+ * record per (event, vertex slot) and one 32-byte fit-ready track record per track (tracks sorted by seed,
+ * in the seed's local frame with W = V^-1 at the seed position) handed from the seed kernel to the
+ * fit kernel.  The histograms live in shared memory ("one block per event").  bytes: HOST out. */
 int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, size_t* bytes);
 
 /* The hot path a1..a6 over a batch.
