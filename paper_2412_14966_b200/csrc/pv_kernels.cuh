@@ -558,6 +558,10 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     }
     return s;
   };
+  int sheld[SLOTS];
+#pragma unroll
+  for (int sl = 0; sl < SLOTS; ++sl) sheld[sl] = -1;
+  static_assert(SLOTS == 2, "sheld[] is filled for two slots");
   for (;;) {
     if (ns == 0) break;
     if (tw == 0) part[lane] = lane + 1 < ns ? (se[lane] + sb[lane + 1]) / 2 : 0x7fffffff;
@@ -566,6 +570,8 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
 #pragma unroll 1
     for (int i0 = tw * 32; i0 < n; i0 += TEAM) {
       const int s = seed_of(i0 + lane);
+      if (i0 < TEAM) sheld[0] = s;                         // seeds of my register-held tracks, reused by the sort
+      else if (i0 < CHUNK) sheld[1] = s;
       const unsigned m = __match_any_sync(FULL, s);
       if (s >= 0 && (m & lanemask_lt()) == 0) cnt[tw * 32 + s] += __popc(m);
       __syncwarp();
@@ -604,8 +610,7 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     cur[lane] = myoff + ((tw && ns > 0) ? cnt[lane] : 0);
   }
   __syncwarp();
-  auto place = [&](const int i, const RawTrk& R, const bool from_memory) {
-    const int s = seed_of(i);
+  auto place = [&](const int i, const RawTrk& R, const bool from_memory, const int s) {
     if (i < n) {
       A.trk_vertex[t0 + i] = s;                            // scratch: seed index, read back by cleanup_kernel
       if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
@@ -633,9 +638,9 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   };
 #pragma unroll
   for (int sl = 0; sl < SLOTS; ++sl)
-    if (sl * TEAM + tw * 32 < n) place(sl * TEAM + tt, held[sl], false);
+    if (sl * TEAM + tw * 32 < n) place(sl * TEAM + tt, held[sl], false, ns > 0 ? sheld[sl] : -1);
 #pragma unroll 1
-  for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) place(i0 + lane, held[0], true);
+  for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) place(i0 + lane, held[0], true, seed_of(i0 + lane));
   // seed records for fit_kernel
   if (tw == 0) {
     int rbase = 0;
