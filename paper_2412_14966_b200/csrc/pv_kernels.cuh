@@ -57,8 +57,8 @@ constexpr int SM_STAGE = SM_MISC + 64;                 // float zp[128], inv[128
 constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // uint16 list[256]  (fill)
 constexpr int SM_BINS = SM_LIST + LIST_CAP * 2;        // int16 binsm[256]     central bins of the first 256 tracks
 constexpr int SM_TAIL_BYTES = SM_BINS + BINS_SM * 2;
-// peak search overlays on the (dead) stage and list: uint16 protostart[2][PROTO_CAP]; int sb1[32], se1[32], sp1[32]
-static_assert(TEAM_WARPS * PROTO_CAP * 2 + 3 * MAXV * 4 <= CHUNK * 12 + LIST_CAP * 2, "peak-search overlays fit");
+// peak search overlay on the (dead) stage and list: uint16 protostart[2][PROTO_CAP]
+static_assert(TEAM_WARPS * PROTO_CAP * 2 <= CHUNK * 12 + LIST_CAP * 2, "peak-search overlay fits");
 static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0 && SM_TAIL_BYTES % 16 == 0, "alignment of the vector accesses");
 
 struct KParams {
@@ -307,10 +307,6 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   int* st_lonb = reinterpret_cast<int*>(st_inv + CHUNK);
   uint16_t* list = reinterpret_cast<uint16_t*>(tail + SM_LIST);
   // overlays of the peak search: stage and list are dead after the fill
-  uint16_t* protostart = reinterpret_cast<uint16_t*>(tail + SM_STAGE) + tw * PROTO_CAP;
-  int* sb1 = reinterpret_cast<int*>(tail + SM_STAGE + TEAM_WARPS * PROTO_CAP * 2);
-  int* se1 = sb1 + MAXV;
-  int* sp1 = se1 + MAXV;
   int16_t* binsm = reinterpret_cast<int16_t*>(tail + SM_BINS);
 
   const int t0 = __ldg(A.offsets + e);
@@ -458,86 +454,103 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   team_sync(bar);
   if (tw == 1) reinterpret_cast<unsigned*>(tb)[lane] = 0;  // clean for the next event (both warps have read it)
 
-  // Each warp takes half of the touched words: proto-cluster starts, then one lane per proto-cluster for the
-  // z-ordered sweep; warp 0 writes its seeds to (sb, se, sp), warp 1 to (sb1, se1, sp1), appended afterwards.
-  int nraw_w = 0;
+  // Both warps look for proto-cluster starts, each in its half of the touched words; then warp 0 alone runs the
+  // z-ordered sweeps with one lane per proto-cluster of the whole event (the number of serial sweep steps is the
+  // longest proto-cluster of the event, once) and computes the seed positions.
+  uint16_t* ps0 = reinterpret_cast<uint16_t*>(tail + SM_STAGE);
+  uint16_t* ps1 = ps0 + PROTO_CAP;
+  // proto-cluster starts of the words [i, iend) -> ps[0 .. return value); stops early (i < iend) when ps is full
+  auto detect = [&](int& i, const int iend, uint16_t* ps) -> int {
+    int prev_w = -2;
+    unsigned prev_m = 0;
+    if (i > 0 && i < iend) {                               // does a run continue from the word before this range?
+      const int pw = twl[i - 1];
+      if (pw == (int)twl[i] - 1) { prev_w = pw; prev_m = (H[pw * 32 + 31] > P.T_bin) ? 0x80000000u : 0u; }
+    }
+    int n_proto = 0;
+#pragma unroll 1
+    for (; i < iend && n_proto + 16 <= PROTO_CAP; ++i) {   // a word of 32 bins starts at most 16 runs
+      const int w = twl[i];
+      const int b = w * 32 + lane;                         // bins beyond nbins are padding and stay 0
+      const unsigned m = __ballot_sync(FULL, H[b] > P.T_bin);
+      const unsigned carry = (prev_w == w - 1) ? (prev_m >> 31) : 0u;
+      const unsigned starts = m & ~((m << 1) | carry);     // first bin of each run of bins above threshold
+      if ((starts >> lane) & 1u) ps[n_proto + __popc(starts & lanemask_lt())] = (uint16_t)b;
+      n_proto += __popc(starts);
+      prev_w = w; prev_m = m;
+    }
+    return n_proto;
+  };
+  int n_raw = 0;                                           // valid in warp 0 until published through misc[4]
+  // sweeps of the n0 + n1 proto-clusters listed in ps0[0..n0) and ps1[0..n1), appended to (sb, se, sp)
+  auto sweep_all = [&](const int n0, const int n1) {
+#pragma unroll 1
+    for (int p0 = 0; p0 < n0 + n1; p0 += 32) {             // one lane per proto-cluster
+      const int p = p0 + lane;
+      const bool act = p < n0 + n1;
+      const int b0 = act ? (int)(p < n0 ? ps0[p] : ps1[p - n0]) : 0;
+      Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
+      int c = 0, base = 0;
+#pragma unroll 1
+      for (int rep = 0; rep < 2; ++rep) {                  // rep 1 (rare): proto-clusters with three or more seeds
+        const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
+        if (!__any_sync(FULL, run)) break;
+        if (run) {
+          const int cc = sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+          if (rep == 0) c = cc;
+        }
+        if (rep == 0) {
+          const int inc = warp_incl_scan(c, lane);
+          base = n_raw + inc - c;
+          if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
+          if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
+          n_raw += __shfl_sync(FULL, inc, 31);
+        }
+      }
+    }
+  };
   {
     const int half = (ntw + 1) >> 1;
     int i = tw ? half : 0;
     const int iend = tw ? ntw : half;
-    int* wb_ = tw ? sb1 : sb;
-    int* we_ = tw ? se1 : se;
-    int* wp_ = tw ? sp1 : sp;
-    int prev_w = -2;
-    unsigned prev_m = 0;
-    if (i > 0 && i < iend) {                               // does a run continue from the other warp's last word?
-      const int pw = twl[i - 1];
-      if (pw == (int)twl[i] - 1) { prev_w = pw; prev_m = (H[pw * 32 + 31] > P.T_bin) ? 0x80000000u : 0u; }
+    const int np_ = detect(i, iend, tw ? ps1 : ps0);
+    if (lane == 0) {
+      misc[2 + tw] = np_;
+      if (i < iend) misc[6] = 1;                           // list full (never with physical histograms): slow path
     }
-#pragma unroll 1
-    while (i < iend) {                                     // rounds of <= PROTO_CAP proto-clusters (one in practice)
-      int n_proto = 0;
-#pragma unroll 1
-      for (; i < iend && n_proto + 16 <= PROTO_CAP; ++i) { // a word of 32 bins starts at most 16 runs
-        const int w = twl[i];
-        const int b = w * 32 + lane;
-        const unsigned m = __ballot_sync(FULL, b < P.nbins && H[b] > P.T_bin);
-        const unsigned carry = (prev_w == w - 1) ? (prev_m >> 31) : 0u;
-        const unsigned starts = m & ~((m << 1) | carry);   // first bin of each run of bins above threshold
-        if ((starts >> lane) & 1u) protostart[n_proto + __popc(starts & lanemask_lt())] = (uint16_t)b;
-        n_proto += __popc(starts);
-        prev_w = w; prev_m = m;
-      }
-      __syncwarp();
-#pragma unroll 1
-      for (int p0 = 0; p0 < n_proto; p0 += 32) {           // one lane per proto-cluster
-        const int p = p0 + lane;
-        const bool act = p < n_proto;
-        const int b0 = act ? (int)protostart[p] : 0;
-        Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
-        int c = 0, base = 0;
-#pragma unroll 1
-        for (int rep = 0; rep < 2; ++rep) {                // rep 1 (rare): proto-clusters with three or more seeds
-          const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
-          if (!__any_sync(FULL, run)) break;
-          if (run) {
-            const int cc = sweep(H, b0, P, rep ? base : -1, wb_, we_, wp_, c0, c1);
-            if (rep == 0) c = cc;
-          }
-          if (rep == 0) {
-            const int inc = warp_incl_scan(c, lane);
-            base = nraw_w + inc - c;
-            if (c > 0 && base < P.max_vtx) { wb_[base] = c0.b; we_[base] = c0.e; wp_[base] = c0.p; }
-            if (c > 1 && base + 1 < P.max_vtx) { wb_[base + 1] = c1.b; we_[base + 1] = c1.e; wp_[base + 1] = c1.p; }
-            nraw_w += __shfl_sync(FULL, inc, 31);
-          }
-        }
-      }
-      __syncwarp();
-    }
-    if (lane == 0) misc[2 + tw] = nraw_w;
   }
   team_sync(bar);
-  const int nraw0 = misc[2];
-  const int n_raw = nraw0 + misc[3];
-  if (tw == 1) {                                           // append warp 1's seeds (they lie above warp 0's in z)
-    const int k = nraw0 + lane;
-    if (lane < min(misc[3], P.max_vtx) && k < P.max_vtx) { sb[k] = sb1[lane]; se[k] = se1[lane]; sp[k] = sp1[lane]; }
+  if (tw == 0) {
+    if (misc[6] == 0) {
+      sweep_all(misc[2], misc[3]);
+    } else {                                               // rounds of <= PROTO_CAP proto-clusters over all words
+      int i = 0;
+#pragma unroll 1
+      while (i < ntw) {
+        __syncwarp();
+        const int np_ = detect(i, ntw, ps0);
+        __syncwarp();
+        sweep_all(np_, 0);
+      }
+    }
+    __syncwarp();
+    const int nsw = min(n_raw, P.max_vtx);
+    if (lane < nsw) {                                      // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
+      const int i = sp[lane];
+      const long long Nm = i > 0 ? H[i - 1] : 0;
+      const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
+      const long long N0 = H[i];
+      const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
+      const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
+      const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
+      zs[lane] = __fmaf_rn(delta, P.dz, zi);
+    }
+    if (lane == 0) { misc[4] = n_raw; misc[6] = 0; }
   }
+  team_sync(bar);
+  n_raw = misc[4];
   int ns = n_raw;
   if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
-  team_sync(bar);
-  if (tw == 0 && lane < ns) {                              // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
-    const int i = sp[lane];
-    const long long Nm = i > 0 ? H[i - 1] : 0;
-    const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
-    const long long N0 = H[i];
-    const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
-    const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
-    const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
-    zs[lane] = __fmaf_rn(delta, P.dz, zi);
-  }
-  team_sync(bar);
   // the histogram is dead from here on: clear what this event touched for the next one
 #pragma unroll 1
   for (int i = tw; i < ntw; i += TEAM_WARPS) H[(int)twl[i] * 32 + lane] = 0;
@@ -686,7 +699,7 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
 #pragma unroll 1
     for (int i = tt; i < nq; i += TEAM) Z[i] = make_int4(0, 0, 0, 0);
   }
-  if (tt == 0) misc[8] = (int)atomicAdd(A.evt_counter, 1u);
+  if (tt == 0) { misc[6] = 0; misc[8] = (int)atomicAdd(A.evt_counter, 1u); }
   team_sync(bar);
   int e = misc[8];
   while (e < A.n_events) {
