@@ -114,6 +114,38 @@ def test_wide_tracks_many_fill_units(pv, oracle):
     assert ref["debug"]["hist"][0].sum() > 100 * (1 << 20)
 
 
+def test_many_proto_clusters_slow_path(pv, oracle):
+    """A comb of 580 isolated narrow tracks 1 mm apart (one proto-cluster each, none with the integral of a seed)
+    plus a few real vertices: more proto-cluster starts than one warp's list holds, so the peak search takes its
+    round-based path; seeds must still come out z-ordered and bit-exact."""
+    rng = np.random.default_rng(7)
+    zc = np.arange(-290.0, 290.0, 1.0)
+    pv_z = np.array([-250.3, -100.1, 10.2, 150.4, 280.6])
+    z = np.concatenate([zc, np.repeat(pv_z, 8)]).astype(np.float32)
+    n = z.size
+    phi = rng.uniform(0, 2 * np.pi, n)
+    sl = 0.3
+    ev = dict(x=rng.normal(0, 0.01, n).astype(np.float32), y=rng.normal(0, 0.01, n).astype(np.float32), z=z,
+              tx=(sl * np.cos(phi)).astype(np.float32), ty=(sl * np.sin(phi)).astype(np.float32),
+              var_x=np.full(n, 1e-4, np.float32), var_y=np.full(n, 1e-4, np.float32),
+              var_tx=np.full(n, 1e-6, np.float32), var_ty=np.full(n, 1e-6, np.float32))
+    perm = rng.permutation(n)
+    ev = {k: v[perm] for k, v in ev.items()}
+    small = events.generate(events.config(0, 2))
+    so = small["offsets"]
+    data = events.from_lists([ev, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, ev])
+    got, ref, rep = _both(pv, oracle, data)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep, allow_ties_frac=0.5)
+    H = ref["debug"]["hist"][0]
+    above = H > int(0.25 * (1 << 20))
+    starts = above & ~np.concatenate([[False], above[:-1]])
+    words = np.flatnonzero(H.reshape(-1, 1)[: (H.size // 32) * 32].reshape(-1, 32).any(axis=1))
+    half = words[(len(words) + 1) // 2 - 1]
+    assert starts[: (half + 1) * 32].sum() > 256                   # the first warp's list overflows
+    assert ref["n_vtx"][0] == 5 and got["n_vtx"][0] == 5 and got["n_vtx"][2] == 5
+
+
 @pytest.mark.parametrize("n", [1000, 10000])
 def test_batch_sweep_config4(pv, oracle, n):
     """configs[4] (seed 5, the configs[1] event model) at the batch sizes the oracle finishes in seconds; the
