@@ -38,11 +38,11 @@ constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
 constexpr int UNIT = 8;             // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
-constexpr int FIT_G = 4;            // lanes per vertex in the fit
+constexpr int FIT_G = 2;            // lanes per vertex in the fit
 constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
-constexpr int FIT_KF = 8;           // register-resident tracks per lane (fast path: <= FIT_G*FIT_KF tracks)
-constexpr int FIT_BLOCK = 128;      // threads per CTA of fit_kernel (warps are autonomous)
-constexpr int FIT_MIN_BLOCKS = 4;   // CTAs per SM the register budget is held to
+constexpr int FIT_KF = 16;          // track slots per lane in shared memory (fast path: <= FIT_G*FIT_KF tracks)
+constexpr int FIT_BLOCK = 64;       // threads per CTA of fit_kernel (warps are autonomous; 12 KB of tracks per warp)
+constexpr int FIT_MIN_BLOCKS = 9;   // CTAs per SM: 9 x (24 KB + 1 KB reserved) fill the shared memory
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
 constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
 
@@ -797,9 +797,10 @@ __device__ __forceinline__ void store_vertex(const KArgs& A, size_t o, float x, 
 // ---- fit_kernel: a5, FIT_G lanes per seed (R-12) ---------------------------------------------------
 // Warps are autonomous (no CTA barrier): a warp takes a window of 32 seed records (one per lane), sorts them by
 // track count with a shuffle bitonic sort (so the FIT_VPW seeds it fits together need the same number of
-// register slots), and fits them in 32 / FIT_VPW passes.  Tracks are read as 32-byte fit-ready records
-// (two 16-byte loads) and stay in registers; the normal equations are reduced with xor-shuffles inside the
-// FIT_G lanes; every lane solves its seed's 3x3 system in closed form.
+// track slots), and fits them in 32 / FIT_VPW passes.  The tracks of a pass are copied once (cp.async, 16 + 8
+// bytes of each fit-ready record) into the warp's shared-memory slice, laid out [slot][lane] so that every
+// iteration reads them back conflict-free; with two lanes per seed one shuffle level reduces the normal
+// equations, and every lane solves its seed's 3x3 system in closed form.
 // Results go to slot (event, seed index) of the vertex arrays; cleanup_kernel compacts them in place.
 __device__ __forceinline__ Trk read_track(const KArgs& A, int rec, int& idx) {
   const float4 a = __ldg(A.ftrk + 2 * (size_t)rec), b = __ldg(A.ftrk + 2 * (size_t)rec + 1);
@@ -811,25 +812,21 @@ __device__ __forceinline__ Trk read_track(const KArgs& A, int rec, int& idx) {
 
 __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __grid_constant__ KParams P,
                                                                         const __grid_constant__ KArgs A) {
-  const int lane = threadIdx.x & 31;
+  __shared__ __align__(16) float4 s_a[FIT_BLOCK / 32][FIT_KF][32];   // {x0, y0, tx, ty}
+  __shared__ __align__(8) float2 s_b[FIT_BLOCK / 32][FIT_KF][32];    // {Wx, Wy}
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int j = lane % FIT_G, gl = lane / FIT_G;
+  float4(*SA)[32] = s_a[warp];
+  float2(*SB)[32] = s_b[warp];
   const int total = (int)*A.seed_counter;
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
   const int wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  // Latency hiding without spare registers: the records of the NEXT window are loaded one window ahead and
-  // their track lines prefetched into L2 during this window; the tracks of the next PASS are prefetched into L1
-  // while this pass iterates.
-  auto prefetch_tracks = [&](int begin, int m, int first, int step, bool l1) {
+  // the records of the NEXT window are loaded one window ahead and their track lines prefetched into L2
+  auto prefetch_l2 = [&](int begin, int m) {
     const char* base = reinterpret_cast<const char*>(A.ftrk + 2 * (size_t)begin);
     const int bytes = m * 32;
-    for (int off = first * 128; off < bytes; off += step * 128) {
-      if (l1) asm volatile("prefetch.global.L1 [%0];" ::"l"(base + off));
-      else asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
-    }
-    if (first == 0 && bytes > 0) {                         // the records are 32-byte aligned, not line aligned
-      if (l1) asm volatile("prefetch.global.L1 [%0];" ::"l"(base + bytes - 1));
-      else asm volatile("prefetch.global.L2 [%0];" ::"l"(base + bytes - 1));
-    }
+    for (int off = 0; off < bytes; off += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
+    if (bytes > 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + bytes - 1));   // records are not line aligned
   };
   int4 wr_next = make_int4(0, 0, 0, 0);
   if (wg * 32 + lane < total) wr_next = __ldg(reinterpret_cast<const int4*>(A.rec) + wg * 32 + lane);
@@ -852,24 +849,12 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
         key = up ? min(key, other) : max(key, other);
       }
     }
-    {                                                      // first pass of this window: L1 prefetch (short lead)
-      const int src = __shfl_sync(FULL, key, gl) & 31;
-      const int pz = __shfl_sync(FULL, wr.z, src), pm = __shfl_sync(FULL, wr.y, src) >> 5;
-      prefetch_tracks(pz, min(pm, FIT_G * FIT_KF), j, FIT_G, true);
-    }
 #pragma unroll 1
     for (int pass = 0; pass < 32 / FIT_VPW; ++pass) {
       const int src = __shfl_sync(FULL, key, pass * FIT_VPW + gl) & 31;   // lane holding my group's record
       int4 r;
       r.x = __shfl_sync(FULL, wr.x, src); r.y = __shfl_sync(FULL, wr.y, src);
       r.z = __shfl_sync(FULL, wr.z, src); r.w = __shfl_sync(FULL, wr.w, src);
-      if (pass + 1 < 32 / FIT_VPW) {                       // tracks of the next pass -> L1
-        const int nsrc = __shfl_sync(FULL, key, (pass + 1) * FIT_VPW + gl) & 31;
-        const int pz = __shfl_sync(FULL, wr.z, nsrc), pm = __shfl_sync(FULL, wr.y, nsrc) >> 5;
-        prefetch_tracks(pz, min(pm, FIT_G * FIT_KF), j, FIT_G, true);
-      } else {                                             // tracks of the next window -> L2 (one record per lane)
-        prefetch_tracks(wr_next.z, min(wr_next.y >> 5, 2 * FIT_G * FIT_KF), 0, 1, false);
-      }
       const int e = r.x, k = r.y & 31;
       int m = r.y >> 5;
       const bool vact = m > 0;                               // every real seed holds >= 2 tracks
@@ -879,41 +864,42 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
       if (big) m = 0;
       const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
       const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-      Trk T[FIT_KF];
-      float fw[FIT_KF];
       int mmax = m;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) mmax = max(mmax, __shfl_xor_sync(FULL, mmax, o));
-      const int nslot = (mmax + FIT_G - 1) / FIT_G;          // warp-uniform number of register slots in use
-      float nvalid = 0.0f;                                   // usable tracks (unit-weight mode: the active count)
+      const int nslot = (mmax + FIT_G - 1) / FIT_G;          // warp-uniform number of track slots in use
+      // ---- stage the tracks of this pass: slot s of my lane holds track j + FIT_G s of my seed, or a dead track
+      __syncwarp();                                          // the previous pass has finished reading the slice
       {
-        // every lane loads unconditionally (clamped record index), all loads in flight at once; absent slots are
-        // replaced by dead tracks afterwards (predicated loads would chain through the predicate registers)
-        float4 qa[FIT_KF];
-        float2 qb[FIT_KF];
-        const int last = max(m - 1, 0);
-#pragma unroll
-        for (int s = 0; s < FIT_KF; ++s) {
-          const float4* q = A.ftrk + 2 * (size_t)(r.z + min(j + FIT_G * s, last));
-          qa[s] = __ldg(q);
-          qb[s] = __ldg(reinterpret_cast<const float2*>(q + 1));
-        }
         const Trk dead = dead_track(P);
-#pragma unroll
-        for (int s = 0; s < FIT_KF; ++s) {
-          const bool have = j + FIT_G * s < m;
-          T[s].x0 = have ? qa[s].x : dead.x0; T[s].y0 = have ? qa[s].y : dead.y0;
-          T[s].tx = have ? qa[s].z : dead.tx; T[s].ty = have ? qa[s].w : dead.ty;
-          T[s].Wx = have ? qb[s].x : dead.Wx; T[s].Wy = have ? qb[s].y : dead.Wy;
-          fw[s] = 0.0f;
-          nvalid += track_is_dead(T[s], P) ? 0.0f : 1.0f;
+#pragma unroll 1
+        for (int s = 0; s < nslot; ++s) {
+          const int t = j + FIT_G * s;
+          if (t < m) {
+            const float4* q = A.ftrk + 2 * (size_t)(r.z + t);
+            const unsigned da = (unsigned)__cvta_generic_to_shared(&SA[s][lane]);
+            const unsigned db = (unsigned)__cvta_generic_to_shared(&SB[s][lane]);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(da), "l"(q) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(db), "l"(q + 1) : "memory");
+          } else {
+            SA[s][lane] = make_float4(dead.x0, dead.y0, dead.tx, dead.ty);
+            SB[s][lane] = make_float2(dead.Wx, dead.Wy);
+          }
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
       }
+      if (pass + 1 == 32 / FIT_VPW) prefetch_l2(wr_next.z, min(wr_next.y >> 5, 2 * FIT_G * FIT_KF));
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncwarp();
+      float nvalid = 0.0f;                                   // usable tracks (unit-weight mode: the active count)
       if (P.unit_weights) {
+#pragma unroll 1
+        for (int s = 0; s < nslot; ++s) nvalid += (SB[s][lane].x > 0.0f) ? 1.0f : 0.0f;
 #pragma unroll
         for (int o = FIT_G / 2; o > 0; o >>= 1) nvalid += __shfl_xor_sync(FULL, nvalid, o);
       }
       float ax = 0.0f, ay = 0.0f, az = 0.0f;
+      float lx = 0.0f, ly = 0.0f, lz = 0.0f;               // position the weights of the last iteration were taken at
       bool run = vact && !big;
       bool sing = false;
       int niter = 0;
@@ -923,10 +909,13 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
       for (int it = 1; it <= P.max_iter; ++it) {
         Sums S;
         sums_zero(S);
-        if (run) {
-#pragma unroll
-          for (int s = 0; s < FIT_KF; ++s)
-            if (s < nslot) fw[s] = track_accum(T[s], ax, ay, az, P, S);
+#pragma unroll 4
+        for (int s = 0; s < nslot; ++s) {
+          const float4 qa = SA[s][lane];
+          const float2 qb = SB[s][lane];
+          Trk T;
+          T.x0 = qa.x; T.y0 = qa.y; T.tx = qa.z; T.ty = qa.w; T.Wx = qb.x; T.Wy = qb.y;
+          track_accum(T, ax, ay, az, P, S);
         }
         sums_reduce<FIT_G>(S);
         if (P.unit_weights) S.nact = nvalid;
@@ -935,6 +924,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
           if (!newton_step(S, dx, dy, dzs, dchi2, C)) {
             sing = true; run = false;
           } else {
+            lx = ax; ly = ay; lz = az;
             ax += dx; ay += dy; az += dzs;
             chi2 = S.chi2; nact = S.nact; niter = it;
             if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) run = false;
@@ -948,17 +938,22 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
           if (j == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
         } else {
           if (j == 0) store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)nact, niter);
-#pragma unroll
-          for (int s = 0; s < FIT_KF; ++s) {
-            const int t = j + FIT_G * s;
-            if (t < m) {
-              const int idx = __float_as_int(__ldg(reinterpret_cast<const float*>(A.ftrk + 2 * (size_t)(r.z + t) + 1) + 2));
-              A.trk_weight[idx] = track_is_dead(T[s], P) ? 0.0f : fw[s];
-            }
+#pragma unroll 4
+          for (int t = j; t < m; t += FIT_G) {             // weights of the last iteration: the same arithmetic again
+            const int s = t / FIT_G;
+            const float4 qa = SA[s][lane];
+            const float2 qb = SB[s][lane];
+            Trk T;
+            T.x0 = qa.x; T.y0 = qa.y; T.tx = qa.z; T.ty = qa.w; T.Wx = qb.x; T.Wy = qb.y;
+            Sums dummy;
+            sums_zero(dummy);
+            const float w = track_accum(T, lx, ly, lz, P, dummy);
+            const int idx = __float_as_int(__ldg(reinterpret_cast<const float*>(A.ftrk + 2 * (size_t)(r.z + t) + 1) + 2));
+            A.trk_weight[idx] = track_is_dead(T, P) ? 0.0f : w;
           }
         }
       }
-      // Seeds with more tracks than the register-resident path holds: the whole warp strides over the seed's
+      // Seeds with more tracks than the shared-memory slots hold: the whole warp strides over the seed's
       // records (contiguous, L1-resident after the first iteration).
       unsigned bigm = __ballot_sync(FULL, vact && big && j == 0);
       while (bigm) {
