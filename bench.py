@@ -98,12 +98,12 @@ def algorithmic_bytes(data, n_vtx_total: int) -> int:
 
 def algorithmic_bytes_by_kernel(data, n_vtx_total: int):
     """The same compulsory bytes attributed to the kernel that first reads / last writes them:
-    seed reads the 6 arrays of Eq. 1 / Eq. 3 and the offsets; fit reads the other 3 (var_y, var_tx, var_ty) and
-    writes trk_weight; cleanup writes the vertices, n_vtx, status and trk_vertex.  Intermediate records (seed
-    records, sorted track lists, per-seed fit slots) and re-reads are NOT algorithmic."""
+    seed reads the nine input arrays and the offsets; fit writes trk_weight; cleanup writes the vertices, n_vtx,
+    status and trk_vertex.  Intermediate records (seed records, the seed-sorted fit-ready track records, per-seed
+    fit slots) and re-reads are NOT algorithmic."""
     T = int(data["offsets"][-1])
     E = int(data["offsets"].size - 1)
-    return {"seed_kernel": T * 24 + (E + 1) * 4, "fit_kernel": T * 12 + T * 4,
+    return {"seed_kernel": T * 36 + (E + 1) * 4, "fit_kernel": T * 4,
             "cleanup_kernel": T * 4 + n_vtx_total * 48 + E * 8}
 
 
