@@ -38,6 +38,8 @@ void pvo_params_default(pvo_params *p) {
   p->merge_ratio = 25.0f;                                        /* P:L245 */
   p->max_beam_dist = 0.3f;                                       /* P:L247 */
   p->max_vtx_per_event = 32;
+  p->flavour = 0;                                                /* explicit association + Tukey (x86 flavour) */
+  p->chi2_window = 25.0f;                                        /* P:L384 "within a certain chi2_i"; value: R-13 */
 }
 
 int pvo_nbins(const pvo_params *p) {
@@ -303,12 +305,26 @@ static void chol3_solve(const double L[3][3], const double b[3], double x[3]) {
   }
 }
 
+/* Eq. 19: w_ij = exp(-chi2_ij / 2) / (exp(-chi2_max / 2) + sum_k exp(-chi2_ik / 2)); the sum runs over
+ * all vertex candidates k including j itself. */
+double pvo_mv_weight(double chi2_own, double chi2_max, const double *chi2_others, int n_others) {
+  double den = exp(-0.5 * chi2_max) + exp(-0.5 * chi2_own);
+  for (int k = 0; k < n_others; ++k) den += exp(-0.5 * chi2_others[k]);
+  return exp(-0.5 * chi2_own) / den;
+}
+/* The same with the part of the denominator that does not depend on vertex j precomputed:
+ * other = exp(-chi2_max / 2) + sum_{k != j} exp(-chi2_ik / 2). */
+static double pvo_mv_weight_den(double chi2_own, double other) {
+  double E = exp(-0.5 * chi2_own);
+  return E / (other + E);
+}
+
 /* One Newton-Raphson iteration (Eq. 6-17) at the vertex position a[]: fills the Tukey weights w[] (Eq. 18),
  * the step (Eq. 13), C (Eq. 14), dchi2 (Eq. 17), chi2 (Eq. 6) and the number of tracks with w > 0.
  * Returns -1 when fewer than 2 tracks are active or the Hessian is not positive definite. */
 static int fit_iteration(int m, const int32_t *idx,
                          const float *x, const float *y, const float *z, const float *tx, const float *ty,
-                         const double *Wx, const double *Wy, const double a[3], double chi2_max,
+                         const double *Wx, const double *Wy, const double a[3], double chi2_max, const double *other,
                          double *w, double step[3], double C[3][3], double *dchi2_o, double *chi2_o, int *nact_o) {
   double A[3][3] = {{0}}, g[3] = {0, 0, 0};
   double chi2 = 0.0;
@@ -321,7 +337,8 @@ static int fit_iteration(int m, const int32_t *idx,
       double rx = (double)x[i] + (a[2] - (double)z[i]) * (double)tx[i] - a[0];
       double ry = (double)y[i] + (a[2] - (double)z[i]) * (double)ty[i] - a[1];
       double chi2_i = rx * rx * Wx[j] + ry * ry * Wy[j];            /* Eq. 7 */
-      if (isinf(chi2_max)) wi = 1.0;
+      if (other) wi = pvo_mv_weight_den(chi2_i, other[j]);          /* Eq. 19, competitors at their seed positions */
+      else if (isinf(chi2_max)) wi = 1.0;
       else if (chi2_i < chi2_max) { double u = 1.0 - chi2_i / chi2_max; wi = u * u; }  /* Eq. 18 */
       /* H_i = [[-1,0,tx],[0,-1,ty]] (Eq. 12); accumulate w H^T W H (Eq. 11 / 2) and w H^T W r (Eq. 10 / 2) */
       double Hm[2][3] = {{-1.0, 0.0, (double)tx[i]}, {0.0, -1.0, (double)ty[i]}};
@@ -362,12 +379,12 @@ static void trace_row(double *trace, int it, const double a[3], double C[3][3], 
   t[9] = dchi2; t[10] = dz;
 }
 
-int pvo_fit(int m, const int32_t *idx,
-            const float *x, const float *y, const float *z, const float *tx, const float *ty,
-            const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-            const double seed[3], const pvo_params *p,
-            double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
-            double *w, double *trace) {
+static int fit_core(int m, const int32_t *idx,
+                    const float *x, const float *y, const float *z, const float *tx, const float *ty,
+                    const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+                    const double seed[3], const pvo_params *p, const double *other,
+                    double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
+                    double *w, double *trace) {
   double a[3] = {seed[0], seed[1], seed[2]};
   double *Wx = (double *)malloc(sizeof(double) * (size_t)(2 * m + 2));
   double *Wy = Wx + m + 1;
@@ -387,11 +404,12 @@ int pvo_fit(int m, const int32_t *idx,
   double C[3][3] = {{0}}, chi2 = 0.0;
   for (int it = 1; it <= p->max_iter; ++it) {
     double step[3], dchi2;
-    if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, a, chi2_max, w, step, C, &dchi2, &chi2, &nact) != 0) { rc = -1; break; }
+    if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, a, chi2_max, other, w, step, C, &dchi2, &chi2, &nact) != 0) { rc = -1; break; }
     for (int k = 0; k < 3; ++k) a[k] += step[k];
     niter = it; rc = 0;
     if (trace && it <= PVO_TRACE_ITERS) trace_row(trace, it, a, C, dchi2, step[2]);
-    /* convergence (x86 flavour) */
+    /* convergence: x86 flavour |dchi2| < 0.01 and |dz| < 1 um; GPU flavour |dz| < 0.5 um only, which
+     * is conv_dchi2 = INFINITY */
     if (fabs(dchi2) < (double)p->conv_dchi2 && fabs(step[2]) < (double)p->conv_dz) break;
   }
   /* Trace only (N1): keep iterating past the stopping point on COPIES, so that a
@@ -401,7 +419,7 @@ int pvo_fit(int m, const int32_t *idx,
     int nactt;
     double *wt = (double *)malloc(sizeof(double) * (size_t)(m + 1));
     for (int it = niter + 1; it <= p->max_iter && it <= PVO_TRACE_ITERS; ++it) {
-      if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, at, chi2_max, wt, stept, Ct, &dchi2t, &chi2t, &nactt) != 0) break;
+      if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, at, chi2_max, other, wt, stept, Ct, &dchi2t, &chi2t, &nactt) != 0) break;
       for (int k = 0; k < 3; ++k) at[k] += stept[k];
       trace_row(trace, it, at, Ct, dchi2t, stept[2]);
     }
@@ -413,7 +431,50 @@ int pvo_fit(int m, const int32_t *idx,
   out_cov[0] = C[0][0]; out_cov[1] = C[0][1]; out_cov[2] = C[0][2];
   out_cov[3] = C[1][1]; out_cov[4] = C[1][2]; out_cov[5] = C[2][2];
   *out_chi2 = chi2; *out_ntrk = nact; *out_niter = niter;
+  if (other) {                                        /* R-13: "associated" = final weight >= 1/2 */
+    int na = 0;
+    for (int j = 0; j < m; ++j) if (w[j] >= 0.5) ++na;
+    *out_ntrk = na;
+  }
   return 0;
+}
+
+int pvo_fit(int m, const int32_t *idx,
+            const float *x, const float *y, const float *z, const float *tx, const float *ty,
+            const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+            const double seed[3], const pvo_params *p,
+            double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
+            double *w, double *trace) {
+  return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, NULL, out_pos, out_cov, out_chi2,
+                  out_ntrk, out_niter, w, trace);
+}
+
+/* Multi-vertex flavour: the same Newton-Raphson fit with the weights of Eq. 19.  other[j] is, for
+ * listed track j, exp(-chi2_max / 2) + sum over the OTHER vertex candidates k of exp(-chi2_jk / 2) with chi2_jk
+ * taken at their initial (seed) positions ("the weight is always calculated using the initial position of the
+ * other vertices").  out_ntrk = tracks with final weight >= 1/2. */
+int pvo_fit_mv(int m, const int32_t *idx,
+               const float *x, const float *y, const float *z, const float *tx, const float *ty,
+               const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+               const double seed[3], const pvo_params *p, const double *other,
+               double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
+               double *w, double *trace) {
+  return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, other, out_pos, out_cov, out_chi2,
+                  out_ntrk, out_niter, w, trace);
+}
+
+/* chi2 of track i relative to a vertex candidate at pos[] "evaluated as in Eq. 7" with W from Eq. 2 at that
+ * position; returns a negative number when the extrapolated variance is unusable (R-7). */
+double pvo_track_chi2(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
+                      const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+                      const double pos[3]) {
+  double dz = pos[2] - (double)z[i];
+  double Vx = (double)var_x[i] + dz * dz * (double)var_tx[i];
+  double Vy = (double)var_y[i] + dz * dz * (double)var_ty[i];
+  if (!((Vx > 0.0) && (Vy > 0.0) && isfinite(Vx) && isfinite(Vy))) return -1.0;
+  double rx = (double)x[i] + dz * (double)tx[i] - pos[0];
+  double ry = (double)y[i] + dz * (double)ty[i] - pos[1];
+  return rx * rx / Vx + ry * ry / Vy;
 }
 
 /* ===================================== whole path, one event ========================================= */
@@ -422,6 +483,7 @@ typedef struct scratch {
   int32_t *H, *bin, *flags, *trk_seed, *cb, *ce, *cp, *idx, *s_ntrk, *s_niter, *fate;
   float *zp, *sp, *zs;
   double *s_pos, *s_cov, *s_chi2, *w, *trace;
+  double *Em, *other, *best_w;         /* multi-vertex flavour: exp(-chi2_ik / 2) at the seed positions [n][max_vtx] */
 } scratch;
 
 static scratch *scratch_new(const pvo_params *p) {
@@ -439,11 +501,13 @@ static scratch *scratch_new(const pvo_params *p) {
   s->s_cov = s->s_pos + 3 * mv; s->s_chi2 = s->s_cov + 6 * mv;
   s->w = (double *)malloc(sizeof(double) * (size_t)nt);
   s->trace = (double *)malloc(sizeof(double) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE);
+  s->Em = (double *)malloc(sizeof(double) * ((size_t)nt * (size_t)mv + 2 * (size_t)nt));
+  s->other = s->Em + (size_t)nt * (size_t)mv; s->best_w = s->other + nt;
   return s;
 }
 
 static void scratch_free(scratch *s) {
-  free(s->H); free(s->bin); free(s->cb); free(s->zp); free(s->zs); free(s->s_pos); free(s->w); free(s->trace); free(s);
+  free(s->H); free(s->bin); free(s->cb); free(s->zp); free(s->zs); free(s->s_pos); free(s->w); free(s->trace); free(s->Em); free(s);
 }
 
 static void find_event(int e, const float *x, const float *y, const float *z, const float *tx, const float *ty,
@@ -477,7 +541,9 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
   if (ns > mv) { ns = mv; status |= PVO_EVT_VTX_OVERFLOW; }      /* first max_vtx in z kept (R-8) */
   for (int k = 0; k < ns; ++k) S->zs[k] = pvo_seed_z(S->H, S->cp[k], p);
   /* step 4: track association */
-  ns = pvo_assign(n, S->bin, S->flags, ns, S->cb, S->ce, S->cp, S->zs, p, S->trk_seed);
+  const int mvf = p->flavour == 1;                /* multi-vertex (GPU) flavour: implicit association */
+  if (!mvf) ns = pvo_assign(n, S->bin, S->flags, ns, S->cb, S->ce, S->cp, S->zs, p, S->trk_seed);
+  else for (int i = 0; i < n; ++i) S->trk_seed[i] = -1;
 
   if (dbg) {
     if (dbg->hist && e < dbg->n_hist_events) memcpy(dbg->hist + (size_t)e * nb, S->H, sizeof(int32_t) * (size_t)nb);
@@ -500,23 +566,61 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
   }
 
   /* step 5: vertex fit, one seed at a time */
+  if (mvf) {
+    /* R-13/R-14: every assignable track is implicitly associated to every vertex candidate; E_ik =
+     * exp(-chi2_ik / 2) with chi2_ik "evaluated as in Eq. 7" at the candidates' initial (seed) positions */
+    for (int i = 0; i < n; ++i) {
+      S->best_w[i] = 0.0;
+      for (int k = 0; k < ns; ++k) {
+        float zs = S->zs[k];
+        double pos[3] = {(double)fmaf(p->beam_tx, zs, p->beam_x), (double)fmaf(p->beam_ty, zs, p->beam_y), (double)zs};
+        double c2 = (S->flags[i] & PVO_TRK_ASSIGNABLE)
+                        ? pvo_track_chi2(i, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0, var_ty + t0, pos)
+                        : -1.0;
+        S->Em[(size_t)i * mv + k] = c2 >= 0.0 ? c2 : -1.0;           /* chi2 kept; negative = not usable */
+      }
+    }
+  }
   for (int k = 0; k < ns; ++k) {
     int m = 0;
-    for (int i = 0; i < n; ++i) if (S->trk_seed[i] == k) S->idx[m++] = i;
+    if (!mvf) {
+      for (int i = 0; i < n; ++i) if (S->trk_seed[i] == k) S->idx[m++] = i;
+    } else {
+      /* "only tracks within a certain chi2_i with respect to the vertex candidate are considered" */
+      for (int i = 0; i < n; ++i) {
+        double c2 = S->Em[(size_t)i * mv + k];
+        if (c2 < 0.0 || !(c2 < (double)p->chi2_window)) continue;
+        double oth = exp(-0.5 * (double)p->chi2_max);
+        for (int l = 0; l < ns; ++l) {
+          double cl = S->Em[(size_t)i * mv + l];
+          if (l != k && cl >= 0.0) oth += exp(-0.5 * cl);
+        }
+        S->other[m] = oth;
+        S->idx[m++] = i;
+      }
+    }
     float zs = S->zs[k];
     /* "its xy position is evaluated using the known beamline" */
     double seed[3] = {(double)fmaf(p->beam_tx, zs, p->beam_x), (double)fmaf(p->beam_ty, zs, p->beam_y), (double)zs};
     double chi2 = 0.0;
     memset(S->trace, 0, sizeof(double) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE);
-    int rc = pvo_fit(m, S->idx, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0,
-                     var_ty + t0, seed, p, S->s_pos + 3 * k, S->s_cov + 6 * k, &chi2, &S->s_ntrk[k], &S->s_niter[k],
-                     S->w, S->trace);
+    int rc = fit_core(m, S->idx, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0,
+                      var_ty + t0, seed, p, mvf ? S->other : NULL, S->s_pos + 3 * k, S->s_cov + 6 * k, &chi2,
+                      &S->s_ntrk[k], &S->s_niter[k], S->w, S->trace);
     S->s_chi2[k] = chi2;
     if (rc != 0) { status |= PVO_EVT_SINGULAR_FIT; S->s_niter[k] = -1; }
-    else for (int j = 0; j < m; ++j) trk_weight[t0 + S->idx[j]] = S->w[j];
+    else if (!mvf) for (int j = 0; j < m; ++j) trk_weight[t0 + S->idx[j]] = S->w[j];
+    else for (int j = 0; j < m; ++j) {                 /* R-13: a track follows the candidate with its largest weight */
+      int i = S->idx[j];
+      if (S->w[j] > S->best_w[i]) { S->best_w[i] = S->w[j]; S->trk_seed[i] = k; }
+    }
     if (dbg && dbg->trace)
       memcpy(dbg->trace + ((size_t)e * mv + k) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE, S->trace,
              sizeof(double) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE);
+  }
+  if (mvf) {
+    for (int i = 0; i < n; ++i) trk_weight[t0 + i] = S->trk_seed[i] >= 0 ? S->best_w[i] : 0.0;
+    if (dbg && dbg->trk_seed) for (int i = 0; i < n; ++i) dbg->trk_seed[t0 + i] = S->trk_seed[i];
   }
 
   /* cleanup O8.  Duplicate removal: greedy sweep in seed (= z) order; duplicate iff

@@ -33,6 +33,10 @@ typedef struct pvo_params {
   float merge_ratio;                   /* 25 */
   float max_beam_dist;                 /* 0.3 mm */
   int32_t max_vtx_per_event;           /* output stride */
+  int32_t flavour;                     /* 0: explicit association + Tukey weights (x86, Eq. 18);
+                                          1: implicit association + multi-vertex weights (GPU, Eq. 19) */
+  float chi2_window;                   /* flavour 1: tracks with chi2 < this at the seed position take part in a
+                                          vertex fit (value 25: reading R-13) */
 } pvo_params;
 
 enum { PVO_S = 1 << 20 };              /* fixed-point unit: one track's full mass */
@@ -81,6 +85,21 @@ int pvo_fit(int m, const int32_t *idx,
             const double seed[3], const pvo_params *p,
             double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
             double *w, double *trace);
+
+/* Eq. 19: multi-vertex weight of a track with chi2_own to this vertex, chi2_others[] to the others. */
+double pvo_mv_weight(double chi2_own, double chi2_max, const double *chi2_others, int n_others);
+/* chi2 of track i relative to a vertex at pos[3] (Eq. 7 with W from Eq. 2 at pos); < 0 = unusable (R-7). */
+double pvo_track_chi2(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
+                      const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+                      const double pos[3]);
+/* O7, multi-vertex flavour: pvo_fit with the weights of Eq. 19; other[j] = exp(-chi2_max / 2) + sum over the
+ * other candidates of exp(-chi2_jk / 2) at their seed positions.  out_ntrk = tracks with w >= 1/2. */
+int pvo_fit_mv(int m, const int32_t *idx,
+               const float *x, const float *y, const float *z, const float *tx, const float *ty,
+               const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+               const double seed[3], const pvo_params *p, const double *other,
+               double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
+               double *w, double *trace);
 
 /* Optional taps of the full pipeline (all nullable). */
 typedef struct pvo_debug {

@@ -36,6 +36,7 @@ class Params(C.Structure):
         ("min_tracks_pv", C.c_int32 * 2), ("chi2_max", C.c_float), ("max_iter", C.c_int32),
         ("conv_dchi2", C.c_float), ("conv_dz", C.c_float), ("merge_ratio", C.c_float),
         ("max_beam_dist", C.c_float), ("max_vtx_per_event", C.c_int32),
+        ("flavour", C.c_int32), ("chi2_window", C.c_float),
     ]
 
 
@@ -79,6 +80,10 @@ def lib():
         L.pvo_assign.restype = C.c_int
         L.pvo_fit.restype = C.c_int
         L.pvo_find.restype = C.c_int
+        L.pvo_fit_mv.restype = C.c_int
+        L.pvo_mv_weight.restype = C.c_double
+        L.pvo_mv_weight.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_int]
+        L.pvo_track_chi2.restype = C.c_double
         _lib = L
     return _lib
 
@@ -175,6 +180,42 @@ def fit(tracks: Dict[str, np.ndarray], idx, seed, p: Params):
                        _ptr(a["ty"]), _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]),
                        _ptr(seed), C.byref(p), _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk), C.byref(niter),
                        _ptr(w), _ptr(trace))
+    return dict(pos=pos, cov=cov, chi2=chi2.value, ntrk=ntrk.value, niter=niter.value, w=w[:idx.size], trace=trace, rc=rc)
+
+
+def mv_params(**over) -> Params:
+    """Parameters of the paper's GPU flavour: implicit association, Eq. 19 weights,
+    convergence on |dz| < 0.5 um alone."""
+    kw = dict(flavour=1, conv_dchi2=float("inf"), conv_dz=5e-4)
+    kw.update(over)
+    return default_params(**kw)
+
+
+def mv_weight(chi2_own: float, chi2_max: float, chi2_others=()) -> float:
+    o = np.ascontiguousarray(chi2_others, dtype=np.float64)
+    return float(lib().pvo_mv_weight(float(chi2_own), float(chi2_max), _ptr(o) if o.size else None, int(o.size)))
+
+
+def track_chi2(tracks: Dict[str, np.ndarray], i: int, pos) -> float:
+    a = {k: _f32(tracks[k]) for k in ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")}
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    return float(lib().pvo_track_chi2(C.c_int(i), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]),
+                                      _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(pos)))
+
+
+def fit_mv(tracks: Dict[str, np.ndarray], idx, seed, other, p: Params):
+    """Multi-vertex fit of one vertex over tracks[idx] with other[j] as in pv_oracle.h."""
+    a = {k: _f32(tracks[k]) for k in ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")}
+    idx = _i32(idx)
+    seed = np.ascontiguousarray(seed, dtype=np.float64)
+    other = np.ascontiguousarray(other, dtype=np.float64)
+    assert other.size == idx.size
+    pos = np.zeros(3); cov = np.zeros(6); chi2 = C.c_double(0); ntrk = C.c_int32(0); niter = C.c_int32(0)
+    w = np.zeros(max(idx.size, 1)); trace = np.zeros((TRACE_ITERS, TRACE_STRIDE))
+    rc = lib().pvo_fit_mv(C.c_int(idx.size), _ptr(idx), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]),
+                          _ptr(a["ty"]), _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]),
+                          _ptr(seed), C.byref(p), _ptr(other), _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk),
+                          C.byref(niter), _ptr(w), _ptr(trace))
     return dict(pos=pos, cov=cov, chi2=chi2.value, ntrk=ntrk.value, niter=niter.value, w=w[:idx.size], trace=trace, rc=rc)
 
 
