@@ -50,7 +50,13 @@ typedef struct pv_params {
   float merge_ratio;                    /* duplicate iff dz^2/(Czz1+Czz2) < 25 */
   float max_beam_dist;                  /* pp vertices farther than 0.3 mm are discarded */
   int32_t max_vtx_per_event;            /* output stride per event, 1..PV_MAX_VTX (default 32) */
+  int32_t flavour;                      /* PV_FLAVOUR_EXPLICIT (default): one track one vertex, Tukey weights   P:L163, Eq. 18
+                                           PV_FLAVOUR_MULTIVERTEX: every track to every vertex, weights Eq. 19 */
+  float chi2_window;                    /* multi-vertex flavour: a track takes part in a vertex fit iff its chi2 at
+                                           the seed position is below this: 25      P:L384 (value: reading R-13) */
 } pv_params;
+
+enum { PV_FLAVOUR_EXPLICIT = 0, PV_FLAVOUR_MULTIVERTEX = 1 };
 
 enum {
   PV_OK = 0,
@@ -73,7 +79,9 @@ enum {
 enum {
   PV_EVT_TOO_MANY_TRACKS = 1,  /* n_tracks(e) > PV_MAX_TRACKS_PER_EVENT: event skipped, n_vtx = 0 */
   PV_EVT_VTX_OVERFLOW = 2,     /* more seed clusters than max_vtx_per_event: the first max_vtx in z are kept */
-  PV_EVT_SINGULAR_FIT = 4      /* a vertex fit had < 2 active tracks or a non-positive pivot: that vertex is dropped */
+  PV_EVT_SINGULAR_FIT = 4,     /* a vertex fit had < 2 active tracks or a non-positive pivot: that vertex is dropped */
+  PV_EVT_RECORD_OVERFLOW = 8   /* multi-vertex flavour: the batch needed more (track, vertex) records than the
+                                  workspace holds (2 per track): the event is left without vertices */
 };
 
 /* Fill *p with the paper's values (citations on the struct above).  p: HOST.  Returns PV_OK / PV_E_NULL. */
@@ -85,7 +93,9 @@ int pv_nbins(const pv_params* p);
 /* Bytes of DEVICE workspace pv_find needs for a batch of this size: 256 B of counters, one 16-byte seed
  * record per (event, vertex slot) and one 32-byte fit-ready track record per track (tracks sorted by seed,
  * in the seed's local frame with W = V^-1 at the seed position) handed from the seed kernel to the
- * fit kernel.  The histograms live in shared memory ("one block per event").  bytes: HOST out. */
+ * fit kernel.  The multi-vertex flavour lists a track once per vertex candidate in its chi2 window: it takes two
+ * records per track and 8 more bytes per track (the largest weight of the track and its vertex).  The histograms
+ * live in shared memory ("one block per event").  bytes: HOST out. */
 int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, size_t* bytes);
 
 /* The hot path a1..a6 over a batch.

@@ -21,6 +21,9 @@ MAX_TRACKS_PER_EVENT = 2047
 EVT_TOO_MANY_TRACKS = 1
 EVT_VTX_OVERFLOW = 2
 EVT_SINGULAR_FIT = 4
+EVT_RECORD_OVERFLOW = 8
+FLAVOUR_EXPLICIT = 0
+FLAVOUR_MULTIVERTEX = 1
 
 FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
@@ -41,6 +44,7 @@ class Params(C.Structure):
         ("min_tracks_pv", C.c_int32 * 2), ("chi2_max", C.c_float), ("max_iter", C.c_int32),
         ("conv_dchi2", C.c_float), ("conv_dz", C.c_float), ("merge_ratio", C.c_float),
         ("max_beam_dist", C.c_float), ("max_vtx_per_event", C.c_int32),
+        ("flavour", C.c_int32), ("chi2_window", C.c_float),
     ]
 
 
@@ -111,6 +115,14 @@ def default_params(**over) -> Params:
         else:
             setattr(p, k, v)
     return p
+
+
+def multivertex_params(**over) -> Params:
+    """The paper's GPU flavour: implicit association, Eq. 19 weights, convergence on
+    |dz| < 0.5 um alone (conv_dchi2 = inf)."""
+    kw = dict(flavour=FLAVOUR_MULTIVERTEX, conv_dchi2=float("inf"), conv_dz=5e-4)
+    kw.update(over)
+    return default_params(**kw)
 
 
 def nbins(p: Params) -> int:

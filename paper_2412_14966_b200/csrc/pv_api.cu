@@ -33,9 +33,9 @@ int cuda_fail(cudaError_t err, const char* what) {
 
 struct DeviceInfo {
   int device = -1, sms = 0, max_smem_optin = 0;
-  bool attr_set[2] = {false, false};
-  int attr_smem[2] = {0, 0};
-  int fit_blocks_per_sm = 0;
+  bool attr_set[4] = {false, false, false, false};    // [debug + 2 * flavour]
+  int attr_smem[4] = {0, 0, 0, 0};
+  int fit_blocks_per_sm[2] = {0, 0};                  // [flavour]
 };
 std::mutex g_mu;
 std::vector<DeviceInfo> g_dev;
@@ -78,6 +78,8 @@ int validate(const pv_params* p, int* nbins_out) {
   if (p->max_iter < 1 || p->max_iter > 16) return PV_E_PARAM;
   if (!(p->chi2_max > 0.0f)) return PV_E_PARAM;
   if (!(p->min_bin_content >= 0.0f)) return PV_E_PARAM;      // only bins a track wrote can start a proto-cluster
+  if (p->flavour != PV_FLAVOUR_EXPLICIT && p->flavour != PV_FLAVOUR_MULTIVERTEX) return PV_E_PARAM;
+  if (p->flavour == PV_FLAVOUR_MULTIVERTEX && (!(p->chi2_window > 0.0f) || isinf(p->chi2_max))) return PV_E_PARAM;
   if (nbins_out) *nbins_out = nbins;
   return PV_OK;
 }
@@ -95,7 +97,10 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->I_min[1] = clamp_i32(to_fixed(p->min_cluster_integral[1]));
   for (int r = 0; r < 2; ++r) { k->min_tracks_seed[r] = p->min_tracks_seed[r]; k->min_tracks_pv[r] = p->min_tracks_pv[r]; }
   k->chi2_max = p->chi2_max;
-  k->unit_weights = isinf(p->chi2_max) ? 1 : 0;
+  k->unit_weights = (isinf(p->chi2_max) && p->flavour == PV_FLAVOUR_EXPLICIT) ? 1 : 0;
+  k->flavour = p->flavour;
+  k->chi2_window = p->chi2_window;
+  k->mv_e0 = expf(-0.5f * p->chi2_max);
   k->inv_chi2_max = k->unit_weights ? 0.0f : 1.0f / p->chi2_max;
   k->max_iter = p->max_iter;
   k->conv_dchi2 = p->conv_dchi2; k->conv_dz = p->conv_dz; k->merge_ratio = p->merge_ratio;
@@ -107,11 +112,17 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
 }
 
 // Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | fit-ready track records,
-// 32 B per track, sorted by seed.
+// 32 B each, sorted by seed: one per track (explicit flavour) or up to two per track (multi-vertex flavour, a track
+// is listed once per seed in its chi2 window) | multi-vertex flavour: 8 B per track (largest weight and its seed).
 constexpr size_t WS_COUNTERS = 256;
 size_t ws_rec_bytes(int n_events, int max_vtx) { return (size_t)n_events * (size_t)max_vtx * sizeof(pvk::SeedRec); }
-size_t ws_bytes(int n_events, long long n_tracks, int max_vtx) {
-  return WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + (size_t)n_tracks * 32 + 16;
+size_t ws_trk_records(long long n_tracks, int flavour) {
+  return (size_t)n_tracks * (flavour == PV_FLAVOUR_MULTIVERTEX ? 2 : 1);
+}
+size_t ws_bytes(int n_events, long long n_tracks, int max_vtx, int flavour) {
+  size_t b = WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + ws_trk_records(n_tracks, flavour) * 32 + 16;
+  if (flavour == PV_FLAVOUR_MULTIVERTEX) b += (size_t)n_tracks * 8 + 16;
+  return b;
 }
 
 
@@ -130,7 +141,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     return PV_E_NULL;
   if (n_tracks > 0 && (!x || !y || !z || !tx || !ty || !var_x || !var_y || !var_tx || !var_ty || !trk_weight || !trk_vertex))
     return PV_E_NULL;
-  if (workspace_bytes < ws_bytes(n_events, n_tracks, params->max_vtx_per_event)) return PV_E_WORKSPACE;
+  if (workspace_bytes < ws_bytes(n_events, n_tracks, params->max_vtx_per_event, params->flavour)) return PV_E_WORKSPACE;
   if (((uintptr_t)workspace & 15) != 0) return PV_E_PARAM;
   cudaStream_t stream = (cudaStream_t)stream_;
 
@@ -149,17 +160,20 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   }
   if (warps < 1) return PV_E_PARAM;
   const int smem = warps * kp.warp_smem_bytes;
-  const int which = dbg ? 1 : 0;
+  const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
+  const int which = (dbg ? 1 : 0) + 2 * mvf;
   if (!di->attr_set[which] || di->attr_smem[which] < smem) {
-    if (which) CK(cudaFuncSetAttribute(pvk::seed_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    else CK(cudaFuncSetAttribute(pvk::seed_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    const void* f = which == 0 ? (const void*)pvk::seed_kernel<false, 0> : which == 1 ? (const void*)pvk::seed_kernel<true, 0>
+                  : which == 2 ? (const void*)pvk::seed_kernel<false, 1> : (const void*)pvk::seed_kernel<true, 1>;
+    CK(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     di->attr_set[which] = true;
     di->attr_smem[which] = smem;
   }
-  if (di->fit_blocks_per_sm == 0) {
+  if (di->fit_blocks_per_sm[mvf] == 0) {
     int nb = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel, pvk::FIT_BLOCK, 0));
-    di->fit_blocks_per_sm = nb > 0 ? nb : 1;
+    if (mvf) CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel<1>, pvk::FIT_BLOCK, 0));
+    else CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel<0>, pvk::FIT_BLOCK, 0));
+    di->fit_blocks_per_sm[mvf] = nb > 0 ? nb : 1;
   }
   g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * pvk::TEAM; g_last_smem = smem;
 
@@ -175,37 +189,51 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.evt_counter = reinterpret_cast<unsigned int*>(ws);
   ka.seed_counter = reinterpret_cast<unsigned int*>(ws + 16);
   ka.rec = reinterpret_cast<pvk::SeedRec*>(ws + WS_COUNTERS);
+  ka.trk_counter = reinterpret_cast<unsigned int*>(ws + 32);
   ka.ftrk = reinterpret_cast<float4*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
+  ka.trk_cap = (unsigned int)ws_trk_records(n_tracks, params->flavour);
+  ka.best = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(ka.ftrk) + (size_t)ka.trk_cap * 32 + 16);
   if (dbg) ka.dbg = *dbg;
 
   const bool timing = g_timing != 0;
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
-  CK(cudaMemsetAsync(workspace, 0, 32, stream));
+  CK(cudaMemsetAsync(workspace, 0, 48, stream));
   // a1..a4: persistent, one CTA per SM, one team of two warps per event
   int grid = di->sms;
   const int need = (n_events + warps - 1) / warps;
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
-  if (dbg) pvk::seed_kernel<true><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
-  else pvk::seed_kernel<false><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+  if (mvf) {
+    if (dbg) pvk::seed_kernel<true, 1><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+    else pvk::seed_kernel<false, 1><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+  } else {
+    if (dbg) pvk::seed_kernel<true, 0><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+    else pvk::seed_kernel<false, 0><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+  }
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
   // a5: FIT_G lanes per seed, warps stride over windows of 32 seed records
   {
-    long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm;
+    long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm[mvf];
     const long long most = ((long long)n_events * params->max_vtx_per_event + pvk::FIT_BLOCK - 1) / pvk::FIT_BLOCK;
     if (fit_grid > most) fit_grid = most;
     if (fit_grid < 1) fit_grid = 1;
-    pvk::fit_kernel<<<(int)fit_grid, pvk::FIT_BLOCK, 0, stream>>>(kp, ka);
+    if (mvf) pvk::fit_kernel<1><<<(int)fit_grid, pvk::FIT_BLOCK, 0, stream>>>(kp, ka);
+    else pvk::fit_kernel<0><<<(int)fit_grid, pvk::FIT_BLOCK, 0, stream>>>(kp, ka);
     CK(cudaGetLastError());
   }
   if (timing) CK(cudaEventRecord(g_ev[2], stream));
   // a6: one warp per event
   {
     const int cgrid = (n_events + 7) / 8;
-    if (dbg) pvk::cleanup_kernel<true><<<cgrid, 256, 0, stream>>>(kp, ka);
-    else pvk::cleanup_kernel<false><<<cgrid, 256, 0, stream>>>(kp, ka);
+    if (mvf) {
+      if (dbg) pvk::cleanup_kernel<true, 1><<<cgrid, 256, 0, stream>>>(kp, ka);
+      else pvk::cleanup_kernel<false, 1><<<cgrid, 256, 0, stream>>>(kp, ka);
+    } else {
+      if (dbg) pvk::cleanup_kernel<true, 0><<<cgrid, 256, 0, stream>>>(kp, ka);
+      else pvk::cleanup_kernel<false, 0><<<cgrid, 256, 0, stream>>>(kp, ka);
+    }
     CK(cudaGetLastError());
   }
   if (timing) { CK(cudaEventRecord(g_ev[3], stream)); g_ev_valid = true; }
@@ -232,6 +260,8 @@ int pv_params_default(pv_params* p) {
   p->merge_ratio = 25.0f;                                           /* P:L245 */
   p->max_beam_dist = 0.3f;                                          /* P:L247 */
   p->max_vtx_per_event = 32;
+  p->flavour = PV_FLAVOUR_EXPLICIT;
+  p->chi2_window = 25.0f;                                           /* P:L384, value: reading R-13 */
   return PV_OK;
 }
 
@@ -247,7 +277,7 @@ int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, siz
   if (rc != PV_OK) return rc;
   if (n_events < 0 || n_tracks < 0) return PV_E_SIZE;
   if (n_tracks > 0x7fffffffLL) return PV_E_SIZE;
-  *bytes = ws_bytes(n_events, n_tracks, p->max_vtx_per_event);
+  *bytes = ws_bytes(n_events, n_tracks, p->max_vtx_per_event, p->flavour);
   return PV_OK;
 }
 
@@ -318,7 +348,7 @@ int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, 
   A((void**)&c->d_pos, E * mv * 12); A((void**)&c->d_cov, E * mv * 24); A((void**)&c->d_chi2, E * mv * 4);
   A((void**)&c->d_ntrk, E * mv * 4); A((void**)&c->d_niter, E * mv * 4); A((void**)&c->d_nvtx, E * 4);
   A((void**)&c->d_w, T * 4); A((void**)&c->d_tv, T * 4); A((void**)&c->d_status, E * 4);
-  c->ws_stride = (ws_bytes(max_events, max_tracks, c->max_vtx) + 255) / 256 * 256;
+  c->ws_stride = (ws_bytes(max_events, max_tracks, c->max_vtx, params->flavour) + 255) / 256 * 256;
   A((void**)&c->d_ws, (size_t)n_streams * c->ws_stride);
   for (int i = 0; i < n_streams && err == cudaSuccess; ++i) {
     cudaStream_t s = nullptr;

@@ -43,6 +43,7 @@ constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
 constexpr int FIT_KF = 16;          // track slots per lane in shared memory (fast path: <= FIT_G*FIT_KF tracks)
 constexpr int FIT_BLOCK = 64;       // threads per CTA of fit_kernel (warps are autonomous; 12 KB of tracks per warp)
 constexpr int FIT_MIN_BLOCKS = 9;   // CTAs per SM: 9 x (24 KB + 1 KB reserved) fill the shared memory
+constexpr int FIT_MIN_BLOCKS_MV = 7;  // multi-vertex flavour: 32 KB of staged records per CTA
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
 constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
 
@@ -75,6 +76,9 @@ struct KParams {
   int max_iter;
   float conv_dchi2, conv_dz, merge_ratio, max_beam_dist2;
   int max_vtx;
+  int flavour;                   // PV_FLAVOUR_*
+  float chi2_window;             // multi-vertex flavour: list a track for a seed iff chi2 at the seed position < this
+  float mv_e0;                   // exp(-chi2_max / 2), the constant of the denominator of Eq. 19
   int region0_words;             // int32 words of the histogram region (multiple of 32)
   int warp_smem_bytes;
 };
@@ -99,7 +103,10 @@ struct KArgs {
   unsigned int* evt_counter;     // workspace: next event of the persistent seed kernel
   unsigned int* seed_counter;    // workspace: seed records written so far
   SeedRec* rec;                  // workspace: [n_events * max_vtx]
-  float4* ftrk;                  // workspace: [T][2] fit-ready track records sorted by seed
+  float4* ftrk;                  // workspace: [T or 2 T][2] fit-ready track records sorted by seed
+  unsigned long long* best;      // workspace, multi-vertex flavour: [T] largest weight of the track << 32 | 31 - seed
+  unsigned int* trk_counter;     // workspace, multi-vertex flavour: track records allocated so far
+  unsigned int trk_cap;          // capacity of ftrk in records
   pv_debug dbg;
 };
 
@@ -249,14 +256,17 @@ __device__ __forceinline__ Proj project(float x, float y, float z, float tx, flo
 // A slot without a usable track (none, or R-7) is DEAD: with Tukey weights it is {x0 = 1e15, Wx = 1, rest 0},
 // so that chi2_i = 1e30 gives w = 0 exactly and every product stays finite and zero -- no select in the loop;
 // with unit weights (chi2_max = inf) it is all zeros (W = 0) and the active-track count is taken at load time.
-// 32 bytes in HBM: {x0, y0, tx, ty} {Wx, Wy, track index, 0}.
-struct Trk { float x0, y0, tx, ty, Wx, Wy; };
+// 32 bytes in HBM: {x0, y0, tx, ty} {Wx, Wy, track index, oth}; oth (multi-vertex flavour only) is the part of the
+// denominator of Eq. 19 that does not depend on this vertex: exp(-chi2_max / 2) + sum over the OTHER candidates k of
+// exp(-chi2_ik / 2) at their seed positions.
+struct Trk { float x0, y0, tx, ty, Wx, Wy, oth; };
 
 __device__ __forceinline__ Trk dead_track(const KParams& P) {
   Trk T;
   T.x0 = P.unit_weights ? 0.0f : 1e15f;
   T.Wx = P.unit_weights ? 0.0f : 1.0f;
   T.y0 = T.tx = T.ty = T.Wy = 0.0f;
+  T.oth = 1.0f;
   return T;
 }
 __device__ __forceinline__ bool track_is_dead(const Trk& T, const KParams& P) {
@@ -277,6 +287,7 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
   const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
   T.Wx = __fdividef(1.0f, Vx);
   T.Wy = __fdividef(1.0f, Vy);
+  T.oth = 1.0f;
   if (!ok) T = dead_track(P);
   return T;
 }
@@ -287,7 +298,7 @@ __device__ __forceinline__ void team_sync(int bar) {
   asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(TEAM) : "memory");
 }
 
-template <bool DBG>
+template <bool DBG, int FLAV>
 __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt, const int bar) {
   const int lane = tt & 31, tw = tt >> 5;
   int* H = reinterpret_cast<int*>(wsm);
@@ -316,7 +327,10 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
 
   if (n > MAX_TRK) {
 #pragma unroll 1
-    for (int i = tt; i < n; i += TEAM) A.trk_vertex[t0 + i] = -1;
+    for (int i = tt; i < n; i += TEAM) {
+      A.trk_vertex[t0 + i] = -1;
+      if (FLAV == PV_FLAVOUR_MULTIVERTEX) A.best[t0 + i] = 0ull;
+    }
     if (DBG && A.dbg.trk_seed) for (int i = tt; i < n; i += TEAM) A.dbg.trk_seed[t0 + i] = -1;
     if (tt == 0) {
       A.n_vtx[e] = 0;
@@ -555,6 +569,141 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
 #pragma unroll 1
   for (int i = tw; i < ntw; i += TEAM_WARPS) H[(int)twl[i] * 32 + lane] = 0;
 
+  // ================= a4', multi-vertex flavour: implicit association (R-13, R-14) =========
+  // Every assignable track is a candidate of every seed: E_ik = exp(-chi2_ik / 2) at the seed positions gives the
+  // denominator of Eq. 19; the track is listed for (gets a fit-ready record under) every seed with chi2_ik below the
+  // window.  No removal loop (that belongs to the explicit association).
+  if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+    auto load_raw = [&](const int i) {
+      const int g = t0 + min(i, n - 1);
+      RawTrk Q;
+      Q.x = __ldg(A.x + g); Q.y = __ldg(A.y + g); Q.z = __ldg(A.z + g); Q.tx = __ldg(A.tx + g); Q.ty = __ldg(A.ty + g);
+      Q.vx = __ldg(A.var_x + g); Q.vy = __ldg(A.var_y + g); Q.vtx = __ldg(A.var_tx + g); Q.vty = __ldg(A.var_ty + g);
+      return Q;
+    };
+    auto chi2_at = [&](const RawTrk& R, const int k) -> float {   // Eq. 7 at seed k, W from Eq. 2; < 0 = unusable (R-7)
+      const float zsv = zs[k];
+      const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+      const float dzv = zsv - R.z, dz2 = dzv * dzv;
+      const float Vx = fmaf(dz2, R.vtx, R.vx), Vy = fmaf(dz2, R.vty, R.vy);
+      const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);
+      const float rx = fmaf(dzv, R.tx, R.x) - sx, ry = fmaf(dzv, R.ty, R.y) - sy;
+      const float c = fmaf(rx * rx, __fdividef(1.0f, Vx), ry * ry * __fdividef(1.0f, Vy));
+      return ok ? c : -1.0f;
+    };
+    auto cand = [&](const int i, const RawTrk& R, unsigned& mask, float& den) {
+      mask = 0u; den = P.mv_e0;
+      const int b = i >= n ? -1 : (i < BINS_SM ? (int)binsm[i] : A.trk_vertex[t0 + i]);
+#pragma unroll 1
+      for (int k = 0; k < ns; ++k) {
+        const float c = chi2_at(R, k);
+        if (b >= 0 && c >= 0.0f) {
+          den += __expf(-0.5f * c);
+          if (c < P.chi2_window) mask |= 1u << k;
+        }
+      }
+    };
+    // visits the listed (track, seed) pairs of 32 tracks in a fixed order: f(k, peers) with k = -1 for idle lanes
+    auto for_bits = [&](unsigned m, auto&& f) {
+#pragma unroll 1
+      while (__any_sync(FULL, m != 0u)) {
+        const int k = m ? __ffs(m) - 1 : -1;
+        m &= m - 1u;
+        f(k, __match_any_sync(FULL, k));
+        __syncwarp();
+      }
+    };
+    int* mycnt = cnt + tw * 32;
+    mycnt[lane] = 0;
+    __syncwarp();
+    unsigned hmask[SLOTS];
+    float hden[SLOTS];
+    auto count = [&](int k, unsigned peers) {
+      if (k >= 0 && (peers & lanemask_lt()) == 0) mycnt[k] += __popc(peers);
+    };
+#pragma unroll
+    for (int sl = 0; sl < SLOTS; ++sl) {
+      hmask[sl] = 0u; hden[sl] = 0.0f;
+      if (sl * TEAM + tw * 32 < n) { cand(sl * TEAM + tt, held[sl], hmask[sl], hden[sl]); for_bits(hmask[sl], count); }
+    }
+#pragma unroll 1
+    for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) {
+      unsigned mk; float dn;
+      cand(i0 + lane, load_raw(i0 + lane), mk, dn);
+      for_bits(mk, count);
+    }
+    team_sync(bar);
+    const int myc = lane < ns ? cnt[lane] + cnt[32 + lane] : 0;
+    const int inc = warp_incl_scan(myc, lane);
+    const int nrec = __shfl_sync(FULL, inc, 31);             // (track, seed) records of the event
+    if (tt == 0) misc[5] = (int)atomicAdd(A.trk_counter, (unsigned)nrec);
+    team_sync(bar);
+    const unsigned rbeg = (unsigned)misc[5];
+    const bool ovf = rbeg + (unsigned)nrec > A.trk_cap || rbeg + (unsigned)nrec < rbeg;
+    if (ovf) { status |= PV_EVT_RECORD_OVERFLOW; ns = 0; }
+    const int myoff = inc - myc;
+    cur[lane] = (int)rbeg + myoff + (tw ? cnt[lane] : 0);
+    __syncwarp();
+    auto emit = [&](const int i, const RawTrk& R, const unsigned mask, const float den) {
+      if (i < n) A.best[t0 + i] = 0ull;
+      for_bits(ovf ? 0u : mask, [&](int k, unsigned peers) {
+        const int rank = __popc(peers & lanemask_lt());
+        if (k >= 0) {
+          const float zsv = zs[k];
+          const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+          const Trk T = make_track(P, R, sx, sy, zsv);
+          const float oth = fmaxf(den - __expf(-0.5f * chi2_at(R, k)), 0.5f * P.mv_e0);
+          float4* o = A.ftrk + 2 * (size_t)(cur[k] + rank);
+          o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
+          o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), oth);
+        }
+        __syncwarp();
+        if (k >= 0 && rank == 0) cur[k] += __popc(peers);
+      });
+    };
+#pragma unroll
+    for (int sl = 0; sl < SLOTS; ++sl)
+      if (sl * TEAM + tw * 32 < n) emit(sl * TEAM + tt, held[sl], hmask[sl], hden[sl]);
+#pragma unroll 1
+    for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) {
+      const RawTrk Q = load_raw(i0 + lane);
+      unsigned mk; float dn;
+      cand(i0 + lane, Q, mk, dn);
+      emit(i0 + lane, Q, mk, dn);
+    }
+    if (tw == 0) {
+      int rbase = 0;
+      if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
+      rbase = __shfl_sync(FULL, rbase, 0);
+      if (lane < ns) {
+        int4 r;
+        r.x = e; r.y = lane | (myc << 5); r.z = (int)rbeg + myoff; r.w = __float_as_int(zs[lane]);
+        reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
+        if (myc == 0) A.vtx_niter[ev + lane] = -1;           // nothing in the window: the fit never sees this seed
+      }
+      if (__any_sync(FULL, lane < ns && myc == 0)) status |= PV_EVT_SINGULAR_FIT;
+      if (lane == 0) {
+        A.n_vtx[e] = ns;                                     // scratch: seeds of the event, replaced by cleanup_kernel
+        A.event_status[e] = status;
+      }
+      if (DBG) {
+        if (lane == 0) {
+          if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
+          if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
+        }
+        if (lane < ns) {
+          if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
+          if (A.dbg.seed_bins) {
+            A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
+            A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
+            A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
+          }
+        }
+      }
+    }
+    return;
+  }
+
   // ================= a4: association (R-11) ====================================================
   // Central bins: the first BINS_SM tracks keep them in shared memory, the rest read them back from the
   // trk_vertex scratch.  part[] is padded with INT_MAX to whole groups of four.  Warp w takes the tracks
@@ -685,7 +834,7 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   }
 }
 
-template <bool DBG>
+template <bool DBG, int FLAV>
 __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_constant__ KParams P,
                                                                    const __grid_constant__ KArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -705,7 +854,7 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
   while (e < A.n_events) {
     int nxt = 0;
     if (tt == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);  // issued now, consumed after this event
-    seed_event<DBG>(e, P, A, wsm, tt, bar);
+    seed_event<DBG, FLAV>(e, P, A, wsm, tt, bar);
     team_sync(bar);                                        // the team is done with this event's shared memory
     if (tt == 0) misc[8] = nxt;
     team_sync(bar);
@@ -742,14 +891,23 @@ __device__ __forceinline__ void sums_reduce(Sums& S) {
   }
 }
 
-// Adds the track to the sums and returns its Tukey weight at the current vertex (ax, ay, az).
+// Adds the track to the sums and returns its weight at the current vertex (ax, ay, az): Tukey (Eq. 18) in the
+// explicit flavour, the multi-vertex weight of Eq. 19 otherwise.
+template <int FLAV>
 __device__ __forceinline__ float track_accum(const Trk& T, float ax, float ay, float az, const KParams& P, Sums& S) {
   const float rx = fmaf(az, T.tx, T.x0) - ax;          // residual, Eq. 9
   const float ry = fmaf(az, T.ty, T.y0) - ay;
   const float chi = fmaf(rx * rx, T.Wx, ry * ry * T.Wy);   // Eq. 7
-  // Tukey bi-square, Eq. 18: (1 - chi/chi_max)^2 below chi_max, else 0; inv_chi2_max = 0 gives unit weights
-  const float u = fmaxf(fmaf(chi, -P.inv_chi2_max, 1.0f), 0.0f);
-  const float w = u * u;
+  float w;
+  if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+    // Eq. 19 with the competitors frozen at their seed positions; a dead slot has chi = 1e30: E = 0, w = 0
+    const float E = __expf(-0.5f * chi);
+    w = __fdividef(E, T.oth + E);
+  } else {
+    // Tukey bi-square, Eq. 18: (1 - chi/chi_max)^2 below chi_max, else 0; inv_chi2_max = 0 gives unit weights
+    const float u = fmaxf(fmaf(chi, -P.inv_chi2_max, 1.0f), 0.0f);
+    w = u * u;
+  }
   const float wWx = w * T.Wx, wWy = w * T.Wy;
   const float p = wWx * T.tx, q = wWy * T.ty;
   S.a += wWx; S.b += wWy; S.c += p; S.d += q;
@@ -805,19 +963,38 @@ __device__ __forceinline__ void store_vertex(const KArgs& A, size_t o, float x, 
 __device__ __forceinline__ Trk read_track(const KArgs& A, int rec, int& idx) {
   const float4 a = __ldg(A.ftrk + 2 * (size_t)rec), b = __ldg(A.ftrk + 2 * (size_t)rec + 1);
   Trk T;
-  T.x0 = a.x; T.y0 = a.y; T.tx = a.z; T.ty = a.w; T.Wx = b.x; T.Wy = b.y;
+  T.x0 = a.x; T.y0 = a.y; T.tx = a.z; T.ty = a.w; T.Wx = b.x; T.Wy = b.y; T.oth = b.w;
   idx = __float_as_int(b.z);
   return T;
 }
 
-__global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __grid_constant__ KParams P,
-                                                                        const __grid_constant__ KArgs A) {
+// second half of a staged record: {Wx, Wy} in the explicit flavour, {Wx, Wy, track index, oth} in the multi-vertex one
+template <int FLAV> struct FitB { using type = float2; };
+template <> struct FitB<PV_FLAVOUR_MULTIVERTEX> { using type = float4; };
+
+template <int FLAV, class B>
+__device__ __forceinline__ Trk slot_track(const float4& qa, const B& qb) {
+  Trk T;
+  T.x0 = qa.x; T.y0 = qa.y; T.tx = qa.z; T.ty = qa.w; T.Wx = qb.x; T.Wy = qb.y;
+  if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) T.oth = qb.w; else T.oth = 1.0f;
+  return T;
+}
+
+// multi-vertex flavour: a track follows the fitted seed with its largest final weight (ties: lower z)
+__device__ __forceinline__ void claim_track(const KArgs& A, int idx, float w, int k) {
+  atomicMax(A.best + idx, ((unsigned long long)__float_as_uint(w) << 32) | (unsigned)(31 - k));
+}
+
+template <int FLAV>
+__global__ void __launch_bounds__(FIT_BLOCK, FLAV ? FIT_MIN_BLOCKS_MV : FIT_MIN_BLOCKS)
+fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
+  using BT = typename FitB<FLAV>::type;
   __shared__ __align__(16) float4 s_a[FIT_BLOCK / 32][FIT_KF][32];   // {x0, y0, tx, ty}
-  __shared__ __align__(8) float2 s_b[FIT_BLOCK / 32][FIT_KF][32];    // {Wx, Wy}
+  __shared__ __align__(16) BT s_b[FIT_BLOCK / 32][FIT_KF][32];       // {Wx, Wy} or {Wx, Wy, track index, oth}
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int j = lane % FIT_G, gl = lane / FIT_G;
   float4(*SA)[32] = s_a[warp];
-  float2(*SB)[32] = s_b[warp];
+  BT(*SB)[32] = s_b[warp];
   const int total = (int)*A.seed_counter;
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
   const int wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -880,10 +1057,14 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
             const unsigned da = (unsigned)__cvta_generic_to_shared(&SA[s][lane]);
             const unsigned db = (unsigned)__cvta_generic_to_shared(&SB[s][lane]);
             asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(da), "l"(q) : "memory");
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(db), "l"(q + 1) : "memory");
+            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX)
+              asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(db), "l"(q + 1) : "memory");
+            else
+              asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(db), "l"(q + 1) : "memory");
           } else {
             SA[s][lane] = make_float4(dead.x0, dead.y0, dead.tx, dead.ty);
-            SB[s][lane] = make_float2(dead.Wx, dead.Wy);
+            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) SB[s][lane] = make_float4(dead.Wx, dead.Wy, 0.0f, dead.oth);
+            else SB[s][lane] = make_float2(dead.Wx, dead.Wy);
           }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
@@ -911,11 +1092,8 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
         sums_zero(S);
 #pragma unroll 4
         for (int s = 0; s < nslot; ++s) {
-          const float4 qa = SA[s][lane];
-          const float2 qb = SB[s][lane];
-          Trk T;
-          T.x0 = qa.x; T.y0 = qa.y; T.tx = qa.z; T.ty = qa.w; T.Wx = qb.x; T.Wy = qb.y;
-          track_accum(T, ax, ay, az, P, S);
+          const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
+          track_accum<FLAV>(T, ax, ay, az, P, S);
         }
         sums_reduce<FIT_G>(S);
         if (P.unit_weights) S.nact = nvalid;
@@ -932,26 +1110,35 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
         }
         if (!__any_sync(FULL, run)) break;
       }
-      if (vact && !big) {
-        const size_t o = (size_t)e * P.max_vtx + k;
-        if (sing) {
-          if (j == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
-        } else {
-          if (j == 0) store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)nact, niter);
+      const bool okv = vact && !big && !sing;
+      float nass = 0.0f;                                     // multi-vertex flavour: tracks with final weight >= 1/2
+      if (okv) {
 #pragma unroll 4
-          for (int t = j; t < m; t += FIT_G) {             // weights of the last iteration: the same arithmetic again
-            const int s = t / FIT_G;
-            const float4 qa = SA[s][lane];
-            const float2 qb = SB[s][lane];
-            Trk T;
-            T.x0 = qa.x; T.y0 = qa.y; T.tx = qa.z; T.ty = qa.w; T.Wx = qb.x; T.Wy = qb.y;
-            Sums dummy;
-            sums_zero(dummy);
-            const float w = track_accum(T, lx, ly, lz, P, dummy);
+        for (int t = j; t < m; t += FIT_G) {               // weights of the last iteration: the same arithmetic again
+          const int s = t / FIT_G;
+          const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
+          Sums dummy;
+          sums_zero(dummy);
+          const float w = track_accum<FLAV>(T, lx, ly, lz, P, dummy);
+          if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+            if (!track_is_dead(T, P)) {
+              claim_track(A, __float_as_int(SB[s][lane].z), w, k);
+              nass += (w >= 0.5f) ? 1.0f : 0.0f;
+            }
+          } else {
             const int idx = __float_as_int(__ldg(reinterpret_cast<const float*>(A.ftrk + 2 * (size_t)(r.z + t) + 1) + 2));
             A.trk_weight[idx] = track_is_dead(T, P) ? 0.0f : w;
           }
         }
+      }
+      if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll
+        for (int o = FIT_G / 2; o > 0; o >>= 1) nass += __shfl_xor_sync(FULL, nass, o);
+      }
+      if (vact && !big && j == 0) {
+        const size_t o = (size_t)e * P.max_vtx + k;
+        if (sing) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
+        else store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)(FLAV ? nass : nact), niter);
       }
       // Seeds with more tracks than the shared-memory slots hold: the whole warp strides over the seed's
       // records (contiguous, L1-resident after the first iteration).
@@ -977,7 +1164,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
             int idx;
             const Trk U = read_track(A, bo + t, idx);
             nv += track_is_dead(U, P) ? 0.0f : 1.0f;
-            track_accum(U, qx, qy, qz, P, S);
+            track_accum<FLAV>(U, qx, qy, qz, P, S);
           }
           sums_reduce<32>(S);
           if (P.unit_weights) {
@@ -993,18 +1180,28 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
           if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
         }
         const size_t o = (size_t)be * P.max_vtx + bk;
-        if (bsing) {
-          if (lane == 0) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
-        } else {
-          if (lane == 0) store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)bnact, bit);
+        float bass = 0.0f;
+        if (!bsing) {
           for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration, recomputed
             int idx;
             const Trk U = read_track(A, bo + t, idx);
             Sums dummy;
             sums_zero(dummy);
-            const float w = track_accum(U, px, py, pz, P, dummy);
-            A.trk_weight[idx] = track_is_dead(U, P) ? 0.0f : w;
+            const float w = track_accum<FLAV>(U, px, py, pz, P, dummy);
+            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+              if (!track_is_dead(U, P)) { claim_track(A, idx, w, bk); bass += (w >= 0.5f) ? 1.0f : 0.0f; }
+            } else {
+              A.trk_weight[idx] = track_is_dead(U, P) ? 0.0f : w;
+            }
           }
+        }
+        if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll
+          for (int o2 = 16; o2 > 0; o2 >>= 1) bass += __shfl_xor_sync(FULL, bass, o2);
+        }
+        if (lane == 0) {
+          if (bsing) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
+          else store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)(FLAV ? bass : bnact), bit);
         }
       }
     }
@@ -1015,7 +1212,7 @@ __global__ void __launch_bounds__(FIT_BLOCK, FIT_MIN_BLOCKS) fit_kernel(const __
 // Lane k holds seed k of the event (position, covariance, ... as fit_kernel left them in slot k of the vertex
 // arrays), the duplicate sweep runs on shuffles, survivors are compacted in place in z order, and every
 // track gets its final vertex index (weight 0 when it has none).
-template <bool DBG>
+template <bool DBG, int FLAV>
 __global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KParams P,
                                                       const __grid_constant__ KArgs A) {
   const int lane = threadIdx.x & 31;
@@ -1028,6 +1225,11 @@ __global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KP
   int sv[4];                                               // seed index of my first four tracks: loads issued now,
 #pragma unroll                                             // consumed after the vertex sweep
   for (int q = 0; q < 4; ++q) sv[q] = (lane + 32 * q < n) ? A.trk_vertex[t0 + lane + 32 * q] : -1;
+  unsigned long long bv[4] = {0ull, 0ull, 0ull, 0ull};     // multi-vertex flavour: largest weight << 32 | 31 - seed
+  if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) bv[q] = (lane + 32 * q < n) ? A.best[t0 + lane + 32 * q] : 0ull;
+  }
   float vp[3] = {0.0f, 0.0f, 0.0f}, vc[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
   float vchi2 = 0.0f;
   int vntrk = 0, vniter = -1;
@@ -1109,16 +1311,24 @@ __global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KP
   }
   if (lane == 0) A.n_vtx[e] = __popc(kept);
   // final per-track outputs; tracks of rejected vertices are released (R-9)
-  auto finish = [&](int i, int s) {
+  auto finish = [&](int i, int s, unsigned long long b) {
+    float w = 0.0f;
+    if (FLAV == PV_FLAVOUR_MULTIVERTEX) {                  // R-13: the track follows the seed with its largest weight
+      w = __uint_as_float((unsigned)(b >> 32));
+      s = w > 0.0f ? 31 - (int)(b & 31ull) : -1;
+      if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
+    }
     int vtx = -1;
     if (s >= 0 && ((kept >> s) & 1u)) vtx = __popc(kept & ((1u << s) - 1u));
     A.trk_vertex[t0 + i] = vtx;
-    if (vtx < 0) A.trk_weight[t0 + i] = 0.0f;
+    if (FLAV == PV_FLAVOUR_MULTIVERTEX) A.trk_weight[t0 + i] = vtx >= 0 ? w : 0.0f;
+    else if (vtx < 0) A.trk_weight[t0 + i] = 0.0f;
   };
 #pragma unroll
   for (int q = 0; q < 4; ++q)
-    if (lane + 32 * q < n) finish(lane + 32 * q, sv[q]);
-  for (int i = 128 + lane; i < n; i += 32) finish(i, A.trk_vertex[t0 + i]);
+    if (lane + 32 * q < n) finish(lane + 32 * q, sv[q], bv[q]);
+  for (int i = 128 + lane; i < n; i += 32)
+    finish(i, A.trk_vertex[t0 + i], FLAV == PV_FLAVOUR_MULTIVERTEX ? A.best[t0 + i] : 0ull);
 }
 
 }  // namespace pvk

@@ -196,6 +196,47 @@ def test_other_parameters(pv, oracle):
     _assert_parity(rep, allow_ties_frac=0.03)
 
 
+def _both_mv(pv, oracle, data, n_hist=None, **over):
+    from oracle import compare
+    p = pv.multivertex_params(**over)
+    po = oracle.mv_params(**over)
+    E = data["offsets"].size - 1
+    nh = E if n_hist is None else min(n_hist, E)
+    got = pv.find(data, p, debug=True, n_hist_events=nh)
+    ref = oracle.find(data, po, debug=True, n_hist_events=nh, trace=True, n_threads=8)
+    return got, ref, compare.compare(got, ref, np.asarray(data["offsets"]), p)
+
+
+@pytest.mark.parametrize("idx,n", [(0, 1000), (1, 3000), (2, 1000), (3, 3000)])
+def test_multivertex_flavour(pv, oracle, idx, n):
+    """The paper's GPU flavour (implicit association, Eq. 19 weights, |dz| < 0.5 um):
+    same a1-a3 (bit-exact seeds), fit within 1e-3 mm / 1e-3 rel, identical vertex counts, >= 99.9 % of the tracks
+    follow the same vertex."""
+    data = events.generate(events.config(idx, n))
+    got, ref, rep = _both_mv(pv, oracle, data, n_hist=200)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep, allow_ties_frac=0.02)
+    assert rep["seed_z_mismatch"] == 0 and rep["assign_agreement"] >= 0.999
+    assert rep["n_vertices"] > 1000
+    assert not (got["event_status"] & 8).any()
+
+
+def test_multivertex_other_parameters_and_reproducibility(pv, oracle):
+    """chi2_max = 4 (the value of Fig. 6), a narrower window, a tilted beamline; two runs are bit-identical."""
+    data = events.generate(events.config(1, 800))
+    _, _, rep = _both_mv(pv, oracle, data, n_hist=50, chi2_max=4.0, chi2_window=16.0)
+    _assert_parity(rep, allow_ties_frac=0.03)
+    d2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in data.items()}
+    d2["x"] = (d2["x"] + 0.8 + 1e-3 * d2["z"]).astype(np.float32)
+    _, _, rep = _both_mv(pv, oracle, d2, n_hist=50, beam_x=0.8, beam_tx=1e-3)
+    _assert_parity(rep, allow_ties_frac=0.03)
+    p = pv.multivertex_params()
+    a = pv.find(data, p)
+    b = pv.find(data, p)
+    for k in a:
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
+
+
 def test_runs_are_reproducible(pv, cfg0):
     """Integer histograms and a fixed summation order: two runs give bit-identical outputs."""
     a = pv.find(cfg0)
