@@ -107,10 +107,10 @@ def algorithmic_bytes_by_kernel(data, n_vtx_total: int):
             "cleanup_kernel": T * 4 + n_vtx_total * 48 + E * 8}
 
 
-def run_oracle(data, n_threads: int):
+def run_oracle(data, n_threads: int, flavour: str = "explicit"):
     from oracle import pvref
     pvref.build()
-    p = pvref.default_params()
+    p = pvref.mv_params() if flavour == "multivertex" else pvref.default_params()
     t = time.perf_counter()
     r = pvref.find(data, p, n_threads=n_threads)
     return time.perf_counter() - t, r
@@ -126,10 +126,10 @@ def main_reference(args):
     sample_events = min(args.events or 100_000, 20_000)
     data, m = gen_batch(args.config, sample_events, 0)
     for _ in range(args.warmup):
-        run_oracle(events.slice_events(data, 0, min(2000, sample_events)), cores)
+        run_oracle(events.slice_events(data, 0, min(2000, sample_events)), cores, args.flavour)
     t = 0.0
     for _ in range(args.steps):
-        dt, _r = run_oracle(data, cores)
+        dt, _r = run_oracle(data, cores, args.flavour)
         t += dt
     value = sample_events * args.steps / t
     sample = f"first {sample_events} events of configs[{args.config}] ({m.name}, seed {m.seed}) per step, OpenMP over events"
@@ -137,7 +137,7 @@ def main_reference(args):
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (fp32 contract for the integer decisions)", "data": "synthetic",
             "config": {"workload": f"configs[{args.config}] {m.name}: bounded sample of {sample_events} events per step",
-                       "events_per_step": sample_events},
+                       "events_per_step": sample_events, "flavour": args.flavour},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -164,7 +164,7 @@ def main_ours(args):
 
     data, m = gen_batch(args.config, args.events, rank)
     E, T = int(data["offsets"].size - 1), int(data["offsets"][-1])
-    p = pv.default_params()
+    p = pv.multivertex_params() if args.flavour == "multivertex" else pv.default_params()
     batch = pv.DeviceBatch(data, p, device=dev)
     stream = torch.cuda.Stream(device=dev)
     L = pv.lib()
@@ -267,8 +267,8 @@ def main_ours(args):
         from synth import events as ev_mod
         ns = min(E, args.cpu_sample)
         sample = ev_mod.slice_events(data, 0, ns)
-        run_oracle(ev_mod.slice_events(data, 0, min(ns, 1000)), cores)
-        dt, ref = run_oracle(sample, cores)
+        run_oracle(ev_mod.slice_events(data, 0, min(ns, 1000)), cores, args.flavour)
+        dt, ref = run_oracle(sample, cores, args.flavour)
         same = bool(np.array_equal(ref["n_vtx"], res["n_vtx"][:ns]))
         cpu = {"value": ns / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {ns} events of the same batch, one pass, OpenMP over events on {cores} threads; "
@@ -279,7 +279,7 @@ def main_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32 (int32 fixed-point histogram)", "data": "synthetic",
         "config": {"workload": f"configs[{args.config}] {m.name}: {E} events, {T} tracks, seed {m.seed}, per GPU",
-                   "events_per_step": E, "tracks_per_step": T, "vertices_per_step": n_vtx_total,
+                   "events_per_step": E, "tracks_per_step": T, "vertices_per_step": n_vtx_total, "flavour": args.flavour,
                    "l2": f"inputs {T * 36 / 1e6:.0f} MB per step exceed the 126 MB L2; no flush needed",
                    "launch": info, "parallelism": f"events sharded over {world} GPU(s), no collective"},
         "clocks": sampler.summary(),
@@ -313,6 +313,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-sample", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flavour", default="explicit", choices=["explicit", "multivertex"],
+                    help="explicit: one track one vertex, Tukey weights (headline); multivertex: the paper's GPU flavour, Eq. 19")
     args = ap.parse_args()
     if args.impl == "reference":
         main_reference(args)
