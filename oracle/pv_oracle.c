@@ -477,6 +477,57 @@ double pvo_track_chi2(int i, const float *x, const float *y, const float *z, con
   return rx * rx / Vx + ry * ry / Vy;
 }
 
+/* ===================================== NEXT-4: impact parameter ====================================== */
+/* "the distance of closest approach of a track to a vertex, called impact parameter (IP) ... the IP chi2,
+ * which is the chi2 difference of a PV reconstructed with and without the track under consideration".
+ * For track i and a vertex (pos, C) that does NOT contain the track: r = Eq. 9 residual at the vertex z,
+ * IP = distance of the straight line to the point; IP chi2 = r^T (V_i + H C H^T)^-1 r with V_i from Eq. 2 (diagonal)
+ * at the vertex z and H of Eq. 12 -- the chi2 increase of the linear least-squares vertex when the track is added.
+ * Returns 0, or -1 when the track covariance is unusable there (R-7) or the 2x2 matrix is not positive definite. */
+int pvo_ip_one(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
+               const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+               const double pos[3], const double C[6], double *ip, double *ip_chi2) {
+  double dz = pos[2] - (double)z[i];
+  double Vx = (double)var_x[i] + dz * dz * (double)var_tx[i];
+  double Vy = (double)var_y[i] + dz * dz * (double)var_ty[i];
+  if (!((Vx > 0.0) && (Vy > 0.0) && isfinite(Vx) && isfinite(Vy))) return -1;
+  double a = (double)tx[i], b = (double)ty[i];
+  double rx = (double)x[i] + dz * a - pos[0];
+  double ry = (double)y[i] + dz * b - pos[1];
+  /* the point of the line at the vertex z is (rx, ry, 0) away; remove the component along (tx, ty, 1) */
+  double along = (rx * a + ry * b) / sqrt(1.0 + a * a + b * b);
+  double d2 = rx * rx + ry * ry - along * along;
+  *ip = sqrt(d2 > 0.0 ? d2 : 0.0);
+  /* H C H^T with H = [[-1, 0, tx], [0, -1, ty]], C = (xx, xy, xz, yy, yz, zz) */
+  double Sxx = Vx + C[0] - 2.0 * a * C[2] + a * a * C[5];
+  double Syy = Vy + C[3] - 2.0 * b * C[4] + b * b * C[5];
+  double Sxy = C[1] - a * C[4] - b * C[2] + a * b * C[5];
+  double det = Sxx * Syy - Sxy * Sxy;
+  if (!(Sxx > 0.0) || !(det > 0.0)) return -1;
+  *ip_chi2 = (Syy * rx * rx - 2.0 * Sxy * rx * ry + Sxx * ry * ry) / det;
+  return 0;
+}
+
+/* Per track of a batch: the vertex of its event with the smallest IP chi2 (ties: lower index), that chi2 and the IP
+ * to that vertex; ip_vertex = -1, ip = ip_chi2 = -1 when the event has no usable vertex for the track. */
+int pvo_track_ip(const float *x, const float *y, const float *z, const float *tx, const float *ty,
+                 const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+                 const int32_t *offsets, int n_events, int max_vtx,
+                 const double *vtx_pos, const double *vtx_cov, const int32_t *n_vtx,
+                 double *ip, double *ip_chi2, int32_t *ip_vertex) {
+  for (int e = 0; e < n_events; ++e)
+    for (int t = offsets[e]; t < offsets[e + 1]; ++t) {
+      ip[t] = -1.0; ip_chi2[t] = -1.0; ip_vertex[t] = -1;
+      for (int v = 0; v < n_vtx[e] && v < max_vtx; ++v) {
+        size_t o = (size_t)e * max_vtx + v;
+        double d, c2;
+        if (pvo_ip_one(t, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, vtx_pos + 3 * o, vtx_cov + 6 * o, &d, &c2) != 0) continue;
+        if (ip_vertex[t] < 0 || c2 < ip_chi2[t]) { ip[t] = d; ip_chi2[t] = c2; ip_vertex[t] = v; }
+      }
+    }
+  return 0;
+}
+
 /* ===================================== whole path, one event ========================================= */
 typedef struct scratch {
   int nbins, max_vtx;

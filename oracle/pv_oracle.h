@@ -101,6 +101,18 @@ int pvo_fit_mv(int m, const int32_t *idx,
                double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
                double *w, double *trace);
 
+/* NEXT-4: impact parameter and IP chi2 of track i to a vertex (pos[3], C[6] upper triangle) that does not
+ * contain it; returns -1 when the covariance is unusable. */
+int pvo_ip_one(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
+               const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+               const double pos[3], const double C[6], double *ip, double *ip_chi2);
+/* per track: the vertex of its event with the smallest IP chi2; -1 if none */
+int pvo_track_ip(const float *x, const float *y, const float *z, const float *tx, const float *ty,
+                 const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
+                 const int32_t *offsets, int n_events, int max_vtx,
+                 const double *vtx_pos, const double *vtx_cov, const int32_t *n_vtx,
+                 double *ip, double *ip_chi2, int32_t *ip_vertex);
+
 /* Optional taps of the full pipeline (all nullable). */
 typedef struct pvo_debug {
   int32_t *hist;        /* [n_hist_events][nbins] */

@@ -84,6 +84,8 @@ def lib():
         L.pvo_mv_weight.restype = C.c_double
         L.pvo_mv_weight.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_int]
         L.pvo_track_chi2.restype = C.c_double
+        L.pvo_ip_one.restype = C.c_int
+        L.pvo_track_ip.restype = C.c_int
         _lib = L
     return _lib
 
@@ -217,6 +219,33 @@ def fit_mv(tracks: Dict[str, np.ndarray], idx, seed, other, p: Params):
                           _ptr(seed), C.byref(p), _ptr(other), _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk),
                           C.byref(niter), _ptr(w), _ptr(trace))
     return dict(pos=pos, cov=cov, chi2=chi2.value, ntrk=ntrk.value, niter=niter.value, w=w[:idx.size], trace=trace, rc=rc)
+
+
+def ip_one(tracks: Dict[str, np.ndarray], i: int, pos, cov):
+    """(rc, ip, ip_chi2) of track i to one vertex."""
+    a = {k: _f32(tracks[k]) for k in ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")}
+    pos = np.ascontiguousarray(pos, dtype=np.float64); cov = np.ascontiguousarray(cov, dtype=np.float64)
+    d = C.c_double(0); c2 = C.c_double(0)
+    rc = lib().pvo_ip_one(C.c_int(i), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]), _ptr(a["var_x"]),
+                          _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(pos), _ptr(cov), C.byref(d), C.byref(c2))
+    return rc, d.value, c2.value
+
+
+def track_ip(data: Dict[str, np.ndarray], vtx_pos, vtx_cov, n_vtx) -> Dict[str, np.ndarray]:
+    """Per track: the vertex of its event with the smallest IP chi2, that chi2 and the IP to it."""
+    a = {k: _f32(data[k]) for k in ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")}
+    off = _i32(data["offsets"])
+    E, T = off.size - 1, a["x"].size
+    vp = np.ascontiguousarray(vtx_pos, dtype=np.float64); vc = np.ascontiguousarray(vtx_cov, dtype=np.float64)
+    nv = _i32(n_vtx)
+    mv = vp.shape[1] if vp.ndim == 3 else 1
+    out = dict(ip=np.zeros(T), ip_chi2=np.zeros(T), ip_vertex=np.zeros(T, np.int32))
+    rc = lib().pvo_track_ip(_ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]), _ptr(a["var_x"]),
+                            _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(off), C.c_int(E), C.c_int(mv),
+                            _ptr(vp), _ptr(vc), _ptr(nv), _ptr(out["ip"]), _ptr(out["ip_chi2"]), _ptr(out["ip_vertex"]))
+    if rc != 0:
+        raise RuntimeError(f"pvo_track_ip failed: {rc}")
+    return out
 
 
 def find(data: Dict[str, np.ndarray], p: Optional[Params] = None, debug: bool = False, n_hist_events: int = 0,
