@@ -213,6 +213,24 @@ def main_ours(args):
     res = batch.results()
     n_vtx_total = int(res["n_vtx"].sum())
 
+    # ---- optional: the IP consumer (NEXT-4) on the vertices just found, timed on its own (not part of `value`) ----
+    ip_info = None
+    if args.with_ip:
+        for _ in range(3):
+            batch.track_ip(stream)
+        stream.synchronize()
+        i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            i0.record(stream)
+            for _ in range(args.steps):
+                batch.track_ip(stream)
+            i1.record(stream)
+        stream.synchronize()
+        ip_ms = i0.elapsed_time(i1) / args.steps
+        ip_bytes = T * 36 + (E + 1) * 4 + E * 4 + n_vtx_total * 36 + T * 12
+        ip_info = {"kernel": "pvk::ip_kernel", "ms": ip_ms, "algorithmic_bytes": ip_bytes,
+                   "achieved_gbs": ip_bytes / (ip_ms * 1e-3) / 1e9, "tracks_per_s": T / (ip_ms * 1e-3)}
+
     # ---- e2e: HOST buffers through pv_find_host (H2D + kernel + D2H inside the timed region) --------------------
     hp = pv.HostPipeline(E, T, p, n_streams=4, device=dev)
     hin = hp.pin_inputs(data)
@@ -296,6 +314,9 @@ def main_ours(args):
                      "note": "issue/latency-bound path, not HBM-bound: see DESIGN.md section 8"},
         "cpu_baseline": cpu,
     }
+    if ip_info is not None:
+        ip_info["frac"] = ip_info["achieved_gbs"] / peak
+        line["ip"] = ip_info
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -313,6 +334,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-sample", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--with-ip", action="store_true", help="also time pv_track_ip (IP / IP chi2 of every track, NEXT-4)")
     ap.add_argument("--flavour", default="explicit", choices=["explicit", "multivertex"],
                     help="explicit: one track one vertex, Tukey weights (headline); multivertex: the paper's GPU flavour, Eq. 19")
     args = ap.parse_args()

@@ -129,6 +129,22 @@ int pv_find(const float* x, const float* y, const float* z, const float* tx, con
             int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
             void* workspace, size_t workspace_bytes, void* stream);
 
+/* Impact parameter of every track w.r.t. the PVs of its event ("the distance of closest approach of a track to
+ * a vertex, called impact parameter (IP) ... the IP chi2, which is the chi2 difference of a PV reconstructed with and
+ * without the track under consideration").  For each track the vertex of its event with the smallest IP chi2 is
+ * taken (ties: lower index); the vertex is treated as not containing the track:
+ *   r = residual of Eq. 9 at the vertex z, IP = distance of the straight line to the vertex position,
+ *   IP chi2 = r^T (V + H C H^T)^-1 r, V from Eq. 2 (diagonal) at the vertex z, H of Eq. 12, C the vertex covariance.
+ * Inputs: the track arrays and offsets of pv_find (DEVICE), and its outputs vtx_pos / vtx_cov / n_vtx (DEVICE,
+ * stride params->max_vtx_per_event).  Outputs (DEVICE, caller-allocated, length T): ip [mm], ip_chi2, ip_vertex
+ * (index within the event); -1 in all three when the event has no vertex usable for the track.
+ * One kernel on `stream`; never allocates or synchronises. */
+int pv_track_ip(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                const float* vtx_pos, const float* vtx_cov, const int32_t* n_vtx,
+                float* ip, float* ip_chi2, int32_t* ip_vertex, void* stream);
+
 /* Parity taps: every member is a nullable DEVICE pointer; no global state. */
 typedef struct pv_debug {
   int32_t* hist;          /* [n_hist_events][nbins]: histogram of the first n_hist_events events (a2) */

@@ -28,7 +28,7 @@ FLAVOUR_MULTIVERTEX = 1
 FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
 EXPORTS = (
-    "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug",
+    "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug", "pv_track_ip",
     "pv_host_ctx_create", "pv_host_ctx_destroy", "pv_find_host", "pv_host_register", "pv_host_unregister",
     "pv_last_launch_info", "pv_kernel_timing", "pv_kernel_time_ms", "pv_kernel_times_ms", "pv_error_string", "pv_last_cuda_error",
 )
@@ -80,6 +80,7 @@ def lib():
         find_args = [vp] * 9 + [vp, i32, i64, C.POINTER(Params)] + [vp] * 9 + [vp, C.c_size_t, vp]
         L.pv_find.argtypes = find_args
         L.pv_find_debug.argtypes = find_args + [C.POINTER(Debug)]
+        L.pv_track_ip.argtypes = [vp] * 9 + [vp, i32, i64, C.POINTER(Params)] + [vp] * 3 + [vp] * 3 + [vp]
         L.pv_host_ctx_create.argtypes = [C.POINTER(vp), i32, i64, C.POINTER(Params), i32]
         L.pv_host_ctx_destroy.argtypes = [vp]
         L.pv_find_host.argtypes = [vp] + [vp] * 9 + [vp, i32, C.POINTER(Params)] + [vp] * 9 + [i32]
@@ -215,6 +216,25 @@ class DeviceBatch:
                 _check(L.pv_find_debug(*args, C.byref(self.dbg_struct)), "pv_find_debug")
             else:
                 _check(L.pv_find(*args), "pv_find")
+
+    def track_ip(self, stream=None) -> None:
+        """Enqueue pv_track_ip on the vertices of the last find(); results in self.ip (ip, ip_chi2, ip_vertex)."""
+        torch = _torch()
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        if not hasattr(self, "ip"):
+            self.ip = dict(ip=torch.zeros(self.T, dtype=torch.float32, device=self.device),
+                           ip_chi2=torch.zeros(self.T, dtype=torch.float32, device=self.device),
+                           ip_vertex=torch.zeros(self.T, dtype=torch.int32, device=self.device))
+        i, o = self.inp, self.out
+        args = [i[k].data_ptr() for k in FIELDS] + [self.offsets.data_ptr(), self.E, self.T, C.byref(self.p)] + [
+            o["vtx_pos"].data_ptr(), o["vtx_cov"].data_ptr(), o["n_vtx"].data_ptr(),
+            self.ip["ip"].data_ptr(), self.ip["ip_chi2"].data_ptr(), self.ip["ip_vertex"].data_ptr(), s.cuda_stream]
+        with torch.cuda.device(self.device):
+            _check(lib().pv_track_ip(*args), "pv_track_ip")
+
+    def ip_results(self) -> Dict[str, np.ndarray]:
+        _torch().cuda.synchronize(self.device)
+        return {k: v.cpu().numpy() for k, v in self.ip.items()}
 
     def results(self) -> Dict[str, np.ndarray]:
         torch = _torch()

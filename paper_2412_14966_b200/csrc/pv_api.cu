@@ -305,6 +305,31 @@ int pv_find_debug(const float* x, const float* y, const float* z, const float* t
                    workspace_bytes, stream, dbg ? dbg : &none);
 }
 
+int pv_track_ip(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                const float* vtx_pos, const float* vtx_cov, const int32_t* n_vtx,
+                float* ip, float* ip_chi2, int32_t* ip_vertex, void* stream_) {
+  int nbins = 0;
+  const int rc = validate(params, &nbins);
+  if (rc != PV_OK) return rc;
+  if (n_events < 0 || n_tracks < 0 || n_tracks > 0x7fffffffLL) return PV_E_SIZE;
+  if (n_events == 0) return PV_OK;
+  if (!offsets || !vtx_pos || !vtx_cov || !n_vtx) return PV_E_NULL;
+  if (n_tracks > 0 && (!x || !y || !z || !tx || !ty || !var_x || !var_y || !var_tx || !var_ty || !ip || !ip_chi2 || !ip_vertex))
+    return PV_E_NULL;
+  pvk::KParams kp;
+  make_kparams(params, nbins, &kp);
+  pvk::KArgs ka;
+  memset(&ka, 0, sizeof(ka));
+  ka.x = x; ka.y = y; ka.z = z; ka.tx = tx; ka.ty = ty;
+  ka.var_x = var_x; ka.var_y = var_y; ka.var_tx = var_tx; ka.var_ty = var_ty;
+  ka.offsets = offsets; ka.n_events = n_events;
+  pvk::ip_kernel<<<(n_events + 7) / 8, 256, 0, (cudaStream_t)stream_>>>(kp, ka, vtx_pos, vtx_cov, n_vtx, ip, ip_chi2, ip_vertex);
+  CK(cudaGetLastError());
+  return PV_OK;
+}
+
 /* ------------------------------------------- host-buffer pipeline ------------------------------------------- */
 struct pv_host_ctx {
   int max_events = 0;
