@@ -2,17 +2,20 @@
 //
 // Three kernels per pv_find call:
 //
-//   seed_kernel     a1..a4  one WARP per event, persistent grid, per-warp int32 shared-memory histogram.
-//                           POCA projection (fp32 contract, bit-exact with the CPU oracle), tracks sorted by
-//                           window length so the fixed-point Gaussian fill runs with full lanes, threshold
-//                           bitmap of the touched histogram words only, one lane per proto-cluster for the
-//                           z-ordered hysteresis sweep, seed positions, association with the removal loop,
-//                           deterministic counting sort of the tracks by seed -> seed records in HBM.
-//   fit_kernel      a5      8 lanes per vertex seed, flat over all seeds of the batch (no histogram, so it
-//                           runs at full occupancy): tracks register-resident, xor-shuffle reduction of the
-//                           normal equations, closed-form solve of the arrow-shaped 3x3 Hessian.
+//   seed_kernel     a1..a4  one TEAM of two warps per event, persistent grid, 13 teams per CTA, one int32
+//                           shared-memory histogram and one named barrier per team.  POCA projection (fp32 contract,
+//                           bit-exact with the CPU oracle), flat list of 8-bin fill units (nine independent CDF edges
+//                           per thread), touched-word flags, one ballot per touched word for the proto-cluster starts,
+//                           one lane per proto-cluster for the z-ordered hysteresis sweep, seed positions,
+//                           association (explicit with the removal loop, or the multi-vertex chi2 window),
+//                           deterministic counting sort -> seed records and fit-ready track records in HBM.
+//   fit_kernel      a5      2 lanes per vertex seed, flat over all seeds of the batch (no histogram): windows of 32
+//                           seed records sorted by track count, tracks staged by cp.async into a conflict-free
+//                           shared-memory slice, xor-shuffle reduction of the normal equations, closed-form solve of
+//                           the arrow-shaped 3x3 Hessian; Tukey (Eq. 18) or multi-vertex (Eq. 19) weights.
 //   cleanup_kernel  a6      one warp per event: z-ordered duplicate sweep, cuts, compaction, final per-track
 //                           vertex index and weight.
+//   ip_kernel       NEXT-4  impact parameter / IP chi2 of every track w.r.t. the PVs of its event (pv_track_ip).
 //
 // The v1 single fused kernel (profiles/r1_v1_fused_kernel.md) was 87 KB of SASS and lost 42 % of its issue
 // slots to instruction-cache misses with 14 warps per SM in different phases; each kernel here is small.
