@@ -40,6 +40,7 @@ void pvo_params_default(pvo_params *p) {
   p->max_vtx_per_event = 32;
   p->flavour = 0;                                                /* explicit association + Tukey (x86 flavour) */
   p->chi2_window = 25.0f;                                        /* P:L384 "within a certain chi2_i"; value: R-13 */
+  p->split_mode = 0;                                             /* z-ordered splitting (GPU variant) */
 }
 
 int pvo_nbins(const pvo_params *p) {
@@ -162,19 +163,77 @@ static int64_t integral(const int32_t *H, int b0, int b1) {
   return s;
 }
 
+/* x86 variant of the splitting: "the CPU implementation considers the smallest minimum between the two
+ * largest maxima and does the splitting recursively".  Reading R-16: on the bin range [s, e) run the hysteresis
+ * sweep of R-4.2; with fewer than two significant maxima the range is a leaf; else take the two highest maxima (ties:
+ * lower bin), the lowest significant minimum between them (ties: lower bin), and split there iff BOTH parts carry the
+ * minimum cluster integral; recurse into the left part, then the right part (the minimum bin opens the
+ * right part, as in R-4.3).  Leaves are seed clusters, emitted in z order. */
+typedef struct peak_out { int cap, n; int32_t *begin, *end, *peak; } peak_out;
+
+static void split_recursive(const int32_t *H, int s, int e, const pvo_params *p, int64_t D, const int64_t I_min[2],
+                            int *ext_bin, peak_out *out) {
+  /* extrema of [s, e): ext_bin[2 j] = bin of MAX j, ext_bin[2 j - 1] = bin of MIN j (between MAX j-1 and MAX j) */
+  int n_max = 0;
+  int look_max = 1;
+  int64_t mx = H[s], mn = 0;
+  int mxp = s, mnp = s;
+  for (int k = s + 1; k < e; ++k) {
+    int64_t h = H[k];
+    if (look_max) {
+      if (h > mx) { mx = h; mxp = k; }
+      else if (h < mx - D) { ext_bin[2 * n_max] = mxp; ++n_max; mn = h; mnp = k; look_max = 0; }
+    } else {
+      if (h < mn) { mn = h; mnp = k; }
+      else if (h > mn + D) { ext_bin[2 * n_max - 1] = mnp; mx = h; mxp = k; look_max = 1; }
+    }
+  }
+  if (look_max) { ext_bin[2 * n_max] = mxp; ++n_max; }
+  if (n_max >= 2) {
+    int a = 0, b = -1;                                   /* indices of the highest and second highest maximum */
+    for (int j = 1; j < n_max; ++j) if (H[ext_bin[2 * j]] > H[ext_bin[2 * a]]) a = j;
+    for (int j = 0; j < n_max; ++j) {
+      if (j == a) continue;
+      if (b < 0 || H[ext_bin[2 * j]] > H[ext_bin[2 * b]]) b = j;
+    }
+    int lo = a < b ? a : b, hi = a < b ? b : a;
+    int c = ext_bin[2 * (lo + 1) - 1];
+    for (int j = lo + 2; j <= hi; ++j) if (H[ext_bin[2 * j - 1]] < H[c]) c = ext_bin[2 * j - 1];
+    int pl = argmax_bin(H, s, c), pr = argmax_bin(H, c, e);
+    if (integral(H, s, c) >= I_min[bin_region(pl, p)] && integral(H, c, e) >= I_min[bin_region(pr, p)]) {
+      /* the extrema buffer is reused by the recursion: nothing of this level is needed afterwards */
+      split_recursive(H, s, c, p, D, I_min, ext_bin, out);
+      split_recursive(H, c, e, p, D, I_min, ext_bin, out);
+      return;
+    }
+  }
+  if (out->n < out->cap) { out->begin[out->n] = s; out->end[out->n] = e; out->peak[out->n] = argmax_bin(H, s, e); }
+  ++out->n;
+}
+
 int pvo_peaks(const int32_t *H, const pvo_params *p, int cap, int32_t *begin, int32_t *end, int32_t *peak) {
   const int nbins = pvo_nbins(p);
   const int64_t T_bin = to_fixed(p->min_bin_content);
   const int64_t D = to_fixed(p->min_dip);
   const int64_t I_min[2] = {to_fixed(p->min_cluster_integral[0]), to_fixed(p->min_cluster_integral[1])};
   int n_out = 0;
-  int *minima = (int *)malloc(sizeof(int) * (size_t)(nbins + 1));
+  int *minima = (int *)malloc(sizeof(int) * (size_t)(2 * nbins + 2));
   int b = 0;
   while (b < nbins) {
     if (!((int64_t)H[b] > T_bin)) { ++b; continue; }
     /* 1. proto-cluster: maximal run of bins "above a threshold" */
     int b0 = b, b1 = b;
     while (b1 < nbins && (int64_t)H[b1] > T_bin) ++b1;
+    if (p->split_mode == 1) {                        /* x86 variant (R-16): recursive splitting */
+      int pk = argmax_bin(H, b0, b1);
+      if (integral(H, b0, b1) >= I_min[bin_region(pk, p)]) {      /* every seed passes the integral cut */
+        peak_out out = {cap, n_out, begin, end, peak};
+        split_recursive(H, b0, b1, p, D, I_min, minima, &out);
+        n_out = out.n;
+      }
+      b = b1;
+      continue;
+    }
     /* 2. "all significant minima and maxima": z-ordered hysteresis sweep (R-4.2).
      *    The emitted extremum list is MAX (MIN MAX)*, only the MINs are needed afterwards. */
     int n_min = 0;

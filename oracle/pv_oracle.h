@@ -37,6 +37,8 @@ typedef struct pvo_params {
                                           1: implicit association + multi-vertex weights (GPU, Eq. 19) */
   float chi2_window;                   /* flavour 1: tracks with chi2 < this at the seed position take part in a
                                           vertex fit (value 25: reading R-13) */
+  int32_t split_mode;                  /* proto-cluster splitting: 0 = minima in z order (GPU variant),
+                                          1 = smallest minimum between the two largest maxima, recursively (x86) */
 } pvo_params;
 
 enum { PVO_S = 1 << 20 };              /* fixed-point unit: one track's full mass */

@@ -31,6 +31,48 @@ def test_handbuilt_histograms(oracle):
                 assert abs(oracle.seed_z(H, int(kk), p) - zexp) < 1e-4, c["name"]
 
 
+def test_handbuilt_histograms_x86_splitter(oracle):
+    """R-16, the recursive x86 variant, against hand-worked cases; the same file also pins what the
+    z-ordered variant gives on them (they differ when a small peak sits between the two largest)."""
+    with open(os.path.join(os.path.dirname(GOLD), "peaks_x86_handbuilt.json")) as f:
+        cases = json.load(f)["cases"]
+    differ = 0
+    for c in cases:
+        H = _hist(c["first_bin"], c["content"])
+        for mode, key in ((1, "clusters"), (0, "clusters_gpu")):
+            b, e, k, n = oracle.peaks(H, oracle.default_params(split_mode=mode))
+            got = [list(map(int, t)) for t in zip(b, e, k)]
+            assert got == c[key], (c["name"], mode)
+            assert n == len(c[key])
+        differ += c["clusters"] != c["clusters_gpu"]
+    assert differ >= 1
+
+
+def test_x86_splitter_invariants_on_events(oracle, cfg0):
+    """On real histograms: clusters disjoint, z-ordered, each with the minimum integral, within one proto-cluster
+    contiguous; both variants cover the same bins whenever they keep a proto-cluster, and agree on most events."""
+    from synth import events
+    p0, p1 = oracle.default_params(), oracle.default_params(split_mode=1)
+    data = events.generate(events.config(3, 600))                 # close pairs: many multi-peak proto-clusters
+    r0 = oracle.find(data, p0, debug=True, n_hist_events=600)
+    H = r0["debug"]["hist"]
+    same = 0
+    for e in range(600):
+        b0, e0, k0, _ = oracle.peaks(H[e], p0)
+        b1, e1, k1, _ = oracle.peaks(H[e], p1)
+        assert np.all(b1[1:] >= e1[:-1]) and np.all(e1 > b1) and np.all((k1 >= b1) & (k1 < e1))
+        for b, en, k in zip(b1, e1, k1):
+            region = 1 if (-550 + 0.25 * (k + 0.5)) < -300 else 0
+            assert H[e][b:en].astype(np.int64).sum() >= int(round((1.75 if region else 2.5) * S))
+            assert H[e][k] == H[e][b:en].max() and (H[e][b:k] < H[e][k]).all()
+        cover0 = np.zeros(3400, bool); cover1 = np.zeros(3400, bool)
+        for b, en in zip(b0, e0): cover0[b:en] = True
+        for b, en in zip(b1, e1): cover1[b:en] = True
+        assert np.array_equal(cover0, cover1)
+        same += (len(b0) == len(b1)) and np.array_equal(b0, b1)
+    assert same > 500
+
+
 def test_seed_delta_properties(oracle):
     """Eq. 5: symmetric peak -> delta = 0; N_{i+1} -> N_i gives delta -> +1/2; delta in [-1/2, 1/2]."""
     p = oracle.default_params()
