@@ -54,9 +54,13 @@ typedef struct pv_params {
                                            PV_FLAVOUR_MULTIVERTEX: every track to every vertex, weights Eq. 19 */
   float chi2_window;                    /* multi-vertex flavour: a track takes part in a vertex fit iff its chi2 at
                                            the seed position is below this: 25      P:L384 (value: reading R-13) */
+  int32_t split_mode;                   /* proto-cluster splitting: PV_SPLIT_Z_ORDERED (default, the paper's GPU
+                                           variant: minima in z order) or PV_SPLIT_RECURSIVE (its x86 variant: the
+                                           smallest minimum between the two largest maxima, recursively; reading R-16) */
 } pv_params;
 
 enum { PV_FLAVOUR_EXPLICIT = 0, PV_FLAVOUR_MULTIVERTEX = 1 };
+enum { PV_SPLIT_Z_ORDERED = 0, PV_SPLIT_RECURSIVE = 1 };
 
 enum {
   PV_OK = 0,

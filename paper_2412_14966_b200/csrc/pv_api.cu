@@ -33,8 +33,8 @@ int cuda_fail(cudaError_t err, const char* what) {
 
 struct DeviceInfo {
   int device = -1, sms = 0, max_smem_optin = 0;
-  bool attr_set[4] = {false, false, false, false};    // [debug + 2 * flavour]
-  int attr_smem[4] = {0, 0, 0, 0};
+  bool attr_set[8] = {false, false, false, false, false, false, false, false};   // [debug + 2 flavour + 4 split]
+  int attr_smem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   int fit_blocks_per_sm[2] = {0, 0};                  // [flavour]
 };
 std::mutex g_mu;
@@ -79,6 +79,7 @@ int validate(const pv_params* p, int* nbins_out) {
   if (!(p->chi2_max > 0.0f)) return PV_E_PARAM;
   if (!(p->min_bin_content >= 0.0f)) return PV_E_PARAM;      // only bins a track wrote can start a proto-cluster
   if (p->flavour != PV_FLAVOUR_EXPLICIT && p->flavour != PV_FLAVOUR_MULTIVERTEX) return PV_E_PARAM;
+  if (p->split_mode != PV_SPLIT_Z_ORDERED && p->split_mode != PV_SPLIT_RECURSIVE) return PV_E_PARAM;
   if (p->flavour == PV_FLAVOUR_MULTIVERTEX && (!(p->chi2_window > 0.0f) || isinf(p->chi2_max))) return PV_E_PARAM;
   if (nbins_out) *nbins_out = nbins;
   return PV_OK;
@@ -99,6 +100,7 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->chi2_max = p->chi2_max;
   k->unit_weights = (isinf(p->chi2_max) && p->flavour == PV_FLAVOUR_EXPLICIT) ? 1 : 0;
   k->flavour = p->flavour;
+  k->split_mode = p->split_mode;
   k->chi2_window = p->chi2_window;
   k->mv_e0 = expf(-0.5f * p->chi2_max);
   k->inv_chi2_max = k->unit_weights ? 0.0f : 1.0f / p->chi2_max;
@@ -161,11 +163,15 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (warps < 1) return PV_E_PARAM;
   const int smem = warps * kp.warp_smem_bytes;
   const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
-  const int which = (dbg ? 1 : 0) + 2 * mvf;
+  const int spl = params->split_mode == PV_SPLIT_RECURSIVE ? 1 : 0;
+  const int which = (dbg ? 1 : 0) + 2 * mvf + 4 * spl;
+  static const void* const seed_fn[8] = {
+      (const void*)pvk::seed_kernel<false, 0, 0>, (const void*)pvk::seed_kernel<true, 0, 0>,
+      (const void*)pvk::seed_kernel<false, 1, 0>, (const void*)pvk::seed_kernel<true, 1, 0>,
+      (const void*)pvk::seed_kernel<false, 0, 1>, (const void*)pvk::seed_kernel<true, 0, 1>,
+      (const void*)pvk::seed_kernel<false, 1, 1>, (const void*)pvk::seed_kernel<true, 1, 1>};
   if (!di->attr_set[which] || di->attr_smem[which] < smem) {
-    const void* f = which == 0 ? (const void*)pvk::seed_kernel<false, 0> : which == 1 ? (const void*)pvk::seed_kernel<true, 0>
-                  : which == 2 ? (const void*)pvk::seed_kernel<false, 1> : (const void*)pvk::seed_kernel<true, 1>;
-    CK(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CK(cudaFuncSetAttribute(seed_fn[which], cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     di->attr_set[which] = true;
     di->attr_smem[which] = smem;
   }
@@ -204,12 +210,9 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   const int need = (n_events + warps - 1) / warps;
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
-  if (mvf) {
-    if (dbg) pvk::seed_kernel<true, 1><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
-    else pvk::seed_kernel<false, 1><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
-  } else {
-    if (dbg) pvk::seed_kernel<true, 0><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
-    else pvk::seed_kernel<false, 0><<<grid, warps * pvk::TEAM, smem, stream>>>(kp, ka);
+  {
+    void* kargs[2] = {(void*)&kp, (void*)&ka};
+    CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(warps * pvk::TEAM), kargs, (size_t)smem, stream));
   }
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
@@ -262,6 +265,7 @@ int pv_params_default(pv_params* p) {
   p->max_vtx_per_event = 32;
   p->flavour = PV_FLAVOUR_EXPLICIT;
   p->chi2_window = 25.0f;                                           /* P:L384, value: reading R-13 */
+  p->split_mode = PV_SPLIT_Z_ORDERED;
   return PV_OK;
 }
 

@@ -80,6 +80,7 @@ struct KParams {
   float conv_dchi2, conv_dz, merge_ratio, max_beam_dist2;
   int max_vtx;
   int flavour;                   // PV_FLAVOUR_*
+  int split_mode;                // PV_SPLIT_*
   float chi2_window;             // multi-vertex flavour: list a track for a seed iff chi2 at the seed position < this
   float mv_e0;                   // exp(-chi2_max / 2), the constant of the denominator of Eq. 19
   int region0_words;             // int32 words of the histogram region (multiple of 32)
@@ -223,6 +224,103 @@ __device__ __forceinline__ int sweep(const int* __restrict__ H, int b0, const KP
   return count;
 }
 
+// ---- a3, x86 variant of the splitting (reading R-16): "the smallest minimum between the two largest maxima,
+// recursively".  Same interface as sweep().  An explicit stack of bin ranges replaces the recursion (left part first,
+// so the leaves come out in z order); every range is analysed with the hysteresis sweep of R-4.2: pass 1 finds the
+// two highest significant maxima, pass 2 the lowest significant minimum between them, pass 3 the integrals and
+// peak bins of the two parts.
+struct Part { int sum, amax, amaxp; };
+
+__device__ __forceinline__ Part part_of(const int* __restrict__ H, int s, int e) {
+  Part r = {0, -1, s};
+#pragma unroll 1
+  for (int k = s; k < e; ++k) {
+    const int h = H[k];
+    r.sum += h;
+    if (h > r.amax) { r.amax = h; r.amaxp = k; }
+  }
+  return r;
+}
+
+__device__ int split_x86(const int* __restrict__ H, int b0, const KParams& P, int wbase,
+                         int* sb, int* se, int* sp, Cl& c0, Cl& c1) {
+  int b1 = b0 + 1;
+#pragma unroll 1
+  while (b1 < P.nbins && H[b1] > P.T_bin) ++b1;
+  int count = 0;
+  {
+    const Part root = part_of(H, b0, b1);
+    if (root.sum < P.I_min[bin_region(root.amaxp, P)]) return 0;   // every seed passes the integral cut
+  }
+  constexpr int DEPTH = 32;
+  unsigned stack[DEPTH];
+  int top = 0;
+  stack[top++] = (unsigned)b0 | ((unsigned)b1 << 16);
+#pragma unroll 1
+  while (top > 0) {
+    const unsigned r = stack[--top];
+    const int s = (int)(r & 0xffffu), e = (int)(r >> 16);
+    // pass 1: significant maxima of [s, e); the highest (ties: lower bin) and the second highest
+    int h1 = -1, j1 = -1, h2 = -1, j2 = -1, n_max = 0;
+    auto new_max = [&](int h) {
+      if (h > h1) { h2 = h1; j2 = j1; h1 = h; j1 = n_max; }
+      else if (h > h2) { h2 = h; j2 = n_max; }
+      ++n_max;
+    };
+    {
+      bool look_max = true;
+      int mx = H[s], mn = 0;
+#pragma unroll 1
+      for (int k = s + 1; k < e; ++k) {
+        const int h = H[k];
+        if (look_max) {
+          if (h > mx) mx = h;
+          else if (mx - h > P.D) { new_max(mx); mn = h; look_max = false; }
+        } else {
+          if (h < mn) mn = h;
+          else if (h - mn > P.D) { mx = h; look_max = true; }
+        }
+      }
+      if (look_max) new_max(mx);
+    }
+    int c = -1;
+    if (n_max >= 2 && top + 2 <= DEPTH) {
+      // pass 2: the lowest significant minimum between them (MIN j lies between MAX j-1 and MAX j)
+      const int lo = min(j1, j2), hi = max(j1, j2);
+      bool look_max = true;
+      int mx = H[s], mn = 0, mnp = s, seen = 0, cmin = 0x7fffffff;
+#pragma unroll 1
+      for (int k = s + 1; k < e; ++k) {
+        const int h = H[k];
+        if (look_max) {
+          if (h > mx) mx = h;
+          else if (mx - h > P.D) { ++seen; mn = h; mnp = k; look_max = false; }
+        } else {
+          if (h < mn) { mn = h; mnp = k; }
+          else if (h - mn > P.D) {
+            if (seen > lo && seen <= hi && mn < cmin) { cmin = mn; c = mnp; }
+            mx = h; look_max = true;
+          }
+        }
+      }
+      // pass 3: split iff both parts carry the minimum cluster integral
+      const Part L = part_of(H, s, c), R = part_of(H, c, e);
+      if (!(L.sum >= P.I_min[bin_region(L.amaxp, P)] && R.sum >= P.I_min[bin_region(R.amaxp, P)])) c = -1;
+    }
+    if (c >= 0) {
+      stack[top++] = (unsigned)c | ((unsigned)e << 16);     // right part, popped after the left one
+      stack[top++] = (unsigned)s | ((unsigned)c << 16);
+    } else {                                               // leaf: a seed cluster
+      const Part leaf = part_of(H, s, e);
+      if (count == 0) { c0.b = s; c0.e = e; c0.p = leaf.amaxp; }
+      if (count == 1) { c1.b = s; c1.e = e; c1.p = leaf.amaxp; }
+      if (wbase >= 0 && wbase + count < P.max_vtx) { sb[wbase + count] = s; se[wbase + count] = e; sp[wbase + count] = leaf.amaxp; }
+      ++count;
+    }
+  }
+  return count;
+}
+
 // ---- a1: POCA projection of one track (Eq. 1, Eq. 3; fp32 contract of DESIGN.md section 3) ---------------------
 struct Proj {
   float zp, sg, inv;             // z_poca, sigma_poca, 1 / (3 sigma_poca)
@@ -301,7 +399,7 @@ __device__ __forceinline__ void team_sync(int bar) {
   asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(TEAM) : "memory");
 }
 
-template <bool DBG, int FLAV>
+template <bool DBG, int FLAV, int SPLIT>
 __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt, const int bar) {
   const int lane = tt & 31, tw = tt >> 5;
   int* H = reinterpret_cast<int*>(wsm);
@@ -513,7 +611,8 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
         const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
         if (!__any_sync(FULL, run)) break;
         if (run) {
-          const int cc = sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+          const int cc = SPLIT ? split_x86(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1)
+                               : sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
           if (rep == 0) c = cc;
         }
         if (rep == 0) {
@@ -837,7 +936,7 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
   }
 }
 
-template <bool DBG, int FLAV>
+template <bool DBG, int FLAV, int SPLIT>
 __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_constant__ KParams P,
                                                                    const __grid_constant__ KArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -857,7 +956,7 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
   while (e < A.n_events) {
     int nxt = 0;
     if (tt == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);  // issued now, consumed after this event
-    seed_event<DBG, FLAV>(e, P, A, wsm, tt, bar);
+    seed_event<DBG, FLAV, SPLIT>(e, P, A, wsm, tt, bar);
     team_sync(bar);                                        // the team is done with this event's shared memory
     if (tt == 0) misc[8] = nxt;
     team_sync(bar);

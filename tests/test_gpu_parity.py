@@ -264,6 +264,57 @@ def test_track_ip(pv, oracle, idx, n):
     assert (got["ip_vertex"][tv >= 0] == tv[tv >= 0]).mean() > 0.97
 
 
+@pytest.mark.parametrize("idx,n,mv", [(3, 3000, False), (2, 1000, False), (2, 600, True)])
+def test_recursive_splitter(pv, oracle, idx, n, mv):
+    """split_mode = PV_SPLIT_RECURSIVE (the paper's x86 splitting, reading R-16) in both flavours: seeds
+    bit-exact against the oracle in the same mode; on high pile-up some events split differently from the
+    z-ordered variant."""
+    from oracle import compare
+    data = events.generate(events.config(idx, n))
+    mk_p, mk_o = (pv.multivertex_params, oracle.mv_params) if mv else (pv.default_params, oracle.default_params)
+    p, po = mk_p(split_mode=1), mk_o(split_mode=1)
+    got = pv.find(data, p, debug=True, n_hist_events=100)
+    ref = oracle.find(data, po, debug=True, n_hist_events=100, trace=True, n_threads=8)
+    rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep, allow_ties_frac=0.03)
+    assert rep["seed_bins_mismatch"] == 0 and rep["seed_z_mismatch"] == 0 and rep["n_seeds_mismatch"] == 0
+
+
+def test_recursive_splitter_differs_on_a_small_middle_peak(pv, oracle):
+    """A constructed event (two 6-track vertices two bins apart from a 1-track bump, on a background of three wide
+    tracks): the z-ordered variant cuts at the first dip, the recursive one at the lower dip between the two largest
+    maxima (hand-worked in tests/golden/peaks_x86_handbuilt.json for the same shape).  Both modes bit-exact vs oracle."""
+    from oracle import compare
+    f = np.float32
+
+    rng = np.random.default_rng(3)
+
+    def trk(b, sig_poca, n):                               # tracks through the beamline at the centre of bin b
+        zc = -550 + 0.25 * (b + 0.5)
+        phi = rng.uniform(0, 2 * np.pi, n)
+        return dict(x=np.zeros(n, f), y=np.zeros(n, f), z=np.full(n, zc, f),
+                    tx=(0.3 * np.cos(phi)).astype(f), ty=(0.3 * np.sin(phi)).astype(f),
+                    var_x=np.full(n, (sig_poca * 0.3) ** 2, f), var_y=np.full(n, (sig_poca * 0.3) ** 2, f),
+                    var_tx=np.full(n, 1e-6, f), var_ty=np.full(n, 1e-6, f))
+    parts = [trk(2200, 0.01, 6), trk(2202, 0.01, 1), trk(2204, 0.01, 6), trk(2201, 0.3, 2), trk(2203, 0.3, 1)]
+    ev = {k: np.concatenate([q[k] for q in parts]) for k in events.FIELDS}
+    small = events.generate(events.config(0, 2))
+    so = small["offsets"]
+    data = events.from_lists([ev, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, ev])
+    seeds = {}
+    for mode in (0, 1):
+        p, po = pv.default_params(split_mode=mode), oracle.default_params(split_mode=mode)
+        got = pv.find(data, p, debug=True, n_hist_events=3)
+        ref = oracle.find(data, po, debug=True, n_hist_events=3, trace=True)
+        rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
+        _assert_parity(rep, allow_ties_frac=1.0)
+        assert rep["seed_bins_mismatch"] == 0 and rep["hist_mismatch"] == 0
+        seeds[mode] = got["debug"]["seed_bins"][0][:got["debug"]["n_seeds_raw"][0]].tolist()
+    assert seeds[0] == [[2200, 2201, 2200], [2201, 2205, 2204]]
+    assert seeds[1] == [[2200, 2203, 2200], [2203, 2205, 2204]]
+
+
 def test_runs_are_reproducible(pv, cfg0):
     """Integer histograms and a fixed summation order: two runs give bit-identical outputs."""
     a = pv.find(cfg0)
