@@ -400,7 +400,8 @@ __device__ __forceinline__ void team_sync(int bar) {
 }
 
 template <bool DBG, int FLAV, int SPLIT>
-__device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt, const int bar) {
+__device__ void seed_event(const int e, const int nxt, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt,
+                           const int bar) {
   const int lane = tt & 31, tw = tt >> 5;
   int* H = reinterpret_cast<int*>(wsm);
   unsigned char* tail = wsm + (size_t)P.region0_words * 4;
@@ -633,6 +634,21 @@ __device__ void seed_event(const int e, const KParams& P, const KArgs& A, unsign
     if (lane == 0) {
       misc[2 + tw] = np_;
       if (i < iend) misc[6] = 1;                           // list full (never with physical histograms): slow path
+    }
+  }
+  if (tw == 1) {
+    // warp 1 now waits for warp 0's sweeps: it uses the time to pull the first chunk of the team's NEXT event
+    // (its lane 0 holds the event index) into L2
+    const int ne = __shfl_sync(FULL, nxt, 0);
+    if (ne < A.n_events) {
+      const int pt0 = __ldg(A.offsets + ne);
+      const int pn = min(__ldg(A.offsets + ne + 1) - pt0, CHUNK);
+      if (lane * 32 < pn + 32) {                           // one 128-byte line per lane and array
+        const size_t o = (size_t)pt0 + lane * 32;
+        const float* arr[9] = {A.x, A.y, A.z, A.tx, A.ty, A.var_x, A.var_y, A.var_tx, A.var_ty};
+#pragma unroll
+        for (int q = 0; q < 9; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr[q] + o));
+      }
     }
   }
   team_sync(bar);
@@ -954,11 +970,11 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
   team_sync(bar);
   int e = misc[8];
   while (e < A.n_events) {
-    int nxt = 0;
-    if (tt == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);  // issued now, consumed after this event
-    seed_event<DBG, FLAV, SPLIT>(e, P, A, wsm, tt, bar);
+    int nxt = 0x7fffffff;
+    if (tt == 32) nxt = (int)atomicAdd(A.evt_counter, 1u); // issued now, consumed by the prefetch and after this event
+    seed_event<DBG, FLAV, SPLIT>(e, nxt, P, A, wsm, tt, bar);
     team_sync(bar);                                        // the team is done with this event's shared memory
-    if (tt == 0) misc[8] = nxt;
+    if (tt == 32) misc[8] = nxt;
     team_sync(bar);
     e = misc[8];
   }
