@@ -35,7 +35,7 @@ constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
 constexpr int TEAM_WARPS = 2;       // warps per event in seed_kernel
 constexpr int TEAM = 32 * TEAM_WARPS;
-constexpr int MAX_TEAMS = 13;       // events in flight per CTA (named barriers 1..13; 13 histograms fill 227 KB)
+constexpr int MAX_TEAMS = 14;       // events in flight per CTA (named barriers 1..14; 14 histograms fill 227 KB)
 constexpr int CHUNK = 128;          // tracks per fill chunk
 constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
 constexpr int UNIT = 8;             // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
@@ -51,18 +51,21 @@ constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
 constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
 
 // Per-team shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
+// The 2 KB that stage the fill (track windows and the unit list) are dead once the histogram is complete; the peak
+// search and the association reuse them, so that 14 teams fit the 227 KB of an SM.
 constexpr int SM_TOUCHED = 0;                          // uint8 tb[128]        histogram words written by the fill
-constexpr int SM_TWL = SM_TOUCHED + MAX_WORDS;         // uint8 twl[128]       list of touched words, ascending
-constexpr int SM_CNT = SM_TWL + MAX_WORDS;             // int cnt[2][32]       tracks per seed, per warp
-constexpr int SM_CUR = SM_CNT + TEAM_WARPS * 32 * 4;   // int cur[2][32]       running record position, per warp
-constexpr int SM_SEED = SM_CUR + TEAM_WARPS * 32 * 4;  // int sb[32], se[32], sp[32]; float zs[32]; int part[32]
-constexpr int SM_MISC = SM_SEED + 5 * MAXV * 4;        // int misc[16]         warp totals, next event
-constexpr int SM_STAGE = SM_MISC + 64;                 // float zp[128], inv[128]; int lonb[128]   (fill)
-constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // uint16 list[256]  (fill)
-constexpr int SM_BINS = SM_LIST + LIST_CAP * 2;        // int16 binsm[256]     central bins of the first 256 tracks
-constexpr int SM_TAIL_BYTES = SM_BINS + BINS_SM * 2;
-// peak search overlay on the (dead) stage and list: uint16 protostart[2][PROTO_CAP]
-static_assert(TEAM_WARPS * PROTO_CAP * 2 <= CHUNK * 12 + LIST_CAP * 2, "peak-search overlay fits");
+constexpr int SM_MISC = SM_TOUCHED + MAX_WORDS;        // int misc[16]         warp totals, next event
+constexpr int SM_BINS = SM_MISC + 64;                  // int16 binsm[256]     central bins of the first 256 tracks
+constexpr int SM_STAGE = SM_BINS + BINS_SM * 2;        // fill:  float zp[128], inv[128]; int lonb[128]
+constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // fill:  uint16 list[256]
+constexpr int SM_PROTO = SM_STAGE;                     // peaks: uint16 protostart[2][PROTO_CAP]      (over the stage)
+constexpr int SM_CUR = SM_STAGE;                       // a4:    int cur[2][32] running record position (over protostart)
+constexpr int SM_SEED = SM_PROTO + TEAM_WARPS * PROTO_CAP * 2;   // peaks..a4: int sb[32], se[32], sp[32]; float zs[32]; int part[32]
+constexpr int SM_CNT = SM_SEED + 5 * MAXV * 4;         // a4:    int cnt[2][32] tracks per seed, per warp
+constexpr int SM_TWL = SM_CNT + TEAM_WARPS * 32 * 4;   // peaks: uint8 twl[128] list of touched words, ascending
+constexpr int SM_TAIL_BYTES = SM_LIST + LIST_CAP * 2;
+static_assert(SM_TWL + MAX_WORDS <= SM_TAIL_BYTES, "the overlays fit the fill stage and unit list");
+static_assert(TEAM_WARPS * 32 * 4 <= TEAM_WARPS * PROTO_CAP * 2, "cur[] fits over protostart[]");
 static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0 && SM_TAIL_BYTES % 16 == 0, "alignment of the vector accesses");
 
 struct KParams {
@@ -573,7 +576,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   // Both warps look for proto-cluster starts, each in its half of the touched words; then warp 0 alone runs the
   // z-ordered sweeps with one lane per proto-cluster of the whole event (the number of serial sweep steps is the
   // longest proto-cluster of the event, once) and computes the seed positions.
-  uint16_t* ps0 = reinterpret_cast<uint16_t*>(tail + SM_STAGE);
+  uint16_t* ps0 = reinterpret_cast<uint16_t*>(tail + SM_PROTO);
   uint16_t* ps1 = ps0 + PROTO_CAP;
   // proto-cluster starts of the words [i, iend) -> ps[0 .. return value); stops early (i < iend) when ps is full
   auto detect = [&](int& i, const int iend, uint16_t* ps) -> int {
@@ -962,7 +965,7 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
   int* misc = reinterpret_cast<int*>(wsm + (size_t)P.region0_words * 4 + SM_MISC);
   {
     int4* Z = reinterpret_cast<int4*>(wsm);                // histogram and touched-word flags start at zero
-    const int nq = (P.region0_words * 4 + SM_TWL) >> 4;
+    const int nq = (P.region0_words * 4 + SM_MISC) >> 4;
 #pragma unroll 1
     for (int i = tt; i < nq; i += TEAM) Z[i] = make_int4(0, 0, 0, 0);
   }
