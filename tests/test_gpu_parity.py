@@ -323,6 +323,27 @@ def test_runs_are_reproducible(pv, cfg0):
         assert np.array_equal(a[k], b[k], equal_nan=True), k
 
 
+@pytest.mark.parametrize("mode", ["explicit", "multivertex", "recursive"])
+def test_repeated_runs_are_bit_identical_on_high_pileup(pv, mode):
+    """Five launches over 3000 high pile-up events (multi-chunk events, many seeds, big-seed fit path): every output
+    bit-identical -- a race in the team protocol or an order-dependent sum would show up here."""
+    data = events.generate(events.config(2, 3000))
+    p = {"explicit": pv.default_params, "multivertex": pv.multivertex_params,
+         "recursive": lambda: pv.default_params(split_mode=1)}[mode]()
+    b = pv.DeviceBatch(data, p)
+    ref = None
+    for _ in range(5):
+        b.find()
+        r = b.results()
+        if ref is None:
+            ref = r
+            continue
+        m = np.arange(p.max_vtx_per_event)[None, :] < r["n_vtx"][:, None]
+        for k in r:
+            a, c = (r[k][m], ref[k][m]) if k.startswith("vtx_") else (r[k], ref[k])
+            assert np.array_equal(a, c, equal_nan=True), k
+
+
 def test_full_size_throughput_config(pv, oracle):
     """configs[1] at its full size (100 000 events), non-debug kernel, the launch configuration bench.py times;
     the oracle (8 threads) is compared on every final output."""
