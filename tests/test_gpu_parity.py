@@ -344,6 +344,37 @@ def test_repeated_runs_are_bit_identical_on_high_pileup(pv, mode):
             assert np.array_equal(a, c, equal_nan=True), k
 
 
+def test_beamline_offset_robustness_scan(pv):
+    """Synthetic version of the paper's Fig. 8: the finder is told a beamline that is off by d from the
+    true one (x direction).  "an efficiency of 99 % within a beamline position uncertainty of 50 um ... 99.9 %
+    within 20 um": efficiency of reconstructible PVs (>= 4 tracks, matched within 5 sigma_z) relative
+    to the zero-offset run, both flavours.  Far off (1 mm) the 0.3 mm beamline-distance cut removes the pp PVs."""
+    data = events.generate(events.config(0, 3000), with_truth=True)
+    tr = data["truth"]
+    order = np.argsort(tr["pv_event"], kind="stable")
+    pe, pz, pn = tr["pv_event"][order], tr["pv_z"][order], tr["pv_ntracks"][order]
+    first = np.searchsorted(pe, np.arange(3001))
+
+    def n_found(r):
+        found = 0
+        for e in range(3000):
+            vz = r["vtx_pos"][e, :r["n_vtx"][e], 2]
+            if not len(vz):
+                continue
+            vs = np.sqrt(r["vtx_cov"][e, :r["n_vtx"][e], 5])
+            for z, n in zip(pz[first[e]:first[e + 1]], pn[first[e]:first[e + 1]]):
+                if n >= 4:
+                    j = int(np.argmin(np.abs(vz - z)))
+                    found += abs(vz[j] - z) < 5 * vs[j]
+        return found
+    for mk in (pv.default_params, pv.multivertex_params):
+        base = n_found(pv.find(data, mk()))
+        assert base > 12000
+        rel = {d: n_found(pv.find(data, mk(beam_x=d))) / base for d in (0.02, 0.05, 1.0)}
+        print(mk.__name__, "relative efficiency vs beamline offset [mm]:", rel)
+        assert rel[0.02] >= 0.999 and rel[0.05] >= 0.99 and rel[1.0] < 0.05
+
+
 def test_full_size_throughput_config(pv, oracle):
     """configs[1] at its full size (100 000 events), non-debug kernel, the launch configuration bench.py times;
     the oracle (8 threads) is compared on every final output."""
