@@ -364,6 +364,14 @@ static void chol3_solve(const double L[3][3], const double b[3], double x[3]) {
   }
 }
 
+/* Eq. 2, one transverse coordinate: V(z) = V_xx + 2 dz V_xtx + dz^2 V_txtx.  The x-y blocks are
+ * uncorrelated in the simplified track fit, so V_xy, V_xty, V_txty do not appear.  cx == NULL (or a NULL
+ * member) means a diagonal input covariance. */
+static double var_at(double v, double vt, const float *cross, int i, double dz) {
+  double c = cross ? (double)cross[i] : 0.0;
+  return v + 2.0 * dz * c + dz * dz * vt;
+}
+
 /* Eq. 19: w_ij = exp(-chi2_ij / 2) / (exp(-chi2_max / 2) + sum_k exp(-chi2_ik / 2)); the sum runs over
  * all vertex candidates k including j itself. */
 double pvo_mv_weight(double chi2_own, double chi2_max, const double *chi2_others, int n_others) {
@@ -441,7 +449,7 @@ static void trace_row(double *trace, int it, const double a[3], double C[3][3], 
 static int fit_core(int m, const int32_t *idx,
                     const float *x, const float *y, const float *z, const float *tx, const float *ty,
                     const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-                    const double seed[3], const pvo_params *p, const double *other,
+                    const double seed[3], const pvo_params *p, const double *other, const pvo_cross *cx,
                     double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
                     double *w, double *trace) {
   double a[3] = {seed[0], seed[1], seed[2]};
@@ -452,8 +460,8 @@ static int fit_core(int m, const int32_t *idx,
   for (int j = 0; j < m; ++j) {
     int i = idx[j];
     double dz = seed[2] - (double)z[i];
-    double Vx = (double)var_x[i] + dz * dz * (double)var_tx[i];
-    double Vy = (double)var_y[i] + dz * dz * (double)var_ty[i];
+    double Vx = var_at((double)var_x[i], (double)var_tx[i], cx ? cx->xtx : NULL, i, dz);
+    double Vy = var_at((double)var_y[i], (double)var_ty[i], cx ? cx->yty : NULL, i, dz);
     int ok = (Vx > 0.0) && (Vy > 0.0) && isfinite(Vx) && isfinite(Vy);
     Wx[j] = ok ? 1.0 / Vx : -1.0;                    /* -1 marks an unusable track: w = 0 always (R-7) */
     Wy[j] = ok ? 1.0 / Vy : -1.0;
@@ -501,10 +509,10 @@ static int fit_core(int m, const int32_t *idx,
 int pvo_fit(int m, const int32_t *idx,
             const float *x, const float *y, const float *z, const float *tx, const float *ty,
             const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-            const double seed[3], const pvo_params *p,
+            const double seed[3], const pvo_params *p, const pvo_cross *cx,
             double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
             double *w, double *trace) {
-  return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, NULL, out_pos, out_cov, out_chi2,
+  return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, NULL, cx, out_pos, out_cov, out_chi2,
                   out_ntrk, out_niter, w, trace);
 }
 
@@ -515,10 +523,10 @@ int pvo_fit(int m, const int32_t *idx,
 int pvo_fit_mv(int m, const int32_t *idx,
                const float *x, const float *y, const float *z, const float *tx, const float *ty,
                const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-               const double seed[3], const pvo_params *p, const double *other,
+               const double seed[3], const pvo_params *p, const double *other, const pvo_cross *cx,
                double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
                double *w, double *trace) {
-  return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, other, out_pos, out_cov, out_chi2,
+  return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, other, cx, out_pos, out_cov, out_chi2,
                   out_ntrk, out_niter, w, trace);
 }
 
@@ -526,10 +534,10 @@ int pvo_fit_mv(int m, const int32_t *idx,
  * position; returns a negative number when the extrapolated variance is unusable (R-7). */
 double pvo_track_chi2(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
                       const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-                      const double pos[3]) {
+                      const pvo_cross *cx, const double pos[3]) {
   double dz = pos[2] - (double)z[i];
-  double Vx = (double)var_x[i] + dz * dz * (double)var_tx[i];
-  double Vy = (double)var_y[i] + dz * dz * (double)var_ty[i];
+  double Vx = var_at((double)var_x[i], (double)var_tx[i], cx ? cx->xtx : NULL, i, dz);
+  double Vy = var_at((double)var_y[i], (double)var_ty[i], cx ? cx->yty : NULL, i, dz);
   if (!((Vx > 0.0) && (Vy > 0.0) && isfinite(Vx) && isfinite(Vy))) return -1.0;
   double rx = (double)x[i] + dz * (double)tx[i] - pos[0];
   double ry = (double)y[i] + dz * (double)ty[i] - pos[1];
@@ -545,10 +553,10 @@ double pvo_track_chi2(int i, const float *x, const float *y, const float *z, con
  * Returns 0, or -1 when the track covariance is unusable there (R-7) or the 2x2 matrix is not positive definite. */
 int pvo_ip_one(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
                const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-               const double pos[3], const double C[6], double *ip, double *ip_chi2) {
+               const pvo_cross *cx, const double pos[3], const double C[6], double *ip, double *ip_chi2) {
   double dz = pos[2] - (double)z[i];
-  double Vx = (double)var_x[i] + dz * dz * (double)var_tx[i];
-  double Vy = (double)var_y[i] + dz * dz * (double)var_ty[i];
+  double Vx = var_at((double)var_x[i], (double)var_tx[i], cx ? cx->xtx : NULL, i, dz);
+  double Vy = var_at((double)var_y[i], (double)var_ty[i], cx ? cx->yty : NULL, i, dz);
   if (!((Vx > 0.0) && (Vy > 0.0) && isfinite(Vx) && isfinite(Vy))) return -1;
   double a = (double)tx[i], b = (double)ty[i];
   double rx = (double)x[i] + dz * a - pos[0];
@@ -571,7 +579,7 @@ int pvo_ip_one(int i, const float *x, const float *y, const float *z, const floa
  * to that vertex; ip_vertex = -1, ip = ip_chi2 = -1 when the event has no usable vertex for the track. */
 int pvo_track_ip(const float *x, const float *y, const float *z, const float *tx, const float *ty,
                  const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-                 const int32_t *offsets, int n_events, int max_vtx,
+                 const pvo_cross *cx, const int32_t *offsets, int n_events, int max_vtx,
                  const double *vtx_pos, const double *vtx_cov, const int32_t *n_vtx,
                  double *ip, double *ip_chi2, int32_t *ip_vertex) {
   for (int e = 0; e < n_events; ++e)
@@ -580,7 +588,7 @@ int pvo_track_ip(const float *x, const float *y, const float *z, const float *tx
       for (int v = 0; v < n_vtx[e] && v < max_vtx; ++v) {
         size_t o = (size_t)e * max_vtx + v;
         double d, c2;
-        if (pvo_ip_one(t, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, vtx_pos + 3 * o, vtx_cov + 6 * o, &d, &c2) != 0) continue;
+        if (pvo_ip_one(t, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, cx, vtx_pos + 3 * o, vtx_cov + 6 * o, &d, &c2) != 0) continue;
         if (ip_vertex[t] < 0 || c2 < ip_chi2[t]) { ip[t] = d; ip_chi2[t] = c2; ip_vertex[t] = v; }
       }
     }
@@ -622,12 +630,14 @@ static void scratch_free(scratch *s) {
 
 static void find_event(int e, const float *x, const float *y, const float *z, const float *tx, const float *ty,
                        const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-                       const int32_t *offsets, const pvo_params *p, scratch *S,
+                       const pvo_cross *cx_all, const int32_t *offsets, const pvo_params *p, scratch *S,
                        double *vtx_pos, double *vtx_cov, double *vtx_chi2, int32_t *vtx_ntracks, int32_t *vtx_niter,
                        int32_t *n_vtx, double *trk_weight, int32_t *trk_vertex, uint32_t *event_status,
                        const pvo_debug *dbg) {
   const int t0 = offsets[e], n = offsets[e + 1] - offsets[e];
   const int mv = p->max_vtx_per_event, nb = S->nbins;
+  pvo_cross cxe = {cx_all && cx_all->xtx ? cx_all->xtx + t0 : NULL, cx_all && cx_all->yty ? cx_all->yty + t0 : NULL};
+  const pvo_cross *cx = cx_all ? &cxe : NULL;             /* the event's slice of the cross terms */
   uint32_t status = 0;
   n_vtx[e] = 0;
   for (int i = 0; i < n; ++i) { trk_vertex[t0 + i] = -1; trk_weight[t0 + i] = 0.0; }
@@ -685,7 +695,7 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
         float zs = S->zs[k];
         double pos[3] = {(double)fmaf(p->beam_tx, zs, p->beam_x), (double)fmaf(p->beam_ty, zs, p->beam_y), (double)zs};
         double c2 = (S->flags[i] & PVO_TRK_ASSIGNABLE)
-                        ? pvo_track_chi2(i, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0, var_ty + t0, pos)
+                        ? pvo_track_chi2(i, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0, var_ty + t0, cx, pos)
                         : -1.0;
         S->Em[(size_t)i * mv + k] = c2 >= 0.0 ? c2 : -1.0;           /* chi2 kept; negative = not usable */
       }
@@ -715,7 +725,7 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
     double chi2 = 0.0;
     memset(S->trace, 0, sizeof(double) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE);
     int rc = fit_core(m, S->idx, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0,
-                      var_ty + t0, seed, p, mvf ? S->other : NULL, S->s_pos + 3 * k, S->s_cov + 6 * k, &chi2,
+                      var_ty + t0, seed, p, mvf ? S->other : NULL, cx, S->s_pos + 3 * k, S->s_cov + 6 * k, &chi2,
                       &S->s_ntrk[k], &S->s_niter[k], S->w, S->trace);
     S->s_chi2[k] = chi2;
     if (rc != 0) { status |= PVO_EVT_SINGULAR_FIT; S->s_niter[k] = -1; }
@@ -791,7 +801,7 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
 
 int pvo_find(const float *x, const float *y, const float *z, const float *tx, const float *ty,
              const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-             const int32_t *offsets, int n_events, const pvo_params *p,
+             const pvo_cross *cx, const int32_t *offsets, int n_events, const pvo_params *p,
              double *vtx_pos, double *vtx_cov, double *vtx_chi2, int32_t *vtx_ntracks, int32_t *vtx_niter,
              int32_t *n_vtx, double *trk_weight, int32_t *trk_vertex, uint32_t *event_status,
              const pvo_debug *dbg, int n_threads) {
@@ -805,7 +815,7 @@ int pvo_find(const float *x, const float *y, const float *z, const float *tx, co
     scratch *S = scratch_new(p);
 #pragma omp for schedule(dynamic, 64)
     for (int e = 0; e < n_events; ++e)
-      find_event(e, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, offsets, p, S, vtx_pos, vtx_cov, vtx_chi2,
+      find_event(e, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, cx, offsets, p, S, vtx_pos, vtx_cov, vtx_chi2,
                  vtx_ntracks, vtx_niter, n_vtx, trk_weight, trk_vertex, event_status, dbg);
     scratch_free(S);
   }

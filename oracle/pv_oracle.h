@@ -41,6 +41,10 @@ typedef struct pvo_params {
                                           1 = smallest minimum between the two largest maxima, recursively (x86) */
 } pvo_params;
 
+/* NEXT-2: the x-tx and y-ty elements of the track covariance (Eq. 2: V_xx(z) = V_xx + 2 dz V_xtx + dz^2 V_txtx).
+ * Optional everywhere: a NULL struct or member is a diagonal covariance. */
+typedef struct pvo_cross { const float *xtx, *yty; } pvo_cross;
+
 enum { PVO_S = 1 << 20 };              /* fixed-point unit: one track's full mass */
 enum { PVO_MAX_TRACKS = 2047, PVO_TRACE_STRIDE = 11, PVO_TRACE_ITERS = 16 };
 enum { PVO_EVT_TOO_MANY_TRACKS = 1, PVO_EVT_VTX_OVERFLOW = 2, PVO_EVT_SINGULAR_FIT = 4 };
@@ -84,7 +88,7 @@ int pvo_assign(int n, const int32_t *bin, const int32_t *flags, int n_seeds,
 int pvo_fit(int m, const int32_t *idx,
             const float *x, const float *y, const float *z, const float *tx, const float *ty,
             const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-            const double seed[3], const pvo_params *p,
+            const double seed[3], const pvo_params *p, const pvo_cross *cx,
             double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
             double *w, double *trace);
 
@@ -93,13 +97,13 @@ double pvo_mv_weight(double chi2_own, double chi2_max, const double *chi2_others
 /* chi2 of track i relative to a vertex at pos[3] (Eq. 7 with W from Eq. 2 at pos); < 0 = unusable (R-7). */
 double pvo_track_chi2(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
                       const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-                      const double pos[3]);
+                      const pvo_cross *cx, const double pos[3]);
 /* O7, multi-vertex flavour: pvo_fit with the weights of Eq. 19; other[j] = exp(-chi2_max / 2) + sum over the
  * other candidates of exp(-chi2_jk / 2) at their seed positions.  out_ntrk = tracks with w >= 1/2. */
 int pvo_fit_mv(int m, const int32_t *idx,
                const float *x, const float *y, const float *z, const float *tx, const float *ty,
                const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-               const double seed[3], const pvo_params *p, const double *other,
+               const double seed[3], const pvo_params *p, const double *other, const pvo_cross *cx,
                double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
                double *w, double *trace);
 
@@ -107,11 +111,11 @@ int pvo_fit_mv(int m, const int32_t *idx,
  * contain it; returns -1 when the covariance is unusable. */
 int pvo_ip_one(int i, const float *x, const float *y, const float *z, const float *tx, const float *ty,
                const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-               const double pos[3], const double C[6], double *ip, double *ip_chi2);
+               const pvo_cross *cx, const double pos[3], const double C[6], double *ip, double *ip_chi2);
 /* per track: the vertex of its event with the smallest IP chi2; -1 if none */
 int pvo_track_ip(const float *x, const float *y, const float *z, const float *tx, const float *ty,
                  const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-                 const int32_t *offsets, int n_events, int max_vtx,
+                 const pvo_cross *cx, const int32_t *offsets, int n_events, int max_vtx,
                  const double *vtx_pos, const double *vtx_cov, const int32_t *n_vtx,
                  double *ip, double *ip_chi2, int32_t *ip_vertex);
 
@@ -143,7 +147,7 @@ typedef struct pvo_debug {
  * timing harness only; results do not depend on it).  Returns 0 or a negative error. */
 int pvo_find(const float *x, const float *y, const float *z, const float *tx, const float *ty,
              const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
-             const int32_t *offsets, int n_events, const pvo_params *p,
+             const pvo_cross *cx, const int32_t *offsets, int n_events, const pvo_params *p,
              double *vtx_pos, double *vtx_cov, double *vtx_chi2, int32_t *vtx_ntracks, int32_t *vtx_niter,
              int32_t *n_vtx, double *trk_weight, int32_t *trk_vertex, uint32_t *event_status,
              const pvo_debug *dbg, int n_threads);

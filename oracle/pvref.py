@@ -90,6 +90,22 @@ def lib():
     return _lib
 
 
+class Cross(C.Structure):
+    """struct pvo_cross: optional x-tx / y-ty covariance elements (Eq. 2)."""
+    _fields_ = [("xtx", C.c_void_p), ("yty", C.c_void_p)]
+
+
+def _cross(tracks):
+    """(ctypes argument, keep-alive list) for the optional "cov_xtx" / "cov_yty" arrays of a track dict."""
+    if "cov_xtx" not in tracks and "cov_yty" not in tracks:
+        return None, []
+    n = np.asarray(tracks["x"]).size
+    a = _f32(tracks.get("cov_xtx", np.zeros(n, np.float32)))
+    b = _f32(tracks.get("cov_yty", np.zeros(n, np.float32)))
+    cx = Cross(a.ctypes.data, b.ctypes.data)
+    return C.byref(cx), [a, b, cx]
+
+
 def default_params(**over) -> Params:
     p = Params()
     lib().pvo_params_default(C.byref(p))
@@ -178,9 +194,10 @@ def fit(tracks: Dict[str, np.ndarray], idx, seed, p: Params):
     seed = np.ascontiguousarray(seed, dtype=np.float64)
     pos = np.zeros(3); cov = np.zeros(6); chi2 = C.c_double(0); ntrk = C.c_int32(0); niter = C.c_int32(0)
     w = np.zeros(max(idx.size, 1)); trace = np.zeros((TRACE_ITERS, TRACE_STRIDE))
+    cx, _keep = _cross(tracks)
     rc = lib().pvo_fit(C.c_int(idx.size), _ptr(idx), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]),
                        _ptr(a["ty"]), _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]),
-                       _ptr(seed), C.byref(p), _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk), C.byref(niter),
+                       _ptr(seed), C.byref(p), cx, _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk), C.byref(niter),
                        _ptr(w), _ptr(trace))
     return dict(pos=pos, cov=cov, chi2=chi2.value, ntrk=ntrk.value, niter=niter.value, w=w[:idx.size], trace=trace, rc=rc)
 
@@ -201,8 +218,9 @@ def mv_weight(chi2_own: float, chi2_max: float, chi2_others=()) -> float:
 def track_chi2(tracks: Dict[str, np.ndarray], i: int, pos) -> float:
     a = {k: _f32(tracks[k]) for k in ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")}
     pos = np.ascontiguousarray(pos, dtype=np.float64)
+    cx, _keep = _cross(tracks)
     return float(lib().pvo_track_chi2(C.c_int(i), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]),
-                                      _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(pos)))
+                                      _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), cx, _ptr(pos)))
 
 
 def fit_mv(tracks: Dict[str, np.ndarray], idx, seed, other, p: Params):
@@ -212,11 +230,12 @@ def fit_mv(tracks: Dict[str, np.ndarray], idx, seed, other, p: Params):
     seed = np.ascontiguousarray(seed, dtype=np.float64)
     other = np.ascontiguousarray(other, dtype=np.float64)
     assert other.size == idx.size
+    cx, _keep = _cross(tracks)
     pos = np.zeros(3); cov = np.zeros(6); chi2 = C.c_double(0); ntrk = C.c_int32(0); niter = C.c_int32(0)
     w = np.zeros(max(idx.size, 1)); trace = np.zeros((TRACE_ITERS, TRACE_STRIDE))
     rc = lib().pvo_fit_mv(C.c_int(idx.size), _ptr(idx), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]),
                           _ptr(a["ty"]), _ptr(a["var_x"]), _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]),
-                          _ptr(seed), C.byref(p), _ptr(other), _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk),
+                          _ptr(seed), C.byref(p), _ptr(other), cx, _ptr(pos), _ptr(cov), C.byref(chi2), C.byref(ntrk),
                           C.byref(niter), _ptr(w), _ptr(trace))
     return dict(pos=pos, cov=cov, chi2=chi2.value, ntrk=ntrk.value, niter=niter.value, w=w[:idx.size], trace=trace, rc=rc)
 
@@ -226,8 +245,9 @@ def ip_one(tracks: Dict[str, np.ndarray], i: int, pos, cov):
     a = {k: _f32(tracks[k]) for k in ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")}
     pos = np.ascontiguousarray(pos, dtype=np.float64); cov = np.ascontiguousarray(cov, dtype=np.float64)
     d = C.c_double(0); c2 = C.c_double(0)
+    cx, _keep = _cross(tracks)
     rc = lib().pvo_ip_one(C.c_int(i), _ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]), _ptr(a["var_x"]),
-                          _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(pos), _ptr(cov), C.byref(d), C.byref(c2))
+                          _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), cx, _ptr(pos), _ptr(cov), C.byref(d), C.byref(c2))
     return rc, d.value, c2.value
 
 
@@ -240,8 +260,9 @@ def track_ip(data: Dict[str, np.ndarray], vtx_pos, vtx_cov, n_vtx) -> Dict[str, 
     nv = _i32(n_vtx)
     mv = vp.shape[1] if vp.ndim == 3 else 1
     out = dict(ip=np.zeros(T), ip_chi2=np.zeros(T), ip_vertex=np.zeros(T, np.int32))
+    cx, _keep = _cross(data)
     rc = lib().pvo_track_ip(_ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]), _ptr(a["var_x"]),
-                            _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(off), C.c_int(E), C.c_int(mv),
+                            _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), cx, _ptr(off), C.c_int(E), C.c_int(mv),
                             _ptr(vp), _ptr(vc), _ptr(nv), _ptr(out["ip"]), _ptr(out["ip_chi2"]), _ptr(out["ip_vertex"]))
     if rc != 0:
         raise RuntimeError(f"pvo_track_ip failed: {rc}")
@@ -289,8 +310,9 @@ def find(data: Dict[str, np.ndarray], p: Optional[Params] = None, debug: bool = 
         out["debug"] = d
         if n_hist_events == 0:
             dbg.hist = None
+    cx, _keep = _cross(data)
     rc = lib().pvo_find(_ptr(a["x"]), _ptr(a["y"]), _ptr(a["z"]), _ptr(a["tx"]), _ptr(a["ty"]), _ptr(a["var_x"]),
-                        _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), _ptr(off), C.c_int(E), C.byref(p),
+                        _ptr(a["var_y"]), _ptr(a["var_tx"]), _ptr(a["var_ty"]), cx, _ptr(off), C.c_int(E), C.byref(p),
                         _ptr(out["vtx_pos"]), _ptr(out["vtx_cov"]), _ptr(out["vtx_chi2"]), _ptr(out["vtx_ntracks"]),
                         _ptr(out["vtx_niter"]), _ptr(out["n_vtx"]), _ptr(out["trk_weight"]), _ptr(out["trk_vertex"]),
                         _ptr(out["event_status"]), C.byref(dbg) if dbg is not None else None, C.c_int(n_threads))
