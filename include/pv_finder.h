@@ -133,6 +133,15 @@ int pv_find(const float* x, const float* y, const float* z, const float* tx, con
             int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
             void* workspace, size_t workspace_bytes, void* stream);
 
+/* Optional x-tx and y-ty elements of the track covariance (Eq. 2: V_xx(z) = V_xx + 2 dz V_xtx + dz^2 V_txtx;
+ * x and y are uncorrelated in the simplified track fit).  DEVICE arrays of length T; a NULL struct or
+ * member means 0 (the diagonal covariance pv_find assumes).  They enter wherever Eq. 2 is evaluated: W of the
+ * vertex fit, the chi2 of the multi-vertex flavour, the IP chi2; sigma_poca (Eq. 3) uses V_xx alone. */
+typedef struct pv_track_cov {
+  const float* cov_xtx;
+  const float* cov_yty;
+} pv_track_cov;
+
 /* Impact parameter of every track w.r.t. the PVs of its event ("the distance of closest approach of a track to
  * a vertex, called impact parameter (IP) ... the IP chi2, which is the chi2 difference of a PV reconstructed with and
  * without the track under consideration").  For each track the vertex of its event with the smallest IP chi2 is
@@ -142,12 +151,13 @@ int pv_find(const float* x, const float* y, const float* z, const float* tx, con
  * Inputs: the track arrays and offsets of pv_find (DEVICE), and its outputs vtx_pos / vtx_cov / n_vtx (DEVICE,
  * stride params->max_vtx_per_event).  Outputs (DEVICE, caller-allocated, length T): ip [mm], ip_chi2, ip_vertex
  * (index within the event); -1 in all three when the event has no vertex usable for the track.
+ * cov: optional covariance cross terms (HOST struct of DEVICE pointers, may be NULL).
  * One kernel on `stream`; never allocates or synchronises. */
 int pv_track_ip(const float* x, const float* y, const float* z, const float* tx, const float* ty,
                 const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
                 const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
                 const float* vtx_pos, const float* vtx_cov, const int32_t* n_vtx,
-                float* ip, float* ip_chi2, int32_t* ip_vertex, void* stream);
+                float* ip, float* ip_chi2, int32_t* ip_vertex, const pv_track_cov* cov /* nullable */, void* stream);
 
 /* Parity taps: every member is a nullable DEVICE pointer; no global state. */
 typedef struct pv_debug {
@@ -176,6 +186,15 @@ int pv_find_debug(const float* x, const float* y, const float* z, const float* t
                   float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
                   int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
                   void* workspace, size_t workspace_bytes, void* stream, const pv_debug* dbg);
+
+/* pv_find with the covariance cross terms of Eq. 2 (cov, nullable) and, optionally, the parity taps (dbg, nullable):
+ * pv_find(...) == pv_find_ext(..., NULL, NULL). */
+int pv_find_ext(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+                void* workspace, size_t workspace_bytes, void* stream, const pv_track_cov* cov, const pv_debug* dbg);
 
 /* ---- host-buffer entry (the paper's host pipeline: "several streams ... each processing a batch",
  * host->device copies overlapped with compute).  A pv_host_ctx owns device buffers, pinned staging and

@@ -28,7 +28,7 @@ FLAVOUR_MULTIVERTEX = 1
 FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
 EXPORTS = (
-    "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug", "pv_track_ip",
+    "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug", "pv_find_ext", "pv_track_ip",
     "pv_host_ctx_create", "pv_host_ctx_destroy", "pv_find_host", "pv_host_register", "pv_host_unregister",
     "pv_last_launch_info", "pv_kernel_timing", "pv_kernel_time_ms", "pv_kernel_times_ms", "pv_error_string", "pv_last_cuda_error",
 )
@@ -59,6 +59,11 @@ class Debug(C.Structure):
     ]
 
 
+class TrackCov(C.Structure):
+    """struct pv_track_cov (include/pv_finder.h): optional x-tx / y-ty covariance elements, DEVICE pointers."""
+    _fields_ = [("cov_xtx", C.c_void_p), ("cov_yty", C.c_void_p)]
+
+
 class PvError(RuntimeError):
     pass
 
@@ -80,7 +85,8 @@ def lib():
         find_args = [vp] * 9 + [vp, i32, i64, C.POINTER(Params)] + [vp] * 9 + [vp, C.c_size_t, vp]
         L.pv_find.argtypes = find_args
         L.pv_find_debug.argtypes = find_args + [C.POINTER(Debug)]
-        L.pv_track_ip.argtypes = [vp] * 9 + [vp, i32, i64, C.POINTER(Params)] + [vp] * 3 + [vp] * 3 + [vp]
+        L.pv_find_ext.argtypes = find_args + [C.POINTER(TrackCov), C.POINTER(Debug)]
+        L.pv_track_ip.argtypes = [vp] * 9 + [vp, i32, i64, C.POINTER(Params)] + [vp] * 3 + [vp] * 3 + [C.POINTER(TrackCov), vp]
         L.pv_host_ctx_create.argtypes = [C.POINTER(vp), i32, i64, C.POINTER(Params), i32]
         L.pv_host_ctx_destroy.argtypes = [vp]
         L.pv_find_host.argtypes = [vp] + [vp] * 9 + [vp, i32, C.POINTER(Params)] + [vp] * 9 + [i32]
@@ -166,6 +172,12 @@ class DeviceBatch:
         dev = self.device
         self.inp = {k: torch.from_numpy(np.ascontiguousarray(data[k], dtype=np.float32)).to(dev) for k in FIELDS}
         self.offsets = torch.from_numpy(off).to(dev)
+        self.cov = None                                    # optional covariance cross terms (Eq. 2)
+        if "cov_xtx" in data or "cov_yty" in data:
+            zero = np.zeros(self.T, np.float32)
+            self.cov_t = [torch.from_numpy(np.ascontiguousarray(data.get(k, zero), dtype=np.float32)).to(dev)
+                          for k in ("cov_xtx", "cov_yty")]
+            self.cov = TrackCov(self.cov_t[0].data_ptr(), self.cov_t[1].data_ptr())
         mv = p.max_vtx_per_event
         E, T = self.E, self.T
         z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev)
@@ -212,7 +224,10 @@ class DeviceBatch:
             o["vtx_niter"].data_ptr(), o["n_vtx"].data_ptr(), o["trk_weight"].data_ptr(), o["trk_vertex"].data_ptr(),
             o["event_status"].data_ptr(), self.workspace.data_ptr(), self.workspace.numel(), s.cuda_stream]
         with torch.cuda.device(self.device):
-            if self.dbg_struct is not None:
+            if self.cov is not None:
+                _check(L.pv_find_ext(*args, C.byref(self.cov), C.byref(self.dbg_struct) if self.dbg_struct is not None else None),
+                       "pv_find_ext")
+            elif self.dbg_struct is not None:
                 _check(L.pv_find_debug(*args, C.byref(self.dbg_struct)), "pv_find_debug")
             else:
                 _check(L.pv_find(*args), "pv_find")
@@ -228,7 +243,8 @@ class DeviceBatch:
         i, o = self.inp, self.out
         args = [i[k].data_ptr() for k in FIELDS] + [self.offsets.data_ptr(), self.E, self.T, C.byref(self.p)] + [
             o["vtx_pos"].data_ptr(), o["vtx_cov"].data_ptr(), o["n_vtx"].data_ptr(),
-            self.ip["ip"].data_ptr(), self.ip["ip_chi2"].data_ptr(), self.ip["ip_vertex"].data_ptr(), s.cuda_stream]
+            self.ip["ip"].data_ptr(), self.ip["ip_chi2"].data_ptr(), self.ip["ip_vertex"].data_ptr(),
+            C.byref(self.cov) if self.cov is not None else None, s.cuda_stream]
         with torch.cuda.device(self.device):
             _check(lib().pv_track_ip(*args), "pv_track_ip")
 

@@ -133,7 +133,8 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
               const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
               float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
               int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
-              void* workspace, size_t workspace_bytes, void* stream_, const pv_debug* dbg) {
+              void* workspace, size_t workspace_bytes, void* stream_, const pv_debug* dbg,
+              const pv_track_cov* cov = nullptr) {
   int nbins = 0;
   int rc = validate(params, &nbins);
   if (rc != PV_OK) return rc;
@@ -187,6 +188,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   memset(&ka, 0, sizeof(ka));
   ka.x = x; ka.y = y; ka.z = z; ka.tx = tx; ka.ty = ty;
   ka.var_x = var_x; ka.var_y = var_y; ka.var_tx = var_tx; ka.var_ty = var_ty;
+  if (cov) { ka.cov_xtx = cov->cov_xtx; ka.cov_yty = cov->cov_yty; }
   ka.offsets = offsets; ka.n_events = n_events;
   ka.vtx_pos = vtx_pos; ka.vtx_cov = vtx_cov; ka.vtx_chi2 = vtx_chi2;
   ka.vtx_ntracks = vtx_ntracks; ka.vtx_niter = vtx_niter; ka.n_vtx = n_vtx;
@@ -309,11 +311,22 @@ int pv_find_debug(const float* x, const float* y, const float* z, const float* t
                    workspace_bytes, stream, dbg ? dbg : &none);
 }
 
+int pv_find_ext(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
+                void* workspace, size_t workspace_bytes, void* stream, const pv_track_cov* cov, const pv_debug* dbg) {
+  return find_impl(x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, offsets, n_events, n_tracks, params, vtx_pos, vtx_cov,
+                   vtx_chi2, vtx_ntracks, vtx_niter, n_vtx, trk_weight, trk_vertex, event_status, workspace,
+                   workspace_bytes, stream, dbg, cov);
+}
+
 int pv_track_ip(const float* x, const float* y, const float* z, const float* tx, const float* ty,
                 const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
                 const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
                 const float* vtx_pos, const float* vtx_cov, const int32_t* n_vtx,
-                float* ip, float* ip_chi2, int32_t* ip_vertex, void* stream_) {
+                float* ip, float* ip_chi2, int32_t* ip_vertex, const pv_track_cov* cov, void* stream_) {
   int nbins = 0;
   const int rc = validate(params, &nbins);
   if (rc != PV_OK) return rc;
@@ -328,6 +341,7 @@ int pv_track_ip(const float* x, const float* y, const float* z, const float* tx,
   memset(&ka, 0, sizeof(ka));
   ka.x = x; ka.y = y; ka.z = z; ka.tx = tx; ka.ty = ty;
   ka.var_x = var_x; ka.var_y = var_y; ka.var_tx = var_tx; ka.var_ty = var_ty;
+  if (cov) { ka.cov_xtx = cov->cov_xtx; ka.cov_yty = cov->cov_yty; }
   ka.offsets = offsets; ka.n_events = n_events;
   pvk::ip_kernel<<<(n_events + 7) / 8, 256, 0, (cudaStream_t)stream_>>>(kp, ka, vtx_pos, vtx_cov, n_vtx, ip, ip_chi2, ip_vertex);
   CK(cudaGetLastError());

@@ -100,6 +100,7 @@ struct SeedRec {
 
 struct KArgs {
   const float *x, *y, *z, *tx, *ty, *var_x, *var_y, *var_tx, *var_ty;
+  const float *cov_xtx, *cov_yty;  // optional x-tx / y-ty covariance elements (Eq. 2), nullptr = diagonal covariance
   const int32_t* offsets;
   int n_events;
   float *vtx_pos, *vtx_cov, *vtx_chi2;
@@ -379,15 +380,18 @@ __device__ __forceinline__ bool track_is_dead(const Trk& T, const KParams& P) {
 
 struct RawTrk { float x, y, z, tx, ty, vx, vy, vtx, vty; };
 
-__device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, float sx, float sy, float zsv) {
+// Eq. 2 for one coordinate at dz = z - z_trk: V_xx + 2 dz V_xtx + dz^2 V_txtx
+__device__ __forceinline__ float var_at(float v, float vt, float c, float dz) { return fmaf(dz, fmaf(dz, vt, 2.0f * c), v); }
+
+// cx, cy: the track's V_xtx, V_yty (0 for a diagonal covariance)
+__device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, float cx, float cy, float sx, float sy, float zsv) {
   Trk T;
   const float zl = R.z - zsv;
   T.tx = R.tx; T.ty = R.ty;
   T.x0 = fmaf(-zl, R.tx, R.x - sx);
   T.y0 = fmaf(-zl, R.ty, R.y - sy);
-  const float dz2 = zl * zl;
-  const float Vx = fmaf(dz2, R.vtx, R.vx);
-  const float Vy = fmaf(dz2, R.vty, R.vy);
+  const float Vx = var_at(R.vx, R.vtx, cx, -zl);
+  const float Vy = var_at(R.vy, R.vty, cy, -zl);
   const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
   T.Wx = __fdividef(1.0f, Vx);
   T.Wy = __fdividef(1.0f, Vy);
@@ -702,11 +706,16 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       Q.vx = __ldg(A.var_x + g); Q.vy = __ldg(A.var_y + g); Q.vtx = __ldg(A.var_tx + g); Q.vty = __ldg(A.var_ty + g);
       return Q;
     };
-    auto chi2_at = [&](const RawTrk& R, const int k) -> float {   // Eq. 7 at seed k, W from Eq. 2; < 0 = unusable (R-7)
+    auto cross_of = [&](const int i, float& cx, float& cy) {   // V_xtx, V_yty of track i (0 = diagonal covariance)
+      const int g = t0 + min(i, n - 1);
+      cx = A.cov_xtx ? __ldg(A.cov_xtx + g) : 0.0f;
+      cy = A.cov_yty ? __ldg(A.cov_yty + g) : 0.0f;
+    };
+    auto chi2_at = [&](const RawTrk& R, const float cx, const float cy, const int k) -> float {   // Eq. 7 at seed k, W from Eq. 2; < 0 = unusable (R-7)
       const float zsv = zs[k];
       const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-      const float dzv = zsv - R.z, dz2 = dzv * dzv;
-      const float Vx = fmaf(dz2, R.vtx, R.vx), Vy = fmaf(dz2, R.vty, R.vy);
+      const float dzv = zsv - R.z;
+      const float Vx = var_at(R.vx, R.vtx, cx, dzv), Vy = var_at(R.vy, R.vty, cy, dzv);
       const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);
       const float rx = fmaf(dzv, R.tx, R.x) - sx, ry = fmaf(dzv, R.ty, R.y) - sy;
       const float c = fmaf(rx * rx, __fdividef(1.0f, Vx), ry * ry * __fdividef(1.0f, Vy));
@@ -715,9 +724,11 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     auto cand = [&](const int i, const RawTrk& R, unsigned& mask, float& den) {
       mask = 0u; den = P.mv_e0;
       const int b = i >= n ? -1 : (i < BINS_SM ? (int)binsm[i] : A.trk_vertex[t0 + i]);
+      float cx, cy;
+      cross_of(i, cx, cy);
 #pragma unroll 1
       for (int k = 0; k < ns; ++k) {
-        const float c = chi2_at(R, k);
+        const float c = chi2_at(R, cx, cy, k);
         if (b >= 0 && c >= 0.0f) {
           den += __expf(-0.5f * c);
           if (c < P.chi2_window) mask |= 1u << k;
@@ -767,13 +778,15 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     __syncwarp();
     auto emit = [&](const int i, const RawTrk& R, const unsigned mask, const float den) {
       if (i < n) A.best[t0 + i] = 0ull;
+      float cx, cy;
+      cross_of(i, cx, cy);
       for_bits(ovf ? 0u : mask, [&](int k, unsigned peers) {
         const int rank = __popc(peers & lanemask_lt());
         if (k >= 0) {
           const float zsv = zs[k];
           const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-          const Trk T = make_track(P, R, sx, sy, zsv);
-          const float oth = fmaxf(den - __expf(-0.5f * chi2_at(R, k)), 0.5f * P.mv_e0);
+          const Trk T = make_track(P, R, cx, cy, sx, sy, zsv);
+          const float oth = fmaxf(den - __expf(-0.5f * chi2_at(R, cx, cy, k)), 0.5f * P.mv_e0);
           float4* o = A.ftrk + 2 * (size_t)(cur[k] + rank);
           o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
           o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), oth);
@@ -910,7 +923,8 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       const float zsv = zs[s];
       const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
       const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-      const Trk T = make_track(P, Q, sx, sy, zsv);
+      const float cx = A.cov_xtx ? __ldg(A.cov_xtx + t0 + i) : 0.0f, cy = A.cov_yty ? __ldg(A.cov_yty + t0 + i) : 0.0f;
+      const Trk T = make_track(P, Q, cx, cy, sx, sy, zsv);
       float4* o = A.ftrk + 2 * (size_t)(t0 + cur[s] + rank);
       o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
       o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), 0.0f);
@@ -1480,10 +1494,11 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
   constexpr int U = 2;                                     // tracks per lane in flight: 18 loads before the first use
 #pragma unroll 1
   for (int i0 = lane; i0 < n; i0 += 32 * U) {
-    float x[U], y[U], z[U], a[U], b[U], vx[U], vy[U], vtx[U], vty[U];
+    float x[U], y[U], z[U], a[U], b[U], vx[U], vy[U], vtx[U], vty[U], cx[U], cy[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int g = t0 + min(i0 + 32 * u, n - 1);
+      cx[u] = A.cov_xtx ? __ldg(A.cov_xtx + g) : 0.0f; cy[u] = A.cov_yty ? __ldg(A.cov_yty + g) : 0.0f;
       x[u] = __ldg(A.x + g); y[u] = __ldg(A.y + g); z[u] = __ldg(A.z + g); a[u] = __ldg(A.tx + g); b[u] = __ldg(A.ty + g);
       vx[u] = __ldg(A.var_x + g); vy[u] = __ldg(A.var_y + g); vtx[u] = __ldg(A.var_tx + g); vty[u] = __ldg(A.var_ty + g);
     }
@@ -1493,7 +1508,7 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       best_c[u] = INFINITY; best_rx[u] = 0.0f; best_ry[u] = 0.0f; best_v[u] = -1;
-      usable[u] = (vx[u] > 0.0f || vtx[u] > 0.0f) && (vy[u] > 0.0f || vty[u] > 0.0f);   // cheap pre-test of R-7
+      usable[u] = true;
     }
 #pragma unroll 1
     for (int v = 0; v < nv; ++v) {
@@ -1501,8 +1516,8 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
       const float q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3], q4 = q[4], q5 = q[5], q6 = q[6], q7 = q[7], q8 = q[8];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
-        const float dz = q2 - z[u], dz2 = dz * dz;
-        const float Vx = fmaf(dz2, vtx[u], vx[u]), Vy = fmaf(dz2, vty[u], vy[u]);
+        const float dz = q2 - z[u];
+        const float Vx = var_at(vx[u], vtx[u], cx[u], dz), Vy = var_at(vy[u], vty[u], cy[u], dz);
         const float rx = fmaf(dz, a[u], x[u] - q0), ry = fmaf(dz, b[u], y[u] - q1);
         const float Sxx = fmaf(a[u], fmaf(a[u], q8, -2.0f * q5), Vx + q3);
         const float Syy = fmaf(b[u], fmaf(b[u], q8, -2.0f * q7), Vy + q6);

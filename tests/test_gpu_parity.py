@@ -344,6 +344,42 @@ def test_repeated_runs_are_bit_identical_on_high_pileup(pv, mode):
             assert np.array_equal(a, c, equal_nan=True), k
 
 
+@pytest.mark.parametrize("mv", [False, True])
+def test_covariance_cross_terms(pv, oracle, mv):
+    """NEXT-2: the x-tx / y-ty elements of Eq. 2 through pv_find_ext and pv_track_ip.  The track states of configs[1]
+    are re-expressed at a z up to 40 mm away (x' = x + L tx, V_xx' = V_xx + L^2 V_tt, V_xtx' = L V_tt), which makes
+    the cross terms essential; kernel vs oracle on the same inputs, both flavours, plus the IP consumer."""
+    from oracle import compare
+    d = events.generate(events.config(1, 2000))
+    rng = np.random.default_rng(12)
+    L = rng.uniform(-40, 40, d["x"].size)
+    t = {k: np.asarray(d[k], np.float64) for k in events.FIELDS}
+    m = dict(d)
+    m["x"] = (t["x"] + L * t["tx"]).astype(np.float32); m["y"] = (t["y"] + L * t["ty"]).astype(np.float32)
+    m["z"] = (t["z"] + L).astype(np.float32)
+    m["var_x"] = (t["var_x"] + L * L * t["var_tx"]).astype(np.float32); m["cov_xtx"] = (L * t["var_tx"]).astype(np.float32)
+    m["var_y"] = (t["var_y"] + L * L * t["var_ty"]).astype(np.float32); m["cov_yty"] = (L * t["var_ty"]).astype(np.float32)
+    p, po = (pv.multivertex_params(), oracle.mv_params()) if mv else (pv.default_params(), oracle.default_params())
+    b = pv.DeviceBatch(m, p, debug=True, n_hist_events=100)
+    b.find()
+    b.track_ip()
+    got, gip = b.results(), b.ip_results()
+    ref = oracle.find(m, po, debug=True, n_hist_events=100, trace=True, n_threads=8)
+    rep = compare.compare(got, ref, np.asarray(m["offsets"]), p)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep, allow_ties_frac=0.03)
+    assert rep["n_vertices"] > 5000
+    # without the cross terms the same inputs give clearly different covariances: the terms are exercised
+    nocov = pv.find({k: v for k, v in m.items() if not k.startswith("cov_")}, p)
+    k = np.arange(32)[None, :] < np.minimum(nocov["n_vtx"], got["n_vtx"])[:, None]
+    assert np.median(np.abs(nocov["vtx_cov"][k][:, 5] / got["vtx_cov"][k][:, 5] - 1)) > 0.2
+    rip = oracle.track_ip(m, got["vtx_pos"], got["vtx_cov"], got["n_vtx"])
+    same = gip["ip_vertex"] == rip["ip_vertex"]
+    assert same.mean() >= 0.999
+    ok = same & (rip["ip_vertex"] >= 0)
+    assert np.all(np.abs(gip["ip_chi2"][ok] - rip["ip_chi2"][ok]) <= 3e-3 * np.maximum(rip["ip_chi2"][ok], 1.0))
+
+
 def test_beamline_offset_robustness_scan(pv):
     """Synthetic version of the paper's Fig. 8: the finder is told a beamline that is off by d from the
     true one (x direction).  "an efficiency of 99 % within a beamline position uncertainty of 50 um ... 99.9 %
