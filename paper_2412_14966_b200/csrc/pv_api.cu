@@ -110,7 +110,7 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->max_vtx = p->max_vtx_per_event;
   const int r0 = ((nbins + 31) / 32) * 32 * 4;                // histogram padded to whole 32-bin words
   k->region0_words = r0 / 4;
-  k->warp_smem_bytes = r0 + pvk::SM_TAIL_BYTES;
+  k->team_smem_bytes = r0 + pvk::SM_TAIL_BYTES;
 }
 
 // Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | fit-ready track records,
@@ -155,14 +155,14 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
 
   pvk::KParams kp;
   make_kparams(params, nbins, &kp);
-  int warps = di->max_smem_optin / kp.warp_smem_bytes;        // teams (events in flight) per CTA
-  if (warps > pvk::MAX_TEAMS) warps = pvk::MAX_TEAMS;
+  int teams = di->max_smem_optin / kp.team_smem_bytes;        // teams (events in flight) per CTA
+  if (teams > pvk::MAX_TEAMS) teams = pvk::MAX_TEAMS;
   if (const char* envw = getenv("PV_TEAMS_PER_CTA")) {
     const int w = atoi(envw);
-    if (w >= 1 && w < warps) warps = w;
+    if (w >= 1 && w < teams) teams = w;
   }
-  if (warps < 1) return PV_E_PARAM;
-  const int smem = warps * kp.warp_smem_bytes;
+  if (teams < 1) return PV_E_PARAM;
+  const int smem = teams * kp.team_smem_bytes;
   const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
   const int spl = params->split_mode == PV_SPLIT_RECURSIVE ? 1 : 0;
   const int which = (dbg ? 1 : 0) + 2 * mvf + 4 * spl;
@@ -182,7 +182,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     else CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel<0>, pvk::FIT_BLOCK, 0));
     di->fit_blocks_per_sm[mvf] = nb > 0 ? nb : 1;
   }
-  g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * pvk::TEAM; g_last_smem = smem;
+  g_last_kernels = 0; g_last_grid = 0; g_last_block = teams * pvk::TEAM; g_last_smem = smem;
 
   pvk::KArgs ka;
   memset(&ka, 0, sizeof(ka));
@@ -207,18 +207,18 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
   CK(cudaMemsetAsync(workspace, 0, 48, stream));
-  // a1..a4: persistent, one CTA per SM, one team of two warps per event
+  // a1..a4: persistent, one CTA per SM, one team of two teams per event
   int grid = di->sms;
-  const int need = (n_events + warps - 1) / warps;
+  const int need = (n_events + teams - 1) / teams;
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
   {
     void* kargs[2] = {(void*)&kp, (void*)&ka};
-    CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(warps * pvk::TEAM), kargs, (size_t)smem, stream));
+    CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(teams * pvk::TEAM), kargs, (size_t)smem, stream));
   }
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
-  // a5: FIT_G lanes per seed, warps stride over windows of 32 seed records
+  // a5: FIT_G lanes per seed, teams stride over windows of 32 seed records
   {
     long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm[mvf];
     const long long most = ((long long)n_events * params->max_vtx_per_event + pvk::FIT_BLOCK - 1) / pvk::FIT_BLOCK;

@@ -87,7 +87,7 @@ struct KParams {
   float chi2_window;             // multi-vertex flavour: list a track for a seed iff chi2 at the seed position < this
   float mv_e0;                   // exp(-chi2_max / 2), the constant of the denominator of Eq. 19
   int region0_words;             // int32 words of the histogram region (multiple of 32)
-  int warp_smem_bytes;
+  int team_smem_bytes;
 };
 
 // One vertex seed handed from seed_kernel to fit_kernel (16 bytes, read as one int4).
@@ -975,7 +975,7 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int team = threadIdx.x / TEAM, tt = threadIdx.x % TEAM;
   const int bar = 1 + team;                                // named barrier of the team (0 is __syncthreads)
-  unsigned char* wsm = smem_raw + (size_t)team * P.warp_smem_bytes;
+  unsigned char* wsm = smem_raw + (size_t)team * P.team_smem_bytes;
   int* misc = reinterpret_cast<int*>(wsm + (size_t)P.region0_words * 4 + SM_MISC);
   {
     int4* Z = reinterpret_cast<int4*>(wsm);                // histogram and touched-word flags start at zero
