@@ -4,7 +4,7 @@
 //
 //   seed_kernel     a1..a4  one TEAM of two warps per event, persistent grid, 13 teams per CTA, one int32
 //                           shared-memory histogram and one named barrier per team.  POCA projection (fp32 contract,
-//                           bit-exact with the CPU oracle), flat list of 8-bin fill units (nine independent CDF edges
+//                           bit-exact with the CPU oracle), flat list of 6-bin fill units (seven independent CDF edges
 //                           per thread), touched-word flags, one ballot per touched word for the proto-cluster starts,
 //                           one lane per proto-cluster for the z-ordered hysteresis sweep, seed positions,
 //                           association (explicit with the removal loop, or the multi-vertex chi2 window),
@@ -38,7 +38,10 @@ constexpr int TEAM = 32 * TEAM_WARPS;
 constexpr int MAX_TEAMS = 14;       // events in flight per CTA (named barriers 1..14; 14 histograms fill 227 KB)
 constexpr int CHUNK = 128;          // tracks per fill chunk
 constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
-constexpr int UNIT = 8;             // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
+#ifndef PV_UNIT
+#define PV_UNIT 6
+#endif
+constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int FIT_G = 2;            // lanes per vertex in the fit
@@ -1347,8 +1350,11 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
 // Lane k holds seed k of the event (position, covariance, ... as fit_kernel left them in slot k of the vertex
 // arrays), the duplicate sweep runs on shuffles, survivors are compacted in place in z order, and every
 // track gets its final vertex index (weight 0 when it has none).
+#ifndef PV_CLEANUP_MIN_BLOCKS
+#define PV_CLEANUP_MIN_BLOCKS 8
+#endif
 template <bool DBG, int FLAV>
-__global__ void __launch_bounds__(256) cleanup_kernel(const __grid_constant__ KParams P,
+__global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(const __grid_constant__ KParams P,
                                                       const __grid_constant__ KArgs A) {
   const int lane = threadIdx.x & 31;
   const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
