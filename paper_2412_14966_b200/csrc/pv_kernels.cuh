@@ -38,12 +38,16 @@ constexpr int TEAM = 32 * TEAM_WARPS;
 constexpr int MAX_TEAMS = 14;       // events in flight per CTA (named barriers 1..14; 14 histograms fill 227 KB)
 constexpr int CHUNK = 128;          // tracks per fill chunk
 constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
+#ifndef PV_FIT_UNROLL
+#define PV_FIT_UNROLL 4
+#endif
 #ifndef PV_UNIT
 #define PV_UNIT 6
 #endif
 constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
+constexpr int FIT_UNROLL = PV_FIT_UNROLL;   // unroll of the track loop of one fit iteration
 constexpr int FIT_G = 2;            // lanes per vertex in the fit
 constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
 constexpr int FIT_KF = 16;          // track slots per lane in shared memory (fast path: <= FIT_G*FIT_KF tracks)
@@ -1228,7 +1232,7 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
       for (int it = 1; it <= P.max_iter; ++it) {
         Sums S;
         sums_zero(S);
-#pragma unroll 4
+#pragma unroll FIT_UNROLL
         for (int s = 0; s < nslot; ++s) {
           const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
           track_accum<FLAV>(T, ax, ay, az, P, S);
