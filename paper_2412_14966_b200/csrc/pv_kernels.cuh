@@ -1140,13 +1140,8 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
   const int total = (int)*A.seed_counter;
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
   const int wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  // the records of the NEXT window are loaded one window ahead and their track lines prefetched into L2
-  auto prefetch_l2 = [&](int begin, int m) {
-    const char* base = reinterpret_cast<const char*>(A.ftrk + 2 * (size_t)begin);
-    const int bytes = m * 32;
-    for (int off = 0; off < bytes; off += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
-    if (bytes > 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + bytes - 1));   // records are not line aligned
-  };
+  // the seed records of the NEXT window are loaded one window ahead (an L2 prefetch of their track lines was
+  // measured slower: 0.408 vs 0.396 ms, and cost 270 MB of DRAM reads evicted before use)
   int4 wr_next = make_int4(0, 0, 0, 0);
   if (wg * 32 + lane < total) wr_next = __ldg(reinterpret_cast<const int4*>(A.rec) + wg * 32 + lane);
 #pragma unroll 1
@@ -1211,7 +1206,6 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
       }
-      if (pass + 1 == 32 / FIT_VPW) prefetch_l2(wr_next.z, min(wr_next.y >> 5, 2 * FIT_G * FIT_KF));
       asm volatile("cp.async.wait_group 0;" ::: "memory");
       __syncwarp();
       float nvalid = 0.0f;                                   // usable tracks (unit-weight mode: the active count)
