@@ -1058,7 +1058,7 @@ __device__ __forceinline__ float track_accum(const Trk& T, float ax, float ay, f
   S.gy = fmaf(wWy, ry, S.gy);
   S.gz = fmaf(p, rx, fmaf(q, ry, S.gz));
   S.chi2 = fmaf(w, chi, S.chi2);
-  S.nact += (w > 0.0f) ? 1.0f : 0.0f;
+  S.nact += __saturatef(w * 1e38f);                    // 1 for w > 0 (a positive weight is >= 3.5e-15 here), else 0
   return w;
 }
 
