@@ -139,6 +139,8 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   int rc = validate(params, &nbins);
   if (rc != PV_OK) return rc;
   if (n_events < 0 || n_tracks < 0 || n_tracks > 0x7fffffffLL) return PV_E_SIZE;
+  // multi-vertex flavour: two track records per track, indexed with 32 bits
+  if (params->flavour == PV_FLAVOUR_MULTIVERTEX && n_tracks > 0x3fffffffLL) return PV_E_SIZE;
   if (n_events == 0) { g_last_kernels = 0; g_last_grid = 0; return PV_OK; }   // empty batch: nothing to enqueue
   if (!offsets || !n_vtx || !event_status || !vtx_pos || !vtx_cov || !vtx_chi2 || !vtx_ntracks || !vtx_niter || !workspace)
     return PV_E_NULL;

@@ -156,6 +156,18 @@ def test_batch_sweep_config4(pv, oracle, n):
     assert rep["assign_agreement"] >= 0.999
 
 
+def test_batch_of_empty_events(pv):
+    """Events but no tracks at all (null track pointers), both flavours and the IP consumer."""
+    data = events.from_lists([{k: np.zeros(0, np.float32) for k in events.FIELDS}] * 5)
+    for p in (pv.default_params(), pv.multivertex_params()):
+        b = pv.DeviceBatch(data, p)
+        b.find()
+        b.track_ip()
+        r = b.results()
+        assert r["n_vtx"].tolist() == [0] * 5 and r["event_status"].tolist() == [0] * 5
+        assert b.ip_results()["ip"].size == 0
+
+
 def test_too_many_tracks_and_vertex_overflow(pv, oracle):
     """An event above PV_MAX_TRACKS_PER_EVENT is skipped with its flag; max_vtx_per_event smaller than the
     number of seeds keeps the first ones in z and flags the event."""
