@@ -201,7 +201,9 @@ int pv_find_ext(const float* x, const float* y, const float* z, const float* tx,
  * streams sized for at most max_events / max_tracks; pv_find_host() takes HOST pointers everywhere
  * (same meaning and layout as pv_find), splits the batch into n_chunks contiguous event ranges, and
  * for each enqueues H2D copies -> pv_find -> D2H copies on one of the context's streams.  It returns
- * after all results are in the caller's host arrays (it synchronises its own streams only). */
+ * after all results are in the caller's host arrays (it synchronises its own streams only).  Both flavours and
+ * both splitting variants are supported (the context is sized for the flavour given at creation); the covariance
+ * cross terms of pv_find_ext are not part of this entry. */
 typedef struct pv_host_ctx pv_host_ctx;
 int pv_host_ctx_create(pv_host_ctx** ctx, int max_events, long long max_tracks, const pv_params* params,
                        int n_streams);

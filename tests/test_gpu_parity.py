@@ -449,9 +449,10 @@ def test_full_size_throughput_config(pv, oracle):
     assert np.quantile(d, 0.99) < 1e-4
 
 
-def test_host_pipeline_matches_device_path(pv, cfg0):
-    """pv_find_host (HOST buffers, chunked over streams) returns exactly what pv_find returns."""
-    p = pv.default_params()
+@pytest.mark.parametrize("mode", ["explicit", "multivertex"])
+def test_host_pipeline_matches_device_path(pv, cfg0, mode):
+    """pv_find_host (HOST buffers, chunked over streams) returns exactly what pv_find returns, in both flavours."""
+    p = pv.default_params() if mode == "explicit" else pv.multivertex_params()
     a = pv.find(cfg0, p)
     E, T = cfg0["offsets"].size - 1, int(cfg0["offsets"][-1])
     hp = pv.HostPipeline(E, T, p, n_streams=3)
