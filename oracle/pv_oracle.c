@@ -334,11 +334,15 @@ int pvo_assign(int n, const int32_t *bin, const int32_t *flags, int n_seeds,
 
 /* ===================================== O7 : adaptive vertex fit ====================================== */
 /* Plain dense Cholesky of a symmetric 3x3, A = L L^T.  Returns -1 if a pivot is <= 0. */
-static int chol3(const double A[3][3], double L[3][3]) {
+static int chol3(const double A[3][3], double L[3][3], double *min_rel_pivot) {
   memset(L, 0, sizeof(double) * 9);
   for (int j = 0; j < 3; ++j) {
     double d = A[j][j];
     for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
+    if (min_rel_pivot) {                              /* diagnostic only: how close the pivot is to its cut (0) */
+      double rel = A[j][j] > 0.0 ? d / A[j][j] : 0.0;
+      if (rel < *min_rel_pivot) *min_rel_pivot = rel;
+    }
     if (!(d > 0.0)) return -1;
     L[j][j] = sqrt(d);
     for (int i = j + 1; i < 3; ++i) {
@@ -386,16 +390,27 @@ static double pvo_mv_weight_den(double chi2_own, double other) {
   return E / (other + E);
 }
 
+/* Diagnostics of one fit for the comparator's near-tie rules (tests only; no output depends on them). */
+typedef struct fit_diag {
+  double edge_last, edge_any;   /* closest track to the active / associated cut: last iteration, any iteration */
+  double pivot_min;             /* smallest Cholesky pivot relative to its diagonal element, over the iterations */
+  int nact_min;                 /* fewest active tracks in an iteration */
+} fit_diag;
+
 /* One Newton-Raphson iteration (Eq. 6-17) at the vertex position a[]: fills the Tukey weights w[] (Eq. 18),
  * the step (Eq. 13), C (Eq. 14), dchi2 (Eq. 17), chi2 (Eq. 6) and the number of tracks with w > 0.
  * Returns -1 when fewer than 2 tracks are active or the Hessian is not positive definite. */
 static int fit_iteration(int m, const int32_t *idx,
                          const float *x, const float *y, const float *z, const float *tx, const float *ty,
                          const double *Wx, const double *Wy, const double a[3], double chi2_max, const double *other,
-                         double *w, double step[3], double C[3][3], double *dchi2_o, double *chi2_o, int *nact_o) {
+                         double *w, double step[3], double C[3][3], double *dchi2_o, double *chi2_o, int *nact_o,
+                         double *edge_o, double *pivot_o) {
   double A[3][3] = {{0}}, g[3] = {0, 0, 0};
   double chi2 = 0.0;
   int nact = 0;
+  double edge = INFINITY;                             /* diagnostic only (comparator near-tie rules): distance of the
+                                                         closest track to the cut that decides "active" / "associated":
+                                                         |chi2_i / chi2_max - 1| (Eq. 18) or |w_i - 1/2| (Eq. 19, R-13) */
   for (int j = 0; j < m; ++j) {
     int i = idx[j];
     double wi = 0.0;
@@ -407,6 +422,10 @@ static int fit_iteration(int m, const int32_t *idx,
       if (other) wi = pvo_mv_weight_den(chi2_i, other[j]);          /* Eq. 19, competitors at their seed positions */
       else if (isinf(chi2_max)) wi = 1.0;
       else if (chi2_i < chi2_max) { double u = 1.0 - chi2_i / chi2_max; wi = u * u; }  /* Eq. 18 */
+      {
+        double d = other ? fabs(wi - 0.5) : (isinf(chi2_max) ? INFINITY : fabs(chi2_i / chi2_max - 1.0));
+        if (d < edge) edge = d;
+      }
       /* H_i = [[-1,0,tx],[0,-1,ty]] (Eq. 12); accumulate w H^T W H (Eq. 11 / 2) and w H^T W r (Eq. 10 / 2) */
       double Hm[2][3] = {{-1.0, 0.0, (double)tx[i]}, {0.0, -1.0, (double)ty[i]}};
       double Wd[2] = {Wx[j], Wy[j]}, r[2] = {rx, ry};
@@ -421,9 +440,10 @@ static int fit_iteration(int m, const int32_t *idx,
     if (wi > 0.0) ++nact;
   }
   *chi2_o = chi2; *nact_o = nact;
+  if (edge_o) *edge_o = edge;
   if (nact < 2) return -1;
   double L[3][3];
-  if (chol3(A, L) != 0) return -1;
+  if (chol3(A, L, pivot_o) != 0) return -1;
   /* Newton-Raphson step Eq. 13: alpha1 = alpha0 - (d2chi2)^-1 dchi2 = alpha0 - A^-1 g */
   double mg[3] = {-g[0], -g[1], -g[2]};
   chol3_solve(L, mg, step);
@@ -451,8 +471,9 @@ static int fit_core(int m, const int32_t *idx,
                     const float *var_x, const float *var_y, const float *var_tx, const float *var_ty,
                     const double seed[3], const pvo_params *p, const double *other, const pvo_cross *cx,
                     double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
-                    double *w, double *trace) {
+                    double *w, double *trace, fit_diag *diag) {
   double a[3] = {seed[0], seed[1], seed[2]};
+  if (diag) { diag->edge_last = INFINITY; diag->edge_any = INFINITY; diag->pivot_min = INFINITY; diag->nact_min = 0x7fffffff; }
   double *Wx = (double *)malloc(sizeof(double) * (size_t)(2 * m + 2));
   double *Wy = Wx + m + 1;
   /* V_i = Eq. 2 at dz = z_seed - z_trk, diagonal input covariance; "evaluated and inverted
@@ -471,7 +492,15 @@ static int fit_core(int m, const int32_t *idx,
   double C[3][3] = {{0}}, chi2 = 0.0;
   for (int it = 1; it <= p->max_iter; ++it) {
     double step[3], dchi2;
-    if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, a, chi2_max, other, w, step, C, &dchi2, &chi2, &nact) != 0) { rc = -1; break; }
+    double edge = INFINITY, pivot = INFINITY;
+    int frc = fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, a, chi2_max, other, w, step, C, &dchi2, &chi2, &nact, &edge, &pivot);
+    if (diag) {
+      diag->edge_last = edge;
+      if (edge < diag->edge_any) diag->edge_any = edge;
+      if (pivot < diag->pivot_min) diag->pivot_min = pivot;
+      if (nact < diag->nact_min) diag->nact_min = nact;
+    }
+    if (frc != 0) { rc = -1; break; }
     for (int k = 0; k < 3; ++k) a[k] += step[k];
     niter = it; rc = 0;
     if (trace && it <= PVO_TRACE_ITERS) trace_row(trace, it, a, C, dchi2, step[2]);
@@ -486,7 +515,7 @@ static int fit_core(int m, const int32_t *idx,
     int nactt;
     double *wt = (double *)malloc(sizeof(double) * (size_t)(m + 1));
     for (int it = niter + 1; it <= p->max_iter && it <= PVO_TRACE_ITERS; ++it) {
-      if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, at, chi2_max, other, wt, stept, Ct, &dchi2t, &chi2t, &nactt) != 0) break;
+      if (fit_iteration(m, idx, x, y, z, tx, ty, Wx, Wy, at, chi2_max, other, wt, stept, Ct, &dchi2t, &chi2t, &nactt, NULL, NULL) != 0) break;
       for (int k = 0; k < 3; ++k) at[k] += stept[k];
       trace_row(trace, it, at, Ct, dchi2t, stept[2]);
     }
@@ -513,7 +542,7 @@ int pvo_fit(int m, const int32_t *idx,
             double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
             double *w, double *trace) {
   return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, NULL, cx, out_pos, out_cov, out_chi2,
-                  out_ntrk, out_niter, w, trace);
+                  out_ntrk, out_niter, w, trace, NULL);
 }
 
 /* Multi-vertex flavour: the same Newton-Raphson fit with the weights of Eq. 19.  other[j] is, for
@@ -527,7 +556,7 @@ int pvo_fit_mv(int m, const int32_t *idx,
                double *out_pos, double *out_cov, double *out_chi2, int32_t *out_ntrk, int32_t *out_niter,
                double *w, double *trace) {
   return fit_core(m, idx, x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, seed, p, other, cx, out_pos, out_cov, out_chi2,
-                  out_ntrk, out_niter, w, trace);
+                  out_ntrk, out_niter, w, trace, NULL);
 }
 
 /* chi2 of track i relative to a vertex candidate at pos[] "evaluated as in Eq. 7" with W from Eq. 2 at that
@@ -601,7 +630,7 @@ typedef struct scratch {
   int32_t *H, *bin, *flags, *trk_seed, *cb, *ce, *cp, *idx, *s_ntrk, *s_niter, *fate;
   float *zp, *sp, *zs;
   double *s_pos, *s_cov, *s_chi2, *w, *trace;
-  double *Em, *other, *best_w;         /* multi-vertex flavour: exp(-chi2_ik / 2) at the seed positions [n][max_vtx] */
+  double *Em, *other, *best_w, *second_w;  /* multi-vertex flavour: exp(-chi2_ik / 2) at the seed positions [n][max_vtx] */
 } scratch;
 
 static scratch *scratch_new(const pvo_params *p) {
@@ -619,8 +648,8 @@ static scratch *scratch_new(const pvo_params *p) {
   s->s_cov = s->s_pos + 3 * mv; s->s_chi2 = s->s_cov + 6 * mv;
   s->w = (double *)malloc(sizeof(double) * (size_t)nt);
   s->trace = (double *)malloc(sizeof(double) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE);
-  s->Em = (double *)malloc(sizeof(double) * ((size_t)nt * (size_t)mv + 2 * (size_t)nt));
-  s->other = s->Em + (size_t)nt * (size_t)mv; s->best_w = s->other + nt;
+  s->Em = (double *)malloc(sizeof(double) * ((size_t)nt * (size_t)mv + 3 * (size_t)nt));
+  s->other = s->Em + (size_t)nt * (size_t)mv; s->best_w = s->other + nt; s->second_w = s->best_w + nt;
   return s;
 }
 
@@ -690,7 +719,7 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
     /* R-13/R-14: every assignable track is implicitly associated to every vertex candidate; E_ik =
      * exp(-chi2_ik / 2) with chi2_ik "evaluated as in Eq. 7" at the candidates' initial (seed) positions */
     for (int i = 0; i < n; ++i) {
-      S->best_w[i] = 0.0;
+      S->best_w[i] = 0.0; S->second_w[i] = 0.0;
       for (int k = 0; k < ns; ++k) {
         float zs = S->zs[k];
         double pos[3] = {(double)fmaf(p->beam_tx, zs, p->beam_x), (double)fmaf(p->beam_ty, zs, p->beam_y), (double)zs};
@@ -724,15 +753,24 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
     double seed[3] = {(double)fmaf(p->beam_tx, zs, p->beam_x), (double)fmaf(p->beam_ty, zs, p->beam_y), (double)zs};
     double chi2 = 0.0;
     memset(S->trace, 0, sizeof(double) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE);
+    fit_diag diag;
     int rc = fit_core(m, S->idx, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, var_y + t0, var_tx + t0,
                       var_ty + t0, seed, p, mvf ? S->other : NULL, cx, S->s_pos + 3 * k, S->s_cov + 6 * k, &chi2,
-                      &S->s_ntrk[k], &S->s_niter[k], S->w, S->trace);
+                      &S->s_ntrk[k], &S->s_niter[k], S->w, S->trace, &diag);
     S->s_chi2[k] = chi2;
+    if (dbg) {
+      size_t o = (size_t)e * mv + k;
+      if (dbg->seed_edge_last) dbg->seed_edge_last[o] = diag.edge_last;
+      if (dbg->seed_edge_any) dbg->seed_edge_any[o] = diag.edge_any;
+      if (dbg->seed_pivot_min) dbg->seed_pivot_min[o] = diag.pivot_min;
+      if (dbg->seed_nact_min) dbg->seed_nact_min[o] = diag.nact_min;
+    }
     if (rc != 0) { status |= PVO_EVT_SINGULAR_FIT; S->s_niter[k] = -1; }
     else if (!mvf) for (int j = 0; j < m; ++j) trk_weight[t0 + S->idx[j]] = S->w[j];
     else for (int j = 0; j < m; ++j) {                 /* R-13: a track follows the candidate with its largest weight */
       int i = S->idx[j];
-      if (S->w[j] > S->best_w[i]) { S->best_w[i] = S->w[j]; S->trk_seed[i] = k; }
+      if (S->w[j] > S->best_w[i]) { S->second_w[i] = S->best_w[i]; S->best_w[i] = S->w[j]; S->trk_seed[i] = k; }
+      else if (S->w[j] > S->second_w[i]) S->second_w[i] = S->w[j];     /* diagnostic only: the runner-up weight */
     }
     if (dbg && dbg->trace)
       memcpy(dbg->trace + ((size_t)e * mv + k) * PVO_TRACE_ITERS * PVO_TRACE_STRIDE, S->trace,
@@ -741,6 +779,7 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
   if (mvf) {
     for (int i = 0; i < n; ++i) trk_weight[t0 + i] = S->trk_seed[i] >= 0 ? S->best_w[i] : 0.0;
     if (dbg && dbg->trk_seed) for (int i = 0; i < n; ++i) dbg->trk_seed[t0 + i] = S->trk_seed[i];
+    if (dbg && dbg->trk_w2) for (int i = 0; i < n; ++i) dbg->trk_w2[t0 + i] = S->second_w[i];
   }
 
   /* cleanup O8.  Duplicate removal: greedy sweep in seed (= z) order; duplicate iff

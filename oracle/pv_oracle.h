@@ -139,6 +139,13 @@ typedef struct pvo_debug {
   int32_t *seed_niter;  /* [E][max_vtx]; -1 = singular */
   int32_t *seed_fate;   /* [E][max_vtx]; final vertex index, or -1 singular, -2 merged, -3 min tracks, -4 beam dist */
   double *trace;        /* [E][max_vtx][PVO_TRACE_ITERS][PVO_TRACE_STRIDE], indexed by seed */
+  /* diagnostics for the comparator's near-tie rules (no output depends on them) */
+  double *seed_edge_last; /* [E][max_vtx] min over the seed's tracks of |chi2_i / chi2_max - 1| (flavour 0) or |w_i - 1/2|
+                             (flavour 1) in the last iteration: how close n_trk is to counting one track more or less */
+  double *seed_edge_any;  /* [E][max_vtx] the same, min over all iterations (decides the < 2 active tracks test) */
+  double *seed_pivot_min; /* [E][max_vtx] smallest Cholesky pivot / diagonal element over the iterations (<= 0: singular) */
+  int32_t *seed_nact_min; /* [E][max_vtx] fewest active tracks in an iteration */
+  double *trk_w2;         /* [T] flavour 1: the second largest final weight of the track over the fitted candidates */
 } pvo_debug;
 
 /* The whole hot path a1..a6 over a batch.  Outputs (host, caller-owned):
