@@ -5,8 +5,13 @@
 
 A step is one pass of the whole hot path (a1..a6, one pv_find call = three kernel launches: seed, fit, cleanup)
 over one batch of synthetic events: configs[1] of BASELINE.json (100 000 events, mu = 5 pp + SMOG2, seed 2), resident in HBM.
-Rank 0 prints ONE JSON line.  Under torchrun (N > 1) every rank processes its own batch of the same model
-(different generator blocks), no data-path collective: events are independent -> "scaling": "weak".
+Rank 0 prints ONE JSON line.
+
+N > 1: ONE batch of N x E events of the same model is cut by paper_2412_14966_b200.shard.event_range into N
+contiguous event ranges of equal track count; rank r keeps range r resident and runs pv_find on it.
+No data-path collective: events are independent -> "scaling": "weak" (E events per GPU).  Started either by
+the driver's torchrun line or plainly as `python bench.py --gpus N`, which re-executes itself under
+torch.distributed.run (one rank per GPU) and fails loudly when the box has fewer than N CUDA devices.
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on the box's host cores instead.
 """
@@ -75,14 +80,45 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def gen_batch(cfg_idx: int, n_events, rank: int):
-    """configs[cfg_idx]; rank r > 0 takes different generator blocks of the same model (distinct events)."""
+def gen_batch(cfg_idx: int, n_events, rank: int = 0, world: int = 1, gather_counts=None):
+    """This rank's share of ONE batch of world x E events of configs[cfg_idx] (E = n_events or the config's own size):
+    the contiguous event range shard.event_range gives it (equal track counts).  Every rank draws
+    only the generator blocks it needs: first its nominal range [rank E, (rank + 1) E) for the per-event track
+    counts, which `gather_counts` (an all_gather of E int64 per rank: control plane, not data path) turns into the
+    global offsets; then the blocks of its actual range (its neighbours' edge blocks at most).
+    Returns (batch, model, (e0, e1), global track count)."""
     from synth import events
+    from paper_2412_14966_b200 import shard
     import dataclasses
     m = events.config(cfg_idx, n_events)
-    if rank > 0:
-        m = dataclasses.replace(m, seed=m.seed + 1000 * rank)
-    return events.generate(m), m
+    E = m.n_events
+    if world == 1:
+        d = events.generate(m)
+        return d, m, (0, E), int(d["offsets"][-1])
+    big = dataclasses.replace(m, n_events=world * E)
+    cache = {}
+    nominal = events.generate_range(big, rank * E, (rank + 1) * E, cache)
+    counts = gather_counts(np.diff(nominal["offsets"]).astype(np.int64))          # [world * E]
+    off = np.concatenate([[0], np.cumsum(counts)])
+    e0, e1 = shard.event_range(off, rank, world)
+    return events.generate_range(big, e0, e1, cache), big, (e0, e1), int(off[-1])
+
+
+def spawn_command(n_gpus: int, argv, port: int):
+    """The command `python bench.py --gpus N ...` re-executes itself with when it was not started by torchrun."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def kernels_sha() -> str:
+    """git blob hashes of the two CUDA sources, joined: recorded beside every ncu DRAM-traffic capture in
+    profiles/dram_traffic.csv so that a capture made with other kernels is recognised as stale."""
+    import hashlib
+    out = []
+    for f in ("pv_kernels.cuh", "pv_api.cu"):
+        b = open(os.path.join(ROOT, "paper_2412_14966_b200", "csrc", f), "rb").read()
+        out.append(hashlib.sha1(b"blob %d\0" % len(b) + b).hexdigest()[:12])
+    return "+".join(out)
 
 
 KERNELS = ("seed_kernel", "fit_kernel", "cleanup_kernel")
@@ -117,14 +153,15 @@ def run_oracle(data, n_threads: int, flavour: str = "explicit"):
 
 
 def main_reference(args):
-    """The reference arm of this tier is the oracle, as it stands, on the host cores (rank 0 only)."""
+    """The reference arm of this tier is the oracle, as it stands, on the host cores (rank 0 only; it uses no GPU,
+    so n_gpus is 1 whatever --gpus says)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from synth import events
     cores = os.cpu_count() or 1
     sample_events = min(args.events or 100_000, 20_000)
-    data, m = gen_batch(args.config, sample_events, 0)
+    data, m, _rng, _T = gen_batch(args.config, sample_events)
     for _ in range(args.warmup):
         run_oracle(events.slice_events(data, 0, min(2000, sample_events)), cores, args.flavour)
     t = 0.0
@@ -133,7 +170,7 @@ def main_reference(args):
         t += dt
     value = sample_events * args.steps / t
     sample = f"first {sample_events} events of configs[{args.config}] ({m.name}, seed {m.seed}) per step, OpenMP over events"
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (fp32 contract for the integer decisions)", "data": "synthetic",
             "config": {"workload": f"configs[{args.config}] {m.name}: bounded sample of {sample_events} events per step",
@@ -144,6 +181,9 @@ def main_reference(args):
     print(json.dumps(line), flush=True)
 
 
+L2_BYTES = 126 * 1024 * 1024
+
+
 def main_ours(args):
     import torch
     import torch.distributed as dist
@@ -152,22 +192,40 @@ def main_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the PV finder has no CPU fallback)")
+    if torch.cuda.device_count() <= local_rank:
+        raise SystemExit(f"bench.py: rank {rank} needs CUDA device {local_rank}, the box has {torch.cuda.device_count()}")
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")                 # the init log names every rank and its device
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
     from paper_2412_14966_b200 import build as pvbuild
     pvbuild.build()
     import paper_2412_14966_b200 as pv
 
-    data, m = gen_batch(args.config, args.events, rank)
+    def gather_counts(c):
+        t = torch.from_numpy(c).to(dev)
+        out = torch.empty(world * t.numel(), dtype=t.dtype, device=dev)
+        dist.all_gather_into_tensor(out, t)
+        return out.cpu().numpy()
+
+    data, m, (ge0, ge1), T_global = gen_batch(args.config, args.events, rank, world, gather_counts)
     E, T = int(data["offsets"].size - 1), int(data["offsets"][-1])
+    E_global = m.n_events
     p = pv.multivertex_params() if args.flavour == "multivertex" else pv.default_params()
+    if args.split == "recursive":
+        p.split_mode = 1
+    if args.fill == "template":
+        p.fill_mode = 1
     batch = pv.DeviceBatch(data, p, device=dev)
     stream = torch.cuda.Stream(device=dev)
     L = pv.lib()
+    # inputs smaller than twice the L2 would be served from it on the second step: write a buffer larger than the
+    # L2 between the timed steps (outside the per-step event pairs)
+    flush = T * 36 < 2 * L2_BYTES
+    fbuf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if flush else None
 
     def barrier():
         if world > 1:
@@ -180,25 +238,40 @@ def main_ours(args):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    L.pv_kernel_timing(1)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    with torch.cuda.stream(stream):
-        ev0.record(stream)
-        for _ in range(args.steps):
-            batch.find(stream)
-        ev1.record(stream)
-    barrier()
+    if not flush:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            ev0.record(stream)
+            for _ in range(args.steps):
+                batch.find(stream)
+            ev1.record(stream)
+        barrier()
+        ms_total = ev0.elapsed_time(ev1)
+    else:
+        pairs = []
+        with torch.cuda.stream(stream):
+            for _ in range(args.steps):
+                fbuf.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                batch.find(stream)
+                b.record(stream)
+                pairs.append((a, b))
+        barrier()
+        ms_total = sum(a.elapsed_time(b) for a, b in pairs)
     sampler.sample()
     sampler.stop()
-    ms_total = ev0.elapsed_time(ev1)
     # per-kernel durations: CUDA events recorded by the library on the launching stream around each of the
     # three launches, read back after every step of a second pass over the same K steps (not part of `value`)
     import ctypes
+    L.pv_kernel_timing(1)
     kt = np.zeros((args.steps, len(KERNELS)))
     buf = (ctypes.c_float * len(KERNELS))()
     for i in range(args.steps):
         with torch.cuda.stream(stream):
+            if flush:
+                fbuf.zero_()
             batch.find(stream)
         stream.synchronize()
         L.pv_kernel_times_ms(buf, len(KERNELS))
@@ -232,7 +305,7 @@ def main_ours(args):
                    "achieved_gbs": ip_bytes / (ip_ms * 1e-3) / 1e9, "tracks_per_s": T / (ip_ms * 1e-3)}
 
     # ---- e2e: HOST buffers through pv_find_host (H2D + kernel + D2H inside the timed region) --------------------
-    hp = pv.HostPipeline(E, T, p, n_streams=4, device=dev)
+    hp = pv.HostPipeline(E, T, p, n_streams=args.e2e_streams, device=dev)
     hin = hp.pin_inputs(data)
     hout = hp.alloc_outputs(E, T)
     for _ in range(2):
@@ -247,11 +320,17 @@ def main_ours(args):
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
-    e2e_ok = bool(np.array_equal(hout["n_vtx"], res["n_vtx"]))
-    mv = p.max_vtx_per_event
-    h2d = T * 36 + (E + 1) * 4
-    d2h = E * mv * 48 + E * 8 + T * 8
+    e2e_ok = hp.matches(hout, res)
+    h2d, d2h = hp.bytes_per_call(hin, hout)
     hp.close()
+    if world > 1:                                                    # whole-job totals for the line
+        tot = torch.tensor([n_vtx_total, E, T, h2d, d2h, int(e2e_ok)], dtype=torch.int64, device=dev)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        n_vtx_job, E_job, T_job, h2d_job, d2h_job, ok_job = [int(v) for v in tot.tolist()]
+        e2e_ok = ok_job == world
+        assert E_job == E_global and T_job == T_global, (E_job, E_global, T_job, T_global)
+    else:
+        n_vtx_job, E_job, T_job, h2d_job, d2h_job = n_vtx_total, E, T, h2d, d2h
 
     if rank != 0:
         if world > 1:
@@ -259,18 +338,26 @@ def main_ours(args):
         return
 
     ms_step = ms_total / args.steps
-    value = world * E * args.steps / (ms_total * 1e-3)
+    value = E_job * args.steps / (ms_total * 1e-3)
     peak, peak_src = hbm_peak()
     alg = algorithmic_bytes(data, n_vtx_total)
     alg_k = algorithmic_bytes_by_kernel(data, n_vtx_total)
     assert sum(alg_k.values()) == alg
-    traffic_k = {}
-    tpath = os.path.join(ROOT, "profiles", "dram_traffic.csv")      # copied from the committed ncu --set full capture
+    # DRAM bytes per launch from the committed `ncu --set full` capture: accepted only when the capture was made with
+    # the kernels of this working tree (hash recorded beside it), else reported as stale
+    traffic_k, traffic_src = {}, "none for this workload"
+    tpath = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    sha = kernels_sha()
     if os.path.exists(tpath):
         import csv
         for row in csv.DictReader(open(tpath)):
-            if int(row["config"]) == args.config and int(row["events"]) == E:
-                traffic_k[row["kernel"]] = int(row["dram_bytes_per_launch"])
+            if int(row["config"]) == args.config and int(row["events"]) == E and row.get("flavour", "explicit") == args.flavour \
+                    and args.split == "z_ordered" and args.fill == "polynomial":
+                if row.get("kernels_sha") == sha:
+                    traffic_k[row["kernel"]] = int(row["dram_bytes_per_launch"])
+                    traffic_src = f"profiles/{row['source']} (ncu dram__bytes_read.sum + dram__bytes_write.sum, kernels {sha})"
+                else:
+                    traffic_src = f"stale: profiles/dram_traffic.csv was captured with kernels {row.get('kernels_sha')}, this tree is {sha}"
     ksum = float(kernel_ms.sum())
     kernels = [{"name": n, "ms": float(kernel_ms[i]), "share": float(kernel_ms[i] / ksum),
                 "algorithmic_bytes": alg_k[n], "achieved_gbs": alg_k[n] / (kernel_ms[i] * 1e-3) / 1e9,
@@ -287,31 +374,41 @@ def main_ours(args):
         sample = ev_mod.slice_events(data, 0, ns)
         run_oracle(ev_mod.slice_events(data, 0, min(ns, 1000)), cores, args.flavour)
         dt, ref = run_oracle(sample, cores, args.flavour)
-        same = bool(np.array_equal(ref["n_vtx"], res["n_vtx"][:ns]))
+        same = bool(np.array_equal(ref["n_vtx"], res["n_vtx"][:ns])) if args.split == "z_ordered" and args.fill == "polynomial" else None
+        n1 = min(E, max(1000, args.cpu_sample // 10))
+        dt1, _r1 = run_oracle(ev_mod.slice_events(data, 0, n1), 1, args.flavour)
         cpu = {"value": ns / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {ns} events of the same batch, one pass, OpenMP over events on {cores} threads; "
-                         f"n_vtx identical to the GPU's on the sample: {same}"}
+                         f"n_vtx identical to the GPU's on the sample: {same}",
+               "single_thread": {"value": n1 / dt1, "unit": UNIT, "cores": 1, "sample": f"first {n1} events, one pass, one thread"}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32 (int32 fixed-point histogram)", "data": "synthetic",
-        "config": {"workload": f"configs[{args.config}] {m.name}: {E} events, {T} tracks, seed {m.seed}, per GPU",
-                   "events_per_step": E, "tracks_per_step": T, "vertices_per_step": n_vtx_total, "flavour": args.flavour,
-                   "l2": f"inputs {T * 36 / 1e6:.0f} MB per step exceed the 126 MB L2; no flush needed",
-                   "launch": info, "parallelism": f"events sharded over {world} GPU(s), no collective"},
+        "config": {"workload": f"configs[{args.config}] {m.name}: {E_job} events, {T_job} tracks, seed {m.seed}"
+                               + (f", cut into {world} event ranges of equal track count (rank 0: events [{ge0}, {ge1}))" if world > 1 else ""),
+                   "events_per_step": E_job, "tracks_per_step": T_job, "vertices_per_step": n_vtx_job, "flavour": args.flavour,
+                   "split": args.split, "fill": args.fill,
+                   "l2": (f"inputs {T * 36 / 1e6:.0f} MB per step and GPU exceed the 126 MB L2; no flush needed" if not flush else
+                          f"inputs {T * 36 / 1e6:.0f} MB per step would fit the 126 MB L2: a {2 * L2_BYTES >> 20} MB buffer is "
+                          "written between the timed steps, each step timed with its own event pair"),
+                   "launch": info, "parallelism": f"events sharded over {world} GPU(s) by shard.event_range, no collective"},
         "clocks": sampler.summary(),
-        "e2e": {"value": world * E * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "steps": args.e2e_steps, "chunks": args.chunks,
-                "api": "pv_find_host (pinned host buffers, 4 streams)", "matches_device_path": e2e_ok},
+        "e2e": {"value": E_job * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d_job,
+                "d2h_bytes_per_step": d2h_job, "steps": args.e2e_steps, "chunks": args.chunks,
+                "api": f"pv_find_host (pinned host buffers, {args.e2e_streams} streams, compacted vertex read-back)",
+                "matches_device_path": e2e_ok},
         "gpu_launches": args.steps * info["n_kernels"],
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": dom["traffic"], "peak_source": peak_src, "kernel": "pvk::" + dom["name"],
+                     "traffic": dom["traffic"], "traffic_source": traffic_src, "peak_source": peak_src,
+                     "kernel": "pvk::" + dom["name"],
                      "algorithmic_bytes_per_launch": dom["algorithmic_bytes"], "kernel_ms": dom["ms"],
                      "kernels": kernels,
                      "path": {"algorithmic_bytes_per_step": alg, "ms_per_step": ms_step,
                               "achieved": alg / (ms_step * 1e-3) / 1e9, "frac": alg / (ms_step * 1e-3) / 1e9 / peak},
-                     "note": "issue/latency-bound path, not HBM-bound: see DESIGN.md section 8"},
+                     "note": "rank 0's kernels; the path is issue-bound, not HBM-bound (DESIGN.md section 8: warp-instructions "
+                             "per step against 148 SMs x 4 schedulers x the SM clock); BASELINE.json asks for the HBM fraction"},
         "cpu_baseline": cpu,
     }
     if ip_info is not None:
@@ -329,19 +426,37 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--events", type=int, default=None, help="override the number of events (configs[4] sweep)")
-    ap.add_argument("--chunks", type=int, default=8, help="pipeline chunks of the e2e host path")
+    ap.add_argument("--events", type=int, default=None, help="events PER GPU (default: the config's own size; configs[4] sweep)")
+    ap.add_argument("--chunks", type=int, default=16, help="pipeline chunks of the e2e host path")
+    ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-sample", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--with-ip", action="store_true", help="also time pv_track_ip (IP / IP chi2 of every track, NEXT-4)")
     ap.add_argument("--flavour", default="explicit", choices=["explicit", "multivertex"],
                     help="explicit: one track one vertex, Tukey weights (headline); multivertex: the paper's GPU flavour, Eq. 19")
+    ap.add_argument("--split", default="z_ordered", choices=["z_ordered", "recursive"], help="proto-cluster splitting (P:L137)")
+    ap.add_argument("--fill", default="polynomial", choices=["polynomial", "template"], help="histogram fill (P:L131)")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
     if args.impl == "reference":
         main_reference(args)
-    else:
-        main_ours(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not started by torchrun: start the N ranks ourselves
+        import socket
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, this box has {have}")
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        raise SystemExit(subprocess.run(spawn_command(args.gpus, sys.argv[1:], port)).returncode)
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ.get('WORLD_SIZE', '1')}")
+    main_ours(args)
 
 
 if __name__ == "__main__":

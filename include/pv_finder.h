@@ -21,7 +21,9 @@
  *     call; they set bits in event_status[e].
  *   - Device base pointers must be 4-byte aligned; per-event offsets need no alignment.
  *   - Thread safety: calls on different streams are independent provided they use different
- *     workspaces and output buffers.
+ *     workspaces and output buffers (launches are serialised by a lock inside the library).  The two
+ *     diagnostics pv_last_launch_info / pv_kernel_timing are process-global: meaningful only while one
+ *     thread is calling.
  */
 #ifndef PV_FINDER_H
 #define PV_FINDER_H
@@ -38,7 +40,8 @@ typedef struct pv_params {
   float z_min, z_max, dz;               /* histogram range and bin size: -550, 300, 0.25 */
   float z_split;                        /* region boundary: -300                          Table 2 */
   float beam_x, beam_y, beam_tx, beam_ty; /* beamline position and direction at z = 0 */
-  float max_sigma_poca[2];              /* max sigma_poca to enter the histogram: 1.5, 10  P:L129, Table 2 */
+  float max_sigma_poca[2];              /* max sigma_poca to enter the histogram: 1.5, 10  P:L129, Table 2
+                                           (6 max_sigma_poca / dz + 4 <= 3072 bins, else PV_E_PARAM) */
   float min_bin_content;                /* proto-cluster bin threshold [tracks]: 0.25      P:L135 (value: reading R-4) */
   float min_dip;                        /* significance of an extremum [tracks]: 0.75      P:L135 (value: reading R-4) */
   float min_cluster_integral[2];        /* min track integral of a seed cluster: 2.5, 1.75 Table 2 */
@@ -84,8 +87,9 @@ enum {
   PV_EVT_TOO_MANY_TRACKS = 1,  /* n_tracks(e) > PV_MAX_TRACKS_PER_EVENT: event skipped, n_vtx = 0 */
   PV_EVT_VTX_OVERFLOW = 2,     /* more seed clusters than max_vtx_per_event: the first max_vtx in z are kept */
   PV_EVT_SINGULAR_FIT = 4,     /* a vertex fit had < 2 active tracks or a non-positive pivot: that vertex is dropped */
-  PV_EVT_RECORD_OVERFLOW = 8   /* multi-vertex flavour: the batch needed more (track, vertex) records than the
-                                  workspace holds (2 per track): the event is left without vertices */
+  PV_EVT_RECORD_OVERFLOW = 8   /* the workspace cannot hold the event's track records: the multi-vertex flavour needed
+                                  more (track, vertex) records than 2 per track of the batch, or n_tracks given to
+                                  pv_find is smaller than offsets[n_events]: the event is left without vertices */
 };
 
 /* Fill *p with the paper's values (citations on the struct above).  p: HOST.  Returns PV_OK / PV_E_NULL. */
@@ -196,14 +200,17 @@ int pv_find_ext(const float* x, const float* y, const float* z, const float* tx,
                 int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
                 void* workspace, size_t workspace_bytes, void* stream, const pv_track_cov* cov, const pv_debug* dbg);
 
-/* ---- host-buffer entry (the paper's host pipeline: "several streams ... each processing a batch",
- * host->device copies overlapped with compute).  A pv_host_ctx owns device buffers, pinned staging and
- * streams sized for at most max_events / max_tracks; pv_find_host() takes HOST pointers everywhere
- * (same meaning and layout as pv_find), splits the batch into n_chunks contiguous event ranges, and
- * for each enqueues H2D copies -> pv_find -> D2H copies on one of the context's streams.  It returns
- * after all results are in the caller's host arrays (it synchronises its own streams only).  Both flavours and
- * both splitting variants are supported (the context is sized for the flavour given at creation); the covariance
- * cross terms of pv_find_ext are not part of this entry. */
+/* ---- host-buffer entries (the paper's host pipeline: "several streams ... each processing a batch",
+ * host->device copies overlapped with compute).  A pv_host_ctx owns device buffers, workspaces, streams and events
+ * sized for at most max_events / max_tracks (no host staging: the caller's buffers are copied from and to directly, so
+ * they should be pinned, see pv_host_register; pageable memory works but the copies then serialise).
+ * pv_find_host() takes HOST pointers everywhere (same meaning and layout as pv_find), splits the batch into n_chunks
+ * (1..256) contiguous event ranges of equal track count, and for each enqueues H2D copies -> pv_find -> D2H copies on
+ * one of the context's streams.  It returns after all results are in the caller's host arrays (it synchronises its
+ * own streams only, also on every error path).  `offsets` is validated on the host (offsets[0] = 0, non-decreasing,
+ * offsets[n_events] <= max_tracks; else PV_E_SIZE).  Both flavours and both splitting variants are supported (the
+ * context is sized for the flavour given at creation); the covariance cross terms of pv_find_ext are not part of
+ * these entries. */
 typedef struct pv_host_ctx pv_host_ctx;
 int pv_host_ctx_create(pv_host_ctx** ctx, int max_events, long long max_tracks, const pv_params* params,
                        int n_streams);
@@ -215,6 +222,31 @@ int pv_find_host(pv_host_ctx* ctx,
                  float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
                  int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
                  int n_chunks);
+
+/* One PV as pv_find_host_compact returns it: the fields of pv_find's vertex arrays side by side (48 bytes). */
+typedef struct pv_vertex {
+  float pos[3];                 /* x, y, z */
+  float cov[6];                 /* xx, xy, xz, yy, yz, zz (Eq. 14) */
+  float chi2;
+  int32_t ntracks, niter;
+} pv_vertex;
+
+/* pv_find_host with a compact read-back: pv_find's fixed-stride vertex arrays are 6/7 scratch at mu = 5 (5 PVs in 32
+ * slots), so the PVs of each chunk are packed on the device (exclusive scan of n_vtx + gather, two small kernels per
+ * chunk) and only sum(n_vtx) records cross PCIe; the per-track vertex index comes back as int8 (an event holds at
+ * most PV_MAX_VTX = 32 PVs).  HOST outputs:
+ *   vertices   pv_vertex[vtx_capacity]   the PVs of event e are vertices[vtx_begin[e] .. vtx_begin[e+1]), ordered in z;
+ *                                        PV_E_SIZE if the batch holds more than vtx_capacity PVs
+ *   vtx_begin  int32[n_events + 1]       exclusive prefix sum of n_vtx
+ *   n_vtx, trk_weight, event_status      as pv_find
+ *   trk_vertex int8[T]                   index of the track's PV within its event, -1 = none
+ * Same values as pv_find / pv_find_host, bit for bit. */
+int pv_find_host_compact(pv_host_ctx* ctx,
+                         const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                         const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                         const int32_t* offsets, int n_events, const pv_params* params,
+                         pv_vertex* vertices, long long vtx_capacity, int32_t* vtx_begin, int32_t* n_vtx,
+                         float* trk_weight, int8_t* trk_vertex, uint32_t* event_status, int n_chunks);
 /* Pin / unpin caller host memory so pv_find_host copies run asynchronously (optional). */
 int pv_host_register(void* ptr, size_t bytes);
 int pv_host_unregister(void* ptr);

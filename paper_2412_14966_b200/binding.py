@@ -29,7 +29,7 @@ FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
 EXPORTS = (
     "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug", "pv_find_ext", "pv_track_ip",
-    "pv_host_ctx_create", "pv_host_ctx_destroy", "pv_find_host", "pv_host_register", "pv_host_unregister",
+    "pv_host_ctx_create", "pv_host_ctx_destroy", "pv_find_host", "pv_find_host_compact", "pv_host_register", "pv_host_unregister",
     "pv_last_launch_info", "pv_kernel_timing", "pv_kernel_time_ms", "pv_kernel_times_ms", "pv_error_string", "pv_last_cuda_error",
 )
 
@@ -64,6 +64,12 @@ class TrackCov(C.Structure):
     _fields_ = [("cov_xtx", C.c_void_p), ("cov_yty", C.c_void_p)]
 
 
+# struct pv_vertex (include/pv_finder.h): one PV as pv_find_host_compact returns it
+VERTEX_DTYPE = np.dtype([("pos", np.float32, 3), ("cov", np.float32, 6), ("chi2", np.float32),
+                         ("ntracks", np.int32), ("niter", np.int32)])
+assert VERTEX_DTYPE.itemsize == 48
+
+
 class PvError(RuntimeError):
     pass
 
@@ -90,6 +96,7 @@ def lib():
         L.pv_host_ctx_create.argtypes = [C.POINTER(vp), i32, i64, C.POINTER(Params), i32]
         L.pv_host_ctx_destroy.argtypes = [vp]
         L.pv_find_host.argtypes = [vp] + [vp] * 9 + [vp, i32, C.POINTER(Params)] + [vp] * 9 + [i32]
+        L.pv_find_host_compact.argtypes = [vp] + [vp] * 9 + [vp, i32, C.POINTER(Params)] + [vp, i64, vp, vp, vp, vp, vp, i32]
         L.pv_host_register.argtypes = [vp, C.c_size_t]
         L.pv_host_unregister.argtypes = [vp]
         L.pv_last_launch_info.argtypes = [C.POINTER(i32)] * 4
@@ -287,17 +294,23 @@ class HostPipeline:
         self.max_events, self.max_tracks = max_events, max_tracks
         self._pinned = []
 
-    def alloc_outputs(self, E: int, T: int, pinned: bool = True) -> Dict[str, np.ndarray]:
+    def alloc_outputs(self, E: int, T: int, pinned: bool = True, compact: bool = True) -> Dict[str, np.ndarray]:
+        """Pinned host output buffers.  compact (pv_find_host_compact): `vertices` (pv_vertex records, capacity
+        E * max_vtx), `vtx_begin` [E + 1], int8 `trk_vertex`; else the fixed-stride arrays of pv_find_host."""
         torch = _torch()
         mv = self.p.max_vtx_per_event
-        spec = dict(vtx_pos=((E, mv, 3), torch.float32), vtx_cov=((E, mv, 6), torch.float32), vtx_chi2=((E, mv), torch.float32),
-                    vtx_ntracks=((E, mv), torch.int32), vtx_niter=((E, mv), torch.int32), n_vtx=((E,), torch.int32),
-                    trk_weight=((T,), torch.float32), trk_vertex=((T,), torch.int32), event_status=((E,), torch.int32))
+        if compact:
+            spec = dict(vertices=((E * mv * 48,), torch.uint8), vtx_begin=((E + 1,), torch.int32), n_vtx=((E,), torch.int32),
+                        trk_weight=((T,), torch.float32), trk_vertex=((T,), torch.int8), event_status=((E,), torch.int32))
+        else:
+            spec = dict(vtx_pos=((E, mv, 3), torch.float32), vtx_cov=((E, mv, 6), torch.float32), vtx_chi2=((E, mv), torch.float32),
+                        vtx_ntracks=((E, mv), torch.int32), vtx_niter=((E, mv), torch.int32), n_vtx=((E,), torch.int32),
+                        trk_weight=((T,), torch.float32), trk_vertex=((T,), torch.int32), event_status=((E,), torch.int32))
         out = {}
         for k, (shape, dt) in spec.items():
             t = torch.zeros(shape, dtype=dt, pin_memory=pinned)
             self._pinned.append(t)
-            out[k] = t.numpy()
+            out[k] = t.numpy().view(VERTEX_DTYPE) if k == "vertices" else t.numpy()
         return out
 
     def pin_inputs(self, data: Dict[str, np.ndarray]) -> Dict[str, np.ndarray]:
@@ -312,16 +325,53 @@ class HostPipeline:
         return out
 
     def find(self, data: Dict[str, np.ndarray], out: Dict[str, np.ndarray], n_chunks: int = 8) -> None:
+        """pv_find_host_compact when `out` holds `vertices` (alloc_outputs(compact=True)), else pv_find_host."""
         torch = _torch()
         E = int(data["offsets"].size - 1)
         ptr = lambda a: a.ctypes.data
         with torch.cuda.device(self.device):
-            rc = lib().pv_find_host(
-                self.ctx, *[ptr(data[k]) for k in FIELDS], ptr(data["offsets"]), E, C.byref(self.p),
-                ptr(out["vtx_pos"]), ptr(out["vtx_cov"]), ptr(out["vtx_chi2"]), ptr(out["vtx_ntracks"]),
-                ptr(out["vtx_niter"]), ptr(out["n_vtx"]), ptr(out["trk_weight"]), ptr(out["trk_vertex"]),
-                ptr(out["event_status"]), n_chunks)
-        _check(rc, "pv_find_host")
+            if "vertices" in out:
+                rc = lib().pv_find_host_compact(
+                    self.ctx, *[ptr(data[k]) for k in FIELDS], ptr(data["offsets"]), E, C.byref(self.p),
+                    ptr(out["vertices"]), out["vertices"].size, ptr(out["vtx_begin"]), ptr(out["n_vtx"]),
+                    ptr(out["trk_weight"]), ptr(out["trk_vertex"]), ptr(out["event_status"]), n_chunks)
+                _check(rc, "pv_find_host_compact")
+            else:
+                rc = lib().pv_find_host(
+                    self.ctx, *[ptr(data[k]) for k in FIELDS], ptr(data["offsets"]), E, C.byref(self.p),
+                    ptr(out["vtx_pos"]), ptr(out["vtx_cov"]), ptr(out["vtx_chi2"]), ptr(out["vtx_ntracks"]),
+                    ptr(out["vtx_niter"]), ptr(out["n_vtx"]), ptr(out["trk_weight"]), ptr(out["trk_vertex"]),
+                    ptr(out["event_status"]), n_chunks)
+                _check(rc, "pv_find_host")
+
+    def bytes_per_call(self, data: Dict[str, np.ndarray], out: Dict[str, np.ndarray]):
+        """(host->device, device->host) bytes the last find() moved, counted from the buffers it copies."""
+        E = int(data["offsets"].size - 1)
+        T = int(data["offsets"][-1])
+        h2d = T * 36 + (E + 1) * 4
+        if "vertices" in out:
+            nv = int(out["vtx_begin"][E])
+            d2h = nv * 48 + E * 8 + T * 5 + 4 * min(E, 256)
+        else:
+            d2h = E * self.p.max_vtx_per_event * 48 + E * 8 + T * 8
+        return h2d, d2h
+
+    def matches(self, out: Dict[str, np.ndarray], dev: Dict[str, np.ndarray]) -> bool:
+        """Bit-for-bit equality of a host-pipeline result with DeviceBatch.results() of the same batch."""
+        mv = self.p.max_vtx_per_event
+        nv = dev["n_vtx"]
+        m = np.arange(mv)[None, :] < nv[:, None]
+        ok = np.array_equal(out["n_vtx"], nv) and np.array_equal(out["event_status"].view(np.uint32), dev["event_status"])
+        ok = ok and np.array_equal(out["trk_weight"], dev["trk_weight"]) and np.array_equal(out["trk_vertex"].astype(np.int32), dev["trk_vertex"])
+        if not ok:
+            return False
+        if "vertices" in out:
+            v = out["vertices"][:int(nv.sum())]
+            return bool(np.array_equal(out["vtx_begin"], np.concatenate([[0], np.cumsum(nv)]).astype(np.int32))
+                        and np.array_equal(v["pos"], dev["vtx_pos"][m]) and np.array_equal(v["cov"], dev["vtx_cov"][m])
+                        and np.array_equal(v["chi2"], dev["vtx_chi2"][m]) and np.array_equal(v["ntracks"], dev["vtx_ntracks"][m])
+                        and np.array_equal(v["niter"], dev["vtx_niter"][m]))
+        return all(np.array_equal(out[k][m], dev[k][m]) for k in ("vtx_pos", "vtx_cov", "vtx_chi2", "vtx_ntracks", "vtx_niter"))
 
     def close(self):
         if self.ctx:

@@ -81,6 +81,9 @@ int validate(const pv_params* p, int* nbins_out) {
   if (p->flavour != PV_FLAVOUR_EXPLICIT && p->flavour != PV_FLAVOUR_MULTIVERTEX) return PV_E_PARAM;
   if (p->split_mode != PV_SPLIT_Z_ORDERED && p->split_mode != PV_SPLIT_RECURSIVE) return PV_E_PARAM;
   if (p->flavour == PV_FLAVOUR_MULTIVERTEX && (!(p->chi2_window > 0.0f) || isinf(p->chi2_max))) return PV_E_PARAM;
+  // the fill cuts a track's +-3 sigma window into units of PV_UNIT bins and numbers them with 9 bits
+  for (int r = 0; r < 2; ++r)
+    if (!(6.0 * (double)p->max_sigma_poca[r] / (double)p->dz + 4.0 <= 512.0 * PV_UNIT)) return PV_E_PARAM;
   if (nbins_out) *nbins_out = nbins;
   return PV_OK;
 }
@@ -134,7 +137,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
               float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
               int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
               void* workspace, size_t workspace_bytes, void* stream_, const pv_debug* dbg,
-              const pv_track_cov* cov = nullptr) {
+              const pv_track_cov* cov = nullptr, int8_t* trk_vertex8 = nullptr) {
   int nbins = 0;
   int rc = validate(params, &nbins);
   if (rc != PV_OK) return rc;
@@ -159,10 +162,12 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   make_kparams(params, nbins, &kp);
   int teams = di->max_smem_optin / kp.team_smem_bytes;        // teams (events in flight) per CTA
   if (teams > pvk::MAX_TEAMS) teams = pvk::MAX_TEAMS;
+#ifdef PV_TUNING                                              // tuning builds only: fewer events in flight per CTA
   if (const char* envw = getenv("PV_TEAMS_PER_CTA")) {
     const int w = atoi(envw);
     if (w >= 1 && w < teams) teams = w;
   }
+#endif
   if (teams < 1) return PV_E_PARAM;
   const int smem = teams * kp.team_smem_bytes;
   const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
@@ -195,6 +200,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.vtx_pos = vtx_pos; ka.vtx_cov = vtx_cov; ka.vtx_chi2 = vtx_chi2;
   ka.vtx_ntracks = vtx_ntracks; ka.vtx_niter = vtx_niter; ka.n_vtx = n_vtx;
   ka.trk_weight = trk_weight; ka.trk_vertex = trk_vertex; ka.event_status = event_status;
+  ka.trk_vertex8 = trk_vertex8;
   unsigned char* ws = reinterpret_cast<unsigned char*>(workspace);
   ka.evt_counter = reinterpret_cast<unsigned int*>(ws);
   ka.seed_counter = reinterpret_cast<unsigned int*>(ws + 16);
@@ -209,7 +215,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
   CK(cudaMemsetAsync(workspace, 0, 48, stream));
-  // a1..a4: persistent, one CTA per SM, one team of two teams per event
+  // a1..a4: persistent, one CTA per SM, one team of two warps per event
   int grid = di->sms;
   const int need = (n_events + teams - 1) / teams;
   if (grid > need) grid = need;
@@ -351,16 +357,24 @@ int pv_track_ip(const float* x, const float* y, const float* z, const float* tx,
 }
 
 /* ------------------------------------------- host-buffer pipeline ------------------------------------------- */
+constexpr int HOST_MAX_CHUNKS = 256;
+
 struct pv_host_ctx {
   int max_events = 0;
   long long max_tracks = 0;
   int max_vtx = 0;
   int n_streams = 0;
   std::vector<cudaStream_t> streams;
+  cudaStream_t vtx_stream = nullptr;          // read-back of the packed vertices (sizes known once a chunk is done)
+  cudaEvent_t done[HOST_MAX_CHUNKS] = {nullptr};
+  int32_t* h_total = nullptr;                 // pinned: vertices found per chunk
   float* d_in[9] = {nullptr};
   int32_t* d_off = nullptr;
   float *d_pos = nullptr, *d_cov = nullptr, *d_chi2 = nullptr, *d_w = nullptr;
   int32_t *d_ntrk = nullptr, *d_niter = nullptr, *d_nvtx = nullptr, *d_tv = nullptr;
+  int8_t* d_tv8 = nullptr;
+  int32_t* d_vbegin = nullptr;                // per chunk: exclusive scan of n_vtx, ne + 1 entries at e0 + chunk index
+  pv_vertex* d_packed = nullptr;              // per chunk: its vertices in event order, starting at record e0 * max_vtx
   uint32_t* d_status = nullptr;
   unsigned char* d_ws = nullptr;   // n_streams workspaces of ws_stride bytes each
   size_t ws_stride = 0;
@@ -369,9 +383,14 @@ struct pv_host_ctx {
 int pv_host_ctx_destroy(pv_host_ctx* c) {
   if (!c) return PV_E_NULL;
   for (auto s : c->streams) cudaStreamDestroy(s);
+  if (c->vtx_stream) cudaStreamDestroy(c->vtx_stream);
+  for (int i = 0; i < HOST_MAX_CHUNKS; ++i)
+    if (c->done[i]) cudaEventDestroy(c->done[i]);
+  if (c->h_total) cudaFreeHost(c->h_total);
   for (int i = 0; i < 9; ++i) cudaFree(c->d_in[i]);
   cudaFree(c->d_off); cudaFree(c->d_pos); cudaFree(c->d_cov); cudaFree(c->d_chi2); cudaFree(c->d_w);
   cudaFree(c->d_ntrk); cudaFree(c->d_niter); cudaFree(c->d_nvtx); cudaFree(c->d_tv); cudaFree(c->d_status);
+  cudaFree(c->d_tv8); cudaFree(c->d_vbegin); cudaFree(c->d_packed);
   cudaFree(c->d_ws);
   delete c;
   return PV_OK;
@@ -393,13 +412,17 @@ int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, 
   A((void**)&c->d_pos, E * mv * 12); A((void**)&c->d_cov, E * mv * 24); A((void**)&c->d_chi2, E * mv * 4);
   A((void**)&c->d_ntrk, E * mv * 4); A((void**)&c->d_niter, E * mv * 4); A((void**)&c->d_nvtx, E * 4);
   A((void**)&c->d_w, T * 4); A((void**)&c->d_tv, T * 4); A((void**)&c->d_status, E * 4);
+  A((void**)&c->d_tv8, T); A((void**)&c->d_vbegin, (E + HOST_MAX_CHUNKS + 1) * 4); A((void**)&c->d_packed, E * mv * sizeof(pv_vertex));
   c->ws_stride = (ws_bytes(max_events, max_tracks, c->max_vtx, params->flavour) + 255) / 256 * 256;
   A((void**)&c->d_ws, (size_t)n_streams * c->ws_stride);
+  if (err == cudaSuccess) err = cudaMallocHost((void**)&c->h_total, HOST_MAX_CHUNKS * sizeof(int32_t));
   for (int i = 0; i < n_streams && err == cudaSuccess; ++i) {
     cudaStream_t s = nullptr;
     err = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
     if (err == cudaSuccess) c->streams.push_back(s);
   }
+  if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&c->vtx_stream, cudaStreamNonBlocking);
+  for (int i = 0; i < HOST_MAX_CHUNKS && err == cudaSuccess; ++i) err = cudaEventCreateWithFlags(&c->done[i], cudaEventDisableTiming);
   if (err != cudaSuccess) {
     pv_host_ctx_destroy(c);
     return cuda_fail(err, "pv_host_ctx_create");
@@ -408,21 +431,37 @@ int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, 
   return PV_OK;
 }
 
-int pv_find_host(pv_host_ctx* c,
-                 const float* x, const float* y, const float* z, const float* tx, const float* ty,
-                 const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
-                 const int32_t* offsets, int n_events, const pv_params* params,
-                 float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
-                 int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status, int n_chunks) {
-  if (!c || !offsets || !params) return PV_E_NULL;
+namespace {
+
+// Both host entries: H2D -> kernels -> D2H per chunk of events, chunks round-robin over the context's streams.
+// compact == false: the fixed-stride [E][max_vtx] vertex arrays come back whole (pv_find_host).
+// compact == true:  the vertices of a chunk are packed on the device (scan of n_vtx + gather) and only sum(n_vtx)
+//                   48-byte records come back, plus int8 vertex indices per track (pv_find_host_compact).
+// No early return once work is enqueued: every error path reaches the synchronisation of all streams, so no copy into
+// the caller's buffers is in flight when the call returns.
+int host_impl(pv_host_ctx* c, const float* const h_in[9], const int32_t* offsets, int n_events, const pv_params* params,
+              bool compact, float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+              pv_vertex* vertices, long long vtx_capacity, int32_t* vtx_begin, int32_t* n_vtx, float* trk_weight,
+              int32_t* trk_vertex, int8_t* trk_vertex8, uint32_t* event_status, int n_chunks) {
+  if (!c || !offsets || !params || !n_vtx || !event_status) return PV_E_NULL;
+  if (compact ? (!vertices || !vtx_begin || vtx_capacity < 0) : (!vtx_pos || !vtx_cov || !vtx_chi2 || !vtx_ntracks || !vtx_niter))
+    return PV_E_NULL;
   if (n_events < 0 || n_events > c->max_events) return PV_E_SIZE;
   if (params->max_vtx_per_event != c->max_vtx) return PV_E_PARAM;
+  if (compact) vtx_begin[0] = 0;
   if (n_events == 0) return PV_OK;
+  // the offsets are the caller's: one pass checks what every later index relies on
+  if (offsets[0] != 0) return PV_E_SIZE;
+  for (int e = 0; e < n_events; ++e)
+    if (offsets[e + 1] < offsets[e]) return PV_E_SIZE;
   const long long T = offsets[n_events];
-  if (offsets[0] != 0 || T < 0 || T > c->max_tracks) return PV_E_SIZE;
+  if (T > c->max_tracks) return PV_E_SIZE;
+  if (T > 0 && (!trk_weight || (compact ? !trk_vertex8 : !trk_vertex))) return PV_E_NULL;
+  for (int i = 0; i < 9; ++i)
+    if (T > 0 && !h_in[i]) return PV_E_NULL;
   if (n_chunks < 1) n_chunks = 1;
   if (n_chunks > n_events) n_chunks = n_events;
-  const float* h_in[9] = {x, y, z, tx, ty, var_x, var_y, var_tx, var_ty};
+  if (n_chunks > HOST_MAX_CHUNKS) n_chunks = HOST_MAX_CHUNKS;
   const size_t mv = (size_t)c->max_vtx;
   // chunk boundaries: equal track counts (events are contiguous in the SoA arrays)
   std::vector<int> eb(n_chunks + 1, 0);
@@ -433,37 +472,100 @@ int pv_find_host(pv_host_ctx* c,
     eb[k] = e < eb[k - 1] ? eb[k - 1] : e;
   }
   int rc = PV_OK;
+  auto ck = [&](cudaError_t err, const char* what) {
+    if (err != cudaSuccess && rc == PV_OK) rc = cuda_fail(err, what);
+    return rc == PV_OK;
+  };
+  int enqueued = 0;
   for (int k = 0; k < n_chunks && rc == PV_OK; ++k) {
     const int e0 = eb[k], e1 = eb[k + 1];
+    c->h_total[k] = 0;
     if (e1 <= e0) continue;
     cudaStream_t s = c->streams[k % c->n_streams];
     const size_t t0 = (size_t)offsets[e0], nt = (size_t)offsets[e1] - t0, ne = (size_t)(e1 - e0);
     // offsets stay absolute: the kernel indexes the un-shifted SoA base pointers
-    CK(cudaMemcpyAsync(c->d_off + e0, offsets + e0, (ne + 1) * 4, cudaMemcpyHostToDevice, s));
-    if (nt > 0)
-      for (int i = 0; i < 9; ++i) CK(cudaMemcpyAsync(c->d_in[i] + t0, h_in[i] + t0, nt * 4, cudaMemcpyHostToDevice, s));
-    rc = find_impl(c->d_in[0], c->d_in[1], c->d_in[2], c->d_in[3], c->d_in[4], c->d_in[5], c->d_in[6], c->d_in[7], c->d_in[8],
-                   c->d_off + e0, (int)ne, (long long)c->max_tracks, params, c->d_pos + e0 * mv * 3, c->d_cov + e0 * mv * 6,
-                   c->d_chi2 + e0 * mv, c->d_ntrk + e0 * mv, c->d_niter + e0 * mv, c->d_nvtx + e0, c->d_w, c->d_tv,
-                   c->d_status + e0, c->d_ws + (size_t)(k % c->n_streams) * c->ws_stride, c->ws_stride, s, nullptr);
+    if (!ck(cudaMemcpyAsync(c->d_off + e0, offsets + e0, (ne + 1) * 4, cudaMemcpyHostToDevice, s), "H2D offsets")) break;
+    for (int i = 0; i < 9 && nt > 0 && rc == PV_OK; ++i)
+      ck(cudaMemcpyAsync(c->d_in[i] + t0, h_in[i] + t0, nt * 4, cudaMemcpyHostToDevice, s), "H2D tracks");
     if (rc != PV_OK) break;
-    CK(cudaMemcpyAsync(vtx_pos + e0 * mv * 3, c->d_pos + e0 * mv * 3, ne * mv * 12, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(vtx_cov + e0 * mv * 6, c->d_cov + e0 * mv * 6, ne * mv * 24, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(vtx_chi2 + e0 * mv, c->d_chi2 + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(vtx_ntracks + e0 * mv, c->d_ntrk + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(vtx_niter + e0 * mv, c->d_niter + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(n_vtx + e0, c->d_nvtx + e0, ne * 4, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(event_status + e0, c->d_status + e0, ne * 4, cudaMemcpyDeviceToHost, s));
+    const int frc = find_impl(c->d_in[0], c->d_in[1], c->d_in[2], c->d_in[3], c->d_in[4], c->d_in[5], c->d_in[6], c->d_in[7],
+                              c->d_in[8], c->d_off + e0, (int)ne, (long long)c->max_tracks, params, c->d_pos + e0 * mv * 3,
+                              c->d_cov + e0 * mv * 6, c->d_chi2 + e0 * mv, c->d_ntrk + e0 * mv, c->d_niter + e0 * mv,
+                              c->d_nvtx + e0, c->d_w, c->d_tv, c->d_status + e0,
+                              c->d_ws + (size_t)(k % c->n_streams) * c->ws_stride, c->ws_stride, s, nullptr, nullptr,
+                              compact ? c->d_tv8 : nullptr);
+    if (frc != PV_OK) { rc = frc; break; }
+    enqueued = k + 1;
+    if (compact) {
+      pvk::KArgs ka;
+      memset(&ka, 0, sizeof(ka));
+      ka.n_events = (int)ne;
+      ka.vtx_pos = c->d_pos + e0 * mv * 3; ka.vtx_cov = c->d_cov + e0 * mv * 6; ka.vtx_chi2 = c->d_chi2 + e0 * mv;
+      ka.vtx_ntracks = c->d_ntrk + e0 * mv; ka.vtx_niter = c->d_niter + e0 * mv;
+      int32_t* vb = c->d_vbegin + e0 + k;
+      pvk::scan_nvtx_kernel<<<1, 1024, 0, s>>>(c->d_nvtx + e0, (int)ne, vb);
+      pvk::pack_vertices_kernel<<<(unsigned)((ne + 7) / 8), 256, 0, s>>>(ka, (int)mv, vb, c->d_packed + e0 * mv);
+      if (!ck(cudaGetLastError(), "pack_vertices_kernel")) break;
+      if (!ck(cudaMemcpyAsync(c->h_total + k, vb + ne, 4, cudaMemcpyDeviceToHost, s), "D2H chunk total")) break;
+      if (!ck(cudaEventRecord(c->done[k], s), "cudaEventRecord")) break;
+    } else {
+      ck(cudaMemcpyAsync(vtx_pos + e0 * mv * 3, c->d_pos + e0 * mv * 3, ne * mv * 12, cudaMemcpyDeviceToHost, s), "D2H");
+      ck(cudaMemcpyAsync(vtx_cov + e0 * mv * 6, c->d_cov + e0 * mv * 6, ne * mv * 24, cudaMemcpyDeviceToHost, s), "D2H");
+      ck(cudaMemcpyAsync(vtx_chi2 + e0 * mv, c->d_chi2 + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s), "D2H");
+      ck(cudaMemcpyAsync(vtx_ntracks + e0 * mv, c->d_ntrk + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s), "D2H");
+      ck(cudaMemcpyAsync(vtx_niter + e0 * mv, c->d_niter + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s), "D2H");
+    }
+    ck(cudaMemcpyAsync(n_vtx + e0, c->d_nvtx + e0, ne * 4, cudaMemcpyDeviceToHost, s), "D2H");
+    ck(cudaMemcpyAsync(event_status + e0, c->d_status + e0, ne * 4, cudaMemcpyDeviceToHost, s), "D2H");
     if (nt > 0) {
-      CK(cudaMemcpyAsync(trk_weight + t0, c->d_w + t0, nt * 4, cudaMemcpyDeviceToHost, s));
-      CK(cudaMemcpyAsync(trk_vertex + t0, c->d_tv + t0, nt * 4, cudaMemcpyDeviceToHost, s));
+      ck(cudaMemcpyAsync(trk_weight + t0, c->d_w + t0, nt * 4, cudaMemcpyDeviceToHost, s), "D2H");
+      if (compact) ck(cudaMemcpyAsync(trk_vertex8 + t0, c->d_tv8 + t0, nt, cudaMemcpyDeviceToHost, s), "D2H");
+      else ck(cudaMemcpyAsync(trk_vertex + t0, c->d_tv + t0, nt * 4, cudaMemcpyDeviceToHost, s), "D2H");
     }
   }
-  for (auto s : c->streams) {
-    cudaError_t err = cudaStreamSynchronize(s);
-    if (err != cudaSuccess && rc == PV_OK) rc = cuda_fail(err, "cudaStreamSynchronize");
+  // second pass (compact): as each chunk finishes, its vertex count is on the host and its packed records are copied
+  // to their final place behind those of the chunks before it
+  long long base = 0;
+  for (int k = 0; compact && k < enqueued && rc == PV_OK; ++k) {
+    const int e0 = eb[k], e1 = eb[k + 1];
+    if (e1 <= e0) continue;
+    if (!ck(cudaEventSynchronize(c->done[k]), "cudaEventSynchronize")) break;
+    const long long nv = c->h_total[k];
+    if (base + nv > vtx_capacity) { rc = PV_E_SIZE; break; }
+    if (nv > 0)
+      ck(cudaMemcpyAsync(vertices + base, c->d_packed + (size_t)e0 * mv, (size_t)nv * sizeof(pv_vertex), cudaMemcpyDeviceToHost,
+                         c->vtx_stream), "D2H vertices");
+    base += nv;
   }
+  for (auto s : c->streams) ck(cudaStreamSynchronize(s), "cudaStreamSynchronize");
+  ck(cudaStreamSynchronize(c->vtx_stream), "cudaStreamSynchronize");
+  if (rc == PV_OK && compact)
+    for (int e = 0; e < n_events; ++e) vtx_begin[e + 1] = vtx_begin[e] + n_vtx[e];
   return rc;
+}
+
+}  // namespace
+
+int pv_find_host(pv_host_ctx* c,
+                 const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                 const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                 const int32_t* offsets, int n_events, const pv_params* params,
+                 float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                 int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status, int n_chunks) {
+  const float* h_in[9] = {x, y, z, tx, ty, var_x, var_y, var_tx, var_ty};
+  return host_impl(c, h_in, offsets, n_events, params, false, vtx_pos, vtx_cov, vtx_chi2, vtx_ntracks, vtx_niter, nullptr, 0,
+                   nullptr, n_vtx, trk_weight, trk_vertex, nullptr, event_status, n_chunks);
+}
+
+int pv_find_host_compact(pv_host_ctx* c,
+                         const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                         const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                         const int32_t* offsets, int n_events, const pv_params* params,
+                         pv_vertex* vertices, long long vtx_capacity, int32_t* vtx_begin, int32_t* n_vtx,
+                         float* trk_weight, int8_t* trk_vertex, uint32_t* event_status, int n_chunks) {
+  const float* h_in[9] = {x, y, z, tx, ty, var_x, var_y, var_tx, var_ty};
+  return host_impl(c, h_in, offsets, n_events, params, true, nullptr, nullptr, nullptr, nullptr, nullptr, vertices, vtx_capacity,
+                   vtx_begin, n_vtx, trk_weight, nullptr, trk_vertex, event_status, n_chunks);
 }
 
 int pv_host_register(void* ptr, size_t bytes) {

@@ -2,7 +2,7 @@
 //
 // Three kernels per pv_find call:
 //
-//   seed_kernel     a1..a4  one TEAM of two warps per event, persistent grid, 13 teams per CTA, one int32
+//   seed_kernel     a1..a4  one TEAM of two warps per event, persistent grid, 14 teams per CTA, one int32
 //                           shared-memory histogram and one named barrier per team.  POCA projection (fp32 contract,
 //                           bit-exact with the CPU oracle), flat list of 6-bin fill units (seven independent CDF edges
 //                           per thread), touched-word flags, one ballot per touched word for the proto-cluster starts,
@@ -115,6 +115,7 @@ struct KArgs {
   float* trk_weight;
   int32_t* trk_vertex;
   uint32_t* event_status;
+  int8_t* trk_vertex8;           // optional (host pipeline): trk_vertex as int8 (an event holds <= 32 PVs), nullptr = not written
   unsigned int* evt_counter;     // workspace: next event of the persistent seed kernel
   unsigned int* seed_counter;    // workspace: seed records written so far
   SeedRec* rec;                  // workspace: [n_events * max_vtx]
@@ -387,8 +388,16 @@ __device__ __forceinline__ bool track_is_dead(const Trk& T, const KParams& P) {
 
 struct RawTrk { float x, y, z, tx, ty, vx, vy, vtx, vty; };
 
-// Eq. 2 for one coordinate at dz = z - z_trk: V_xx + 2 dz V_xtx + dz^2 V_txtx
-__device__ __forceinline__ float var_at(float v, float vt, float c, float dz) { return fmaf(dz, fmaf(dz, vt, 2.0f * c), v); }
+// Eq. 2 for one coordinate at dz = z - z_trk: V_xx + 2 dz V_xtx + dz^2 V_txtx.  With a cross term the three
+// terms cancel when the state is given far from the vertex (at 150 mm they are 25 x the result), so that one expression
+// is evaluated in double (once per record, not per iteration); the diagonal case has only positive terms.
+__device__ __forceinline__ float var_at(float v, float vt, float c, float dz) {
+  if (c != 0.0f) {
+    const double d = (double)dz;
+    return (float)fma(d, fma(d, (double)vt, 2.0 * (double)c), (double)v);
+  }
+  return fmaf(dz, dz * vt, v);
+}
 
 // cx, cy: the track's V_xtx, V_yty (0 for a diagonal covariance)
 __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, float cx, float cy, float sx, float sy, float zsv) {
@@ -441,7 +450,9 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   const size_t ev = (size_t)e * P.max_vtx;
   unsigned status = 0;
 
-  if (n > MAX_TRK) {
+  // explicit flavour: the fit-ready records of the event go to ftrk[t0 .. t0 + n): refuse what the workspace cannot hold
+  const bool no_room = FLAV == PV_FLAVOUR_EXPLICIT && (unsigned)t0 + (unsigned)n > A.trk_cap;
+  if (n > MAX_TRK || no_room) {
 #pragma unroll 1
     for (int i = tt; i < n; i += TEAM) {
       A.trk_vertex[t0 + i] = -1;
@@ -450,7 +461,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     if (DBG && A.dbg.trk_seed) for (int i = tt; i < n; i += TEAM) A.dbg.trk_seed[t0 + i] = -1;
     if (tt == 0) {
       A.n_vtx[e] = 0;
-      A.event_status[e] = PV_EVT_TOO_MANY_TRACKS;
+      A.event_status[e] = n > MAX_TRK ? PV_EVT_TOO_MANY_TRACKS : PV_EVT_RECORD_OVERFLOW;
       if (DBG && A.dbg.n_seeds) A.dbg.n_seeds[e] = 0;
       if (DBG && A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = 0;
     }
@@ -954,7 +965,9 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       int4 r;
       r.x = e; r.y = lane | (myc << 5); r.z = t0 + myoff; r.w = __float_as_int(zs[lane]);
       reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
+      if (myc == 0) A.vtx_niter[ev + lane] = -1;             // only with min_tracks_seed < 1: the fit never sees this seed
     }
+    if (__any_sync(FULL, lane < ns && myc == 0)) status |= PV_EVT_SINGULAR_FIT;
     if (lane == 0) {
       A.n_vtx[e] = ns;                                     // scratch: seeds of the event, replaced by cleanup_kernel
       A.event_status[e] = status;
@@ -1460,6 +1473,7 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
     int vtx = -1;
     if (s >= 0 && ((kept >> s) & 1u)) vtx = __popc(kept & ((1u << s) - 1u));
     A.trk_vertex[t0 + i] = vtx;
+    if (A.trk_vertex8) A.trk_vertex8[t0 + i] = (int8_t)vtx;
     if (FLAV == PV_FLAVOUR_MULTIVERTEX) A.trk_weight[t0 + i] = vtx >= 0 ? w : 0.0f;
     else if (vtx < 0) A.trk_weight[t0 + i] = 0.0f;
   };
@@ -1468,6 +1482,53 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
     if (lane + 32 * q < n) finish(lane + 32 * q, sv[q], bv[q]);
   for (int i = 128 + lane; i < n; i += 32)
     finish(i, A.trk_vertex[t0 + i], FLAV == PV_FLAVOUR_MULTIVERTEX ? A.best[t0 + i] : 0ull);
+}
+
+// ---- host pipeline: the PVs of a chunk of events packed into 48-byte records in event order, so that the
+// device-to-host copy moves sum(n_vtx) records instead of n_events * max_vtx slots.
+// scan_nvtx_kernel: one CTA; begin[e] = sum of n_vtx[0..e), begin[n_events] = total (exclusive scan, tiles of 1024).
+__global__ void __launch_bounds__(1024) scan_nvtx_kernel(const int32_t* __restrict__ n_vtx, int n_events,
+                                                         int32_t* __restrict__ begin) {
+  __shared__ int wsum[32];
+  __shared__ int carry_s;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < n_events; base += 1024) {
+    const int e = base + threadIdx.x;
+    const int v = e < n_events ? n_vtx[e] : 0;
+    const int inc = warp_incl_scan(v, lane);
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    const int carry = carry_s;
+    int wv = wsum[lane];
+    const int winc = warp_incl_scan(wv, lane);                 // every warp scans the 32 warp totals
+    const int woff = __shfl_sync(FULL, winc - wv, warp);
+    if (e < n_events) begin[e] = carry + woff + inc - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry_s = carry + woff + inc;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) begin[n_events] = carry_s;
+}
+
+// pack_vertices_kernel: one warp per event, lane k = vertex k of the event -> record begin[e] + k.
+__global__ void __launch_bounds__(256) pack_vertices_kernel(const __grid_constant__ KArgs A, int max_vtx,
+                                                            const int32_t* __restrict__ begin, pv_vertex* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (e >= A.n_events) return;
+  const int b = begin[e], nv = begin[e + 1] - b;
+  if (lane < nv) {
+    const size_t o = (size_t)e * max_vtx + lane;
+    float4 q0, q1, q2;
+    q0.x = A.vtx_pos[o * 3 + 0]; q0.y = A.vtx_pos[o * 3 + 1]; q0.z = A.vtx_pos[o * 3 + 2]; q0.w = A.vtx_cov[o * 6 + 0];
+    q1.x = A.vtx_cov[o * 6 + 1]; q1.y = A.vtx_cov[o * 6 + 2]; q1.z = A.vtx_cov[o * 6 + 3]; q1.w = A.vtx_cov[o * 6 + 4];
+    q2.x = A.vtx_cov[o * 6 + 5]; q2.y = A.vtx_chi2[o];
+    q2.z = __int_as_float(A.vtx_ntracks[o]); q2.w = __int_as_float(A.vtx_niter[o]);
+    float4* dst = reinterpret_cast<float4*>(out + b + lane);
+    dst[0] = q0; dst[1] = q1; dst[2] = q2;
+  }
 }
 
 // ---- ip_kernel: NEXT-4, impact parameter and IP chi2 of every track w.r.t. the PVs of its event ---------

@@ -40,6 +40,7 @@ class EventModel:
     trk_smog_mean: float = 15.0
     slope_smog: float = 0.15
     pair_separations: Optional[tuple] = None  # configs[3]: dz sweep, by event index mod len
+    aniso: bool = False                # per-track var_y = k var_x, k in [1/4, 4]; var_tx, var_ty in [0.5, 2] x 1e-6, independent
 
 
 def config(idx: int, n_events: Optional[int] = None) -> EventModel:
@@ -109,8 +110,9 @@ def _gen_block(m: EventModel, block: int, n_ev: int, ev0: int):
     tx_true = np.clip(rng.normal(0.0, 1.0, nreal) * slope_sigma, -0.4, 0.4)
     ty_true = np.clip(rng.normal(0.0, 1.0, nreal) * slope_sigma, -0.4, 0.4)
     sig = rng.uniform(0.01, 0.1, nreal)
+    sig_y = sig * np.sqrt(np.exp(rng.uniform(np.log(0.25), np.log(4.0), nreal))) if m.aniso else sig
     x = pv_x[t_pv] + sig * rng.normal(0.0, 1.0, nreal)
-    y = pv_y[t_pv] + sig * rng.normal(0.0, 1.0, nreal)
+    y = pv_y[t_pv] + sig_y * rng.normal(0.0, 1.0, nreal)
     z = pv_z[t_pv]
     tx = tx_true + rng.normal(0.0, 1e-3, nreal)
     ty = ty_true + rng.normal(0.0, 1e-3, nreal)
@@ -123,6 +125,7 @@ def _gen_block(m: EventModel, block: int, n_ev: int, ev0: int):
     g_tx = np.clip(rng.normal(0.0, m.slope_pp, ng), -0.4, 0.4) + rng.normal(0.0, 1e-3, ng)
     g_ty = np.clip(rng.normal(0.0, m.slope_pp, ng), -0.4, 0.4) + rng.normal(0.0, 1e-3, ng)
     g_sig = rng.uniform(0.01, 0.1, ng)
+    g_sig_y = g_sig * np.sqrt(np.exp(rng.uniform(np.log(0.25), np.log(4.0), ng))) if m.aniso else g_sig
     g_x = rng.uniform(-0.5, 0.5, ng)
     g_y = rng.uniform(-0.5, 0.5, ng)
     g_z = rng.uniform(-300.0, 300.0, ng)
@@ -134,15 +137,20 @@ def _gen_block(m: EventModel, block: int, n_ev: int, ev0: int):
         "tx": np.concatenate([tx, g_tx]), "ty": np.concatenate([ty, g_ty]),
     }
     s_all = np.concatenate([sig, g_sig])
+    s_all_y = np.concatenate([sig_y, g_sig_y])
+    if m.aniso:
+        v_tx = 1e-6 * np.exp(rng.uniform(np.log(0.5), np.log(2.0), ev.size))
+        v_ty = 1e-6 * np.exp(rng.uniform(np.log(0.5), np.log(2.0), ev.size))
+    else:
+        v_tx = v_ty = np.full(ev.size, 1e-6)
     # ---- shuffle inside each event ----------------------------------------------------------
     key = rng.random(ev.size)
     order = np.lexsort((key, ev))
     out = {k: v[order].astype(np.float32) for k, v in cols.items()}
-    var = (s_all[order] ** 2).astype(np.float32)
-    out["var_x"] = var
-    out["var_y"] = var.copy()
-    out["var_tx"] = np.full(ev.size, 1e-6, dtype=np.float32)
-    out["var_ty"] = np.full(ev.size, 1e-6, dtype=np.float32)
+    out["var_x"] = (s_all[order] ** 2).astype(np.float32)
+    out["var_y"] = (s_all_y[order] ** 2).astype(np.float32)
+    out["var_tx"] = v_tx[order].astype(np.float32)
+    out["var_ty"] = v_ty[order].astype(np.float32)
     counts = np.bincount(ev, minlength=n_ev).astype(np.int64)
     truth = {
         "pv_event": pv_ev + ev0, "pv_x": pv_x, "pv_y": pv_y, "pv_z": pv_z,
@@ -197,6 +205,38 @@ def generate(m: EventModel, with_truth: bool = False) -> Dict[str, np.ndarray]:
     out["n_events"] = m.n_events
     if with_truth:
         out["truth"] = {k: np.concatenate([t[k] for t in truths]) for k in truths[0]} if truths else {}
+    return out
+
+
+def generate_range(m: EventModel, e0: int, e1: int, cache: Optional[dict] = None) -> Dict[str, np.ndarray]:
+    """The events [e0, e1) of model m as a stand-alone batch (offsets rebased to 0), drawing only the generator
+    blocks that overlap the range: identical to slice_events(generate(m), e0, e1) for e1 <= m.n_events.
+    `cache` (block index -> block) lets a caller reuse blocks between calls (bench.py --gpus N: every rank draws its
+    own share of one large batch)."""
+    if not 0 <= e0 <= e1:
+        raise ValueError("need 0 <= e0 <= e1")
+    parts = {k: [] for k in FIELDS}
+    counts = []
+    for block in range(e0 // BLOCK, (e1 + BLOCK - 1) // BLOCK if e1 > e0 else e0 // BLOCK):
+        if cache is not None and block in cache:
+            full, cnt = cache[block]
+        else:
+            full, cnt, _tr = _gen_block(m, block, BLOCK, block * BLOCK)
+            if cache is not None:
+                cache[block] = (full, cnt)
+        a, b = max(e0, block * BLOCK) - block * BLOCK, min(e1, (block + 1) * BLOCK) - block * BLOCK
+        first = np.concatenate([[0], np.cumsum(cnt)])
+        for k in FIELDS:
+            parts[k].append(full[k][first[a]:first[b]])
+        counts.append(cnt[a:b])
+    out = {k: np.ascontiguousarray(np.concatenate(parts[k])) if parts[k] else np.zeros(0, np.float32) for k in FIELDS}
+    cnt = np.concatenate(counts) if counts else np.zeros(0, np.int64)
+    off = np.zeros(e1 - e0 + 1, dtype=np.int64)
+    np.cumsum(cnt, out=off[1:])
+    if off[-1] >= 2 ** 31:
+        raise ValueError("track count exceeds int32 offsets")
+    out["offsets"] = off.astype(np.int32)
+    out["n_events"] = e1 - e0
     return out
 
 

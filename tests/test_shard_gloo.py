@@ -80,3 +80,46 @@ def test_sharded_equals_unsharded_over_gloo():
     m = np.arange(pos.shape[1])[None, :] < ref["n_vtx"][:, None]
     assert np.array_equal(pos[m], ref["vtx_pos"][m])
     assert trk.sum() == data["offsets"][-1] and abs(int(trk[0]) - int(trk[1])) < 600
+
+
+def test_bench_gpus_n_spawns_n_ranks_over_shard():
+    """`python bench.py --gpus N` (no torchrun around it) re-executes itself under torch.distributed.run with one rank
+    per GPU, refuses to start when the box has fewer devices, and every rank takes shard.event_range of ONE batch of
+    N x E events."""
+    import subprocess
+    import bench
+    from synth import events
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "3"], 29517)
+    assert cmd[0] == sys.executable and cmd[1:3] == ["-m", "torch.distributed.run"]
+    assert "--nnodes=1" in cmd and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29517"
+    assert cmd[-5].endswith("bench.py") and cmd[-4:] == ["--gpus", "4", "--steps", "3"]
+    import torch
+    if not torch.cuda.is_available():
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3"],
+                           capture_output=True, text=True, timeout=300)
+        assert r.returncode != 0 and "needs 2 CUDA devices" in (r.stderr + r.stdout)
+    # the batches of a 3-rank job: drawn independently by every rank, together exactly the 3 x E events
+    E, world = 400, 3
+    import dataclasses
+    whole = events.generate(dataclasses.replace(events.config(1, E), n_events=world * E))
+    counts = np.diff(whole["offsets"]).astype(np.int64)
+    parts = []
+    for rank in range(world):
+        seen = {}
+
+        def gather(mine, rank=rank, seen=seen):
+            assert np.array_equal(mine, counts[rank * E:(rank + 1) * E])          # the rank drew its nominal range
+            seen["called"] = True
+            return counts
+        d, m, (e0, e1), T = bench.gen_batch(1, E, rank, world, gather)
+        assert seen["called"] and m.n_events == world * E and T == whole["offsets"][-1]
+        parts.append((e0, e1, d))
+    assert parts[0][0] == 0 and parts[-1][1] == world * E
+    assert all(parts[k][1] == parts[k + 1][0] for k in range(world - 1))
+    for k in events.FIELDS:
+        assert np.array_equal(np.concatenate([d[k] for _a, _b, d in parts]), whole[k]), k
+    trk = [int(d["offsets"][-1]) for _a, _b, d in parts]
+    assert max(trk) - min(trk) <= 2 * counts.max()                                # equal track counts per GPU
+    d1, m1, rng1, T1 = bench.gen_batch(1, E)
+    assert rng1 == (0, E) and np.array_equal(d1["x"], whole["x"][:whole["offsets"][E]])
