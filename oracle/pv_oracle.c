@@ -780,6 +780,7 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
     for (int i = 0; i < n; ++i) trk_weight[t0 + i] = S->trk_seed[i] >= 0 ? S->best_w[i] : 0.0;
     if (dbg && dbg->trk_seed) for (int i = 0; i < n; ++i) dbg->trk_seed[t0 + i] = S->trk_seed[i];
     if (dbg && dbg->trk_w2) for (int i = 0; i < n; ++i) dbg->trk_w2[t0 + i] = S->second_w[i];
+    if (dbg && dbg->trk_w1) for (int i = 0; i < n; ++i) dbg->trk_w1[t0 + i] = S->best_w[i];
   }
 
   /* cleanup O8.  Duplicate removal: greedy sweep in seed (= z) order; duplicate iff

@@ -146,6 +146,7 @@ typedef struct pvo_debug {
   double *seed_pivot_min; /* [E][max_vtx] smallest Cholesky pivot / diagonal element over the iterations (<= 0: singular) */
   int32_t *seed_nact_min; /* [E][max_vtx] fewest active tracks in an iteration */
   double *trk_w2;         /* [T] flavour 1: the second largest final weight of the track over the fitted candidates */
+  double *trk_w1;         /* [T] flavour 1: the largest one (trk_weight before cleanup releases tracks) */
 } pvo_debug;
 
 /* The whole hot path a1..a6 over a batch.  Outputs (host, caller-owned):

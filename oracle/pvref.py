@@ -48,7 +48,7 @@ class Debug(C.Structure):
         ("trk_seed", C.c_void_p), ("seed_pos", C.c_void_p), ("seed_cov", C.c_void_p), ("seed_chi2", C.c_void_p),
         ("seed_ntrk", C.c_void_p), ("seed_niter", C.c_void_p), ("seed_fate", C.c_void_p), ("trace", C.c_void_p),
         ("seed_edge_last", C.c_void_p), ("seed_edge_any", C.c_void_p), ("seed_pivot_min", C.c_void_p),
-        ("seed_nact_min", C.c_void_p), ("trk_w2", C.c_void_p),
+        ("seed_nact_min", C.c_void_p), ("trk_w2", C.c_void_p), ("trk_w1", C.c_void_p),
     ]
 
 
@@ -300,7 +300,7 @@ def find(data: Dict[str, np.ndarray], p: Optional[Params] = None, debug: bool = 
             seed_chi2=np.zeros((E, mv)), seed_ntrk=np.zeros((E, mv), np.int32),
             seed_niter=np.zeros((E, mv), np.int32), seed_fate=np.zeros((E, mv), np.int32),
             seed_edge_last=np.full((E, mv), np.inf), seed_edge_any=np.full((E, mv), np.inf),
-            seed_pivot_min=np.full((E, mv), np.inf), seed_nact_min=np.zeros((E, mv), np.int32), trk_w2=np.zeros(T))
+            seed_pivot_min=np.full((E, mv), np.inf), seed_nact_min=np.zeros((E, mv), np.int32), trk_w2=np.zeros(T), trk_w1=np.zeros(T))
         if trace:
             d["trace"] = np.zeros((E, mv, TRACE_ITERS, TRACE_STRIDE))
         dbg = Debug()

@@ -143,3 +143,27 @@ def test_mv_pipeline_sanity_on_synthetic_events(oracle, cfg0):
     assert np.median(it) <= 4 and (it == 10).mean() < 0.02
     w = r["trk_weight"][r["trk_vertex"] >= 0]
     assert np.all(w > 0) and np.all(w < 1)
+
+
+def test_handworked_event_pins_the_association_glue(oracle):
+    """tests/golden/mv_handworked.json: window membership, the 'other candidates' part of the denominator of Eq. 19
+    (all candidates, listed or not), the followed candidate and the associated-track count of find_event."""
+    import json
+    import os
+    from synth import events
+    with open(os.path.join(os.path.dirname(__file__), "golden", "mv_handworked.json")) as f:
+        g = json.load(f)
+    ev = {k: np.asarray(g["event"][k], np.float32) for k in events.FIELDS}
+    data = events.from_lists([ev])
+    for c in g["cases"]:
+        p = oracle.mv_params(chi2_window=c["chi2_window"], **g["params"])
+        r = oracle.find(data, p, debug=True, n_hist_events=1)
+        d = r["debug"]
+        assert d["n_seeds"][0] == 2 and list(d["seed_z"][0, :2]) == [0.125, 10.125]          # delta = 0 (Eq. 5)
+        assert list(d["seed_bins"][0, :2, 2]) == [2200, 2240]
+        assert d["hist"][0, 2212] == 0                                                      # T5 is not histogrammed
+        assert list(d["trk_seed"]) == c["trk_seed"], c["_why"]
+        assert list(r["trk_vertex"]) == c["trk_seed"]
+        assert np.allclose(r["trk_weight"], c["trk_weight"], atol=2e-6, rtol=0), (c["_why"], r["trk_weight"])
+        assert np.allclose(d["trk_w2"], c["runner_up_weight"], atol=2e-6, rtol=0), (c["_why"], d["trk_w2"])
+        assert r["n_vtx"][0] == 2 and list(r["vtx_ntracks"][0, :2]) == c["vtx_ntracks"], c["_why"]
