@@ -18,6 +18,9 @@ its diagnostic taps), never at the size of the disagreement:
     or (singular flag) a Cholesky pivot within PIVOT_REL of zero.
   * N2 cleanup decisions (merge ratio, beamline distance, min tracks): a differing fate is accepted when the oracle's
     deciding quantity is within NEAR_REL of its cut, or the event holds an N1 / N2 vertex.
+  * N5 ill-conditioned fits: when the oracle's smallest Cholesky pivot (relative to its diagonal element) is below
+    PIVOT_REL the Newton step is a rounding-level numerator over a tiny pivot; a differing iteration count is then
+    handled like N1 (comparison with the trace entry at the GPU's count).
   * N3 argmax (multi-vertex flavour): accepted only when the oracle's two largest weights of that track differ by at
     most W_TOL.  N4 chi2 window: a track listed on one side only must carry a weight below W_TOL there.
 Without the GPU's taps (product kernels, debug=False) the same rules are applied from the final outputs: the
@@ -141,6 +144,11 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
                 near = (np.isfinite(cuts[0]) and abs(dchi2 - cuts[0]) <= NEAR_REL * cuts[0]) or \
                        (abs(dz - cuts[1]) <= NEAR_REL * cuts[1])
                 why = f"oracle |dchi2| {dchi2:.6g} (cut {cuts[0]:g}), |dz| {dz:.6g} (cut {cuts[1]:g}) at iteration {it}"
+                if not near and abs(rd["seed_pivot_min"][e, k]) <= PIVOT_REL:
+                    # N5: an ill-conditioned fit (two nearly parallel tracks): the step is a small difference divided by
+                    # a pivot of relative size <= PIVOT_REL, which fp32 cannot resolve to the convergence cut
+                    near = True
+                    why += f"; ill-conditioned fit, smallest relative pivot {rd['seed_pivot_min'][e, k]:.3g}"
                 if near:
                     ok = True
                     ref_pos[e, k] = trace[e, k, g_it - 1, 0:3]
@@ -229,7 +237,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
         rep["n_fitted_seeds"] = int((ks & (rn > 0)).sum())
         rep["n_niter_diff"] = int((g_it != r_it).sum())
         for e, k, gi, ri in zip(ee[g_it != r_it], kk[g_it != r_it], g_it[g_it != r_it], r_it[g_it != r_it]):
-            ok = 1 <= gi <= trace.shape[2] and near_cut(e, k, min(int(gi), int(ri)))
+            ok = 1 <= gi <= trace.shape[2] and (near_cut(e, k, min(int(gi), int(ri))) or abs(rd["seed_pivot_min"][e, k]) <= PIVOT_REL)
             if ok:
                 ref_pos[e, k] = trace[e, k, gi - 1, 0:3]
                 ref_cov[e, k] = trace[e, k, gi - 1, 3:9]

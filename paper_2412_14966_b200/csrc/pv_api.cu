@@ -118,7 +118,8 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
 
 // Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | fit-ready track records,
 // 32 B each, sorted by seed: one per track (explicit flavour) or up to two per track (multi-vertex flavour, a track
-// is listed once per seed in its chi2 window) | multi-vertex flavour: 8 B per track (largest weight and its seed).
+// is listed once per seed in its chi2 window) | explicit flavour: 4 B per track record (its Tukey weight, record order);
+// multi-vertex flavour: 8 B per track (largest weight and its seed).
 constexpr size_t WS_COUNTERS = 256;
 size_t ws_rec_bytes(int n_events, int max_vtx) { return (size_t)n_events * (size_t)max_vtx * sizeof(pvk::SeedRec); }
 size_t ws_trk_records(long long n_tracks, int flavour) {
@@ -126,7 +127,8 @@ size_t ws_trk_records(long long n_tracks, int flavour) {
 }
 size_t ws_bytes(int n_events, long long n_tracks, int max_vtx, int flavour) {
   size_t b = WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + ws_trk_records(n_tracks, flavour) * 32 + 16;
-  if (flavour == PV_FLAVOUR_MULTIVERTEX) b += (size_t)n_tracks * 8 + 16;
+  if (flavour == PV_FLAVOUR_MULTIVERTEX) b += (size_t)n_tracks * 8 + 16;     // best[]
+  else b += (size_t)n_tracks * 4 + 16;                                       // wrec[]
   return b;
 }
 
@@ -206,15 +208,17 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.seed_counter = reinterpret_cast<unsigned int*>(ws + 16);
   ka.rec = reinterpret_cast<pvk::SeedRec*>(ws + WS_COUNTERS);
   ka.trk_counter = reinterpret_cast<unsigned int*>(ws + 32);
+  ka.fit_counter = reinterpret_cast<unsigned int*>(ws + 48);
   ka.ftrk = reinterpret_cast<float4*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
   ka.trk_cap = (unsigned int)ws_trk_records(n_tracks, params->flavour);
   ka.best = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(ka.ftrk) + (size_t)ka.trk_cap * 32 + 16);
+  ka.wrec = reinterpret_cast<float*>(ka.best);                // the two flavours use the same place differently
   if (dbg) ka.dbg = *dbg;
 
   const bool timing = g_timing != 0;
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
-  CK(cudaMemsetAsync(workspace, 0, 48, stream));
+  CK(cudaMemsetAsync(workspace, 0, 64, stream));
   // a1..a4: persistent, one CTA per SM, one team of two warps per event
   int grid = di->sms;
   const int need = (n_events + teams - 1) / teams;

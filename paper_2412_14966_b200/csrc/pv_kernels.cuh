@@ -48,9 +48,8 @@ constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int FIT_UNROLL = PV_FIT_UNROLL;   // unroll of the track loop of one fit iteration
-constexpr int FIT_G = 2;            // lanes per vertex in the fit
-constexpr int FIT_VPW = 32 / FIT_G; // vertices per warp pass
-constexpr int FIT_KF = 16;          // track slots per lane in shared memory (fast path: <= FIT_G*FIT_KF tracks)
+constexpr int FIT_KF = 16;          // track slots per lane in shared memory: G lanes hold a seed of up to G * FIT_KF tracks
+constexpr int FIT_WIN = 256;        // seed records of one window of the fit (its sorted order is held as 8 bytes per lane)
 constexpr int FIT_BLOCK = 64;       // threads per CTA of fit_kernel (warps are autonomous; 12 KB of tracks per warp)
 constexpr int FIT_MIN_BLOCKS = 9;   // CTAs per SM: 9 x (24 KB + 1 KB reserved) fill the shared memory
 constexpr int FIT_MIN_BLOCKS_MV = 7;  // multi-vertex flavour: 32 KB of staged records per CTA
@@ -118,8 +117,10 @@ struct KArgs {
   int8_t* trk_vertex8;           // optional (host pipeline): trk_vertex as int8 (an event holds <= 32 PVs), nullptr = not written
   unsigned int* evt_counter;     // workspace: next event of the persistent seed kernel
   unsigned int* seed_counter;    // workspace: seed records written so far
+  unsigned int* fit_counter;     // workspace: next window of seed records of the fit kernel
   SeedRec* rec;                  // workspace: [n_events * max_vtx]
   float4* ftrk;                  // workspace: [T or 2 T][2] fit-ready track records sorted by seed
+  float* wrec;                   // workspace, explicit flavour: [T] Tukey weight of every track record (record order)
   unsigned long long* best;      // workspace, multi-vertex flavour: [T] largest weight of the track << 32 | 31 - seed
   unsigned int* trk_counter;     // workspace, multi-vertex flavour: track records allocated so far
   unsigned int trk_cap;          // capacity of ftrk in records
@@ -404,8 +405,12 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
   Trk T;
   const float zl = R.z - zsv;
   T.tx = R.tx; T.ty = R.ty;
-  T.x0 = fmaf(-zl, R.tx, R.x - sx);
-  T.y0 = fmaf(-zl, R.ty, R.y - sy);
+  // the change of frame in double, once per record: for a state given far from the vertex (x ~ 30 mm at 150 mm and a
+  // slope of 0.2) x - zl tx cancels to O(0.1 mm), and the fp32 rounding of the large terms (2e-6 mm) is what the
+  // Tukey weights of a non-converged fit amplify
+  const double zld = (double)R.z - (double)zsv;
+  T.x0 = (float)fma(-zld, (double)R.tx, (double)R.x - (double)sx);
+  T.y0 = (float)fma(-zld, (double)R.ty, (double)R.y - (double)sy);
   const float Vx = var_at(R.vx, R.vtx, cx, -zl);
   const float Vy = var_at(R.vy, R.vty, cy, -zl);
   const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
@@ -925,12 +930,14 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   }
   __syncwarp();
   auto place = [&](const int i, const RawTrk& R, const bool from_memory, const int s) {
-    if (i < n) {
-      A.trk_vertex[t0 + i] = s;                            // scratch: seed index, read back by cleanup_kernel
-      if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
-    }
     const unsigned m = __match_any_sync(FULL, s);
     const int rank = __popc(m & lanemask_lt());
+    if (i < n) {
+      // scratch for cleanup_kernel: seed index | position of the track's record within the event << 5 (the fit
+      // leaves the track's weight at that record position)
+      A.trk_vertex[t0 + i] = s >= 0 ? (s | ((cur[s] + rank) << 5)) : -1;
+      if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
+    }
     if (s >= 0) {
       RawTrk Q = R;
       if (from_memory) {
@@ -1107,14 +1114,21 @@ __device__ __forceinline__ void store_vertex(const KArgs& A, size_t o, float x, 
   A.vtx_chi2[o] = chi2; A.vtx_ntracks[o] = ntrk; A.vtx_niter[o] = niter;
 }
 
-// ---- fit_kernel: a5, FIT_G lanes per seed (R-12) ---------------------------------------------------
-// Warps are autonomous (no CTA barrier): a warp takes a window of 32 seed records (one per lane), sorts them by
-// track count with a shuffle bitonic sort (so the FIT_VPW seeds it fits together need the same number of
-// track slots), and fits them in 32 / FIT_VPW passes.  The tracks of a pass are copied once (cp.async, 16 + 8
-// bytes of each fit-ready record) into the warp's shared-memory slice, laid out [slot][lane] so that every
-// iteration reads them back conflict-free; with two lanes per seed one shuffle level reduces the normal
-// equations, and every lane solves its seed's 3x3 system in closed form.
+// ---- fit_kernel: a5 (R-12) ---------------------------------------------------------------------------
+// Warps are autonomous (no CTA barrier).  A warp takes a WINDOW of up to 256 seed records, counting-sorts them by
+// (lanes per seed, track slots per lane) and then works through the sorted list as a queue:
+//   * G = 2, 4, 8, 16 or 32 lanes per seed (seeds of up to 32, 64, ... 512 tracks), 32 / G seeds in flight; the
+//     tracks of a seed sit in the shared-memory columns of its lanes, laid out [slot][lane] so that every iteration
+//     reads them back conflict-free (cp.async of 16 + 8 bytes of each fit-ready record);
+//   * one TICK of the warp is one Newton-Raphson iteration of every seed in flight.  A seed that has converged
+//     spends one more tick writing its track weights (the same arithmetic at the position its last iteration used,
+//     hence the same bits), stores its vertex, and its lanes immediately take the next record of the queue: a seed
+//     costs its own iterations, not those of the slowest of its neighbours (the round-1 kernel iterated 16 seeds
+//     until the last had converged: 9.3 iterations on average for a mean of 5.5);
+//   * because the queue is sorted, the seeds in flight need about the same number of slots, and a lane's column
+//     only ever holds live tracks below a high-water mark (dead tracks above it), so a tick has no per-slot test.
 // Results go to slot (event, seed index) of the vertex arrays; cleanup_kernel compacts them in place.
+// Every seed's result depends only on its own tracks and on G: bit-reproducible whatever the scheduling.
 __device__ __forceinline__ Trk read_track(const KArgs& A, int rec, int& idx) {
   const float4 a = __ldg(A.ftrk + 2 * (size_t)rec), b = __ldg(A.ftrk + 2 * (size_t)rec + 1);
   Trk T;
@@ -1140,6 +1154,248 @@ __device__ __forceinline__ void claim_track(const KArgs& A, int idx, float w, in
   atomicMax(A.best + idx, ((unsigned long long)__float_as_uint(w) << 32) | (unsigned)(31 - k));
 }
 
+__device__ __forceinline__ void sums_reduce_rt(Sums& S, const int G) {
+#pragma unroll 1
+  for (int o = G >> 1; o > 0; o >>= 1) {
+    S.a += __shfl_xor_sync(FULL, S.a, o);
+    S.b += __shfl_xor_sync(FULL, S.b, o);
+    S.c += __shfl_xor_sync(FULL, S.c, o);
+    S.d += __shfl_xor_sync(FULL, S.d, o);
+    S.e += __shfl_xor_sync(FULL, S.e, o);
+    S.gx += __shfl_xor_sync(FULL, S.gx, o);
+    S.gy += __shfl_xor_sync(FULL, S.gy, o);
+    S.gz += __shfl_xor_sync(FULL, S.gz, o);
+    S.chi2 += __shfl_xor_sync(FULL, S.chi2, o);
+    S.nact += __shfl_xor_sync(FULL, S.nact, o);
+  }
+}
+
+template <int FLAV>
+__device__ __forceinline__ void store_dead(float4 (*SA)[32], typename FitB<FLAV>::type (*SB)[32], int s, int lane, const Trk& dead) {
+  SA[s][lane] = make_float4(dead.x0, dead.y0, dead.tx, dead.ty);
+  if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) SB[s][lane] = make_float4(dead.Wx, dead.Wy, 0.0f, dead.oth);
+  else SB[s][lane] = make_float2(dead.Wx, dead.Wy);
+}
+
+enum { FS_EMPTY = 0, FS_LOAD = 1, FS_ITER = 2, FS_FINAL = 3, FS_DONE = 4 };
+#ifndef PV_FIT_LOADWAIT
+#define PV_FIT_LOADWAIT 0        // ticks a group sits out after starting the copy of its next seed before it waits for the data
+                                 // (measured on configs[1]: 0 -> 0.387 ms, 1 -> 0.405 ms; an L2 prefetch one seed ahead did not help)
+#endif
+
+// One phase of a window: the records order[pb .. pe) of the window starting at record wb, G = 1 << lg lanes per seed.
+// ord0 / ord1: the sorted window (record index within the window, one byte each), 8 entries per lane.
+// Explicit flavour: every iteration leaves its Tukey weights at the tracks' record positions in wrec[], so the weights
+// of the last iteration are simply what is there when the seed stops (cleanup_kernel moves them to track order);
+// a converged seed frees its column in the same tick.  Multi-vertex flavour: one more tick (FS_FINAL) recomputes the
+// weights at the position the last iteration used and lets every track claim its best vertex.
+template <int FLAV>
+__device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, float4 (*SA)[32],
+                                          typename FitB<FLAV>::type (*SB)[32], const int lg, const int wb, const int pb,
+                                          const int pe, const unsigned ord0, const unsigned ord1, int& filled,
+                                          const int lane) {
+  using BT = typename FitB<FLAV>::type;
+  const int G = 1 << lg, j = lane & (G - 1);
+  const unsigned below_group = (1u << (lane - j)) - 1u;        // lanes of the groups before mine
+  const unsigned leaders = lg == 5 ? 1u : 0xffffffffu / ((1u << G) - 1u);   // lane 0 of every group
+  const Trk dead = dead_track(P);
+  int qnext = pb;                                              // next queue position to hand out (warp-uniform)
+  int st = FS_DONE;                                            // every group starts by taking a record
+  int loadwait = 0;
+  int4 cur = make_int4(0, 0, 0, 0), nxt = make_int4(0, 0, 0, 0);
+  // the record after the current one is fetched one seed ahead, so taking it never waits on memory
+  auto fetch = [&](const unsigned wantm, const bool mine) {
+    const int q = qnext + __popc(wantm & below_group);
+    qnext += __popc(wantm);
+    const int qq = min(q, 255);
+    const unsigned v0 = __shfl_sync(FULL, ord0, qq >> 3), v1 = __shfl_sync(FULL, ord1, qq >> 3);
+    const unsigned idx = (((qq & 4) ? v1 : v0) >> (8 * (qq & 3))) & 0xffu;
+    if (mine) {
+      nxt = make_int4(0, 0, 0, 0);
+      if (q < pe) nxt = __ldg(reinterpret_cast<const int4*>(A.rec) + wb + idx);
+    }
+  };
+  fetch(leaders, true);
+  float ax = 0.0f, ay = 0.0f, az = 0.0f;
+  float lx = 0.0f, ly = 0.0f, lz = 0.0f;                   // position the weights of the last iteration were taken at
+  float C[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+  float chi2 = 0.0f, nact = 0.0f, nvalid = 0.0f;
+  int niter = 0, myslots = 0;
+#pragma unroll 1
+  for (;;) {
+    // ---- groups without a seed take their prefetched record, start the copy of its tracks, prefetch another record
+    const bool sw = st == FS_DONE;
+    const unsigned swm = __ballot_sync(FULL, sw) & leaders;
+    if (swm) {
+      if (sw) cur = nxt;
+      fetch(swm, sw);
+      if (sw) {
+        const int m = cur.y >> 5;
+        st = FS_EMPTY; myslots = 0;
+        if (m > 0) {
+          const int mine = m > j ? (m - j + G - 1) >> lg : 0;   // my tracks: j, j + G, ... < m
+          const float4* q = A.ftrk + 2 * (size_t)(cur.z + j);
+          unsigned da = (unsigned)__cvta_generic_to_shared(&SA[0][lane]);
+          unsigned db = (unsigned)__cvta_generic_to_shared(&SB[0][lane]);
+          const char* qc = reinterpret_cast<const char*>(q);
+          const unsigned qstep = 32u << lg;                    // bytes from my track to my next one
+#pragma unroll 2
+          for (int s = 0; s < mine; ++s) {
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(da), "l"(qc) : "memory");
+            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX)
+              asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(db), "l"(qc + 16) : "memory");
+            else
+              asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(db), "l"(qc + 16) : "memory");
+            qc += qstep; da += 32 * sizeof(float4); db += 32 * sizeof(BT);
+          }
+#pragma unroll 1
+          for (int s = mine; s < filled; ++s) store_dead<FLAV>(SA, SB, s, lane, dead);   // above my tracks: dead
+          filled = mine; myslots = mine;
+          st = FS_LOAD; loadwait = PV_FIT_LOADWAIT;
+          ax = ay = az = 0.0f; niter = 0;
+        }
+      }
+    }
+    // ---- has my copy landed?  (a group sits out PV_FIT_LOADWAIT ticks first, so the wait finds the data there)
+    if (st == FS_LOAD) {
+      if (loadwait > 0) --loadwait;
+      else {
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        st = FS_ITER;
+        if (P.unit_weights) {                                // unit weights: the active tracks are the usable ones
+          nvalid = 0.0f;
+#pragma unroll 1
+          for (int s = 0; s < myslots; ++s) nvalid += (SB[s][lane].x > 0.0f) ? 1.0f : 0.0f;
+        }
+      }
+    }
+    __syncwarp();
+    if (!__any_sync(FULL, st != FS_EMPTY)) break;            // queue empty and nothing in flight
+    const bool act = st == FS_ITER || st == FS_FINAL;
+    const int nslot_w = __reduce_max_sync(FULL, act ? myslots : 0);
+    if (nslot_w == 0) continue;                              // only copies in flight
+    const bool fin = st == FS_FINAL;
+    const float px = fin ? lx : ax, py = fin ? ly : ay, pz = fin ? lz : az;
+    const int e = cur.x, k = cur.y & 31;
+    Sums S;
+    sums_zero(S);
+    float nass = 0.0f;                                       // multi-vertex flavour: tracks with final weight >= 1/2
+    float* wp = A.wrec + cur.z + j;                          // explicit flavour: my tracks' places in wrec[]
+    const int wslots = st == FS_ITER ? myslots : 0;
+#pragma unroll FIT_UNROLL
+    for (int s = 0; s < nslot_w; ++s) {
+      const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
+      float w = track_accum<FLAV>(T, px, py, pz, P, S);
+      if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+        if (fin && s < myslots && !track_is_dead(T, P)) {    // the weights of the last iteration are the outputs
+          claim_track(A, __float_as_int(SB[s][lane].z), w, k);
+          nass += (w >= 0.5f) ? 1.0f : 0.0f;
+        }
+      } else {
+        if (s < wslots) wp[s << lg] = w;                     // a dead track has w = 0 (unit weights: see below)
+      }
+    }
+    if (P.unit_weights) {
+      S.nact = nvalid;
+      if (FLAV != PV_FLAVOUR_MULTIVERTEX)                    // unit weights give a dead (R-7) track w = 1: its output is 0
+        for (int s = 0; s < wslots; ++s)
+          if (!(SB[s][lane].x > 0.0f)) wp[s << lg] = 0.0f;
+    }
+    sums_reduce_rt(S, G);
+    if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll 1
+      for (int o = G >> 1; o > 0; o >>= 1) nass += __shfl_xor_sync(FULL, nass, o);
+    }
+    bool store = false;
+    if (st == FS_ITER) {
+      float dx, dy, dzs, dchi2;
+      if (!newton_step(S, dx, dy, dzs, dchi2, C)) {            // singular: the vertex is dropped (R-12)
+        if (j == 0) {
+          A.vtx_niter[(size_t)e * P.max_vtx + k] = -1;
+          atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT);
+        }
+        st = FS_DONE;
+      } else {
+        lx = ax; ly = ay; lz = az;
+        ax += dx; ay += dy; az += dzs;
+        chi2 = S.chi2; nact = S.nact; ++niter;
+        if ((fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) || niter >= P.max_iter) {
+          st = FLAV == PV_FLAVOUR_MULTIVERTEX ? FS_FINAL : FS_DONE;
+          store = FLAV != PV_FLAVOUR_MULTIVERTEX;
+        }
+      }
+    } else if (fin) {
+      st = FS_DONE;
+      store = true;
+    }
+    if (store && j == 0) {
+      const float zsv = __int_as_float(cur.w);
+      const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);    // "xy position ... using the known beamline"
+      const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+      store_vertex(A, (size_t)e * P.max_vtx + k, sx + ax, sy + ay, zsv + az, C, chi2, (int)(FLAV ? nass : nact), niter);
+    }
+  }
+}
+
+// Seeds with more tracks than 32 lanes x FIT_KF slots hold (> 512; only constructed events): the whole warp strides
+// over the seed's records in global memory (contiguous, L1-resident after the first iteration).
+template <int FLAV>
+__device__ void fit_huge(const KParams& P, const KArgs& A, const int4 r, const int lane) {
+  const int be = r.x, bk = r.y & 31, bm_ = r.y >> 5, bo = r.z;
+  const float bz = __int_as_float(r.w);
+  const float bx = __fmaf_rn(P.beam_tx, bz, P.beam_x), by = __fmaf_rn(P.beam_ty, bz, P.beam_y);
+  float qx = 0.0f, qy = 0.0f, qz = 0.0f;               // current position (local frame)
+  float px = 0.0f, py = 0.0f, pz = 0.0f;               // position the last weights were taken at
+  float C[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+  bool bsing = false;
+  int bit = 0;
+  float bchi2 = 0.0f, bnact = 0.0f;
+#pragma unroll 1
+  for (int it = 1; it <= P.max_iter; ++it) {
+    Sums S;
+    sums_zero(S);
+    float nv = 0.0f;
+    for (int t = lane; t < bm_; t += 32) {
+      int idx;
+      const Trk U = read_track(A, bo + t, idx);
+      nv += track_is_dead(U, P) ? 0.0f : 1.0f;
+      track_accum<FLAV>(U, qx, qy, qz, P, S);
+    }
+    if (P.unit_weights) S.nact = nv;
+    sums_reduce_rt(S, 32);
+    float dx, dy, dzs, dchi2;
+    if (!newton_step(S, dx, dy, dzs, dchi2, C)) { bsing = true; break; }
+    px = qx; py = qy; pz = qz;
+    qx += dx; qy += dy; qz += dzs;
+    bchi2 = S.chi2; bnact = S.nact; bit = it;
+    if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
+  }
+  const size_t o = (size_t)be * P.max_vtx + bk;
+  float bass = 0.0f;
+  if (!bsing) {
+    for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration, recomputed
+      int idx;
+      const Trk U = read_track(A, bo + t, idx);
+      Sums dummy;
+      sums_zero(dummy);
+      const float w = track_accum<FLAV>(U, px, py, pz, P, dummy);
+      if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+        if (!track_is_dead(U, P)) { claim_track(A, idx, w, bk); bass += (w >= 0.5f) ? 1.0f : 0.0f; }
+      } else {
+        A.wrec[bo + t] = track_is_dead(U, P) ? 0.0f : w;
+      }
+    }
+  }
+  if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) bass += __shfl_xor_sync(FULL, bass, o2);
+  }
+  if (lane == 0) {
+    if (bsing) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
+    else store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)(FLAV ? bass : bnact), bit);
+  }
+}
+
 template <int FLAV>
 __global__ void __launch_bounds__(FIT_BLOCK, FLAV ? FIT_MIN_BLOCKS_MV : FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
@@ -1147,212 +1403,80 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
   __shared__ __align__(16) float4 s_a[FIT_BLOCK / 32][FIT_KF][32];   // {x0, y0, tx, ty}
   __shared__ __align__(16) BT s_b[FIT_BLOCK / 32][FIT_KF][32];       // {Wx, Wy} or {Wx, Wy, track index, oth}
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int j = lane % FIT_G, gl = lane / FIT_G;
   float4(*SA)[32] = s_a[warp];
   BT(*SB)[32] = s_b[warp];
   const int total = (int)*A.seed_counter;
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
-  const int wg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  // the seed records of the NEXT window are loaded one window ahead (an L2 prefetch of their track lines was
-  // measured slower: 0.408 vs 0.396 ms, and cost 270 MB of DRAM reads evicted before use)
-  int4 wr_next = make_int4(0, 0, 0, 0);
-  if (wg * 32 + lane < total) wr_next = __ldg(reinterpret_cast<const int4*>(A.rec) + wg * 32 + lane);
+  // window size: one window per warp when the batch allows (all warps then finish together), at most FIT_WIN
+  int win = (total + nwarps - 1) / nwarps;
+  win = min(max((win + 31) & ~31, 32), FIT_WIN);
+  const int nwin = (total + win - 1) / win;
+  const Trk dead = dead_track(P);
+  int filled = FIT_KF;                                       // slots of my column that may hold something else than a dead track
 #pragma unroll 1
-  for (int wb = wg * 32; wb < total; wb += nwarps * 32) {
-    const int4 wr = wr_next;
+  for (;;) {
+    int w = 0;
+    if (lane == 0) w = (int)atomicAdd(A.fit_counter, 1u);
+    w = __shfl_sync(FULL, w, 0);
+    if (w >= nwin) break;
+    const int wb = w * win, wn = min(win, total - wb);
+    // ---- counting sort of the window's records by key = phase * 16 + 16 - slots per lane (scratch: rows 0, 1 of SA)
+    int* hist = reinterpret_cast<int*>(&SA[0][0]);            // 96 counters, then their exclusive scan
+    uint8_t* ordb = reinterpret_cast<uint8_t*>(&SA[1][0]);     // the sorted window, one byte per record
+    hist[lane] = 0; hist[lane + 32] = 0; hist[lane + 64] = 0;
+    __syncwarp();
+    int key[FIT_WIN / 32], pos[FIT_WIN / 32];
+#pragma unroll
+    for (int i = 0; i < FIT_WIN / 32; ++i) {
+      const int r = i * 32 + lane;
+      key[i] = -1; pos[i] = 0;
+      if (r < wn) {
+        const int m = __ldg(&A.rec[wb + r].k_cnt) >> 5;
+        if (m > 0) {
+          const int ph = m <= 2 * FIT_KF ? 0 : m <= 4 * FIT_KF ? 1 : m <= 8 * FIT_KF ? 2 : m <= 16 * FIT_KF ? 3 : m <= 32 * FIT_KF ? 4 : 5;
+          const int slots = ph < 5 ? (m + (2 << ph) - 1) >> (ph + 1) : 1;
+          key[i] = ph * 16 + 16 - slots;                         // within a phase: most slots first, so the drain at the
+                                                                   // end of the phase (idle lanes) runs on short ticks
+          pos[i] = atomicAdd(&hist[key[i]], 1);
+        }
+      }
+    }
+    __syncwarp();
+    int pendv;                                                // lane ph < 5: end of phase ph in the sorted window; lane 5: all
     {
-      const int nb = wb + nwarps * 32 + lane;
-      wr_next = make_int4(0, 0, 0, 0);
-      if (nb < total) wr_next = __ldg(reinterpret_cast<const int4*>(A.rec) + nb);
-    }
-    // bitonic sort of (track count, lane) keys, ascending; absent records (count 0) come first
-    int key = ((wr.y >> 5) << 5) | lane;
-#pragma unroll
-    for (int kk = 2; kk <= 32; kk <<= 1) {
-#pragma unroll
-      for (int jj = kk >> 1; jj > 0; jj >>= 1) {
-        const int other = __shfl_xor_sync(FULL, key, jj);
-        const bool up = ((lane & kk) == 0) == ((lane & jj) == 0);     // keep the smaller key
-        key = up ? min(key, other) : max(key, other);
-      }
-    }
-#pragma unroll 1
-    for (int pass = 0; pass < 32 / FIT_VPW; ++pass) {
-      const int src = __shfl_sync(FULL, key, pass * FIT_VPW + gl) & 31;   // lane holding my group's record
-      int4 r;
-      r.x = __shfl_sync(FULL, wr.x, src); r.y = __shfl_sync(FULL, wr.y, src);
-      r.z = __shfl_sync(FULL, wr.z, src); r.w = __shfl_sync(FULL, wr.w, src);
-      const int e = r.x, k = r.y & 31;
-      int m = r.y >> 5;
-      const bool vact = m > 0;                               // every real seed holds >= 2 tracks
-      if (!__any_sync(FULL, vact)) continue;
-      const float zsv = __int_as_float(r.w);
-      const bool big = m > FIT_G * FIT_KF;
-      if (big) m = 0;
-      const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
-      const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-      int mmax = m;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) mmax = max(mmax, __shfl_xor_sync(FULL, mmax, o));
-      const int nslot = (mmax + FIT_G - 1) / FIT_G;          // warp-uniform number of track slots in use
-      // ---- stage the tracks of this pass: slot s of my lane holds track j + FIT_G s of my seed, or a dead track
-      __syncwarp();                                          // the previous pass has finished reading the slice
-      {
-        const Trk dead = dead_track(P);
-#pragma unroll 1
-        for (int s = 0; s < nslot; ++s) {
-          const int t = j + FIT_G * s;
-          if (t < m) {
-            const float4* q = A.ftrk + 2 * (size_t)(r.z + t);
-            const unsigned da = (unsigned)__cvta_generic_to_shared(&SA[s][lane]);
-            const unsigned db = (unsigned)__cvta_generic_to_shared(&SB[s][lane]);
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(da), "l"(q) : "memory");
-            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX)
-              asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(db), "l"(q + 1) : "memory");
-            else
-              asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(db), "l"(q + 1) : "memory");
-          } else {
-            SA[s][lane] = make_float4(dead.x0, dead.y0, dead.tx, dead.ty);
-            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) SB[s][lane] = make_float4(dead.Wx, dead.Wy, 0.0f, dead.oth);
-            else SB[s][lane] = make_float2(dead.Wx, dead.Wy);
-          }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-      }
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      const int h0 = hist[3 * lane], h1 = hist[3 * lane + 1], h2 = hist[3 * lane + 2];
+      const int tot = h0 + h1 + h2;
+      const int inc = warp_incl_scan(tot, lane);
       __syncwarp();
-      float nvalid = 0.0f;                                   // usable tracks (unit-weight mode: the active count)
-      if (P.unit_weights) {
+      hist[3 * lane] = inc - tot; hist[3 * lane + 1] = inc - tot + h0; hist[3 * lane + 2] = inc - tot + h0 + h1;
+      __syncwarp();
+      const int nvalid_w = __shfl_sync(FULL, inc, 31);
+      pendv = lane < 5 ? hist[(lane + 1) * 16] : nvalid_w;
+    }
+#pragma unroll
+    for (int i = 0; i < FIT_WIN / 32; ++i)
+      if (key[i] >= 0) ordb[hist[key[i]] + pos[i]] = (uint8_t)(i * 32 + lane);
+    __syncwarp();
+    const unsigned ord0 = reinterpret_cast<const unsigned*>(ordb)[2 * lane], ord1 = reinterpret_cast<const unsigned*>(ordb)[2 * lane + 1];
+    __syncwarp();
 #pragma unroll 1
-        for (int s = 0; s < nslot; ++s) nvalid += (SB[s][lane].x > 0.0f) ? 1.0f : 0.0f;
-#pragma unroll
-        for (int o = FIT_G / 2; o > 0; o >>= 1) nvalid += __shfl_xor_sync(FULL, nvalid, o);
-      }
-      float ax = 0.0f, ay = 0.0f, az = 0.0f;
-      float lx = 0.0f, ly = 0.0f, lz = 0.0f;               // position the weights of the last iteration were taken at
-      bool run = vact && !big;
-      bool sing = false;
-      int niter = 0;
-      float C[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
-      float chi2 = 0.0f, nact = 0.0f;
+    for (int s = 0; s < max(filled, 2); ++s) store_dead<FLAV>(SA, SB, s, lane, dead);
+    filled = 0;
+    __syncwarp();
+    // ---- the queue, phase by phase
+    int pb = 0;
 #pragma unroll 1
-      for (int it = 1; it <= P.max_iter; ++it) {
-        Sums S;
-        sums_zero(S);
-#pragma unroll FIT_UNROLL
-        for (int s = 0; s < nslot; ++s) {
-          const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
-          track_accum<FLAV>(T, ax, ay, az, P, S);
-        }
-        sums_reduce<FIT_G>(S);
-        if (P.unit_weights) S.nact = nvalid;
-        if (run) {
-          float dx, dy, dzs, dchi2;
-          if (!newton_step(S, dx, dy, dzs, dchi2, C)) {
-            sing = true; run = false;
-          } else {
-            lx = ax; ly = ay; lz = az;
-            ax += dx; ay += dy; az += dzs;
-            chi2 = S.chi2; nact = S.nact; niter = it;
-            if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) run = false;
-          }
-        }
-        if (!__any_sync(FULL, run)) break;
-      }
-      const bool okv = vact && !big && !sing;
-      float nass = 0.0f;                                     // multi-vertex flavour: tracks with final weight >= 1/2
-      if (okv) {
-#pragma unroll 4
-        for (int t = j; t < m; t += FIT_G) {               // weights of the last iteration: the same arithmetic again
-          const int s = t / FIT_G;
-          const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
-          Sums dummy;
-          sums_zero(dummy);
-          const float w = track_accum<FLAV>(T, lx, ly, lz, P, dummy);
-          if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
-            if (!track_is_dead(T, P)) {
-              claim_track(A, __float_as_int(SB[s][lane].z), w, k);
-              nass += (w >= 0.5f) ? 1.0f : 0.0f;
-            }
-          } else {
-            const int idx = __float_as_int(__ldg(reinterpret_cast<const float*>(A.ftrk + 2 * (size_t)(r.z + t) + 1) + 2));
-            A.trk_weight[idx] = track_is_dead(T, P) ? 0.0f : w;
-          }
-        }
-      }
-      if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
-#pragma unroll
-        for (int o = FIT_G / 2; o > 0; o >>= 1) nass += __shfl_xor_sync(FULL, nass, o);
-      }
-      if (vact && !big && j == 0) {
-        const size_t o = (size_t)e * P.max_vtx + k;
-        if (sing) { A.vtx_niter[o] = -1; atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT); }
-        else store_vertex(A, o, sx + ax, sy + ay, zsv + az, C, chi2, (int)(FLAV ? nass : nact), niter);
-      }
-      // Seeds with more tracks than the shared-memory slots hold: the whole warp strides over the seed's
-      // records (contiguous, L1-resident after the first iteration).
-      unsigned bigm = __ballot_sync(FULL, vact && big && j == 0);
-      while (bigm) {
-        const int bsrc = __ffs(bigm) - 1;
-        bigm &= bigm - 1;
-        const int be = __shfl_sync(FULL, e, bsrc), bk = __shfl_sync(FULL, k, bsrc);
-        const int bm_ = __shfl_sync(FULL, r.y, bsrc) >> 5, bo = __shfl_sync(FULL, r.z, bsrc);
-        const float bz = __shfl_sync(FULL, zsv, bsrc);
-        const float bx = __fmaf_rn(P.beam_tx, bz, P.beam_x), by = __fmaf_rn(P.beam_ty, bz, P.beam_y);
-        float qx = 0.0f, qy = 0.0f, qz = 0.0f;               // current position (local frame)
-        float px = 0.0f, py = 0.0f, pz = 0.0f;               // position the last weights were taken at
-        bool bsing = false;
-        int bit = 0;
-        float bchi2 = 0.0f, bnact = 0.0f;
+    for (int ph = 0; ph < 5; ++ph) {
+      const int pe = __shfl_sync(FULL, pendv, ph);
+      if (pe > pb) fit_phase<FLAV>(P, A, SA, SB, ph + 1, wb, pb, pe, ord0, ord1, filled, lane);
+      pb = pe;
+    }
+    const int pall = __shfl_sync(FULL, pendv, 5);
 #pragma unroll 1
-        for (int it = 1; it <= P.max_iter; ++it) {
-          Sums S;
-          sums_zero(S);
-          float nv = 0.0f;
-          for (int t = lane; t < bm_; t += 32) {
-            int idx;
-            const Trk U = read_track(A, bo + t, idx);
-            nv += track_is_dead(U, P) ? 0.0f : 1.0f;
-            track_accum<FLAV>(U, qx, qy, qz, P, S);
-          }
-          sums_reduce<32>(S);
-          if (P.unit_weights) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) nv += __shfl_xor_sync(FULL, nv, o);
-            S.nact = nv;
-          }
-          float dx, dy, dzs, dchi2;
-          if (!newton_step(S, dx, dy, dzs, dchi2, C)) { bsing = true; break; }
-          px = qx; py = qy; pz = qz;
-          qx += dx; qy += dy; qz += dzs;
-          bchi2 = S.chi2; bnact = S.nact; bit = it;
-          if (fabsf(dchi2) < P.conv_dchi2 && fabsf(dzs) < P.conv_dz) break;
-        }
-        const size_t o = (size_t)be * P.max_vtx + bk;
-        float bass = 0.0f;
-        if (!bsing) {
-          for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration, recomputed
-            int idx;
-            const Trk U = read_track(A, bo + t, idx);
-            Sums dummy;
-            sums_zero(dummy);
-            const float w = track_accum<FLAV>(U, px, py, pz, P, dummy);
-            if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
-              if (!track_is_dead(U, P)) { claim_track(A, idx, w, bk); bass += (w >= 0.5f) ? 1.0f : 0.0f; }
-            } else {
-              A.trk_weight[idx] = track_is_dead(U, P) ? 0.0f : w;
-            }
-          }
-        }
-        if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
-#pragma unroll
-          for (int o2 = 16; o2 > 0; o2 >>= 1) bass += __shfl_xor_sync(FULL, bass, o2);
-        }
-        if (lane == 0) {
-          if (bsing) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
-          else store_vertex(A, o, bx + qx, by + qy, bz + qz, C, bchi2, (int)(FLAV ? bass : bnact), bit);
-        }
-      }
+    for (int q = pb; q < pall; ++q) {
+      const unsigned v0 = __shfl_sync(FULL, ord0, q >> 3), v1 = __shfl_sync(FULL, ord1, q >> 3);
+      const unsigned idx = (((q & 4) ? v1 : v0) >> (8 * (q & 3))) & 0xffu;
+      fit_huge<FLAV>(P, A, __ldg(reinterpret_cast<const int4*>(A.rec) + wb + idx), lane);
     }
   }
 }
@@ -1362,7 +1486,7 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
 // arrays), the duplicate sweep runs on shuffles, survivors are compacted in place in z order, and every
 // track gets its final vertex index (weight 0 when it has none).
 #ifndef PV_CLEANUP_MIN_BLOCKS
-#define PV_CLEANUP_MIN_BLOCKS 8
+#define PV_CLEANUP_MIN_BLOCKS 6
 #endif
 template <bool DBG, int FLAV>
 __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(const __grid_constant__ KParams P,
@@ -1465,17 +1589,21 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   // final per-track outputs; tracks of rejected vertices are released (R-9)
   auto finish = [&](int i, int s, unsigned long long b) {
     float w = 0.0f;
+    int pos = 0;
     if (FLAV == PV_FLAVOUR_MULTIVERTEX) {                  // R-13: the track follows the seed with its largest weight
       w = __uint_as_float((unsigned)(b >> 32));
       s = w > 0.0f ? 31 - (int)(b & 31ull) : -1;
       if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
+    } else if (s >= 0) {                                   // explicit flavour: seed | record position << 5 (seed_kernel)
+      pos = s >> 5;
+      s &= 31;
     }
     int vtx = -1;
     if (s >= 0 && ((kept >> s) & 1u)) vtx = __popc(kept & ((1u << s) - 1u));
     A.trk_vertex[t0 + i] = vtx;
     if (A.trk_vertex8) A.trk_vertex8[t0 + i] = (int8_t)vtx;
-    if (FLAV == PV_FLAVOUR_MULTIVERTEX) A.trk_weight[t0 + i] = vtx >= 0 ? w : 0.0f;
-    else if (vtx < 0) A.trk_weight[t0 + i] = 0.0f;
+    if (FLAV != PV_FLAVOUR_MULTIVERTEX && vtx >= 0) w = A.wrec[t0 + pos];   // the fit left it at the record's position
+    A.trk_weight[t0 + i] = vtx >= 0 ? w : 0.0f;
   };
 #pragma unroll
   for (int q = 0; q < 4; ++q)
