@@ -427,7 +427,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--events", type=int, default=None, help="events PER GPU (default: the config's own size; configs[4] sweep)")
-    ap.add_argument("--chunks", type=int, default=16, help="pipeline chunks of the e2e host path")
+    ap.add_argument("--chunks", type=int, default=8, help="pipeline chunks of the e2e host path")
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-sample", type=int, default=100_000)

@@ -369,8 +369,12 @@ struct pv_host_ctx {
   int max_vtx = 0;
   int n_streams = 0;
   std::vector<cudaStream_t> streams;
+  cudaStream_t h2d_stream = nullptr;          // every input copy, in chunk order: the host-to-device engine never waits
+  cudaStream_t d2h_stream = nullptr;          // every fixed-size result copy
   cudaStream_t vtx_stream = nullptr;          // read-back of the packed vertices (sizes known once a chunk is done)
-  cudaEvent_t done[HOST_MAX_CHUNKS] = {nullptr};
+  cudaEvent_t up[HOST_MAX_CHUNKS] = {nullptr};     // inputs of the chunk are on the device
+  cudaEvent_t done[HOST_MAX_CHUNKS] = {nullptr};   // kernels of the chunk have finished
+  cudaEvent_t back[HOST_MAX_CHUNKS] = {nullptr};   // the chunk's vertex count is on the host
   int32_t* h_total = nullptr;                 // pinned: vertices found per chunk
   float* d_in[9] = {nullptr};
   int32_t* d_off = nullptr;
@@ -388,8 +392,13 @@ int pv_host_ctx_destroy(pv_host_ctx* c) {
   if (!c) return PV_E_NULL;
   for (auto s : c->streams) cudaStreamDestroy(s);
   if (c->vtx_stream) cudaStreamDestroy(c->vtx_stream);
-  for (int i = 0; i < HOST_MAX_CHUNKS; ++i)
+  if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+  if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
+  for (int i = 0; i < HOST_MAX_CHUNKS; ++i) {
+    if (c->up[i]) cudaEventDestroy(c->up[i]);
     if (c->done[i]) cudaEventDestroy(c->done[i]);
+    if (c->back[i]) cudaEventDestroy(c->back[i]);
+  }
   if (c->h_total) cudaFreeHost(c->h_total);
   for (int i = 0; i < 9; ++i) cudaFree(c->d_in[i]);
   cudaFree(c->d_off); cudaFree(c->d_pos); cudaFree(c->d_cov); cudaFree(c->d_chi2); cudaFree(c->d_w);
@@ -426,7 +435,13 @@ int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, 
     if (err == cudaSuccess) c->streams.push_back(s);
   }
   if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&c->vtx_stream, cudaStreamNonBlocking);
-  for (int i = 0; i < HOST_MAX_CHUNKS && err == cudaSuccess; ++i) err = cudaEventCreateWithFlags(&c->done[i], cudaEventDisableTiming);
+  if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking);
+  if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking);
+  for (int i = 0; i < HOST_MAX_CHUNKS && err == cudaSuccess; ++i) {
+    err = cudaEventCreateWithFlags(&c->up[i], cudaEventDisableTiming);
+    if (err == cudaSuccess) err = cudaEventCreateWithFlags(&c->done[i], cudaEventDisableTiming);
+    if (err == cudaSuccess) err = cudaEventCreateWithFlags(&c->back[i], cudaEventDisableTiming);
+  }
   if (err != cudaSuccess) {
     pv_host_ctx_destroy(c);
     return cuda_fail(err, "pv_host_ctx_create");
@@ -467,13 +482,22 @@ int host_impl(pv_host_ctx* c, const float* const h_in[9], const int32_t* offsets
   if (n_chunks > n_events) n_chunks = n_events;
   if (n_chunks > HOST_MAX_CHUNKS) n_chunks = HOST_MAX_CHUNKS;
   const size_t mv = (size_t)c->max_vtx;
-  // chunk boundaries: equal track counts (events are contiguous in the SoA arrays)
+  // chunk boundaries by track count (events are contiguous in the SoA arrays).  The chunks ramp up and down in size
+  // (1, 2, 4, 8, 8, ..., 8, 4, 2, 1): the first kernels start after a short copy, the last results leave after a short
+  // one, and the bulk moves in few large copies (every cudaMemcpyAsync costs ~5 us of PCIe time on top of its bytes).
   std::vector<int> eb(n_chunks + 1, 0);
   eb[n_chunks] = n_events;
-  for (int k = 1, e = 0; k < n_chunks; ++k) {
-    const long long target = T * k / n_chunks;
-    while (e < n_events && offsets[e] < target) ++e;
-    eb[k] = e < eb[k - 1] ? eb[k - 1] : e;
+  {
+    std::vector<long long> wsum(n_chunks + 1, 0);
+    for (int k = 0; k < n_chunks; ++k) {
+      const int d = k < n_chunks - 1 - k ? k : n_chunks - 1 - k;   // distance to the nearer end
+      wsum[k + 1] = wsum[k] + (1LL << (d < 3 ? d : 3));
+    }
+    for (int k = 1, e = 0; k < n_chunks; ++k) {
+      const long long target = (long long)((double)T * (double)wsum[k] / (double)wsum[n_chunks]);
+      while (e < n_events && offsets[e] < target) ++e;
+      eb[k] = e < eb[k - 1] ? eb[k - 1] : e;
+    }
   }
   int rc = PV_OK;
   auto ck = [&](cudaError_t err, const char* what) {
@@ -487,11 +511,14 @@ int host_impl(pv_host_ctx* c, const float* const h_in[9], const int32_t* offsets
     if (e1 <= e0) continue;
     cudaStream_t s = c->streams[k % c->n_streams];
     const size_t t0 = (size_t)offsets[e0], nt = (size_t)offsets[e1] - t0, ne = (size_t)(e1 - e0);
-    // offsets stay absolute: the kernel indexes the un-shifted SoA base pointers
-    if (!ck(cudaMemcpyAsync(c->d_off + e0, offsets + e0, (ne + 1) * 4, cudaMemcpyHostToDevice, s), "H2D offsets")) break;
+    // inputs: one stream for all chunks (offsets stay absolute: the kernel indexes the un-shifted SoA base pointers)
+    if (!ck(cudaMemcpyAsync(c->d_off + e0, offsets + e0, (ne + 1) * 4, cudaMemcpyHostToDevice, c->h2d_stream), "H2D offsets")) break;
     for (int i = 0; i < 9 && nt > 0 && rc == PV_OK; ++i)
-      ck(cudaMemcpyAsync(c->d_in[i] + t0, h_in[i] + t0, nt * 4, cudaMemcpyHostToDevice, s), "H2D tracks");
+      ck(cudaMemcpyAsync(c->d_in[i] + t0, h_in[i] + t0, nt * 4, cudaMemcpyHostToDevice, c->h2d_stream), "H2D tracks");
     if (rc != PV_OK) break;
+    if (!ck(cudaEventRecord(c->up[k], c->h2d_stream), "cudaEventRecord")) break;
+    // kernels: round-robin over the compute streams (each with its own workspace)
+    if (!ck(cudaStreamWaitEvent(s, c->up[k], 0), "cudaStreamWaitEvent")) break;
     const int frc = find_impl(c->d_in[0], c->d_in[1], c->d_in[2], c->d_in[3], c->d_in[4], c->d_in[5], c->d_in[6], c->d_in[7],
                               c->d_in[8], c->d_off + e0, (int)ne, (long long)c->max_tracks, params, c->d_pos + e0 * mv * 3,
                               c->d_cov + e0 * mv * 6, c->d_chi2 + e0 * mv, c->d_ntrk + e0 * mv, c->d_niter + e0 * mv,
@@ -500,31 +527,37 @@ int host_impl(pv_host_ctx* c, const float* const h_in[9], const int32_t* offsets
                               compact ? c->d_tv8 : nullptr);
     if (frc != PV_OK) { rc = frc; break; }
     enqueued = k + 1;
+    int32_t* vb = c->d_vbegin + e0 + k;
     if (compact) {
       pvk::KArgs ka;
       memset(&ka, 0, sizeof(ka));
       ka.n_events = (int)ne;
       ka.vtx_pos = c->d_pos + e0 * mv * 3; ka.vtx_cov = c->d_cov + e0 * mv * 6; ka.vtx_chi2 = c->d_chi2 + e0 * mv;
       ka.vtx_ntracks = c->d_ntrk + e0 * mv; ka.vtx_niter = c->d_niter + e0 * mv;
-      int32_t* vb = c->d_vbegin + e0 + k;
       pvk::scan_nvtx_kernel<<<1, 1024, 0, s>>>(c->d_nvtx + e0, (int)ne, vb);
       pvk::pack_vertices_kernel<<<(unsigned)((ne + 7) / 8), 256, 0, s>>>(ka, (int)mv, vb, c->d_packed + e0 * mv);
       if (!ck(cudaGetLastError(), "pack_vertices_kernel")) break;
-      if (!ck(cudaMemcpyAsync(c->h_total + k, vb + ne, 4, cudaMemcpyDeviceToHost, s), "D2H chunk total")) break;
-      if (!ck(cudaEventRecord(c->done[k], s), "cudaEventRecord")) break;
-    } else {
-      ck(cudaMemcpyAsync(vtx_pos + e0 * mv * 3, c->d_pos + e0 * mv * 3, ne * mv * 12, cudaMemcpyDeviceToHost, s), "D2H");
-      ck(cudaMemcpyAsync(vtx_cov + e0 * mv * 6, c->d_cov + e0 * mv * 6, ne * mv * 24, cudaMemcpyDeviceToHost, s), "D2H");
-      ck(cudaMemcpyAsync(vtx_chi2 + e0 * mv, c->d_chi2 + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s), "D2H");
-      ck(cudaMemcpyAsync(vtx_ntracks + e0 * mv, c->d_ntrk + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s), "D2H");
-      ck(cudaMemcpyAsync(vtx_niter + e0 * mv, c->d_niter + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, s), "D2H");
     }
-    ck(cudaMemcpyAsync(n_vtx + e0, c->d_nvtx + e0, ne * 4, cudaMemcpyDeviceToHost, s), "D2H");
-    ck(cudaMemcpyAsync(event_status + e0, c->d_status + e0, ne * 4, cudaMemcpyDeviceToHost, s), "D2H");
+    if (!ck(cudaEventRecord(c->done[k], s), "cudaEventRecord")) break;
+    // results: one stream for all chunks
+    cudaStream_t r = c->d2h_stream;
+    if (!ck(cudaStreamWaitEvent(r, c->done[k], 0), "cudaStreamWaitEvent")) break;
+    if (compact) {
+      ck(cudaMemcpyAsync(c->h_total + k, vb + ne, 4, cudaMemcpyDeviceToHost, r), "D2H chunk total");
+      ck(cudaEventRecord(c->back[k], r), "cudaEventRecord");
+    } else {
+      ck(cudaMemcpyAsync(vtx_pos + e0 * mv * 3, c->d_pos + e0 * mv * 3, ne * mv * 12, cudaMemcpyDeviceToHost, r), "D2H");
+      ck(cudaMemcpyAsync(vtx_cov + e0 * mv * 6, c->d_cov + e0 * mv * 6, ne * mv * 24, cudaMemcpyDeviceToHost, r), "D2H");
+      ck(cudaMemcpyAsync(vtx_chi2 + e0 * mv, c->d_chi2 + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, r), "D2H");
+      ck(cudaMemcpyAsync(vtx_ntracks + e0 * mv, c->d_ntrk + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, r), "D2H");
+      ck(cudaMemcpyAsync(vtx_niter + e0 * mv, c->d_niter + e0 * mv, ne * mv * 4, cudaMemcpyDeviceToHost, r), "D2H");
+    }
+    ck(cudaMemcpyAsync(n_vtx + e0, c->d_nvtx + e0, ne * 4, cudaMemcpyDeviceToHost, r), "D2H");
+    ck(cudaMemcpyAsync(event_status + e0, c->d_status + e0, ne * 4, cudaMemcpyDeviceToHost, r), "D2H");
     if (nt > 0) {
-      ck(cudaMemcpyAsync(trk_weight + t0, c->d_w + t0, nt * 4, cudaMemcpyDeviceToHost, s), "D2H");
-      if (compact) ck(cudaMemcpyAsync(trk_vertex8 + t0, c->d_tv8 + t0, nt, cudaMemcpyDeviceToHost, s), "D2H");
-      else ck(cudaMemcpyAsync(trk_vertex + t0, c->d_tv + t0, nt * 4, cudaMemcpyDeviceToHost, s), "D2H");
+      ck(cudaMemcpyAsync(trk_weight + t0, c->d_w + t0, nt * 4, cudaMemcpyDeviceToHost, r), "D2H");
+      if (compact) ck(cudaMemcpyAsync(trk_vertex8 + t0, c->d_tv8 + t0, nt, cudaMemcpyDeviceToHost, r), "D2H");
+      else ck(cudaMemcpyAsync(trk_vertex + t0, c->d_tv + t0, nt * 4, cudaMemcpyDeviceToHost, r), "D2H");
     }
   }
   // second pass (compact): as each chunk finishes, its vertex count is on the host and its packed records are copied
@@ -533,7 +566,7 @@ int host_impl(pv_host_ctx* c, const float* const h_in[9], const int32_t* offsets
   for (int k = 0; compact && k < enqueued && rc == PV_OK; ++k) {
     const int e0 = eb[k], e1 = eb[k + 1];
     if (e1 <= e0) continue;
-    if (!ck(cudaEventSynchronize(c->done[k]), "cudaEventSynchronize")) break;
+    if (!ck(cudaEventSynchronize(c->back[k]), "cudaEventSynchronize")) break;
     const long long nv = c->h_total[k];
     if (base + nv > vtx_capacity) { rc = PV_E_SIZE; break; }
     if (nv > 0)
@@ -541,6 +574,8 @@ int host_impl(pv_host_ctx* c, const float* const h_in[9], const int32_t* offsets
                          c->vtx_stream), "D2H vertices");
     base += nv;
   }
+  ck(cudaStreamSynchronize(c->h2d_stream), "cudaStreamSynchronize");
+  ck(cudaStreamSynchronize(c->d2h_stream), "cudaStreamSynchronize");
   for (auto s : c->streams) ck(cudaStreamSynchronize(s), "cudaStreamSynchronize");
   ck(cudaStreamSynchronize(c->vtx_stream), "cudaStreamSynchronize");
   if (rc == PV_OK && compact)

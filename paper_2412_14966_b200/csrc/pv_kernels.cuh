@@ -405,12 +405,17 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
   Trk T;
   const float zl = R.z - zsv;
   T.tx = R.tx; T.ty = R.ty;
-  // the change of frame in double, once per record: for a state given far from the vertex (x ~ 30 mm at 150 mm and a
-  // slope of 0.2) x - zl tx cancels to O(0.1 mm), and the fp32 rounding of the large terms (2e-6 mm) is what the
-  // Tukey weights of a non-converged fit amplify
-  const double zld = (double)R.z - (double)zsv;
-  T.x0 = (float)fma(-zld, (double)R.tx, (double)R.x - (double)sx);
-  T.y0 = (float)fma(-zld, (double)R.ty, (double)R.y - (double)sy);
+  if (fabsf(zl) > 4.0f) {
+    // a state given far from the vertex: x - zl tx cancels (x ~ 30 mm at 150 mm and a slope of 0.2, against a result
+    // of O(0.1 mm)); the fp32 rounding of the large terms (2e-6 mm) is what the Tukey weights of a non-converged fit
+    // amplify, so this change of frame is done in double (once per record; never taken for states at their vertex)
+    const double zld = (double)R.z - (double)zsv;
+    T.x0 = (float)fma(-zld, (double)R.tx, (double)R.x - (double)sx);
+    T.y0 = (float)fma(-zld, (double)R.ty, (double)R.y - (double)sy);
+  } else {
+    T.x0 = fmaf(-zl, R.tx, R.x - sx);
+    T.y0 = fmaf(-zl, R.ty, R.y - sy);
+  }
   const float Vx = var_at(R.vx, R.vtx, cx, -zl);
   const float Vy = var_at(R.vy, R.vty, cy, -zl);
   const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
@@ -1501,6 +1506,11 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   int sv[4];                                               // seed index of my first four tracks: loads issued now,
 #pragma unroll                                             // consumed after the vertex sweep
   for (int q = 0; q < 4; ++q) sv[q] = (lane + 32 * q < n) ? A.trk_vertex[t0 + lane + 32 * q] : -1;
+  float wv[4] = {0.0f, 0.0f, 0.0f, 0.0f};                  // explicit flavour: the weight the fit left at the track's record
+  if (FLAV != PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) wv[q] = sv[q] >= 0 ? A.wrec[t0 + (sv[q] >> 5)] : 0.0f;
+  }
   unsigned long long bv[4] = {0ull, 0ull, 0ull, 0ull};     // multi-vertex flavour: largest weight << 32 | 31 - seed
   if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
 #pragma unroll
@@ -1587,29 +1597,28 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   }
   if (lane == 0) A.n_vtx[e] = __popc(kept);
   // final per-track outputs; tracks of rejected vertices are released (R-9)
-  auto finish = [&](int i, int s, unsigned long long b) {
-    float w = 0.0f;
-    int pos = 0;
+  auto finish = [&](int i, int s, unsigned long long b, float w) {
     if (FLAV == PV_FLAVOUR_MULTIVERTEX) {                  // R-13: the track follows the seed with its largest weight
       w = __uint_as_float((unsigned)(b >> 32));
       s = w > 0.0f ? 31 - (int)(b & 31ull) : -1;
       if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
     } else if (s >= 0) {                                   // explicit flavour: seed | record position << 5 (seed_kernel)
-      pos = s >> 5;
       s &= 31;
     }
     int vtx = -1;
     if (s >= 0 && ((kept >> s) & 1u)) vtx = __popc(kept & ((1u << s) - 1u));
     A.trk_vertex[t0 + i] = vtx;
     if (A.trk_vertex8) A.trk_vertex8[t0 + i] = (int8_t)vtx;
-    if (FLAV != PV_FLAVOUR_MULTIVERTEX && vtx >= 0) w = A.wrec[t0 + pos];   // the fit left it at the record's position
     A.trk_weight[t0 + i] = vtx >= 0 ? w : 0.0f;
   };
 #pragma unroll
   for (int q = 0; q < 4; ++q)
-    if (lane + 32 * q < n) finish(lane + 32 * q, sv[q], bv[q]);
-  for (int i = 128 + lane; i < n; i += 32)
-    finish(i, A.trk_vertex[t0 + i], FLAV == PV_FLAVOUR_MULTIVERTEX ? A.best[t0 + i] : 0ull);
+    if (lane + 32 * q < n) finish(lane + 32 * q, sv[q], bv[q], wv[q]);
+  for (int i = 128 + lane; i < n; i += 32) {
+    const int s = A.trk_vertex[t0 + i];
+    const float w = (FLAV != PV_FLAVOUR_MULTIVERTEX && s >= 0) ? A.wrec[t0 + (s >> 5)] : 0.0f;
+    finish(i, s, FLAV == PV_FLAVOUR_MULTIVERTEX ? A.best[t0 + i] : 0ull, w);
+  }
 }
 
 // ---- host pipeline: the PVs of a chunk of events packed into 48-byte records in event order, so that the

@@ -35,7 +35,9 @@ def _both(pv, oracle, data, n_hist=None, **over):
     return got, ref, rep
 
 
-def _assert_parity(rep, allow_ties_frac=0.01):
+def _assert_parity(rep, allow_ties_frac=5e-4):
+    """No failure, and no more logged near-ties than twice the largest rate measured on B200 (2e-4 of the fitted
+    seeds, multi-vertex flavour on high pile-up; 1e-5 on configs[1] at full size; 0 on most cases)."""
     assert not rep["failures"], "\n".join(rep["failures"][:10])
     for t in rep["near_ties"][:10]:
         print("LOGGED", t)
@@ -154,7 +156,7 @@ def test_wide_tracks_many_fill_units(pv, oracle):
     data = events.from_lists([wide, mixed, gas_event(40, 0.02, 0.05, 0.15)])
     got, ref, rep = _both(pv, oracle, data)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
-    _assert_parity(rep, allow_ties_frac=0.5)
+    _assert_parity(rep)
     sp = ref["debug"]["sigma_poca"][:200]
     assert (sp > 5.0).sum() > 30 and rep["hist_mismatch"] == 0      # units per chunk well above the list capacity
     assert ref["debug"]["hist"][0].sum() > 100 * (1 << 20)
@@ -182,7 +184,7 @@ def test_many_proto_clusters_slow_path(pv, oracle):
     data = events.from_lists([ev, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, ev])
     got, ref, rep = _both(pv, oracle, data)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
-    _assert_parity(rep, allow_ties_frac=0.5)
+    _assert_parity(rep)
     H = ref["debug"]["hist"][0]
     above = H > int(0.25 * (1 << 20))
     starts = above & ~np.concatenate([[False], above[:-1]])
@@ -227,12 +229,12 @@ def test_too_many_tracks_and_vertex_overflow(pv, oracle):
     lst = [huge, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, exact, {k: small[k][so[1]:so[2]] for k in events.FIELDS}]
     data = events.from_lists(lst)
     got, ref, rep = _both(pv, oracle, data, max_vtx_per_event=32)
-    _assert_parity(rep, allow_ties_frac=0.05)
+    _assert_parity(rep)
     assert got["event_status"][0] & 1 and got["n_vtx"][0] == 0
     assert np.all(got["trk_vertex"][:2200] == -1) and np.all(got["trk_weight"][:2200] == 0)
     assert got["n_vtx"][2] > 10                                   # 2047 tracks of 40 merged pile-up events
     got, ref, rep = _both(pv, oracle, events.generate(events.config(2, 300)), max_vtx_per_event=4)
-    _assert_parity(rep, allow_ties_frac=0.05)
+    _assert_parity(rep)
     assert (got["event_status"] & 2).sum() > 100 and np.array_equal(got["event_status"] & 2, ref["event_status"] & 2)
 
 
@@ -251,7 +253,7 @@ def test_other_parameters(pv, oracle):
     _, _, rep = _both(pv, oracle, data, n_hist=100, dz=0.5, min_dip=0.5, min_bin_content=0.4)
     _assert_parity(rep)
     _, _, rep = _both(pv, oracle, data, n_hist=100, conv_dz=1e-4, conv_dchi2=1e-3, max_iter=16, merge_ratio=9.0)
-    _assert_parity(rep, allow_ties_frac=0.03)
+    _assert_parity(rep)
 
 
 def _both_mv(pv, oracle, data, n_hist=None, **over):
@@ -273,7 +275,7 @@ def test_multivertex_flavour(pv, oracle, idx, n):
     data = events.generate(events.config(idx, n))
     got, ref, rep = _both_mv(pv, oracle, data, n_hist=200)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
-    _assert_parity(rep, allow_ties_frac=0.02)
+    _assert_parity(rep)
     assert rep["seed_z_mismatch"] == 0 and rep["assign_agreement"] >= 0.999
     assert rep["n_vertices"] > 1000
     assert not (got["event_status"] & 8).any()
@@ -283,11 +285,11 @@ def test_multivertex_other_parameters_and_reproducibility(pv, oracle):
     """chi2_max = 4 (the value of Fig. 6), a narrower window, a tilted beamline; two runs are bit-identical."""
     data = events.generate(events.config(1, 800))
     _, _, rep = _both_mv(pv, oracle, data, n_hist=50, chi2_max=4.0, chi2_window=16.0)
-    _assert_parity(rep, allow_ties_frac=0.03)
+    _assert_parity(rep)
     d2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in data.items()}
     d2["x"] = (d2["x"] + 0.8 + 1e-3 * d2["z"]).astype(np.float32)
     _, _, rep = _both_mv(pv, oracle, d2, n_hist=50, beam_x=0.8, beam_tx=1e-3)
-    _assert_parity(rep, allow_ties_frac=0.03)
+    _assert_parity(rep)
     p = pv.multivertex_params()
     a = pv.find(data, p)
     b = pv.find(data, p)
@@ -335,7 +337,7 @@ def test_recursive_splitter(pv, oracle, idx, n, mv):
     ref = oracle.find(data, po, debug=True, n_hist_events=100, trace=True, n_threads=NTHREADS)
     rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
-    _assert_parity(rep, allow_ties_frac=0.03)
+    _assert_parity(rep)
     assert rep["seed_bins_mismatch"] == 0 and rep["seed_z_mismatch"] == 0 and rep["n_seeds_mismatch"] == 0
 
 
@@ -366,7 +368,7 @@ def test_recursive_splitter_differs_on_a_small_middle_peak(pv, oracle):
         got = pv.find(data, p, debug=True, n_hist_events=3)
         ref = oracle.find(data, po, debug=True, n_hist_events=3, trace=True)
         rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
-        _assert_parity(rep, allow_ties_frac=1.0)
+        _assert_parity(rep)
         assert rep["seed_bins_mismatch"] == 0 and rep["hist_mismatch"] == 0
         seeds[mode] = got["debug"]["seed_bins"][0][:got["debug"]["n_seeds_raw"][0]].tolist()
     assert seeds[0] == [[2200, 2201, 2200], [2201, 2205, 2204]]
@@ -425,7 +427,7 @@ def test_covariance_cross_terms(pv, oracle, mv):
     ref = oracle.find(m, po, debug=True, n_hist_events=100, trace=True, n_threads=NTHREADS)
     rep = compare.compare(got, ref, np.asarray(m["offsets"]), p)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
-    _assert_parity(rep, allow_ties_frac=0.03)
+    _assert_parity(rep)
     assert rep["n_vertices"] > 5000
     # without the cross terms the same inputs give clearly different covariances: the terms are exercised
     nocov = pv.find({k: v for k, v in m.items() if not k.startswith("cov_")}, p)
@@ -543,7 +545,7 @@ def test_record_overflow_is_flagged_per_event(pv, oracle):
     g, r = _select(got, E, T, keep, tkeep), _select(ref, E, T, keep, tkeep)
     rep = compare.compare(g, r, sub_off, p)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
-    _assert_parity(rep, allow_ties_frac=0.05)
+    _assert_parity(rep)
     assert rep["n_vertices"] > 100
 
 
@@ -552,7 +554,7 @@ def test_unusual_parameters_reach_their_guards(pv, oracle):
     a sigma cut whose window would need more fill units than the list can number is refused (PV_E_PARAM)."""
     data = events.generate(events.config(0, 400))
     got, ref, rep = _both(pv, oracle, data, n_hist=50, min_tracks_seed=(0, 0), min_cluster_integral=(0.5, 0.5), min_tracks_pv=(1, 1))
-    _assert_parity(rep, allow_ties_frac=0.02)
+    _assert_parity(rep)
     assert rep["n_vertices"] > 1500
     with pytest.raises(pv.PvError):
         pv.find(data, pv.default_params(max_sigma_poca=(1.5, 200.0)))
