@@ -60,10 +60,16 @@ typedef struct pv_params {
   int32_t split_mode;                   /* proto-cluster splitting: PV_SPLIT_Z_ORDERED (default, the paper's GPU
                                            variant: minima in z order) or PV_SPLIT_RECURSIVE (its x86 variant: the
                                            smallest minimum between the two largest maxima, recursively; reading R-16) */
+  int32_t fill_mode;                    /* histogram fill: PV_FILL_POLYNOMIAL (default, the paper's GPU variant: a
+                                           polynomial approximation of the cumulative density per track, reading R-6) or
+                                           PV_FILL_TEMPLATE (its x86 variant: "a finite set of template histograms,
+                                           selected based on the value of sigma_poca"; reading R-17: classes
+                                           sigma_k = 0.08 dz 2^(k/4) x 8 positions of z_poca inside its bin) */
 } pv_params;
 
 enum { PV_FLAVOUR_EXPLICIT = 0, PV_FLAVOUR_MULTIVERTEX = 1 };
 enum { PV_SPLIT_Z_ORDERED = 0, PV_SPLIT_RECURSIVE = 1 };
+enum { PV_FILL_POLYNOMIAL = 0, PV_FILL_TEMPLATE = 1 };
 
 enum {
   PV_OK = 0,
@@ -103,7 +109,9 @@ int pv_nbins(const pv_params* p);
  * in the seed's local frame with W = V^-1 at the seed position) handed from the seed kernel to the
  * fit kernel.  The multi-vertex flavour lists a track once per vertex candidate in its chi2 window: it takes two
  * records per track and 8 more bytes per track (the largest weight of the track and its vertex).  The histograms
- * live in shared memory ("one block per event").  bytes: HOST out. */
+ * live in shared memory ("one block per event").  With PV_FILL_TEMPLATE the workspace also holds the table of
+ * template histograms (tens of KB; rebuilt by a small kernel at every call: the library keeps no device state).
+ * bytes: HOST out. */
 int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, size_t* bytes);
 
 /* The hot path a1..a6 over a batch.
@@ -252,7 +260,7 @@ int pv_host_register(void* ptr, size_t bytes);
 int pv_host_unregister(void* ptr);
 
 /* Launch statistics of the most recent pv_find / pv_find_debug call of this process (for bench.py):
- * kernels launched (3: seed, fit, cleanup), and grid size, block size, dynamic shared memory per block of
+ * kernels launched (3: seed, fit, cleanup; 4 with PV_FILL_TEMPLATE: the template table first), and grid size, block size, dynamic shared memory per block of
  * the seed kernel.  All HOST out, nullable. */
 int pv_last_launch_info(int* n_kernels, int* grid, int* block, int* smem_bytes);
 

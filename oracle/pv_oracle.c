@@ -41,6 +41,7 @@ void pvo_params_default(pvo_params *p) {
   p->flavour = 0;                                                /* explicit association + Tukey (x86 flavour) */
   p->chi2_window = 25.0f;                                        /* P:L384 "within a certain chi2_i"; value: R-13 */
   p->split_mode = 0;                                             /* z-ordered splitting (GPU variant) */
+  p->fill_mode = 0;                                              /* polynomial CDF per track (GPU variant) */
 }
 
 int pvo_nbins(const pvo_params *p) {
@@ -122,6 +123,77 @@ void pvo_fill(int n, const float *z_poca, const float *sigma_poca, const int32_t
       int32_t q1 = pvo_edge_q(b + 1, z_poca[i], sigma_poca[i], p);
       H[b] += q1 - q0;
       q0 = q1;
+    }
+  }
+}
+
+/* ---- O3, x86 variant: template histograms selected by sigma_poca (reading R-17) ---------------------------
+ * fp32 contract like the rest of O3 (every operation rounded once), so that the integer bins are reproducible. */
+static const float PVO_TMPL_CENTRE[4] = {1.0f, 0x1.306fe0p+0f, 0x1.6a09e6p+0f, 0x1.ae89fap+0f};   /* 2^(0, 1/4, 1/2, 3/4) */
+static const float PVO_TMPL_EDGE[4] = {0x1.172b84p+0f, 0x1.4bfdaep+0f, 0x1.8ace54p+0f, 0x1.d5818ep+0f}; /* 2^(1/8, 3/8, 5/8, 7/8) */
+
+/* centre of sigma class k in bins: 0.08 * 2^(k/4) */
+static float tmpl_centre(int k) { return ldexpf(PVO_TMPL_CENTRE[k & 3], k >> 2) * 0.08f; }
+
+/* nearest class in log sigma, before clamping: with v = sigma / (0.08 dz) = m 2^E, m in [1, 2): 4 E + the number of
+ * class edges 2^((2 q + 1) / 8) that m has reached */
+static int tmpl_class_raw(float sigma, float inv_dz) {
+  float v = (sigma * inv_dz) * 12.5f;
+  if (!(v >= 1.0f)) return 0;                        /* below the first centre (or NaN) */
+  if (!(v < 0x1p+20f)) return 80;                    /* far beyond any sigma cut */
+  int E;
+  float m = 2.0f * frexpf(v, &E);                    /* v = m 2^(E - 1), m in [1, 2) */
+  int k = 4 * (E - 1);
+  for (int q = 0; q < 4; ++q) k += (m >= PVO_TMPL_EDGE[q]) ? 1 : 0;
+  return k;
+}
+
+int pvo_tmpl_class(float sigma_poca, const pvo_params *p) {
+  float inv_dz = 1.0f / p->dz;
+  float smax = p->max_sigma_poca[0] > p->max_sigma_poca[1] ? p->max_sigma_poca[0] : p->max_sigma_poca[1];
+  int kmax = tmpl_class_raw(smax, inv_dz);           /* the finite set: classes 0 .. class of the largest sigma cut */
+  int k = tmpl_class_raw(sigma_poca, inv_dz);
+  return k < kmax ? k : kmax;
+}
+
+int pvo_tmpl_halfwidth(int k) { return (int)ceilf(3.0f * tmpl_centre(k)); }
+
+/* fixed-point CDF (the contract of pvo_edge_q) at bin edge i, in bins relative to the lower edge of the central bin,
+ * for a track at zrel inside that bin with 1 / (3 sigma) = inv */
+static int32_t tmpl_edge_q(int i, float zrel, float inv) {
+  float s = ((float)i - zrel) * inv;
+  if (s <= -1.0f) return 0;
+  if (s >= 1.0f) return PVO_S;
+  float t = s * s;
+  float g = PVO_G[6];
+  for (int j = 5; j >= 0; --j) g = fmaf(g, t, PVO_G[j]);
+  float c = fmaf(s, g, 0.5f);
+  if (c < 0.0f) c = 0.0f;
+  if (c > 1.0f) c = 1.0f;
+  return (int32_t)lrintf(c * 1048576.0f);
+}
+
+int32_t pvo_tmpl_bin(int k, int j, int i) {
+  float zrel = ((float)j + 0.5f) * (1.0f / (float)PVO_TMPL_J);  /* centre of the j-th eighth of the central bin */
+  float inv = 1.0f / (PVO_U * tmpl_centre(k));
+  return tmpl_edge_q(i + 1, zrel, inv) - tmpl_edge_q(i, zrel, inv);
+}
+
+void pvo_fill_template(int n, const float *z_poca, const float *sigma_poca, const int32_t *bin, const int32_t *flags,
+                       const pvo_params *p, int32_t *H) {
+  int nbins = pvo_nbins(p);
+  float inv_dz = 1.0f / p->dz;
+  for (int t = 0; t < n; ++t) {
+    if (!(flags[t] & PVO_TRK_HISTOGRAMMED)) continue;
+    int k = pvo_tmpl_class(sigma_poca[t], p);         /* "selected based on the value of sigma_poca" */
+    float fb = (z_poca[t] - p->z_min) * inv_dz;       /* the expression that gave the central bin (O1) */
+    float frac = fb - floorf(fb);
+    int j = (int)(frac * (float)PVO_TMPL_J);
+    if (j > PVO_TMPL_J - 1) j = PVO_TMPL_J - 1;
+    int W = pvo_tmpl_halfwidth(k);
+    for (int i = -W; i <= W; ++i) {
+      int b = bin[t] + i;
+      if (b >= 0 && b < nbins) H[b] += pvo_tmpl_bin(k, j, i);   /* bins beyond the range are dropped, as in pvo_fill */
     }
   }
 }
@@ -683,7 +755,8 @@ static void find_event(int e, const float *x, const float *y, const float *z, co
   pvo_project(n, x + t0, y + t0, z + t0, tx + t0, ty + t0, var_x + t0, p, S->zp, S->sp, S->bin, S->flags);
   /* step 2: histogram filling */
   memset(S->H, 0, sizeof(int32_t) * (size_t)nb);
-  pvo_fill(n, S->zp, S->sp, S->flags, p, S->H, 0);
+  if (p->fill_mode == 1) pvo_fill_template(n, S->zp, S->sp, S->bin, S->flags, p, S->H);
+  else pvo_fill(n, S->zp, S->sp, S->flags, p, S->H, 0);
   /* step 3: peak search; clusters come out ordered in z */
   int n_raw = pvo_peaks(S->H, p, mv, S->cb, S->ce, S->cp);
   int ns = n_raw;

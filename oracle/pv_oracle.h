@@ -39,6 +39,9 @@ typedef struct pvo_params {
                                           vertex fit (value 25: reading R-13) */
   int32_t split_mode;                  /* proto-cluster splitting: 0 = minima in z order (GPU variant),
                                           1 = smallest minimum between the two largest maxima, recursively (x86) */
+  int32_t fill_mode;                   /* histogram fill: 0 = polynomial CDF per track (GPU variant, R-6),
+                                          1 = "a finite set of template histograms, selected based on the value of
+                                          sigma_poca" (x86 variant, reading R-17) */
 } pvo_params;
 
 /* NEXT-2: the x-tx and y-ty elements of the track covariance (Eq. 2: V_xx(z) = V_xx + 2 dz V_xtx + dz^2 V_txtx).
@@ -66,6 +69,21 @@ int32_t pvo_edge_q(int k, float z_poca, float sigma_poca, const pvo_params *p);
  * full_range == 0 evaluates a conservative window only (identical result, see tests). */
 void pvo_fill(int n, const float *z_poca, const float *sigma_poca, const int32_t *flags,
               const pvo_params *p, int32_t *H, int full_range);
+/* O3, x86 variant (reading R-17): the track's bin contents are taken from a TEMPLATE histogram instead of being
+ * integrated for its own z_poca and sigma_poca.  Templates exist for sigma classes k = 0, 1, ... with centres
+ * sigma_k = 0.08 dz 2^(k/4) (a track takes the class nearest in log sigma, clamped to the classes the sigma cuts allow)
+ * and for PVO_TMPL_J = 8 positions of z_poca inside its central bin (the centre of the eighth it falls in).  A template
+ * is the fixed-point CDF contract of pvo_edge_q evaluated in bin units for (sigma_k, position): bin i relative to the
+ * central bin gets Q(i + 1) - Q(i), i in [-W_k, W_k], W_k = ceil(3 sigma_k / dz); it sums to exactly 2^20.
+ * pvo_tmpl_class: class of a sigma_poca; pvo_tmpl_halfwidth: W_k; pvo_tmpl_bin: content of relative bin i of template
+ * (k, j); pvo_fill_template: the fill (H accumulated into, like pvo_fill). */
+enum { PVO_TMPL_J = 8 };
+int pvo_tmpl_class(float sigma_poca, const pvo_params *p);
+int pvo_tmpl_halfwidth(int k);
+int32_t pvo_tmpl_bin(int k, int j, int i);
+void pvo_fill_template(int n, const float *z_poca, const float *sigma_poca, const int32_t *bin, const int32_t *flags,
+                       const pvo_params *p, int32_t *H);
+
 /* O3 definition layer L0: exact Gaussian bin integrals via erf in double, untruncated. */
 void pvo_fill_exact(int n, const float *z_poca, const float *sigma_poca, const int32_t *flags,
                     const pvo_params *p, double *H0);

@@ -36,7 +36,7 @@ class Params(C.Structure):
         ("min_tracks_pv", C.c_int32 * 2), ("chi2_max", C.c_float), ("max_iter", C.c_int32),
         ("conv_dchi2", C.c_float), ("conv_dz", C.c_float), ("merge_ratio", C.c_float),
         ("max_beam_dist", C.c_float), ("max_vtx_per_event", C.c_int32),
-        ("flavour", C.c_int32), ("chi2_window", C.c_float), ("split_mode", C.c_int32),
+        ("flavour", C.c_int32), ("chi2_window", C.c_float), ("split_mode", C.c_int32), ("fill_mode", C.c_int32),
     ]
 
 
@@ -83,6 +83,12 @@ def lib():
         L.pvo_fit.restype = C.c_int
         L.pvo_find.restype = C.c_int
         L.pvo_fit_mv.restype = C.c_int
+        L.pvo_tmpl_class.argtypes = [C.c_float, C.POINTER(Params)]
+        L.pvo_tmpl_class.restype = C.c_int
+        L.pvo_tmpl_halfwidth.argtypes = [C.c_int]
+        L.pvo_tmpl_halfwidth.restype = C.c_int
+        L.pvo_tmpl_bin.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.pvo_tmpl_bin.restype = C.c_int32
         L.pvo_mv_weight.restype = C.c_double
         L.pvo_mv_weight.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_int]
         L.pvo_track_chi2.restype = C.c_double
@@ -155,6 +161,27 @@ def fill(zp, sp, flags, p: Params, full_range: bool = False) -> np.ndarray:
     zp, sp, flags = _f32(zp), _f32(sp), _i32(flags)
     H = np.zeros(nbins(p), np.int32)
     lib().pvo_fill(C.c_int(zp.size), _ptr(zp), _ptr(sp), _ptr(flags), C.byref(p), _ptr(H), C.c_int(int(full_range)))
+    return H
+
+
+def tmpl_class(sigma_poca: float, p: Params) -> int:
+    return int(lib().pvo_tmpl_class(C.c_float(sigma_poca), C.byref(p)))
+
+
+def tmpl_halfwidth(k: int) -> int:
+    return int(lib().pvo_tmpl_halfwidth(int(k)))
+
+
+def tmpl(k: int, j: int) -> np.ndarray:
+    """Template histogram (k, j): contents of the relative bins -W_k .. W_k."""
+    W = tmpl_halfwidth(k)
+    return np.array([lib().pvo_tmpl_bin(int(k), int(j), i) for i in range(-W, W + 1)], np.int64)
+
+
+def fill_template(zp, sp, bins, flags, p: Params) -> np.ndarray:
+    zp, sp, bins, flags = _f32(zp), _f32(sp), _i32(bins), _i32(flags)
+    H = np.zeros(nbins(p), np.int32)
+    lib().pvo_fill_template(C.c_int(zp.size), _ptr(zp), _ptr(sp), _ptr(bins), _ptr(flags), C.byref(p), _ptr(H))
     return H
 
 

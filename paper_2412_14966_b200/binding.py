@@ -24,6 +24,8 @@ EVT_SINGULAR_FIT = 4
 EVT_RECORD_OVERFLOW = 8
 FLAVOUR_EXPLICIT = 0
 FLAVOUR_MULTIVERTEX = 1
+FILL_POLYNOMIAL = 0
+FILL_TEMPLATE = 1
 
 FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
@@ -44,7 +46,7 @@ class Params(C.Structure):
         ("min_tracks_pv", C.c_int32 * 2), ("chi2_max", C.c_float), ("max_iter", C.c_int32),
         ("conv_dchi2", C.c_float), ("conv_dz", C.c_float), ("merge_ratio", C.c_float),
         ("max_beam_dist", C.c_float), ("max_vtx_per_event", C.c_int32),
-        ("flavour", C.c_int32), ("chi2_window", C.c_float), ("split_mode", C.c_int32),
+        ("flavour", C.c_int32), ("chi2_window", C.c_float), ("split_mode", C.c_int32), ("fill_mode", C.c_int32),
     ]
 
 

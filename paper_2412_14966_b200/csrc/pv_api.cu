@@ -33,8 +33,8 @@ int cuda_fail(cudaError_t err, const char* what) {
 
 struct DeviceInfo {
   int device = -1, sms = 0, max_smem_optin = 0;
-  bool attr_set[8] = {false, false, false, false, false, false, false, false};   // [debug + 2 flavour + 4 split]
-  int attr_smem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  bool attr_set[16] = {false};                         // [debug + 2 flavour + 4 split + 8 fill]
+  int attr_smem[16] = {0};
   int fit_blocks_per_sm[2] = {0, 0};                  // [flavour]
 };
 std::mutex g_mu;
@@ -80,12 +80,45 @@ int validate(const pv_params* p, int* nbins_out) {
   if (!(p->min_bin_content >= 0.0f)) return PV_E_PARAM;      // only bins a track wrote can start a proto-cluster
   if (p->flavour != PV_FLAVOUR_EXPLICIT && p->flavour != PV_FLAVOUR_MULTIVERTEX) return PV_E_PARAM;
   if (p->split_mode != PV_SPLIT_Z_ORDERED && p->split_mode != PV_SPLIT_RECURSIVE) return PV_E_PARAM;
+  if (p->fill_mode != PV_FILL_POLYNOMIAL && p->fill_mode != PV_FILL_TEMPLATE) return PV_E_PARAM;
   if (p->flavour == PV_FLAVOUR_MULTIVERTEX && (!(p->chi2_window > 0.0f) || isinf(p->chi2_max))) return PV_E_PARAM;
   // the fill cuts a track's +-3 sigma window into units of PV_UNIT bins and numbers them with 9 bits
   for (int r = 0; r < 2; ++r)
     if (!(6.0 * (double)p->max_sigma_poca[r] / (double)p->dz + 4.0 <= 512.0 * PV_UNIT)) return PV_E_PARAM;
   if (nbins_out) *nbins_out = nbins;
   return PV_OK;
+}
+
+// Template fill (reading R-17): host restatement of the class arithmetic of pv_kernels.cuh (fp32, one rounding
+// per operation), used to lay out the table: class of a sigma, centre of a class in bins.
+int tmpl_class_raw_host(float sigma, float inv_dz) {
+  const float v = (sigma * inv_dz) * 12.5f;
+  if (!(v >= 1.0f)) return 0;
+  if (!(v < 0x1p+20f)) return 80;
+  int E;
+  const float m = 2.0f * frexpf(v, &E);
+  return 4 * (E - 1) + (m >= 0x1.172b84p+0f ? 1 : 0) + (m >= 0x1.4bfdaep+0f ? 1 : 0) + (m >= 0x1.8ace54p+0f ? 1 : 0) +
+         (m >= 0x1.d5818ep+0f ? 1 : 0);
+}
+float tmpl_centre_host(int k) {
+  static const float c[4] = {1.0f, 0x1.306fe0p+0f, 0x1.6a09e6p+0f, 0x1.ae89fap+0f};
+  return ldexpf(c[k & 3], k >> 2) * 0.08f;
+}
+
+// entries (int32) of the template table for these parameters; fills the layout fields of *k when given
+size_t tmpl_layout(const pv_params* p, pvk::KParams* k) {
+  const float inv_dz = 1.0f / p->dz;
+  const float smax = p->max_sigma_poca[0] > p->max_sigma_poca[1] ? p->max_sigma_poca[0] : p->max_sigma_poca[1];
+  int kmax = tmpl_class_raw_host(smax, inv_dz);
+  if (kmax > pvk::TMPL_MAXK - 1) kmax = pvk::TMPL_MAXK - 1;       // validate() keeps sigma / dz below 512: class <= 51
+  size_t n = 0;
+  for (int c = 0; c <= kmax; ++c) {
+    const int W = (int)ceilf(3.0f * tmpl_centre_host(c));
+    if (k) { k->tmpl_off[c] = (int)n; k->tmpl_w[c] = (short)W; }
+    n += (size_t)pvk::TMPL_J * (size_t)(2 * W + 1);
+  }
+  if (k) k->tmpl_kmax = kmax;
+  return n;
 }
 
 void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
@@ -114,6 +147,7 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   const int r0 = ((nbins + 31) / 32) * 32 * 4;                // histogram padded to whole 32-bin words
   k->region0_words = r0 / 4;
   k->team_smem_bytes = r0 + pvk::SM_TAIL_BYTES;
+  if (p->fill_mode == PV_FILL_TEMPLATE) tmpl_layout(p, k);
 }
 
 // Workspace layout: [0, 256) counters | seed records, 16 B each, n_events * max_vtx | fit-ready track records,
@@ -125,10 +159,15 @@ size_t ws_rec_bytes(int n_events, int max_vtx) { return (size_t)n_events * (size
 size_t ws_trk_records(long long n_tracks, int flavour) {
   return (size_t)n_tracks * (flavour == PV_FLAVOUR_MULTIVERTEX ? 2 : 1);
 }
-size_t ws_bytes(int n_events, long long n_tracks, int max_vtx, int flavour) {
+size_t ws_core_bytes(int n_events, long long n_tracks, int max_vtx, int flavour) {
   size_t b = WS_COUNTERS + ws_rec_bytes(n_events, max_vtx) + ws_trk_records(n_tracks, flavour) * 32 + 16;
   if (flavour == PV_FLAVOUR_MULTIVERTEX) b += (size_t)n_tracks * 8 + 16;     // best[]
   else b += (size_t)n_tracks * 4 + 16;                                       // wrec[]
+  return (b + 15) / 16 * 16;
+}
+size_t ws_bytes(int n_events, long long n_tracks, const pv_params* p) {
+  size_t b = ws_core_bytes(n_events, n_tracks, p->max_vtx_per_event, p->flavour);
+  if (p->fill_mode == PV_FILL_TEMPLATE) b += tmpl_layout(p, nullptr) * sizeof(int32_t) + 16;   // template table
   return b;
 }
 
@@ -151,7 +190,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     return PV_E_NULL;
   if (n_tracks > 0 && (!x || !y || !z || !tx || !ty || !var_x || !var_y || !var_tx || !var_ty || !trk_weight || !trk_vertex))
     return PV_E_NULL;
-  if (workspace_bytes < ws_bytes(n_events, n_tracks, params->max_vtx_per_event, params->flavour)) return PV_E_WORKSPACE;
+  if (workspace_bytes < ws_bytes(n_events, n_tracks, params)) return PV_E_WORKSPACE;
   if (((uintptr_t)workspace & 15) != 0) return PV_E_PARAM;
   cudaStream_t stream = (cudaStream_t)stream_;
 
@@ -174,12 +213,17 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   const int smem = teams * kp.team_smem_bytes;
   const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
   const int spl = params->split_mode == PV_SPLIT_RECURSIVE ? 1 : 0;
-  const int which = (dbg ? 1 : 0) + 2 * mvf + 4 * spl;
-  static const void* const seed_fn[8] = {
-      (const void*)pvk::seed_kernel<false, 0, 0>, (const void*)pvk::seed_kernel<true, 0, 0>,
-      (const void*)pvk::seed_kernel<false, 1, 0>, (const void*)pvk::seed_kernel<true, 1, 0>,
-      (const void*)pvk::seed_kernel<false, 0, 1>, (const void*)pvk::seed_kernel<true, 0, 1>,
-      (const void*)pvk::seed_kernel<false, 1, 1>, (const void*)pvk::seed_kernel<true, 1, 1>};
+  const int tfl = params->fill_mode == PV_FILL_TEMPLATE ? 1 : 0;
+  const int which = (dbg ? 1 : 0) + 2 * mvf + 4 * spl + 8 * tfl;
+  static const void* const seed_fn[16] = {
+      (const void*)pvk::seed_kernel<false, 0, 0, 0>, (const void*)pvk::seed_kernel<true, 0, 0, 0>,
+      (const void*)pvk::seed_kernel<false, 1, 0, 0>, (const void*)pvk::seed_kernel<true, 1, 0, 0>,
+      (const void*)pvk::seed_kernel<false, 0, 1, 0>, (const void*)pvk::seed_kernel<true, 0, 1, 0>,
+      (const void*)pvk::seed_kernel<false, 1, 1, 0>, (const void*)pvk::seed_kernel<true, 1, 1, 0>,
+      (const void*)pvk::seed_kernel<false, 0, 0, 1>, (const void*)pvk::seed_kernel<true, 0, 0, 1>,
+      (const void*)pvk::seed_kernel<false, 1, 0, 1>, (const void*)pvk::seed_kernel<true, 1, 0, 1>,
+      (const void*)pvk::seed_kernel<false, 0, 1, 1>, (const void*)pvk::seed_kernel<true, 0, 1, 1>,
+      (const void*)pvk::seed_kernel<false, 1, 1, 1>, (const void*)pvk::seed_kernel<true, 1, 1, 1>};
   if (!di->attr_set[which] || di->attr_smem[which] < smem) {
     CK(cudaFuncSetAttribute(seed_fn[which], cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     di->attr_set[which] = true;
@@ -213,6 +257,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.trk_cap = (unsigned int)ws_trk_records(n_tracks, params->flavour);
   ka.best = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(ka.ftrk) + (size_t)ka.trk_cap * 32 + 16);
   ka.wrec = reinterpret_cast<float*>(ka.best);                // the two flavours use the same place differently
+  ka.tmpl = reinterpret_cast<int32_t*>(ws + ws_core_bytes(n_events, n_tracks, params->max_vtx_per_event, params->flavour));
   if (dbg) ka.dbg = *dbg;
 
   const bool timing = g_timing != 0;
@@ -224,6 +269,10 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   const int need = (n_events + teams - 1) / teams;
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
+  if (tfl) {                                                  // the table of template histograms, ~10^4 entries
+    pvk::tmpl_kernel<<<kp.tmpl_kmax + 1, 256, 0, stream>>>(kp, ka.tmpl);
+    CK(cudaGetLastError());
+  }
   {
     void* kargs[2] = {(void*)&kp, (void*)&ka};
     CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(teams * pvk::TEAM), kargs, (size_t)smem, stream));
@@ -254,7 +303,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     CK(cudaGetLastError());
   }
   if (timing) { CK(cudaEventRecord(g_ev[3], stream)); g_ev_valid = true; }
-  g_last_kernels = N_KERNELS; g_last_grid = grid;
+  g_last_kernels = N_KERNELS + tfl; g_last_grid = grid;
   return PV_OK;
 }
 
@@ -280,6 +329,7 @@ int pv_params_default(pv_params* p) {
   p->flavour = PV_FLAVOUR_EXPLICIT;
   p->chi2_window = 25.0f;                                           /* P:L384, value: reading R-13 */
   p->split_mode = PV_SPLIT_Z_ORDERED;
+  p->fill_mode = PV_FILL_POLYNOMIAL;
   return PV_OK;
 }
 
@@ -295,7 +345,7 @@ int pv_workspace_bytes(int n_events, long long n_tracks, const pv_params* p, siz
   if (rc != PV_OK) return rc;
   if (n_events < 0 || n_tracks < 0) return PV_E_SIZE;
   if (n_tracks > 0x7fffffffLL) return PV_E_SIZE;
-  *bytes = ws_bytes(n_events, n_tracks, p->max_vtx_per_event, p->flavour);
+  *bytes = ws_bytes(n_events, n_tracks, p);
   return PV_OK;
 }
 
@@ -426,7 +476,7 @@ int pv_host_ctx_create(pv_host_ctx** out, int max_events, long long max_tracks, 
   A((void**)&c->d_ntrk, E * mv * 4); A((void**)&c->d_niter, E * mv * 4); A((void**)&c->d_nvtx, E * 4);
   A((void**)&c->d_w, T * 4); A((void**)&c->d_tv, T * 4); A((void**)&c->d_status, E * 4);
   A((void**)&c->d_tv8, T); A((void**)&c->d_vbegin, (E + HOST_MAX_CHUNKS + 1) * 4); A((void**)&c->d_packed, E * mv * sizeof(pv_vertex));
-  c->ws_stride = (ws_bytes(max_events, max_tracks, c->max_vtx, params->flavour) + 255) / 256 * 256;
+  c->ws_stride = (ws_bytes(max_events, max_tracks, params) + 255) / 256 * 256;
   A((void**)&c->d_ws, (size_t)n_streams * c->ws_stride);
   if (err == cudaSuccess) err = cudaMallocHost((void**)&c->h_total, HOST_MAX_CHUNKS * sizeof(int32_t));
   for (int i = 0; i < n_streams && err == cudaSuccess; ++i) {

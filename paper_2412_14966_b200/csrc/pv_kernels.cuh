@@ -55,6 +55,8 @@ constexpr int FIT_MIN_BLOCKS = 9;   // CTAs per SM: 9 x (24 KB + 1 KB reserved) 
 constexpr int FIT_MIN_BLOCKS_MV = 7;  // multi-vertex flavour: 32 KB of staged records per CTA
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
 constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
+constexpr int TMPL_J = 8;           // template fill: positions of z_poca inside its central bin
+constexpr int TMPL_MAXK = 56;       // template fill: sigma classes (validate() bounds max_sigma_poca / dz)
 
 // Per-team shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
 // The 2 KB that stage the fill (track windows and the unit list) are dead once the histogram is complete; the peak
@@ -94,6 +96,9 @@ struct KParams {
   float mv_e0;                   // exp(-chi2_max / 2), the constant of the denominator of Eq. 19
   int region0_words;             // int32 words of the histogram region (multiple of 32)
   int team_smem_bytes;
+  int tmpl_kmax;                 // template fill (R-17): class of the largest sigma cut = last class
+  int tmpl_off[TMPL_MAXK];       // first table entry of class k; its TMPL_J templates of 2 W_k + 1 bins follow each other
+  short tmpl_w[TMPL_MAXK];       // W_k = ceil(3 sigma_k / dz)
 };
 
 // One vertex seed handed from seed_kernel to fit_kernel (16 bytes, read as one int4).
@@ -120,6 +125,7 @@ struct KArgs {
   unsigned int* fit_counter;     // workspace: next window of seed records of the fit kernel
   SeedRec* rec;                  // workspace: [n_events * max_vtx]
   float4* ftrk;                  // workspace: [T or 2 T][2] fit-ready track records sorted by seed
+  int32_t* tmpl;                 // workspace, template fill: the table of template histograms (tmpl_kernel)
   float* wrec;                   // workspace, explicit flavour: [T] Tukey weight of every track record (record order)
   unsigned long long* best;      // workspace, multi-vertex flavour: [T] largest weight of the track << 32 | 31 - seed
   unsigned int* trk_counter;     // workspace, multi-vertex flavour: track records allocated so far
@@ -139,9 +145,13 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 // The contract's forced Q = 0 for s <= -1 and Q = 2^20 for s >= 1 are reproduced by clamping s to [-1, 1]: the
 // frozen polynomial gives G(1) = 0x1.000098p-1 > 1/2 in this Horner order, so fma(+-1, G(1), 0.5) saturates to
 // exactly 1 / 0.
+__device__ __forceinline__ int cdf_bits(float s);
 __device__ __forceinline__ int edge_r(float kf, float zp, float inv, const KParams& P) {
   const float e = __fmaf_rn(kf, P.dz, P.z_min);
-  float s = __fmul_rn(__fsub_rn(e, zp), inv);
+  return cdf_bits(__fmul_rn(__fsub_rn(e, zp), inv));
+}
+// the CDF of the contract at s = (edge - z_poca) / (3 sigma_poca), as the bits of c + 8
+__device__ __forceinline__ int cdf_bits(float s) {
   s = fminf(fmaxf(s, -1.0f), 1.0f);
   const float t = __fmul_rn(s, s);
   float g = 0x1.3e0392p-3f;
@@ -158,6 +168,40 @@ __device__ __forceinline__ int edge_r(float kf, float zp, float inv, const KPara
 __device__ __forceinline__ int bin_region(int b, const KParams& P) {
   const float centre = __fmaf_rn(__fadd_rn((float)b, 0.5f), P.dz, P.z_min);
   return centre < P.z_split ? 1 : 0;
+}
+
+// ---- template fill ("a finite set of template histograms, selected based on the value of sigma_poca"; R-17) ----
+// Class k has its centre at sigma_k = 0.08 dz 2^(k/4); a track takes the class nearest in log sigma: with
+// v = sigma / (0.08 dz) = m 2^E, m in [1, 2), that is 4 E + the number of class edges 2^((2 q + 1) / 8) m has reached.
+__device__ __forceinline__ int tmpl_class_raw(float sigma, float inv_dz) {
+  const float v = __fmul_rn(__fmul_rn(sigma, inv_dz), 12.5f);
+  if (!(v >= 1.0f)) return 0;
+  if (!(v < 0x1p+20f)) return 80;
+  const unsigned b = __float_as_uint(v);
+  const int E = (int)(b >> 23) - 127;
+  const float m = __uint_as_float((b & 0x007fffffu) | 0x3f800000u);
+  return 4 * E + (m >= 0x1.172b84p+0f ? 1 : 0) + (m >= 0x1.4bfdaep+0f ? 1 : 0) + (m >= 0x1.8ace54p+0f ? 1 : 0) +
+         (m >= 0x1.d5818ep+0f ? 1 : 0);
+}
+__device__ __forceinline__ float tmpl_centre(int k) {          // sigma_k in bins
+  const float c = (k & 3) == 0 ? 1.0f : (k & 3) == 1 ? 0x1.306fe0p+0f : (k & 3) == 2 ? 0x1.6a09e6p+0f : 0x1.ae89fap+0f;
+  return __fmul_rn(ldexpf(c, k >> 2), 0.08f);
+}
+
+// tmpl_kernel: the table of template histograms, one block per sigma class.  Template (k, j) holds, for the relative
+// bins i = -W_k .. W_k, the contract's fixed-point CDF difference Q(i + 1) - Q(i) of a track of width sigma_k whose
+// z_poca is the centre of the j-th eighth of the central bin; it sums to exactly 2^20.
+__global__ void __launch_bounds__(256) tmpl_kernel(const __grid_constant__ KParams P, int32_t* __restrict__ tab) {
+  const int k = blockIdx.x;
+  const int W = P.tmpl_w[k], nb = 2 * W + 1;
+  const float inv = __fdiv_rn(1.0f, __fmul_rn(3.0f, tmpl_centre(k)));
+  for (int idx = threadIdx.x; idx < TMPL_J * nb; idx += blockDim.x) {
+    const int j = idx / nb, i = idx - j * nb - W;
+    const float zrel = __fmul_rn(__fadd_rn((float)j, 0.5f), 1.0f / (float)TMPL_J);
+    const int q0 = cdf_bits(__fmul_rn(__fsub_rn((float)i, zrel), inv));
+    const int q1 = cdf_bits(__fmul_rn(__fsub_rn((float)(i + 1), zrel), inv));
+    tab[P.tmpl_off[k] + idx] = q1 - q0;
+  }
 }
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
@@ -337,13 +381,14 @@ __device__ int split_x86(const int* __restrict__ H, int b0, const KParams& P, in
 // ---- a1: POCA projection of one track (Eq. 1, Eq. 3; fp32 contract of DESIGN.md section 3) ---------------------
 struct Proj {
   float zp, sg, inv;             // z_poca, sigma_poca, 1 / (3 sigma_poca)
+  float frac;                    // position of z_poca inside its central bin, in bins
   int bin;                       // central bin, -1 = not assignable
   bool fill;                     // enters the histogram
 };
 
 __device__ __forceinline__ Proj project(float x, float y, float z, float tx, float ty, float vx, const KParams& P) {
   Proj r;
-  r.zp = __int_as_float(0x7fc00000); r.sg = r.zp; r.inv = 0.0f; r.bin = -1; r.fill = false;
+  r.zp = __int_as_float(0x7fc00000); r.sg = r.zp; r.inv = 0.0f; r.frac = 0.0f; r.bin = -1; r.fill = false;
   const float dtx = __fsub_rn(tx, P.beam_tx), dty = __fsub_rn(ty, P.beam_ty);
   const float den = __fmaf_rn(dty, dty, __fmul_rn(dtx, dtx));
   if (den >= 1e-12f) {                                    // R-3: not parallel to the beamline
@@ -351,9 +396,11 @@ __device__ __forceinline__ Proj project(float x, float y, float z, float tx, flo
     const float num = __fmaf_rn(dty, __fsub_rn(by, y), __fmul_rn(dtx, __fsub_rn(bx, x)));
     r.zp = __fadd_rn(z, __fdiv_rn(num, den));
     r.sg = __fsqrt_rn(__fdiv_rn(vx, den));
-    const float fb = floorf(__fmul_rn(__fsub_rn(r.zp, P.z_min), P.inv_dz));
+    const float fbin = __fmul_rn(__fsub_rn(r.zp, P.z_min), P.inv_dz);
+    const float fb = floorf(fbin);
     if (fb >= 0.0f && fb < (float)P.nbins) {
       r.bin = (int)fb;
+      r.frac = __fsub_rn(fbin, fb);
       const int region = r.zp < P.z_split ? 1 : 0;        // R-5
       r.inv = __fdiv_rn(1.0f, __fmul_rn(3.0f, r.sg));
       r.fill = r.sg > 0.0f && r.sg <= P.max_sigma[region] && r.inv < INFINITY;
@@ -432,7 +479,7 @@ __device__ __forceinline__ void team_sync(int bar) {
   asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(TEAM) : "memory");
 }
 
-template <bool DBG, int FLAV, int SPLIT>
+template <bool DBG, int FLAV, int SPLIT, int FILL>
 __device__ void seed_event(const int e, const int nxt, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt,
                            const int bar) {
   const int lane = tt & 31, tw = tt >> 5;
@@ -520,7 +567,18 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
           if (A.dbg.sigma_poca) A.dbg.sigma_poca[t0 + i] = r.sg;
           if (A.dbg.trk_bin) A.dbg.trk_bin[t0 + i] = r.bin;
         }
-        if (r.fill) {
+        if (r.fill && FILL == PV_FILL_TEMPLATE) {
+          // template fill (R-17): class of sigma_poca, eighth of the bin z_poca falls in; the units of the
+          // window then copy table entries instead of evaluating CDF edges
+          const int k = min(tmpl_class_raw(r.sg, P.inv_dz), P.tmpl_kmax);
+          const int j = min((int)__fmul_rn(r.frac, (float)TMPL_J), TMPL_J - 1);
+          const int W = P.tmpl_w[k];
+          const int lo = max(r.bin - W, 0), hi = min(r.bin + W + 1, P.nbins);
+          const int nb = hi - lo;
+          nun[s] = (nb + UNIT - 1) / UNIT;
+          st_zp[s * TEAM + tt] = __int_as_float(P.tmpl_off[k] + j * (2 * W + 1) + (lo - (r.bin - W)));
+          st_lonb[s * TEAM + tt] = lo | (nb << 12);
+        } else if (r.fill) {
           // window: a superset of the +-3 sigma support; edges outside it give exactly 0 or 2^20
           const float w3 = 3.0f * r.sg;
           const float fa = floorf((r.zp - w3 - P.z_min) * P.inv_dz - P.win_eps);
@@ -570,14 +628,24 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
           tb[b0 >> 5] = 1;
           tb[(b0 + min(rem, UNIT) - 1) >> 5] = 1;
         }
-        const float kf = (float)b0;
-        int r[UNIT + 1];
+        if constexpr (FILL == PV_FILL_TEMPLATE) {
+          const int32_t* tp = A.tmpl + __float_as_int(zp) + u * UNIT;
+          int d[UNIT];
 #pragma unroll
-        for (int j = 0; j <= UNIT; ++j) r[j] = edge_r(kf + (float)j, zp, inv, P);
+          for (int j = 0; j < UNIT; ++j) d[j] = j < rem ? __ldg(tp + j) : 0;
 #pragma unroll
-        for (int j = 0; j < UNIT; ++j) {
-          const int d = r[j + 1] - r[j];
-          if (j < rem && d != 0) atomicAdd(&H[b0 + j], d);
+          for (int j = 0; j < UNIT; ++j)
+            if (d[j] != 0) atomicAdd(&H[b0 + j], d[j]);
+        } else {
+          const float kf = (float)b0;
+          int r[UNIT + 1];
+#pragma unroll
+          for (int j = 0; j <= UNIT; ++j) r[j] = edge_r(kf + (float)j, zp, inv, P);
+#pragma unroll
+          for (int j = 0; j < UNIT; ++j) {
+            const int d = r[j + 1] - r[j];
+            if (j < rem && d != 0) atomicAdd(&H[b0 + j], d);
+          }
         }
       }
     }
@@ -1001,7 +1069,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   }
 }
 
-template <bool DBG, int FLAV, int SPLIT>
+template <bool DBG, int FLAV, int SPLIT, int FILL>
 __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_constant__ KParams P,
                                                                    const __grid_constant__ KArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1021,7 +1089,7 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
   while (e < A.n_events) {
     int nxt = 0x7fffffff;
     if (tt == 32) nxt = (int)atomicAdd(A.evt_counter, 1u); // issued now, consumed by the prefetch and after this event
-    seed_event<DBG, FLAV, SPLIT>(e, nxt, P, A, wsm, tt, bar);
+    seed_event<DBG, FLAV, SPLIT, FILL>(e, nxt, P, A, wsm, tt, bar);
     team_sync(bar);                                        // the team is done with this event's shared memory
     if (tt == 32) misc[8] = nxt;
     team_sync(bar);

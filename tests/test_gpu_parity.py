@@ -491,12 +491,12 @@ def test_full_size_throughput_config(pv, oracle, mode):
     assert rep["n_fragile_events_excused"] <= 0.002 * 100_000
 
 
-@pytest.mark.parametrize("mode", ["explicit", "multivertex", "recursive", "recursive_multivertex"])
+@pytest.mark.parametrize("mode", ["explicit", "multivertex", "recursive", "recursive_multivertex", "template", "template_recursive_multivertex"])
 def test_product_kernels_equal_the_tap_kernels(pv, mode):
     """pv_find (templates without taps) and pv_find_debug (the instantiations the tap tests check against the oracle)
     give bit-identical final outputs: ties every <false, ...> kernel to a tap-checked one.  High pile-up and SMOG2 events."""
     mk = pv.multivertex_params if "multivertex" in mode else pv.default_params
-    p = mk(split_mode=1 if "recursive" in mode else 0)
+    p = mk(split_mode=1 if "recursive" in mode else 0, fill_mode=1 if "template" in mode else 0)
     for idx, n in ((2, 2000), (1, 4000)):
         data = events.generate(events.config(idx, n))
         a = pv.find(data, p)
@@ -593,3 +593,71 @@ def test_host_pipeline_matches_device_path(pv, cfg0, mode):
     with pytest.raises(pv.PvError):
         hp.find(data, small, n_chunks=4)
     hp.close()
+
+
+@pytest.mark.parametrize("idx,n,mv", [(0, 1000, False), (1, 3000, False), (2, 1000, False), (3, 3000, False), (1, 1500, True)])
+def test_template_fill(pv, oracle, idx, n, mv):
+    """fill_mode = PV_FILL_TEMPLATE (the paper's x86 fill, reading R-17): histograms bit-exact against the
+    oracle in the same mode (the table of templates is rebuilt on the device at every call), every later tap as for the
+    polynomial fill; the product kernel equals the tap kernel."""
+    from oracle import compare
+    data = events.generate(events.config(idx, n))
+    mk_p, mk_o = (pv.multivertex_params, oracle.mv_params) if mv else (pv.default_params, oracle.default_params)
+    p, po = mk_p(fill_mode=1), mk_o(fill_mode=1)
+    got = pv.find(data, p, debug=True, n_hist_events=400)
+    assert pv.last_launch_info()["n_kernels"] == 4
+    ref = oracle.find(data, po, debug=True, n_hist_events=400, trace=True, n_threads=NTHREADS)
+    rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep)
+    assert rep["hist_mismatch"] == 0 and rep["seed_bins_mismatch"] == 0 and rep["seed_z_mismatch"] == 0
+    # it is another histogram than the polynomial fill's
+    poly = oracle.find(data, mk_o(), debug=True, n_hist_events=400, n_threads=NTHREADS)
+    assert (poly["debug"]["hist"] != ref["debug"]["hist"]).any()
+    plain = pv.find(data, p)
+    m = np.arange(p.max_vtx_per_event)[None, :] < plain["n_vtx"][:, None]
+    for k in plain:
+        x, y = (plain[k][m], got[k][m]) if k.startswith("vtx_") else (plain[k], got[k])
+        assert np.array_equal(x, y, equal_nan=True), k
+
+
+def test_template_fill_other_binning_and_wide_tracks(pv, oracle):
+    """Another bin size (the classes are defined in bins), a larger sigma cut (more classes), recursive splitting, and
+    p-gas tracks several mm wide whose templates span hundreds of bins and leave the range at its lower end."""
+    data = events.generate(events.config(1, 1200))
+    _, _, rep = _both(pv, oracle, data, n_hist=200, fill_mode=1, dz=0.5, split_mode=1)
+    _assert_parity(rep)
+    _, _, rep = _both(pv, oracle, data, n_hist=200, fill_mode=1, max_sigma_poca=(3.0, 20.0))
+    _assert_parity(rep)
+    rng = np.random.default_rng(17)
+    n = 150
+    sig = rng.uniform(0.2, 0.7, n).astype(np.float32)
+    ev = dict(x=(sig * rng.normal(0, 1, n)).astype(np.float32), y=(sig * rng.normal(0, 1, n)).astype(np.float32),
+              z=np.full(n, -535.0, np.float32), tx=rng.normal(0, 0.08, n).astype(np.float32),
+              ty=rng.normal(0, 0.08, n).astype(np.float32), var_x=sig * sig, var_y=sig * sig,
+              var_tx=np.full(n, 1e-6, np.float32), var_ty=np.full(n, 1e-6, np.float32))
+    got, ref, rep = _both(pv, oracle, events.from_lists([ev, ev]), fill_mode=1)
+    _assert_parity(rep)
+    assert rep["hist_mismatch"] == 0 and (ref["debug"]["sigma_poca"][:n] > 4.0).sum() > 20 and ref["debug"]["hist"][0][:8].sum() > 0
+
+
+def test_fill_and_splitting_variants_on_close_pairs(pv):
+    """the alternatives of P:L131 / P:L137 compared on configs[3] -- the fraction of events in which
+    two vertices are reconstructed, by pair separation (0.1 .. 5 mm), for polynomial / template fill and z-ordered /
+    recursive splitting.  "the algorithm cannot separate vertices that are closer than about 2 mm"."""
+    data = events.generate(events.config(3, 6000))
+    sep = np.array([0.1, 0.2, 0.5, 1.0, 2.0, 5.0])
+    which = np.arange(6000) % 6
+    table = {}
+    for fill in (0, 1):
+        for split in (0, 1):
+            r = pv.find(data, pv.default_params(fill_mode=fill, split_mode=split))
+            table[(fill, split)] = [float((r["n_vtx"][which == q] >= 2).mean()) for q in range(6)]
+            print("fill", ["polynomial", "template"][fill], "split", ["z-ordered", "recursive"][split],
+                  dict(zip(sep.tolist(), np.round(table[(fill, split)], 3).tolist())))
+    for key, frac in table.items():
+        assert frac[0] < 0.02 and frac[1] < 0.05 and frac[5] > 0.97, (key, frac)   # merged at 0.1-0.2 mm, resolved at 5 mm
+        assert frac[3] < frac[4] <= frac[5] + 1e-9                               # resolution turns on between 1 and 2 mm
+    ref = np.array(table[(0, 0)])
+    for key, frac in table.items():
+        assert np.abs(np.array(frac) - ref).max() < 0.08, (key, frac)             # the variants agree to a few per cent
