@@ -522,6 +522,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       if (DBG && A.dbg.n_seeds) A.dbg.n_seeds[e] = 0;
       if (DBG && A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = 0;
     }
+    team_sync(bar);                                          // every path through an event holds a team barrier (seed_kernel)
     return;
   }
 
@@ -844,34 +845,12 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     int* mycnt = cnt + tw * 32;
     mycnt[lane] = 0;
     __syncwarp();
-    unsigned hmask[SLOTS];
-    float hden[SLOTS];
     auto count = [&](int k, unsigned peers) {
       if (k >= 0 && (peers & lanemask_lt()) == 0) mycnt[k] += __popc(peers);
     };
-#pragma unroll
-    for (int sl = 0; sl < SLOTS; ++sl) {
-      hmask[sl] = 0u; hden[sl] = 0.0f;
-      if (sl * TEAM + tw * 32 < n) { cand(sl * TEAM + tt, held[sl], hmask[sl], hden[sl]); for_bits(hmask[sl], count); }
-    }
-#pragma unroll 1
-    for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) {
-      unsigned mk; float dn;
-      cand(i0 + lane, load_raw(i0 + lane), mk, dn);
-      for_bits(mk, count);
-    }
-    team_sync(bar);
-    const int myc = lane < ns ? cnt[lane] + cnt[32 + lane] : 0;
-    const int inc = warp_incl_scan(myc, lane);
-    const int nrec = __shfl_sync(FULL, inc, 31);             // (track, seed) records of the event
-    if (tt == 0) misc[5] = (int)atomicAdd(A.trk_counter, (unsigned)nrec);
-    team_sync(bar);
-    const unsigned rbeg = (unsigned)misc[5];
-    const bool ovf = rbeg + (unsigned)nrec > A.trk_cap || rbeg + (unsigned)nrec < rbeg;
-    if (ovf) { status |= PV_EVT_RECORD_OVERFLOW; ns = 0; }
-    const int myoff = inc - myc;
-    cur[lane] = (int)rbeg + myoff + (tw ? cnt[lane] : 0);
-    __syncwarp();
+    int myc = 0, myoff = 0;
+    unsigned rbeg = 0u;
+    bool ovf = false;
     auto emit = [&](const int i, const RawTrk& R, const unsigned mask, const float den) {
       if (i < n) A.best[t0 + i] = 0ull;
       float cx, cy;
@@ -891,15 +870,47 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         if (k >= 0 && rank == 0) cur[k] += __popc(peers);
       });
     };
-#pragma unroll
-    for (int sl = 0; sl < SLOTS; ++sl)
-      if (sl * TEAM + tw * 32 < n) emit(sl * TEAM + tt, held[sl], hmask[sl], hden[sl]);
+    // Two passes over the tracks in the same order: pass 0 counts the (track, seed) pairs per seed, pass 1 writes their
+    // records at the counted places.  ONE loop body serves both passes and both kinds of tracks (the first CHUNK are
+    // still in registers, the others are read again): with the candidate and record code inlined once instead of
+    // four / three times the kernel is 30 % smaller, and its 28 warps in different phases stopped missing the
+    // instruction cache (3.3 no-instruction stall cycles per issue before).
+    static_assert(SLOTS == 2, "the two register-held tracks of a lane are selected by hand");
+    unsigned hm0 = 0u, hm1 = 0u;                             // seeds listing my two register-held tracks, their Eq. 19 denominators
+    float hd0 = 0.0f, hd1 = 0.0f;
 #pragma unroll 1
-    for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) {
-      const RawTrk Q = load_raw(i0 + lane);
-      unsigned mk; float dn;
-      cand(i0 + lane, Q, mk, dn);
-      emit(i0 + lane, Q, mk, dn);
+    for (int pass = 0; pass < 2; ++pass) {
+#pragma unroll 1
+      for (int it = 0, i0 = tw * 32; i0 < n; ++it, i0 += TEAM) {
+        const int i = i0 + lane;
+        RawTrk Q;
+        if (it < SLOTS) Q = it == 0 ? held[0] : held[1];
+        else Q = load_raw(i);
+        unsigned mk = it == 0 ? hm0 : hm1;
+        float dn = it == 0 ? hd0 : hd1;
+        if (pass == 0 || it >= SLOTS) cand(i, Q, mk, dn);
+        if (pass == 0) {
+          if (it == 0) { hm0 = mk; hd0 = dn; }
+          else if (it == 1) { hm1 = mk; hd1 = dn; }
+          for_bits(mk, count);
+        } else {
+          emit(i, Q, mk, dn);
+        }
+      }
+      if (pass == 0) {
+        team_sync(bar);
+        myc = lane < ns ? cnt[lane] + cnt[32 + lane] : 0;
+        const int inc = warp_incl_scan(myc, lane);
+        const int nrec = __shfl_sync(FULL, inc, 31);         // (track, seed) records of the event
+        if (tt == 0) misc[5] = (int)atomicAdd(A.trk_counter, (unsigned)nrec);
+        team_sync(bar);
+        rbeg = (unsigned)misc[5];
+        ovf = rbeg + (unsigned)nrec > A.trk_cap || rbeg + (unsigned)nrec < rbeg;
+        if (ovf) { status |= PV_EVT_RECORD_OVERFLOW; ns = 0; }
+        myoff = inc - myc;
+        cur[lane] = (int)rbeg + myoff + (tw ? cnt[lane] : 0);
+        __syncwarp();
+      }
     }
     if (tw == 0) {
       int rbase = 0;
@@ -1090,7 +1101,8 @@ __global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_
     int nxt = 0x7fffffff;
     if (tt == 32) nxt = (int)atomicAdd(A.evt_counter, 1u); // issued now, consumed by the prefetch and after this event
     seed_event<DBG, FLAV, SPLIT, FILL>(e, nxt, P, A, wsm, tt, bar);
-    team_sync(bar);                                        // the team is done with this event's shared memory
+    // misc[8] was last read before this event, and both warps have met at a barrier inside it since: the next event can
+    // be published ahead of the barrier that also says the team is done with this event's shared memory
     if (tt == 32) misc[8] = nxt;
     team_sync(bar);
     e = misc[8];
@@ -1251,6 +1263,9 @@ __device__ __forceinline__ void store_dead(float4 (*SA)[32], typename FitB<FLAV>
 }
 
 enum { FS_EMPTY = 0, FS_LOAD = 1, FS_ITER = 2, FS_FINAL = 3, FS_DONE = 4 };
+#ifndef PV_FIT_WPW
+#define PV_FIT_WPW 2        // measured on configs[1]: 1 -> 0.387 ms (multi-vertex 0.540), 2 -> 0.366 (0.384), 4 -> 0.366 (0.414)
+#endif
 #ifndef PV_FIT_LOADWAIT
 #define PV_FIT_LOADWAIT 0        // ticks a group sits out after starting the copy of its next seed before it waits for the data
                                  // (measured on configs[1]: 0 -> 0.387 ms, 1 -> 0.405 ms; an L2 prefetch one seed ahead did not help)
@@ -1480,8 +1495,9 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
   BT(*SB)[32] = s_b[warp];
   const int total = (int)*A.seed_counter;
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
-  // window size: one window per warp when the batch allows (all warps then finish together), at most FIT_WIN
-  int win = (total + nwarps - 1) / nwarps;
+  // window size: PV_FIT_WPW windows per warp when the batch allows, claimed one after the other (the windows of a
+  // batch take different times; several per warp even that out), at most FIT_WIN records
+  int win = (total + PV_FIT_WPW * nwarps - 1) / (PV_FIT_WPW * nwarps);
   win = min(max((win + 31) & ~31, 32), FIT_WIN);
   const int nwin = (total + win - 1) / win;
   const Trk dead = dead_track(P);
