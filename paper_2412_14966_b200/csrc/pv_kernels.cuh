@@ -757,18 +757,19 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   }
   team_sync(bar);
   if (tw == 0) {
-    if (misc[6] == 0) {
-      sweep_all(misc[2], misc[3]);
-    } else {                                               // rounds of <= PROTO_CAP proto-clusters over all words
-      int i = 0;
+    // normally one call over the two lists; after a list overflow (misc[6]), rounds of <= PROTO_CAP proto-clusters
+    // over all words.  One call site, so that the sweep is inlined once.
+    const bool rounds = misc[6] != 0;
+    int i = 0, n0 = misc[2], n1 = misc[3];
 #pragma unroll 1
-      while (i < ntw) {
+    do {
+      if (rounds) {
         __syncwarp();
-        const int np_ = detect(i, ntw, ps0);
+        n0 = detect(i, ntw, ps0); n1 = 0;
         __syncwarp();
-        sweep_all(np_, 0);
       }
-    }
+      sweep_all(n0, n1);
+    } while (rounds && i < ntw);
     __syncwarp();
     const int nsw = min(n_raw, P.max_vtx);
     if (lane < nsw) {                                      // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
@@ -1042,11 +1043,15 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     if (s >= 0 && rank == 0) cur[s] += __popc(m);
     __syncwarp();
   };
-#pragma unroll
-  for (int sl = 0; sl < SLOTS; ++sl)
-    if (sl * TEAM + tw * 32 < n) place(sl * TEAM + tt, held[sl], false, ns > 0 ? sheld[sl] : -1);
+  // one loop body for the register-held tracks (the first two of a lane) and for those read again from memory: the
+  // record code is inlined once (a smaller kernel misses the instruction cache less, see the multi-vertex branch)
 #pragma unroll 1
-  for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) place(i0 + lane, held[0], true, seed_of(i0 + lane));
+  for (int it = 0, i0 = tw * 32; i0 < n; ++it, i0 += TEAM) {
+    const bool regs = it < SLOTS;
+    const RawTrk Q = it == 0 ? held[0] : held[1];
+    const int s = !regs ? seed_of(i0 + lane) : (ns > 0 ? (it == 0 ? sheld[0] : sheld[1]) : -1);
+    place(i0 + lane, Q, !regs, s);
+  }
   // seed records for fit_kernel
   if (tw == 0) {
     int rbase = 0;
