@@ -1043,15 +1043,11 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     if (s >= 0 && rank == 0) cur[s] += __popc(m);
     __syncwarp();
   };
-  // one loop body for the register-held tracks (the first two of a lane) and for those read again from memory: the
-  // record code is inlined once (a smaller kernel misses the instruction cache less, see the multi-vertex branch)
+#pragma unroll
+  for (int sl = 0; sl < SLOTS; ++sl)
+    if (sl * TEAM + tw * 32 < n) place(sl * TEAM + tt, held[sl], false, ns > 0 ? sheld[sl] : -1);
 #pragma unroll 1
-  for (int it = 0, i0 = tw * 32; i0 < n; ++it, i0 += TEAM) {
-    const bool regs = it < SLOTS;
-    const RawTrk Q = it == 0 ? held[0] : held[1];
-    const int s = !regs ? seed_of(i0 + lane) : (ns > 0 ? (it == 0 ? sheld[0] : sheld[1]) : -1);
-    place(i0 + lane, Q, !regs, s);
-  }
+  for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) place(i0 + lane, held[0], true, seed_of(i0 + lane));
   // seed records for fit_kernel
   if (tw == 0) {
     int rbase = 0;
@@ -1580,7 +1576,7 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
 // arrays), the duplicate sweep runs on shuffles, survivors are compacted in place in z order, and every
 // track gets its final vertex index (weight 0 when it has none).
 #ifndef PV_CLEANUP_MIN_BLOCKS
-#define PV_CLEANUP_MIN_BLOCKS 6
+#define PV_CLEANUP_MIN_BLOCKS 8
 #endif
 template <bool DBG, int FLAV>
 __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(const __grid_constant__ KParams P,
@@ -1635,9 +1631,10 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
       const int nv = __shfl_sync(FULL, vntrk, v);
       bool take = true;
       if (s >= 0) {
-        const float dzv = zv - zs_;
-        const float ratio = dzv * dzv / (cv + cs_);
-        if (ratio < P.merge_ratio) {
+        const float dzv = zv - zs_, csum = cv + cs_;
+        // dz^2 / (Czz_v + Czz_s) < merge_ratio without the division (the sum of two variances is positive)
+        const bool dup = csum > 0.0f ? dzv * dzv < P.merge_ratio * csum : dzv * dzv / csum < P.merge_ratio;
+        if (dup) {
           if (nv > ns_) merged |= 1u << s;
           else { merged |= 1u << v; take = false; }
         }
