@@ -48,11 +48,21 @@ constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT
 constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
 constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int FIT_UNROLL = PV_FIT_UNROLL;   // unroll of the track loop of one fit iteration
-constexpr int FIT_KF = 16;          // track slots per lane in shared memory: G lanes hold a seed of up to G * FIT_KF tracks
+#ifndef PV_FIT_KF
+#define PV_FIT_KF 14
+#endif
+#ifndef PV_FIT_KF_MV
+#define PV_FIT_KF_MV 12
+#endif
+// track slots per lane in shared memory: G lanes hold a seed of up to G * KF tracks.  Fewer slots send more seeds to
+// the next group size but let more warps live on an SM; measured on configs[1], explicit flavour (24 B per slot and
+// lane): 16 slots / 18 warps 0.366 ms, 14 / 20 0.344, 12 / 22 0.367, 10 / 26 0.429; multi-vertex (32 B): 16 / 12 0.383, 12 / 16 0.362
+constexpr int FIT_KF = PV_FIT_KF;
+constexpr int FIT_KF_MV = PV_FIT_KF_MV;
 constexpr int FIT_WIN = 256;        // seed records of one window of the fit (its sorted order is held as 8 bytes per lane)
 constexpr int FIT_BLOCK = 64;       // threads per CTA of fit_kernel (warps are autonomous; 12 KB of tracks per warp)
-constexpr int FIT_MIN_BLOCKS = 9;   // CTAs per SM: 9 x (24 KB + 1 KB reserved) fill the shared memory
-constexpr int FIT_MIN_BLOCKS_MV = 7;  // multi-vertex flavour: 32 KB of staged records per CTA
+constexpr int FIT_MIN_BLOCKS = 10;  // CTAs per SM: 10 x (21 KB + 1 KB reserved) fill the shared memory
+constexpr int FIT_MIN_BLOCKS_MV = 8;  // multi-vertex flavour: 24 KB of staged records per CTA
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
 constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
 constexpr int TMPL_J = 8;           // template fill: positions of z_poca inside its central bin
@@ -1426,7 +1436,7 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
   }
 }
 
-// Seeds with more tracks than 32 lanes x FIT_KF slots hold (> 512; only constructed events): the whole warp strides
+// Seeds with more tracks than 32 lanes x KF slots hold (> 448 / 384; only constructed events): the whole warp strides
 // over the seed's records in global memory (contiguous, L1-resident after the first iteration).
 template <int FLAV>
 __device__ void fit_huge(const KParams& P, const KArgs& A, const int4 r, const int lane) {
@@ -1489,8 +1499,9 @@ template <int FLAV>
 __global__ void __launch_bounds__(FIT_BLOCK, FLAV ? FIT_MIN_BLOCKS_MV : FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
   using BT = typename FitB<FLAV>::type;
-  __shared__ __align__(16) float4 s_a[FIT_BLOCK / 32][FIT_KF][32];   // {x0, y0, tx, ty}
-  __shared__ __align__(16) BT s_b[FIT_BLOCK / 32][FIT_KF][32];       // {Wx, Wy} or {Wx, Wy, track index, oth}
+  constexpr int KF = FLAV == PV_FLAVOUR_MULTIVERTEX ? FIT_KF_MV : FIT_KF;
+  __shared__ __align__(16) float4 s_a[FIT_BLOCK / 32][KF][32];       // {x0, y0, tx, ty}
+  __shared__ __align__(16) BT s_b[FIT_BLOCK / 32][KF][32];           // {Wx, Wy} or {Wx, Wy, track index, oth}
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float4(*SA)[32] = s_a[warp];
   BT(*SB)[32] = s_b[warp];
@@ -1502,7 +1513,7 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
   win = min(max((win + 31) & ~31, 32), FIT_WIN);
   const int nwin = (total + win - 1) / win;
   const Trk dead = dead_track(P);
-  int filled = FIT_KF;                                       // slots of my column that may hold something else than a dead track
+  int filled = KF;                                           // slots of my column that may hold something else than a dead track
 #pragma unroll 1
   for (;;) {
     int w = 0;
@@ -1523,7 +1534,7 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
       if (r < wn) {
         const int m = __ldg(&A.rec[wb + r].k_cnt) >> 5;
         if (m > 0) {
-          const int ph = m <= 2 * FIT_KF ? 0 : m <= 4 * FIT_KF ? 1 : m <= 8 * FIT_KF ? 2 : m <= 16 * FIT_KF ? 3 : m <= 32 * FIT_KF ? 4 : 5;
+          const int ph = m <= 2 * KF ? 0 : m <= 4 * KF ? 1 : m <= 8 * KF ? 2 : m <= 16 * KF ? 3 : m <= 32 * KF ? 4 : 5;
           const int slots = ph < 5 ? (m + (2 << ph) - 1) >> (ph + 1) : 1;
           key[i] = ph * 16 + 16 - slots;                         // within a phase: most slots first, so the drain at the
                                                                    // end of the phase (idle lanes) runs on short ticks
