@@ -405,7 +405,10 @@ int pv_track_ip(const float* x, const float* y, const float* z, const float* tx,
   ka.var_x = var_x; ka.var_y = var_y; ka.var_tx = var_tx; ka.var_ty = var_ty;
   if (cov) { ka.cov_xtx = cov->cov_xtx; ka.cov_yty = cov->cov_yty; }
   ka.offsets = offsets; ka.n_events = n_events;
-  pvk::ip_kernel<<<(n_events + 7) / 8, 256, 0, (cudaStream_t)stream_>>>(kp, ka, vtx_pos, vtx_cov, n_vtx, ip, ip_chi2, ip_vertex);
+  if (ka.cov_xtx || ka.cov_yty)
+    pvk::ip_kernel<true><<<(n_events + 7) / 8, 256, 0, (cudaStream_t)stream_>>>(kp, ka, vtx_pos, vtx_cov, n_vtx, ip, ip_chi2, ip_vertex);
+  else
+    pvk::ip_kernel<false><<<(n_events + 7) / 8, 256, 0, (cudaStream_t)stream_>>>(kp, ka, vtx_pos, vtx_cov, n_vtx, ip, ip_chi2, ip_vertex);
   CK(cudaGetLastError());
   return PV_OK;
 }

@@ -449,8 +449,9 @@ struct RawTrk { float x, y, z, tx, ty, vx, vy, vtx, vty; };
 // Eq. 2 for one coordinate at dz = z - z_trk: V_xx + 2 dz V_xtx + dz^2 V_txtx.  With a cross term the three
 // terms cancel when the state is given far from the vertex (at 150 mm they are 25 x the result), so that one expression
 // is evaluated in double (once per record, not per iteration); the diagonal case has only positive terms.
-__device__ __forceinline__ float var_at(float v, float vt, float c, float dz) {
-  if (c != 0.0f) {
+// `cross` (warp-uniform: cross terms were passed to the call) keeps the double path out of the diagonal case.
+__device__ __forceinline__ float var_at(float v, float vt, float c, float dz, bool cross) {
+  if (cross && c != 0.0f) {
     const double d = (double)dz;
     return (float)fma(d, fma(d, (double)vt, 2.0 * (double)c), (double)v);
   }
@@ -458,7 +459,8 @@ __device__ __forceinline__ float var_at(float v, float vt, float c, float dz) {
 }
 
 // cx, cy: the track's V_xtx, V_yty (0 for a diagonal covariance)
-__device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, float cx, float cy, float sx, float sy, float zsv) {
+__device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, float cx, float cy, float sx, float sy, float zsv,
+                                          bool cross) {
   Trk T;
   const float zl = R.z - zsv;
   T.tx = R.tx; T.ty = R.ty;
@@ -473,8 +475,8 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
     T.x0 = fmaf(-zl, R.tx, R.x - sx);
     T.y0 = fmaf(-zl, R.ty, R.y - sy);
   }
-  const float Vx = var_at(R.vx, R.vtx, cx, -zl);
-  const float Vy = var_at(R.vy, R.vty, cy, -zl);
+  const float Vx = var_at(R.vx, R.vtx, cx, -zl, cross);
+  const float Vy = var_at(R.vy, R.vty, cy, -zl, cross);
   const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);   // R-7
   T.Wx = __fdividef(1.0f, Vx);
   T.Wy = __fdividef(1.0f, Vy);
@@ -515,6 +517,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   const int t0 = __ldg(A.offsets + e);
   const int n = __ldg(A.offsets + e + 1) - t0;
   const size_t ev = (size_t)e * P.max_vtx;
+  const bool have_cross = A.cov_xtx != nullptr || A.cov_yty != nullptr;   // Eq. 2 with its x-tx / y-ty elements
   unsigned status = 0;
 
   // explicit flavour: the fit-ready records of the event go to ftrk[t0 .. t0 + n): refuse what the workspace cannot hold
@@ -823,7 +826,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       const float zsv = zs[k];
       const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
       const float dzv = zsv - R.z;
-      const float Vx = var_at(R.vx, R.vtx, cx, dzv), Vy = var_at(R.vy, R.vty, cy, dzv);
+      const float Vx = var_at(R.vx, R.vtx, cx, dzv, have_cross), Vy = var_at(R.vy, R.vty, cy, dzv, have_cross);
       const bool ok = (Vx > 0.0f) && (Vy > 0.0f) && (Vx < INFINITY) && (Vy < INFINITY);
       const float rx = fmaf(dzv, R.tx, R.x) - sx, ry = fmaf(dzv, R.ty, R.y) - sy;
       const float c = fmaf(rx * rx, __fdividef(1.0f, Vx), ry * ry * __fdividef(1.0f, Vy));
@@ -871,7 +874,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         if (k >= 0) {
           const float zsv = zs[k];
           const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-          const Trk T = make_track(P, R, cx, cy, sx, sy, zsv);
+          const Trk T = make_track(P, R, cx, cy, sx, sy, zsv, have_cross);
           const float oth = fmaxf(den - __expf(-0.5f * chi2_at(R, cx, cy, k)), 0.5f * P.mv_e0);
           float4* o = A.ftrk + 2 * (size_t)(cur[k] + rank);
           o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
@@ -1044,7 +1047,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
       const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
       const float cx = A.cov_xtx ? __ldg(A.cov_xtx + t0 + i) : 0.0f, cy = A.cov_yty ? __ldg(A.cov_yty + t0 + i) : 0.0f;
-      const Trk T = make_track(P, Q, cx, cy, sx, sy, zsv);
+      const Trk T = make_track(P, Q, cx, cy, sx, sy, zsv, have_cross);
       float4* o = A.ftrk + 2 * (size_t)(t0 + cur[s] + rank);
       o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
       o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), 0.0f);
@@ -1771,6 +1774,7 @@ __global__ void __launch_bounds__(256) pack_vertices_kernel(const __grid_constan
 // For a vertex that does not contain the track: r = Eq. 9 residual at the vertex z, IP = distance of the line to the
 // point, IP chi2 = r^T (V + H C H^T)^-1 r with V from Eq. 2 (diagonal) at the vertex z, H of Eq. 12.
 // One pass over 36 B/track in, 12 B/track out: HBM-bound.
+template <bool CROSS>
 __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A,
                                                  const float* __restrict__ vpos, const float* __restrict__ vcov,
                                                  const int32_t* __restrict__ nvtx, float* __restrict__ ip,
@@ -1782,6 +1786,7 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
   const int t0 = __ldg(A.offsets + e);
   const int n = __ldg(A.offsets + e + 1) - t0;
   const int nv = min(__ldg(nvtx + e), P.max_vtx);
+  constexpr bool have_cross = CROSS;                       // compiled twice: the diagonal case carries no double arithmetic
   if (lane < nv) {
     const size_t o = (size_t)e * P.max_vtx + lane;
 #pragma unroll
@@ -1797,7 +1802,7 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const int g = t0 + min(i0 + 32 * u, n - 1);
-      cx[u] = A.cov_xtx ? __ldg(A.cov_xtx + g) : 0.0f; cy[u] = A.cov_yty ? __ldg(A.cov_yty + g) : 0.0f;
+      cx[u] = (CROSS && A.cov_xtx) ? __ldg(A.cov_xtx + g) : 0.0f; cy[u] = (CROSS && A.cov_yty) ? __ldg(A.cov_yty + g) : 0.0f;
       x[u] = __ldg(A.x + g); y[u] = __ldg(A.y + g); z[u] = __ldg(A.z + g); a[u] = __ldg(A.tx + g); b[u] = __ldg(A.ty + g);
       vx[u] = __ldg(A.var_x + g); vy[u] = __ldg(A.var_y + g); vtx[u] = __ldg(A.var_tx + g); vty[u] = __ldg(A.var_ty + g);
     }
@@ -1816,7 +1821,7 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const float dz = q2 - z[u];
-        const float Vx = var_at(vx[u], vtx[u], cx[u], dz), Vy = var_at(vy[u], vty[u], cy[u], dz);
+        const float Vx = var_at(vx[u], vtx[u], cx[u], dz, have_cross), Vy = var_at(vy[u], vty[u], cy[u], dz, have_cross);
         const float rx = fmaf(dz, a[u], x[u] - q0), ry = fmaf(dz, b[u], y[u] - q1);
         const float Sxx = fmaf(a[u], fmaf(a[u], q8, -2.0f * q5), Vx + q3);
         const float Syy = fmaf(b[u], fmaf(b[u], q8, -2.0f * q7), Vy + q6);
