@@ -9,12 +9,15 @@
 //                           one lane per proto-cluster for the z-ordered hysteresis sweep, seed positions,
 //                           association (explicit with the removal loop, or the multi-vertex chi2 window),
 //                           deterministic counting sort -> seed records and fit-ready track records in HBM.
-//   fit_kernel      a5      2 lanes per vertex seed, flat over all seeds of the batch (no histogram): windows of 32
-//                           seed records sorted by track count, tracks staged by cp.async into a conflict-free
-//                           shared-memory slice, xor-shuffle reduction of the normal equations, closed-form solve of
-//                           the arrow-shaped 3x3 Hessian; Tukey (Eq. 18) or multi-vertex (Eq. 19) weights.
+//   fit_kernel      a5      flat over all seeds of the batch (no histogram): a warp counting-sorts a window of seed
+//                           records and works through it as a queue, 2 / 4 / ... 32 lanes per seed, tracks staged by
+//                           cp.async into conflict-free shared-memory columns; one tick = one Newton iteration of every
+//                           seed in flight; a converged seed frees its lanes in the same tick; closed-form solve of the
+//                           arrow-shaped 3x3 Hessian; Tukey (Eq. 18) or multi-vertex (Eq. 19) weights.
 //   cleanup_kernel  a6      one warp per event: z-ordered duplicate sweep, cuts, compaction, final per-track
 //                           vertex index and weight.
+//   tmpl_kernel     a2'     table of template histograms for the x86 variant of the fill, rebuilt per call.
+//   scan_nvtx_kernel, pack_vertices_kernel   compact read-back of the host pipeline.
 //   ip_kernel       NEXT-4  impact parameter / IP chi2 of every track w.r.t. the PVs of its event (pv_track_ip).
 //
 // The v1 single fused kernel (profiles/r1_v1_fused_kernel.md) was 87 KB of SASS and lost 42 % of its issue
