@@ -345,7 +345,7 @@ def main_ours(args):
     assert sum(alg_k.values()) == alg
     # DRAM bytes per launch from the committed `ncu --set full` capture: accepted only when the capture was made with
     # the kernels of this working tree (hash recorded beside it), else reported as stale
-    traffic_k, traffic_src = {}, "none for this workload"
+    traffic_k, inst_k, traffic_src = {}, {}, "none for this workload"
     tpath = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     sha = kernels_sha()
     if os.path.exists(tpath):
@@ -355,6 +355,8 @@ def main_ours(args):
                     and args.split == "z_ordered" and args.fill == "polynomial":
                 if row.get("kernels_sha") == sha:
                     traffic_k[row["kernel"]] = int(row["dram_bytes_per_launch"])
+                    if row.get("warp_inst_per_launch"):
+                        inst_k[row["kernel"]] = int(row["warp_inst_per_launch"])
                     traffic_src = f"profiles/{row['source']} (ncu dram__bytes_read.sum + dram__bytes_write.sum, kernels {sha})"
                 else:
                     traffic_src = f"stale: profiles/dram_traffic.csv was captured with kernels {row.get('kernels_sha')}, this tree is {sha}"
@@ -364,6 +366,17 @@ def main_ours(args):
                 "traffic": traffic_k.get(n)} for i, n in enumerate(KERNELS)]
     dom = max(kernels, key=lambda k: k["ms"])
     achieved = dom["achieved_gbs"]
+    # what actually binds the path: warp-instructions issued against 148 SMs x 4 schedulers x the
+    # SM clock; instruction counts from the same ncu capture as the traffic (same staleness check), time measured live
+    issue = None
+    if len(inst_k) == len(KERNELS):
+        clk = sampler.summary().get("sm_mhz") or 1965.0
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_issue = sms * 4 * clk * 1e6 / 1e9
+        ach = sum(inst_k.values()) / (ms_step * 1e-3) / 1e9
+        issue = {"bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-instructions/s", "frac": ach / peak_issue,
+                 "warp_instructions_per_step": sum(inst_k.values()),
+                 "peak_source": f"{sms} SMs x 4 schedulers x {clk:.0f} MHz (one warp-instruction per scheduler and cycle)"}
 
     # ---- cpu_baseline: the oracle, as it stands, on this box's host cores --------------------------------------
     cores = os.cpu_count() or 1
@@ -407,8 +420,9 @@ def main_ours(args):
                      "kernels": kernels,
                      "path": {"algorithmic_bytes_per_step": alg, "ms_per_step": ms_step,
                               "achieved": alg / (ms_step * 1e-3) / 1e9, "frac": alg / (ms_step * 1e-3) / 1e9 / peak},
-                     "note": "rank 0's kernels; the path is issue-bound, not HBM-bound (DESIGN.md section 8: warp-instructions "
-                             "per step against 148 SMs x 4 schedulers x the SM clock); BASELINE.json asks for the HBM fraction"},
+                     "issue": issue,
+                     "note": "rank 0's kernels; the path is issue- and latency-bound, not HBM-bound (DESIGN.md section 8; "
+                             "`issue` holds that roofline); BASELINE.json asks for the HBM fraction, reported here"},
         "cpu_baseline": cpu,
     }
     if ip_info is not None:

@@ -661,3 +661,40 @@ def test_fill_and_splitting_variants_on_close_pairs(pv):
     ref = np.array(table[(0, 0)])
     for key, frac in table.items():
         assert np.abs(np.array(frac) - ref).max() < 0.08, (key, frac)             # the variants agree to a few per cent
+
+
+@pytest.mark.parametrize("mv", [False, True])
+def test_seeds_of_every_group_size(pv, oracle, mv):
+    """One vertex per event with 5 .. 1900 tracks: the fit handles a seed with 2, 4, 8, 16 or 32 lanes according to its
+    track count (up to 28, 56, 112, 224, 448 tracks in the explicit flavour; 24 .. 384 in the multi-vertex one) and with
+    the whole-warp global-memory loop beyond that; every size class must give the oracle's vertex."""
+    from oracle import compare
+    rng = np.random.default_rng(31)
+    evs = []
+    sizes = [5, 27, 28, 29, 40, 56, 57, 100, 112, 113, 200, 224, 225, 300, 384, 385, 448, 449, 700, 1200, 1900, 23, 24, 25, 48, 49, 96, 97, 192, 193]
+    for n in sizes:
+        z0 = rng.uniform(-100, 100)
+        sig = rng.uniform(0.01, 0.1, n).astype(np.float32)
+        evs.append(dict(x=(sig * rng.normal(0, 1, n)).astype(np.float32), y=(sig * rng.normal(0, 1, n)).astype(np.float32),
+                        z=np.full(n, z0, np.float32), tx=np.clip(rng.normal(0, 0.25, n), -0.4, 0.4).astype(np.float32),
+                        ty=np.clip(rng.normal(0, 0.25, n), -0.4, 0.4).astype(np.float32), var_x=sig * sig, var_y=sig * sig,
+                        var_tx=np.full(n, 1e-6, np.float32), var_ty=np.full(n, 1e-6, np.float32)))
+    small = events.generate(events.config(0, 40))
+    so = small["offsets"]
+    for e in range(40):                                       # ordinary events in between, so that windows mix the sizes
+        evs.insert(rng.integers(0, len(evs) + 1), {k: small[k][so[e]:so[e + 1]] for k in events.FIELDS})
+    data = events.from_lists(evs)
+    p, po = (pv.multivertex_params(), oracle.mv_params()) if mv else (pv.default_params(), oracle.default_params())
+    got = pv.find(data, p, debug=True, n_hist_events=len(evs))
+    ref = oracle.find(data, po, debug=True, n_hist_events=len(evs), trace=True, n_threads=NTHREADS)
+    rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep)
+    big = np.diff(data["offsets"]) >= 5
+    nt = ref["debug"]["seed_ntrk"].max(axis=1)
+    assert set(np.diff(data["offsets"])[big]) >= set(sizes) and nt.max() > 1500      # the large seeds really are single seeds
+    plain = pv.find(data, p)
+    m = np.arange(p.max_vtx_per_event)[None, :] < plain["n_vtx"][:, None]
+    for k in plain:
+        a, b = (plain[k][m], got[k][m]) if k.startswith("vtx_") else (plain[k], got[k])
+        assert np.array_equal(a, b, equal_nan=True), k
