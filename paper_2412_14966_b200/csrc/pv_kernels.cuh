@@ -253,11 +253,14 @@ __device__ __forceinline__ int sweep(const int* __restrict__ H, int b0, const KP
   };
   int k = b0 + 1;
   // The state machine is written with selects: one step is ~30 straight-line instructions (the branchy form
-  // cost ~45 with the register moves at its merge points); only the rare split is a branch.
+  // cost ~45 with the register moves at its merge points); only the rare split is a branch.  The next bin is loaded
+  // one step ahead: the sweep is a serial chain, and the shared-memory latency would sit on it at every step.
+  int hn = H[min(k, P.nbins - 1)];
 #pragma unroll 1
   for (; k < P.nbins; ++k) {
-    h = H[k];
+    h = hn;
     if (!(h > P.T_bin)) break;
+    hn = H[min(k + 1, P.nbins - 1)];
     const bool c_up = h > mx, c_dn = mx - h > P.D, c_lt = h < mn, c_rise = h - mn > P.D;
     const bool to_min = look_max && !c_up && c_dn;          // a significant maximum lies behind: look for the minimum
     const bool new_min = to_min || (!look_max && c_lt);     // this bin is the running minimum
