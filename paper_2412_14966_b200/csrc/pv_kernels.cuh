@@ -1389,6 +1389,8 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
     sums_zero(S);
     float nass = 0.0f;                                       // multi-vertex flavour: tracks with final weight >= 1/2
     float* wp = A.wrec + cur.z + j;                          // explicit flavour: my tracks' places in wrec[]
+    char* wq = reinterpret_cast<char*>(wp);                  // walked slot by slot (one pointer add instead of re-deriving
+    const unsigned wstep = 4u << lg;                         // the address from the slot index: 8 -> 4 instructions per slot)
     const int wslots = st == FS_ITER ? myslots : 0;
 #pragma unroll FIT_UNROLL
     for (int s = 0; s < nslot_w; ++s) {
@@ -1400,7 +1402,8 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
           nass += (w >= 0.5f) ? 1.0f : 0.0f;
         }
       } else {
-        if (s < wslots) wp[s << lg] = w;                     // a dead track has w = 0 (unit weights: see below)
+        if (s < wslots) *reinterpret_cast<float*>(wq) = w;   // a dead track has w = 0 (unit weights: see below)
+        wq += wstep;
       }
     }
     if (P.unit_weights) {
