@@ -144,9 +144,6 @@ void make_kparams(const pv_params* p, int nbins, pvk::KParams* k) {
   k->conv_dchi2 = p->conv_dchi2; k->conv_dz = p->conv_dz; k->merge_ratio = p->merge_ratio;
   k->max_beam_dist2 = p->max_beam_dist * p->max_beam_dist;
   k->max_vtx = p->max_vtx_per_event;
-  const int r0 = ((nbins + 31) / 32) * 32 * 4;                // histogram padded to whole 32-bin words
-  k->region0_words = r0 / 4;
-  k->team_smem_bytes = r0 + pvk::SM_TAIL_BYTES;
   if (p->fill_mode == PV_FILL_TEMPLATE) tmpl_layout(p, k);
 }
 
@@ -201,16 +198,27 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
 
   pvk::KParams kp;
   make_kparams(params, nbins, &kp);
-  int teams = di->max_smem_optin / kp.team_smem_bytes;        // teams (events in flight) per CTA
-  if (teams > pvk::MAX_TEAMS) teams = pvk::MAX_TEAMS;
+  // seed_kernel: one warp per event, SEED_WARPS of them per CTA; what the warps' own state leaves of the shared memory
+  // is the CTA's pool of histogram blocks (a NULL word first)
+  int warps = pvk::SEED_WARPS;
 #ifdef PV_TUNING                                              // tuning builds only: fewer events in flight per CTA
-  if (const char* envw = getenv("PV_TEAMS_PER_CTA")) {
+  if (const char* envw = getenv("PV_WARPS_PER_CTA")) {
     const int w = atoi(envw);
-    if (w >= 1 && w < teams) teams = w;
+    if (w >= 1 && w < warps) warps = w;
   }
 #endif
-  if (teams < 1) return PV_E_PARAM;
-  const int smem = teams * kp.team_smem_bytes;
+  const int fixed = 128 + pvk::SM_HDR_BYTES + warps * pvk::WARP_SMEM;
+  int n_blocks = (di->max_smem_optin - fixed) / (pvk::BLK_WORDS * 128);
+  if (n_blocks > pvk::SM_HDR_BYTES * 8) n_blocks = pvk::SM_HDR_BYTES * 8;
+#ifdef PV_TUNING
+  if (const char* envb = getenv("PV_POOL_BLOCKS")) {
+    const int w = atoi(envb);
+    if (w >= 1 && w < n_blocks) n_blocks = w;
+  }
+#endif
+  if (n_blocks < pvk::MAX_WORDS / pvk::BLK_WORDS) return PV_E_PARAM;   // one event may need every word of the histogram
+  kp.n_blocks = n_blocks;
+  const int smem = fixed + n_blocks * pvk::BLK_WORDS * 128;
   const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
   const int spl = params->split_mode == PV_SPLIT_RECURSIVE ? 1 : 0;
   const int tfl = params->fill_mode == PV_FILL_TEMPLATE ? 1 : 0;
@@ -235,7 +243,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     else CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pvk::fit_kernel<0>, pvk::FIT_BLOCK, 0));
     di->fit_blocks_per_sm[mvf] = nb > 0 ? nb : 1;
   }
-  g_last_kernels = 0; g_last_grid = 0; g_last_block = teams * pvk::TEAM; g_last_smem = smem;
+  g_last_kernels = 0; g_last_grid = 0; g_last_block = warps * 32; g_last_smem = smem;
 
   pvk::KArgs ka;
   memset(&ka, 0, sizeof(ka));
@@ -264,9 +272,9 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
   CK(cudaMemsetAsync(workspace, 0, 64, stream));
-  // a1..a4: persistent, one CTA per SM, one team of two warps per event
+  // a1..a4: persistent, one CTA per SM, one warp per event
   int grid = di->sms;
-  const int need = (n_events + teams - 1) / teams;
+  const int need = (n_events + warps - 1) / warps;
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
   if (tfl) {                                                  // the table of template histograms, ~10^4 entries
@@ -275,7 +283,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   }
   {
     void* kargs[2] = {(void*)&kp, (void*)&ka};
-    CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(teams * pvk::TEAM), kargs, (size_t)smem, stream));
+    CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(warps * 32), kargs, (size_t)smem, stream));
   }
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));

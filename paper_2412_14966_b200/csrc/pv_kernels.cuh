@@ -36,11 +36,9 @@ namespace pvk {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
-constexpr int TEAM_WARPS = 2;       // warps per event in seed_kernel
-constexpr int TEAM = 32 * TEAM_WARPS;
-constexpr int MAX_TEAMS = 14;       // events in flight per CTA (named barriers 1..14; 14 histograms fill 227 KB)
-constexpr int CHUNK = 128;          // tracks per fill chunk
-constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
+constexpr int SEED_WARPS = 32;      // warps per CTA of seed_kernel = events in flight per SM (one warp per event)
+constexpr int CHUNK = 64;           // tracks per fill chunk
+constexpr int SLOTS = CHUNK / 32;   // tracks per lane and chunk
 #ifndef PV_FIT_UNROLL
 #define PV_FIT_UNROLL 4
 #endif
@@ -48,8 +46,10 @@ constexpr int SLOTS = CHUNK / TEAM; // register slots per thread
 #define PV_UNIT 6
 #endif
 constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
-constexpr int LIST_CAP = 256;       // fill units of one round (a chunk of median tracks needs ~200)
-constexpr int BINS_SM = 256;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
+constexpr int LIST_CAP = 192;       // fill units of one round (a chunk of median tracks needs ~100)
+constexpr int BINS_SM = 128;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
+constexpr int SEEDOF_SM = 128;      // ... whose seed index stays in shared memory between the count and the sort of a4
+constexpr int BLK_WORDS = 8;        // histogram words (of 32 bins) per block of the CTA's pool
 constexpr int FIT_UNROLL = PV_FIT_UNROLL;   // unroll of the track loop of one fit iteration
 #ifndef PV_FIT_KF
 #define PV_FIT_KF 14
@@ -67,27 +67,31 @@ constexpr int FIT_BLOCK = 64;       // threads per CTA of fit_kernel (warps are 
 constexpr int FIT_MIN_BLOCKS = 10;  // CTAs per SM: 10 x (21 KB + 1 KB reserved) fill the shared memory
 constexpr int FIT_MIN_BLOCKS_MV = 8;  // multi-vertex flavour: 24 KB of staged records per CTA
 constexpr int MAX_WORDS = PV_MAX_BINS / 32;   // 128 histogram words of 32 bins
-constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round of a warp (<= 16 per touched word)
+constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round (<= 16 per word)
 constexpr int TMPL_J = 8;           // template fill: positions of z_poca inside its central bin
 constexpr int TMPL_MAXK = 56;       // template fill: sigma classes (validate() bounds max_sigma_poca / dz)
 
-// Per-team shared memory of seed_kernel, in bytes after the histogram (region 0, nbins padded to whole words).
-// The 2 KB that stage the fill (track windows and the unit list) are dead once the histogram is complete; the peak
-// search and the association reuse them, so that 14 teams fit the 227 KB of an SM.
-constexpr int SM_TOUCHED = 0;                          // uint8 tb[128]        histogram words written by the fill
-constexpr int SM_MISC = SM_TOUCHED + MAX_WORDS;        // int misc[16]         warp totals, next event
-constexpr int SM_BINS = SM_MISC + 64;                  // int16 binsm[256]     central bins of the first 256 tracks
-constexpr int SM_STAGE = SM_BINS + BINS_SM * 2;        // fill:  float zp[128], inv[128]; int lonb[128]
-constexpr int SM_LIST = SM_STAGE + CHUNK * 12;         // fill:  uint16 list[256]
-constexpr int SM_PROTO = SM_STAGE;                     // peaks: uint16 protostart[2][PROTO_CAP]      (over the stage)
-constexpr int SM_CUR = SM_STAGE;                       // a4:    int cur[2][32] running record position (over protostart)
-constexpr int SM_SEED = SM_PROTO + TEAM_WARPS * PROTO_CAP * 2;   // peaks..a4: int sb[32], se[32], sp[32]; float zs[32]; int part[32]
-constexpr int SM_CNT = SM_SEED + 5 * MAXV * 4;         // a4:    int cnt[2][32] tracks per seed, per warp
-constexpr int SM_TWL = SM_CNT + TEAM_WARPS * 32 * 4;   // peaks: uint8 twl[128] list of touched words, ascending
-constexpr int SM_TAIL_BYTES = SM_LIST + LIST_CAP * 2;
-static_assert(SM_TWL + MAX_WORDS <= SM_TAIL_BYTES, "the overlays fit the fill stage and unit list");
-static_assert(TEAM_WARPS * 32 * 4 <= TEAM_WARPS * PROTO_CAP * 2, "cur[] fits over protostart[]");
-static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0 && SM_TAIL_BYTES % 16 == 0, "alignment of the vector accesses");
+// Shared memory of seed_kernel: [pool: 1 NULL word + n_blocks * BLK_WORDS words of 32 int32 bins][block bitmap]
+// [SEED_WARPS x WARP_SMEM].  Per warp, in bytes; the 1152 bytes that stage the fill (track windows and the unit list)
+// are dead once the histogram is complete: the peak search and the association reuse them.
+constexpr int SM_HDR_BYTES = 32;                           // unsigned bm[8]       free blocks of the pool, one bit each
+constexpr int SM_MAP = 0;                                  // uint16 map[128]      histogram word -> pool word (0 = NULL word)
+constexpr int SM_TB = SM_MAP + MAX_WORDS * 2;              // uint8 tb[128]        histogram words of the chunk's windows
+constexpr int SM_MISC = SM_TB + MAX_WORDS;                 // unsigned mapped[4]   words that have a pool word (+ spare)
+constexpr int SM_BLK = SM_MISC + 64;                       // uint16 blk[16]       blocks of this event (+ spare)
+constexpr int SM_BINS = SM_BLK + 64;                       // int16 binsm[128]     central bins of the first 128 tracks
+constexpr int SM_STAGE = SM_BINS + BINS_SM * 2;            // fill:  float zp[64], inv[64]; int lonb[64]
+constexpr int SM_LIST = SM_STAGE + CHUNK * 12;             // fill:  uint16 list[192]
+constexpr int SM_PROTO = SM_STAGE;                         // peaks: uint16 ps[PROTO_CAP]                 (over the stage)
+constexpr int SM_CNT = SM_PROTO;                           // a4:    int cnt[32] tracks per seed          (over ps)
+constexpr int SM_CUR = SM_CNT + 128;                       // a4:    int cur[32] running record position  (over ps)
+constexpr int SM_SEEDOF = SM_CUR + 128;                    // a4:    int8 seedsm[128] seed of the first 128 tracks (over ps)
+constexpr int SM_SEED = SM_PROTO + PROTO_CAP * 2;          // peaks..a4: int sb[32], se[32], sp[32]; float zs[32]; int part[32]
+constexpr int WARP_SMEM = SM_LIST + LIST_CAP * 2;
+static_assert(SM_SEED + 5 * MAXV * 4 <= WARP_SMEM, "the overlays fit the fill stage and unit list");
+static_assert(SM_SEEDOF + SEEDOF_SM <= SM_SEED, "cnt, cur and seedsm fit over the proto-cluster list");
+static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0 && WARP_SMEM % 16 == 0, "alignment of the vector accesses");
+static_assert(MAX_WORDS / BLK_WORDS <= 16 && MAX_WORDS <= 128, "blk[] and mapped[] sizes");
 
 struct KParams {
   float z_min, dz, inv_dz, z_split;
@@ -107,8 +111,7 @@ struct KParams {
   int split_mode;                // PV_SPLIT_*
   float chi2_window;             // multi-vertex flavour: list a track for a seed iff chi2 at the seed position < this
   float mv_e0;                   // exp(-chi2_max / 2), the constant of the denominator of Eq. 19
-  int region0_words;             // int32 words of the histogram region (multiple of 32)
-  int team_smem_bytes;
+  int n_blocks;                  // blocks of BLK_WORDS histogram words in the pool of a CTA of seed_kernel
   int tmpl_kmax;                 // template fill (R-17): class of the largest sigma cut = last class
   int tmpl_off[TMPL_MAXK];       // first table entry of class k; its TMPL_J templates of 2 W_k + 1 bins follow each other
   short tmpl_w[TMPL_MAXK];       // W_k = ceil(3 sigma_k / dz)
@@ -178,6 +181,12 @@ __device__ __forceinline__ int cdf_bits(float s) {
   return __float_as_int(__fadd_rn(c, 8.0f));
 }
 
+// integer add to a shared-memory bin (byte address in the shared window) unless the addend is zero, as ONE predicated
+// instruction: `if (d != 0) atomicAdd(...)` compiles to a branch with a convergence barrier around every add
+__device__ __forceinline__ void red_add_nz(unsigned saddr, int d) {
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %1, 0;\n\t@q red.shared.add.s32 [%0], %1;\n\t}" ::"r"(saddr), "r"(d) : "memory");
+}
+
 __device__ __forceinline__ int bin_region(int b, const KParams& P) {
   const float centre = __fmaf_rn(__fadd_rn((float)b, 0.5f), P.dz, P.z_min);
   return centre < P.z_split ? 1 : 0;
@@ -232,7 +241,8 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 // (Single call site, inside a loop, so that the code exists once.)
 struct Cl { int b, e, p; };
 
-__device__ __forceinline__ int sweep(const int* __restrict__ H, int b0, const KParams& P, int wbase,
+template <class HT>
+__device__ __forceinline__ int sweep(const HT& H, int b0, const KParams& P, int wbase,
                                      int* sb, int* se, int* sp, Cl& c0, Cl& c1) {
   int start = b0;
   int h = H[b0];
@@ -304,7 +314,8 @@ __device__ __forceinline__ int sweep(const int* __restrict__ H, int b0, const KP
 // peak bins of the two parts.
 struct Part { int sum, amax, amaxp; };
 
-__device__ __forceinline__ Part part_of(const int* __restrict__ H, int s, int e) {
+template <class HT>
+__device__ __forceinline__ Part part_of(const HT& H, int s, int e) {
   Part r = {0, -1, s};
 #pragma unroll 1
   for (int k = s; k < e; ++k) {
@@ -315,7 +326,8 @@ __device__ __forceinline__ Part part_of(const int* __restrict__ H, int s, int e)
   return r;
 }
 
-__device__ int split_x86(const int* __restrict__ H, int b0, const KParams& P, int wbase,
+template <class HT>
+__device__ int split_x86(const HT& H, int b0, const KParams& P, int wbase,
                          int* sb, int* se, int* sp, Cl& c0, Cl& c1) {
   int b1 = b0 + 1;
 #pragma unroll 1
@@ -491,34 +503,64 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
   return T;
 }
 
-// ---- seed_kernel: a1..a4 for one event, one TEAM of two warps ---------------------------------------------------
-// The CTA holds up to MAX_TEAMS teams, each with its own histogram in shared memory and its own named barrier.
-__device__ __forceinline__ void team_sync(int bar) {
-  asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(TEAM) : "memory");
+// ---- seed_kernel: a1..a4, ONE WARP per event ---------------------------------------------------------------------
+// Persistent grid, one CTA of SEED_WARPS warps per SM, every warp works through whole events on its own (events are
+// handed out by an atomic counter): no CTA or team barrier anywhere, __syncwarp only.
+// Histograms are SPARSE: an event touches ~13 of its 107 words of 32 bins (configs[1]; ~33 at high pile-up), so a dense
+// int32 histogram per event (13.6 KB) would hold the SM to 14 events in flight.  Instead the CTA owns a pool of blocks
+// of BLK_WORDS words; a warp maps the words its tracks touch to pool words as it meets them (map[], one uint16 per
+// histogram word; pool word 0 is the NULL word, always zero, where every untouched word points) and takes blocks from
+// a shared bitmap as it needs them.  When the pool runs dry a warp that holds blocks gives them back and starts its
+// event again (no hold-and-wait, hence no deadlock); a warp that holds none simply waits.
+struct Hist {
+  const int* pool;
+  const uint16_t* map;
+  __device__ __forceinline__ int operator[](int b) const { return pool[((int)map[b >> 5] << 5) + (b & 31)]; }
+};
+
+// one free block of the pool (warp-collective; the same value in every lane), -1 when there is none right now
+__device__ __forceinline__ int blk_try_alloc(unsigned* bm, const int nbw, const int lane) {
+  unsigned m = lane < nbw ? reinterpret_cast<volatile unsigned*>(bm)[lane] : 0u;
+  for (;;) {
+    const unsigned has = __ballot_sync(FULL, m != 0u);
+    if (!has) return -1;
+    const int src = __ffs(has) - 1;
+    int got = -1;
+    if (lane == src) {
+      const int b = __ffs(m) - 1;
+      const unsigned bit = 1u << b;
+      const unsigned old = atomicAnd(&bm[lane], ~bit);
+      if (old & bit) got = lane * 32 + b;
+      m = old & ~bit;
+    }
+    got = __shfl_sync(FULL, got, src);
+    if (got >= 0) return got;
+  }
 }
 
 template <bool DBG, int FLAV, int SPLIT, int FILL>
-__device__ void seed_event(const int e, const int nxt, const KParams& P, const KArgs& A, unsigned char* wsm, const int tt,
-                           const int bar) {
-  const int lane = tt & 31, tw = tt >> 5;
-  int* H = reinterpret_cast<int*>(wsm);
-  unsigned char* tail = wsm + (size_t)P.region0_words * 4;
-  uint8_t* tb = reinterpret_cast<uint8_t*>(tail + SM_TOUCHED);
-  uint8_t* twl = reinterpret_cast<uint8_t*>(tail + SM_TWL);
-  int* cnt = reinterpret_cast<int*>(tail + SM_CNT);          // cnt[warp][seed]
-  int* cur = reinterpret_cast<int*>(tail + SM_CUR) + tw * 32;   // my warp's running record positions
-  int* sb = reinterpret_cast<int*>(tail + SM_SEED);
+__device__ void seed_event(const int e, const int nxt, const KParams& P, const KArgs& A, int* pool, unsigned* bm,
+                           unsigned char* wsm, const int lane) {
+  uint16_t* map = reinterpret_cast<uint16_t*>(wsm + SM_MAP);
+  uint8_t* tb = reinterpret_cast<uint8_t*>(wsm + SM_TB);
+  unsigned* mapped = reinterpret_cast<unsigned*>(wsm + SM_MISC);   // mapped[c]: words 32 c .. 32 c + 31 that have a pool word
+  uint16_t* blk = reinterpret_cast<uint16_t*>(wsm + SM_BLK);
+  int16_t* binsm = reinterpret_cast<int16_t*>(wsm + SM_BINS);
+  float* st_zp = reinterpret_cast<float*>(wsm + SM_STAGE);
+  float* st_inv = st_zp + CHUNK;
+  int* st_lonb = reinterpret_cast<int*>(st_inv + CHUNK);
+  uint16_t* list = reinterpret_cast<uint16_t*>(wsm + SM_LIST);
+  // overlays: stage and list are dead after the fill, the proto-cluster list after the sweeps
+  uint16_t* ps = reinterpret_cast<uint16_t*>(wsm + SM_PROTO);
+  int* cnt = reinterpret_cast<int*>(wsm + SM_CNT);
+  int* cur = reinterpret_cast<int*>(wsm + SM_CUR);
+  int8_t* seedsm = reinterpret_cast<int8_t*>(wsm + SM_SEEDOF);
+  int* sb = reinterpret_cast<int*>(wsm + SM_SEED);
   int* se = sb + MAXV;
   int* sp = se + MAXV;
   float* zs = reinterpret_cast<float*>(sp + MAXV);
   int* part = reinterpret_cast<int*>(zs + MAXV);
-  int* misc = reinterpret_cast<int*>(tail + SM_MISC);
-  float* st_zp = reinterpret_cast<float*>(tail + SM_STAGE);
-  float* st_inv = st_zp + CHUNK;
-  int* st_lonb = reinterpret_cast<int*>(st_inv + CHUNK);
-  uint16_t* list = reinterpret_cast<uint16_t*>(tail + SM_LIST);
-  // overlays of the peak search: stage and list are dead after the fill
-  int16_t* binsm = reinterpret_cast<int16_t*>(tail + SM_BINS);
+  const Hist H{pool, map};
 
   const int t0 = __ldg(A.offsets + e);
   const int n = __ldg(A.offsets + e + 1) - t0;
@@ -530,238 +572,281 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   const bool no_room = FLAV == PV_FLAVOUR_EXPLICIT && (unsigned)t0 + (unsigned)n > A.trk_cap;
   if (n > MAX_TRK || no_room) {
 #pragma unroll 1
-    for (int i = tt; i < n; i += TEAM) {
+    for (int i = lane; i < n; i += 32) {
       A.trk_vertex[t0 + i] = -1;
       if (FLAV == PV_FLAVOUR_MULTIVERTEX) A.best[t0 + i] = 0ull;
     }
-    if (DBG && A.dbg.trk_seed) for (int i = tt; i < n; i += TEAM) A.dbg.trk_seed[t0 + i] = -1;
-    if (tt == 0) {
+    if (DBG && A.dbg.trk_seed) for (int i = lane; i < n; i += 32) A.dbg.trk_seed[t0 + i] = -1;
+    if (lane == 0) {
       A.n_vtx[e] = 0;
       A.event_status[e] = n > MAX_TRK ? PV_EVT_TOO_MANY_TRACKS : PV_EVT_RECORD_OVERFLOW;
       if (DBG && A.dbg.n_seeds) A.dbg.n_seeds[e] = 0;
       if (DBG && A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = 0;
     }
-    team_sync(bar);                                          // every path through an event holds a team barrier (seed_kernel)
     return;
   }
 
+  const int nwc = (P.nwords + 31) >> 5;                    // chunks of 32 histogram words
+  const int nbw = (P.n_blocks + 31) >> 5;                  // words of the block bitmap
+  int nslots = 0, nblk = 0;                                // pool words / blocks of this event (warp-uniform)
+  // zero my pool words, unmap them and give the blocks back: leaves the warp's histogram state as it is between events
+  auto release = [&]() {
+#pragma unroll 1
+    for (int c = 0; c < nwc; ++c) {
+      const unsigned mc = mapped[c];
+      unsigned m = mc;
+#pragma unroll 1
+      while (m) {
+        const int w = 32 * c + __ffs(m) - 1;
+        m &= m - 1u;
+        pool[((int)map[w] << 5) + lane] = 0;
+      }
+      __syncwarp();
+      if ((mc >> lane) & 1u) map[32 * c + lane] = 0;
+      if (lane == 0) mapped[c] = 0u;
+    }
+    __threadfence_block();                                 // the zeros are in place before another warp can take a block
+    __syncwarp();
+    if (lane < nblk) { const int b = blk[lane]; atomicOr(&bm[b >> 5], 1u << (b & 31)); }
+    nslots = 0; nblk = 0;
+    __syncwarp();
+  };
+
   // ================= a1 + a2: projection (Eq. 1, Eq. 3) and histogram fill ===================
-  // Chunks of CHUNK tracks, SLOTS per thread.  The window of a histogrammed track is cut into units of UNIT
-  // bins; the units of the chunk form one flat list, and a fill pass gives every thread one unit: UNIT + 1
+  // Chunks of CHUNK tracks, SLOTS per lane.  The window of a histogrammed track is cut into units of UNIT
+  // bins; the units of the chunk form one flat list, and a fill pass gives every lane one unit: UNIT + 1
   // independent CDF edges (instruction-level parallelism instead of one dependent Horner chain) and UNIT
   // predicated integer adds.  The adds are integers, so the order changes nothing.
-  RawTrk held[SLOTS];                                      // the first CHUNK tracks stay in registers until a4 has
-#pragma unroll                                             // sorted them by seed (no second trip to memory)
-  for (int s = 0; s < SLOTS; ++s) held[s] = RawTrk{0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+  const unsigned pool_s = (unsigned)__cvta_generic_to_shared(pool);
 #pragma unroll 1
-  for (int c0 = 0; c0 < n; c0 += CHUNK) {
-    float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
+  for (bool filled = false; !filled;) {
+    filled = true;
+#pragma unroll 1
+    for (int c0 = 0; c0 < n; c0 += CHUNK) {
+      float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
 #pragma unroll
-    for (int s = 0; s < SLOTS; ++s) {                      // all loads first
-      const int i = c0 + s * TEAM + tt;
-      const int t = t0 + (i < n ? i : n - 1);
-      lx[s] = __ldg(A.x + t); ly[s] = __ldg(A.y + t); lz[s] = __ldg(A.z + t);
-      ltx[s] = __ldg(A.tx + t); lty[s] = __ldg(A.ty + t); lvx[s] = __ldg(A.var_x + t);
-      if (c0 == 0) {
-        held[s].vy = __ldg(A.var_y + t); held[s].vtx = __ldg(A.var_tx + t); held[s].vty = __ldg(A.var_ty + t);
+      for (int s = 0; s < SLOTS; ++s) {                    // all loads first
+        const int t = t0 + min(c0 + s * 32 + lane, n - 1);
+        lx[s] = __ldg(A.x + t); ly[s] = __ldg(A.y + t); lz[s] = __ldg(A.z + t);
+        ltx[s] = __ldg(A.tx + t); lty[s] = __ldg(A.ty + t); lvx[s] = __ldg(A.var_x + t);
       }
-    }
-    if (c0 == 0) {
+      int nun[SLOTS];                                      // fill units of my tracks
+      int myunits = 0;
 #pragma unroll
       for (int s = 0; s < SLOTS; ++s) {
-        held[s].x = lx[s]; held[s].y = ly[s]; held[s].z = lz[s];
-        held[s].tx = ltx[s]; held[s].ty = lty[s]; held[s].vx = lvx[s];
-      }
-    }
-    int nun[SLOTS];                                        // fill units of my tracks
-    int myunits = 0;
-#pragma unroll
-    for (int s = 0; s < SLOTS; ++s) {
-      const int i = c0 + s * TEAM + tt;
-      nun[s] = 0;
-      if (i < n) {
-        const Proj r = project(lx[s], ly[s], lz[s], ltx[s], lty[s], lvx[s], P);
-        if (i < BINS_SM) binsm[i] = (int16_t)r.bin; else A.trk_vertex[t0 + i] = r.bin;   // large events: HBM scratch, read back in a4
-        if (DBG) {
-          if (A.dbg.z_poca) A.dbg.z_poca[t0 + i] = r.zp;
-          if (A.dbg.sigma_poca) A.dbg.sigma_poca[t0 + i] = r.sg;
-          if (A.dbg.trk_bin) A.dbg.trk_bin[t0 + i] = r.bin;
-        }
-        if (r.fill && FILL == PV_FILL_TEMPLATE) {
-          // template fill (R-17): class of sigma_poca, eighth of the bin z_poca falls in; the units of the
-          // window then copy table entries instead of evaluating CDF edges
-          const int k = min(tmpl_class_raw(r.sg, P.inv_dz), P.tmpl_kmax);
-          const int j = min((int)__fmul_rn(r.frac, (float)TMPL_J), TMPL_J - 1);
-          const int W = P.tmpl_w[k];
-          const int lo = max(r.bin - W, 0), hi = min(r.bin + W + 1, P.nbins);
-          const int nb = hi - lo;
-          nun[s] = (nb + UNIT - 1) / UNIT;
-          st_zp[s * TEAM + tt] = __int_as_float(P.tmpl_off[k] + j * (2 * W + 1) + (lo - (r.bin - W)));
-          st_lonb[s * TEAM + tt] = lo | (nb << 12);
-        } else if (r.fill) {
-          // window: a superset of the +-3 sigma support; edges outside it give exactly 0 or 2^20
-          const float w3 = 3.0f * r.sg;
-          const float fa = floorf((r.zp - w3 - P.z_min) * P.inv_dz - P.win_eps);
-          const float fb2 = floorf((r.zp + w3 - P.z_min) * P.inv_dz + P.win_eps) + 1.0f;
-          const int lo = (int)fmaxf(fa, 0.0f);
-          const int hi = (int)fminf(fb2, (float)P.nbins);
-          const int nb = hi - lo;
+        const int i = c0 + s * 32 + lane;
+        nun[s] = 0;
+        if (i < n) {
+          const Proj r = project(lx[s], ly[s], lz[s], ltx[s], lty[s], lvx[s], P);
+          if (i < BINS_SM) binsm[i] = (int16_t)r.bin; else A.trk_vertex[t0 + i] = r.bin;   // large events: HBM scratch, read back in a4
+          if (DBG) {
+            if (A.dbg.z_poca) A.dbg.z_poca[t0 + i] = r.zp;
+            if (A.dbg.sigma_poca) A.dbg.sigma_poca[t0 + i] = r.sg;
+            if (A.dbg.trk_bin) A.dbg.trk_bin[t0 + i] = r.bin;
+          }
+          int lo = 0, nb = 0;
+          if (r.fill && FILL == PV_FILL_TEMPLATE) {
+            // template fill (R-17): class of sigma_poca, eighth of the bin z_poca falls in; the units of the
+            // window then copy table entries instead of evaluating CDF edges
+            const int k = min(tmpl_class_raw(r.sg, P.inv_dz), P.tmpl_kmax);
+            const int j = min((int)__fmul_rn(r.frac, (float)TMPL_J), TMPL_J - 1);
+            const int W = P.tmpl_w[k];
+            lo = max(r.bin - W, 0);
+            nb = min(r.bin + W + 1, P.nbins) - lo;
+            st_zp[s * 32 + lane] = __int_as_float(P.tmpl_off[k] + j * (2 * W + 1) + (lo - (r.bin - W)));
+          } else if (r.fill) {
+            // window: a superset of the +-3 sigma support; edges outside it give exactly 0 or 2^20
+            const float w3 = 3.0f * r.sg;
+            const float fa = floorf((r.zp - w3 - P.z_min) * P.inv_dz - P.win_eps);
+            const float fb2 = floorf((r.zp + w3 - P.z_min) * P.inv_dz + P.win_eps) + 1.0f;
+            lo = (int)fmaxf(fa, 0.0f);
+            nb = (int)fminf(fb2, (float)P.nbins) - lo;
+            st_zp[s * 32 + lane] = r.zp; st_inv[s * 32 + lane] = r.inv;
+          }
           if (nb > 0) {
             nun[s] = (nb + UNIT - 1) / UNIT;
-            st_zp[s * TEAM + tt] = r.zp; st_inv[s * TEAM + tt] = r.inv; st_lonb[s * TEAM + tt] = lo | (nb << 12);
+            st_lonb[s * 32 + lane] = lo | (nb << 12);
+#pragma unroll 1
+            for (int w = lo >> 5; w <= (lo + nb - 1) >> 5; ++w) tb[w] = 1;   // histogram words of the window
           }
         }
+        myunits += nun[s];
       }
-      myunits += nun[s];
-    }
-    const int incl = warp_incl_scan(myunits, lane);
-    if (lane == 31) misc[tw] = incl;
-    team_sync(bar);
-    const int total = misc[0] + misc[1];
-    const int first = incl - myunits + (tw ? misc[0] : 0);  // list position of my first unit
+      __syncwarp();
+      // ---- words met for the first time get a pool word (and the event another block when it needs one)
 #pragma unroll 1
-    for (int R = 0; R < total; R += LIST_CAP) {            // one round unless the chunk holds very wide tracks
-      if (R > 0) team_sync(bar);
-      {
-        int g = first - R;
+      for (int c = 0; c < nwc; ++c) {
+        const int f = tb[32 * c + lane];
+        const unsigned m = __ballot_sync(FULL, f != 0);
+        if (m == 0u) continue;
+        if (f) tb[32 * c + lane] = 0;
+        const unsigned newm = m & ~mapped[c];
+        if (newm == 0u) continue;
+        const int cntn = __popc(newm);
+        const int need = (nslots + cntn + BLK_WORDS - 1) / BLK_WORDS;
+        int spins = 0;
+#pragma unroll 1
+        while (nblk < need) {
+          const int b = blk_try_alloc(bm, nbw, lane);
+          if (b >= 0) {
+            if (lane == 0) blk[nblk] = (uint16_t)b;
+            ++nblk;
+            continue;
+          }
+          if (nblk > 0 && ++spins > 32) break;             // pool dry while I hold blocks: give them back, start again
+          __nanosleep(200);
+        }
+        if (nblk < need) { filled = false; break; }
+        __threadfence_block();
+        __syncwarp();
+        if ((newm >> lane) & 1u) {
+          const int slot = nslots + __popc(newm & lanemask_lt());
+          map[32 * c + lane] = (uint16_t)(1 + (int)blk[slot / BLK_WORDS] * BLK_WORDS + (slot % BLK_WORDS));
+        }
+        nslots += cntn;
+        __syncwarp();
+        if (lane == 0) mapped[c] |= newm;
+        __syncwarp();
+      }
+      if (!filled) break;
+      const int incl = warp_incl_scan(myunits, lane);
+      const int total = __shfl_sync(FULL, incl, 31);
+      const int first = incl - myunits;                    // list position of my first unit
+#pragma unroll 1
+      for (int R = 0; R < total; R += LIST_CAP) {          // one round unless the chunk holds very wide tracks
+        __syncwarp();
+        {
+          int g = first - R;
 #pragma unroll
-        for (int s = 0; s < SLOTS; ++s) {
-          const int tk = s * TEAM + tt;
+          for (int s = 0; s < SLOTS; ++s) {
+            const int tk = s * 32 + lane;
 #pragma unroll 1
-          for (int u = 0; u < nun[s]; ++u, ++g)
-            if ((unsigned)g < (unsigned)LIST_CAP) list[g] = (uint16_t)(tk | (u << 7));
+            for (int u = 0; u < nun[s]; ++u, ++g)
+              if ((unsigned)g < (unsigned)LIST_CAP) list[g] = (uint16_t)(tk | (u << 7));
+          }
         }
-      }
-      team_sync(bar);
-      const int nl = min(total - R, LIST_CAP);
+        __syncwarp();
+        const int nl = min(total - R, LIST_CAP);
 #pragma unroll 1
-      for (int p0 = tw * 32; p0 < nl; p0 += TEAM) {
-        const int idx = p0 + lane;
-        const bool act = idx < nl;
-        const int ent = list[act ? idx : nl - 1];
-        const int tk = ent & 127, u = ent >> 7;
-        const float zp = st_zp[tk], inv = st_inv[tk];
-        const int lonb = st_lonb[tk];
-        const int b0 = (lonb & 0xfff) + u * UNIT;
-        const int rem = act ? (lonb >> 12) - u * UNIT : 0;   // bins of this unit: min(rem, UNIT)
-        if (act) {                                         // histogram words this unit writes
-          tb[b0 >> 5] = 1;
-          tb[(b0 + min(rem, UNIT) - 1) >> 5] = 1;
-        }
-        if constexpr (FILL == PV_FILL_TEMPLATE) {
-          const int32_t* tp = A.tmpl + __float_as_int(zp) + u * UNIT;
+        for (int p0 = 0; p0 < nl; p0 += 32) {
+          const int idx = p0 + lane;
+          const bool act = idx < nl;
+          const int ent = list[act ? idx : nl - 1];
+          const int tk = ent & 127, u = ent >> 7;
+          const float zp = st_zp[tk], inv = st_inv[tk];
+          const int lonb = st_lonb[tk];
+          const int b0 = (lonb & 0xfff) + u * UNIT;
+          const int rem = act ? (lonb >> 12) - u * UNIT : 0; // bins of this unit: min(rem, UNIT)
+          // the unit's bins lie in one or two histogram words: their pool addresses (shared-memory byte addresses)
+          const int nfirst = 32 - (b0 & 31);                 // bins before the word boundary
+          const unsigned a0 = pool_s + ((unsigned)map[b0 >> 5] << 7) + ((unsigned)(b0 & 31) << 2);
+          const unsigned a1 = pool_s + ((unsigned)map[min((b0 >> 5) + 1, MAX_WORDS - 1)] << 7);
           int d[UNIT];
+          if constexpr (FILL == PV_FILL_TEMPLATE) {
+            const int32_t* tp = A.tmpl + __float_as_int(zp) + u * UNIT;
 #pragma unroll
-          for (int j = 0; j < UNIT; ++j) d[j] = j < rem ? __ldg(tp + j) : 0;
+            for (int j = 0; j < UNIT; ++j) d[j] = j < rem ? __ldg(tp + j) : 0;
+          } else {
+            const float kf = (float)b0;
+            int r[UNIT + 1];
 #pragma unroll
-          for (int j = 0; j < UNIT; ++j)
-            if (d[j] != 0) atomicAdd(&H[b0 + j], d[j]);
-        } else {
-          const float kf = (float)b0;
-          int r[UNIT + 1];
+            for (int j = 0; j <= UNIT; ++j) r[j] = edge_r(kf + (float)j, zp, inv, P);
 #pragma unroll
-          for (int j = 0; j <= UNIT; ++j) r[j] = edge_r(kf + (float)j, zp, inv, P);
-#pragma unroll
-          for (int j = 0; j < UNIT; ++j) {
-            const int d = r[j + 1] - r[j];
-            if (j < rem && d != 0) atomicAdd(&H[b0 + j], d);
+            for (int j = 0; j < UNIT; ++j) d[j] = j < rem ? r[j + 1] - r[j] : 0;
           }
+#pragma unroll
+          for (int j = 0; j < UNIT; ++j) red_add_nz(j < nfirst ? a0 + 4u * j : a1 + 4u * (j - nfirst), d[j]);
         }
       }
+      __syncwarp();                                        // the next chunk overwrites the stage
     }
-    team_sync(bar);
+    if (!filled) {                                         // the pool ran dry: back off and start the event again
+      reinterpret_cast<unsigned*>(tb)[lane] = 0u;
+      __syncwarp();
+      release();
+      __nanosleep(2000);
+    }
   }
+  __syncwarp();
 
   if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
-    for (int b = tt; b < P.nbins; b += TEAM) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
+    for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
 
   // ================= a3: peak search and seed position (Eq. 4-5) ==============================
-  // List of the touched histogram words, ascending; only these can hold bins above the threshold.
-  int ntw;
+  // The mapped words, ascending, are the only ones that can hold bins above the threshold: one ballot per word finds
+  // the first bin of every run above threshold (proto-cluster), then one lane per proto-cluster runs the z-ordered
+  // hysteresis sweep (select-based state machine: the serial length is the longest proto-cluster).
+  int n_raw = 0;
   {
-    const unsigned f4 = reinterpret_cast<const unsigned*>(tb)[lane];   // flags of words 4 lane .. 4 lane + 3
-    const int c = (f4 & 1u) + ((f4 >> 8) & 1u) + ((f4 >> 16) & 1u) + ((f4 >> 24) & 1u);
-    const int inc = warp_incl_scan(c, lane);
-    ntw = __shfl_sync(FULL, inc, 31);
-    if (tw == 0) {
-      int o = inc - c;
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if ((f4 >> (8 * q)) & 1u) twl[o++] = (uint8_t)(4 * lane + q);
-    }
-  }
-  team_sync(bar);
-  if (tw == 1) reinterpret_cast<unsigned*>(tb)[lane] = 0;  // clean for the next event (both warps have read it)
-
-  // Both warps look for proto-cluster starts, each in its half of the touched words; then warp 0 alone runs the
-  // z-ordered sweeps with one lane per proto-cluster of the whole event (the number of serial sweep steps is the
-  // longest proto-cluster of the event, once) and computes the seed positions.
-  uint16_t* ps0 = reinterpret_cast<uint16_t*>(tail + SM_PROTO);
-  uint16_t* ps1 = ps0 + PROTO_CAP;
-  // proto-cluster starts of the words [i, iend) -> ps[0 .. return value); stops early (i < iend) when ps is full
-  auto detect = [&](int& i, const int iend, uint16_t* ps) -> int {
+    int dc = 0;
+    unsigned dm = mapped[0];
     int prev_w = -2;
-    unsigned prev_m = 0;
-    if (i > 0 && i < iend) {                               // does a run continue from the word before this range?
-      const int pw = twl[i - 1];
-      if (pw == (int)twl[i] - 1) { prev_w = pw; prev_m = (H[pw * 32 + 31] > P.T_bin) ? 0x80000000u : 0u; }
-    }
-    int n_proto = 0;
+    unsigned prev_top = 0u;
 #pragma unroll 1
-    for (; i < iend && n_proto + 16 <= PROTO_CAP; ++i) {   // a word of 32 bins starts at most 16 runs
-      const int w = twl[i];
-      const int b = w * 32 + lane;                         // bins beyond nbins are padding and stay 0
-      const unsigned m = __ballot_sync(FULL, H[b] > P.T_bin);
-      const unsigned carry = (prev_w == w - 1) ? (prev_m >> 31) : 0u;
-      const unsigned starts = m & ~((m << 1) | carry);     // first bin of each run of bins above threshold
-      if ((starts >> lane) & 1u) ps[n_proto + __popc(starts & lanemask_lt())] = (uint16_t)b;
-      n_proto += __popc(starts);
-      prev_w = w; prev_m = m;
-    }
-    return n_proto;
-  };
-  int n_raw = 0;                                           // valid in warp 0 until published through misc[4]
-  // sweeps of the n0 + n1 proto-clusters listed in ps0[0..n0) and ps1[0..n1), appended to (sb, se, sp)
-  auto sweep_all = [&](const int n0, const int n1) {
+    do {
+      int np = 0;
 #pragma unroll 1
-    for (int p0 = 0; p0 < n0 + n1; p0 += 32) {             // one lane per proto-cluster
-      const int p = p0 + lane;
-      const bool act = p < n0 + n1;
-      const int b0 = act ? (int)(p < n0 ? ps0[p] : ps1[p - n0]) : 0;
-      Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
-      int c = 0, base = 0;
-#pragma unroll 1
-      for (int rep = 0; rep < 2; ++rep) {                  // rep 1 (rare): proto-clusters with three or more seeds
-        const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
-        if (!__any_sync(FULL, run)) break;
-        if (run) {
-          const int cc = SPLIT ? split_x86(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1)
-                               : sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
-          if (rep == 0) c = cc;
+      while (dc < nwc && np + 16 <= PROTO_CAP) {           // a word of 32 bins starts at most 16 runs
+        if (dm == 0u) {
+          ++dc;
+          dm = dc < nwc ? mapped[dc] : 0u;
+          continue;
         }
-        if (rep == 0) {
-          const int inc = warp_incl_scan(c, lane);
-          base = n_raw + inc - c;
-          if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
-          if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
-          n_raw += __shfl_sync(FULL, inc, 31);
+        const int w = 32 * dc + __ffs(dm) - 1;
+        dm &= dm - 1u;
+        const int h = pool[((int)map[w] << 5) + lane];     // bins beyond nbins are padding and stay 0
+        const unsigned m = __ballot_sync(FULL, h > P.T_bin);
+        const unsigned carry = (prev_w == w - 1) ? prev_top : 0u;
+        const unsigned starts = m & ~((m << 1) | carry);   // first bin of each run of bins above threshold
+        if ((starts >> lane) & 1u) ps[np + __popc(starts & lanemask_lt())] = (uint16_t)(32 * w + lane);
+        np += __popc(starts);
+        prev_w = w; prev_top = m >> 31;
+      }
+      __syncwarp();
+#pragma unroll 1
+      for (int p0 = 0; p0 < np; p0 += 32) {                // one lane per proto-cluster
+        const int p = p0 + lane;
+        const bool act = p < np;
+        const int b0 = act ? (int)ps[p] : 0;
+        Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
+        int c = 0, base = 0;
+#pragma unroll 1
+        for (int rep = 0; rep < 2; ++rep) {                // rep 1 (rare): proto-clusters with three or more seeds
+          const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
+          if (!__any_sync(FULL, run)) break;
+          if (run) {
+            const int cc = SPLIT ? split_x86(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1)
+                                 : sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+            if (rep == 0) c = cc;
+          }
+          if (rep == 0) {
+            const int inc = warp_incl_scan(c, lane);
+            base = n_raw + inc - c;
+            if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
+            if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
+            n_raw += __shfl_sync(FULL, inc, 31);
+          }
         }
       }
-    }
-  };
-  {
-    const int half = (ntw + 1) >> 1;
-    int i = tw ? half : 0;
-    const int iend = tw ? ntw : half;
-    const int np_ = detect(i, iend, tw ? ps1 : ps0);
-    if (lane == 0) {
-      misc[2 + tw] = np_;
-      if (i < iend) misc[6] = 1;                           // list full (never with physical histograms): slow path
-    }
+      __syncwarp();
+    } while (dc < nwc);
   }
-  if (tw == 1) {
-    // warp 1 now waits for warp 0's sweeps: it uses the time to pull the first chunk of the team's NEXT event
-    // (its lane 0 holds the event index) into L2
+  int ns = n_raw;
+  if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
+  if (lane < ns) {                                         // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
+    const int i = sp[lane];
+    const long long Nm = i > 0 ? H[i - 1] : 0;
+    const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
+    const long long N0 = H[i];
+    const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
+    const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
+    const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
+    zs[lane] = __fmaf_rn(delta, P.dz, zi);
+  }
+  __syncwarp();
+  release();                                               // the histogram is dead from here on
+  {
+    // pull the first chunk of my NEXT event (lane 0 holds its index) into L2 while this one is associated
     const int ne = __shfl_sync(FULL, nxt, 0);
     if (ne < A.n_events) {
       const int pt0 = __ldg(A.offsets + ne);
@@ -774,60 +859,27 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       }
     }
   }
-  team_sync(bar);
-  if (tw == 0) {
-    // normally one call over the two lists; after a list overflow (misc[6]), rounds of <= PROTO_CAP proto-clusters
-    // over all words.  One call site, so that the sweep is inlined once.
-    const bool rounds = misc[6] != 0;
-    int i = 0, n0 = misc[2], n1 = misc[3];
-#pragma unroll 1
-    do {
-      if (rounds) {
-        __syncwarp();
-        n0 = detect(i, ntw, ps0); n1 = 0;
-        __syncwarp();
-      }
-      sweep_all(n0, n1);
-    } while (rounds && i < ntw);
-    __syncwarp();
-    const int nsw = min(n_raw, P.max_vtx);
-    if (lane < nsw) {                                      // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
-      const int i = sp[lane];
-      const long long Nm = i > 0 ? H[i - 1] : 0;
-      const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
-      const long long N0 = H[i];
-      const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
-      const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
-      const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
-      zs[lane] = __fmaf_rn(delta, P.dz, zi);
-    }
-    if (lane == 0) { misc[4] = n_raw; misc[6] = 0; }
-  }
-  team_sync(bar);
-  n_raw = misc[4];
-  int ns = n_raw;
-  if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
-  // the histogram is dead from here on: clear what this event touched for the next one
-#pragma unroll 1
-  for (int i = tw; i < ntw; i += TEAM_WARPS) H[(int)twl[i] * 32 + lane] = 0;
+
+  auto load_raw = [&](const int i) {
+    const int g = t0 + min(i, n - 1);
+    RawTrk Q;
+    Q.x = __ldg(A.x + g); Q.y = __ldg(A.y + g); Q.z = __ldg(A.z + g); Q.tx = __ldg(A.tx + g); Q.ty = __ldg(A.ty + g);
+    Q.vx = __ldg(A.var_x + g); Q.vy = __ldg(A.var_y + g); Q.vtx = __ldg(A.var_tx + g); Q.vty = __ldg(A.var_ty + g);
+    return Q;
+  };
+  auto cross_of = [&](const int i, float& cx, float& cy) {   // V_xtx, V_yty of track i (0 = diagonal covariance)
+    const int g = t0 + min(i, n - 1);
+    cx = A.cov_xtx ? __ldg(A.cov_xtx + g) : 0.0f;
+    cy = A.cov_yty ? __ldg(A.cov_yty + g) : 0.0f;
+  };
+  int myc = 0, myoff = 0;                                  // lane k: records of seed k, its first record within the event
+  unsigned rbeg = 0u;                                      // first record of the event in ftrk[]
 
   // ================= a4', multi-vertex flavour: implicit association (R-13, R-14) =========
   // Every assignable track is a candidate of every seed: E_ik = exp(-chi2_ik / 2) at the seed positions gives the
   // denominator of Eq. 19; the track is listed for (gets a fit-ready record under) every seed with chi2_ik below the
   // window.  No removal loop (that belongs to the explicit association).
   if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
-    auto load_raw = [&](const int i) {
-      const int g = t0 + min(i, n - 1);
-      RawTrk Q;
-      Q.x = __ldg(A.x + g); Q.y = __ldg(A.y + g); Q.z = __ldg(A.z + g); Q.tx = __ldg(A.tx + g); Q.ty = __ldg(A.ty + g);
-      Q.vx = __ldg(A.var_x + g); Q.vy = __ldg(A.var_y + g); Q.vtx = __ldg(A.var_tx + g); Q.vty = __ldg(A.var_ty + g);
-      return Q;
-    };
-    auto cross_of = [&](const int i, float& cx, float& cy) {   // V_xtx, V_yty of track i (0 = diagonal covariance)
-      const int g = t0 + min(i, n - 1);
-      cx = A.cov_xtx ? __ldg(A.cov_xtx + g) : 0.0f;
-      cy = A.cov_yty ? __ldg(A.cov_yty + g) : 0.0f;
-    };
     auto chi2_at = [&](const RawTrk& R, const float cx, const float cy, const int k) -> float {   // Eq. 7 at seed k, W from Eq. 2; < 0 = unusable (R-7)
       const float zsv = zs[k];
       const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x), sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
@@ -862,14 +914,11 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         __syncwarp();
       }
     };
-    int* mycnt = cnt + tw * 32;
-    mycnt[lane] = 0;
+    cnt[lane] = 0;
     __syncwarp();
     auto count = [&](int k, unsigned peers) {
-      if (k >= 0 && (peers & lanemask_lt()) == 0) mycnt[k] += __popc(peers);
+      if (k >= 0 && (peers & lanemask_lt()) == 0) cnt[k] += __popc(peers);
     };
-    int myc = 0, myoff = 0;
-    unsigned rbeg = 0u;
     bool ovf = false;
     auto emit = [&](const int i, const RawTrk& R, const unsigned mask, const float den) {
       if (i < n) A.best[t0 + i] = 0ull;
@@ -891,24 +940,20 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       });
     };
     // Two passes over the tracks in the same order: pass 0 counts the (track, seed) pairs per seed, pass 1 writes their
-    // records at the counted places.  ONE loop body serves both passes and both kinds of tracks (the first CHUNK are
-    // still in registers, the others are read again): with the candidate and record code inlined once instead of
-    // four / three times the kernel is 30 % smaller, and its 28 warps in different phases stopped missing the
-    // instruction cache (3.3 no-instruction stall cycles per issue before).
-    static_assert(SLOTS == 2, "the two register-held tracks of a lane are selected by hand");
-    unsigned hm0 = 0u, hm1 = 0u;                             // seeds listing my two register-held tracks, their Eq. 19 denominators
+    // records at the counted places.  ONE loop body serves both passes (the candidate and record code exists once: the
+    // kernel stays small enough for the instruction cache); the masks and denominators of the first MV_KEEP * 32 tracks
+    // are kept in registers from pass 0 to pass 1, the others are computed again.
+    unsigned hm0 = 0u, hm1 = 0u;
     float hd0 = 0.0f, hd1 = 0.0f;
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
 #pragma unroll 1
-      for (int it = 0, i0 = tw * 32; i0 < n; ++it, i0 += TEAM) {
+      for (int it = 0, i0 = 0; i0 < n; ++it, i0 += 32) {
         const int i = i0 + lane;
-        RawTrk Q;
-        if (it < SLOTS) Q = it == 0 ? held[0] : held[1];
-        else Q = load_raw(i);
+        const RawTrk Q = load_raw(i);
         unsigned mk = it == 0 ? hm0 : hm1;
         float dn = it == 0 ? hd0 : hd1;
-        if (pass == 0 || it >= SLOTS) cand(i, Q, mk, dn);
+        if (pass == 0 || it >= 2) cand(i, Q, mk, dn);
         if (pass == 0) {
           if (it == 0) { hm0 = mk; hd0 = dn; }
           else if (it == 1) { hm1 = mk; hd1 = dn; }
@@ -918,99 +963,58 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         }
       }
       if (pass == 0) {
-        team_sync(bar);
-        myc = lane < ns ? cnt[lane] + cnt[32 + lane] : 0;
+        __syncwarp();
+        myc = lane < ns ? cnt[lane] : 0;
         const int inc = warp_incl_scan(myc, lane);
         const int nrec = __shfl_sync(FULL, inc, 31);         // (track, seed) records of the event
-        if (tt == 0) misc[5] = (int)atomicAdd(A.trk_counter, (unsigned)nrec);
-        team_sync(bar);
-        rbeg = (unsigned)misc[5];
+        if (lane == 0) rbeg = atomicAdd(A.trk_counter, (unsigned)nrec);
+        rbeg = __shfl_sync(FULL, rbeg, 0);
         ovf = rbeg + (unsigned)nrec > A.trk_cap || rbeg + (unsigned)nrec < rbeg;
         if (ovf) { status |= PV_EVT_RECORD_OVERFLOW; ns = 0; }
         myoff = inc - myc;
-        cur[lane] = (int)rbeg + myoff + (tw ? cnt[lane] : 0);
+        cur[lane] = (int)rbeg + myoff;
         __syncwarp();
       }
     }
-    if (tw == 0) {
-      int rbase = 0;
-      if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
-      rbase = __shfl_sync(FULL, rbase, 0);
-      if (lane < ns) {
-        int4 r;
-        r.x = e; r.y = lane | (myc << 5); r.z = (int)rbeg + myoff; r.w = __float_as_int(zs[lane]);
-        reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
-        if (myc == 0) A.vtx_niter[ev + lane] = -1;           // nothing in the window: the fit never sees this seed
-      }
-      if (__any_sync(FULL, lane < ns && myc == 0)) status |= PV_EVT_SINGULAR_FIT;
-      if (lane == 0) {
-        A.n_vtx[e] = ns;                                     // scratch: seeds of the event, replaced by cleanup_kernel
-        A.event_status[e] = status;
-      }
-      if (DBG) {
-        if (lane == 0) {
-          if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
-          if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
-        }
-        if (lane < ns) {
-          if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
-          if (A.dbg.seed_bins) {
-            A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
-            A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
-            A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
-          }
-        }
-      }
-    }
-    return;
-  }
-
-  // ================= a4: association (R-11) ====================================================
-  // Central bins: the first BINS_SM tracks keep them in shared memory, the rest read them back from the
-  // trk_vertex scratch.  part[] is padded with INT_MAX to whole groups of four.  Warp w takes the tracks
-  // [64 k + 32 w, 64 k + 32 w + 32).
-  auto seed_of = [&](int i) -> int {                       // seed index of track i, -1 = none
-    if (i >= n || ns == 0) return -1;
-    const int b = i < BINS_SM ? (int)binsm[i] : A.trk_vertex[t0 + i];
-    if (b < 0) return -1;
-    int s = 0;
+  } else {
+    // ================= a4: association (R-11) ====================================================
+    // Central bins: the first BINS_SM tracks keep them in shared memory, the rest read them back from the
+    // trk_vertex scratch.  part[] is padded with INT_MAX to whole groups of four.
+    auto seed_of = [&](int i) -> int {                     // seed index of track i, -1 = none
+      if (i >= n || ns == 0) return -1;
+      const int b = i < BINS_SM ? (int)binsm[i] : A.trk_vertex[t0 + i];
+      if (b < 0) return -1;
+      int s = 0;
 #pragma unroll 1
-    for (int k = 0; k + 1 < ns; k += 4) {                  // bins < part[k] belong to seed <= k
-      const int4 pk = *reinterpret_cast<const int4*>(part + k);
-      s += (b >= pk.x ? 1 : 0) + (b >= pk.y ? 1 : 0) + (b >= pk.z ? 1 : 0) + (b >= pk.w ? 1 : 0);
-    }
-    return s;
-  };
-  int sheld[SLOTS];
-#pragma unroll
-  for (int sl = 0; sl < SLOTS; ++sl) sheld[sl] = -1;
-  static_assert(SLOTS == 2, "sheld[] is filled for two slots");
-  for (;;) {
-    if (ns == 0) break;
-    if (tw == 0) part[lane] = lane + 1 < ns ? (se[lane] + sb[lane + 1]) / 2 : 0x7fffffff;
-    cnt[tw * 32 + lane] = 0;
-    team_sync(bar);
+      for (int k = 0; k + 1 < ns; k += 4) {                // bins < part[k] belong to seed <= k
+        const int4 pk = *reinterpret_cast<const int4*>(part + k);
+        s += (b >= pk.x ? 1 : 0) + (b >= pk.y ? 1 : 0) + (b >= pk.z ? 1 : 0) + (b >= pk.w ? 1 : 0);
+      }
+      return s;
+    };
 #pragma unroll 1
-    for (int i0 = tw * 32; i0 < n; i0 += TEAM) {
-      const int s = seed_of(i0 + lane);
-      if (i0 < TEAM) sheld[0] = s;                         // seeds of my register-held tracks, reused by the sort
-      else if (i0 < CHUNK) sheld[1] = s;
-      const unsigned m = __match_any_sync(FULL, s);
-      if (s >= 0 && (m & lanemask_lt()) == 0) cnt[tw * 32 + s] += __popc(m);
+    for (;;) {
+      if (ns == 0) break;
+      part[lane] = lane + 1 < ns ? (se[lane] + sb[lane + 1]) / 2 : 0x7fffffff;
+      cnt[lane] = 0;
       __syncwarp();
-    }
-    team_sync(bar);
-    // "the seed cluster is removed ... and the procedure is repeated": least populated, ties lowest z
-    int key = 0x7fffffff;
-    if (lane < ns) {
-      const int region = zs[lane] < P.z_split ? 1 : 0;
-      const int c = cnt[lane] + cnt[32 + lane];
-      if (c < P.min_tracks_seed[region]) key = (c << 6) | lane;
-    }
-    key = __reduce_min_sync(FULL, key);                    // both warps take the same decision
-    if (key == 0x7fffffff) break;
-    team_sync(bar);                                        // rare path: everyone has read the seed arrays
-    if (tw == 0) {
+#pragma unroll 1
+      for (int i0 = 0; i0 < n; i0 += 32) {
+        const int s = seed_of(i0 + lane);
+        if (i0 + lane < SEEDOF_SM) seedsm[i0 + lane] = (int8_t)s;   // reused by the sort (the last pass of this loop is final)
+        const unsigned m = __match_any_sync(FULL, s);
+        if (s >= 0 && (m & lanemask_lt()) == 0) cnt[s] += __popc(m);
+        __syncwarp();
+      }
+      // "the seed cluster is removed ... and the procedure is repeated": least populated, ties lowest z
+      int key = 0x7fffffff;
+      if (lane < ns) {
+        const int region = zs[lane] < P.z_split ? 1 : 0;
+        const int c = cnt[lane];
+        if (c < P.min_tracks_seed[region]) key = (c << 6) | lane;
+      }
+      key = __reduce_min_sync(FULL, key);
+      if (key == 0x7fffffff) break;
       const int worst = key & 63;
       int nb = 0, ne = 0, np = 0;
       float nz = 0.0f;
@@ -1018,114 +1022,111 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       if (mv) { nb = sb[lane + 1]; ne = se[lane + 1]; np = sp[lane + 1]; nz = zs[lane + 1]; }
       __syncwarp();
       if (mv) { sb[lane] = nb; se[lane] = ne; sp[lane] = np; zs[lane] = nz; }
+      --ns;
+      __syncwarp();
     }
-    --ns;
-    team_sync(bar);
-  }
-  // counting sort of the tracks by seed: a seed's records are warp 0's tracks in track order, then warp 1's
-  // (deterministic); every assigned track is written as a fit-ready record (local frame of its seed, W at the
-  // seed position) at its sorted place
-  int myc = 0, myoff = 0;
-  {
-    myc = (ns > 0 && lane < ns) ? cnt[lane] + cnt[32 + lane] : 0;
-    const int inc = warp_incl_scan(myc, lane);
-    myoff = inc - myc;
-    cur[lane] = myoff + ((tw && ns > 0) ? cnt[lane] : 0);
-  }
-  __syncwarp();
-  auto place = [&](const int i, const RawTrk& R, const bool from_memory, const int s) {
-    const unsigned m = __match_any_sync(FULL, s);
-    const int rank = __popc(m & lanemask_lt());
-    if (i < n) {
-      // scratch for cleanup_kernel: seed index | position of the track's record within the event << 5 (the fit
-      // leaves the track's weight at that record position)
-      A.trk_vertex[t0 + i] = s >= 0 ? (s | ((cur[s] + rank) << 5)) : -1;
-      if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
+    // counting sort of the tracks by seed (a seed's records are its tracks in track order: deterministic); every
+    // assigned track is written as a fit-ready record (local frame of its seed, W at the seed position) at its place
+    myc = (ns > 0 && lane < ns) ? cnt[lane] : 0;
+    {
+      const int inc = warp_incl_scan(myc, lane);
+      myoff = inc - myc;
+      cur[lane] = myoff;
     }
-    if (s >= 0) {
-      RawTrk Q = R;
-      if (from_memory) {
-        const int g = t0 + i;
-        Q.x = __ldg(A.x + g); Q.y = __ldg(A.y + g); Q.z = __ldg(A.z + g); Q.tx = __ldg(A.tx + g); Q.ty = __ldg(A.ty + g);
-        Q.vx = __ldg(A.var_x + g); Q.vy = __ldg(A.var_y + g); Q.vtx = __ldg(A.var_tx + g); Q.vty = __ldg(A.var_ty + g);
-      }
-      const float zsv = zs[s];
-      const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
-      const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
-      const float cx = A.cov_xtx ? __ldg(A.cov_xtx + t0 + i) : 0.0f, cy = A.cov_yty ? __ldg(A.cov_yty + t0 + i) : 0.0f;
-      const Trk T = make_track(P, Q, cx, cy, sx, sy, zsv, have_cross);
-      float4* o = A.ftrk + 2 * (size_t)(t0 + cur[s] + rank);
-      o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
-      o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), 0.0f);
-    }
+    rbeg = (unsigned)t0;
     __syncwarp();
-    if (s >= 0 && rank == 0) cur[s] += __popc(m);
-    __syncwarp();
-  };
-#pragma unroll
-  for (int sl = 0; sl < SLOTS; ++sl)
-    if (sl * TEAM + tw * 32 < n) place(sl * TEAM + tt, held[sl], false, ns > 0 ? sheld[sl] : -1);
 #pragma unroll 1
-  for (int i0 = CHUNK + tw * 32; i0 < n; i0 += TEAM) place(i0 + lane, held[0], true, seed_of(i0 + lane));
-  // seed records for fit_kernel
-  if (tw == 0) {
-    int rbase = 0;
-    if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
-    rbase = __shfl_sync(FULL, rbase, 0);
-    if (lane < ns) {
-      int4 r;
-      r.x = e; r.y = lane | (myc << 5); r.z = t0 + myoff; r.w = __float_as_int(zs[lane]);
-      reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
-      if (myc == 0) A.vtx_niter[ev + lane] = -1;             // only with min_tracks_seed < 1: the fit never sees this seed
-    }
-    if (__any_sync(FULL, lane < ns && myc == 0)) status |= PV_EVT_SINGULAR_FIT;
-    if (lane == 0) {
-      A.n_vtx[e] = ns;                                     // scratch: seeds of the event, replaced by cleanup_kernel
-      A.event_status[e] = status;
-    }
-    if (DBG) {
-      if (lane == 0) {
-        if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
-        if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
+    for (int i0 = 0; i0 < n; i0 += 32) {
+      const int i = i0 + lane;
+      const RawTrk Q = load_raw(i);                          // issued ahead of the seed look-up
+      float cx, cy;
+      cross_of(i, cx, cy);
+      const int s = ns == 0 ? -1 : (i < SEEDOF_SM ? (i < n ? (int)seedsm[i] : -1) : seed_of(i));
+      const unsigned m = __match_any_sync(FULL, s);
+      const int rank = __popc(m & lanemask_lt());
+      if (i < n) {
+        // scratch for cleanup_kernel: seed index | position of the track's record within the event << 5 (the fit
+        // leaves the track's weight at that record position)
+        A.trk_vertex[t0 + i] = s >= 0 ? (s | ((cur[s] + rank) << 5)) : -1;
+        if (DBG && A.dbg.trk_seed) A.dbg.trk_seed[t0 + i] = s;
       }
-      if (lane < ns) {
-        if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
-        if (A.dbg.seed_bins) {
-          A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
-          A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
-          A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
-        }
+      if (s >= 0) {
+        const float zsv = zs[s];
+        const float sx = __fmaf_rn(P.beam_tx, zsv, P.beam_x);  // "xy position ... using the known beamline"
+        const float sy = __fmaf_rn(P.beam_ty, zsv, P.beam_y);
+        const Trk T = make_track(P, Q, cx, cy, sx, sy, zsv, have_cross);
+        float4* o = A.ftrk + 2 * (size_t)(t0 + cur[s] + rank);
+        o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
+        o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), 0.0f);
+      }
+      __syncwarp();
+      if (s >= 0 && rank == 0) cur[s] += __popc(m);
+      __syncwarp();
+    }
+  }
+
+  // seed records for fit_kernel
+  int rbase = 0;
+  if (lane == 0 && ns > 0) rbase = (int)atomicAdd(A.seed_counter, (unsigned)ns);
+  rbase = __shfl_sync(FULL, rbase, 0);
+  if (lane < ns) {
+    int4 r;
+    r.x = e; r.y = lane | (myc << 5); r.z = (int)rbeg + myoff; r.w = __float_as_int(zs[lane]);
+    reinterpret_cast<int4*>(A.rec)[rbase + lane] = r;
+    if (myc == 0) A.vtx_niter[ev + lane] = -1;               // nothing listed (or min_tracks_seed < 1): the fit never sees this seed
+  }
+  if (__any_sync(FULL, lane < ns && myc == 0)) status |= PV_EVT_SINGULAR_FIT;
+  if (lane == 0) {
+    A.n_vtx[e] = ns;                                       // scratch: seeds of the event, replaced by cleanup_kernel
+    A.event_status[e] = status;
+  }
+  if (DBG) {
+    if (lane == 0) {
+      if (A.dbg.n_seeds) A.dbg.n_seeds[e] = ns;
+      if (A.dbg.n_seeds_raw) A.dbg.n_seeds_raw[e] = n_raw;
+    }
+    if (lane < ns) {
+      if (A.dbg.seed_z) A.dbg.seed_z[ev + lane] = zs[lane];
+      if (A.dbg.seed_bins) {
+        A.dbg.seed_bins[(ev + lane) * 3 + 0] = sb[lane];
+        A.dbg.seed_bins[(ev + lane) * 3 + 1] = se[lane];
+        A.dbg.seed_bins[(ev + lane) * 3 + 2] = sp[lane];
       }
     }
   }
+  __syncwarp();                                            // the next event overwrites the seed arrays
 }
 
 template <bool DBG, int FLAV, int SPLIT, int FILL>
-__global__ void __launch_bounds__(MAX_TEAMS * TEAM, 1) seed_kernel(const __grid_constant__ KParams P,
-                                                                   const __grid_constant__ KArgs A) {
+__global__ void __launch_bounds__(SEED_WARPS * 32, 1) seed_kernel(const __grid_constant__ KParams P,
+                                                                 const __grid_constant__ KArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int team = threadIdx.x / TEAM, tt = threadIdx.x % TEAM;
-  const int bar = 1 + team;                                // named barrier of the team (0 is __syncthreads)
-  unsigned char* wsm = smem_raw + (size_t)team * P.team_smem_bytes;
-  int* misc = reinterpret_cast<int*>(wsm + (size_t)P.region0_words * 4 + SM_MISC);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int* pool = reinterpret_cast<int*>(smem_raw);            // [1 + n_blocks * BLK_WORDS] words of 32 bins; word 0 = NULL word
+  const int pool_bytes = (1 + P.n_blocks * BLK_WORDS) * 128;
+  unsigned* bm = reinterpret_cast<unsigned*>(smem_raw + pool_bytes);   // free blocks, one bit each
+  unsigned char* wsm = smem_raw + pool_bytes + SM_HDR_BYTES + (size_t)warp * WARP_SMEM;
   {
-    int4* Z = reinterpret_cast<int4*>(wsm);                // histogram and touched-word flags start at zero
-    const int nq = (P.region0_words * 4 + SM_MISC) >> 4;
+    int4* Z = reinterpret_cast<int4*>(smem_raw);           // the pool and every warp's map / flags start at zero
+    const int nq = (pool_bytes + SM_HDR_BYTES + (int)blockDim.x / 32 * WARP_SMEM) >> 4;
 #pragma unroll 1
-    for (int i = tt; i < nq; i += TEAM) Z[i] = make_int4(0, 0, 0, 0);
+    for (int i = threadIdx.x; i < nq; i += blockDim.x) Z[i] = make_int4(0, 0, 0, 0);
   }
-  if (tt == 0) { misc[6] = 0; misc[8] = (int)atomicAdd(A.evt_counter, 1u); }
-  team_sync(bar);
-  int e = misc[8];
+  __syncthreads();
+  if (threadIdx.x < SM_HDR_BYTES / 4) {
+    const int lo = threadIdx.x * 32;
+    bm[threadIdx.x] = P.n_blocks >= lo + 32 ? 0xffffffffu : P.n_blocks > lo ? (1u << (P.n_blocks - lo)) - 1u : 0u;
+  }
+  __syncthreads();
+  int e = 0;
+  if (lane == 0) e = (int)atomicAdd(A.evt_counter, 1u);
+  e = __shfl_sync(FULL, e, 0);
+#pragma unroll 1
   while (e < A.n_events) {
     int nxt = 0x7fffffff;
-    if (tt == 32) nxt = (int)atomicAdd(A.evt_counter, 1u); // issued now, consumed by the prefetch and after this event
-    seed_event<DBG, FLAV, SPLIT, FILL>(e, nxt, P, A, wsm, tt, bar);
-    // misc[8] was last read before this event, and both warps have met at a barrier inside it since: the next event can
-    // be published ahead of the barrier that also says the team is done with this event's shared memory
-    if (tt == 32) misc[8] = nxt;
-    team_sync(bar);
-    e = misc[8];
+    if (lane == 0) nxt = (int)atomicAdd(A.evt_counter, 1u);  // issued now, consumed by the prefetch and after this event
+    seed_event<DBG, FLAV, SPLIT, FILL>(e, nxt, P, A, pool, bm, wsm, lane);
+    e = __shfl_sync(FULL, nxt, 0);
   }
 }
 
