@@ -208,17 +208,17 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   }
 #endif
   const int fixed = 128 + pvk::SM_HDR_BYTES + warps * pvk::WARP_SMEM;
-  int n_blocks = (di->max_smem_optin - fixed) / (pvk::BLK_WORDS * 128);
-  if (n_blocks > pvk::SM_HDR_BYTES * 8) n_blocks = pvk::SM_HDR_BYTES * 8;
+  int n_pool = (di->max_smem_optin - fixed) / 128;            // words of 32 bins
+  if (n_pool > pvk::SM_HDR_BYTES * 8) n_pool = pvk::SM_HDR_BYTES * 8;
 #ifdef PV_TUNING
-  if (const char* envb = getenv("PV_POOL_BLOCKS")) {
+  if (const char* envb = getenv("PV_POOL_WORDS")) {
     const int w = atoi(envb);
-    if (w >= 1 && w < n_blocks) n_blocks = w;
+    if (w >= 1 && w < n_pool) n_pool = w;
   }
 #endif
-  if (n_blocks < pvk::MAX_WORDS / pvk::BLK_WORDS) return PV_E_PARAM;   // one event may need every word of the histogram
-  kp.n_blocks = n_blocks;
-  const int smem = fixed + n_blocks * pvk::BLK_WORDS * 128;
+  if (n_pool < pvk::MAX_WORDS) return PV_E_PARAM;             // one event may need every word of the histogram
+  kp.n_pool = n_pool;
+  const int smem = fixed + n_pool * 128;
   const int mvf = params->flavour == PV_FLAVOUR_MULTIVERTEX ? 1 : 0;
   const int spl = params->split_mode == PV_SPLIT_RECURSIVE ? 1 : 0;
   const int tfl = params->fill_mode == PV_FILL_TEMPLATE ? 1 : 0;

@@ -49,7 +49,6 @@ constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT
 constexpr int LIST_CAP = 192;       // fill units of one round (a chunk of median tracks needs ~100)
 constexpr int BINS_SM = 128;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int SEEDOF_SM = 128;      // ... whose seed index stays in shared memory between the count and the sort of a4
-constexpr int BLK_WORDS = 8;        // histogram words (of 32 bins) per block of the CTA's pool
 constexpr int FIT_UNROLL = PV_FIT_UNROLL;   // unroll of the track loop of one fit iteration
 #ifndef PV_FIT_KF
 #define PV_FIT_KF 14
@@ -71,14 +70,14 @@ constexpr int PROTO_CAP = 256;      // proto-cluster starts of one sweep round (
 constexpr int TMPL_J = 8;           // template fill: positions of z_poca inside its central bin
 constexpr int TMPL_MAXK = 56;       // template fill: sigma classes (validate() bounds max_sigma_poca / dz)
 
-// Shared memory of seed_kernel: [pool: 1 NULL word + n_blocks * BLK_WORDS words of 32 int32 bins][block bitmap]
+// Shared memory of seed_kernel: [pool: 1 NULL word + n_pool words of 32 int32 bins][bitmap of the free pool words]
 // [SEED_WARPS x WARP_SMEM].  Per warp, in bytes; the 1152 bytes that stage the fill (track windows and the unit list)
 // are dead once the histogram is complete: the peak search and the association reuse them.
-constexpr int SM_HDR_BYTES = 32;                           // unsigned bm[8]       free blocks of the pool, one bit each
+constexpr int SM_HDR_BYTES = 256;                          // unsigned bm[64]      free words of the pool, one bit each
 constexpr int SM_MAP = 0;                                  // uint16 map[128]      histogram word -> pool word (0 = NULL word)
-constexpr int SM_TB = SM_MAP + MAX_WORDS * 2;              // uint8 tb[128]        histogram words of the chunk's windows
+constexpr int SM_TB = SM_MAP + MAX_WORDS * 2;              // uint8 tb[128]        fill: unmapped words of the chunk's windows; peaks: list of the mapped words
 constexpr int SM_MISC = SM_TB + MAX_WORDS;                 // unsigned mapped[4]   words that have a pool word (+ spare)
-constexpr int SM_BLK = SM_MISC + 64;                       // uint16 blk[16]       blocks of this event (+ spare)
+constexpr int SM_BLK = SM_MISC + 64;                       // uint16 got[32]       pool words just taken
 constexpr int SM_BINS = SM_BLK + 64;                       // int16 binsm[128]     central bins of the first 128 tracks
 constexpr int SM_STAGE = SM_BINS + BINS_SM * 2;            // fill:  float zp[64], inv[64]; int lonb[64]
 constexpr int SM_LIST = SM_STAGE + CHUNK * 12;             // fill:  uint16 list[192]
@@ -91,7 +90,7 @@ constexpr int WARP_SMEM = SM_LIST + LIST_CAP * 2;
 static_assert(SM_SEED + 5 * MAXV * 4 <= WARP_SMEM, "the overlays fit the fill stage and unit list");
 static_assert(SM_SEEDOF + SEEDOF_SM <= SM_SEED, "cnt, cur and seedsm fit over the proto-cluster list");
 static_assert(SM_STAGE % 16 == 0 && SM_SEED % 16 == 0 && WARP_SMEM % 16 == 0, "alignment of the vector accesses");
-static_assert(MAX_WORDS / BLK_WORDS <= 16 && MAX_WORDS <= 128, "blk[] and mapped[] sizes");
+static_assert(MAX_WORDS <= 128, "mapped[] holds four masks of 32 words");
 
 struct KParams {
   float z_min, dz, inv_dz, z_split;
@@ -111,7 +110,7 @@ struct KParams {
   int split_mode;                // PV_SPLIT_*
   float chi2_window;             // multi-vertex flavour: list a track for a seed iff chi2 at the seed position < this
   float mv_e0;                   // exp(-chi2_max / 2), the constant of the denominator of Eq. 19
-  int n_blocks;                  // blocks of BLK_WORDS histogram words in the pool of a CTA of seed_kernel
+  int n_pool;                    // words (of 32 bins) in the histogram pool of a CTA of seed_kernel, without the NULL word
   int tmpl_kmax;                 // template fill (R-17): class of the largest sigma cut = last class
   int tmpl_off[TMPL_MAXK];       // first table entry of class k; its TMPL_J templates of 2 W_k + 1 bins follow each other
   short tmpl_w[TMPL_MAXK];       // W_k = ceil(3 sigma_k / dz)
@@ -507,35 +506,57 @@ __device__ __forceinline__ Trk make_track(const KParams& P, const RawTrk& R, flo
 // Persistent grid, one CTA of SEED_WARPS warps per SM, every warp works through whole events on its own (events are
 // handed out by an atomic counter): no CTA or team barrier anywhere, __syncwarp only.
 // Histograms are SPARSE: an event touches ~13 of its 107 words of 32 bins (configs[1]; ~33 at high pile-up), so a dense
-// int32 histogram per event (13.6 KB) would hold the SM to 14 events in flight.  Instead the CTA owns a pool of blocks
-// of BLK_WORDS words; a warp maps the words its tracks touch to pool words as it meets them (map[], one uint16 per
-// histogram word; pool word 0 is the NULL word, always zero, where every untouched word points) and takes blocks from
-// a shared bitmap as it needs them.  When the pool runs dry a warp that holds blocks gives them back and starts its
-// event again (no hold-and-wait, hence no deadlock); a warp that holds none simply waits.
+// int32 histogram per event (13.6 KB) would hold the SM to 14 events in flight.  Instead the CTA owns a pool of words;
+// a warp maps the histogram words its tracks touch to pool words as it meets them (map[], one uint16 per histogram
+// word; pool word 0 is the NULL word, always zero, where every untouched word points) and takes them from a shared
+// bitmap.  When the pool runs dry a warp that holds words gives them back and starts its event again (no
+// hold-and-wait, hence no deadlock); a warp that holds none simply waits.
 struct Hist {
   const int* pool;
   const uint16_t* map;
   __device__ __forceinline__ int operator[](int b) const { return pool[((int)map[b >> 5] << 5) + (b & 31)]; }
 };
 
-// one free block of the pool (warp-collective; the same value in every lane), -1 when there is none right now
-__device__ __forceinline__ int blk_try_alloc(unsigned* bm, const int nbw, const int lane) {
-  unsigned m = lane < nbw ? reinterpret_cast<volatile unsigned*>(bm)[lane] : 0u;
-  for (;;) {
-    const unsigned has = __ballot_sync(FULL, m != 0u);
-    if (!has) return -1;
-    const int src = __ffs(has) - 1;
-    int got = -1;
-    if (lane == src) {
-      const int b = __ffs(m) - 1;
-      const unsigned bit = 1u << b;
-      const unsigned old = atomicAnd(&bm[lane], ~bit);
-      if (old & bit) got = lane * 32 + b;
-      m = old & ~bit;
+// One pool word for every lane set in `want` (warp-collective): every lane looks at its own two words of the bitmap
+// and takes one free bit, as many lanes as words are still missing, counted from lane `rot` on (every warp and event
+// starts somewhere else, so that the warps of the CTA do not all fight for the same bitmap word); the words taken are
+// handed to the wanting lanes in lane order through got[].  Returns false (nothing kept) when the pool stays dry
+// while this warp holds words (`holding`): the caller gives everything back and starts its event again.  A warp that
+// holds nothing waits.
+__device__ __forceinline__ bool pool_alloc(unsigned* bm, const int nbw, const unsigned want, const int holding, const int rot,
+                                           const int lane, uint16_t* got, int& id) {
+  const int k = __popc(want);
+  const unsigned before = (1u << ((lane - rot) & 31)) - 1u;  // lanes counted before mine, in the rotated order
+  int have = 0, spins = 0;
+#pragma unroll 1
+  while (have < k) {
+    const unsigned m0 = reinterpret_cast<volatile unsigned*>(bm)[lane];
+    const unsigned m1 = lane + 32 < nbw ? reinterpret_cast<volatile unsigned*>(bm)[lane + 32] : 0u;
+    const int idx = m0 ? lane : lane + 32;
+    const unsigned m = m0 ? m0 : m1;
+    const unsigned cand = __ballot_sync(FULL, m != 0u);
+    int mine = -1;
+    if (m != 0u && __popc(__funnelshift_r(cand, cand, rot) & before) < k - have) {
+      const unsigned bit = 1u << (__ffs(m) - 1);
+      if (atomicAnd(&bm[idx], ~bit) & bit) mine = idx * 32 + __ffs(m) - 1;
     }
-    got = __shfl_sync(FULL, got, src);
-    if (got >= 0) return got;
+    const unsigned okm = __ballot_sync(FULL, mine >= 0);
+    if (mine >= 0) got[have + __popc(okm & lanemask_lt())] = (uint16_t)(1 + mine);
+    have += __popc(okm);
+    if (cand == 0u) {                                        // the pool is dry (a lost race is simply tried again)
+      if (holding + have > 0 && ++spins > 32) {              // give back what this call took
+        __syncwarp();
+        if (lane < have) { const int w = (int)got[lane] - 1; atomicOr(&bm[w >> 5], 1u << (w & 31)); }
+        __syncwarp();
+        return false;
+      }
+      __nanosleep(200);
+    }
   }
+  __syncwarp();
+  if ((want >> lane) & 1u) id = got[__popc(want & lanemask_lt())];
+  __syncwarp();
+  return true;
 }
 
 template <bool DBG, int FLAV, int SPLIT, int FILL>
@@ -544,7 +565,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   uint16_t* map = reinterpret_cast<uint16_t*>(wsm + SM_MAP);
   uint8_t* tb = reinterpret_cast<uint8_t*>(wsm + SM_TB);
   unsigned* mapped = reinterpret_cast<unsigned*>(wsm + SM_MISC);   // mapped[c]: words 32 c .. 32 c + 31 that have a pool word
-  uint16_t* blk = reinterpret_cast<uint16_t*>(wsm + SM_BLK);
+  uint16_t* got = reinterpret_cast<uint16_t*>(wsm + SM_BLK);
   int16_t* binsm = reinterpret_cast<int16_t*>(wsm + SM_BINS);
   float* st_zp = reinterpret_cast<float*>(wsm + SM_STAGE);
   float* st_inv = st_zp + CHUNK;
@@ -587,28 +608,28 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   }
 
   const int nwc = (P.nwords + 31) >> 5;                    // chunks of 32 histogram words
-  const int nbw = (P.n_blocks + 31) >> 5;                  // words of the block bitmap
-  int nslots = 0, nblk = 0;                                // pool words / blocks of this event (warp-uniform)
-  // zero my pool words, unmap them and give the blocks back: leaves the warp's histogram state as it is between events
+  const int nbw = (P.n_pool + 31) >> 5;                    // words of the pool bitmap
+  int nheld = 0;                                           // pool words of this event (warp-uniform)
+  // zero my pool words, unmap them and give them back: leaves the warp's histogram state as it is between events.
+  // Lane l takes the word 32 c + l: sixteen bytes at a time, starting at a different place in every lane.
   auto release = [&]() {
 #pragma unroll 1
     for (int c = 0; c < nwc; ++c) {
-      const unsigned mc = mapped[c];
-      unsigned m = mc;
-#pragma unroll 1
-      while (m) {
-        const int w = 32 * c + __ffs(m) - 1;
-        m &= m - 1u;
-        pool[((int)map[w] << 5) + lane] = 0;
+      const bool mine = (mapped[c] >> lane) & 1u;
+      int id = 0;
+      if (mine) {
+        id = map[32 * c + lane];
+        int4* q = reinterpret_cast<int4*>(pool + (id << 5));
+#pragma unroll
+        for (int j = 0; j < 8; ++j) q[(j + lane) & 7] = make_int4(0, 0, 0, 0);
+        map[32 * c + lane] = 0;
       }
+      __threadfence_block();                               // the zeros are in place before another warp can take the word
       __syncwarp();
-      if ((mc >> lane) & 1u) map[32 * c + lane] = 0;
+      if (mine) atomicOr(&bm[(id - 1) >> 5], 1u << ((id - 1) & 31));
       if (lane == 0) mapped[c] = 0u;
     }
-    __threadfence_block();                                 // the zeros are in place before another warp can take a block
-    __syncwarp();
-    if (lane < nblk) { const int b = blk[lane]; atomicOr(&bm[b >> 5], 1u << (b & 31)); }
-    nslots = 0; nblk = 0;
+    nheld = 0;
     __syncwarp();
   };
 
@@ -632,6 +653,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       }
       int nun[SLOTS];                                      // fill units of my tracks
       int myunits = 0;
+      bool sawnew = false;
 #pragma unroll
       for (int s = 0; s < SLOTS; ++s) {
         const int i = c0 + s * 32 + lane;
@@ -667,45 +689,26 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
             nun[s] = (nb + UNIT - 1) / UNIT;
             st_lonb[s * 32 + lane] = lo | (nb << 12);
 #pragma unroll 1
-            for (int w = lo >> 5; w <= (lo + nb - 1) >> 5; ++w) tb[w] = 1;   // histogram words of the window
+            for (int w = lo >> 5; w <= (lo + nb - 1) >> 5; ++w)   // histogram words of the window without a pool word
+              if (map[w] == 0) { tb[w] = 1; sawnew = true; }
           }
         }
         myunits += nun[s];
       }
       __syncwarp();
-      // ---- words met for the first time get a pool word (and the event another block when it needs one)
+      // ---- words met for the first time get a pool word
+      if (__any_sync(FULL, sawnew)) {
 #pragma unroll 1
-      for (int c = 0; c < nwc; ++c) {
-        const int f = tb[32 * c + lane];
-        const unsigned m = __ballot_sync(FULL, f != 0);
-        if (m == 0u) continue;
-        if (f) tb[32 * c + lane] = 0;
-        const unsigned newm = m & ~mapped[c];
-        if (newm == 0u) continue;
-        const int cntn = __popc(newm);
-        const int need = (nslots + cntn + BLK_WORDS - 1) / BLK_WORDS;
-        int spins = 0;
-#pragma unroll 1
-        while (nblk < need) {
-          const int b = blk_try_alloc(bm, nbw, lane);
-          if (b >= 0) {
-            if (lane == 0) blk[nblk] = (uint16_t)b;
-            ++nblk;
-            continue;
-          }
-          if (nblk > 0 && ++spins > 32) break;             // pool dry while I hold blocks: give them back, start again
-          __nanosleep(200);
+        for (int c = 0; c < nwc; ++c) {
+          const int f = tb[32 * c + lane];
+          const unsigned newm = __ballot_sync(FULL, f != 0);
+          if (newm == 0u) continue;
+          int id = 0;
+          if (!pool_alloc(bm, nbw, newm, nheld, (e * 7 + c0 + 8 * c) & 31, lane, got, id)) { filled = false; break; }   // pool dry: start again
+          if (f) { tb[32 * c + lane] = 0; map[32 * c + lane] = (uint16_t)id; }
+          nheld += __popc(newm);
+          if (lane == 0) mapped[c] |= newm;
         }
-        if (nblk < need) { filled = false; break; }
-        __threadfence_block();
-        __syncwarp();
-        if ((newm >> lane) & 1u) {
-          const int slot = nslots + __popc(newm & lanemask_lt());
-          map[32 * c + lane] = (uint16_t)(1 + (int)blk[slot / BLK_WORDS] * BLK_WORDS + (slot % BLK_WORDS));
-        }
-        nslots += cntn;
-        __syncwarp();
-        if (lane == 0) mapped[c] |= newm;
         __syncwarp();
       }
       if (!filled) break;
@@ -773,35 +776,63 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
 
   // ================= a3: peak search and seed position (Eq. 4-5) ==============================
-  // The mapped words, ascending, are the only ones that can hold bins above the threshold: one ballot per word finds
-  // the first bin of every run above threshold (proto-cluster), then one lane per proto-cluster runs the z-ordered
-  // hysteresis sweep (select-based state machine: the serial length is the longest proto-cluster).
+  // The mapped words, ascending, are the only ones that can hold bins above the threshold.  One LANE per mapped word
+  // reads its 32 bins (sixteen bytes at a time, starting at a different place in every lane) into a bit mask of the
+  // bins above threshold; the first bin of every run (proto-cluster) follows from the mask and the top bit of the
+  // word before.  Then one lane per proto-cluster runs the z-ordered hysteresis sweep (select-based state machine: the
+  // serial length is the longest proto-cluster).
   int n_raw = 0;
   {
-    int dc = 0;
-    unsigned dm = mapped[0];
-    int prev_w = -2;
-    unsigned prev_top = 0u;
+    uint8_t* twl = tb;                                     // list of the mapped words (the flags of the fill are all zero now)
+    int ntw = 0;
 #pragma unroll 1
-    do {
-      int np = 0;
+    for (int c = 0; c < nwc; ++c) {
+      const unsigned mc = mapped[c];
+      if ((mc >> lane) & 1u) twl[ntw + __popc(mc & lanemask_lt())] = (uint8_t)(32 * c + lane);
+      ntw += __popc(mc);
+    }
+    __syncwarp();
+    int carry_w = -2;                                      // last word of the pass before and its mask
+    unsigned carry_m = 0u;
 #pragma unroll 1
-      while (dc < nwc && np + 16 <= PROTO_CAP) {           // a word of 32 bins starts at most 16 runs
-        if (dm == 0u) {
-          ++dc;
-          dm = dc < nwc ? mapped[dc] : 0u;
-          continue;
+    for (int r0 = 0; r0 < ntw;) {
+      int step = min(32, ntw - r0);
+      const int w = lane < step ? (int)twl[r0 + lane] : -5;
+      unsigned m = 0u;
+      if (lane < step) {
+        const int4* q = reinterpret_cast<const int4*>(pool + ((int)map[w] << 5));   // bins beyond nbins are padding and stay 0
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int g = (j + lane) & 7;
+          const int4 v = q[g];
+          const unsigned nib = (v.x > P.T_bin ? 1u : 0u) | (v.y > P.T_bin ? 2u : 0u) | (v.z > P.T_bin ? 4u : 0u) | (v.w > P.T_bin ? 8u : 0u);
+          m |= nib << (4 * g);
         }
-        const int w = 32 * dc + __ffs(dm) - 1;
-        dm &= dm - 1u;
-        const int h = pool[((int)map[w] << 5) + lane];     // bins beyond nbins are padding and stay 0
-        const unsigned m = __ballot_sync(FULL, h > P.T_bin);
-        const unsigned carry = (prev_w == w - 1) ? prev_top : 0u;
-        const unsigned starts = m & ~((m << 1) | carry);   // first bin of each run of bins above threshold
-        if ((starts >> lane) & 1u) ps[np + __popc(starts & lanemask_lt())] = (uint16_t)(32 * w + lane);
-        np += __popc(starts);
-        prev_w = w; prev_top = m >> 31;
       }
+      unsigned pm = __shfl_up_sync(FULL, m, 1);
+      int pw = __shfl_up_sync(FULL, w, 1);
+      if (lane == 0) { pm = carry_m; pw = carry_w; }
+      const unsigned carry = (pw == w - 1) ? pm >> 31 : 0u;
+      unsigned starts = m & ~((m << 1) | carry);           // first bin of each run of bins above threshold
+      int c = __popc(starts);
+      int inc = warp_incl_scan(c, lane);
+      if (__shfl_sync(FULL, inc, 31) > PROTO_CAP) {        // never with physical histograms: a word starts at most 16 runs
+        step = min(step, PROTO_CAP / 16);
+        if (lane >= step) { c = 0; starts = 0u; }
+        inc = warp_incl_scan(c, lane);
+      }
+      const int np = __shfl_sync(FULL, inc, 31);
+      {
+        int o = inc - c;
+#pragma unroll 1
+        while (starts) {
+          ps[o++] = (uint16_t)(32 * w + __ffs(starts) - 1);
+          starts &= starts - 1u;
+        }
+      }
+      carry_w = __shfl_sync(FULL, w, step - 1);
+      carry_m = __shfl_sync(FULL, m, step - 1);
+      r0 += step;
       __syncwarp();
 #pragma unroll 1
       for (int p0 = 0; p0 < np; p0 += 32) {                // one lane per proto-cluster
@@ -809,27 +840,28 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         const bool act = p < np;
         const int b0 = act ? (int)ps[p] : 0;
         Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
-        int c = 0, base = 0;
+        int cl = 0, base = 0;
 #pragma unroll 1
         for (int rep = 0; rep < 2; ++rep) {                // rep 1 (rare): proto-clusters with three or more seeds
-          const bool run = act && (rep == 0 || (c > 2 && base + 2 < P.max_vtx));
+          const bool run = act && (rep == 0 || (cl > 2 && base + 2 < P.max_vtx));
           if (!__any_sync(FULL, run)) break;
           if (run) {
             const int cc = SPLIT ? split_x86(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1)
                                  : sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
-            if (rep == 0) c = cc;
+            if (rep == 0) cl = cc;
           }
           if (rep == 0) {
-            const int inc = warp_incl_scan(c, lane);
-            base = n_raw + inc - c;
-            if (c > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
-            if (c > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
-            n_raw += __shfl_sync(FULL, inc, 31);
+            const int inc2 = warp_incl_scan(cl, lane);
+            base = n_raw + inc2 - cl;
+            if (cl > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
+            if (cl > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
+            n_raw += __shfl_sync(FULL, inc2, 31);
           }
         }
       }
       __syncwarp();
-    } while (dc < nwc);
+    }
+    reinterpret_cast<unsigned*>(tb)[lane] = 0u;            // the flags of the next fill start at zero
   }
   int ns = n_raw;
   if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
@@ -1002,10 +1034,9 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       for (int i0 = 0; i0 < n; i0 += 32) {
         const int s = seed_of(i0 + lane);
         if (i0 + lane < SEEDOF_SM) seedsm[i0 + lane] = (int8_t)s;   // reused by the sort (the last pass of this loop is final)
-        const unsigned m = __match_any_sync(FULL, s);
-        if (s >= 0 && (m & lanemask_lt()) == 0) cnt[s] += __popc(m);
-        __syncwarp();
+        if (s >= 0) atomicAdd(&cnt[s], 1);                     // a count: the order does not matter
       }
+      __syncwarp();
       // "the seed cluster is removed ... and the procedure is repeated": least populated, ties lowest z
       int key = 0x7fffffff;
       if (lane < ns) {
@@ -1102,9 +1133,9 @@ __global__ void __launch_bounds__(SEED_WARPS * 32, 1) seed_kernel(const __grid_c
                                                                  const __grid_constant__ KArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  int* pool = reinterpret_cast<int*>(smem_raw);            // [1 + n_blocks * BLK_WORDS] words of 32 bins; word 0 = NULL word
-  const int pool_bytes = (1 + P.n_blocks * BLK_WORDS) * 128;
-  unsigned* bm = reinterpret_cast<unsigned*>(smem_raw + pool_bytes);   // free blocks, one bit each
+  int* pool = reinterpret_cast<int*>(smem_raw);            // [1 + n_pool] words of 32 bins; word 0 = NULL word
+  const int pool_bytes = (1 + P.n_pool) * 128;
+  unsigned* bm = reinterpret_cast<unsigned*>(smem_raw + pool_bytes);   // free pool words, one bit each (bit i = pool word 1 + i)
   unsigned char* wsm = smem_raw + pool_bytes + SM_HDR_BYTES + (size_t)warp * WARP_SMEM;
   {
     int4* Z = reinterpret_cast<int4*>(smem_raw);           // the pool and every warp's map / flags start at zero
@@ -1115,7 +1146,7 @@ __global__ void __launch_bounds__(SEED_WARPS * 32, 1) seed_kernel(const __grid_c
   __syncthreads();
   if (threadIdx.x < SM_HDR_BYTES / 4) {
     const int lo = threadIdx.x * 32;
-    bm[threadIdx.x] = P.n_blocks >= lo + 32 ? 0xffffffffu : P.n_blocks > lo ? (1u << (P.n_blocks - lo)) - 1u : 0u;
+    bm[threadIdx.x] = P.n_pool >= lo + 32 ? 0xffffffffu : P.n_pool > lo ? (1u << (P.n_pool - lo)) - 1u : 0u;
   }
   __syncthreads();
   int e = 0;
