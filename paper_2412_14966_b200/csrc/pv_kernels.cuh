@@ -77,8 +77,7 @@ constexpr int SM_HDR_BYTES = 256;                          // unsigned bm[64]   
 constexpr int SM_MAP = 0;                                  // uint16 map[128]      histogram word -> pool word (0 = NULL word)
 constexpr int SM_TB = SM_MAP + MAX_WORDS * 2;              // uint8 tb[128]        fill: unmapped words of the chunk's windows; peaks: list of the mapped words
 constexpr int SM_MISC = SM_TB + MAX_WORDS;                 // unsigned mapped[4]   words that have a pool word (+ spare)
-constexpr int SM_BLK = SM_MISC + 64;                       // uint16 got[32]       pool words just taken
-constexpr int SM_BINS = SM_BLK + 64;                       // int16 binsm[128]     central bins of the first 128 tracks
+constexpr int SM_BINS = SM_MISC + 64;                      // int16 binsm[128]     central bins of the first 128 tracks
 constexpr int SM_STAGE = SM_BINS + BINS_SM * 2;            // fill:  float zp[64], inv[64]; int lonb[64]
 constexpr int SM_LIST = SM_STAGE + CHUNK * 12;             // fill:  uint16 list[192]
 constexpr int SM_PROTO = SM_STAGE;                         // peaks: uint16 ps[PROTO_CAP]                 (over the stage)
@@ -517,15 +516,13 @@ struct Hist {
   __device__ __forceinline__ int operator[](int b) const { return pool[((int)map[b >> 5] << 5) + (b & 31)]; }
 };
 
-// One pool word for every lane set in `want` (warp-collective): every lane looks at its own two words of the bitmap
-// and takes one free bit, as many lanes as words are still missing, counted from lane `rot` on (every warp and event
-// starts somewhere else, so that the warps of the CTA do not all fight for the same bitmap word); the words taken are
-// handed to the wanting lanes in lane order through got[].  Returns false (nothing kept) when the pool stays dry
-// while this warp holds words (`holding`): the caller gives everything back and starts its event again.  A warp that
-// holds nothing waits.
-__device__ __forceinline__ bool pool_alloc(unsigned* bm, const int nbw, const unsigned want, const int holding, const int rot,
-                                           const int lane, uint16_t* got, int& id) {
-  const int k = __popc(want);
+// k words of the pool into got[0 .. k) (warp-collective): every lane looks at its own two words of the bitmap and
+// takes one free bit per round, as many lanes as words are still missing, counted from lane `rot` on (every warp and
+// event starts somewhere else, so that the warps of the CTA do not all fight for the same bitmap word).  Returns
+// false (nothing kept) when the pool stays dry while this warp holds words (`holding`): the caller gives everything
+// back and starts its event again.  A warp that holds nothing waits.
+__device__ __forceinline__ bool pool_alloc(unsigned* bm, const int nbw, const int k, const int holding, const int rot,
+                                           const int lane, uint16_t* got) {
   const unsigned before = (1u << ((lane - rot) & 31)) - 1u;  // lanes counted before mine, in the rotated order
   int have = 0, spins = 0;
 #pragma unroll 1
@@ -546,15 +543,14 @@ __device__ __forceinline__ bool pool_alloc(unsigned* bm, const int nbw, const un
     if (cand == 0u) {                                        // the pool is dry (a lost race is simply tried again)
       if (holding + have > 0 && ++spins > 32) {              // give back what this call took
         __syncwarp();
-        if (lane < have) { const int w = (int)got[lane] - 1; atomicOr(&bm[w >> 5], 1u << (w & 31)); }
+#pragma unroll 1
+        for (int i = lane; i < have; i += 32) { const int w = (int)got[i] - 1; atomicOr(&bm[w >> 5], 1u << (w & 31)); }
         __syncwarp();
         return false;
       }
       __nanosleep(200);
     }
   }
-  __syncwarp();
-  if ((want >> lane) & 1u) id = got[__popc(want & lanemask_lt())];
   __syncwarp();
   return true;
 }
@@ -565,7 +561,6 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   uint16_t* map = reinterpret_cast<uint16_t*>(wsm + SM_MAP);
   uint8_t* tb = reinterpret_cast<uint8_t*>(wsm + SM_TB);
   unsigned* mapped = reinterpret_cast<unsigned*>(wsm + SM_MISC);   // mapped[c]: words 32 c .. 32 c + 31 that have a pool word
-  uint16_t* got = reinterpret_cast<uint16_t*>(wsm + SM_BLK);
   int16_t* binsm = reinterpret_cast<int16_t*>(wsm + SM_BINS);
   float* st_zp = reinterpret_cast<float*>(wsm + SM_STAGE);
   float* st_inv = st_zp + CHUNK;
@@ -611,17 +606,19 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   const int nbw = (P.n_pool + 31) >> 5;                    // words of the pool bitmap
   int nheld = 0;                                           // pool words of this event (warp-uniform)
   // zero my pool words, unmap them and give them back: leaves the warp's histogram state as it is between events.
-  // Lane l takes the word 32 c + l: sixteen bytes at a time, starting at a different place in every lane.
+  // Lane l takes the word 32 c + l, sixteen bytes at a time.
   auto release = [&]() {
 #pragma unroll 1
     for (int c = 0; c < nwc; ++c) {
-      const bool mine = (mapped[c] >> lane) & 1u;
+      const unsigned mc = mapped[c];
+      if (mc == 0u) continue;
+      const bool mine = (mc >> lane) & 1u;
       int id = 0;
       if (mine) {
         id = map[32 * c + lane];
         int4* q = reinterpret_cast<int4*>(pool + (id << 5));
 #pragma unroll
-        for (int j = 0; j < 8; ++j) q[(j + lane) & 7] = make_int4(0, 0, 0, 0);
+        for (int j = 0; j < 8; ++j) q[j] = make_int4(0, 0, 0, 0);
         map[32 * c + lane] = 0;
       }
       __threadfence_block();                               // the zeros are in place before another warp can take the word
@@ -639,9 +636,10 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   // independent CDF edges (instruction-level parallelism instead of one dependent Horner chain) and UNIT
   // predicated integer adds.  The adds are integers, so the order changes nothing.
   const unsigned pool_s = (unsigned)__cvta_generic_to_shared(pool);
+  int n_raw = 0;
 #pragma unroll 1
-  for (bool filled = false; !filled;) {
-    filled = true;
+  for (;;) {
+    bool filled = true;
 #pragma unroll 1
     for (int c0 = 0; c0 < n; c0 += CHUNK) {
       float lx[SLOTS], ly[SLOTS], lz[SLOTS], ltx[SLOTS], lty[SLOTS], lvx[SLOTS];
@@ -696,18 +694,29 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         myunits += nun[s];
       }
       __syncwarp();
-      // ---- words met for the first time get a pool word
+      // ---- words met for the first time get a pool word (the unit list, not yet built, takes the words from the pool)
       if (__any_sync(FULL, sawnew)) {
-#pragma unroll 1
-        for (int c = 0; c < nwc; ++c) {
-          const int f = tb[32 * c + lane];
-          const unsigned newm = __ballot_sync(FULL, f != 0);
-          if (newm == 0u) continue;
-          int id = 0;
-          if (!pool_alloc(bm, nbw, newm, nheld, (e * 7 + c0 + 8 * c) & 31, lane, got, id)) { filled = false; break; }   // pool dry: start again
-          if (f) { tb[32 * c + lane] = 0; map[32 * c + lane] = (uint16_t)id; }
-          nheld += __popc(newm);
-          if (lane == 0) mapped[c] |= newm;
+        unsigned nm[4];
+        int k = 0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          nm[c] = __ballot_sync(FULL, c < nwc && tb[32 * c + lane] != 0);
+          k += __popc(nm[c]);
+        }
+        if (!pool_alloc(bm, nbw, k, nheld, (e * 7 + c0) & 31, lane, list)) filled = false;   // pool dry: start again
+        else {
+          int base = 0;
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            if (nm[c] == 0u) continue;
+            if ((nm[c] >> lane) & 1u) {
+              map[32 * c + lane] = list[base + __popc(nm[c] & lanemask_lt())];
+              tb[32 * c + lane] = 0;
+            }
+            base += __popc(nm[c]);
+            if (lane == 0) mapped[c] |= nm[c];
+          }
+          nheld += k;
         }
         __syncwarp();
       }
@@ -763,25 +772,19 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       }
       __syncwarp();                                        // the next chunk overwrites the stage
     }
-    if (!filled) {                                         // the pool ran dry: back off and start the event again
-      reinterpret_cast<unsigned*>(tb)[lane] = 0u;
-      __syncwarp();
-      release();
-      __nanosleep(2000);
-    }
-  }
-  __syncwarp();
+    if (!filled) reinterpret_cast<unsigned*>(tb)[lane] = 0u;
+    __syncwarp();
+    if (filled) {
 
   if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
     for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
 
   // ================= a3: peak search and seed position (Eq. 4-5) ==============================
   // The mapped words, ascending, are the only ones that can hold bins above the threshold.  One LANE per mapped word
-  // reads its 32 bins (sixteen bytes at a time, starting at a different place in every lane) into a bit mask of the
+  // reads its 32 bins (sixteen bytes at a time) into a bit mask of the
   // bins above threshold; the first bin of every run (proto-cluster) follows from the mask and the top bit of the
   // word before.  Then one lane per proto-cluster runs the z-ordered hysteresis sweep (select-based state machine: the
   // serial length is the longest proto-cluster).
-  int n_raw = 0;
   {
     uint8_t* twl = tb;                                     // list of the mapped words (the flags of the fill are all zero now)
     int ntw = 0;
@@ -803,10 +806,9 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
         const int4* q = reinterpret_cast<const int4*>(pool + ((int)map[w] << 5));   // bins beyond nbins are padding and stay 0
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          const int g = (j + lane) & 7;
-          const int4 v = q[g];
+          const int4 v = q[j];
           const unsigned nib = (v.x > P.T_bin ? 1u : 0u) | (v.y > P.T_bin ? 2u : 0u) | (v.z > P.T_bin ? 4u : 0u) | (v.w > P.T_bin ? 8u : 0u);
-          m |= nib << (4 * g);
+          m |= nib << (4 * j);
         }
       }
       unsigned pm = __shfl_up_sync(FULL, m, 1);
@@ -863,9 +865,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     }
     reinterpret_cast<unsigned*>(tb)[lane] = 0u;            // the flags of the next fill start at zero
   }
-  int ns = n_raw;
-  if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
-  if (lane < ns) {                                         // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
+  if (lane < min(n_raw, P.max_vtx)) {                      // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
     const int i = sp[lane];
     const long long Nm = i > 0 ? H[i - 1] : 0;
     const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
@@ -875,8 +875,13 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
     zs[lane] = __fmaf_rn(delta, P.dz, zi);
   }
-  __syncwarp();
-  release();                                               // the histogram is dead from here on
+    }                                                      // if (filled)
+    __syncwarp();
+    release();                                             // the histogram is dead from here on
+    if (filled) break;
+    __nanosleep(2000);                                     // the pool ran dry: back off and start the event again
+    n_raw = 0;
+  }
   {
     // pull the first chunk of my NEXT event (lane 0 holds its index) into L2 while this one is associated
     const int ne = __shfl_sync(FULL, nxt, 0);
@@ -892,6 +897,8 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     }
   }
 
+  int ns = n_raw;
+  if (ns > P.max_vtx) { ns = P.max_vtx; status |= PV_EVT_VTX_OVERFLOW; }   // R-8: first max_vtx in z kept
   auto load_raw = [&](const int i) {
     const int g = t0 + min(i, n - 1);
     RawTrk Q;
