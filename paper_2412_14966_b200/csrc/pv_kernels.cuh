@@ -36,7 +36,13 @@ namespace pvk {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
-constexpr int SEED_WARPS = 32;      // warps per CTA of seed_kernel = events in flight per SM (one warp per event)
+#ifndef PV_PREFETCH_TRACKS
+#define PV_PREFETCH_TRACKS 128    // tracks of a warp's next event pulled into L2 while the current one is associated
+#endif
+#ifndef PV_SEED_WARPS
+#define PV_SEED_WARPS 32
+#endif
+constexpr int SEED_WARPS = PV_SEED_WARPS;      // warps per CTA of seed_kernel = events in flight per SM (one warp per event)
 constexpr int CHUNK = 64;           // tracks per fill chunk
 constexpr int SLOTS = CHUNK / 32;   // tracks per lane and chunk
 #ifndef PV_FIT_UNROLL
@@ -883,11 +889,11 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     n_raw = 0;
   }
   {
-    // pull the first chunk of my NEXT event (lane 0 holds its index) into L2 while this one is associated
+    // pull the first tracks of my NEXT event (lane 0 holds its index) into L2 while this one is associated
     const int ne = __shfl_sync(FULL, nxt, 0);
     if (ne < A.n_events) {
       const int pt0 = __ldg(A.offsets + ne);
-      const int pn = min(__ldg(A.offsets + ne + 1) - pt0, CHUNK);
+      const int pn = min(__ldg(A.offsets + ne + 1) - pt0, PV_PREFETCH_TRACKS);
       if (lane * 32 < pn + 32) {                           // one 128-byte line per lane and array
         const size_t o = (size_t)pt0 + lane * 32;
         const float* arr[9] = {A.x, A.y, A.z, A.tx, A.ty, A.var_x, A.var_y, A.var_tx, A.var_ty};
