@@ -2,12 +2,13 @@
 //
 // Three kernels per pv_find call:
 //
-//   seed_kernel     a1..a4  one TEAM of two warps per event, persistent grid, 14 teams per CTA, one int32
-//                           shared-memory histogram and one named barrier per team.  POCA projection (fp32 contract,
-//                           bit-exact with the CPU oracle), flat list of 6-bin fill units (seven independent CDF edges
-//                           per thread), touched-word flags, one ballot per touched word for the proto-cluster starts,
-//                           one lane per proto-cluster for the z-ordered hysteresis sweep, seed positions,
-//                           association (explicit with the removal loop, or the multi-vertex chi2 window),
+//   seed_kernel     a1..a4  ONE WARP per event, persistent grid, 32 warps (events in flight) per SM, no CTA barrier.
+//                           Sparse int32 histograms: the words (32 bins) an event touches are taken from a pool in
+//                           shared memory shared by the CTA (bitmap allocator, word map per warp).  POCA projection
+//                           (fp32 contract, bit-exact with the CPU oracle), flat list of 6-bin fill units (seven
+//                           independent CDF edges per lane, predicated integer adds), one lane per mapped word for the
+//                           proto-cluster starts, one lane per proto-cluster for the z-ordered hysteresis sweep, seed
+//                           positions, association (explicit with the removal loop, or the multi-vertex chi2 window),
 //                           deterministic counting sort -> seed records and fit-ready track records in HBM.
 //   fit_kernel      a5      flat over all seeds of the batch (no histogram): a warp counting-sorts a window of seed
 //                           records and works through it as a queue, 2 / 4 / ... 32 lanes per seed, tracks staged by
@@ -21,7 +22,9 @@
 //   ip_kernel       NEXT-4  impact parameter / IP chi2 of every track w.r.t. the PVs of its event (pv_track_ip).
 //
 // The v1 single fused kernel (profiles/r1_v1_fused_kernel.md) was 87 KB of SASS and lost 42 % of its issue
-// slots to instruction-cache misses with 14 warps per SM in different phases; each kernel here is small.
+// slots to instruction-cache misses with 14 warps per SM in different phases; each kernel here is smaller.
+// Until round 2 the seed kernel gave every event a TEAM of two warps and a dense 13.6 KB histogram (14 events in
+// flight per SM, a fifth of the warp time spent at team barriers): profiles/r2_kernels.md has both.
 // This file shares nothing with oracle/ (the frozen CDF coefficients below are the numbers of
 // DESIGN.md section 3, restated).
 #pragma once
