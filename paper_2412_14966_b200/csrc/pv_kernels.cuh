@@ -39,6 +39,12 @@ namespace pvk {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
+#ifndef PV_DET_UNROLL
+#define PV_DET_UNROLL 2
+#endif
+// unroll of the loop that reads a histogram word 16 bytes at a time (a3); measured on configs[1]: 8 (all) 0.632 ms,
+// 2 0.620 ms: the kernel is short of issue slots and of instruction cache there, not of parallelism
+constexpr int DET_UNROLL = PV_DET_UNROLL;
 #ifndef PV_PREFETCH_TRACKS
 #define PV_PREFETCH_TRACKS 128    // tracks of a warp's next event pulled into L2 while the current one is associated
 #endif
@@ -813,7 +819,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
       unsigned m = 0u;
       if (lane < step) {
         const int4* q = reinterpret_cast<const int4*>(pool + ((int)map[w] << 5));   // bins beyond nbins are padding and stay 0
-#pragma unroll
+#pragma unroll DET_UNROLL
         for (int j = 0; j < 8; ++j) {
           const int4 v = q[j];
           const unsigned nib = (v.x > P.T_bin ? 1u : 0u) | (v.y > P.T_bin ? 2u : 0u) | (v.z > P.T_bin ? 4u : 0u) | (v.w > P.T_bin ? 8u : 0u);
