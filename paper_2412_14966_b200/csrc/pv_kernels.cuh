@@ -194,8 +194,8 @@ __device__ __forceinline__ int cdf_bits(float s) {
   return __float_as_int(__fadd_rn(c, 8.0f));
 }
 
-// integer add to a shared-memory bin (byte address in the shared window) unless the addend is zero, as ONE predicated
-// instruction: `if (d != 0) atomicAdd(...)` compiles to a branch with a convergence barrier around every add
+// integer add to a shared-memory bin (byte address in the shared window) unless the addend is zero (ptxas turns the
+// predicate into a branch; adding the zeros as well, without any test, was measured slower: 0.630 against 0.620 ms)
 __device__ __forceinline__ void red_add_nz(unsigned saddr, int d) {
   asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %1, 0;\n\t@q red.shared.add.s32 [%0], %1;\n\t}" ::"r"(saddr), "r"(d) : "memory");
 }
