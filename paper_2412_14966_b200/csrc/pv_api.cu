@@ -274,7 +274,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   CK(cudaMemsetAsync(workspace, 0, 64, stream));
   // a1..a4: persistent, one CTA per SM, one warp per event
   int grid = di->sms;
-  const int need = (n_events + warps - 1) / warps;
+  const int need = n_events;                                  // a small batch is spread over the SMs, not packed into few CTAs
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
   if (tfl) {                                                  // the table of template histograms, ~10^4 entries

@@ -987,7 +987,7 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
           const float oth = fmaxf(den - __expf(-0.5f * chi2_at(R, cx, cy, k)), 0.5f * P.mv_e0);
           float4* o = A.ftrk + 2 * (size_t)(cur[k] + rank);
           o[0] = make_float4(T.x0, T.y0, T.tx, T.ty);
-          o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), oth);
+          o[1] = make_float4(T.Wx, T.Wy, __int_as_float(t0 + i), oth);   // (streaming stores were measured: no difference)
         }
         __syncwarp();
         if (k >= 0 && rank == 0) cur[k] += __popc(peers);
