@@ -39,6 +39,10 @@ namespace pvk {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int MAX_TRK = PV_MAX_TRACKS_PER_EVENT;
 constexpr int MAXV = PV_MAX_VTX;
+#ifndef PV_MV_KEEP
+#define PV_MV_KEEP 4
+#endif
+constexpr int MV_KEEP = PV_MV_KEEP;   // multi-vertex association: groups of 32 tracks whose candidate masks stay in registers between its two passes
 #ifndef PV_DET_UNROLL
 #define PV_DET_UNROLL 2
 #endif
@@ -997,20 +1001,22 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     // records at the counted places.  ONE loop body serves both passes (the candidate and record code exists once: the
     // kernel stays small enough for the instruction cache); the masks and denominators of the first MV_KEEP * 32 tracks
     // are kept in registers from pass 0 to pass 1, the others are computed again.
-    unsigned hm0 = 0u, hm1 = 0u;
-    float hd0 = 0.0f, hd1 = 0.0f;
+    unsigned hm0 = 0u, hm1 = 0u, hm2 = 0u, hm3 = 0u;
+    float hd0 = 0.0f, hd1 = 0.0f, hd2 = 0.0f, hd3 = 0.0f;
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
 #pragma unroll 1
       for (int it = 0, i0 = 0; i0 < n; ++it, i0 += 32) {
         const int i = i0 + lane;
         const RawTrk Q = load_raw(i);
-        unsigned mk = it == 0 ? hm0 : hm1;
-        float dn = it == 0 ? hd0 : hd1;
-        if (pass == 0 || it >= 2) cand(i, Q, mk, dn);
+        unsigned mk = it == 0 ? hm0 : it == 1 ? hm1 : it == 2 ? hm2 : hm3;
+        float dn = it == 0 ? hd0 : it == 1 ? hd1 : it == 2 ? hd2 : hd3;
+        if (pass == 0 || it >= MV_KEEP) cand(i, Q, mk, dn);
         if (pass == 0) {
           if (it == 0) { hm0 = mk; hd0 = dn; }
           else if (it == 1) { hm1 = mk; hd1 = dn; }
+          else if (it == 2) { hm2 = mk; hd2 = dn; }
+          else if (it == 3) { hm3 = mk; hd3 = dn; }
           for_bits(mk, count);
         } else {
           emit(i, Q, mk, dn);
