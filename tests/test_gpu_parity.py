@@ -386,7 +386,7 @@ def test_runs_are_reproducible(pv, cfg0):
 @pytest.mark.parametrize("mode", ["explicit", "multivertex", "recursive"])
 def test_repeated_runs_are_bit_identical_on_high_pileup(pv, mode):
     """Five launches over 3000 high pile-up events (multi-chunk events, many seeds, big-seed fit path): every output
-    bit-identical -- a race in the team protocol or an order-dependent sum would show up here."""
+    bit-identical -- a race in the shared-memory pool or an order-dependent sum would show up here."""
     data = events.generate(events.config(2, 3000))
     p = {"explicit": pv.default_params, "multivertex": pv.multivertex_params,
          "recursive": lambda: pv.default_params(split_mode=1)}[mode]()
