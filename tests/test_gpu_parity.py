@@ -163,35 +163,81 @@ def test_wide_tracks_many_fill_units(pv, oracle):
 
 
 def test_many_proto_clusters_slow_path(pv, oracle):
-    """A comb of 580 isolated narrow tracks 1 mm apart (one proto-cluster each, none with the integral of a seed)
-    plus a few real vertices: more proto-cluster starts than one warp's list holds, so the peak search takes its
-    round-based path; seeds must still come out z-ordered and bit-exact."""
+    """Combs of isolated narrow tracks (one proto-cluster each, none with the integral of a seed) plus a few real
+    vertices.  Event 0 and 2: 580 tracks 1 mm apart (8 runs per histogram word).  Event 3: 400 tracks 0.5 mm apart, each
+    in the middle of its bin (16 runs per word, the most a word can start): more than 256 proto-cluster starts in one
+    pass of 32 words, so the peak search falls back to passes of 16 words; seeds must still come out z-ordered and
+    bit-exact."""
     rng = np.random.default_rng(7)
-    zc = np.arange(-290.0, 290.0, 1.0)
     pv_z = np.array([-250.3, -100.1, 10.2, 150.4, 280.6])
-    z = np.concatenate([zc, np.repeat(pv_z, 8)]).astype(np.float32)
-    n = z.size
-    phi = rng.uniform(0, 2 * np.pi, n)
-    sl = 0.3
-    ev = dict(x=rng.normal(0, 0.01, n).astype(np.float32), y=rng.normal(0, 0.01, n).astype(np.float32), z=z,
-              tx=(sl * np.cos(phi)).astype(np.float32), ty=(sl * np.sin(phi)).astype(np.float32),
-              var_x=np.full(n, 1e-4, np.float32), var_y=np.full(n, 1e-4, np.float32),
-              var_tx=np.full(n, 1e-6, np.float32), var_ty=np.full(n, 1e-6, np.float32))
-    perm = rng.permutation(n)
-    ev = {k: v[perm] for k, v in ev.items()}
+
+    def comb(zc):
+        z = np.concatenate([zc, np.repeat(pv_z, 8)]).astype(np.float32)
+        n = z.size
+        phi = rng.uniform(0, 2 * np.pi, n)
+        sl = 0.3
+        ev = dict(x=rng.normal(0, 0.01, n).astype(np.float32), y=rng.normal(0, 0.01, n).astype(np.float32), z=z,
+                  tx=(sl * np.cos(phi)).astype(np.float32), ty=(sl * np.sin(phi)).astype(np.float32),
+                  var_x=np.full(n, 1e-4, np.float32), var_y=np.full(n, 1e-4, np.float32),
+                  var_tx=np.full(n, 1e-6, np.float32), var_ty=np.full(n, 1e-6, np.float32))
+        perm = rng.permutation(n)
+        return {k: v[perm] for k, v in ev.items()}
+    ev = comb(np.arange(-290.0, 290.0, 1.0))
+    dense = comb(-80.0 + 0.125 + 0.5 * np.arange(400))
+    # exact positions for the dense comb: on the beamline, so that z_poca is the state's z and stays inside its bin
+    dense["x"][:] = 0.0
+    dense["y"][:] = 0.0
     small = events.generate(events.config(0, 2))
     so = small["offsets"]
-    data = events.from_lists([ev, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, ev])
+    data = events.from_lists([ev, {k: small[k][so[0]:so[1]] for k in events.FIELDS}, ev, dense])
     got, ref, rep = _both(pv, oracle, data)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
     _assert_parity(rep)
-    H = ref["debug"]["hist"][0]
-    above = H > int(0.25 * (1 << 20))
-    starts = above & ~np.concatenate([[False], above[:-1]])
-    words = np.flatnonzero(H.reshape(-1, 1)[: (H.size // 32) * 32].reshape(-1, 32).any(axis=1))
-    half = words[(len(words) + 1) // 2 - 1]
-    assert starts[: (half + 1) * 32].sum() > 256                   # the first warp's list overflows
-    assert ref["n_vtx"][0] == 5 and got["n_vtx"][0] == 5 and got["n_vtx"][2] == 5
+
+    def most_starts_in_32_words(H):
+        above = H > int(0.25 * (1 << 20))
+        starts = above & ~np.concatenate([[False], above[:-1]])
+        per_word = starts[: (H.size // 32) * 32].reshape(-1, 32).sum(axis=1)
+        touched = np.flatnonzero(H[: (H.size // 32) * 32].reshape(-1, 32).any(axis=1))
+        return max(per_word[touched[i:i + 32]].sum() for i in range(0, len(touched), 32))
+    assert most_starts_in_32_words(ref["debug"]["hist"][0]) >= 250
+    assert most_starts_in_32_words(ref["debug"]["hist"][3]) > 256      # the list of one pass overflows
+    assert ref["n_vtx"][0] == 5 and got["n_vtx"][0] == 5 and got["n_vtx"][2] == 5 and got["n_vtx"][3] == ref["n_vtx"][3]
+
+
+def test_histogram_pool_runs_dry(pv, oracle):
+    """The seed kernel takes the histogram words an event touches from a pool shared by the 32 warps of an SM (1333
+    words).  Here every event spreads 136 isolated tracks over the whole z range (about 100 of its 107 words touched; 32 such
+    events want twice the pool), in a batch large enough to keep every warp of the GPU busy: warps wait for words, and
+    warps that hold words while the pool is dry give them back and start their event again.  The results must not
+    show any of it: bit-exact against the oracle, and bit-identical from run to run."""
+    rng = np.random.default_rng(23)
+    E, n = 6000, 160
+    # 136 isolated tracks on a jittered grid of 6.17 mm (one proto-cluster each, none a seed) + two real vertices
+    z = (-545.0 + 6.17 * np.arange(n)[None, :] + rng.uniform(-1.0, 1.0, (E, n))).astype(np.float32)
+    z[:, :24] = np.repeat(rng.uniform(-100.0, 100.0, (E, 2)), 12, axis=1)
+    z = rng.permuted(z, axis=1)
+    phi = rng.uniform(0, 2 * np.pi, (E, n))
+    sl = rng.uniform(0.1, 0.4, (E, n))
+    sig = rng.uniform(0.01, 0.05, (E, n)).astype(np.float32)
+    arr = dict(x=(sig * rng.normal(0, 1, (E, n))).astype(np.float32), y=(sig * rng.normal(0, 1, (E, n))).astype(np.float32), z=z,
+               tx=(sl * np.cos(phi)).astype(np.float32), ty=(sl * np.sin(phi)).astype(np.float32),
+               var_x=sig * sig, var_y=sig * sig, var_tx=np.full((E, n), 1e-6, np.float32), var_ty=np.full((E, n), 1e-6, np.float32))
+    data = {k: v.reshape(-1) for k, v in arr.items()}
+    data["offsets"] = (np.arange(E + 1) * n).astype(np.int32)
+    data["n_events"] = E
+    got, ref, rep = _both(pv, oracle, data, n_hist=400)
+    print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
+    _assert_parity(rep)
+    H = ref["debug"]["hist"][:400]
+    words = (H[:, : (H.shape[1] // 32) * 32].reshape(400, -1, 32) != 0).any(axis=2).sum(axis=1)
+    assert words.mean() > 70 and words.mean() * 32 > 1.5 * 1333, words.mean()
+    assert rep["hist_mismatch"] == 0 and rep["seed_z_mismatch"] == 0 and rep["trk_seed_mismatch"] == 0
+    assert (ref["n_vtx"] >= 1).mean() > 0.9
+    again = pv.find(data, pv.default_params(), debug=True, n_hist_events=400)
+    for k in ("vtx_pos", "vtx_cov", "n_vtx", "trk_vertex", "trk_weight", "event_status"):
+        assert np.array_equal(got[k], again[k]), k
+    assert np.array_equal(got["debug"]["hist"], again["debug"]["hist"])
 
 
 @pytest.mark.parametrize("n", [1000, 10000])
