@@ -287,7 +287,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   }
   CK(cudaGetLastError());
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
-  // a5: FIT_G lanes per seed, teams stride over windows of 32 seed records
+  // a5: autonomous warps work through windows of seed records
   {
     long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm[mvf];
     const long long most = ((long long)n_events * params->max_vtx_per_event + pvk::FIT_BLOCK - 1) / pvk::FIT_BLOCK;

@@ -794,106 +794,105 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     if (!filled) reinterpret_cast<unsigned*>(tb)[lane] = 0u;
     __syncwarp();
     if (filled) {
+      if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
+        for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
 
-  if (DBG && A.dbg.hist && e < A.dbg.n_hist_events)
-    for (int b = lane; b < P.nbins; b += 32) A.dbg.hist[(size_t)e * P.nbins + b] = H[b];
-
-  // ================= a3: peak search and seed position (Eq. 4-5) ==============================
-  // The mapped words, ascending, are the only ones that can hold bins above the threshold.  One LANE per mapped word
-  // reads its 32 bins (sixteen bytes at a time) into a bit mask of the
-  // bins above threshold; the first bin of every run (proto-cluster) follows from the mask and the top bit of the
-  // word before.  Then one lane per proto-cluster runs the z-ordered hysteresis sweep (select-based state machine: the
-  // serial length is the longest proto-cluster).
-  {
-    uint8_t* twl = tb;                                     // list of the mapped words (the flags of the fill are all zero now)
-    int ntw = 0;
-#pragma unroll 1
-    for (int c = 0; c < nwc; ++c) {
-      const unsigned mc = mapped[c];
-      if ((mc >> lane) & 1u) twl[ntw + __popc(mc & lanemask_lt())] = (uint8_t)(32 * c + lane);
-      ntw += __popc(mc);
-    }
-    __syncwarp();
-    int carry_w = -2;                                      // last word of the pass before and its mask
-    unsigned carry_m = 0u;
-#pragma unroll 1
-    for (int r0 = 0; r0 < ntw;) {
-      int step = min(32, ntw - r0);
-      const int w = lane < step ? (int)twl[r0 + lane] : -5;
-      unsigned m = 0u;
-      if (lane < step) {
-        const int4* q = reinterpret_cast<const int4*>(pool + ((int)map[w] << 5));   // bins beyond nbins are padding and stay 0
-#pragma unroll DET_UNROLL
-        for (int j = 0; j < 8; ++j) {
-          const int4 v = q[j];
-          const unsigned nib = (v.x > P.T_bin ? 1u : 0u) | (v.y > P.T_bin ? 2u : 0u) | (v.z > P.T_bin ? 4u : 0u) | (v.w > P.T_bin ? 8u : 0u);
-          m |= nib << (4 * j);
-        }
-      }
-      unsigned pm = __shfl_up_sync(FULL, m, 1);
-      int pw = __shfl_up_sync(FULL, w, 1);
-      if (lane == 0) { pm = carry_m; pw = carry_w; }
-      const unsigned carry = (pw == w - 1) ? pm >> 31 : 0u;
-      unsigned starts = m & ~((m << 1) | carry);           // first bin of each run of bins above threshold
-      int c = __popc(starts);
-      int inc = warp_incl_scan(c, lane);
-      if (__shfl_sync(FULL, inc, 31) > PROTO_CAP) {        // never with physical histograms: a word starts at most 16 runs
-        step = min(step, PROTO_CAP / 16);
-        if (lane >= step) { c = 0; starts = 0u; }
-        inc = warp_incl_scan(c, lane);
-      }
-      const int np = __shfl_sync(FULL, inc, 31);
+      // ================= a3: peak search and seed position (Eq. 4-5) ==============================
+      // The mapped words, ascending, are the only ones that can hold bins above the threshold.  One LANE per mapped
+      // word reads its 32 bins (sixteen bytes at a time) into a bit mask of the bins above threshold; the first bin
+      // of every run (proto-cluster) follows from the mask and the top bit of the word before.  Then one lane per
+      // proto-cluster runs the z-ordered hysteresis sweep (select-based state machine: the serial length is the
+      // longest proto-cluster).
       {
-        int o = inc - c;
+        uint8_t* twl = tb;                                 // list of the mapped words (the fill's flags are all zero now)
+        int ntw = 0;
 #pragma unroll 1
-        while (starts) {
-          ps[o++] = (uint16_t)(32 * w + __ffs(starts) - 1);
-          starts &= starts - 1u;
+        for (int c = 0; c < nwc; ++c) {
+          const unsigned mc = mapped[c];
+          if ((mc >> lane) & 1u) twl[ntw + __popc(mc & lanemask_lt())] = (uint8_t)(32 * c + lane);
+          ntw += __popc(mc);
         }
-      }
-      carry_w = __shfl_sync(FULL, w, step - 1);
-      carry_m = __shfl_sync(FULL, m, step - 1);
-      r0 += step;
-      __syncwarp();
+        __syncwarp();
+        int carry_w = -2;                                      // last word of the pass before and its mask
+        unsigned carry_m = 0u;
 #pragma unroll 1
-      for (int p0 = 0; p0 < np; p0 += 32) {                // one lane per proto-cluster
-        const int p = p0 + lane;
-        const bool act = p < np;
-        const int b0 = act ? (int)ps[p] : 0;
-        Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
-        int cl = 0, base = 0;
+        for (int r0 = 0; r0 < ntw;) {
+          int step = min(32, ntw - r0);
+          const int w = lane < step ? (int)twl[r0 + lane] : -5;
+          unsigned m = 0u;
+          if (lane < step) {
+            const int4* q = reinterpret_cast<const int4*>(pool + ((int)map[w] << 5));   // bins beyond nbins are padding and stay 0
+#pragma unroll DET_UNROLL
+            for (int j = 0; j < 8; ++j) {
+              const int4 v = q[j];
+              const unsigned nib = (v.x > P.T_bin ? 1u : 0u) | (v.y > P.T_bin ? 2u : 0u) | (v.z > P.T_bin ? 4u : 0u) | (v.w > P.T_bin ? 8u : 0u);
+              m |= nib << (4 * j);
+            }
+          }
+          unsigned pm = __shfl_up_sync(FULL, m, 1);
+          int pw = __shfl_up_sync(FULL, w, 1);
+          if (lane == 0) { pm = carry_m; pw = carry_w; }
+          const unsigned carry = (pw == w - 1) ? pm >> 31 : 0u;
+          unsigned starts = m & ~((m << 1) | carry);           // first bin of each run of bins above threshold
+          int c = __popc(starts);
+          int inc = warp_incl_scan(c, lane);
+          if (__shfl_sync(FULL, inc, 31) > PROTO_CAP) {        // never with physical histograms: a word starts at most 16 runs
+            step = min(step, PROTO_CAP / 16);
+            if (lane >= step) { c = 0; starts = 0u; }
+            inc = warp_incl_scan(c, lane);
+          }
+          const int np = __shfl_sync(FULL, inc, 31);
+          {
+            int o = inc - c;
 #pragma unroll 1
-        for (int rep = 0; rep < 2; ++rep) {                // rep 1 (rare): proto-clusters with three or more seeds
-          const bool run = act && (rep == 0 || (cl > 2 && base + 2 < P.max_vtx));
-          if (!__any_sync(FULL, run)) break;
-          if (run) {
-            const int cc = SPLIT ? split_x86(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1)
-                                 : sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
-            if (rep == 0) cl = cc;
+            while (starts) {
+              ps[o++] = (uint16_t)(32 * w + __ffs(starts) - 1);
+              starts &= starts - 1u;
+            }
           }
-          if (rep == 0) {
-            const int inc2 = warp_incl_scan(cl, lane);
-            base = n_raw + inc2 - cl;
-            if (cl > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
-            if (cl > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
-            n_raw += __shfl_sync(FULL, inc2, 31);
+          carry_w = __shfl_sync(FULL, w, step - 1);
+          carry_m = __shfl_sync(FULL, m, step - 1);
+          r0 += step;
+          __syncwarp();
+#pragma unroll 1
+          for (int p0 = 0; p0 < np; p0 += 32) {                // one lane per proto-cluster
+            const int p = p0 + lane;
+            const bool act = p < np;
+            const int b0 = act ? (int)ps[p] : 0;
+            Cl c0 = {0, 0, 0}, c1 = {0, 0, 0};
+            int cl = 0, base = 0;
+#pragma unroll 1
+            for (int rep = 0; rep < 2; ++rep) {                // rep 1 (rare): proto-clusters with three or more seeds
+              const bool run = act && (rep == 0 || (cl > 2 && base + 2 < P.max_vtx));
+              if (!__any_sync(FULL, run)) break;
+              if (run) {
+                const int cc = SPLIT ? split_x86(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1)
+                                     : sweep(H, b0, P, rep ? base : -1, sb, se, sp, c0, c1);
+                if (rep == 0) cl = cc;
+              }
+              if (rep == 0) {
+                const int inc2 = warp_incl_scan(cl, lane);
+                base = n_raw + inc2 - cl;
+                if (cl > 0 && base < P.max_vtx) { sb[base] = c0.b; se[base] = c0.e; sp[base] = c0.p; }
+                if (cl > 1 && base + 1 < P.max_vtx) { sb[base + 1] = c1.b; se[base + 1] = c1.e; sp[base + 1] = c1.p; }
+                n_raw += __shfl_sync(FULL, inc2, 31);
+              }
+            }
           }
+          __syncwarp();
         }
+        reinterpret_cast<unsigned*>(tb)[lane] = 0u;            // the flags of the next fill start at zero
       }
-      __syncwarp();
-    }
-    reinterpret_cast<unsigned*>(tb)[lane] = 0u;            // the flags of the next fill start at zero
-  }
-  if (lane < min(n_raw, P.max_vtx)) {                      // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
-    const int i = sp[lane];
-    const long long Nm = i > 0 ? H[i - 1] : 0;
-    const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
-    const long long N0 = H[i];
-    const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
-    const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
-    const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
-    zs[lane] = __fmaf_rn(delta, P.dz, zi);
-  }
+      if (lane < min(n_raw, P.max_vtx)) {                      // Eq. 4-5: neighbours are raw bins, 0 beyond the ends
+        const int i = sp[lane];
+        const long long Nm = i > 0 ? H[i - 1] : 0;
+        const long long Np = i < P.nbins - 1 ? H[i + 1] : 0;
+        const long long N0 = H[i];
+        const long long num = Np - Nm, den = 2 * N0 - Np - Nm;
+        const float delta = den > 0 ? __fmul_rn(0.5f, __fdiv_rn((float)num, (float)den)) : 0.0f;
+        const float zi = __fmaf_rn(__fadd_rn((float)i, 0.5f), P.dz, P.z_min);
+        zs[lane] = __fmaf_rn(delta, P.dz, zi);
+      }
     }                                                      // if (filled)
     __syncwarp();
     release();                                             // the histogram is dead from here on
