@@ -1673,10 +1673,14 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   int sv[4];                                               // seed index of my first four tracks: loads issued now,
 #pragma unroll                                             // consumed after the vertex sweep
   for (int q = 0; q < 4; ++q) sv[q] = (lane + 32 * q < n) ? A.trk_vertex[t0 + lane + 32 * q] : -1;
-  float wv[4] = {0.0f, 0.0f, 0.0f, 0.0f};                  // explicit flavour: the weight the fit left at the track's record
+  // explicit flavour: the weight the fit left at the track's record.  The records of an event are the event's own
+  // range of wrec[]: its first 128 weights are loaded in order, together with the seed indices (not behind them), and
+  // picked from shared memory afterwards: two dependent levels of loads instead of three.
+  __shared__ float s_w[8][128];
+  float wl[4] = {0.0f, 0.0f, 0.0f, 0.0f};
   if (FLAV != PV_FLAVOUR_MULTIVERTEX) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) wv[q] = sv[q] >= 0 ? A.wrec[t0 + (sv[q] >> 5)] : 0.0f;
+    for (int q = 0; q < 4; ++q) wl[q] = (lane + 32 * q < n) ? A.wrec[t0 + lane + 32 * q] : 0.0f;
   }
   unsigned long long bv[4] = {0ull, 0ull, 0ull, 0ull};     // multi-vertex flavour: largest weight << 32 | 31 - seed
   if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
@@ -1686,15 +1690,25 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   float vp[3] = {0.0f, 0.0f, 0.0f}, vc[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
   float vchi2 = 0.0f;
   int vntrk = 0, vniter = -1;
-  if (lane < ns) {
+  if (lane < ns) {                                         // (a slot the fit never wrote holds niter = -1 and is not used)
     const size_t o = ev + lane;
     vniter = A.vtx_niter[o];
-    if (vniter >= 0) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) vp[c] = A.vtx_pos[o * 3 + c];
+    for (int c = 0; c < 3; ++c) vp[c] = A.vtx_pos[o * 3 + c];
 #pragma unroll
-      for (int c = 0; c < 6; ++c) vc[c] = A.vtx_cov[o * 6 + c];
-      vchi2 = A.vtx_chi2[o]; vntrk = A.vtx_ntracks[o];
+    for (int c = 0; c < 6; ++c) vc[c] = A.vtx_cov[o * 6 + c];
+    vchi2 = A.vtx_chi2[o]; vntrk = A.vtx_ntracks[o];
+  }
+  float wv[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  if (FLAV != PV_FLAVOUR_MULTIVERTEX) {
+    const int warp = (threadIdx.x >> 5) & 7;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) s_w[warp][lane + 32 * q] = wl[q];
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int r = sv[q] >> 5;                              // position of the track's record within the event
+      wv[q] = sv[q] < 0 ? 0.0f : (r < 128 ? s_w[warp][r] : A.wrec[t0 + r]);
     }
   }
   const unsigned alive = __ballot_sync(FULL, lane < ns && vniter >= 0);
