@@ -198,6 +198,29 @@ __device__ __forceinline__ int cdf_bits(float s) {
   return __float_as_int(__fadd_rn(c, 8.0f));
 }
 
+// Two edges at once with the packed fp32 instructions of sm_100 (FFMA2 / FADD2 / FMUL2: two IEEE fp32 operations, each
+// rounded once, in one issue slot): bit for bit the results of edge_r, for half the instructions of the Horner chains.
+__device__ __forceinline__ void edge_r2(float kf0, float kf1, float zp, float inv, const KParams& P, int& r0, int& r1) {
+  const float2 e = __ffma2_rn(make_float2(kf0, kf1), make_float2(P.dz, P.dz), make_float2(P.z_min, P.z_min));
+  float2 s = __fmul2_rn(__fadd2_rn(e, make_float2(-zp, -zp)), make_float2(inv, inv));
+  s.x = fminf(fmaxf(s.x, -1.0f), 1.0f);
+  s.y = fminf(fmaxf(s.y, -1.0f), 1.0f);
+  const float2 t = __fmul2_rn(s, s);
+  float2 g = make_float2(0x1.3e0392p-3f, 0x1.3e0392p-3f);
+  g = __ffma2_rn(g, t, make_float2(-0x1.862240p-1f, -0x1.862240p-1f));
+  g = __ffma2_rn(g, t, make_float2(0x1.b67296p+0f, 0x1.b67296p+0f));
+  g = __ffma2_rn(g, t, make_float2(-0x1.3336f8p+1f, -0x1.3336f8p+1f));
+  g = __ffma2_rn(g, t, make_float2(0x1.32067cp+1f, 0x1.32067cp+1f));
+  g = __ffma2_rn(g, t, make_float2(-0x1.cbf272p+0f, -0x1.cbf272p+0f));
+  g = __ffma2_rn(g, t, make_float2(0x1.3331cep+0f, 0x1.3331cep+0f));
+  float2 c = __ffma2_rn(s, g, make_float2(0.5f, 0.5f));
+  c.x = __saturatef(c.x);
+  c.y = __saturatef(c.y);
+  const float2 q = __fadd2_rn(c, make_float2(8.0f, 8.0f));
+  r0 = __float_as_int(q.x);
+  r1 = __float_as_int(q.y);
+}
+
 // integer add to a shared-memory bin (byte address in the shared window) unless the addend is zero (ptxas turns the
 // predicate into a branch; adding the zeros as well, without any test, was measured slower: 0.630 against 0.620 ms)
 __device__ __forceinline__ void red_add_nz(unsigned saddr, int d) {
@@ -781,7 +804,8 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
             const float kf = (float)b0;
             int r[UNIT + 1];
 #pragma unroll
-            for (int j = 0; j <= UNIT; ++j) r[j] = edge_r(kf + (float)j, zp, inv, P);
+            for (int j = 0; j + 1 <= UNIT; j += 2) edge_r2(kf + (float)j, kf + (float)(j + 1), zp, inv, P, r[j], r[j + 1]);
+            if ((UNIT & 1) == 0) r[UNIT] = edge_r(kf + (float)UNIT, zp, inv, P);
 #pragma unroll
             for (int j = 0; j < UNIT; ++j) d[j] = j < rem ? r[j + 1] - r[j] : 0;
           }
@@ -1246,6 +1270,47 @@ __device__ __forceinline__ float track_accum(const Trk& T, float ax, float ay, f
   return w;
 }
 
+// The same with the packed fp32 instructions of sm_100: x and y of a track sit side by side in its staged record
+// ({x0, y0, tx, ty}, {Wx, Wy}), so residuals, weights and most sums come in pairs -- 18 instead of 27 floating-point
+// instructions per track and iteration.  e and gz are kept as two partial sums (x and y part) until the loop ends.
+struct Sums2 {
+  float2 ab, cd, e2, g, gz2;
+  float chi2, nact;
+};
+__device__ __forceinline__ void sums2_zero(Sums2& S) {
+  S.ab = S.cd = S.e2 = S.g = S.gz2 = make_float2(0.0f, 0.0f);
+  S.chi2 = S.nact = 0.0f;
+}
+__device__ __forceinline__ void sums2_close(const Sums2& Q, Sums& S) {
+  S.a = Q.ab.x; S.b = Q.ab.y; S.c = Q.cd.x; S.d = Q.cd.y; S.e = Q.e2.x + Q.e2.y;
+  S.gx = Q.g.x; S.gy = Q.g.y; S.gz = Q.gz2.x + Q.gz2.y; S.chi2 = Q.chi2; S.nact = Q.nact;
+}
+template <int FLAV>
+__device__ __forceinline__ float track_accum2(const float2 xy0, const float2 txy, const float2 W, const float oth,
+                                              const float2 naxy, const float az, const KParams& P, Sums2& S) {
+  const float2 r = __fadd2_rn(__ffma2_rn(make_float2(az, az), txy, xy0), naxy);   // residual, Eq. 9 (naxy = -(ax, ay))
+  const float2 m = __fmul2_rn(__fmul2_rn(r, r), W);
+  const float chi = m.x + m.y;                                                    // Eq. 7
+  float w;
+  if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+    const float E = __expf(-0.5f * chi);
+    w = __fdividef(E, oth + E);
+  } else {
+    const float u = fmaxf(fmaf(chi, -P.inv_chi2_max, 1.0f), 0.0f);
+    w = u * u;
+  }
+  const float2 wW = __fmul2_rn(make_float2(w, w), W);
+  const float2 pq = __fmul2_rn(wW, txy);
+  S.ab = __fadd2_rn(S.ab, wW);
+  S.cd = __fadd2_rn(S.cd, pq);
+  S.e2 = __ffma2_rn(pq, txy, S.e2);
+  S.g = __ffma2_rn(wW, r, S.g);
+  S.gz2 = __ffma2_rn(pq, r, S.gz2);
+  S.chi2 = fmaf(w, chi, S.chi2);
+  S.nact += __saturatef(w * 1e38f);
+  return w;
+}
+
 // Newton-Raphson step Eq. 13 on the arrow-shaped Hessian A = [[a,0,-c],[0,b,-d],[-c,-d,e]]:
 // returns false when the fit is singular (fewer than 2 active tracks or a non-positive pivot).
 // C = A^-1 (Eq. 14), upper triangle xx xy xz yy yz zz.
@@ -1445,7 +1510,9 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
     const float px = fin ? lx : ax, py = fin ? ly : ay, pz = fin ? lz : az;
     const int e = cur.x, k = cur.y & 31;
     Sums S;
-    sums_zero(S);
+    Sums2 Q;
+    sums2_zero(Q);
+    const float2 naxy = make_float2(-px, -py);
     float nass = 0.0f;                                       // multi-vertex flavour: tracks with final weight >= 1/2
     float* wp = A.wrec + cur.z + j;                          // explicit flavour: my tracks' places in wrec[]
     char* wq = reinterpret_cast<char*>(wp);                  // walked slot by slot (one pointer add instead of re-deriving
@@ -1453,10 +1520,15 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
     const int wslots = st == FS_ITER ? myslots : 0;
 #pragma unroll FIT_UNROLL
     for (int s = 0; s < nslot_w; ++s) {
-      const Trk T = slot_track<FLAV>(SA[s][lane], SB[s][lane]);
-      float w = track_accum<FLAV>(T, px, py, pz, P, S);
+      const float4 qa = SA[s][lane];
+      const BT qb = SB[s][lane];
+      float oth = 1.0f;
+      if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) oth = qb.w;
+      const float w = track_accum2<FLAV>(make_float2(qa.x, qa.y), make_float2(qa.z, qa.w), make_float2(qb.x, qb.y), oth, naxy, pz,
+                                         P, Q);
       if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
-        if (fin && s < myslots && !track_is_dead(T, P)) {    // the weights of the last iteration are the outputs
+        const bool deadt = P.unit_weights ? !(qb.x > 0.0f) : (qa.x == 1e15f);
+        if (fin && s < myslots && !deadt) {                  // the weights of the last iteration are the outputs
           claim_track(A, __float_as_int(SB[s][lane].z), w, k);
           nass += (w >= 0.5f) ? 1.0f : 0.0f;
         }
@@ -1465,6 +1537,7 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
         wq += wstep;
       }
     }
+    sums2_close(Q, S);
     if (P.unit_weights) {
       S.nact = nvalid;
       if (FLAV != PV_FLAVOUR_MULTIVERTEX)                    // unit weights give a dead (R-7) track w = 1: its output is 0
