@@ -1969,24 +1969,44 @@ __global__ void __launch_bounds__(256) ip_kernel(const __grid_constant__ KParams
       best_c[u] = INFINITY; best_rx[u] = 0.0f; best_ry[u] = 0.0f; best_v[u] = -1;
       usable[u] = true;
     }
+    // The two tracks of a lane go through the vertex loop side by side in packed fp32 pairs (FFMA2 / FADD2 / FMUL2 of
+    // sm_100): the same operations in the same order as the scalar form, half the floating-point instructions.
+    static_assert(U == 2, "the two tracks of a lane are packed in pairs");
+    const float2 X = make_float2(x[0], x[1]), Y = make_float2(y[0], y[1]), nZ = make_float2(-z[0], -z[1]);
+    const float2 Aa = make_float2(a[0], a[1]), Bb = make_float2(b[0], b[1]), nBb = make_float2(-b[0], -b[1]);
+    const float2 VX = make_float2(vx[0], vx[1]), VY = make_float2(vy[0], vy[1]);
+    const float2 VTX = make_float2(vtx[0], vtx[1]), VTY = make_float2(vty[0], vty[1]);
+    auto dup = [](const float v) { return make_float2(v, v); };
 #pragma unroll 1
     for (int v = 0; v < nv; ++v) {
       const float* q = sv[warp][v];
       const float q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3], q4 = q[4], q5 = q[5], q6 = q[6], q7 = q[7], q8 = q[8];
+      const float2 dz = __fadd2_rn(dup(q2), nZ);
+      float2 Vx, Vy;
+      if (have_cross) {
+        Vx = make_float2(var_at(vx[0], vtx[0], cx[0], dz.x, true), var_at(vx[1], vtx[1], cx[1], dz.y, true));
+        Vy = make_float2(var_at(vy[0], vty[0], cy[0], dz.x, true), var_at(vy[1], vty[1], cy[1], dz.y, true));
+      } else {
+        Vx = __ffma2_rn(dz, __fmul2_rn(dz, VTX), VX);
+        Vy = __ffma2_rn(dz, __fmul2_rn(dz, VTY), VY);
+      }
+      const float2 rx = __ffma2_rn(dz, Aa, __fadd2_rn(X, dup(-q0))), ry = __ffma2_rn(dz, Bb, __fadd2_rn(Y, dup(-q1)));
+      const float2 Sxx = __ffma2_rn(Aa, __ffma2_rn(Aa, dup(q8), dup(-2.0f * q5)), __fadd2_rn(Vx, dup(q3)));
+      const float2 Syy = __ffma2_rn(Bb, __ffma2_rn(Bb, dup(q8), dup(-2.0f * q7)), __fadd2_rn(Vy, dup(q6)));
+      const float2 Sxy = __ffma2_rn(Aa, __ffma2_rn(Bb, dup(q8), dup(-q7)), __ffma2_rn(nBb, dup(q5), dup(q4)));
+      const float2 sq = __fmul2_rn(Sxy, Sxy);
+      const float2 det = __ffma2_rn(Sxx, Syy, make_float2(-sq.x, -sq.y));
+      const float2 cr = __fmul2_rn(__fmul2_rn(__fmul2_rn(dup(-2.0f), Sxy), rx), ry);
+      const float2 num = __ffma2_rn(__fmul2_rn(Syy, rx), rx, __ffma2_rn(__fmul2_rn(Sxx, ry), ry, cr));
+      const float c2[U] = {__fdividef(num.x, det.x), __fdividef(num.y, det.y)};
+      const float Vxs[U] = {Vx.x, Vx.y}, Vys[U] = {Vy.x, Vy.y}, Sxxs[U] = {Sxx.x, Sxx.y}, dets[U] = {det.x, det.y};
+      const float rxs[U] = {rx.x, rx.y}, rys[U] = {ry.x, ry.y};
 #pragma unroll
       for (int u = 0; u < U; ++u) {
-        const float dz = q2 - z[u];
-        const float Vx = var_at(vx[u], vtx[u], cx[u], dz, have_cross), Vy = var_at(vy[u], vty[u], cy[u], dz, have_cross);
-        const float rx = fmaf(dz, a[u], x[u] - q0), ry = fmaf(dz, b[u], y[u] - q1);
-        const float Sxx = fmaf(a[u], fmaf(a[u], q8, -2.0f * q5), Vx + q3);
-        const float Syy = fmaf(b[u], fmaf(b[u], q8, -2.0f * q7), Vy + q6);
-        const float Sxy = fmaf(a[u], fmaf(b[u], q8, -q7), fmaf(-b[u], q5, q4));
-        const float det = fmaf(Sxx, Syy, -Sxy * Sxy);
-        const float num = fmaf(Syy * rx, rx, fmaf(Sxx * ry, ry, -2.0f * Sxy * rx * ry));
-        const float c2 = __fdividef(num, det);
         // R-7 and positive definiteness: Vx, Vy positive and finite, Sxx > 0, det > 0 (NaN fails every test)
-        const bool ok = usable[u] && Vx > 0.0f && Vy > 0.0f && Vx < INFINITY && Vy < INFINITY && Sxx > 0.0f && det > 0.0f;
-        if (ok && c2 < best_c[u]) { best_c[u] = c2; best_rx[u] = rx; best_ry[u] = ry; best_v[u] = v; }
+        const bool ok = usable[u] && Vxs[u] > 0.0f && Vys[u] > 0.0f && Vxs[u] < INFINITY && Vys[u] < INFINITY && Sxxs[u] > 0.0f &&
+                        dets[u] > 0.0f;
+        if (ok && c2[u] < best_c[u]) { best_c[u] = c2[u]; best_rx[u] = rxs[u]; best_ry[u] = rys[u]; best_v[u] = v; }
       }
     }
     float best_d[U];
