@@ -59,7 +59,10 @@ constexpr int SEED_WARPS = PV_SEED_WARPS;      // warps per CTA of seed_kernel =
 constexpr int CHUNK = 64;           // tracks per fill chunk
 constexpr int SLOTS = CHUNK / 32;   // tracks per lane and chunk
 #ifndef PV_FIT_UNROLL
-#define PV_FIT_UNROLL 4
+#define PV_FIT_UNROLL 2
+#endif
+#ifndef PV_FIT_UNROLL_MV
+#define PV_FIT_UNROLL_MV 4
 #endif
 #ifndef PV_UNIT
 #define PV_UNIT 6
@@ -68,7 +71,10 @@ constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT
 constexpr int LIST_CAP = 192;       // fill units of one round (a chunk of median tracks needs ~100)
 constexpr int BINS_SM = 128;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int SEEDOF_SM = 128;      // ... whose seed index stays in shared memory between the count and the sort of a4
-constexpr int FIT_UNROLL = PV_FIT_UNROLL;   // unroll of the track loop of one fit iteration
+// unroll of the track loop of one fit iteration; with the packed loop, configs[1]: explicit 1 / 2 / 3 / 4 / 8 -> 0.345 / 0.333 /
+// 0.339 / 0.338 / 0.345 ms, multi-vertex 2 / 4 -> 0.343 / 0.333 ms
+constexpr int FIT_UNROLL = PV_FIT_UNROLL;
+constexpr int FIT_UNROLL_MV = PV_FIT_UNROLL_MV;
 #ifndef PV_FIT_KF
 #define PV_FIT_KF 14
 #endif
@@ -1408,7 +1414,10 @@ __device__ __forceinline__ void store_dead(float4 (*SA)[32], typename FitB<FLAV>
 
 enum { FS_EMPTY = 0, FS_LOAD = 1, FS_ITER = 2, FS_FINAL = 3, FS_DONE = 4 };
 #ifndef PV_FIT_WPW
-#define PV_FIT_WPW 2        // measured on configs[1]: 1 -> 0.387 ms (multi-vertex 0.540), 2 -> 0.366 (0.384), 4 -> 0.366 (0.414)
+#define PV_FIT_WPW 3        // explicit flavour; measured on configs[1]: 1 -> 0.359 ms, 2 -> 0.338, 3 -> 0.336 (configs[2]: 0.393 -> 0.387)
+#endif
+#ifndef PV_FIT_WPW_MV
+#define PV_FIT_WPW_MV 2     // multi-vertex flavour; measured on configs[1] (round 2, first half): 1 -> 0.540 ms, 2 -> 0.384, 4 -> 0.414
 #endif
 #ifndef PV_FIT_LOADWAIT
 #define PV_FIT_LOADWAIT 0        // ticks a group sits out after starting the copy of its next seed before it waits for the data
@@ -1518,7 +1527,7 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
     char* wq = reinterpret_cast<char*>(wp);                  // walked slot by slot (one pointer add instead of re-deriving
     const unsigned wstep = 4u << lg;                         // the address from the slot index: 8 -> 4 instructions per slot)
     const int wslots = st == FS_ITER ? myslots : 0;
-#pragma unroll FIT_UNROLL
+#pragma unroll(FLAV == PV_FLAVOUR_MULTIVERTEX ? FIT_UNROLL_MV : FIT_UNROLL)
     for (int s = 0; s < nslot_w; ++s) {
       const float4 qa = SA[s][lane];
       const BT qb = SB[s][lane];
@@ -1653,7 +1662,8 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
   const int nwarps = (gridDim.x * blockDim.x) >> 5;
   // window size: PV_FIT_WPW windows per warp when the batch allows, claimed one after the other (the windows of a
   // batch take different times; several per warp even that out), at most FIT_WIN records
-  int win = (total + PV_FIT_WPW * nwarps - 1) / (PV_FIT_WPW * nwarps);
+  constexpr int WPW = FLAV == PV_FLAVOUR_MULTIVERTEX ? PV_FIT_WPW_MV : PV_FIT_WPW;
+  int win = (total + WPW * nwarps - 1) / (WPW * nwarps);
   win = min(max((win + 31) & ~31, 32), FIT_WIN);
   const int nwin = (total + win - 1) / win;
   const Trk dead = dead_track(P);
