@@ -77,7 +77,8 @@ enum {
   PV_E_PARAM = -2,      /* invalid parameter (dz <= 0, range not a whole number of bins, too many bins, ...) */
   PV_E_WORKSPACE = -3,  /* workspace too small */
   PV_E_CUDA = -4,       /* a CUDA runtime call or kernel launch failed (see pv_last_cuda_error) */
-  PV_E_SIZE = -5        /* negative n_events / n_tracks, or a host staging capacity exceeded */
+  PV_E_SIZE = -5,       /* negative n_events / n_tracks, or a host staging capacity exceeded */
+  PV_E_STATIC_LIMIT = -6 /* pv_find_static only: the batch needs more scratch than PV_STATIC_WORKSPACE_BYTES */
 };
 
 /* Compile-time limits of this build. */
@@ -85,7 +86,8 @@ enum {
   PV_MAX_BINS = 4096,          /* (z_max - z_min) / dz must be <= this */
   PV_MAX_VTX = 32,             /* max_vtx_per_event must be <= this */
   PV_MAX_TRACKS_PER_EVENT = 2047, /* larger events get PV_EVT_TOO_MANY_TRACKS and zero vertices */
-  PV_FIXED_ONE = 1 << 20       /* histogram fixed-point unit: the full mass of one track */
+  PV_FIXED_ONE = 1 << 20,      /* histogram fixed-point unit: the full mass of one track */
+  PV_STATIC_WORKSPACE_BYTES = 16 << 20 /* scratch built into the library for pv_find_static (16 MiB per GPU) */
 };
 
 /* event_status bit flags */
@@ -207,6 +209,45 @@ int pv_find_ext(const float* x, const float* y, const float* z, const float* tx,
                 float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
                 int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status,
                 void* workspace, size_t workspace_bytes, void* stream, const pv_track_cov* cov, const pv_debug* dbg);
+
+/* pv_find for callers that have no device memory to give as a workspace and may not allocate any.
+ *
+ * Who that is: a plug-in inside a host framework that took the GPU's memory at start-up and hands out slices of its
+ * own arena only to its own algorithms (the trigger framework the paper runs in works like this, and so does any
+ * service with a memory budget fixed at launch), so that a cudaMalloc from a third-party library either fails or
+ * breaks the budget; an event loop with a latency bound, whose house rules forbid cudaMalloc / cudaFree after
+ * initialisation because both may synchronise the whole device and take an unbounded time; and a plain C caller
+ * that simply has no device allocator at hand beyond the buffers it was given for inputs and outputs.
+ *
+ * Same arguments, same kernels and bit-for-bit the same results as pv_find, except that there is no workspace
+ * argument: the scratch (counters, seed records, fit-ready track records, pv_workspace_bytes() of them) lives in an
+ * array of PV_STATIC_WORKSPACE_BYTES = 16 MiB that is part of the library's device image.  Every GPU on which the
+ * library's kernels are loaded holds those 16 MiB until the process exits, whether or not this entry is ever called.
+ * Inputs and outputs are still the caller's DEVICE buffers.
+ *
+ * Limit: pv_workspace_bytes(n_events, n_tracks, params) must be <= PV_STATIC_WORKSPACE_BYTES, else nothing is
+ * enqueued and PV_E_STATIC_LIMIT is returned.  With the default parameters that is about 3 400 events of the paper's
+ * mu = 5 mix (117 tracks per event; 256 + 512 B per event + 36 B per track) in the explicit flavour and about 1 800
+ * in the multi-vertex flavour (76 B per track) -- several of the paper's batches of "several hundred events".
+ * Larger batches: split them, or use pv_find with a workspace of your own.
+ *
+ * The call makes no cudaMalloc / cudaFree / cudaMallocAsync and calls no library routine that allocates device
+ * memory; it refuses to run while pv_kernel_timing(1) is on (PV_E_PARAM), because the timing events would have to be
+ * created.  The first call on each device looks up the device address of the array (once per device, with that device
+ * current; the caller must have made the device of its buffers current, as for every entry of this header) and, like
+ * any first launch, lets the CUDA runtime load the kernels: make that first call during initialisation, before any
+ * stream capture and outside the latency-critical loop.
+ *
+ * Sharing: all calls on one device use the same array, from every thread and stream of the process.  Calls ordered
+ * on one stream (or ordered by events) are safe; two calls that can overlap on the GPU race on the scratch and give
+ * wrong results without any error.  The array keeps whatever the previous call left in it; no result depends on
+ * that: each call clears the counters that must start at zero on `stream` before its first kernel, and takes its
+ * results only from records it has written itself. */
+int pv_find_static(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                   const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                   const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                   float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                   int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status, void* stream);
 
 /* ---- host-buffer entries (the paper's host pipeline: "several streams ... each processing a batch",
  * host->device copies overlapped with compute).  A pv_host_ctx owns device buffers, workspaces, streams and events

@@ -22,6 +22,8 @@ EVT_TOO_MANY_TRACKS = 1
 EVT_VTX_OVERFLOW = 2
 EVT_SINGULAR_FIT = 4
 EVT_RECORD_OVERFLOW = 8
+STATIC_WORKSPACE_BYTES = 16 << 20
+E_STATIC_LIMIT = -6
 FLAVOUR_EXPLICIT = 0
 FLAVOUR_MULTIVERTEX = 1
 FILL_POLYNOMIAL = 0
@@ -30,7 +32,7 @@ FILL_TEMPLATE = 1
 FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
 EXPORTS = (
-    "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug", "pv_find_ext", "pv_track_ip",
+    "pv_params_default", "pv_nbins", "pv_workspace_bytes", "pv_find", "pv_find_debug", "pv_find_ext", "pv_find_static", "pv_track_ip",
     "pv_host_ctx_create", "pv_host_ctx_destroy", "pv_find_host", "pv_find_host_compact", "pv_host_register", "pv_host_unregister",
     "pv_last_launch_info", "pv_kernel_timing", "pv_kernel_time_ms", "pv_kernel_times_ms", "pv_error_string", "pv_last_cuda_error",
 )
@@ -94,6 +96,7 @@ def lib():
         L.pv_find.argtypes = find_args
         L.pv_find_debug.argtypes = find_args + [C.POINTER(Debug)]
         L.pv_find_ext.argtypes = find_args + [C.POINTER(TrackCov), C.POINTER(Debug)]
+        L.pv_find_static.argtypes = find_args[:-3] + [vp]
         L.pv_track_ip.argtypes = [vp] * 9 + [vp, i32, i64, C.POINTER(Params)] + [vp] * 3 + [vp] * 3 + [C.POINTER(TrackCov), vp]
         L.pv_host_ctx_create.argtypes = [C.POINTER(vp), i32, i64, C.POINTER(Params), i32]
         L.pv_host_ctx_destroy.argtypes = [vp]
@@ -240,6 +243,22 @@ class DeviceBatch:
                 _check(L.pv_find_debug(*args, C.byref(self.dbg_struct)), "pv_find_debug")
             else:
                 _check(L.pv_find(*args), "pv_find")
+
+    def find_static(self, stream=None) -> None:
+        """Enqueue pv_find_static on `stream`: pv_find for callers that may not allocate device memory (a plug-in of a
+        framework that owns the GPU's memory, a loop in which cudaMalloc is forbidden).  Its scratch is the 16 MiB
+        array built into the library instead of self.workspace, so the batch must need no more than
+        STATIC_WORKSPACE_BYTES (PvError with code -6 otherwise), and calls that may overlap on the GPU must not be
+        issued.  No taps, no covariance cross terms."""
+        torch = _torch()
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        i, o = self.inp, self.out
+        args = [i[k].data_ptr() for k in FIELDS] + [self.offsets.data_ptr(), self.E, self.T, C.byref(self.p)] + [
+            o["vtx_pos"].data_ptr(), o["vtx_cov"].data_ptr(), o["vtx_chi2"].data_ptr(), o["vtx_ntracks"].data_ptr(),
+            o["vtx_niter"].data_ptr(), o["n_vtx"].data_ptr(), o["trk_weight"].data_ptr(), o["trk_vertex"].data_ptr(),
+            o["event_status"].data_ptr(), s.cuda_stream]
+        with torch.cuda.device(self.device):
+            _check(lib().pv_find_static(*args), "pv_find_static")
 
     def track_ip(self, stream=None) -> None:
         """Enqueue pv_track_ip on the vertices of the last find(); results in self.ip (ip, ip_chi2, ip_vertex)."""

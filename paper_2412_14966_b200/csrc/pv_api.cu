@@ -317,7 +317,58 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
 
 }  // namespace
 
+/* ---- pv_find_static: the workspace of callers that cannot allocate device memory (include/pv_finder.h) ----
+ * The scratch of the three kernels, as a part of this library's device image: 16 MiB on every GPU that loads it.
+ * In host code the name g_static_ws is only a handle for the runtime (a host-side shadow symbol); its value is NOT
+ * where the array lives on the GPU, and a kernel given it would fault or scribble over host memory.  The address the
+ * kernels need comes from cudaGetSymbolAddress, asked once per device with that device current. */
+static __device__ __align__(256) unsigned char g_static_ws[PV_STATIC_WORKSPACE_BYTES];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+void* g_static_ws_ptr[STATIC_MAX_DEVICES] = {nullptr};   // device address of g_static_ws, per device ordinal
+
+// Device address of g_static_ws on the current device; looked up at the first call on that device.
+int static_workspace(void** out) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return PV_E_SIZE;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ws_ptr[dev]) {
+    void* ptr = nullptr;
+    CK(cudaGetSymbolAddress((void**)&ptr, g_static_ws));
+    if (!ptr || ((uintptr_t)ptr & 255) != 0) return PV_E_CUDA;
+    g_static_ws_ptr[dev] = ptr;
+  }
+  *out = g_static_ws_ptr[dev];
+  return PV_OK;
+}
+
+}  // namespace
+
 extern "C" {
+
+int pv_find_static(const float* x, const float* y, const float* z, const float* tx, const float* ty,
+                   const float* var_x, const float* var_y, const float* var_tx, const float* var_ty,
+                   const int32_t* offsets, int n_events, long long n_tracks, const pv_params* params,
+                   float* vtx_pos, float* vtx_cov, float* vtx_chi2, int32_t* vtx_ntracks, int32_t* vtx_niter,
+                   int32_t* n_vtx, float* trk_weight, int32_t* trk_vertex, uint32_t* event_status, void* stream) {
+  const int rc = validate(params, nullptr);
+  if (rc != PV_OK) return rc;
+  if (n_events < 0 || n_tracks < 0 || n_tracks > 0x7fffffffLL) return PV_E_SIZE;
+  if (g_timing) return PV_E_PARAM;                            // the timing events would have to be created
+  if (ws_bytes(n_events, n_tracks, params) > (size_t)PV_STATIC_WORKSPACE_BYTES) return PV_E_STATIC_LIMIT;
+  void* ws = nullptr;
+  const int src = static_workspace(&ws);
+  if (src != PV_OK) return src;
+  // from here on the path of pv_find: it clears the 64 bytes of counters at the head of the workspace on `stream`
+  // and launches the kernels; none of it allocates
+  return find_impl(x, y, z, tx, ty, var_x, var_y, var_tx, var_ty, offsets, n_events, n_tracks, params, vtx_pos, vtx_cov,
+                   vtx_chi2, vtx_ntracks, vtx_niter, n_vtx, trk_weight, trk_vertex, event_status, ws,
+                   (size_t)PV_STATIC_WORKSPACE_BYTES, stream, nullptr);
+}
 
 int pv_params_default(pv_params* p) {
   if (!p) return PV_E_NULL;
@@ -719,6 +770,7 @@ const char* pv_error_string(int code) {
     case PV_E_WORKSPACE: return "workspace too small";
     case PV_E_CUDA: return "CUDA error (see pv_last_cuda_error)";
     case PV_E_SIZE: return "invalid size or capacity exceeded";
+    case PV_E_STATIC_LIMIT: return "batch needs more scratch than the built-in workspace of pv_find_static (PV_STATIC_WORKSPACE_BYTES): split it or use pv_find";
     default: return "unknown error code";
   }
 }
