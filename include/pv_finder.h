@@ -41,7 +41,8 @@ typedef struct pv_params {
   float z_split;                        /* region boundary: -300                          Table 2 */
   float beam_x, beam_y, beam_tx, beam_ty; /* beamline position and direction at z = 0 */
   float max_sigma_poca[2];              /* max sigma_poca to enter the histogram: 1.5, 10  P:L129, Table 2
-                                           (6 max_sigma_poca / dz + 4 <= 3072 bins, else PV_E_PARAM) */
+                                           (6 max_sigma_poca / dz + 4 <= 3072 bins, and with PV_FILL_TEMPLATE the
+                                           window of the widest class as well, else PV_E_PARAM) */
   float min_bin_content;                /* proto-cluster bin threshold [tracks]: 0.25      P:L135 (value: reading R-4) */
   float min_dip;                        /* significance of an extremum [tracks]: 0.75      P:L135 (value: reading R-4) */
   float min_cluster_integral[2];        /* min track integral of a seed cluster: 2.5, 1.75 Table 2 */
@@ -254,8 +255,9 @@ int pv_find_static(const float* x, const float* y, const float* z, const float* 
  * sized for at most max_events / max_tracks (no host staging: the caller's buffers are copied from and to directly, so
  * they should be pinned, see pv_host_register; pageable memory works but the copies then serialise).
  * pv_find_host() takes HOST pointers everywhere (same meaning and layout as pv_find), splits the batch into n_chunks
- * (1..256) contiguous event ranges of equal track count, and for each enqueues H2D copies -> pv_find -> D2H copies on
- * one of the context's streams.  It returns after all results are in the caller's host arrays (it synchronises its
+ * (1..256) contiguous event ranges whose track counts ramp up and down as 1, 2, 4, 8, 8, ..., 8, 4, 2, 1 (the first
+ * kernels start after a short copy, the last results leave after a short one), and for each enqueues H2D copies ->
+ * pv_find -> D2H copies on one of the context's streams.  It returns after all results are in the caller's host arrays (it synchronises its
  * own streams only, also on every error path).  `offsets` is validated on the host (offsets[0] = 0, non-decreasing,
  * offsets[n_events] <= max_tracks; else PV_E_SIZE).  Both flavours and both splitting variants are supported (the
  * context is sized for the flavour given at creation); the covariance cross terms of pv_find_ext are not part of
@@ -309,7 +311,9 @@ int pv_last_launch_info(int* n_kernels, int* grid, int* block, int* smem_bytes);
  * caller can time the kernels live.  pv_kernel_timing(1) enables, (0) disables; pv_kernel_time_ms()
  * synchronises the last call's events and returns the duration of its three kernels in ms (< 0 if none);
  * pv_kernel_times_ms() writes up to n per-kernel durations (seed a1-a4, fit a5, cleanup a6) to ms (HOST)
- * and returns the number of kernels (3), or a negative PV_E_*. */
+ * and returns the number of kernels (3), or a negative PV_E_*.  With PV_FILL_TEMPLATE the small kernel that builds
+ * the table of templates runs inside the first interval: "seed" then means table + seed kernel.
+ * Bench / diagnostic use only: the events and the flag are process-global (see "Thread safety" above). */
 int pv_kernel_timing(int enable);
 float pv_kernel_time_ms(void);
 int pv_kernel_times_ms(float* ms, int n);

@@ -66,6 +66,8 @@ int clamp_i32(long long v) {
   return (int)v;
 }
 
+size_t tmpl_layout(const pv_params* p, pvk::KParams* k);
+
 int validate(const pv_params* p, int* nbins_out) {
   if (!p) return PV_E_NULL;
   if (!(p->dz > 0.0f) || !(p->z_max > p->z_min)) return PV_E_PARAM;
@@ -83,8 +85,16 @@ int validate(const pv_params* p, int* nbins_out) {
   if (p->fill_mode != PV_FILL_POLYNOMIAL && p->fill_mode != PV_FILL_TEMPLATE) return PV_E_PARAM;
   if (p->flavour == PV_FLAVOUR_MULTIVERTEX && (!(p->chi2_window > 0.0f) || isinf(p->chi2_max))) return PV_E_PARAM;
   // the fill cuts a track's +-3 sigma window into units of PV_UNIT bins and numbers them with 9 bits
+  constexpr int max_window = pvk::MAX_FILL_UNITS * pvk::UNIT;
   for (int r = 0; r < 2; ++r)
-    if (!(6.0 * (double)p->max_sigma_poca[r] / (double)p->dz + 4.0 <= 512.0 * PV_UNIT)) return PV_E_PARAM;
+    if (!(6.0 * (double)p->max_sigma_poca[r] / (double)p->dz + 4.0 <= (double)max_window)) return PV_E_PARAM;
+  // template fill: the window is that of the class centre, up to 2^(1/8) wider than the track's own sigma
+  if (p->fill_mode == PV_FILL_TEMPLATE) {
+    pvk::KParams k;
+    tmpl_layout(p, &k);
+    const int widest = 2 * (int)k.tmpl_w[k.tmpl_kmax] + 1;
+    if ((widest < nbins ? widest : nbins) > max_window) return PV_E_PARAM;
+  }
   if (nbins_out) *nbins_out = nbins;
   return PV_OK;
 }
@@ -263,6 +273,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.fit_counter = reinterpret_cast<unsigned int*>(ws + 48);
   ka.ftrk = reinterpret_cast<float4*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
   ka.trk_cap = (unsigned int)ws_trk_records(n_tracks, params->flavour);
+  ka.n_trk = (unsigned int)n_tracks;
   ka.best = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(ka.ftrk) + (size_t)ka.trk_cap * 32 + 16);
   ka.wrec = reinterpret_cast<float*>(ka.best);                // the two flavours use the same place differently
   ka.tmpl = reinterpret_cast<int32_t*>(ws + ws_core_bytes(n_events, n_tracks, params->max_vtx_per_event, params->flavour));

@@ -43,6 +43,7 @@ constexpr int MAXV = PV_MAX_VTX;
 #define PV_MV_KEEP 4
 #endif
 constexpr int MV_KEEP = PV_MV_KEEP;   // multi-vertex association: groups of 32 tracks whose candidate masks stay in registers between its two passes
+static_assert(MV_KEEP >= 0 && MV_KEEP <= 4, "the association keeps four mask / denominator register pairs (hm0..3, hd0..3)");
 #ifndef PV_DET_UNROLL
 #define PV_DET_UNROLL 2
 #endif
@@ -68,6 +69,9 @@ constexpr int SLOTS = CHUNK / 32;   // tracks per lane and chunk
 #define PV_UNIT 6
 #endif
 constexpr int UNIT = PV_UNIT;       // bins per fill unit: a lane evaluates UNIT + 1 independent CDF edges
+constexpr int MAX_FILL_UNITS = 512; // units of one track's window: the unit list packs (unit << 7 | staged track) in 16 bits
+static_assert(UNIT >= 1 && ((MAX_FILL_UNITS - 1) << 7 | 127) == 0xffff, "unit index: 9 bits above the 7 of the staged track");
+// (validate() in pv_api.cu refuses parameters whose widest fill window exceeds MAX_FILL_UNITS * UNIT bins)
 constexpr int LIST_CAP = 192;       // fill units of one round (a chunk of median tracks needs ~100)
 constexpr int BINS_SM = 128;        // tracks per event whose central bin stays in shared memory (else HBM scratch)
 constexpr int SEEDOF_SM = 128;      // ... whose seed index stays in shared memory between the count and the sort of a4
@@ -86,6 +90,8 @@ constexpr int FIT_UNROLL_MV = PV_FIT_UNROLL_MV;
 // lane): 16 slots / 18 warps 0.366 ms, 14 / 20 0.344, 12 / 22 0.367, 10 / 26 0.429; multi-vertex (32 B): 16 / 12 0.383, 12 / 16 0.362
 constexpr int FIT_KF = PV_FIT_KF;
 constexpr int FIT_KF_MV = PV_FIT_KF_MV;
+static_assert(FIT_KF >= 2 && FIT_KF <= 15 && FIT_KF_MV >= 2 && FIT_KF_MV <= 15,
+              "the fit's sort key is phase * 16 + 16 - slots (slots <= KF), counted in 96 bins");
 constexpr int FIT_WIN = 256;        // seed records of one window of the fit (its sorted order is held as 8 bytes per lane)
 constexpr int FIT_BLOCK = 64;       // threads per CTA of fit_kernel (warps are autonomous; 12 KB of tracks per warp)
 constexpr int FIT_MIN_BLOCKS = 10;  // CTAs per SM: 10 x (21 KB + 1 KB reserved) fill the shared memory
@@ -169,6 +175,7 @@ struct KArgs {
   unsigned long long* best;      // workspace, multi-vertex flavour: [T] largest weight of the track << 32 | 31 - seed
   unsigned int* trk_counter;     // workspace, multi-vertex flavour: track records allocated so far
   unsigned int trk_cap;          // capacity of ftrk in records
+  unsigned int n_trk;            // the n_tracks given to pv_find: the per-track parts of the workspace hold this many
   pv_debug dbg;
 };
 
@@ -632,13 +639,14 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
   const bool have_cross = A.cov_xtx != nullptr || A.cov_yty != nullptr;   // Eq. 2 with its x-tx / y-ty elements
   unsigned status = 0;
 
-  // explicit flavour: the fit-ready records of the event go to ftrk[t0 .. t0 + n): refuse what the workspace cannot hold
-  const bool no_room = FLAV == PV_FLAVOUR_EXPLICIT && (unsigned)t0 + (unsigned)n > A.trk_cap;
+  // the per-track parts of the workspace (explicit flavour: ftrk[] and wrec[], multi-vertex flavour: best[]) are
+  // indexed with the event's own track range and hold the n_tracks given to pv_find: refuse an event beyond them
+  const bool no_room = (unsigned)t0 + (unsigned)n > A.n_trk;
   if (n > MAX_TRK || no_room) {
 #pragma unroll 1
     for (int i = lane; i < n; i += 32) {
       A.trk_vertex[t0 + i] = -1;
-      if (FLAV == PV_FLAVOUR_MULTIVERTEX) A.best[t0 + i] = 0ull;
+      if (FLAV == PV_FLAVOUR_MULTIVERTEX && !no_room) A.best[t0 + i] = 0ull;   // (cleanup skips best[] of a no_room event)
     }
     if (DBG && A.dbg.trk_seed) for (int i = lane; i < n; i += 32) A.dbg.trk_seed[t0 + i] = -1;
     if (lane == 0) {
@@ -1753,6 +1761,8 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   const int t0 = __ldg(A.offsets + e);
   const int n = __ldg(A.offsets + e + 1) - t0;
   const size_t ev = (size_t)e * P.max_vtx;
+  // an event beyond the n_tracks given to pv_find (PV_EVT_RECORD_OVERFLOW, no seeds) has no place in wrec[] / best[]
+  const int nl = (unsigned)t0 + (unsigned)n > A.n_trk ? 0 : n;
   int sv[4];                                               // seed index of my first four tracks: loads issued now,
 #pragma unroll                                             // consumed after the vertex sweep
   for (int q = 0; q < 4; ++q) sv[q] = (lane + 32 * q < n) ? A.trk_vertex[t0 + lane + 32 * q] : -1;
@@ -1763,12 +1773,12 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   float wl[4] = {0.0f, 0.0f, 0.0f, 0.0f};
   if (FLAV != PV_FLAVOUR_MULTIVERTEX) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) wl[q] = (lane + 32 * q < n) ? A.wrec[t0 + lane + 32 * q] : 0.0f;
+    for (int q = 0; q < 4; ++q) wl[q] = (lane + 32 * q < nl) ? A.wrec[t0 + lane + 32 * q] : 0.0f;
   }
   unsigned long long bv[4] = {0ull, 0ull, 0ull, 0ull};     // multi-vertex flavour: largest weight << 32 | 31 - seed
   if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) bv[q] = (lane + 32 * q < n) ? A.best[t0 + lane + 32 * q] : 0ull;
+    for (int q = 0; q < 4; ++q) bv[q] = (lane + 32 * q < nl) ? A.best[t0 + lane + 32 * q] : 0ull;
   }
   float vp[3] = {0.0f, 0.0f, 0.0f}, vc[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
   float vchi2 = 0.0f;
@@ -1882,7 +1892,7 @@ __global__ void __launch_bounds__(256, PV_CLEANUP_MIN_BLOCKS) cleanup_kernel(con
   for (int i = 128 + lane; i < n; i += 32) {
     const int s = A.trk_vertex[t0 + i];
     const float w = (FLAV != PV_FLAVOUR_MULTIVERTEX && s >= 0) ? A.wrec[t0 + (s >> 5)] : 0.0f;
-    finish(i, s, FLAV == PV_FLAVOUR_MULTIVERTEX ? A.best[t0 + i] : 0ull, w);
+    finish(i, s, (FLAV == PV_FLAVOUR_MULTIVERTEX && i < nl) ? A.best[t0 + i] : 0ull, w);
   }
 }
 

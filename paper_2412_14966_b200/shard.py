@@ -12,9 +12,9 @@ FIELDS = ("x", "y", "z", "tx", "ty", "var_x", "var_y", "var_tx", "var_ty")
 
 
 def event_range(offsets: np.ndarray, rank: int, world: int) -> Tuple[int, int]:
-    """[e0, e1) of `rank`: boundaries at the events whose first track is the first at or beyond rank * T / world
-    (the chunking rule of pv_find_host), so the ranges are disjoint, ordered, cover every event, and hold about
-    T / world tracks each."""
+    """[e0, e1) of `rank`: boundaries at the events whose first track is the first at or beyond rank * T / world, so
+    the ranges are disjoint, ordered, cover every event, and hold about T / world tracks each.  (pv_find_host places
+    its chunk boundaries the same way, at targets that follow its ramped chunk weights instead of k / world.)"""
     offsets = np.asarray(offsets)
     E = int(offsets.size - 1)
     if world < 1 or not 0 <= rank < world:

@@ -69,6 +69,11 @@ def test_argument_validation_happens_before_cuda(pv):
         assert L.pv_nbins(C.byref(q)) == -2, bad                              # PV_E_PARAM
         args = [None] * 9 + [None, 0, 0, C.byref(q)] + [None] * 9 + [None, 0, None]
         assert L.pv_find(*args) == -2, bad
+    # template fill: the window of the widest class (2^(1/8) wider than the sigma cut) must fit the unit list too
+    wide = dict(max_sigma_poca=(1.5, 127.0))
+    assert L.pv_nbins(C.byref(pv.default_params(**wide))) == 3400             # polynomial window: 3052 bins <= 3072
+    assert L.pv_nbins(C.byref(pv.default_params(fill_mode=1, **wide))) == -2  # class 51: 2 * 1654 + 1 = 3309 bins
+    assert L.pv_nbins(C.byref(pv.default_params(fill_mode=1, max_sigma_poca=(1.5, 100.0)))) == 3400
     args = [None] * 9 + [None, 1, 0, C.byref(p)] + [None] * 9 + [None, 0, None]
     assert L.pv_find(*args) == -1                                             # NULL pointers
     assert L.pv_error_string(-2).decode() == "invalid parameter"

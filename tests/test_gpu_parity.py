@@ -595,6 +595,42 @@ def test_record_overflow_is_flagged_per_event(pv, oracle):
     assert rep["n_vertices"] > 100
 
 
+@pytest.mark.parametrize("mode", ["explicit", "multivertex"])
+def test_n_tracks_smaller_than_the_offsets(pv, mode):
+    """pv_find is told fewer tracks than offsets[n_events] holds, and gets a workspace sized for that smaller number:
+    events inside the given count come out as in a correct call, the others carry PV_EVT_RECORD_OVERFLOW, no vertex,
+    no assignment -- and nothing is written past the workspace (a guard area behind it keeps its pattern)."""
+    import torch
+    data = events.generate(events.config(1, 2000))
+    off = np.asarray(data["offsets"])
+    E = off.size - 1
+    p = pv.default_params() if mode == "explicit" else pv.multivertex_params()
+    want = pv.find(data, p)
+    b = pv.DeviceBatch(data, p)
+    T_given = int(off[E // 2]) + 3                           # ends inside event E/2
+    need = pv.workspace_bytes(E, T_given, p)
+    guard = 4 << 20
+    b.workspace = torch.full((need + guard,), 0xA5, dtype=torch.uint8, device=b.device)
+    b.T = T_given
+    for _ in range(2):
+        b.find()
+    got = b.results()
+    assert bool((b.workspace[need:] == 0xA5).all()), "the kernels wrote behind the workspace"
+    inside = off[1:] <= T_given
+    assert inside[:E // 2].all() and not inside[E // 2:].any()
+    ev_of_trk = np.repeat(np.arange(E), np.diff(off))
+    tin = inside[ev_of_trk]
+    assert np.all((got["event_status"][~inside] & 8) != 0) and np.all(got["n_vtx"][~inside] == 0)
+    assert np.all(got["trk_vertex"][~tin] == -1) and np.all(got["trk_weight"][~tin] == 0)
+    assert np.array_equal(got["event_status"][inside], want["event_status"][inside])
+    assert np.array_equal(got["n_vtx"][inside], want["n_vtx"][inside]) and want["n_vtx"][inside].sum() > 1000
+    assert np.array_equal(got["trk_vertex"][tin], want["trk_vertex"][tin])
+    assert np.array_equal(got["trk_weight"][tin], want["trk_weight"][tin])
+    m = (np.arange(p.max_vtx_per_event)[None, :] < want["n_vtx"][:, None]) & inside[:, None]
+    for k in ("vtx_pos", "vtx_cov", "vtx_chi2", "vtx_ntracks", "vtx_niter"):
+        assert np.array_equal(got[k][m], want[k][m]), k
+
+
 def test_unusual_parameters_reach_their_guards(pv, oracle):
     """min_tracks_seed = 0 keeps seeds without any track: they are singular fits on both sides, not stale slots;
     a sigma cut whose window would need more fill units than the list can number is refused (PV_E_PARAM)."""

@@ -106,6 +106,88 @@ def test_newton_step_vs_numerical_minimiser(oracle):
         assert abs(r["chi2"] - float(np.sum(wexp * c))) < 1e-9
 
 
+def _chi2_at(t, al, seed_z, w=None):
+    """chi2 = sum_i w_i r_i^T W_i r_i (Eq. 6-9) written out in numpy; W from Eq. 2 at the seed z."""
+    a = {k: t[k].astype(np.float64) for k in K}
+    dz = seed_z - a["z"]
+    Wx = 1 / (a["var_x"] + dz ** 2 * a["var_tx"]); Wy = 1 / (a["var_y"] + dz ** 2 * a["var_ty"])
+    rx = a["x"] + (al[2] - a["z"]) * a["tx"] - al[0]
+    ry = a["y"] + (al[2] - a["z"]) * a["ty"] - al[1]
+    c = rx * rx * Wx + ry * ry * Wy
+    return c if w is None else float(np.sum(w * c))
+
+
+def test_delta_chi2_is_the_change_of_the_quadratic_chi2(oracle):
+    """Eq. 15-17 (L212-221): with the weights held fixed chi2 is quadratic in alpha, so the Newton step changes it by
+    exactly dchi2 = 1/2 (alpha1 - alpha0) . dchi2/dalpha.  (a) unit weights: chi2(alpha1) - chi2(seed), both written
+    out in numpy, equals the oracle's dchi2 of iteration 1; (b) Tukey weights: the same at every iteration with the
+    weights frozen at that iteration's values (recomputed here from Eq. 18 at the pre-step position).  A wrong factor
+    in Eq. 17 (2x, 1/2x, a sign) fails both."""
+    rng = np.random.default_rng(21)
+    for trial in range(12):
+        P = (rng.normal(0, 0.04), rng.normal(0, 0.04), rng.normal(0, 45))
+        n = int(rng.integers(4, 50))
+        t = _tracks(rng, n, P, zstate=P[2] + rng.uniform(-20, 20, n))
+        seed = np.array([0.0, 0.0, P[2] + rng.uniform(-0.5, 0.5)])
+        # (a) unit weights
+        r = oracle.fit(t, np.arange(n), tuple(seed), oracle.default_params(chi2_max=np.inf))
+        ones = np.ones(n)
+        d = _chi2_at(t, r["trace"][0, :3], seed[2], ones) - _chi2_at(t, seed, seed[2], ones)
+        assert d < -1e-3 and abs(d - r["trace"][0, 9]) <= 1e-9 * abs(d), (d, r["trace"][0, 9])
+        # (b) Tukey weights, every iteration
+        t["x"][:2] += np.float32(0.3)
+        r = oracle.fit(t, np.arange(n), tuple(seed), oracle.default_params(conv_dchi2=1e-12, conv_dz=1e-9))
+        assert r["rc"] == 0 and r["niter"] >= 3
+        prev = seed
+        for it in range(r["niter"]):
+            c = _chi2_at(t, prev, seed[2])
+            w = np.where(c < 12, (1 - c / 12) ** 2, 0.0)                         # Eq. 18 at the pre-step position
+            nxt = r["trace"][it, :3]
+            d = _chi2_at(t, nxt, seed[2], w) - _chi2_at(t, prev, seed[2], w)
+            assert d <= 0 and abs(d - r["trace"][it, 9]) <= 1e-9 * abs(d) + 1e-13, (trial, it, d, r["trace"][it, 9])
+            assert abs((nxt[2] - prev[2]) - r["trace"][it, 10]) < 1e-12           # the dz the stop rule looks at
+            prev = nxt
+
+
+def test_stop_rule_needs_both_conditions_and_the_papers_thresholds(oracle):
+    """L225: the fit stops when |dchi2| < 0.01 AND |dz| < 1 um.  Unit weights make every case exact: the first step
+    lands on the least-squares point (L223), the second is zero, so niter is 1 if iteration 1 already satisfies the
+    rule and 2 otherwise.  Noiseless tracks from P, all given at z = P.z with sigma = 0.05 mm (W = 400 / mm^2 each):
+    a seed off by (dx, 0, dz) has chi2 = sum_i W (dx - dz tx_i)^2 + W (dz ty_i)^2, and that is -dchi2 of step 1."""
+    rng = np.random.default_rng(22)
+    P = (0.01, -0.02, 12.5)
+    n = 4
+    t = _tracks(rng, n, P, sig=(0.05, 0.05), noise=False)
+    p = oracle.default_params(chi2_max=np.inf)
+    W = 400.0
+
+    def run(dx, dz):
+        seed = (P[0] + dx, P[1], P[2] + dz)
+        r = oracle.fit(t, np.arange(n), seed, p)
+        assert r["rc"] == 0 and np.allclose(r["pos"], P, atol=1e-6)
+        want = -float(np.sum(W * (dx - dz * t["tx"].astype(np.float64)) ** 2 + W * (dz * t["ty"].astype(np.float64)) ** 2))
+        assert abs(r["trace"][0, 9] - want) < 2e-5 * max(abs(want), 1e-3), (r["trace"][0, 9], want)   # fp32 inputs
+        return r["niter"], r["trace"][0, 9], r["trace"][0, 10]
+
+    # |dz| = 5 um > 1 um while |dchi2| ~ 1e-3 < 0.01: must go on ("or" in the rule, or a rule on dchi2 alone, stops at 1)
+    ni, dc, dz = run(0.0, 0.005)
+    assert abs(dc) < 0.01 and abs(dz) > 0.001 and ni == 2
+    # |dz| = 0.5 um < 1 um while |dchi2| = 16 > 0.01: must go on ("or", or a rule on dz alone, stops at 1)
+    ni, dc, dz = run(0.1, 0.0005)
+    assert abs(dc) > 0.01 and abs(dz) < 0.001 and ni == 2
+    # both satisfied: stops at once
+    ni, dc, dz = run(0.001, 0.0005)
+    assert abs(dc) < 0.01 and abs(dz) < 0.001 and ni == 1
+    # the thresholds themselves: |dchi2| = 0.0075 stops (a dchi2 computed 2x too large would not) ...
+    ni, dc, dz = run(np.sqrt(0.0075 / (n * W)), 0.0)
+    assert 0.007 < abs(dc) < 0.008 and ni == 1
+    # ... and |dchi2| = 0.015 goes on (a dchi2 computed 2x too small would stop)
+    ni, dc, dz = run(np.sqrt(0.015 / (n * W)), 0.0)
+    assert 0.014 < abs(dc) < 0.016 and ni == 2
+    # same for dz: 0.75 um stops, 1.5 um goes on (dchi2 ~ 1e-4 in both)
+    assert run(0.0, 0.00075)[0] == 1 and run(0.0, 0.0015)[0] == 2
+
+
 def test_fit_invariants(oracle, cfg0, cfg0_oracle):
     """dchi2 <= 0 (Eq. 17 with positive-definite A), C symmetric positive definite, iterations in 1..10,
     'typically three to seven' (L225)."""
