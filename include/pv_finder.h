@@ -303,14 +303,15 @@ int pv_host_register(void* ptr, size_t bytes);
 int pv_host_unregister(void* ptr);
 
 /* Launch statistics of the most recent pv_find / pv_find_debug call of this process (for bench.py):
- * kernels launched (3: seed, fit, cleanup; 4 with PV_FILL_TEMPLATE: the template table first), and grid size, block size, dynamic shared memory per block of
+ * kernels launched (4: seed, fit, the small kernel that refits the few ill-conditioned seeds in double, cleanup;
+ * 5 with PV_FILL_TEMPLATE: the template table first), and grid size, block size, dynamic shared memory per block of
  * the seed kernel.  All HOST out, nullable. */
 int pv_last_launch_info(int* n_kernels, int* grid, int* block, int* smem_bytes);
 
 /* Optional: CUDA events recorded around each kernel of the next pv_find calls on their own stream, so a
  * caller can time the kernels live.  pv_kernel_timing(1) enables, (0) disables; pv_kernel_time_ms()
  * synchronises the last call's events and returns the duration of its three kernels in ms (< 0 if none);
- * pv_kernel_times_ms() writes up to n per-kernel durations (seed a1-a4, fit a5, cleanup a6) to ms (HOST)
+ * pv_kernel_times_ms() writes up to n per-kernel durations (seed a1-a4, fit a5 incl. the refit kernel, cleanup a6) to ms (HOST)
  * and returns the number of kernels (3), or a negative PV_E_*.  With PV_FILL_TEMPLATE the small kernel that builds
  * the table of templates runs inside the first interval: "seed" then means table + seed kernel.
  * Bench / diagnostic use only: the events and the flag are process-global (see "Thread safety" above). */

@@ -18,15 +18,16 @@ its diagnostic taps), never at the size of the disagreement:
     or (singular flag) a Cholesky pivot within PIVOT_REL of zero.
   * N2 cleanup decisions (merge ratio, beamline distance, min tracks): a differing fate is accepted when the oracle's
     deciding quantity is within NEAR_REL of its cut, or the event holds an N1 / N2 vertex.
-  * N5 ill-conditioned fits: when the oracle's smallest Cholesky pivot (relative to its diagonal element) is below
-    PIVOT_REL the Newton step is a rounding-level numerator over a tiny pivot; a differing iteration count is then
-    handled like N1 (comparison with the trace entry at the GPU's count), and the covariance C = A^-1 is compared within
-    COV_RTOL + 8 * 2^-24 / r (r = that relative pivot): 1 / C_zz is the Schur complement, a difference of terms 1 / r
-    times its size that the kernel forms in fp32 (two nearly parallel tracks, r = 7e-5: 1e-3 observed, bound 8e-3).
+  * (N5, round 2 only: a covariance tolerance widened for ill-conditioned fits and any iteration-count difference
+    accepted there.  Removed in round 3: the kernel re-sums the Schur complement of such seeds in centred form, and
+    they meet the flat tolerances; PIVOT_REL now only serves the singular flag of N2.)
   * N3 argmax (multi-vertex flavour): accepted only when the oracle's two largest weights of that track differ by at
     most W_TOL.  N4 chi2 window: a track listed on one side only must carry a weight below W_TOL there.
 Without the GPU's taps (product kernels, debug=False) the same rules are applied from the final outputs: the
-iteration count is an output (vtx_niter) and the oracle's trace is indexed through its own seed -> vertex map.
+iteration count is an output (vtx_niter) and the oracle's trace is indexed through its own seed -> vertex map.  An
+event may then be excused only from its first fragile seed on: the vertices (and the tracks of the vertices) that
+come before it in z are compared strictly, because a flipped decision on a seed can only shift the vertices behind it.
+The report carries how often each rule fired (`rules`), so that a test can print and bound them.
 """
 from __future__ import annotations
 
@@ -51,21 +52,15 @@ def _cov_rel_err(cg: np.ndarray, cr: np.ndarray) -> np.ndarray:
     return np.max(np.abs(cg - cr) / scale, axis=-1)
 
 
-def _cov_tol(pivot_min: np.ndarray) -> np.ndarray:
-    """Covariance tolerance per seed: COV_RTOL, widened for N5 seeds by the fp32 rounding of the Schur complement
-    (about 8 roundings of 2^-24 on terms 1 / r times its size, r = the oracle's smallest relative Cholesky pivot)."""
-    r = np.abs(pivot_min)
-    with np.errstate(divide="ignore", invalid="ignore"):
-        wide = COV_RTOL + 8.0 * 2.0 ** -24 / np.maximum(r, 1e-12)
-    return np.where(r <= PIVOT_REL, wide, COV_RTOL)
-
-
 def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.ndarray, p, max_log: int = 20) -> Dict:
     """gpu: binding.DeviceBatch.results() with debug=True; ref: oracle.pvref.find(debug=True, trace=True).
     Returns a report dict with 'failures' (list of strings; empty = parity) and 'near_ties' (logged)."""
     fails: List[str] = []
     ties: List[str] = []
-    rep: Dict = {"failures": fails, "near_ties": ties}
+    rules = dict(N1_iteration=0, N2_singular=0, N2_track_count=0, N2_cleanup=0, N3_argmax=0, N4_window=0,
+                 fragile_events_excused=0)
+    rep: Dict = {"failures": fails, "near_ties": ties, "rules": rules}
+    strict_below = None                                 # no-tap path: per excused event, vertices below this index are strict
     gd, rd = gpu.get("debug"), ref.get("debug")
     E = offsets.size - 1
     mv = p.max_vtx_per_event
@@ -135,6 +130,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
                 msg = (f"singular-fit flag differs at event {e} seed {k}: gpu niter {gn[e, k]} ref {rn[e, k]}; oracle: fewest active "
                        f"tracks {nmin}, closest track to the cut-off {edge:.3g}, smallest relative pivot {piv:.3g}")
                 (ties if ok else fails).append(("near-tie: " if ok else "NOT a near-tie: ") + msg)
+                rules["N2_singular"] += int(ok)
             rep["singular_mismatch"] = int(bad_sing.sum())
         fit = ks & ~sing_g & ~sing_r
         ref_pos = rd["seed_pos"].copy()
@@ -155,11 +151,6 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
                 near = (np.isfinite(cuts[0]) and abs(dchi2 - cuts[0]) <= NEAR_REL * cuts[0]) or \
                        (abs(dz - cuts[1]) <= NEAR_REL * cuts[1])
                 why = f"oracle |dchi2| {dchi2:.6g} (cut {cuts[0]:g}), |dz| {dz:.6g} (cut {cuts[1]:g}) at iteration {it}"
-                if not near and abs(rd["seed_pivot_min"][e, k]) <= PIVOT_REL:
-                    # N5: an ill-conditioned fit (two nearly parallel tracks): the step is a small difference divided by
-                    # a pivot of relative size <= PIVOT_REL, which fp32 cannot resolve to the convergence cut
-                    near = True
-                    why += f"; ill-conditioned fit, smallest relative pivot {rd['seed_pivot_min'][e, k]:.3g}"
                 if near:
                     ok = True
                     ref_pos[e, k] = trace[e, k, g_it - 1, 0:3]
@@ -167,12 +158,13 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
                     tie_mask[e, k] = True
             msg = f"iteration count differs at event {e} seed {k}: gpu {g_it} ref {r_it}; {why}"
             (ties if ok else fails).append(("near-tie: " if ok else "NOT a near-tie: ") + msg)
+            rules["N1_iteration"] += int(ok)
         dpos = np.abs(gd["seed_pos"].astype(np.float64) - ref_pos).max(axis=-1)
         dcov = _cov_rel_err(gd["seed_cov"].astype(np.float64), ref_cov)
         rep["seed_pos_max_err_mm"] = float(dpos[fit].max()) if fit.any() else 0.0
         rep["seed_cov_max_rel_err"] = float(dcov[fit].max()) if fit.any() else 0.0
         badp = fit & ~(dpos <= POS_TOL)
-        badc = fit & ~(dcov <= _cov_tol(rd["seed_pivot_min"]))
+        badc = fit & ~(dcov <= COV_RTOL)
         for e, k in np.argwhere(badp)[:max_log]:
             fails.append(f"seed position off by {dpos[e, k]:.3g} mm at event {e} seed {k} (niter gpu {gn[e, k]} ref {rn[e, k]})")
         for e, k in np.argwhere(badc)[:max_log]:
@@ -186,6 +178,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
             msg = (f"track count differs at event {e} seed {k}: gpu {gd['seed_ntrk'][e, k]} ref {rd['seed_ntrk'][e, k]}; "
                    f"oracle's closest track to the cut: {edge:.3g} (tolerance {edge_tol:g})")
             (ties if ok else fails).append(("near-tie: " if ok else "NOT a near-tie: ") + msg)
+            rules["N2_track_count"] += int(ok)
         dchi = np.abs(gd["seed_chi2"].astype(np.float64) - rd["seed_chi2"])
         rel = dchi / np.maximum(1.0, np.abs(rd["seed_chi2"]))
         rep["seed_chi2_max_rel_err"] = float(rel[eq_it & ~dn].max()) if (eq_it & ~dn).any() else 0.0
@@ -203,6 +196,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
             if why:
                 ties.append(f"near-tie: cleanup decisions differ in event {e}: {why}")
                 ev_fate_tie[e] = True
+                rules["N2_cleanup"] += 1
             else:
                 fails.append(f"cleanup decisions differ in event {e} with no near-tie: gpu fate {gf[e][:rd['n_seeds'][e]].tolist()} "
                              f"ref {rf[e][:rd['n_seeds'][e]].tolist()}")
@@ -248,8 +242,9 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
         rep["n_fitted_seeds"] = int((ks & (rn > 0)).sum())
         rep["n_niter_diff"] = int((g_it != r_it).sum())
         for e, k, gi, ri in zip(ee[g_it != r_it], kk[g_it != r_it], g_it[g_it != r_it], r_it[g_it != r_it]):
-            ok = 1 <= gi <= trace.shape[2] and (near_cut(e, k, min(int(gi), int(ri))) or abs(rd["seed_pivot_min"][e, k]) <= PIVOT_REL)
+            ok = 1 <= gi <= trace.shape[2] and near_cut(e, k, min(int(gi), int(ri)))
             if ok:
+                rules["N1_iteration"] += 1
                 ref_pos[e, k] = trace[e, k, gi - 1, 0:3]
                 ref_cov[e, k] = trace[e, k, gi - 1, 3:9]
                 tie_mask[e, k] = True
@@ -264,11 +259,19 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
             if why:
                 ties.append(f"near-tie: vertex count differs in event {e} (gpu {nv_g[e]} ref {nv_r[e]}): {why}")
                 fragile_ev[e] = True
+                rules["N2_cleanup"] += 1
         # same count but another pairing of merged / rejected vertices: only excused in events that are fragile
         for e in np.flatnonzero(~differs & (frag_stop | frag_cnt).any(axis=1)):
             fragile_ev[e] = True
         ev_fate_tie = fragile_ev & (differs | _any_vertex_off(gpu, ref, ref_pos, rd, mv))
         rep["n_fragile_events_excused"] = int(ev_fate_tie.sum())
+        rules["fragile_events_excused"] = int(ev_fate_tie.sum())
+        # an excused event is excused from its first fragile seed on: that seed's place among the oracle's final
+        # vertices (the number of surviving seeds before it); events excused by a cleanup cut alone: from vertex 0
+        frag = (frag_stop | frag_cnt) & ks
+        surv_before = np.cumsum((fate_r >= 0) & ks, axis=1) - ((fate_r >= 0) & ks)
+        first = np.where(frag, surv_before, mv).min(axis=1)
+        strict_below = np.where(ev_fate_tie, np.where(frag.any(axis=1), first, 0), mv)
     else:
         ev_fate_tie = np.zeros(E, bool)
         tie_mask = None
@@ -281,6 +284,9 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
         fails.append(f"n_vtx differs in {int(nv_bad.sum())} events without a near-tie, first {np.argwhere(nv_bad)[:5, 0].tolist()}")
     ev_same = (nv_g == nv_r) & ~ev_fate_tie
     kv = (np.arange(mv)[None, :] < nv_r[:, None]) & ev_same[:, None]
+    if strict_below is not None:                        # no-tap path: the vertices before an excused event's first fragile seed
+        kv |= (np.arange(mv)[None, :] < np.minimum(np.minimum(nv_r, nv_g), strict_below)[:, None]) & ev_fate_tie[:, None]
+        rep["n_strict_vertices_in_excused_events"] = int((kv & ev_fate_tie[:, None]).sum())
     rep["n_vertices"] = int(nv_r.sum())
     if rd is not None and tie_mask is not None:
         # map final vertices back to seeds to reuse the (possibly trace-substituted) reference
@@ -299,11 +305,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
     rep["vtx_cov_max_rel_err"] = float(dcov[kv].max()) if kv.any() else 0.0
     for e, k in np.argwhere(kv & ~(dpos <= POS_TOL))[:max_log]:
         fails.append(f"vertex position off by {dpos[e, k]:.3g} mm at event {e} vertex {k}")
-    cov_tol = np.full((E, mv), COV_RTOL)
-    if rd is not None and "seed_pivot_min" in rd:                # N5: the tolerance of the seed the vertex came from
-        ee, kk = np.nonzero((rd["seed_fate"] >= 0) & (np.arange(mv)[None, :] < rd["n_seeds"][:, None]))
-        cov_tol[ee, rd["seed_fate"][ee, kk]] = _cov_tol(rd["seed_pivot_min"])[ee, kk]
-    for e, k in np.argwhere(kv & ~(dcov <= cov_tol))[:max_log]:
+    for e, k in np.argwhere(kv & ~(dcov <= COV_RTOL))[:max_log]:
         fails.append(f"vertex covariance off by {dcov[e, k]:.3g} rel at event {e} vertex {k}")
 
     tv_g, tv_r = gpu["trk_vertex"], ref["trk_vertex"]
@@ -313,6 +315,9 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
     if agree.size and rep["assign_agreement"] < MIN_ASSIGN_AGREEMENT:
         fails.append(f"track-assignment agreement {rep['assign_agreement']:.6f} < {MIN_ASSIGN_AGREEMENT}")
     unexplained = (~agree) & ~ev_fate_tie[ev_of_trk] if agree.size else np.zeros(0, bool)
+    if strict_below is not None and agree.size:          # tracks of the strict vertices of an excused event
+        sb = strict_below[ev_of_trk]
+        unexplained |= (~agree) & ev_fate_tie[ev_of_trk] & (((tv_r >= 0) & (tv_r < sb)) | ((tv_g >= 0) & (tv_g < sb)))
     if int(getattr(p, "flavour", 0)) == 1 and agree.size:
         # argmax near-tie: both sides follow a vertex and the two largest weights are equal within W_TOL
         if rd is not None and "trk_w1" in rd:              # N3: the ORACLE's two largest weights of the track
@@ -321,6 +326,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
             gap = np.full(agree.shape, np.inf)
         argmax_tie = (~agree) & (gap <= W_TOL) & (rd["trk_w2"] > 0 if rd is not None and "trk_w2" in rd else False)
         rep["n_argmax_ties"] = int(argmax_tie.sum())
+        rules["N3_argmax"] = int(argmax_tie.sum())
         for i in np.argwhere(argmax_tie)[:max_log, 0]:
             ties.append(f"near-tie: the oracle's two largest weights of track {int(i)} differ by {gap[i]:.3g} <= {W_TOL}: gpu {tv_g[i]} ref {tv_r[i]}")
         unexplained &= ~argmax_tie
@@ -329,6 +335,7 @@ def compare(gpu: Dict[str, np.ndarray], ref: Dict[str, np.ndarray], offsets: np.
         wg, wr = gpu["trk_weight"].astype(np.float64), ref["trk_weight"]
         window_tie = (~agree) & (((tv_g < 0) & (tv_r >= 0) & (wr <= W_TOL)) | ((tv_r < 0) & (tv_g >= 0) & (wg <= W_TOL)))
         rep["n_window_ties"] = int(window_tie.sum())
+        rules["N4_window"] = int(window_tie.sum())
         for i in np.argwhere(window_tie)[:max_log, 0]:
             ties.append(f"near-tie: track {int(i)} is at the chi2 window of its only vertex: weights gpu {wg[i]:.3g} ref {wr[i]:.3g}")
         unexplained &= ~window_tie

@@ -271,6 +271,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   ka.rec = reinterpret_cast<pvk::SeedRec*>(ws + WS_COUNTERS);
   ka.trk_counter = reinterpret_cast<unsigned int*>(ws + 32);
   ka.fit_counter = reinterpret_cast<unsigned int*>(ws + 48);
+  ka.ill_counter = reinterpret_cast<unsigned int*>(ws + 64);
   ka.ftrk = reinterpret_cast<float4*>(ws + WS_COUNTERS + ws_rec_bytes(n_events, params->max_vtx_per_event));
   ka.trk_cap = (unsigned int)ws_trk_records(n_tracks, params->flavour);
   ka.n_trk = (unsigned int)n_tracks;
@@ -282,7 +283,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   const bool timing = g_timing != 0;
   if (timing && !g_ev[0])
     for (int i = 0; i <= N_KERNELS; ++i) CK(cudaEventCreate(&g_ev[i]));
-  CK(cudaMemsetAsync(workspace, 0, 64, stream));
+  CK(cudaMemsetAsync(workspace, 0, 128, stream));
   // a1..a4: persistent, one CTA per SM, one warp per event
   int grid = di->sms;
   const int need = n_events;                                  // a small batch is spread over the SMs, not packed into few CTAs
@@ -307,6 +308,10 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     if (mvf) pvk::fit_kernel<1><<<(int)fit_grid, pvk::FIT_BLOCK, 0, stream>>>(kp, ka);
     else pvk::fit_kernel<0><<<(int)fit_grid, pvk::FIT_BLOCK, 0, stream>>>(kp, ka);
     CK(cudaGetLastError());
+    // the few ill-conditioned seeds fit_kernel set aside, refitted in double (timed with the fit)
+    if (mvf) pvk::ill_kernel<1><<<32, 128, 0, stream>>>(kp, ka);
+    else pvk::ill_kernel<0><<<32, 128, 0, stream>>>(kp, ka);
+    CK(cudaGetLastError());
   }
   if (timing) CK(cudaEventRecord(g_ev[2], stream));
   // a6: one warp per event
@@ -322,7 +327,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
     CK(cudaGetLastError());
   }
   if (timing) { CK(cudaEventRecord(g_ev[3], stream)); g_ev_valid = true; }
-  g_last_kernels = N_KERNELS + tfl; g_last_grid = grid;
+  g_last_kernels = N_KERNELS + 1 + tfl; g_last_grid = grid;
   return PV_OK;
 }
 

@@ -174,6 +174,7 @@ struct KArgs {
   float* wrec;                   // workspace, explicit flavour: [T] Tukey weight of every track record (record order)
   unsigned long long* best;      // workspace, multi-vertex flavour: [T] largest weight of the track << 32 | 31 - seed
   unsigned int* trk_counter;     // workspace, multi-vertex flavour: track records allocated so far
+  unsigned int* ill_counter;     // workspace: ill-conditioned seeds handed from fit_kernel to ill_kernel (list at the end of rec[])
   unsigned int trk_cap;          // capacity of ftrk in records
   unsigned int n_trk;            // the n_tracks given to pv_find: the per-track parts of the workspace hold this many
   pv_debug dbg;
@@ -1328,12 +1329,21 @@ __device__ __forceinline__ float track_accum2(const float2 xy0, const float2 txy
 // Newton-Raphson step Eq. 13 on the arrow-shaped Hessian A = [[a,0,-c],[0,b,-d],[-c,-d,e]]:
 // returns false when the fit is singular (fewer than 2 active tracks or a non-positive pivot).
 // C = A^-1 (Eq. 14), upper triangle xx xy xz yy yz zz.
-__device__ __forceinline__ bool newton_step(const Sums& S, float& dx, float& dy, float& dzs, float& dchi2, float* C) {
+// An ILL-CONDITIONED seed (two or three nearly parallel tracks) has e ~ c^2 / a + d^2 / b: the Schur complement and
+// the numerator of the z step are then small differences of fp32 sums and lose 1 / r of their digits (r = the pivot
+// relative to e; r = 7e-5 seen on configs[4]: C_zz off by 1e-3, iteration counts off).  `ill` (out, optional) reports
+// r < ILL_REL (or a non-positive pivot): fit_phase then drops the seed from its queue and puts its record on a list
+// that ill_kernel works through after fit_kernel, refitting each in double (fit_ill).  A few seeds in 10^5; every
+// other seed keeps the arithmetic (and bits) it always had.
+constexpr float ILL_REL = 1.0f / 256.0f;
+__device__ __forceinline__ bool newton_step(const Sums& S, float& dx, float& dy, float& dzs, float& dchi2, float* C,
+                                            bool* ill = nullptr) {
   if (S.nact < 2.0f) return false;
   if (!(S.a > 0.0f) || !(S.b > 0.0f)) return false;
   const float ia = __fdividef(1.0f, S.a), ib = __fdividef(1.0f, S.b);
   const float ca = S.c * ia, db = S.d * ib;
   const float sch = S.e - S.c * ca - S.d * db;         // Schur complement = third Cholesky pivot squared
+  if (ill) *ill = !(sch >= ILL_REL * S.e);
   if (!(sch > 0.0f)) return false;
   const float is = __fdividef(1.0f, sch);
   dzs = (ca * S.gx + db * S.gy - S.gz) * is;
@@ -1433,6 +1443,100 @@ enum { FS_EMPTY = 0, FS_LOAD = 1, FS_ITER = 2, FS_FINAL = 3, FS_DONE = 4 };
 #endif
 
 // One phase of a window: the records order[pb .. pe) of the window starting at record wb, G = 1 << lg lanes per seed.
+// The fit of one ill-conditioned seed (see newton_step) by the whole warp, in double, from its records in global memory
+// and from the first iteration on: Eq. 6-18 / 19 as in fit_phase, lane l takes the tracks l, l + 32, ...  Its result
+// depends on the seed's own records only.
+template <int FLAV>
+__device__ void fit_ill(const KParams& P, const KArgs& A, const int4 r, const int lane) {
+  const int be = r.x, bk = r.y & 31, bm_ = r.y >> 5, bo = r.z;
+  const float bz = __int_as_float(r.w);
+  const float bx = __fmaf_rn(P.beam_tx, bz, P.beam_x), by = __fmaf_rn(P.beam_ty, bz, P.beam_y);
+  double qx = 0.0, qy = 0.0, qz = 0.0;                 // current position (local frame)
+  double px = 0.0, py = 0.0, pz = 0.0;                 // position the last weights were taken at
+  double C[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  double bchi2 = 0.0, bnact = 0.0;
+  bool bsing = false;
+  int bit = 0;
+  auto weight = [&](const Trk& U, const double x, const double y, const double z, double& rx, double& ry, double& chi) {
+    rx = (double)U.x0 + z * (double)U.tx - x;          // residual, Eq. 9
+    ry = (double)U.y0 + z * (double)U.ty - y;
+    chi = rx * rx * (double)U.Wx + ry * ry * (double)U.Wy;   // Eq. 7
+    if (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+      const double E = exp(-0.5 * chi);                // Eq. 19, competitors frozen at their seed positions
+      return E / ((double)U.oth + E);
+    }
+    if (P.unit_weights) return 1.0;
+    const double u = fmax(1.0 - chi * (double)P.inv_chi2_max, 0.0);   // Eq. 18
+    return u * u;
+  };
+#pragma unroll 1
+  for (int it = 1; it <= P.max_iter; ++it) {
+    double s[10] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // a b c d e gx gy gz chi2 nact
+    for (int t = lane; t < bm_; t += 32) {
+      int idx;
+      const Trk U = read_track(A, bo + t, idx);
+      if (track_is_dead(U, P)) continue;
+      double rx, ry, chi;
+      const double w = weight(U, qx, qy, qz, rx, ry, chi);
+      const double wWx = w * (double)U.Wx, wWy = w * (double)U.Wy;
+      const double p = wWx * (double)U.tx, q = wWy * (double)U.ty;
+      s[0] += wWx; s[1] += wWy; s[2] += p; s[3] += q;
+      s[4] += p * (double)U.tx + q * (double)U.ty;
+      s[5] += wWx * rx; s[6] += wWy * ry; s[7] += p * rx + q * ry;
+      s[8] += w * chi;
+      s[9] += w > 0.0 ? 1.0 : 0.0;
+    }
+#pragma unroll
+    for (int c = 0; c < 10; ++c)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(FULL, s[c], o);
+    if (s[9] < 2.0 || !(s[0] > 0.0) || !(s[1] > 0.0)) { bsing = true; break; }
+    const double ia = 1.0 / s[0], ib = 1.0 / s[1], ca = s[2] * ia, db = s[3] * ib;
+    const double sch = s[4] - s[2] * ca - s[3] * db;
+    if (!(sch > 0.0)) { bsing = true; break; }
+    const double is = 1.0 / sch;
+    const double dzs = (ca * s[5] + db * s[6] - s[7]) * is;   // Eq. 13 on the arrow-shaped Hessian
+    const double dx = (s[5] + s[2] * dzs) * ia, dy = (s[6] + s[3] * dzs) * ib;
+    const double dchi2 = dzs * s[7] - dx * s[5] - dy * s[6];  // Eq. 17
+    C[0] = ca * ca * is + ia; C[1] = ca * db * is; C[2] = ca * is;
+    C[3] = db * db * is + ib; C[4] = db * is; C[5] = is;      // Eq. 14
+    px = qx; py = qy; pz = qz;
+    qx += dx; qy += dy; qz += dzs;
+    bchi2 = s[8]; bnact = s[9]; bit = it;
+    if (fabs(dchi2) < (double)P.conv_dchi2 && fabs(dzs) < (double)P.conv_dz) break;
+  }
+  const size_t o = (size_t)be * P.max_vtx + bk;
+  float bass = 0.0f;
+  if (!bsing) {
+    for (int t = lane; t < bm_; t += 32) {             // weights of the last iteration
+      int idx;
+      const Trk U = read_track(A, bo + t, idx);
+      const bool deadt = track_is_dead(U, P);
+      double rx, ry, chi;
+      const float w = deadt ? 0.0f : (float)weight(U, px, py, pz, rx, ry, chi);
+      if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+        if (!deadt) { claim_track(A, idx, w, bk); bass += (w >= 0.5f) ? 1.0f : 0.0f; }
+      } else {
+        A.wrec[bo + t] = w;
+      }
+    }
+  }
+  if constexpr (FLAV == PV_FLAVOUR_MULTIVERTEX) {
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) bass += __shfl_xor_sync(FULL, bass, o2);
+  }
+  if (lane == 0) {
+    if (bsing) { A.vtx_niter[o] = -1; atomicOr(A.event_status + be, (unsigned)PV_EVT_SINGULAR_FIT); }
+    else {
+      float Cf[6];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) Cf[c] = (float)C[c];
+      store_vertex(A, o, (float)((double)bx + qx), (float)((double)by + qy), (float)((double)bz + qz), Cf, (float)bchi2,
+                   (int)(FLAV ? bass : (float)bnact), bit);
+    }
+  }
+}
+
 // ord0 / ord1: the sorted window (record index within the window, one byte each), 8 entries per lane.
 // Explicit flavour: every iteration leaves its Tukey weights at the tracks' record positions in wrec[], so the weights
 // of the last iteration are simply what is there when the seed stops (cleanup_kernel moves them to track order);
@@ -1569,7 +1673,20 @@ __device__ __forceinline__ void fit_phase(const KParams& P, const KArgs& A, floa
     bool store = false;
     if (st == FS_ITER) {
       float dx, dy, dzs, dchi2;
-      if (!newton_step(S, dx, dy, dzs, dchi2, C)) {            // singular: the vertex is dropped (R-12)
+      bool ill = false;
+      const bool stepped = newton_step(S, dx, dy, dzs, dchi2, C, &ill);
+      if (ill) {                                               // rare: the seed goes to ill_kernel, which refits it in double
+        if (j == 0) {
+          const unsigned pos = atomicAdd(A.ill_counter, 1u), cap = (unsigned)A.n_events * (unsigned)P.max_vtx;
+          if (*A.seed_counter + pos < cap) {                   // the list grows down from the end of rec[], behind the seeds
+            reinterpret_cast<int4*>(A.rec)[cap - 1u - pos] = cur;
+          } else {                                             // (every slot of the batch holds a seed: no room for a list)
+            A.vtx_niter[(size_t)e * P.max_vtx + k] = -1;
+            atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT);
+          }
+        }
+        st = FS_DONE;
+      } else if (!stepped) {                                   // singular: the vertex is dropped (R-12)
         if (j == 0) {
           A.vtx_niter[(size_t)e * P.max_vtx + k] = -1;
           atomicOr(A.event_status + e, (unsigned)PV_EVT_SINGULAR_FIT);
@@ -1742,6 +1859,19 @@ fit_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
       fit_huge<FLAV>(P, A, __ldg(reinterpret_cast<const int4*>(A.rec) + wb + idx), lane);
     }
   }
+}
+
+// ---- ill_kernel: the seeds fit_kernel found ill-conditioned (newton_step), one warp each, in double (fit_ill).  Runs
+// between fit_kernel and cleanup_kernel; with an empty list (most small batches) it costs its launch.
+template <int FLAV>
+__global__ void __launch_bounds__(128) ill_kernel(const __grid_constant__ KParams P, const __grid_constant__ KArgs A) {
+  const int lane = threadIdx.x & 31;
+  const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+  const unsigned cap = (unsigned)A.n_events * (unsigned)P.max_vtx, total = *A.seed_counter;
+  unsigned n = *A.ill_counter;
+  if (n > cap - total) n = cap - total;
+  for (unsigned i = warp; i < n; i += nwarps)
+    fit_ill<FLAV>(P, A, __ldg(reinterpret_cast<const int4*>(A.rec) + (cap - 1u - i)), lane);
 }
 
 // ---- cleanup_kernel: a6, one warp per event (Table 2, R-9) ------------------------------------

@@ -1,6 +1,7 @@
 """Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
 All tests here need a B200 (`-m gpu`)."""
 import dataclasses
+import json
 import os
 
 import numpy as np
@@ -35,9 +36,22 @@ def _both(pv, oracle, data, n_hist=None, **over):
     return got, ref, rep
 
 
+def _log_rules(rep, **extra):
+    """One JSON line per comparison: how often each near-tie rule of the comparator fired (also appended to the file
+    named by PV_PARITY_LOG, so that a run can be summarised in DESIGN.md section 6)."""
+    test = os.environ.get("PYTEST_CURRENT_TEST", "").split("::")[-1].replace(" (call)", "")
+    line = json.dumps(dict(test=test, fitted_seeds=rep.get("n_fitted_seeds"), vertices=rep.get("n_vertices"),
+                           near_ties=rep.get("n_near_ties"), rules=rep.get("rules"), failures=len(rep["failures"]), **extra))
+    print("PARITY_RULES", line)
+    if os.environ.get("PV_PARITY_LOG"):
+        with open(os.environ["PV_PARITY_LOG"], "a") as f:
+            f.write(line + "\n")
+
+
 def _assert_parity(rep, allow_ties_frac=5e-4):
     """No failure, and no more logged near-ties than twice the largest rate measured on B200 (2e-4 of the fitted
     seeds, multi-vertex flavour on high pile-up; 1e-5 on configs[1] at full size; 0 on most cases)."""
+    _log_rules(rep)
     assert not rep["failures"], "\n".join(rep["failures"][:10])
     for t in rep["near_ties"][:10]:
         print("LOGGED", t)
@@ -528,13 +542,54 @@ def test_full_size_throughput_config(pv, oracle, mode):
     p, po = (pv.default_params(), oracle.default_params()) if mode == "explicit" else (pv.multivertex_params(), oracle.mv_params())
     got = pv.find(data, p)
     info = pv.last_launch_info()
-    assert info["n_kernels"] == 3 and info["grid"] >= 100
+    assert info["n_kernels"] == 4 and info["grid"] >= 100
     ref = oracle.find(data, po, debug=True, trace=True, n_threads=NTHREADS)
     rep = compare.compare(got, ref, data["offsets"], p)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})
     _assert_parity(rep)
     assert rep["assign_agreement"] >= 0.999 and rep["n_vertices"] > 500_000
+    # events excused from their first fragile seed on: twice the number measured on B200 (round 3: FRAGILE_MEASURED)
     assert rep["n_fragile_events_excused"] <= 0.002 * 100_000
+
+
+@pytest.mark.parametrize("mode", ["explicit", "multivertex"])
+def test_one_million_events(pv, oracle, mode):
+    """configs[4] at its largest batch (10^6 events, 1.15 10^8 tracks: track-record indices up to 1.15 10^8, twice that
+    in the multi-vertex flavour) through the product kernels against the oracle run without taps or trace (the trace
+    alone would be 45 GB).  Without the oracle's deciding quantities no near-tie can be explained, so the check is the
+    one that holds at any size: the vertex count differs in fewer than 2 in 10^4 events (the near-tie rate measured with
+    taps at 10^5 events), assignment agrees on >= 99.9 % of the tracks, and every vertex of an event with the same
+    count and the same iteration counts meets the position and covariance tolerances."""
+    from oracle import compare
+    data = events.generate(events.config(4, 1_000_000))
+    p, po = (pv.default_params(), oracle.default_params()) if mode == "explicit" else (pv.multivertex_params(), oracle.mv_params())
+    got = pv.find(data, p)
+    ref = oracle.find(data, po, n_threads=NTHREADS)
+    E, mv = 1_000_000, p.max_vtx_per_event
+    assert int(data["offsets"][-1]) > 100_000_000
+    assert np.array_equal(got["event_status"] & ~np.uint32(4), ref["event_status"] & ~np.uint32(4))
+    same_n = got["n_vtx"] == ref["n_vtx"]
+    agree = float((got["trk_vertex"] == ref["trk_vertex"]).mean())
+    m = (np.arange(mv)[None, :] < ref["n_vtx"][:, None]) & same_n[:, None]
+    same_it = np.where(m, got["vtx_niter"] == ref["vtx_niter"], True).all(axis=1)
+    m &= same_it[:, None]
+    dpos = np.abs(got["vtx_pos"].astype(np.float64) - ref["vtx_pos"]).max(axis=-1)
+    dcov = compare._cov_rel_err(got["vtx_cov"].astype(np.float64), ref["vtx_cov"])
+    bad = m & ~((dpos <= compare.POS_TOL) & (dcov <= compare.COV_RTOL))
+    summary = dict(test=f"test_one_million_events[{mode}]", events=E, vertices=int(ref["n_vtx"].sum()),
+                   n_vtx_differs=int((~same_n).sum()), niter_differs_events=int((same_n & ~same_it).sum()),
+                   assign_agreement=agree, vertices_compared=int(m.sum()), vertices_off=int(bad.sum()),
+                   pos_max_err_mm=float(dpos[m & ~bad].max()), cov_max_rel_err=float(dcov[m & ~bad].max()))
+    print("PARITY_1M", json.dumps(summary))
+    if os.environ.get("PV_PARITY_LOG"):
+        with open(os.environ["PV_PARITY_LOG"], "a") as f:
+            f.write(json.dumps(summary) + "\n")
+    assert (~same_n).sum() <= 2e-4 * E, summary
+    assert agree >= 0.999, summary
+    assert m.sum() >= 0.97 * ref["n_vtx"].sum(), summary
+    # a vertex off with equal counts is an event whose cleanup paired the seeds differently (a near-tie upstream):
+    # as rare as the differing counts
+    assert bad.sum() <= 2e-4 * E, (summary, np.argwhere(bad)[:5].tolist())
 
 
 @pytest.mark.parametrize("mode", ["explicit", "multivertex", "recursive", "recursive_multivertex", "template", "template_recursive_multivertex"])
@@ -687,7 +742,7 @@ def test_template_fill(pv, oracle, idx, n, mv):
     mk_p, mk_o = (pv.multivertex_params, oracle.mv_params) if mv else (pv.default_params, oracle.default_params)
     p, po = mk_p(fill_mode=1), mk_o(fill_mode=1)
     got = pv.find(data, p, debug=True, n_hist_events=400)
-    assert pv.last_launch_info()["n_kernels"] == 4
+    assert pv.last_launch_info()["n_kernels"] == 5
     ref = oracle.find(data, po, debug=True, n_hist_events=400, trace=True, n_threads=NTHREADS)
     rep = compare.compare(got, ref, np.asarray(data["offsets"]), p)
     print({k: v for k, v in rep.items() if k not in ("failures", "near_ties")})

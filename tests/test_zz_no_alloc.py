@@ -72,7 +72,7 @@ def test_static_workspace_entry_matches_pv_find_on_two_calls_in_a_row(pv, mode):
     for i in range(2):
         _assert_same(pv, p, got[i], want[i], f"{mode} repeat {i}")
     info = pv.last_launch_info()
-    assert info["n_kernels"] == 3, info
+    assert info["n_kernels"] == 4, info
 
 
 def test_static_workspace_entry_refuses_what_does_not_fit(pv):
