@@ -160,20 +160,31 @@ def main_reference(args):
         return
     from synth import events
     cores = os.cpu_count() or 1
-    sample_events = min(args.events or 100_000, 20_000)
-    data, m, _rng, _T = gen_batch(args.config, sample_events)
-    for _ in range(args.warmup):
-        run_oracle(events.slice_events(data, 0, min(2000, sample_events)), cores, args.flavour)
+    data, m, _rng, _T = gen_batch(args.config, args.events)
+    full_events = int(data["offsets"].size - 1)
+    # every step is the workload of the GPU arm whenever the host cores finish it in time (about two minutes for all
+    # steps, judged from the warm-up's rate); otherwise a prefix of it, rounded down to 1000 events
+    rate = 0.0
+    for _ in range(max(args.warmup, 1)):
+        n0 = min(2000, full_events)
+        dt, _r = run_oracle(events.slice_events(data, 0, n0), cores, args.flavour)
+        rate = max(rate, n0 / dt)
+    sample_events = min(full_events, max(1000, int(rate * 120.0 / max(args.steps, 1)) // 1000 * 1000))
+    if sample_events < full_events:
+        data = events.slice_events(data, 0, sample_events)
     t = 0.0
     for _ in range(args.steps):
         dt, _r = run_oracle(data, cores, args.flavour)
         t += dt
     value = sample_events * args.steps / t
-    sample = f"first {sample_events} events of configs[{args.config}] ({m.name}, seed {m.seed}) per step, OpenMP over events"
+    whole = sample_events == full_events
+    sample = (f"{'all' if whole else 'first'} {sample_events} events of configs[{args.config}] ({m.name}, seed {m.seed}) per step, "
+              f"OpenMP over events on {cores} threads")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (fp32 contract for the integer decisions)", "data": "synthetic",
-            "config": {"workload": f"configs[{args.config}] {m.name}: bounded sample of {sample_events} events per step",
+            "config": {"workload": (f"configs[{args.config}] {m.name}: {full_events} events, {_T} tracks, seed {m.seed}" if whole else
+                                    f"configs[{args.config}] {m.name}: bounded sample of {sample_events} of {full_events} events per step"),
                        "events_per_step": sample_events, "flavour": args.flavour},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -345,7 +356,7 @@ def main_ours(args):
     assert sum(alg_k.values()) == alg
     # DRAM bytes per launch from the committed `ncu --set full` capture: accepted only when the capture was made with
     # the kernels of this working tree (hash recorded beside it), else reported as stale
-    traffic_k, inst_k, traffic_src = {}, {}, "none for this workload"
+    traffic_k, inst_k, tinst_k, traffic_src = {}, {}, {}, "none for this workload"
     tpath = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     sha = kernels_sha()
     if os.path.exists(tpath):
@@ -357,6 +368,8 @@ def main_ours(args):
                     traffic_k[row["kernel"]] = int(row["dram_bytes_per_launch"])
                     if row.get("warp_inst_per_launch"):
                         inst_k[row["kernel"]] = int(row["warp_inst_per_launch"])
+                    if row.get("thread_inst_per_launch"):
+                        tinst_k[row["kernel"]] = int(row["thread_inst_per_launch"])
                     traffic_src = f"profiles/{row['source']} (ncu dram__bytes_read.sum + dram__bytes_write.sum, kernels {sha})"
                 else:
                     traffic_src = f"stale: profiles/dram_traffic.csv was captured with kernels {row.get('kernels_sha')}, this tree is {sha}"
@@ -368,15 +381,26 @@ def main_ours(args):
     achieved = dom["achieved_gbs"]
     # what actually binds the path: warp-instructions issued against 148 SMs x 4 schedulers x the
     # SM clock; instruction counts from the same ncu capture as the traffic (same staleness check), time measured live
+    # `issue` is a UTILISATION (every executed instruction counts, the bookkeeping included), not a roofline fraction.
     issue = None
-    if len(inst_k) == len(KERNELS):
-        clk = sampler.summary().get("sm_mhz") or 1965.0
-        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    clk = sampler.summary().get("sm_mhz") or 1965.0
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    if len(inst_k) >= len(KERNELS):
         peak_issue = sms * 4 * clk * 1e6 / 1e9
         ach = sum(inst_k.values()) / (ms_step * 1e-3) / 1e9
-        issue = {"bound": "alu", "achieved": ach, "peak": peak_issue, "unit": "G warp-instructions/s", "frac": ach / peak_issue,
+        issue = {"achieved": ach, "peak": peak_issue, "unit": "G warp-instructions/s", "utilisation": ach / peak_issue,
                  "warp_instructions_per_step": sum(inst_k.values()),
                  "peak_source": f"{sms} SMs x 4 schedulers x {clk:.0f} MHz (one warp-instruction per scheduler and cycle)"}
+    # The ALU roofline of SURVEY.md 8(d): the METHOD's own arithmetic (about 330 fp32 flop per track: projection 25,
+    # fill ~100 for ~8 edges, fit 35 x 5.5 + 10; plus ~10 000 integer operations per event for the peak search)
+    # against the fp32 peak of the SMs.  `overhead` = thread-instructions the kernels executed per algorithmic operation.
+    alg_ops = 330.0 * T + 10_000.0 * E
+    peak_alu = sms * 128 * 2 * clk * 1e6 / 1e12
+    alu = {"bound": "alu", "algorithmic_ops_per_event": alg_ops / E, "achieved": alg_ops / (ms_step * 1e-3) / 1e12,
+           "peak": peak_alu, "unit": "Tops/s", "frac": alg_ops / (ms_step * 1e-3) / 1e12 / peak_alu,
+           "peak_source": f"{sms} SMs x 128 fp32 lanes x 2 (FMA) x {clk:.0f} MHz",
+           "overhead": (sum(tinst_k.values()) / alg_ops) if len(tinst_k) >= len(KERNELS) else None,
+           "overhead_by_kernel": ({k: v / alg_ops for k, v in tinst_k.items()} if len(tinst_k) >= len(KERNELS) else None)}
 
     # ---- cpu_baseline: the oracle, as it stands, on this box's host cores --------------------------------------
     cores = os.cpu_count() or 1
@@ -420,9 +444,10 @@ def main_ours(args):
                      "kernels": kernels,
                      "path": {"algorithmic_bytes_per_step": alg, "ms_per_step": ms_step,
                               "achieved": alg / (ms_step * 1e-3) / 1e9, "frac": alg / (ms_step * 1e-3) / 1e9 / peak},
-                     "issue": issue,
-                     "note": "rank 0's kernels; the path is issue- and latency-bound, not HBM-bound (DESIGN.md section 8; "
-                             "`issue` holds that roofline); BASELINE.json asks for the HBM fraction, reported here"},
+                     "alu": alu, "issue": issue,
+                     "note": "rank 0's kernels; the path is issue- and latency-bound, not HBM-bound (DESIGN.md section 8): "
+                             "`frac` / `path.frac` are the HBM fractions BASELINE.json asks for, `alu.frac` the method's own "
+                             "arithmetic against the fp32 peak, `issue.utilisation` the issue slots the kernels keep busy"},
         "cpu_baseline": cpu,
     }
     if ip_info is not None:

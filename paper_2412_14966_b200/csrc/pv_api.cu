@@ -10,9 +10,17 @@
 #include <mutex>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; the ranges cost nothing measurable when no profiler is attached
+
 #include "pv_kernels.cuh"
 
 namespace {
+
+// NVTX range around the launches of one stage of pv_find: shows up per stage in a timeline.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 thread_local char g_cuda_err[512] = "";
 int g_last_kernels = 0, g_last_grid = 0, g_last_block = 0, g_last_smem = 0;
@@ -290,10 +298,12 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (grid > need) grid = need;
   if (timing) CK(cudaEventRecord(g_ev[0], stream));
   if (tfl) {                                                  // the table of template histograms, ~10^4 entries
+    NvtxRange range("pv_find: template table");
     pvk::tmpl_kernel<<<kp.tmpl_kmax + 1, 256, 0, stream>>>(kp, ka.tmpl);
     CK(cudaGetLastError());
   }
   {
+    NvtxRange range("pv_find: a1-a4 seed");
     void* kargs[2] = {(void*)&kp, (void*)&ka};
     CK(cudaLaunchKernel(seed_fn[which], dim3(grid), dim3(warps * 32), kargs, (size_t)smem, stream));
   }
@@ -301,6 +311,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (timing) CK(cudaEventRecord(g_ev[1], stream));
   // a5: autonomous warps work through windows of seed records
   {
+    NvtxRange range("pv_find: a5 fit");
     long long fit_grid = (long long)di->sms * di->fit_blocks_per_sm[mvf];
     const long long most = ((long long)n_events * params->max_vtx_per_event + pvk::FIT_BLOCK - 1) / pvk::FIT_BLOCK;
     if (fit_grid > most) fit_grid = most;
@@ -316,6 +327,7 @@ int find_impl(const float* x, const float* y, const float* z, const float* tx, c
   if (timing) CK(cudaEventRecord(g_ev[2], stream));
   // a6: one warp per event
   {
+    NvtxRange range("pv_find: a6 cleanup");
     const int cgrid = (n_events + 7) / 8;
     if (mvf) {
       if (dbg) pvk::cleanup_kernel<true, 1><<<cgrid, 256, 0, stream>>>(kp, ka);
