@@ -371,7 +371,7 @@ def main_ours(args):
                     if row.get("thread_inst_per_launch"):
                         tinst_k[row["kernel"]] = int(row["thread_inst_per_launch"])
                     traffic_src = f"profiles/{row['source']} (ncu dram__bytes_read.sum + dram__bytes_write.sum, kernels {sha})"
-                else:
+                elif not traffic_k:                                  # (rows of earlier rounds stay in the file as history)
                     traffic_src = f"stale: profiles/dram_traffic.csv was captured with kernels {row.get('kernels_sha')}, this tree is {sha}"
     ksum = float(kernel_ms.sum())
     kernels = [{"name": n, "ms": float(kernel_ms[i]), "share": float(kernel_ms[i] / ksum),
