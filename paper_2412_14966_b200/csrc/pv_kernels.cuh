@@ -53,6 +53,9 @@ constexpr int DET_UNROLL = PV_DET_UNROLL;
 #ifndef PV_PREFETCH_TRACKS
 #define PV_PREFETCH_TRACKS 128    // tracks of a warp's next event pulled into L2 while the current one is associated
 #endif
+#ifndef PV_BULK_PREFETCH
+#define PV_BULK_PREFETCH 0        // 1: that prefetch as nine cp.async.bulk.prefetch.L2 (TMA unit) instead of 9 x 5 prefetch.global.L2
+#endif                            // lines; measured on configs[1] (profiles/r3_kernels.md)
 #ifndef PV_SEED_WARPS
 #define PV_SEED_WARPS 32
 #endif
@@ -945,12 +948,26 @@ __device__ void seed_event(const int e, const int nxt, const KParams& P, const K
     if (ne < A.n_events) {
       const int pt0 = __ldg(A.offsets + ne);
       const int pn = min(__ldg(A.offsets + ne + 1) - pt0, PV_PREFETCH_TRACKS);
+#if PV_BULK_PREFETCH
+      // the TMA unit's bulk prefetch: lane q < 9 asks for the whole range of array q in one instruction (both ends
+      // rounded to 16 bytes inwards / outwards within the event's own range)
+      if (lane < 9 && pn > 0) {
+        const float* ptr = A.x;
+        ptr = lane == 1 ? A.y : ptr; ptr = lane == 2 ? A.z : ptr; ptr = lane == 3 ? A.tx : ptr; ptr = lane == 4 ? A.ty : ptr;
+        ptr = lane == 5 ? A.var_x : ptr; ptr = lane == 6 ? A.var_y : ptr; ptr = lane == 7 ? A.var_tx : ptr;
+        ptr = lane == 8 ? A.var_ty : ptr;
+        const unsigned long long b0 = (unsigned long long)(ptr + pt0) & ~15ull;
+        const unsigned long long b1 = (unsigned long long)(ptr + pt0 + pn) & ~15ull;
+        if (b1 > b0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(b0), "r"((unsigned)(b1 - b0)) : "memory");
+      }
+#else
       if (lane * 32 < pn + 32) {                           // one 128-byte line per lane and array
         const size_t o = (size_t)pt0 + lane * 32;
         const float* arr[9] = {A.x, A.y, A.z, A.tx, A.ty, A.var_x, A.var_y, A.var_tx, A.var_ty};
 #pragma unroll
         for (int q = 0; q < 9; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr[q] + o));
       }
+#endif
     }
   }
 
